@@ -1,0 +1,103 @@
+/* sla.h -- C ABI of the B200-native Scattered Linear Attention (SLA) library.
+ *
+ * Operation (ScatterFormer, arxiv 2401.00912; citations are PAPER.md line numbers):
+ *   All voxels of a scene are one flat sequence ordered by window; window w owns rows
+ *   off[w] .. off[w+1]-1.  SLA(Q,K,V) = Concat_w LA(Q^w,K^w,V^w)                 (Eq. 2)
+ *   LA:  o_i = phi(q_i) S_w / (phi(q_i) . z_w),  S_w = sum_j phi(k_j)^T v_j  (d_h x d_h),
+ *        z_w = sum_j phi(k_j)  (d_h),  sums over the voxels j of the window      (Eq. 3)
+ *   applied independently per head.  phi(x) = elu(x)+1 = (x>0 ? x+1 : exp(x)), the map
+ *   of the linear attention "[17]" that Eq. 3 cites; no epsilon, no 1/sqrt(d), non-causal
+ *   (DESIGN.md "Readings" A1-A4).
+ *
+ * Conventions for every entry point
+ *   - Pointers marked DEV are device pointers valid on the current CUDA device; HOST are host pointers.
+ *   - Tensors q,k,v,out,d_out,dq,dk,dv are contiguous row-major [N, H, d_h] of `dt`
+ *     (SLA_F32 / SLA_F16 / SLA_BF16); base pointers 16-byte aligned; H*d_h*sizeof(dt) a multiple of 16.
+ *   - window_offsets: int32[W+1], off[0]=0, off[W]=N, non-decreasing (zero-length windows legal and
+ *     produce nothing).  Violations are undefined behaviour (not checked on the device).
+ *   - The caller owns every buffer, including `workspace`; the library never frees or keeps them.
+ *     Inputs are read-only; outputs must not alias inputs.
+ *   - Device entry points only enqueue work on `stream` and return; they never synchronise.
+ *   - Return value: sla_status_t.  Never throws, never exits.  N==0 or W==0 -> SLA_OK, nothing launched.
+ *   - d_h in {16, 32}.  1 <= H.  N < 2^31.
+ *   - Accumulation is fp32 for every dtype; outputs are rounded (RNE) to `dt`.
+ */
+#ifndef SLA_H_
+#define SLA_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  SLA_OK = 0,
+  SLA_ERR_INVALID_ARG = 1,  /* NULL pointer, negative size, N >= 2^31 */
+  SLA_ERR_UNSUPPORTED = 2,  /* d_h not in {16,32}, misaligned pointer, bad dtype */
+  SLA_ERR_WORKSPACE = 3,    /* workspace NULL or smaller than sla_workspace_bytes() */
+  SLA_ERR_CUDA = 4          /* a CUDA runtime call failed (sticky error left for the caller) */
+} sla_status_t;
+
+typedef enum { SLA_F32 = 0, SLA_F16 = 1, SLA_BF16 = 2 } sla_dtype_t;
+
+/* Opaque CUDA stream handle (a cudaStream_t / CUstream); NULL = the legacy default stream. */
+typedef struct CUstream_st* sla_stream_t;
+
+/* Human-readable name of a status code (static storage). */
+const char* sla_status_string(int status);
+
+/* Library version string, e.g. "sla-b200 0.1 (sm_100a)". */
+const char* sla_version(void);
+
+/* Bytes of device workspace sla_forward (for_backward=0) or sla_backward (for_backward=1) needs for a
+ * problem of this shape.  The workspace holds the fp32 window states [W,H,d_h+1,d_h] of windows that
+ * are split across thread blocks (row d_h of each state is z_w), and for backward also dS/dz.
+ * Returns 0 on invalid arguments. */
+size_t sla_workspace_bytes(int64_t N, int32_t W, int32_t H, int32_t d_h, int dt, int for_backward);
+
+/* Offsets prep ("offsets generation", Fig. 5; flat window-sorted layout PAPER.md:77).
+ *   win_id          DEV int32[N]   window index of each voxel, non-decreasing, each in [0, W)
+ *   window_offsets  DEV int32[W+1] out: off[w] = #{ i : win_id[i] < w }   (bit-exact integer result)
+ * Gaps in the ids give zero-length windows (reading A10). */
+int sla_offsets_from_window_ids(const int32_t* win_id, int64_t N, int32_t W,
+                                int32_t* window_offsets, sla_stream_t stream);
+
+/* SLA forward (Eq. 2-3).
+ *   q,k,v           DEV [N,H,d_h] of dt (read-only)
+ *   window_offsets  DEV int32[W+1]
+ *   out             DEV [N,H,d_h] of dt
+ *   workspace       DEV, >= sla_workspace_bytes(N,W,H,d_h,dt,0) bytes, 16-byte aligned; contents
+ *                   are scratch (overwritten). */
+int sla_forward(const void* q, const void* k, const void* v, const int32_t* window_offsets,
+                int64_t N, int32_t W, int32_t H, int32_t d_h, int dt, void* out,
+                void* workspace, size_t workspace_bytes, sla_stream_t stream);
+
+/* SLA backward: gradients of L = sum(d_out * SLA(q,k,v)) (the paper is silent on backward; these are
+ * the analytic derivatives of Eq. 3):
+ *   dnum_i = g_i/den_i, dden_i = -(g_i.o_i)/den_i, da_i = dnum_i S^T + dden_i z, dq_i = da_i*phi'(q_i)
+ *   dS = sum_i a_i^T dnum_i, dz = sum_i dden_i a_i, dk_j = (v_j dS^T + dz)*phi'(k_j), dv_j = b_j dS.
+ *   d_out           DEV [N,H,d_h] of dt (upstream gradient g)
+ *   dq,dk,dv        DEV [N,H,d_h] of dt (outputs)
+ *   workspace       DEV, >= sla_workspace_bytes(N,W,H,d_h,dt,1) bytes.
+ * The window states are recomputed from k,v; nothing is carried over from sla_forward. */
+int sla_backward(const void* q, const void* k, const void* v, const int32_t* window_offsets,
+                 int64_t N, int32_t W, int32_t H, int32_t d_h, int dt, const void* d_out,
+                 void* dq, void* dk, void* dv,
+                 void* workspace, size_t workspace_bytes, sla_stream_t stream);
+
+/* End-to-end host entry (what a user with host data calls): copies q,k,v (and win_id) from HOST
+ * memory to the device, runs sla_offsets_from_window_ids + sla_forward, copies `out` back to HOST
+ * memory and synchronises `stream` before returning.  Device scratch is taken from the stream-ordered
+ * CUDA memory pool and returned to it before the call ends.
+ *   q,k,v   HOST [N,H,d_h] of dt (pinned memory recommended)      win_id  HOST int32[N]
+ *   out     HOST [N,H,d_h] of dt */
+int sla_forward_host(const void* q, const void* k, const void* v, const int32_t* win_id,
+                     int64_t N, int32_t W, int32_t H, int32_t d_h, int dt, void* out,
+                     sla_stream_t stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SLA_H_ */

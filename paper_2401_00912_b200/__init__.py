@@ -1,0 +1,7 @@
+"""B200-native Scattered Linear Attention (ScatterFormer, arxiv 2401.00912): a C-ABI CUDA library
+(include/sla.h, csrc/) plus this thin ctypes binding.  `workloads` holds the seeded synthetic scene
+generators shared by tests and bench (no method arithmetic)."""
+from .binding import (  # noqa: F401
+    SLA_BF16, SLA_F16, SLA_F32, SYMBOLS, SlaError, load_library, sla_backward, sla_forward,
+    sla_forward_host, sla_offsets_from_window_ids, workspace_bytes,
+)

@@ -1,0 +1,171 @@
+"""Thin Python binding of the C-ABI library declared in include/sla.h.
+
+Argument marshalling only: torch supplies device memory and the current stream; every step of the SLA
+path runs in the library's CUDA kernels.  There is NO fallback: if the library is missing or a call
+fails, an exception is raised.  This module never imports anything under oracle/.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsla_b200.so")
+
+SLA_OK = 0
+SLA_F32, SLA_F16, SLA_BF16 = 0, 1, 2
+
+# Every symbol include/sla.h declares (tests check the library exports exactly these).
+SYMBOLS = (
+    "sla_status_string", "sla_version", "sla_workspace_bytes", "sla_offsets_from_window_ids",
+    "sla_forward", "sla_backward", "sla_forward_host",
+)
+
+_lib = None
+
+
+class SlaError(RuntimeError):
+    pass
+
+
+def load_library(path: str | None = None) -> ctypes.CDLL:
+    """dlopen the in-tree library and declare the C signatures.  Fails loudly if it is not built."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    p = path or LIB_PATH
+    if not os.path.exists(p):
+        raise SlaError(f"{p} not found: build it with `python -m paper_2401_00912_b200.build` "
+                       "(there is no CPU or PyTorch fallback)")
+    L = ctypes.CDLL(p)
+    vp, i32, i64, sz, ci = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_size_t, ctypes.c_int
+    L.sla_status_string.argtypes = [ci]
+    L.sla_status_string.restype = ctypes.c_char_p
+    L.sla_version.argtypes = []
+    L.sla_version.restype = ctypes.c_char_p
+    L.sla_workspace_bytes.argtypes = [i64, i32, i32, i32, ci, ci]
+    L.sla_workspace_bytes.restype = sz
+    L.sla_offsets_from_window_ids.argtypes = [vp, i64, i32, vp, vp]
+    L.sla_offsets_from_window_ids.restype = ci
+    L.sla_forward.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp, sz, vp]
+    L.sla_forward.restype = ci
+    L.sla_backward.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp, vp, vp, vp, sz, vp]
+    L.sla_backward.restype = ci
+    L.sla_forward_host.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp]
+    L.sla_forward_host.restype = ci
+    if path is None:
+        _lib = L
+    return L
+
+
+def _check(rc: int, what: str):
+    if rc != SLA_OK:
+        raise SlaError(f"{what} failed: {load_library().sla_status_string(rc).decode()} ({rc})")
+
+
+def _dt(t) -> int:
+    import torch
+    try:
+        return {torch.float32: SLA_F32, torch.float16: SLA_F16, torch.bfloat16: SLA_BF16}[t.dtype]
+    except KeyError:
+        raise SlaError(f"unsupported dtype {t.dtype}") from None
+
+
+def _stream(stream=None) -> int:
+    import torch
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return int(s.cuda_stream)
+
+
+def _chk_dev(*ts):
+    for t in ts:
+        if not t.is_cuda:
+            raise SlaError("device entry points need CUDA tensors (no CPU fallback)")
+        if not t.is_contiguous():
+            raise SlaError("tensors must be contiguous [N,H,d_h]")
+
+
+def workspace_bytes(N: int, W: int, H: int, d_h: int, dt: int, for_backward: bool = False) -> int:
+    return int(load_library().sla_workspace_bytes(N, W, H, d_h, dt, 1 if for_backward else 0))
+
+
+def _workspace(like, N, W, H, d_h, dt, for_backward, workspace):
+    import torch
+    need = workspace_bytes(N, W, H, d_h, dt, for_backward)
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=like.device)
+    return workspace, workspace.numel() * workspace.element_size()
+
+
+def sla_offsets_from_window_ids(win_id, W: int, out=None, stream=None):
+    """win_id: CUDA int32[N] non-decreasing in [0,W) -> CUDA int32[W+1] offsets (include/sla.h)."""
+    import torch
+    L = load_library()
+    _chk_dev(win_id)
+    if win_id.dtype != torch.int32:
+        raise SlaError("win_id must be int32")
+    N = win_id.numel()
+    if out is None:
+        out = torch.empty(W + 1, dtype=torch.int32, device=win_id.device)
+    _check(L.sla_offsets_from_window_ids(win_id.data_ptr(), N, W, out.data_ptr(), _stream(stream)),
+           "sla_offsets_from_window_ids")
+    return out
+
+
+def sla_forward(q, k, v, window_offsets, out=None, workspace=None, stream=None):
+    """q,k,v: CUDA [N,H,d_h] (fp32/fp16/bf16); window_offsets: CUDA int32[W+1] -> out [N,H,d_h]."""
+    import torch
+    L = load_library()
+    _chk_dev(q, k, v, window_offsets)
+    if not (q.shape == k.shape == v.shape and q.dim() == 3 and q.dtype == k.dtype == v.dtype):
+        raise SlaError("q,k,v must share shape [N,H,d_h] and dtype")
+    if window_offsets.dtype != torch.int32:
+        raise SlaError("window_offsets must be int32")
+    N, H, d = q.shape
+    W = window_offsets.numel() - 1
+    dt = _dt(q)
+    if out is None:
+        out = torch.empty_like(q)
+    workspace, wsb = _workspace(q, N, W, H, d, dt, False, workspace)
+    _check(L.sla_forward(q.data_ptr(), k.data_ptr(), v.data_ptr(), window_offsets.data_ptr(), N, W, H, d,
+                         dt, out.data_ptr(), workspace.data_ptr(), wsb, _stream(stream)), "sla_forward")
+    return out
+
+
+def sla_backward(q, k, v, window_offsets, d_out, dq=None, dk=None, dv=None, workspace=None, stream=None):
+    """Gradients of sum(d_out * SLA(q,k,v)) -> (dq, dk, dv), each [N,H,d_h] of the input dtype."""
+    import torch
+    L = load_library()
+    _chk_dev(q, k, v, window_offsets, d_out)
+    if not (q.shape == k.shape == v.shape == d_out.shape and q.dim() == 3
+            and q.dtype == k.dtype == v.dtype == d_out.dtype):
+        raise SlaError("q,k,v,d_out must share shape [N,H,d_h] and dtype")
+    if window_offsets.dtype != torch.int32:
+        raise SlaError("window_offsets must be int32")
+    N, H, d = q.shape
+    W = window_offsets.numel() - 1
+    dt = _dt(q)
+    dq = torch.empty_like(q) if dq is None else dq
+    dk = torch.empty_like(q) if dk is None else dk
+    dv = torch.empty_like(q) if dv is None else dv
+    workspace, wsb = _workspace(q, N, W, H, d, dt, True, workspace)
+    _check(L.sla_backward(q.data_ptr(), k.data_ptr(), v.data_ptr(), window_offsets.data_ptr(), N, W, H, d,
+                          dt, d_out.data_ptr(), dq.data_ptr(), dk.data_ptr(), dv.data_ptr(),
+                          workspace.data_ptr(), wsb, _stream(stream)), "sla_backward")
+    return dq, dk, dv
+
+
+def sla_forward_host(q, k, v, win_id, W: int, out=None, stream=None):
+    """End-to-end host entry: q,k,v,win_id are HOST (CPU, ideally pinned) torch tensors; returns a
+    HOST tensor.  H2D copies, prep, forward and the D2H copy all happen inside the C call."""
+    import torch
+    L = load_library()
+    for t in (q, k, v, win_id):
+        if t.is_cuda or not t.is_contiguous():
+            raise SlaError("sla_forward_host takes contiguous host tensors")
+    N, H, d = q.shape
+    if out is None:
+        out = torch.empty_like(q, pin_memory=q.is_pinned())
+    _check(L.sla_forward_host(q.data_ptr(), k.data_ptr(), v.data_ptr(), win_id.data_ptr(), N, W, H, d,
+                              _dt(q), out.data_ptr(), _stream(stream)), "sla_forward_host")
+    return out

@@ -1,0 +1,135 @@
+// sla_api.cu -- the extern "C" boundary declared in include/sla.h: argument validation, workspace
+// carving and kernel dispatch.  No torch types; plain pointers and sizes.
+#include "sla_internal.cuh"
+
+namespace {
+
+inline size_t esize(int dt) { return dt == SLA_F32 ? 4 : 2; }
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+// fp32 accumulators for windows split across thread blocks: one slot per possible split window.
+inline size_t state_slots(int64_t N) { return (size_t)(N / (sla::kFuseMax + 1)) + 1; }
+inline size_t state_bytes(int64_t N, int H, int d) {
+  return state_slots(N) * (size_t)H * (size_t)(d + 1) * (size_t)d * sizeof(float);
+}
+
+int check_common(int64_t N, int32_t W, int32_t H, int32_t d_h, int dt) {
+  if (N < 0 || W < 0 || H < 1 || N >= (int64_t(1) << 31)) return SLA_ERR_INVALID_ARG;
+  if (dt != SLA_F32 && dt != SLA_F16 && dt != SLA_BF16) return SLA_ERR_UNSUPPORTED;
+  if (d_h != 16 && d_h != 32) return SLA_ERR_UNSUPPORTED;
+  if (((size_t)H * d_h * esize(dt)) % 16 != 0) return SLA_ERR_UNSUPPORTED;
+  return SLA_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* sla_status_string(int status) {
+  switch (status) {
+    case SLA_OK: return "SLA_OK";
+    case SLA_ERR_INVALID_ARG: return "SLA_ERR_INVALID_ARG";
+    case SLA_ERR_UNSUPPORTED: return "SLA_ERR_UNSUPPORTED";
+    case SLA_ERR_WORKSPACE: return "SLA_ERR_WORKSPACE";
+    case SLA_ERR_CUDA: return "SLA_ERR_CUDA";
+    default: return "SLA_ERR_UNKNOWN";
+  }
+}
+
+const char* sla_version(void) { return "sla-b200 0.1 (sm_100a)"; }
+
+size_t sla_workspace_bytes(int64_t N, int32_t W, int32_t H, int32_t d_h, int dt, int for_backward) {
+  if (check_common(N, W, H, d_h, dt) != SLA_OK) return 0;
+  const size_t one = state_bytes(N, H, d_h);
+  return for_backward ? 2 * one : one;
+}
+
+int sla_offsets_from_window_ids(const int32_t* win_id, int64_t N, int32_t W, int32_t* window_offsets,
+                                sla_stream_t stream) {
+  if (N < 0 || W < 0 || N >= (int64_t(1) << 31)) return SLA_ERR_INVALID_ARG;
+  if (!window_offsets || (N > 0 && !win_id)) return SLA_ERR_INVALID_ARG;
+  if (N > 0 && W == 0) return SLA_ERR_INVALID_ARG;
+  cudaError_t e = sla::launch_offsets(win_id, (int)N, W, window_offsets, (cudaStream_t)stream);
+  return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
+}
+
+int sla_forward(const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
+                int32_t W, int32_t H, int32_t d_h, int dt, void* out, void* workspace,
+                size_t workspace_bytes, sla_stream_t stream) {
+  int rc = check_common(N, W, H, d_h, dt);
+  if (rc != SLA_OK) return rc;
+  if (N == 0 || W == 0) return SLA_OK;
+  if (!q || !k || !v || !window_offsets || !out) return SLA_ERR_INVALID_ARG;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out)) return SLA_ERR_UNSUPPORTED;
+  const size_t need = state_bytes(N, H, d_h);
+  if (!workspace || workspace_bytes < need || !aligned16(workspace)) return SLA_ERR_WORKSPACE;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (cudaMemsetAsync(workspace, 0, need, st) != cudaSuccess) return SLA_ERR_CUDA;
+  sla::Problem p{};
+  p.q = q; p.k = k; p.v = v; p.out = out; p.off = window_offsets;
+  p.ws_state = static_cast<float*>(workspace);
+  p.N = (int)N; p.W = W; p.H = H; p.d = d_h;
+  cudaError_t e = sla::launch_forward_generic(p, dt, st);
+  return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
+}
+
+int sla_backward(const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
+                 int32_t W, int32_t H, int32_t d_h, int dt, const void* d_out, void* dq, void* dk,
+                 void* dv, void* workspace, size_t workspace_bytes, sla_stream_t stream) {
+  int rc = check_common(N, W, H, d_h, dt);
+  if (rc != SLA_OK) return rc;
+  if (N == 0 || W == 0) return SLA_OK;
+  if (!q || !k || !v || !window_offsets || !d_out || !dq || !dk || !dv) return SLA_ERR_INVALID_ARG;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(d_out) || !aligned16(dq) ||
+      !aligned16(dk) || !aligned16(dv))
+    return SLA_ERR_UNSUPPORTED;
+  const size_t one = state_bytes(N, H, d_h);
+  if (!workspace || workspace_bytes < 2 * one || !aligned16(workspace)) return SLA_ERR_WORKSPACE;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (cudaMemsetAsync(workspace, 0, 2 * one, st) != cudaSuccess) return SLA_ERR_CUDA;
+  sla::Problem p{};
+  p.q = q; p.k = k; p.v = v; p.g = d_out; p.dq = dq; p.dk = dk; p.dv = dv; p.off = window_offsets;
+  p.ws_state = static_cast<float*>(workspace);
+  p.ws_dstate = reinterpret_cast<float*>(static_cast<char*>(workspace) + one);
+  p.N = (int)N; p.W = W; p.H = H; p.d = d_h;
+  cudaError_t e = sla::launch_backward_generic(p, dt, st);
+  return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
+}
+
+int sla_forward_host(const void* q, const void* k, const void* v, const int32_t* win_id, int64_t N,
+                     int32_t W, int32_t H, int32_t d_h, int dt, void* out, sla_stream_t stream) {
+  int rc = check_common(N, W, H, d_h, dt);
+  if (rc != SLA_OK) return rc;
+  if (N == 0 || W == 0) return SLA_OK;
+  if (!q || !k || !v || !win_id || !out) return SLA_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t tb = (size_t)N * H * d_h * esize(dt);           // bytes per tensor
+  const size_t tb_al = (tb + 255) / 256 * 256;
+  const size_t ids_al = ((size_t)N * 4 + 255) / 256 * 256;
+  const size_t off_al = ((size_t)(W + 1) * 4 + 255) / 256 * 256;
+  const size_t ws = state_bytes(N, H, d_h);
+  char* base = nullptr;
+  if (cudaMallocAsync(reinterpret_cast<void**>(&base), 4 * tb_al + ids_al + off_al + ws, st) !=
+      cudaSuccess)
+    return SLA_ERR_CUDA;
+  char* dq_ = base; char* dk_ = base + tb_al; char* dv_ = base + 2 * tb_al; char* do_ = base + 3 * tb_al;
+  int32_t* dids = reinterpret_cast<int32_t*>(base + 4 * tb_al);
+  int32_t* doff = reinterpret_cast<int32_t*>(base + 4 * tb_al + ids_al);
+  void* dws = base + 4 * tb_al + ids_al + off_al;
+  bool ok = true;
+  ok = ok && cudaMemcpyAsync(dids, win_id, (size_t)N * 4, cudaMemcpyHostToDevice, st) == cudaSuccess;
+  ok = ok && cudaMemcpyAsync(dk_, k, tb, cudaMemcpyHostToDevice, st) == cudaSuccess;
+  ok = ok && cudaMemcpyAsync(dv_, v, tb, cudaMemcpyHostToDevice, st) == cudaSuccess;
+  ok = ok && cudaMemcpyAsync(dq_, q, tb, cudaMemcpyHostToDevice, st) == cudaSuccess;
+  if (ok) rc = sla_offsets_from_window_ids(dids, N, W, doff, stream);
+  if (ok && rc == SLA_OK)
+    rc = sla_forward(dq_, dk_, dv_, doff, N, W, H, d_h, dt, do_, dws, ws, stream);
+  ok = ok && rc == SLA_OK;
+  ok = ok && cudaMemcpyAsync(out, do_, tb, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+  cudaFreeAsync(base, st);
+  if (cudaStreamSynchronize(st) != cudaSuccess) ok = false;
+  if (rc != SLA_OK) return rc;
+  return ok ? SLA_OK : SLA_ERR_CUDA;
+}
+
+}  // extern "C"

@@ -1,0 +1,71 @@
+// sla_internal.cuh -- shared device helpers of the CUDA path (dtype traits, feature map, launch
+// declarations).  Product code: shares nothing with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+
+#include "../../include/sla.h"
+
+namespace sla {
+
+// ---- dtype traits: load/store one element as fp32 ------------------------------------------------
+template <typename T> struct Elem;
+template <> struct Elem<float> {
+  static __device__ __forceinline__ float ld(const float* p) { return __ldg(p); }
+  static __device__ __forceinline__ void st(float* p, float x) { *p = x; }
+};
+template <> struct Elem<__half> {
+  static __device__ __forceinline__ float ld(const __half* p) {
+    return __half2float(__ushort_as_half(__ldg(reinterpret_cast<const unsigned short*>(p))));
+  }
+  static __device__ __forceinline__ void st(__half* p, float x) { *p = __float2half_rn(x); }
+};
+template <> struct Elem<__nv_bfloat16> {
+  static __device__ __forceinline__ float ld(const __nv_bfloat16* p) {
+    return __uint_as_float(((unsigned)__ldg(reinterpret_cast<const unsigned short*>(p))) << 16);
+  }
+  static __device__ __forceinline__ void st(__nv_bfloat16* p, float x) { *p = __float2bfloat16_rn(x); }
+};
+
+// ---- feature map phi(x) = elu(x)+1 (reading A1; Eq. 3 cites [17]) and its derivative --
+// fp32 path: full-precision expf (the fp32 tolerance is 1e-5 relative).
+__device__ __forceinline__ float phi_f32(float x) { return x > 0.f ? x + 1.f : expf(x); }
+__device__ __forceinline__ float dphi_f32(float x) { return x > 0.f ? 1.f : expf(x); }
+
+// ---- window search: largest w in [0,W) with off[w] <= row  (off[0]=0 <= row < off[W]) -------------
+__device__ __forceinline__ int window_of_row(const int32_t* __restrict__ off, int W, int row) {
+  int lo = 0, hi = W;  // invariant: off[lo] <= row < off[hi]
+  while (hi - lo > 1) {
+    int mid = (lo + hi) >> 1;
+    if (__ldg(off + mid) <= row) lo = mid; else hi = mid;
+  }
+  return lo;
+}
+
+// Tiling constants of the generic (CUDA-core, fp32-math) path.
+//   TILE_ROWS: rows of the flat sequence per thread block ("chunk", Fig. 3a).
+//   FUSE_MAX : a window of at most this many rows is processed whole by the block that owns its
+//              first row (state never leaves the SM); longer windows are split by tile and their
+//              partial states are reduced in global memory (workspace) with fp32 atomics.
+constexpr int kTileRows = 64;
+constexpr int kFuseMax = 256;
+constexpr int kRowBatch = 8;  // rows staged per inner step
+
+struct Problem {
+  const void* q; const void* k; const void* v; const void* g;
+  void* out; void* dq; void* dk; void* dv;
+  const int32_t* off;
+  float* ws_state;   // [W,H,d+1,d] fp32 (S rows 0..d-1, z in row d) for split windows
+  float* ws_dstate;  // [W,H,d+1,d] fp32 (dS, dz) for split windows (backward)
+  int N, W, H, d;
+};
+
+// Launchers (defined in the .cu files); all enqueue on `st` and return the last CUDA error.
+cudaError_t launch_offsets(const int32_t* win_id, int N, int W, int32_t* off, cudaStream_t st);
+cudaError_t launch_forward_generic(const Problem& p, int dt, cudaStream_t st);
+cudaError_t launch_backward_generic(const Problem& p, int dt, cudaStream_t st);
+
+}  // namespace sla

@@ -1,0 +1,201 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 CPU oracle, element by element on
+the same seeded inputs.  Tolerances (BASELINE.json north_star; reading A11):
+  |gpu - ref| <= atol + rtol*|ref|,  fp32: rtol 1e-5, atol 1e-6;  fp16/bf16: rtol 2e-2, atol 1e-3.
+Gradients additionally: relative L2 error <= 1e-2 (fp16/bf16), 1e-5 (fp32)."""
+import numpy as np
+import pytest
+
+import paper_2401_00912_b200 as pkg
+from paper_2401_00912_b200 import workloads as wl
+from oracle import sla_oracle
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f32": (1e-5, 1e-6), "f16": (2e-2, 1e-3), "bf16": (2e-2, 1e-3)}
+REL_L2 = {"f32": 1e-5, "f16": 1e-2, "bf16": 1e-2}
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def to_dev(a, dtype):
+    torch = _torch()
+    tdt = {"f32": torch.float32, "f16": torch.float16, "bf16": torch.bfloat16}[dtype]
+    return torch.from_numpy(a).cuda().to(tdt)   # values are already exactly representable
+
+
+def check(name, got_t, want, dtype, lengths=None):
+    rtol, atol = TOL[dtype]
+    got = got_t.double().cpu().numpy()
+    assert np.isfinite(got).all(), f"{name}: non-finite output"
+    err = np.abs(got - want) / (atol + rtol * np.abs(want))
+    worst = np.unravel_index(np.argmax(err), err.shape)
+    msg = f"{name}: worst err/tol {err.max():.3f} at {worst} got {got[worst]} want {want[worst]}"
+    if lengths is not None:
+        off = np.concatenate([[0], np.cumsum(lengths)])
+        w = int(np.searchsorted(off, worst[0], side="right") - 1)
+        msg += f" (window {w}, length {int(lengths[w])})"
+    assert err.max() <= 1.0, msg
+    return float(err.max())
+
+
+def run_forward(sc, workspace=None):
+    torch = _torch()
+    q, k, v = sc.tensor("q"), sc.tensor("k"), sc.tensor("v")
+    off = torch.from_numpy(sc.offsets).cuda()
+    out = pkg.sla_forward(to_dev(q, sc.dtype), to_dev(k, sc.dtype), to_dev(v, sc.dtype), off)
+    torch.cuda.synchronize()
+    ref = sla_oracle.forward(q, k, v, sc.offsets, nthreads=8)
+    return out, ref
+
+
+def run_backward(sc):
+    torch = _torch()
+    q, k, v, g = sc.tensor("q"), sc.tensor("k"), sc.tensor("v"), sc.tensor("do")
+    off = torch.from_numpy(sc.offsets).cuda()
+    grads = pkg.sla_backward(to_dev(q, sc.dtype), to_dev(k, sc.dtype), to_dev(v, sc.dtype), off,
+                             to_dev(g, sc.dtype))
+    torch.cuda.synchronize()
+    ref = sla_oracle.backward(q, k, v, g, sc.offsets, nthreads=8)
+    return grads, ref
+
+
+def check_grads(grads, ref, sc):
+    for name, got, want in zip(("dq", "dk", "dv"), grads, ref):
+        check(f"{sc.name}.{name}", got, want, sc.dtype, sc.lengths)
+        gotd = got.double().cpu().numpy()
+        rel = np.linalg.norm(gotd - want) / max(np.linalg.norm(want), 1e-300)
+        assert rel <= REL_L2[sc.dtype], f"{sc.name}.{name}: relative L2 {rel:.3e}"
+
+
+# ---- prep kernel: bit-exact ----------------------------------------------------------------------
+@pytest.mark.parametrize("case", ["config0", "config1", "config3", "gaps", "single", "empty_tail", "n0"])
+def test_offsets_bit_exact(case):
+    torch = _torch()
+    if case.startswith("config"):
+        sc = wl.make_config(int(case[-1]))
+        lengths = sc.lengths
+    elif case == "gaps":
+        lengths = np.array([0, 0, 3, 0, 1, 0, 0, 0, 700, 0, 2, 0, 0])
+    elif case == "single":
+        lengths = np.array([1000])
+    elif case == "empty_tail":
+        lengths = np.array([5, 0, 0, 0])
+    else:
+        lengths = np.array([0, 0, 0])
+    W = len(lengths)
+    ids = np.repeat(np.arange(W, dtype=np.int32), lengths)
+    want = sla_oracle.offsets_from_window_ids(ids, W)
+    got = pkg.sla_offsets_from_window_ids(torch.from_numpy(ids).cuda(), W)
+    torch.cuda.synchronize()
+    assert np.array_equal(got.cpu().numpy(), want)
+    assert np.array_equal(want, np.concatenate([[0], np.cumsum(lengths)]).astype(np.int32))
+
+
+# ---- the five BASELINE.json configs, full size, every element --------------------------------------
+@pytest.mark.parametrize("c", [0, 1, 2, 3])
+def test_forward_configs(c):
+    sc = wl.make_config(c)
+    out, ref = run_forward(sc)
+    check(f"{sc.name}.out", out, ref, sc.dtype, sc.lengths)
+
+
+def test_forward_backward_config4():
+    sc = wl.make_config(4)
+    out, ref = run_forward(sc)
+    check(f"{sc.name}.out", out, ref, sc.dtype, sc.lengths)
+    grads, gref = run_backward(sc)
+    check_grads(grads, gref, sc)
+
+
+@pytest.mark.parametrize("c", [0, 2, 3])
+def test_backward_other_configs(c):
+    sc = wl.make_config(c)
+    grads, gref = run_backward(sc)
+    check_grads(grads, gref, sc)
+
+
+# ---- edge cases (SURVEY.md §8c list) ---------------------------------------------------------------
+EDGE_LAYOUTS = {
+    "one_window": [777],
+    "all_len1": [1] * 333,
+    "empty_start_end_consecutive": [0, 0, 5, 0, 0, 0, 9, 40, 0],
+    "around_rowbatch_4_8": [3, 4, 5, 7, 8, 9, 15, 16, 17, 31, 32, 33],
+    "around_tile_64": [63, 64, 65, 1, 127, 128, 129],
+    "around_fuse_256": [255, 256, 257, 2, 258, 1, 511, 513],
+    "huge_and_tiny": [1, 2, 3000, 1, 1, 2, 4097, 3],
+    "ragged_not_mult16": [13, 29, 101, 7],
+}
+
+
+@pytest.mark.parametrize("layout", sorted(EDGE_LAYOUTS))
+@pytest.mark.parametrize("dtype,H,d", [("f32", 4, 32), ("f32", 2, 16), ("f16", 8, 16), ("f16", 8, 32),
+                                       ("bf16", 8, 32), ("bf16", 4, 16), ("f16", 1, 16), ("f32", 1, 32),
+                                       ("f16", 3, 16), ("bf16", 16, 32)])
+def test_edge_layouts_forward_backward(layout, dtype, H, d):
+    sc = wl.make_scene(EDGE_LAYOUTS[layout], H, d, dtype, seed=77 + len(layout), name=layout)
+    out, ref = run_forward(sc)
+    check(f"{layout}.out", out, ref, dtype, sc.lengths)
+    grads, gref = run_backward(sc)
+    check_grads(grads, gref, sc)
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f16", "bf16"])
+def test_large_magnitude_inputs(dtype):
+    """q,k entries of +-20: phi spans e^-20 .. 21; the normaliser must stay finite and accurate."""
+    sc = wl.make_scene([1, 2, 9, 40, 300], 4, 16, dtype, seed=5)
+    rng = np.random.Generator(np.random.PCG64(99))
+    q, k, v = sc.tensor("q"), sc.tensor("k"), sc.tensor("v")
+    sel = rng.random(q.shape) < 0.2
+    q = wl.round_to_dtype(np.where(sel, np.sign(q) * 20.0, q).astype(np.float32), dtype)
+    sel = rng.random(k.shape) < 0.2
+    k = wl.round_to_dtype(np.where(sel, np.sign(k) * 20.0, k).astype(np.float32), dtype)
+    torch = _torch()
+    off = torch.from_numpy(sc.offsets).cuda()
+    out = pkg.sla_forward(to_dev(q, dtype), to_dev(k, dtype), to_dev(v, dtype), off)
+    ref = sla_oracle.forward(q, k, v, sc.offsets)
+    check("large_magnitude.out", out, ref, dtype, sc.lengths)
+
+
+def test_n0_w0_and_errors():
+    torch = _torch()
+    q = torch.empty(0, 8, 16, dtype=torch.float16, device="cuda")
+    off = torch.zeros(1, dtype=torch.int32, device="cuda")
+    assert pkg.sla_forward(q, q, q, off).shape == (0, 8, 16)
+    off3 = torch.zeros(4, dtype=torch.int32, device="cuda")
+    assert pkg.sla_forward(q, q, q, off3).shape == (0, 8, 16)
+    q2 = torch.zeros(4, 8, 16, dtype=torch.float16, device="cuda")
+    off2 = torch.tensor([0, 4], dtype=torch.int32, device="cuda")
+    small = torch.empty(16, dtype=torch.uint8, device="cuda")
+    with pytest.raises(pkg.SlaError, match="WORKSPACE"):
+        pkg.sla_forward(q2, q2, q2, off2, workspace=small)
+    q3 = torch.zeros(4, 8, 24, dtype=torch.float16, device="cuda")
+    with pytest.raises(pkg.SlaError, match="UNSUPPORTED"):
+        pkg.sla_forward(q3, q3, q3, off2)
+
+
+def test_closed_forms_on_gpu():
+    """Pins that need no oracle: length-1 windows return v (Eq. 3 with m=1); equal values returned."""
+    torch = _torch()
+    sc = wl.make_scene([1] * 50 + [7, 90], 8, 16, "f16", seed=3)
+    q, k, v = (to_dev(sc.tensor(n), "f16") for n in ("q", "k", "v"))
+    off = torch.from_numpy(sc.offsets).cuda()
+    out = pkg.sla_forward(q, k, v, off)
+    assert torch.allclose(out[:50].float(), v[:50].float(), rtol=2e-3, atol=1e-3)
+    v2 = v.clone()
+    v2[50:57] = v[50]
+    out2 = pkg.sla_forward(q, k, v2, off)
+    assert torch.allclose(out2[50:57].float(), v2[50:57].float(), rtol=2e-3, atol=1e-3)
+
+
+def test_host_entry_matches_device_entry():
+    torch = _torch()
+    sc = wl.make_config(0)
+    q, k, v = (torch.from_numpy(sc.tensor(n)).pin_memory() for n in ("q", "k", "v"))
+    ids = torch.from_numpy(sc.window_ids).pin_memory()
+    out_h = pkg.sla_forward_host(q, k, v, ids, sc.W)
+    off = torch.from_numpy(sc.offsets).cuda()
+    out_d = pkg.sla_forward(q.cuda(), k.cuda(), v.cuda(), off)
+    assert torch.equal(out_h, out_d.cpu())
