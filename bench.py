@@ -1,0 +1,327 @@
+#!/usr/bin/env python
+"""bench.py -- SLA forward throughput on the Waymo-like scene (BASELINE.json configs[1]).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path over one synthetic scene:
+sla_offsets_from_window_ids (prep) + sla_forward, through the C ABI.  Prints ONE JSON line (rank 0).
+
+Timing protocol: CUDA events on the launching stream, W>=3 warm-up steps, cold L2 (each step uses
+the next of R rotating buffer sets whose total footprint exceeds 2x the 126 MB L2), nvidia-smi clocks
+sampled during the timed region, max over ranks.  N>1: one process per GPU (torchrun), every rank
+runs its own scene (windows/scenes are independent, Eq. 2 PAPER.md:79 -> no collective), "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "sla_fwd_voxels_per_sec"
+UNIT = "voxels/s"
+WORKLOAD = "config1_waymo_like_N60000_H8_dh16_fp16"
+L2_BYTES = 126 * 1024 * 1024
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (bench line = 1)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples nvidia-smi SM clocks and throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self._stop, self._t = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
+                for line in out.strip().splitlines():
+                    self.rows.append([x.strip() for x in line.split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def __enter__(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._t.join(timeout=10)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for n, val in zip(names, r[2:6]):
+                if val.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def init_dist(n_gpus: int):
+    """One process per GPU under torchrun; returns (rank, world, local_rank)."""
+    import torch
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29511")
+        torch.cuda.set_device(local)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    else:
+        torch.cuda.set_device(0)
+    return rank, world, local
+
+
+def barrier(world):
+    import torch
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+    torch.cuda.synchronize()
+
+
+def max_over_ranks(x: float, world: int) -> float:
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device="cuda")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def sum_over_ranks(x: float, world: int) -> float:
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device="cuda")
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def make_scene(config: int, rank: int):
+    """Config `config` of BASELINE.json; rank r > 0 draws its own scene of the same recipe."""
+    from paper_2401_00912_b200 import workloads as wl
+    sc = wl.make_config(config)
+    if rank > 0 and config == 1:
+        s = wl.SEED_BASE + 100 * rank + config
+        sc = wl.Scene(sc.name, wl.lengths_waymo_like(s, 60000), sc.H, sc.d_h, sc.dtype, sc.scale, s)
+    elif rank > 0:
+        sc = wl.Scene(sc.name, sc.lengths, sc.H, sc.d_h, sc.dtype, sc.scale, sc.seed + 100 * rank)
+    return sc
+
+
+def cpu_oracle_time(sc, reps: int = 3):
+    """The fp64 oracle, as it stands, on all host cores: best-of-`reps` seconds for one scene."""
+    from oracle import sla_oracle
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    q, k, v = sc.tensor("q"), sc.tensor("k"), sc.tensor("v")
+    best = float("inf")
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        ids_off = sla_oracle.offsets_from_window_ids(sc.window_ids, sc.W)
+        sla_oracle.forward(q, k, v, ids_off, nthreads=cores)
+        best = min(best, time.perf_counter() - t0)
+    return best, cores
+
+
+def run_ours(args):
+    import torch
+    import paper_2401_00912_b200 as pkg
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (the product has no CPU fallback)")
+    rank, world, local = init_dist(args.gpus)
+    dev = torch.device("cuda", local if world > 1 else 0)
+    sc = make_scene(args.config, rank)
+    tdt = {"f32": torch.float32, "f16": torch.float16, "bf16": torch.bfloat16}[sc.dtype]
+    esz = 4 if sc.dtype == "f32" else 2
+    N, W, H, d = sc.N, sc.W, sc.H, sc.d_h
+    tensor_bytes = N * H * d * esz
+    alg_bytes = 4 * tensor_bytes + 4 * (W + 1)          # read Q,K,V + offsets, write O
+    # cold-L2 protocol: rotate R buffer sets whose total footprint exceeds 2x L2
+    R = max(2, -(-2 * L2_BYTES // (4 * tensor_bytes)) + 1)
+    host = [torch.from_numpy(sc.tensor(n)).to(tdt).pin_memory() for n in ("q", "k", "v")]
+    ids_host = torch.from_numpy(sc.window_ids).pin_memory()
+    sets = []
+    for r in range(R):
+        q, k, v = (h.to(dev) for h in host)
+        if r:  # same scene layout, decorrelated values (rolled) so sets are distinct memory, same stats
+            q, k, v = (t.roll(r * 17, 0).contiguous() for t in (q, k, v))
+        sets.append((q, k, v, torch.empty_like(q)))
+    ids = ids_host.to(dev)
+    off = torch.empty(W + 1, dtype=torch.int32, device=dev)
+    ws = torch.empty(max(16, pkg.workspace_bytes(N, W, H, d, pkg.binding._dt(sets[0][0]))),
+                     dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step(i):
+        q, k, v, o = sets[i % R]
+        pkg.sla_offsets_from_window_ids(ids, W, out=off, stream=stream)
+        pkg.sla_forward(q, k, v, off, out=o, workspace=ws, stream=stream)
+
+    for i in range(max(3, args.warmup)):
+        step(i)
+    barrier(world)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local if world > 1 else 0) as clk:
+        e0.record(stream)
+        for i in range(args.steps):
+            step(i)
+        e1.record(stream)
+        barrier(world)
+        ms_total = e0.elapsed_time(e1)
+        # keep the GPU busy a little longer so the sampler sees clocks under this load
+        t_end = time.time() + 0.6
+        j = 0
+        while time.time() < t_end:
+            step(j); j += 1
+        torch.cuda.synchronize()
+    ms_step = max_over_ranks(ms_total / args.steps, world)
+    total_voxels = sum_over_ranks(float(N), world)
+    value = total_voxels / (ms_step * 1e-3)
+
+    # dominant call (sla_forward alone: workspace memset + its kernels), per-launch event pairs, cold L2
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+           for _ in range(args.steps)]
+    for i, (a, b) in enumerate(evs):
+        q, k, v, o = sets[i % R]
+        a.record(stream)
+        pkg.sla_forward(q, k, v, off, out=o, workspace=ws, stream=stream)
+        b.record(stream)
+    torch.cuda.synchronize()
+    fwd_ms = sorted(a.elapsed_time(b) for a, b in evs)
+    fwd_ms_avg = sum(fwd_ms) / len(fwd_ms)
+    peak, peak_src = measured_peaks()
+    achieved = alg_bytes / (fwd_ms_avg * 1e-3) / 1e9
+
+    # end to end through the host entry point (pinned host buffers; H2D + prep + forward + D2H inside)
+    out_host = torch.empty_like(host[0]).pin_memory()
+    n_e2e = max(3, min(args.steps, 20))
+    for _ in range(2):
+        pkg.sla_forward_host(host[0], host[1], host[2], ids_host, W, out=out_host, stream=stream)
+    barrier(world)
+    t0 = time.perf_counter()
+    for _ in range(n_e2e):
+        pkg.sla_forward_host(host[0], host[1], host[2], ids_host, W, out=out_host, stream=stream)
+    torch.cuda.synchronize()
+    e2e_s = max_over_ranks((time.perf_counter() - t0) / n_e2e, world)
+    e2e_value = total_voxels / e2e_s
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(3, args.warmup), "ms_per_step": ms_step, "us_per_scene": ms_step * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": sc.dtype,
+        "data": "synthetic", "impl": "ours",
+        "config": {"workload": WORKLOAD if args.config == 1 else sc.name, "N": N, "W": W, "H": H,
+                   "d_h": d, "step": "sla_offsets_from_window_ids + sla_forward (C ABI)",
+                   "l2_protocol": f"cold: {R} rotating buffer sets, {R * 4 * tensor_bytes / 1e6:.0f} MB > 2x126 MB L2",
+                   "parallelism": f"replicas x{world} (one scene per rank, no collective)"},
+        "clocks": clk.summary(),
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 3 * tensor_bytes + 4 * N,
+                "d2h_bytes_per_step": tensor_bytes, "ms_per_step": e2e_s * 1e3,
+                "api": "sla_forward_host (pinned host buffers)"},
+        "gpu_launches": args.steps * KERNELS_PER_STEP,
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES, "peak_source": peak_src,
+                     "kernel": "sla_forward (all launches of one call)", "algorithmic_bytes": alg_bytes,
+                     "us_per_launch_avg": fwd_ms_avg * 1e3, "us_per_launch_median": fwd_ms[len(fwd_ms) // 2] * 1e3,
+                     "frac_of_nominal_8TBs": achieved / 8000.0},
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        secs, cores = cpu_oracle_time(sc)
+        line["cpu_baseline"] = {"value": N / secs, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": "the full scene of this workload, best of 3 runs",
+                                "us_per_scene": secs * 1e6}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+# kernels of ours launched per step: prep (1) + sla_forward (main + split-output) -- DESIGN.md
+KERNELS_PER_STEP = 3
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel from profiles/ (None until captured)
+NCU_TRAFFIC_BYTES = None
+
+
+def run_reference(args):
+    """Reference arm for this tier = the CPU oracle as it stands, on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    sc = make_scene(args.config, 0)
+    steps = max(1, min(args.steps, 20))
+    warm = max(1, min(args.warmup, 2))
+    for _ in range(warm):
+        cpu_oracle_time(sc, reps=1)
+    cores, tot = 1, 0.0
+    for _ in range(steps):
+        t, cores = cpu_oracle_time(sc, reps=1)   # times the oracle calls only, not the input generator
+        tot += t
+    secs = tot / steps
+    value = sc.N / secs
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps, "warmup": warm,
+        "ms_per_step": secs * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "impl": "reference",
+        "config": {"workload": WORKLOAD if args.config == 1 else sc.name, "N": sc.N, "W": sc.W, "H": sc.H,
+                   "d_h": sc.d_h, "step": "oracle offsets + oracle forward on the full scene (fp64, host cores)"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": "the full scene of this workload per step"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line), flush=True)
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

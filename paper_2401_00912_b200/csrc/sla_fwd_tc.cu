@@ -1,0 +1,333 @@
+// sla_fwd_tc.cu -- SLA forward for fp16 / bf16 I/O on sm_100a: TMA-streamed, warp-per-head,
+// tensor-core (mma.sync m16n8k16, fp32 accumulate) contractions, window state kept in registers.
+//
+// Design:
+//   * The flat window-sorted matrix is cut into equal row spans, one per CTA
+//     (load balance by rows/chunks, not by window -- PAPER.md:93 Fig. 3a).  A CTA owns every window
+//     of <= FUSE_MAX rows whose first row lies in its span (processed whole, state never leaves the
+//     SM) and, for longer windows, the piece that intersects its span (partial state -> fp32
+//     atomics into the workspace; outputs by the second kernel).
+//   * Memory streaming is decoupled from the window structure: two producer warps stream the CTA's
+//     rows of K,V and of Q through two shared-memory rings with 2-D TMA (128-byte swizzle) and
+//     mbarriers, regardless of where windows begin and end.
+//   * Consumer warp h owns head h of the slab (8 heads).  Per 16-row tile it forms
+//       S^T += V^T phi(K)   (Eq. 3 numerator state; contraction over voxels)
+//       z   += 1^T phi(K)   (normaliser)
+//     with ldmatrix.trans operands, then per 16-row Q tile  O = phi(Q) S / (phi(Q) z).
+//     The accumulator fragment of S^T is exactly the B fragment of S for the output mma.
+//   * Precision: phi() in fp32; operands are fp16.  Windows of <= HL_MAX rows use split operands
+//     (x = hi + lo, both fp16) so that the products carry ~22 bits; long windows use one term with
+//     the state scaled by 2^-ceil(log2 m) (the ratio of Eq. 3 is scale invariant).
+#include <cuda.h>
+
+#include "sla_internal.cuh"
+
+namespace sla {
+namespace {
+
+constexpr int NW = 8;                       // consumer warps = heads per slab
+constexpr int NST = 4;                      // ring stages per stream
+constexpr int TC_THREADS = (NW + 2) * 32;   // + KV producer warp + Q producer warp
+constexpr int HL_MAX = 32;                  // windows up to this length use hi+lo operands
+
+template <int D> struct Cfg {
+  static constexpr int SR = (D == 16) ? 32 : 16;          // rows per ring stage
+  static constexpr int NBOX = NW * D / 64;                // 128-byte column boxes per slab row
+  static constexpr int BOX_BYTES = SR * 128;
+  static constexpr int T_STAGE = NBOX * BOX_BYTES;        // bytes of one tensor's stage (8 KB)
+  static constexpr int KV_STAGE = 2 * T_STAGE;
+  static constexpr int RING_BYTES = NST * (KV_STAGE + T_STAGE);
+  static constexpr int SMEM_DYN = RING_BYTES + 1024;      // + alignment slack (swizzle needs 1 KB)
+};
+
+// ---- PTX wrappers ---------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred P1;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\n\t"
+        "selp.b32 %0, 1, 0, P1;\n\t}"
+        : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+  } while (!done);
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int x, int y) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cta.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+      ::"r"(dst), "l"(tm), "r"(bar), "r"(x), "r"(y) : "memory");
+}
+__device__ __forceinline__ void ldsm_x4(uint32_t addr, uint32_t (&r)[4]) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void ldsm_x4_t(uint32_t addr, uint32_t (&r)[4]) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+// D(16x8,f32) += A(16x16,f16,row) * B(16x8,f16,col)
+__device__ __forceinline__ void mma16816(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
+                                         uint32_t b0, uint32_t b1) {
+  asm volatile(
+      "mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+      : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+      : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+
+// ---- element helpers ------------------------------------------------------------------------------
+template <bool BF16>
+__device__ __forceinline__ float2 unpack2(uint32_t r) {   // two packed I/O elements -> fp32
+  if (BF16) return make_float2(__uint_as_float(r << 16), __uint_as_float(r & 0xffff0000u));
+  return __half22float2(*reinterpret_cast<const __half2*>(&r));
+}
+__device__ __forceinline__ uint32_t pack_h2(float lo, float hi) {
+  __half2 h = __floats2half2_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&h);
+}
+template <bool BF16>
+__device__ __forceinline__ uint32_t pack_out(float lo, float hi) {
+  if (BF16) {
+    __nv_bfloat162 b = __floats2bfloat162_rn(lo, hi);
+    return *reinterpret_cast<uint32_t*>(&b);
+  }
+  return pack_h2(lo, hi);
+}
+// phi(x) = elu(x)+1 (reading A1); fast exp (ex2.approx) -- relative error ~2^-21, far below fp16 operands
+__device__ __forceinline__ float phi_fast(float x) { return x > 0.f ? x + 1.f : __expf(x); }
+
+// fp32 pair -> fp16x2 "hi" and the fp16x2 residual "lo"
+__device__ __forceinline__ void split_h2(float x0, float x1, uint32_t& hi, uint32_t& lo) {
+  __half2 h = __floats2half2_rn(x0, x1);
+  float2 hf = __half22float2(h);
+  hi = *reinterpret_cast<uint32_t*>(&h);
+  lo = pack_h2(x0 - hf.x, x1 - hf.y);
+}
+
+// ---- per-warp consumer view of one ring -----------------------------------------------------------
+// Stage st of a stream holds rows [R0 + st*SR, R0 + (st+1)*SR).  `waited` = stages whose full barrier
+// this warp has observed; `released` = stages this warp has handed back to the producer.
+struct RingView {
+  uint32_t base;      // shared address of slot 0
+  uint32_t full;      // shared address of full barriers [NST]
+  uint32_t empty;     // shared address of empty barriers [NST]
+  int waited;
+  int released;
+};
+
+__device__ __forceinline__ void ring_wait_upto(RingView& rv, int stage_last) {
+  while (rv.waited <= stage_last) {
+    mbar_wait(rv.full + 8u * (rv.waited % NST), (uint32_t)((rv.waited / NST) & 1));
+    ++rv.waited;
+  }
+}
+// Release every stage that lies entirely below relative row `rel` (rows are relative to R0).
+template <int SR>
+__device__ __forceinline__ void ring_release_below(RingView& rv, int rel) {
+  while ((rv.released + 1) * SR <= rel) {
+    ring_wait_upto(rv, rv.released);   // never release a stage before it has landed (phase pacing)
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) mbar_arrive(rv.empty + 8u * (rv.released % NST));
+    ++rv.released;
+  }
+}
+
+// Shared address of (relative row rel, 16-byte chunk `chunk` of this slab row) inside a ring whose
+// slots are `slot_bytes` apart; the tensor's stage starts `toff` bytes into the slot.
+template <int D>
+__device__ __forceinline__ uint32_t ring_addr(uint32_t base, int slot_bytes, int toff, int rel, int chunk) {
+  using C = Cfg<D>;
+  const int st = rel / C::SR, r = rel % C::SR;
+  const int box = chunk >> 3, cib = chunk & 7;
+  return base + (uint32_t)((st % NST) * slot_bytes + toff + box * C::BOX_BYTES + r * 128 +
+                           ((cib ^ (r & 7)) << 4));
+}
+
+// ---- state of one (window, head) in mma fragments --------------------------------------------------
+//   ST[mt][nt][c]: S^T[r][p], r = 16*mt + g + 8*(c/2), p = 8*nt + 2*t + (c%2)   (g = lane/4, t = lane%4)
+//   Z[nt][c]     : z[p], p = 8*nt + 2*t + (c%2)  (same value in every row)
+template <int D> struct State {
+  float ST[D / 16][D / 8][4];
+  float Z[D / 8][4];
+  __device__ __forceinline__ void clear() {
+#pragma unroll
+    for (int a = 0; a < D / 16; ++a)
+#pragma unroll
+      for (int b = 0; b < D / 8; ++b)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) ST[a][b][c] = 0.f;
+#pragma unroll
+    for (int b = 0; b < D / 8; ++b)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) Z[b][c] = 0.f;
+  }
+};
+
+// One 16-row K/V tile starting at relative row `rel0` with `nvalid` rows of the current window.
+template <int D, bool BF16, bool PRECISE>
+__device__ __forceinline__ void kv_tile(const RingView& rv, int hl, int rel0, int nvalid, State<D>& s) {
+  using C = Cfg<D>;
+  const int lane = threadIdx.x & 31;
+  const int t = lane & 3;
+  const int mi = lane >> 3;
+  int trow = (lane & 7) + 8 * (mi >> 1);           // tile row this lane addresses for ldmatrix
+  if (trow >= nvalid) trow = 0;                    // clamp: row 0 of the tile is always valid
+  const int csel = mi & 1;
+  const uint32_t ones = 0x3C003C00u;               // fp16 {1,1}
+#pragma unroll
+  for (int cp = 0; cp < D / 16; ++cp) {            // 16-channel column pairs of the head
+    const int chunk = hl * (D / 8) + 2 * cp + csel;
+    uint32_t kr[4], vr[4];
+    ldsm_x4_t(ring_addr<D>(rv.base, C::KV_STAGE, 0, rel0 + trow, chunk), kr);
+    ldsm_x4_t(ring_addr<D>(rv.base, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), vr);
+    // phi(K) fragments: kr[0],kr[1] hold voxels j = 2t,2t+1; kr[2],kr[3] hold j = 2t+8,2t+9
+    uint32_t bhi[4], blo[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int j0 = 2 * t + 8 * (i >> 1);
+      float2 x = unpack2<BF16>(kr[i]);
+      float b0 = (j0 < nvalid) ? phi_fast(x.x) : 0.f;
+      float b1 = (j0 + 1 < nvalid) ? phi_fast(x.y) : 0.f;
+      if (PRECISE) split_h2(b0, b1, bhi[i], blo[i]);
+      else { bhi[i] = pack_h2(b0, b1); blo[i] = 0u; }
+    }
+    if (BF16) {                                     // V: bf16 -> fp16 (exact in the normal range)
+#pragma unroll
+      for (int i = 0; i < 4; ++i) { float2 x = unpack2<true>(vr[i]); vr[i] = pack_h2(x.x, x.y); }
+    }
+    // K fragment registers: n-tile 2cp   -> (b0,b1) = (r0,r2);  n-tile 2cp+1 -> (r1,r3)
+    // V fragment registers: m-tile cp    -> (a0,a1,a2,a3) = (r0,r1,r2,r3)
+#pragma unroll
+    for (int half = 0; half < 2; ++half) {
+      const int nt = 2 * cp + half;
+      const uint32_t b0 = bhi[half], b1 = bhi[2 + half];
+      mma16816(s.Z[nt], ones, ones, ones, ones, b0, b1);
+      if (PRECISE) mma16816(s.Z[nt], ones, ones, ones, ones, blo[half], blo[2 + half]);
+    }
+    // every m-tile of V^T meets every n-tile of phi(K): keep V fragments of all column pairs
+    // (D=16: one pair; D=32: handled by the second pass below)
+    if (D == 16) {
+#pragma unroll
+      for (int half = 0; half < 2; ++half) {
+        mma16816(s.ST[0][half], vr[0], vr[1], vr[2], vr[3], bhi[half], bhi[2 + half]);
+        if (PRECISE) mma16816(s.ST[0][half], vr[0], vr[1], vr[2], vr[3], blo[half], blo[2 + half]);
+      }
+    } else {
+      // D == 32: load both V column pairs for this K column pair
+#pragma unroll
+      for (int mt = 0; mt < D / 16; ++mt) {
+        uint32_t va[4];
+        if (mt == cp) { va[0] = vr[0]; va[1] = vr[1]; va[2] = vr[2]; va[3] = vr[3]; }
+        else {
+          const int vchunk = hl * (D / 8) + 2 * mt + csel;
+          ldsm_x4_t(ring_addr<D>(rv.base, C::KV_STAGE, C::T_STAGE, rel0 + trow, vchunk), va);
+          if (BF16) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) { float2 x = unpack2<true>(va[i]); va[i] = pack_h2(x.x, x.y); }
+          }
+        }
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+          const int nt = 2 * cp + half;
+          mma16816(s.ST[mt][nt], va[0], va[1], va[2], va[3], bhi[half], bhi[2 + half]);
+          if (PRECISE) mma16816(s.ST[mt][nt], va[0], va[1], va[2], va[3], blo[half], blo[2 + half]);
+        }
+      }
+    }
+  }
+}
+
+// B operands of the output mma, built once per (window, head) from the state.
+//   B[n2][ks] covers output channels r = 8*n2 .. 8*n2+7 and contraction p = 16*ks .. 16*ks+15.
+template <int D> struct OutOperands {
+  uint32_t hi[D / 8][D / 16][2], lo[D / 8][D / 16][2];
+  uint32_t zhi[D / 16][2], zlo[D / 16][2];
+};
+
+template <int D, bool PRECISE>
+__device__ __forceinline__ void make_out_operands(const State<D>& s, float scale, OutOperands<D>& o) {
+#pragma unroll
+  for (int n2 = 0; n2 < D / 8; ++n2)
+#pragma unroll
+    for (int ks = 0; ks < D / 16; ++ks)
+#pragma unroll
+      for (int b = 0; b < 2; ++b) {
+        const float x0 = s.ST[n2 / 2][2 * ks + b][2 * (n2 & 1)] * scale;
+        const float x1 = s.ST[n2 / 2][2 * ks + b][2 * (n2 & 1) + 1] * scale;
+        if (PRECISE) split_h2(x0, x1, o.hi[n2][ks][b], o.lo[n2][ks][b]);
+        else { o.hi[n2][ks][b] = pack_h2(x0, x1); o.lo[n2][ks][b] = 0u; }
+      }
+#pragma unroll
+  for (int ks = 0; ks < D / 16; ++ks)
+#pragma unroll
+    for (int b = 0; b < 2; ++b) {
+      const float x0 = s.Z[2 * ks + b][0] * scale, x1 = s.Z[2 * ks + b][1] * scale;
+      if (PRECISE) split_h2(x0, x1, o.zhi[ks][b], o.zlo[ks][b]);
+      else { o.zhi[ks][b] = pack_h2(x0, x1); o.zlo[ks][b] = 0u; }
+    }
+}
+
+// One 16-row Q tile: out rows [row0, row0+nvalid) of head h.
+template <int D, bool BF16, bool PRECISE, typename T>
+__device__ __forceinline__ void q_tile(const RingView& rv, int hl, int rel0, int nvalid,
+                                       const OutOperands<D>& o, T* __restrict__ out_rows /*row0, head col*/,
+                                       int C_total) {
+  using C = Cfg<D>;
+  const int lane = threadIdx.x & 31;
+  const int g = lane >> 2, t = lane & 3;
+  const int mi = lane >> 3;
+  int trow = (lane & 7) + 8 * (mi >> 1);
+  if (trow >= nvalid) trow = 0;
+  const int csel = mi & 1;
+  uint32_t ahi[D / 16][4], alo[D / 16][4];
+#pragma unroll
+  for (int ks = 0; ks < D / 16; ++ks) {
+    uint32_t qr[4];
+    ldsm_x4(ring_addr<D>(rv.base, C::T_STAGE, 0, rel0 + trow, hl * (D / 8) + 2 * ks + csel), qr);
+    // registers (rows0-7,c0),(rows0-7,c1),(rows8-15,c0),(rows8-15,c1) -> a0=r0, a1=r2, a2=r1, a3=r3
+    const int perm[4] = {0, 2, 1, 3};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      float2 x = unpack2<BF16>(qr[perm[i]]);
+      const float a0 = phi_fast(x.x), a1 = phi_fast(x.y);
+      if (PRECISE) split_h2(a0, a1, ahi[ks][i], alo[ks][i]);
+      else { ahi[ks][i] = pack_h2(a0, a1); alo[ks][i] = 0u; }
+    }
+  }
+  float den[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+  for (int ks = 0; ks < D / 16; ++ks) {
+    mma16816(den, ahi[ks][0], ahi[ks][1], ahi[ks][2], ahi[ks][3], o.zhi[ks][0], o.zhi[ks][1]);
+    if (PRECISE) {
+      mma16816(den, alo[ks][0], alo[ks][1], alo[ks][2], alo[ks][3], o.zhi[ks][0], o.zhi[ks][1]);
+      mma16816(den, ahi[ks][0], ahi[ks][1], ahi[ks][2], ahi[ks][3], o.zlo[ks][0], o.zlo[ks][1]);
+    }
+  }
+  const float inv0 = 1.f / den[0], inv1 = 1.f / den[2];
+#pragma unroll
+  for (int n2 = 0; n2 < D / 8; ++n2) {
+    float acc[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+    for (int ks = 0; ks < D / 16; ++ks) {
+      mma16816(acc, ahi[ks][0], ahi[ks][1], ahi[ks][2], ahi[ks][3], o.hi[n2][ks][0], o.hi[n2][ks][1]);
+      if (PRECISE) {
+        mma16816(acc, alo[ks][0], alo[ks][1], alo[ks][2], alo[ks][3], o.hi[n2][ks][0], o.hi[n2][ks][1]);
+        mma16816(acc, ahi[ks][0], ahi[ks][1], ahi[ks][2], ahi[ks][3], o.lo[n2][ks][0], o.lo[n2][ks][1]);
+      }
+    }
+    uint32_t* p0 = reinterpret_cast<uint32_t*>(out_rows + (size_t)g * C_total + 8 * n2 + 2 * t);
+    uint32_t* p1 = reinterpret_cast<uint32_t*>(out_rows + (size_t)(g + 8) * C_total + 8 * n2 + 2 * t);
+    if (g < nvalid) *p0 = pack_out<BF16>(acc[0] * inv0, acc[1] * inv0);
+    if (g + 8 < nvalid) *p1 = pack_out<BF16>(acc[2] * inv1, acc[3] * inv1);
+  }
+}

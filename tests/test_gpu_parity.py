@@ -66,8 +66,10 @@ def check_grads(grads, ref, sc):
     for name, got, want in zip(("dq", "dk", "dv"), grads, ref):
         check(f"{sc.name}.{name}", got, want, sc.dtype, sc.lengths)
         gotd = got.double().cpu().numpy()
-        rel = np.linalg.norm(gotd - want) / max(np.linalg.norm(want), 1e-300)
-        assert rel <= REL_L2[sc.dtype], f"{sc.name}.{name}: relative L2 {rel:.3e}"
+        # mixed criterion: ||diff|| <= REL_L2*||want|| + atol*sqrt(n)  (length-1 windows have dq = dk = 0
+        # exactly, so a purely relative norm is meaningless there)
+        bound = REL_L2[sc.dtype] * np.linalg.norm(want) + TOL[sc.dtype][1] * np.sqrt(want.size)
+        assert np.linalg.norm(gotd - want) <= bound, f"{sc.name}.{name}: L2 error {np.linalg.norm(gotd - want):.3e} > {bound:.3e}"
 
 
 # ---- prep kernel: bit-exact ----------------------------------------------------------------------
