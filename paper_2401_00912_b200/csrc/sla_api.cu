@@ -1,5 +1,7 @@
 // sla_api.cu -- the extern "C" boundary declared in include/sla.h: argument validation, workspace
 // carving and kernel dispatch.  No torch types; plain pointers and sizes.
+#include <cstdlib>
+
 #include "sla_internal.cuh"
 
 namespace {
@@ -69,7 +71,9 @@ int sla_forward(const void* q, const void* k, const void* v, const int32_t* wind
   p.q = q; p.k = k; p.v = v; p.out = out; p.off = window_offsets;
   p.ws_state = static_cast<float*>(workspace);
   p.N = (int)N; p.W = W; p.H = H; p.d = d_h;
-  cudaError_t e = sla::launch_forward_generic(p, dt, st);
+  const char* force = getenv("SLA_FORCE_GENERIC");            // debugging/A-B switch, not a fallback
+  const bool tc = !(force && force[0] == '1') && sla::forward_tc_supported(p, dt);
+  cudaError_t e = tc ? sla::launch_forward_tc(p, dt, st) : sla::launch_forward_generic(p, dt, st);
   return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
 }
 

@@ -331,3 +331,291 @@ __device__ __forceinline__ void q_tile(const RingView& rv, int hl, int rel0, int
     if (g + 8 < nvalid) *p1 = pack_out<BF16>(acc[2] * inv1, acc[3] * inv1);
   }
 }
+
+// ---- CTA-level shared control block ----------------------------------------------------------------
+struct Ctrl {
+  unsigned long long full_kv[NST], empty_kv[NST], full_q[NST], empty_q[NST];
+  int wa;            // window containing row R0
+  int stream_end;    // one past the last row any owned item touches (>= R0)
+};
+
+// Largest w in [0,W) with off[w] <= row (row < off[W] = N), found by one warp with 32-way probes.
+__device__ __forceinline__ int warp_window_of_row(const int32_t* __restrict__ off, int W, int row) {
+  const int lane = threadIdx.x & 31;
+  int lo = 0, hi = W;
+  while (hi - lo > 1) {
+    const int step = (hi - lo + 31) / 32;
+    const int idx = lo + (lane + 1) * step;
+    const bool ok = idx < hi && __ldg(off + idx) <= row;
+    const int cnt = __popc(__ballot_sync(0xffffffffu, ok));
+    const int nlo = lo + cnt * step;
+    hi = min(hi, nlo + step);
+    lo = nlo;
+  }
+  return lo;
+}
+
+// One whole (fused) window [s,e) for head slot hl: state pass over K,V then output pass over Q.
+template <int D, bool BF16, bool PRECISE, typename T>
+__device__ __forceinline__ void process_window(RingView& kv, RingView& qv, int hl, int R0, int s, int e,
+                                               T* __restrict__ out_head /*out + head column*/, int Ctot) {
+  using C = Cfg<D>;
+  State<D> st;
+  st.clear();
+  for (int r = s; r < e; r += 16) {
+    const int nv = min(16, e - r), rel = r - R0;
+    ring_release_below<C::SR>(kv, rel);   // skipped rows first: a wait must never pin older stages
+    ring_wait_upto(kv, (rel + nv - 1) / C::SR);
+    kv_tile<D, BF16, PRECISE>(kv, hl, rel, nv, st);
+    ring_release_below<C::SR>(kv, rel + nv);
+  }
+  const int m = e - s;
+  const int lg = 32 - __clz(m - 1);                       // ceil(log2 m), 0 for m = 1
+  const float scale = __int_as_float((127 - lg) << 23);   // 2^-lg: keeps fp16 operands O(1)
+  OutOperands<D> oo;
+  make_out_operands<D, PRECISE>(st, scale, oo);
+  for (int r = s; r < e; r += 16) {
+    const int nv = min(16, e - r), rel = r - R0;
+    ring_release_below<C::SR>(qv, rel);
+    ring_wait_upto(qv, (rel + nv - 1) / C::SR);
+    q_tile<D, BF16, PRECISE, T>(qv, hl, rel, nv, oo, out_head + (size_t)r * Ctot, Ctot);
+    ring_release_below<C::SR>(qv, rel + nv);
+  }
+}
+
+// The piece [ps,pe) of a split window that starts at row s: partial state -> workspace atomics.
+template <int D, bool BF16>
+__device__ __forceinline__ void process_piece(RingView& kv, int hl, int R0, int ps, int pe,
+                                              float* __restrict__ slot) {
+  using C = Cfg<D>;
+  const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  State<D> st;
+  st.clear();
+  for (int r = ps; r < pe; r += 16) {
+    const int nv = min(16, pe - r), rel = r - R0;
+    ring_release_below<C::SR>(kv, rel);
+    ring_wait_upto(kv, (rel + nv - 1) / C::SR);
+    kv_tile<D, BF16, false>(kv, hl, rel, nv, st);
+    ring_release_below<C::SR>(kv, rel + nv);
+  }
+#pragma unroll
+  for (int mt = 0; mt < D / 16; ++mt)
+#pragma unroll
+    for (int nt = 0; nt < D / 8; ++nt)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const int r = 16 * mt + g + 8 * (c >> 1), p = 8 * nt + 2 * t + (c & 1);
+        atomicAdd(slot + p * D + r, st.ST[mt][nt][c]);
+      }
+  if (g == 0) {
+#pragma unroll
+    for (int nt = 0; nt < D / 8; ++nt)
+#pragma unroll
+      for (int c = 0; c < 2; ++c) atomicAdd(slot + D * D + 8 * nt + 2 * t + c, st.Z[nt][c]);
+  }
+}
+
+template <int D, bool BF16, typename T>
+__global__ void __launch_bounds__(TC_THREADS, 2)
+sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
+                  const __grid_constant__ CUtensorMap tmV, const int32_t* __restrict__ off,
+                  T* __restrict__ out, float* __restrict__ ws, int N, int W, int H, int span) {
+  using C = Cfg<D>;
+  extern __shared__ uint8_t dyn_smem[];
+  __shared__ Ctrl ctrl;
+  const uint32_t ring = (smem_u32(dyn_smem) + 1023u) & ~1023u;
+  const uint32_t kv_base = ring, q_base = ring + NST * C::KV_STAGE;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int R0 = blockIdx.x * span, R1 = min(R0 + span, N);
+  const int h0 = blockIdx.y * NW;
+  const int nact = min(NW, H - h0);
+  const int Ctot = H * D;
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < NST; ++i) {
+      mbar_init(smem_u32(&ctrl.full_kv[i]), 1);
+      mbar_init(smem_u32(&ctrl.empty_kv[i]), nact);
+      mbar_init(smem_u32(&ctrl.full_q[i]), 1);
+      mbar_init(smem_u32(&ctrl.empty_q[i]), nact);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  if (warp >= NW) {
+    // ---------------- producer warps: warp NW streams K,V; warp NW+1 streams Q ----------------
+    const bool is_kv = (warp == NW);
+    const uint32_t full = smem_u32(is_kv ? ctrl.full_kv : ctrl.full_q);
+    const uint32_t empty = smem_u32(is_kv ? ctrl.empty_kv : ctrl.empty_q);
+    const uint32_t base = is_kv ? kv_base : q_base;
+    const int slot_bytes = is_kv ? C::KV_STAGE : C::T_STAGE;
+    auto issue = [&](int st) {
+      const int slot = st % NST;
+      const uint32_t bar = full + 8u * slot;
+      const uint32_t dst = base + slot * slot_bytes;
+      const int y = R0 + st * C::SR;
+      mbar_expect_tx(bar, (uint32_t)slot_bytes);
+#pragma unroll
+      for (int b = 0; b < C::NBOX; ++b) {
+        const int x = h0 * D + 64 * b;
+        if (is_kv) {
+          tma_load_2d(dst + b * C::BOX_BYTES, &tmK, bar, x, y);
+          tma_load_2d(dst + C::T_STAGE + b * C::BOX_BYTES, &tmV, bar, x, y);
+        } else {
+          tma_load_2d(dst + b * C::BOX_BYTES, &tmQ, bar, x, y);
+        }
+      }
+    };
+    const int first = min(NST, (N - R0 + C::SR - 1) / C::SR);   // speculative first fill
+    if (lane == 0)
+      for (int st = 0; st < first; ++st) issue(st);
+    __syncthreads();                                           // setup published (ctrl.stream_end)
+    if (lane == 0) {
+      const int total = (ctrl.stream_end - R0 + C::SR - 1) / C::SR;
+      for (int st = first; st < total; ++st) {
+        mbar_wait(empty + 8u * (st % NST), (uint32_t)(((st / NST) - 1) & 1));
+        issue(st);
+      }
+      const int issued = max(first, total);
+      for (int st = max(0, issued - NST); st < issued; ++st)    // no TMA may be in flight at exit
+        mbar_wait(full + 8u * (st % NST), (uint32_t)((st / NST) & 1));
+    }
+    return;
+  }
+
+  // ---------------- consumer warps ----------------
+  if (warp == 0) {
+    const int wa = warp_window_of_row(off, W, R0);
+    const int wl = warp_window_of_row(off, W, R1 - 1);
+    if (lane == 0) {
+      const int sl = __ldg(off + wl), el = __ldg(off + wl + 1);
+      int se;
+      if (el - sl <= kFuseMax) se = (sl >= R0) ? el : R0;   // last window fused: owned iff it starts here
+      else se = R1;                                         // split: this CTA's piece ends at R1
+      ctrl.wa = wa;
+      ctrl.stream_end = se;
+    }
+  }
+  __syncthreads();
+  if (warp >= nact) return;
+
+  const int hl = warp;
+  const int stream_end = ctrl.stream_end;
+  const int total = (stream_end - R0 + C::SR - 1) / C::SR;
+  RingView kv{kv_base, smem_u32(ctrl.full_kv), smem_u32(ctrl.empty_kv), 0, 0};
+  RingView qv{q_base, smem_u32(ctrl.full_q), smem_u32(ctrl.empty_q), 0, 0};
+  T* out_head = out + (size_t)(h0 + hl) * D;
+
+  // window walk with a 32-entry register cache of the offsets (one global round trip per 31 windows)
+  int wbase = ctrl.wa;
+  int cur = __ldg(off + min(wbase + lane, W));
+  int nxt = __ldg(off + min(wbase + 31 + lane, W));
+  for (int w = wbase; w < W; ++w) {
+    int i = w - wbase;
+    if (i >= 31) {
+      wbase += 31;
+      cur = nxt;
+      nxt = __ldg(off + min(wbase + 31 + lane, W));
+      i = 0;
+    }
+    const int s = __shfl_sync(0xffffffffu, cur, i), e = __shfl_sync(0xffffffffu, cur, i + 1);
+    if (s >= R1) break;
+    const int m = e - s;
+    if (m <= 0) continue;
+    if (m <= kFuseMax) {
+      if (s < R0) continue;   // owned by the CTA whose span holds its first row
+      if (m <= HL_MAX) process_window<D, BF16, true, T>(kv, qv, hl, R0, s, e, out_head, Ctot);
+      else process_window<D, BF16, false, T>(kv, qv, hl, R0, s, e, out_head, Ctot);
+    } else {
+      float* slot = ws + ((size_t)(s / (kFuseMax + 1)) * H + (h0 + hl)) * (size_t)((D + 1) * D);
+      process_piece<D, BF16>(kv, hl, R0, max(s, R0), min(e, R1), slot);
+    }
+  }
+  // hand back every remaining stage the producers will issue (rows of split windows' Q, tail rows)
+  ring_release_below<C::SR>(kv, total * C::SR);
+  ring_release_below<C::SR>(qv, total * C::SR);
+}
+
+// ---- host side -------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
+                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                  CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = []() -> EncodeTiledFn {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      return nullptr;
+    return reinterpret_cast<EncodeTiledFn>(p);
+  }();
+  return fn;
+}
+
+// 2-D map over a row-major [N, C] 16-bit tensor; box = 64 columns (128 B) x box_rows, 128-B swizzle.
+bool make_map(CUtensorMap* tm, const void* base, int N, int C, int box_rows) {
+  EncodeTiledFn enc = encode_fn();
+  if (!enc) return false;
+  const cuuint64_t dims[2] = {(cuuint64_t)C, (cuuint64_t)N};
+  const cuuint64_t strides[1] = {(cuuint64_t)C * 2};
+  const cuuint32_t box[2] = {64u, (cuuint32_t)box_rows};
+  const cuuint32_t estr[2] = {1u, 1u};
+  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+int sm_count() {
+  static int n = []() {
+    int dev = 0, v = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
+    return v > 0 ? v : 148;
+  }();
+  return n;
+}
+
+template <int D, bool BF16, typename T>
+cudaError_t tc_launch(const Problem& p, cudaStream_t st) {
+  using C = Cfg<D>;
+  CUtensorMap tq, tk, tv;
+  const int Ctot = p.H * D;
+  if (!make_map(&tq, p.q, p.N, Ctot, C::SR) || !make_map(&tk, p.k, p.N, Ctot, C::SR) ||
+      !make_map(&tv, p.v, p.N, Ctot, C::SR))
+    return cudaErrorInvalidValue;
+  auto kern = sla_fwd_tc_kernel<D, BF16, T>;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_DYN);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  const int slabs = (p.H + NW - 1) / NW;
+  int nx = (2 * sm_count() + slabs - 1) / slabs;             // two CTAs per SM
+  int span = (p.N + nx - 1) / nx;
+  span = (span + 15) / 16 * 16;
+  if (span < 64) span = 64;
+  nx = (p.N + span - 1) / span;
+  dim3 grid(nx, slabs);
+  kern<<<grid, TC_THREADS, C::SMEM_DYN, st>>>(tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H, span);
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+bool forward_tc_supported(const Problem& p, int dt) {
+  if (dt != SLA_F16 && dt != SLA_BF16) return false;
+  if ((p.H * p.d) % 64 != 0) return false;                     // slab rows are whole 128-byte boxes
+  return encode_fn() != nullptr;
+}
+
+cudaError_t launch_forward_tc(const Problem& p, int dt, cudaStream_t st) {
+  cudaError_t e;
+  if (p.d == 16) e = (dt == SLA_F16) ? tc_launch<16, false, __half>(p, st) : tc_launch<16, true, __nv_bfloat16>(p, st);
+  else e = (dt == SLA_F16) ? tc_launch<32, false, __half>(p, st) : tc_launch<32, true, __nv_bfloat16>(p, st);
+  if (e != cudaSuccess) return e;
+  return launch_forward_generic_split_only(p, dt, st);        // outputs of split windows
+}
+
+}  // namespace sla

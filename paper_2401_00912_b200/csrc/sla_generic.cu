@@ -486,6 +486,16 @@ cudaError_t fwd_launch(const Problem& p, cudaStream_t st) {
 }
 
 template <typename T, int D>
+cudaError_t fwd_split_launch(const Problem& p, cudaStream_t st) {
+  const int CB = block_threads(p.H, D);
+  const int HB = CB / D;
+  dim3 grid((p.N + kTileRows - 1) / kTileRows, (p.H + HB - 1) / HB);
+  sla_fwd_generic_split_kernel<T, D><<<grid, CB, 0, st>>>((const T*)p.q, p.off, (T*)p.out, p.ws_state,
+                                                          p.N, p.W, p.H);
+  return cudaGetLastError();
+}
+
+template <typename T, int D>
 cudaError_t bwd_launch(const Problem& p, cudaStream_t st) {
   const int CB = block_threads(p.H, D);
   const int HB = CB / D;
@@ -513,6 +523,17 @@ cudaError_t launch_forward_generic(const Problem& p, int dt, cudaStream_t st) {
   if (dt == SLA_F32) return fwd_launch<float, 32>(p, st);
   if (dt == SLA_F16) return fwd_launch<__half, 32>(p, st);
   return fwd_launch<__nv_bfloat16, 32>(p, st);
+}
+
+cudaError_t launch_forward_generic_split_only(const Problem& p, int dt, cudaStream_t st) {
+  if (p.d == 16) {
+    if (dt == SLA_F32) return fwd_split_launch<float, 16>(p, st);
+    if (dt == SLA_F16) return fwd_split_launch<__half, 16>(p, st);
+    return fwd_split_launch<__nv_bfloat16, 16>(p, st);
+  }
+  if (dt == SLA_F32) return fwd_split_launch<float, 32>(p, st);
+  if (dt == SLA_F16) return fwd_split_launch<__half, 32>(p, st);
+  return fwd_split_launch<__nv_bfloat16, 32>(p, st);
 }
 
 cudaError_t launch_backward_generic(const Problem& p, int dt, cudaStream_t st) {
