@@ -12,7 +12,8 @@ inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 
 // fp32 accumulators for windows split across thread blocks: one slot per possible split window.
 inline size_t state_slots(int64_t N) { return (size_t)(N / (sla::kFuseMax + 1)) + 1; }
 inline size_t state_bytes(int64_t N, int H, int d) {
-  return state_slots(N) * (size_t)H * (size_t)(d + 1) * (size_t)d * sizeof(float);
+  return sla::kWsHeaderFloats * sizeof(float) +
+         state_slots(N) * (size_t)H * (size_t)(d + 1) * (size_t)d * sizeof(float);
 }
 
 int check_common(int64_t N, int32_t W, int32_t H, int32_t d_h, int dt) {

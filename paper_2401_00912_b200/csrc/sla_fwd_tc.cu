@@ -20,21 +20,24 @@
 //     the state scaled by 2^-ceil(log2 m) (the ratio of Eq. 3 is scale invariant).
 #include <cuda.h>
 
+#include <cstdlib>
+
 #include "sla_internal.cuh"
 
 namespace sla {
 namespace {
 
 constexpr int NW = 8;                       // consumer warps = heads per slab
-constexpr int NST = 4;                      // ring stages per stream
-constexpr int TC_THREADS = (NW + 2) * 32;   // + KV producer warp + Q producer warp
-constexpr int HL_MAX = 32;                  // windows up to this length use hi+lo operands
+constexpr int NST = 4;                      // ring stages per stream (power of two)
+constexpr int TC_THREADS = (NW + 1) * 32;   // + one producer warp (lane 0: K,V stream; lane 1: Q stream)
+constexpr int HL_MAX = 16;                  // windows up to this length use hi+lo operands
+constexpr int QUAD_MAX = 16;                // windows up to this length are packed into quadratic-form tiles
 
 template <int D> struct Cfg {
-  static constexpr int SR = (D == 16) ? 32 : 16;          // rows per ring stage
+  static constexpr int SR = 16;                           // rows per ring stage
   static constexpr int NBOX = NW * D / 64;                // 128-byte column boxes per slab row
   static constexpr int BOX_BYTES = SR * 128;
-  static constexpr int T_STAGE = NBOX * BOX_BYTES;        // bytes of one tensor's stage (8 KB)
+  static constexpr int T_STAGE = NBOX * BOX_BYTES;        // bytes of one tensor's stage (4 / 8 KB)
   static constexpr int KV_STAGE = 2 * T_STAGE;
   static constexpr int RING_BYTES = NST * (KV_STAGE + T_STAGE);
   static constexpr int SMEM_DYN = RING_BYTES + 1024;      // + alignment slack (swizzle needs 1 KB)
@@ -58,9 +61,9 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   do {
     asm volatile(
         "{\n\t.reg .pred P1;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2, %3;\n\t"
         "selp.b32 %0, 1, 0, P1;\n\t}"
-        : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+        : "=r"(done) : "r"(bar), "r"(parity), "r"(20000u) : "memory");
   } while (!done);
 }
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int x, int y) {
@@ -105,6 +108,26 @@ __device__ __forceinline__ uint32_t pack_out(float lo, float hi) {
 }
 // phi(x) = elu(x)+1 (reading A1); fast exp (ex2.approx) -- relative error ~2^-21, far below fp16 operands
 __device__ __forceinline__ float phi_fast(float x) { return x > 0.f ? x + 1.f : __expf(x); }
+
+// phi on two packed I/O elements, evaluated in fp16x2 (long windows only: the operand is rounded to
+// fp16 anyway; x+1 is the same single rounding, exp(x) = ex2(x*log2e) costs ~2 extra fp16 ulps on
+// negative inputs, whose phi < 1).  Result: fp16x2 {phi(x0), phi(x1)}.
+template <bool BF16>
+__device__ __forceinline__ uint32_t phi_h2(uint32_t raw) {
+  uint32_t x = raw;
+  if (BF16) { float2 f = unpack2<true>(raw); x = pack_h2(f.x, f.y); }
+  uint32_t e, p1, m;
+  const uint32_t log2e = 0x3DC53DC5u, one = 0x3C003C00u, zero = 0u;   // fp16 1.4424, 1.0
+  asm("{\n\t.reg .b32 t;\n\tmul.f16x2 t, %1, %2;\n\tex2.approx.f16x2 %0, t;\n\t}" : "=r"(e) : "r"(x), "r"(log2e));
+  asm("add.f16x2 %0, %1, %2;" : "=r"(p1) : "r"(x), "r"(one));
+  asm("set.gt.u32.f16x2 %0, %1, %2;" : "=r"(m) : "r"(x), "r"(zero));     // 0xFFFF per lane where x > 0
+  return (p1 & m) | (e & ~m);
+}
+__device__ __forceinline__ float fast_rcp(float x) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
 
 // fp32 pair -> fp16x2 "hi" and the fp16x2 residual "lo"
 __device__ __forceinline__ void split_h2(float x0, float x1, uint32_t& hi, uint32_t& lo) {
@@ -192,14 +215,26 @@ __device__ __forceinline__ void kv_tile(const RingView& rv, int hl, int rel0, in
     ldsm_x4_t(ring_addr<D>(rv.base, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), vr);
     // phi(K) fragments: kr[0],kr[1] hold voxels j = 2t,2t+1; kr[2],kr[3] hold j = 2t+8,2t+9
     uint32_t bhi[4], blo[4];
+    if (PRECISE) {
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      const int j0 = 2 * t + 8 * (i >> 1);
-      float2 x = unpack2<BF16>(kr[i]);
-      float b0 = (j0 < nvalid) ? phi_fast(x.x) : 0.f;
-      float b1 = (j0 + 1 < nvalid) ? phi_fast(x.y) : 0.f;
-      if (PRECISE) split_h2(b0, b1, bhi[i], blo[i]);
-      else { bhi[i] = pack_h2(b0, b1); blo[i] = 0u; }
+      for (int i = 0; i < 4; ++i) {
+        const int j0 = 2 * t + 8 * (i >> 1);
+        float2 x = unpack2<BF16>(kr[i]);
+        float b0 = (j0 < nvalid) ? phi_fast(x.x) : 0.f;
+        float b1 = (j0 + 1 < nvalid) ? phi_fast(x.y) : 0.f;
+        split_h2(b0, b1, bhi[i], blo[i]);
+      }
+    } else {
+#pragma unroll
+      for (int i = 0; i < 4; ++i) { bhi[i] = phi_h2<BF16>(kr[i]); blo[i] = 0u; }
+      if (nvalid < 16) {                            // ragged last tile of the window: zero phi(K) rows
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const int j0 = 2 * t + 8 * (i >> 1);
+          const uint32_t msk = ((j0 < nvalid) ? 0x0000FFFFu : 0u) | ((j0 + 1 < nvalid) ? 0xFFFF0000u : 0u);
+          bhi[i] &= msk;
+        }
+      }
     }
     if (BF16) {                                     // V: bf16 -> fp16 (exact in the normal range)
 #pragma unroll
@@ -298,10 +333,13 @@ __device__ __forceinline__ void q_tile(const RingView& rv, int hl, int rel0, int
     const int perm[4] = {0, 2, 1, 3};
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-      float2 x = unpack2<BF16>(qr[perm[i]]);
-      const float a0 = phi_fast(x.x), a1 = phi_fast(x.y);
-      if (PRECISE) split_h2(a0, a1, ahi[ks][i], alo[ks][i]);
-      else { ahi[ks][i] = pack_h2(a0, a1); alo[ks][i] = 0u; }
+      if (PRECISE) {
+        float2 x = unpack2<BF16>(qr[perm[i]]);
+        split_h2(phi_fast(x.x), phi_fast(x.y), ahi[ks][i], alo[ks][i]);
+      } else {
+        ahi[ks][i] = phi_h2<BF16>(qr[perm[i]]);
+        alo[ks][i] = 0u;
+      }
     }
   }
   float den[4] = {0.f, 0.f, 0.f, 0.f};
@@ -313,7 +351,7 @@ __device__ __forceinline__ void q_tile(const RingView& rv, int hl, int rel0, int
       mma16816(den, ahi[ks][0], ahi[ks][1], ahi[ks][2], ahi[ks][3], o.zlo[ks][0], o.zlo[ks][1]);
     }
   }
-  const float inv0 = 1.f / den[0], inv1 = 1.f / den[2];
+  const float inv0 = fast_rcp(den[0]), inv1 = fast_rcp(den[2]);
 #pragma unroll
   for (int n2 = 0; n2 < D / 8; ++n2) {
     float acc[4] = {0.f, 0.f, 0.f, 0.f};
@@ -332,71 +370,174 @@ __device__ __forceinline__ void q_tile(const RingView& rv, int hl, int rel0, int
   }
 }
 
+// ---- packed short windows: masked quadratic form inside one 16-row tile -----------------------------
+// Several WHOLE windows of <= 16 rows each are packed into one tile of <= 16 consecutive rows and
+// evaluated in the (mathematically identical) quadratic form
+//   P = phi(Q) phi(K)^T  masked to same-window pairs,   O = (P / rowsum P) V
+// so a 1-voxel window costs 1/16 of a tile instead of a whole one.  phi(Q), phi(K) and the normalised
+// P are split into fp16 hi+lo operands (~22-bit products).  `wid` = window ordinal of tile row `lane`
+// (lanes >= nvalid hold -1).
+template <int D, bool BF16, typename T>
+__device__ __forceinline__ void quad_tile(const RingView& kv, const RingView& qv, int hl, int rel0,
+                                          int nvalid, int wid, T* __restrict__ out_rows, int C_total) {
+  using C = Cfg<D>;
+  const int lane = threadIdx.x & 31;
+  const int g = lane >> 2, t = lane & 3;
+  const int mi = lane >> 3;
+  int trow = (lane & 7) + 8 * (mi >> 1);
+  if (trow >= nvalid) trow = 0;
+  const int csel = mi & 1;
+  // P[jt][c]: rows i = g (c<2) / g+8 (c>=2), cols j = 8*jt + 2t + (c&1)
+  float P[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+#pragma unroll
+  for (int ks = 0; ks < D / 16; ++ks) {
+    const int chunk = hl * (D / 8) + 2 * ks + csel;
+    uint32_t qr[4], kr[4];
+    ldsm_x4(ring_addr<D>(qv.base, C::T_STAGE, 0, rel0 + trow, chunk), qr);
+    ldsm_x4(ring_addr<D>(kv.base, C::KV_STAGE, 0, rel0 + trow, chunk), kr);
+    uint32_t ahi[4], alo[4], bhi[4], blo[4];
+    const int perm[4] = {0, 2, 1, 3};   // (rows0-7,c0),(rows0-7,c1),(rows8-15,c0),(rows8-15,c1) -> a0..a3
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      float2 x = unpack2<BF16>(qr[perm[i]]);
+      split_h2(phi_fast(x.x), phi_fast(x.y), ahi[i], alo[i]);
+      float2 y = unpack2<BF16>(kr[i]);
+      split_h2(phi_fast(y.x), phi_fast(y.y), bhi[i], blo[i]);
+    }
+    // K (non-transposed) as B operand: j-tile 0 -> (b0,b1) = (r0,r1); j-tile 1 -> (r2,r3)
+#pragma unroll
+    for (int jt = 0; jt < 2; ++jt) {
+      mma16816(P[jt], ahi[0], ahi[1], ahi[2], ahi[3], bhi[2 * jt], bhi[2 * jt + 1]);
+      mma16816(P[jt], alo[0], alo[1], alo[2], alo[3], bhi[2 * jt], bhi[2 * jt + 1]);
+      mma16816(P[jt], ahi[0], ahi[1], ahi[2], ahi[3], blo[2 * jt], blo[2 * jt + 1]);
+    }
+  }
+  // same-window mask and row sums
+  const int wi0 = __shfl_sync(0xffffffffu, wid, g), wi1 = __shfl_sync(0xffffffffu, wid, g + 8);
+  float rs0 = 0.f, rs1 = 0.f;
+#pragma unroll
+  for (int jt = 0; jt < 2; ++jt)
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+      const int wj = __shfl_sync(0xffffffffu, wid, 8 * jt + 2 * t + c);
+      P[jt][c] = (wj == wi0 && wj >= 0) ? P[jt][c] : 0.f;
+      P[jt][2 + c] = (wj == wi1 && wj >= 0) ? P[jt][2 + c] : 0.f;
+      rs0 += P[jt][c];
+      rs1 += P[jt][2 + c];
+    }
+  rs0 += __shfl_xor_sync(0xffffffffu, rs0, 1); rs0 += __shfl_xor_sync(0xffffffffu, rs0, 2);
+  rs1 += __shfl_xor_sync(0xffffffffu, rs1, 1); rs1 += __shfl_xor_sync(0xffffffffu, rs1, 2);
+  const float inv0 = (g < nvalid) ? fast_rcp(rs0) : 0.f, inv1 = (g + 8 < nvalid) ? fast_rcp(rs1) : 0.f;
+  // normalised weights as A operand (k = j): a0=(g,2t..) a1=(g+8,2t..) a2=(g,2t+8..) a3=(g+8,2t+8..)
+  uint32_t phi_[4], plo_[4];
+  split_h2(P[0][0] * inv0, P[0][1] * inv0, phi_[0], plo_[0]);
+  split_h2(P[0][2] * inv1, P[0][3] * inv1, phi_[1], plo_[1]);
+  split_h2(P[1][0] * inv0, P[1][1] * inv0, phi_[2], plo_[2]);
+  split_h2(P[1][2] * inv1, P[1][3] * inv1, phi_[3], plo_[3]);
+#pragma unroll
+  for (int cp = 0; cp < D / 16; ++cp) {
+    uint32_t vr[4];
+    ldsm_x4_t(ring_addr<D>(kv.base, C::KV_STAGE, C::T_STAGE, rel0 + trow, hl * (D / 8) + 2 * cp + csel), vr);
+    if (BF16) {
+#pragma unroll
+      for (int i = 0; i < 4; ++i) { float2 x = unpack2<true>(vr[i]); vr[i] = pack_h2(x.x, x.y); }
+    }
+    // V (transposed) as B operand: n-tile 2cp -> (r0,r2); n-tile 2cp+1 -> (r1,r3)
+#pragma unroll
+    for (int half = 0; half < 2; ++half) {
+      const int nt = 2 * cp + half;
+      float acc[4] = {0.f, 0.f, 0.f, 0.f};
+      mma16816(acc, phi_[0], phi_[1], phi_[2], phi_[3], vr[half], vr[2 + half]);
+      mma16816(acc, plo_[0], plo_[1], plo_[2], plo_[3], vr[half], vr[2 + half]);
+      uint32_t* p0 = reinterpret_cast<uint32_t*>(out_rows + (size_t)g * C_total + 8 * nt + 2 * t);
+      uint32_t* p1 = reinterpret_cast<uint32_t*>(out_rows + (size_t)(g + 8) * C_total + 8 * nt + 2 * t);
+      if (g < nvalid) *p0 = pack_out<BF16>(acc[0], acc[1]);
+      if (g + 8 < nvalid) *p1 = pack_out<BF16>(acc[2], acc[3]);
+    }
+  }
+}
+
 // ---- CTA-level shared control block ----------------------------------------------------------------
 struct Ctrl {
   unsigned long long full_kv[NST], empty_kv[NST], full_q[NST], empty_q[NST];
   int wa;            // window containing row R0
-  int stream_end;    // one past the last row any owned item touches (>= R0)
+  int stream_begin;  // S0: first row any owned item touches
+  int stream_end;    // one past the last row any owned item touches (>= S0)
 };
 
-// Largest w in [0,W) with off[w] <= row (row < off[W] = N), found by one warp with 32-way probes.
-__device__ __forceinline__ int warp_window_of_row(const int32_t* __restrict__ off, int W, int row) {
+// For two rows at once (independent probes in flight together): the largest w in [0,W) with
+// off[w] <= row (row < off[W] = N), found by one warp with 32-way probes per round.
+__device__ __forceinline__ void warp_windows_of_rows(const int32_t* __restrict__ off, int W, int rowa,
+                                                     int rowb, int& wa, int& wb) {
   const int lane = threadIdx.x & 31;
-  int lo = 0, hi = W;
-  while (hi - lo > 1) {
-    const int step = (hi - lo + 31) / 32;
-    const int idx = lo + (lane + 1) * step;
-    const bool ok = idx < hi && __ldg(off + idx) <= row;
-    const int cnt = __popc(__ballot_sync(0xffffffffu, ok));
-    const int nlo = lo + cnt * step;
-    hi = min(hi, nlo + step);
-    lo = nlo;
+  int lo[2] = {0, 0}, hi[2] = {W, W};
+  const int row[2] = {rowa, rowb};
+  while (hi[0] - lo[0] > 1 || hi[1] - lo[1] > 1) {
+    int step[2], idx[2], val[2];
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      step[k] = max(1, (hi[k] - lo[k] + 31) / 32);
+      idx[k] = lo[k] + (lane + 1) * step[k];
+      val[k] = __ldg(off + min(idx[k], W));
+    }
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const bool ok = idx[k] < hi[k] && val[k] <= row[k];
+      const int cnt = __popc(__ballot_sync(0xffffffffu, ok));
+      const int nlo = lo[k] + cnt * step[k];
+      hi[k] = min(hi[k], nlo + step[k]);
+      lo[k] = nlo;
+    }
   }
-  return lo;
+  wa = lo[0];
+  wb = lo[1];
 }
 
 // One whole (fused) window [s,e) for head slot hl: state pass over K,V then output pass over Q.
+// Rows are addressed relative to S0, the first row of this CTA's streams.  Two 16-row tiles per
+// iteration: one wait/release bookkeeping step per 32 rows and two independent dependency chains.
 template <int D, bool BF16, bool PRECISE, typename T>
-__device__ __forceinline__ void process_window(RingView& kv, RingView& qv, int hl, int R0, int s, int e,
+__device__ __forceinline__ void process_window(RingView& kv, RingView& qv, int hl, int S0, int s, int e,
                                                T* __restrict__ out_head /*out + head column*/, int Ctot) {
   using C = Cfg<D>;
   State<D> st;
   st.clear();
-  for (int r = s; r < e; r += 16) {
-    const int nv = min(16, e - r), rel = r - R0;
+  for (int r = s; r < e; r += 32) {
+    const int nv = min(32, e - r), rel = r - S0;
     ring_release_below<C::SR>(kv, rel);   // skipped rows first: a wait must never pin older stages
     ring_wait_upto(kv, (rel + nv - 1) / C::SR);
-    kv_tile<D, BF16, PRECISE>(kv, hl, rel, nv, st);
-    ring_release_below<C::SR>(kv, rel + nv);
+    kv_tile<D, BF16, PRECISE>(kv, hl, rel, min(16, nv), st);
+    if (nv > 16) kv_tile<D, BF16, PRECISE>(kv, hl, rel + 16, nv - 16, st);
   }
   const int m = e - s;
   const int lg = 32 - __clz(m - 1);                       // ceil(log2 m), 0 for m = 1
   const float scale = __int_as_float((127 - lg) << 23);   // 2^-lg: keeps fp16 operands O(1)
   OutOperands<D> oo;
   make_out_operands<D, PRECISE>(st, scale, oo);
-  for (int r = s; r < e; r += 16) {
-    const int nv = min(16, e - r), rel = r - R0;
+  for (int r = s; r < e; r += 32) {
+    const int nv = min(32, e - r), rel = r - S0;
     ring_release_below<C::SR>(qv, rel);
     ring_wait_upto(qv, (rel + nv - 1) / C::SR);
-    q_tile<D, BF16, PRECISE, T>(qv, hl, rel, nv, oo, out_head + (size_t)r * Ctot, Ctot);
-    ring_release_below<C::SR>(qv, rel + nv);
+    q_tile<D, BF16, PRECISE, T>(qv, hl, rel, min(16, nv), oo, out_head + (size_t)r * Ctot, Ctot);
+    if (nv > 16)
+      q_tile<D, BF16, PRECISE, T>(qv, hl, rel + 16, nv - 16, oo, out_head + (size_t)(r + 16) * Ctot, Ctot);
   }
 }
 
-// The piece [ps,pe) of a split window that starts at row s: partial state -> workspace atomics.
+// The piece [ps,pe) of a split window: partial state -> workspace atomics.
 template <int D, bool BF16>
-__device__ __forceinline__ void process_piece(RingView& kv, int hl, int R0, int ps, int pe,
+__device__ __forceinline__ void process_piece(RingView& kv, int hl, int S0, int ps, int pe,
                                               float* __restrict__ slot) {
   using C = Cfg<D>;
   const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   State<D> st;
   st.clear();
-  for (int r = ps; r < pe; r += 16) {
-    const int nv = min(16, pe - r), rel = r - R0;
+  for (int r = ps; r < pe; r += 32) {
+    const int nv = min(32, pe - r), rel = r - S0;
     ring_release_below<C::SR>(kv, rel);
     ring_wait_upto(kv, (rel + nv - 1) / C::SR);
-    kv_tile<D, BF16, false>(kv, hl, rel, nv, st);
-    ring_release_below<C::SR>(kv, rel + nv);
+    kv_tile<D, BF16, false>(kv, hl, rel, min(16, nv), st);
+    if (nv > 16) kv_tile<D, BF16, false>(kv, hl, rel + 16, nv - 16, st);
   }
 #pragma unroll
   for (int mt = 0; mt < D / 16; ++mt)
@@ -416,10 +557,10 @@ __device__ __forceinline__ void process_piece(RingView& kv, int hl, int R0, int 
 }
 
 template <int D, bool BF16, typename T>
-__global__ void __launch_bounds__(TC_THREADS, 2)
+__global__ void __launch_bounds__(TC_THREADS, (D == 16 ? 3 : 2))
 sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                   const __grid_constant__ CUtensorMap tmV, const int32_t* __restrict__ off,
-                  T* __restrict__ out, float* __restrict__ ws, int N, int W, int H, int span) {
+                  T* __restrict__ out, float* __restrict__ ws, int N, int W, int H, int span, int dbg) {
   using C = Cfg<D>;
   extern __shared__ uint8_t dyn_smem[];
   __shared__ Ctrl ctrl;
@@ -443,17 +584,18 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   __syncthreads();
 
   if (warp >= NW) {
-    // ---------------- producer warps: warp NW streams K,V; warp NW+1 streams Q ----------------
-    const bool is_kv = (warp == NW);
+    // ---------------- producer warp: lane 0 streams K,V; lane 1 streams Q ----------------
+    const bool is_kv = (lane == 0);
     const uint32_t full = smem_u32(is_kv ? ctrl.full_kv : ctrl.full_q);
     const uint32_t empty = smem_u32(is_kv ? ctrl.empty_kv : ctrl.empty_q);
     const uint32_t base = is_kv ? kv_base : q_base;
     const int slot_bytes = is_kv ? C::KV_STAGE : C::T_STAGE;
+    int S0 = R0;
     auto issue = [&](int st) {
       const int slot = st % NST;
       const uint32_t bar = full + 8u * slot;
       const uint32_t dst = base + slot * slot_bytes;
-      const int y = R0 + st * C::SR;
+      const int y = S0 + st * C::SR;
       mbar_expect_tx(bar, (uint32_t)slot_bytes);
 #pragma unroll
       for (int b = 0; b < C::NBOX; ++b) {
@@ -466,18 +608,15 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
         }
       }
     };
-    const int first = min(NST, (N - R0 + C::SR - 1) / C::SR);   // speculative first fill
-    if (lane == 0)
-      for (int st = 0; st < first; ++st) issue(st);
-    __syncthreads();                                           // setup published (ctrl.stream_end)
-    if (lane == 0) {
-      const int total = (ctrl.stream_end - R0 + C::SR - 1) / C::SR;
-      for (int st = first; st < total; ++st) {
-        mbar_wait(empty + 8u * (st % NST), (uint32_t)(((st / NST) - 1) & 1));
+    __syncthreads();                                           // setup published (stream bounds)
+    if (lane < 2) {
+      S0 = ctrl.stream_begin;
+      const int total = (ctrl.stream_end - S0 + C::SR - 1) / C::SR;
+      for (int st = 0; st < total; ++st) {
+        if (st >= NST) mbar_wait(empty + 8u * (st % NST), (uint32_t)(((st / NST) - 1) & 1));
         issue(st);
       }
-      const int issued = max(first, total);
-      for (int st = max(0, issued - NST); st < issued; ++st)    // no TMA may be in flight at exit
+      for (int st = max(0, total - NST); st < total; ++st)      // no TMA may be in flight at exit
         mbar_wait(full + 8u * (st % NST), (uint32_t)((st / NST) & 1));
     }
     return;
@@ -485,51 +624,92 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
 
   // ---------------- consumer warps ----------------
   if (warp == 0) {
-    const int wa = warp_window_of_row(off, W, R0);
-    const int wl = warp_window_of_row(off, W, R1 - 1);
+    int wa, wl;
+    warp_windows_of_rows(off, W, R0, R1 - 1, wa, wl);
     if (lane == 0) {
+      const int sa = __ldg(off + wa), ea = __ldg(off + wa + 1);
       const int sl = __ldg(off + wl), el = __ldg(off + wl + 1);
+      // the window holding R0 belongs to an earlier CTA if it is fused and starts before R0
+      const int sb = (ea - sa <= kFuseMax && sa < R0) ? ea : R0;
       int se;
-      if (el - sl <= kFuseMax) se = (sl >= R0) ? el : R0;   // last window fused: owned iff it starts here
+      if (el - sl <= kFuseMax) se = (sl >= R0) ? el : sb;   // last window fused: owned iff it starts here
       else se = R1;                                         // split: this CTA's piece ends at R1
       ctrl.wa = wa;
-      ctrl.stream_end = se;
+      ctrl.stream_begin = sb;
+      ctrl.stream_end = (dbg & 2) ? sb : max(se, sb);   // dbg 2: setup only, nothing streamed
     }
   }
   __syncthreads();
   if (warp >= nact) return;
 
   const int hl = warp;
-  const int stream_end = ctrl.stream_end;
-  const int total = (stream_end - R0 + C::SR - 1) / C::SR;
+  const int S0 = ctrl.stream_begin;
+  const int total = (ctrl.stream_end - S0 + C::SR - 1) / C::SR;
   RingView kv{kv_base, smem_u32(ctrl.full_kv), smem_u32(ctrl.empty_kv), 0, 0};
   RingView qv{q_base, smem_u32(ctrl.full_q), smem_u32(ctrl.empty_q), 0, 0};
   T* out_head = out + (size_t)(h0 + hl) * D;
+  if (dbg & 1) {   // debug: stream only, no compute
+    ring_release_below<C::SR>(kv, total * C::SR);
+    ring_release_below<C::SR>(qv, total * C::SR);
+    return;
+  }
 
   // window walk with a 32-entry register cache of the offsets (one global round trip per 31 windows)
   int wbase = ctrl.wa;
   int cur = __ldg(off + min(wbase + lane, W));
   int nxt = __ldg(off + min(wbase + 31 + lane, W));
-  for (int w = wbase; w < W; ++w) {
+  auto bounds = [&](int w, int& s, int& e) {      // off[w], off[w+1]; w is non-decreasing across calls
     int i = w - wbase;
     if (i >= 31) {
       wbase += 31;
       cur = nxt;
       nxt = __ldg(off + min(wbase + 31 + lane, W));
-      i = 0;
+      i = w - wbase;
     }
-    const int s = __shfl_sync(0xffffffffu, cur, i), e = __shfl_sync(0xffffffffu, cur, i + 1);
+    s = __shfl_sync(0xffffffffu, cur, i);
+    e = __shfl_sync(0xffffffffu, cur, i + 1);
+  };
+  int w = wbase;
+  while (w < W) {
+    int s, e;
+    bounds(w, s, e);
     if (s >= R1) break;
     const int m = e - s;
-    if (m <= 0) continue;
-    if (m <= kFuseMax) {
-      if (s < R0) continue;   // owned by the CTA whose span holds its first row
-      if (m <= HL_MAX) process_window<D, BF16, true, T>(kv, qv, hl, R0, s, e, out_head, Ctot);
-      else process_window<D, BF16, false, T>(kv, qv, hl, R0, s, e, out_head, Ctot);
-    } else {
-      float* slot = ws + ((size_t)(s / (kFuseMax + 1)) * H + (h0 + hl)) * (size_t)((D + 1) * D);
-      process_piece<D, BF16>(kv, hl, R0, max(s, R0), min(e, R1), slot);
+    if (m <= 0 || (m <= kFuseMax && s < R0)) { ++w; continue; }   // empty, or owned by an earlier CTA
+    if (m <= QUAD_MAX) {
+      // pack following whole short windows (each <= QUAD_MAX rows, owned) into one 16-row tile
+      int rows = 0, ord = 0, wid = -1;
+      while (w < W) {
+        int s2, e2;
+        bounds(w, s2, e2);
+        const int m2 = e2 - s2;
+        if (m2 > 0) {
+          if (m2 > QUAD_MAX || rows + m2 > 16 || s2 >= R1) break;
+          if (lane >= rows && lane < rows + m2) wid = ord;
+          rows += m2;
+          ++ord;
+        }
+        ++w;
+      }
+      const int rel = s - S0;
+      ring_release_below<C::SR>(kv, rel);
+      ring_release_below<C::SR>(qv, rel);
+      ring_wait_upto(kv, (rel + rows - 1) / C::SR);
+      ring_wait_upto(qv, (rel + rows - 1) / C::SR);
+      quad_tile<D, BF16, T>(kv, qv, hl, rel, rows, wid, out_head + (size_t)s * Ctot, Ctot);
+      ring_release_below<C::SR>(kv, rel + rows);
+      ring_release_below<C::SR>(qv, rel + rows);
+      continue;
     }
+    if (m <= kFuseMax) {
+      if (m <= HL_MAX) process_window<D, BF16, true, T>(kv, qv, hl, S0, s, e, out_head, Ctot);
+      else process_window<D, BF16, false, T>(kv, qv, hl, S0, s, e, out_head, Ctot);
+    } else {
+      float* slot = ws + kWsHeaderFloats + ((size_t)(s / (kFuseMax + 1)) * H + (h0 + hl)) * (size_t)((D + 1) * D);
+      if (hl == 0 && lane == 0) reinterpret_cast<volatile int*>(ws)[0] = 1;   // tell the output kernel
+      process_piece<D, BF16>(kv, hl, S0, max(s, R0), min(e, R1), slot);
+    }
+    ++w;
   }
   // hand back every remaining stage the producers will issue (rows of split windows' Q, tail rows)
   ring_release_below<C::SR>(kv, total * C::SR);
@@ -592,13 +772,21 @@ cudaError_t tc_launch(const Problem& p, cudaStream_t st) {
     attr_set = true;
   }
   const int slabs = (p.H + NW - 1) / NW;
-  int nx = (2 * sm_count() + slabs - 1) / slabs;             // two CTAs per SM
+  static const int per_sm = []() {                          // resident CTAs per SM the grid is sized for
+    const char* e = getenv("SLA_TC_CTAS_PER_SM");
+    const int v = e ? atoi(e) : 0;
+    return v > 0 ? v : (D == 16 ? 3 : 2);
+  }();
+  int nx = (per_sm * sm_count() + slabs - 1) / slabs;
   int span = (p.N + nx - 1) / nx;
+  static const int dbg_env = []() { const char* e = getenv("SLA_TC_DBG"); return e ? atoi(e) : 0; }();
+  static const int span_env = []() { const char* e = getenv("SLA_TC_SPAN"); return e ? atoi(e) : 0; }();
+  if (span_env > 0) span = span_env;
   span = (span + 15) / 16 * 16;
-  if (span < 64) span = 64;
+  if (span < 32) span = 32;
   nx = (p.N + span - 1) / span;
   dim3 grid(nx, slabs);
-  kern<<<grid, TC_THREADS, C::SMEM_DYN, st>>>(tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H, span);
+  kern<<<grid, TC_THREADS, C::SMEM_DYN, st>>>(tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H, span, dbg_env);
   return cudaGetLastError();
 }
 

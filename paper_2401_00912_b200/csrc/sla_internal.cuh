@@ -53,6 +53,9 @@ __device__ __forceinline__ int window_of_row(const int32_t* __restrict__ off, in
 constexpr int kTileRows = 64;
 constexpr int kFuseMax = 256;
 constexpr int kRowBatch = 8;  // rows staged per inner step
+// The workspace starts with a 16-byte header (int flag: 1 = some window was split in this call),
+// followed by the fp32 state slots.  Zeroed by the memset at the start of every call.
+constexpr int kWsHeaderFloats = 4;
 
 struct Problem {
   const void* q; const void* k; const void* v; const void* g;

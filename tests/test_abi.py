@@ -34,8 +34,9 @@ def test_status_strings_and_version(lib):
 
 def test_workspace_bytes(lib):
     # one fp32 [H,d+1,d] slot per possible split window (> 256 rows): N//257 + 1 slots
-    assert lib.sla_workspace_bytes(60000, 1340, 8, 16, pkg.SLA_F16, 0) == (60000 // 257 + 1) * 8 * 17 * 16 * 4
-    assert lib.sla_workspace_bytes(60000, 1340, 8, 16, pkg.SLA_F16, 1) == 2 * (60000 // 257 + 1) * 8 * 17 * 16 * 4
+    one = 16 + (60000 // 257 + 1) * 8 * 17 * 16 * 4        # 16-byte header + slots
+    assert lib.sla_workspace_bytes(60000, 1340, 8, 16, pkg.SLA_F16, 0) == one
+    assert lib.sla_workspace_bytes(60000, 1340, 8, 16, pkg.SLA_F16, 1) == 2 * one
     assert lib.sla_workspace_bytes(100, 4, 8, 24, pkg.SLA_F16, 0) == 0      # unsupported d_h
     assert lib.sla_workspace_bytes(-1, 4, 8, 16, pkg.SLA_F16, 0) == 0
 
