@@ -33,7 +33,7 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     global _lib
     if _lib is not None and path is None:
         return _lib
-    p = path or LIB_PATH
+    p = path or os.environ.get("SLA_LIB_PATH") or LIB_PATH   # SLA_LIB_PATH: A/B-test another build
     if not os.path.exists(p):
         raise SlaError(f"{p} not found: build it with `python -m paper_2401_00912_b200.build` "
                        "(there is no CPU or PyTorch fallback)")

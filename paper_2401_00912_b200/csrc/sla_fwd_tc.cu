@@ -28,19 +28,32 @@ namespace sla {
 namespace {
 
 constexpr int NW = 8;                       // consumer warps = heads per slab
-constexpr int NST = 4;                      // ring stages per stream (power of two)
-constexpr int TC_THREADS = (NW + 1) * 32;   // + one producer warp (lane 0: K,V stream; lane 1: Q stream)
-constexpr int HL_MAX = 16;                  // windows up to this length use hi+lo operands
+#ifndef SLA_HPW
+#define SLA_HPW 1
+#endif
+#ifndef SLA_MINB
+#define SLA_MINB 3
+#endif
+#ifndef SLA_NST
+#define SLA_NST 3
+#endif
+#ifndef SLA_SR
+#define SLA_SR 32
+#endif
+constexpr int NST = SLA_NST;                // ring stages per stream (power of two)
 constexpr int QUAD_MAX = 16;                // windows up to this length are packed into quadratic-form tiles
 
 template <int D> struct Cfg {
-  static constexpr int SR = 16;                           // rows per ring stage
+  static constexpr int SR = SLA_SR;                       // rows per ring stage
   static constexpr int NBOX = NW * D / 64;                // 128-byte column boxes per slab row
   static constexpr int BOX_BYTES = SR * 128;
   static constexpr int T_STAGE = NBOX * BOX_BYTES;        // bytes of one tensor's stage (4 / 8 KB)
   static constexpr int KV_STAGE = 2 * T_STAGE;
   static constexpr int RING_BYTES = NST * (KV_STAGE + T_STAGE);
   static constexpr int SMEM_DYN = RING_BYTES + 1024;      // + alignment slack (swizzle needs 1 KB)
+  static constexpr int HPW = (D == 16) ? SLA_HPW : 1;     // heads per consumer warp (ILP, shared bookkeeping)
+  static constexpr int NCW = NW / HPW;                    // consumer warps per CTA
+  static constexpr int THREADS = (NCW + 1) * 32;          // + one producer warp
 };
 
 // ---- PTX wrappers ---------------------------------------------------------------------------------
@@ -82,7 +95,7 @@ __device__ __forceinline__ void ldsm_x4_t(uint32_t addr, uint32_t (&r)[4]) {
 // D(16x8,f32) += A(16x16,f16,row) * B(16x8,f16,col)
 __device__ __forceinline__ void mma16816(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
                                          uint32_t b0, uint32_t b1) {
-  asm volatile(
+  asm(
       "mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
       : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
       : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
@@ -146,11 +159,12 @@ struct RingView {
   uint32_t empty;     // shared address of empty barriers [NST]
   int waited;
   int released;
+  int nowait;         // debug: pretend every stage has landed (timing experiments only)
 };
 
 __device__ __forceinline__ void ring_wait_upto(RingView& rv, int stage_last) {
   while (rv.waited <= stage_last) {
-    mbar_wait(rv.full + 8u * (rv.waited % NST), (uint32_t)((rv.waited / NST) & 1));
+    if (!rv.nowait) mbar_wait(rv.full + 8u * (rv.waited % NST), (uint32_t)((rv.waited / NST) & 1));
     ++rv.waited;
   }
 }
@@ -160,7 +174,7 @@ __device__ __forceinline__ void ring_release_below(RingView& rv, int rel) {
   while ((rv.released + 1) * SR <= rel) {
     ring_wait_upto(rv, rv.released);   // never release a stage before it has landed (phase pacing)
     __syncwarp();
-    if ((threadIdx.x & 31) == 0) mbar_arrive(rv.empty + 8u * (rv.released % NST));
+    if ((threadIdx.x & 31) == 0 && !rv.nowait) mbar_arrive(rv.empty + 8u * (rv.released % NST));
     ++rv.released;
   }
 }
@@ -197,8 +211,9 @@ template <int D> struct State {
 };
 
 // One 16-row K/V tile starting at relative row `rel0` with `nvalid` rows of the current window.
-template <int D, bool BF16, bool PRECISE>
-__device__ __forceinline__ void kv_tile(const RingView& rv, int hl, int rel0, int nvalid, State<D>& s) {
+template <int D, bool BF16, bool PRECISE, bool FULL = false>
+__device__ __forceinline__ void kv_tile(const RingView& rv, int hl, int rel0, int nvalid_in, State<D>& s) {
+  const int nvalid = FULL ? 16 : nvalid_in;
   using C = Cfg<D>;
   const int lane = threadIdx.x & 31;
   const int t = lane & 3;
@@ -313,10 +328,11 @@ __device__ __forceinline__ void make_out_operands(const State<D>& s, float scale
 }
 
 // One 16-row Q tile: out rows [row0, row0+nvalid) of head h.
-template <int D, bool BF16, bool PRECISE, typename T>
-__device__ __forceinline__ void q_tile(const RingView& rv, int hl, int rel0, int nvalid,
+template <int D, bool BF16, bool PRECISE, typename T, bool FULL = false>
+__device__ __forceinline__ void q_tile(const RingView& rv, int hl, int rel0, int nvalid_in,
                                        const OutOperands<D>& o, T* __restrict__ out_rows /*row0, head col*/,
                                        int C_total) {
+  const int nvalid = FULL ? 16 : nvalid_in;
   using C = Cfg<D>;
   const int lane = threadIdx.x & 31;
   const int g = lane >> 2, t = lane & 3;
@@ -457,6 +473,20 @@ __device__ __forceinline__ void quad_tile(const RingView& kv, const RingView& qv
   }
 }
 
+#ifdef SLA_TRACE
+__device__ unsigned long long g_trace[8192 * 4];
+__device__ __forceinline__ unsigned long long gtime() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+  return t;
+}
+#define TRACE(slot) do { if (threadIdx.x == 0 && blockIdx.x < 8192) g_trace[blockIdx.x * 4 + (slot)] = gtime(); } while (0)
+#define TRACE_SM() do { if (threadIdx.x == 0 && blockIdx.x < 8192) { unsigned sm; asm("mov.u32 %0, %smid;" : "=r"(sm)); g_trace[blockIdx.x * 4 + 3] = sm; } } while (0)
+#else
+#define TRACE(slot) do {} while (0)
+#define TRACE_SM() do {} while (0)
+#endif
+
 // ---- CTA-level shared control block ----------------------------------------------------------------
 struct Ctrl {
   unsigned long long full_kv[NST], empty_kv[NST], full_q[NST], empty_q[NST];
@@ -497,67 +527,99 @@ __device__ __forceinline__ void warp_windows_of_rows(const int32_t* __restrict__
 // Rows are addressed relative to S0, the first row of this CTA's streams.  Two 16-row tiles per
 // iteration: one wait/release bookkeeping step per 32 rows and two independent dependency chains.
 template <int D, bool BF16, bool PRECISE, typename T>
-__device__ __forceinline__ void process_window(RingView& kv, RingView& qv, int hl, int S0, int s, int e,
-                                               T* __restrict__ out_head /*out + head column*/, int Ctot) {
+__device__ __forceinline__ void process_window(RingView& kv, RingView& qv, int hl, int nh, int S0, int s,
+                                               int e, T* __restrict__ out_head /*out + head column*/,
+                                               int Ctot) {
   using C = Cfg<D>;
-  State<D> st;
-  st.clear();
+  State<D> st[C::HPW];
+#pragma unroll
+  for (int j = 0; j < C::HPW; ++j) st[j].clear();
   for (int r = s; r < e; r += 32) {
     const int nv = min(32, e - r), rel = r - S0;
     ring_release_below<C::SR>(kv, rel);   // skipped rows first: a wait must never pin older stages
     ring_wait_upto(kv, (rel + nv - 1) / C::SR);
-    kv_tile<D, BF16, PRECISE>(kv, hl, rel, min(16, nv), st);
-    if (nv > 16) kv_tile<D, BF16, PRECISE>(kv, hl, rel + 16, nv - 16, st);
+#pragma unroll
+    for (int j = 0; j < C::HPW; ++j)
+      if (j < nh) {
+        if (nv == 32) {   // two full tiles, one basic block: the two dependency chains interleave
+          kv_tile<D, BF16, PRECISE, true>(kv, hl + j, rel, 16, st[j]);
+          kv_tile<D, BF16, PRECISE, true>(kv, hl + j, rel + 16, 16, st[j]);
+        } else {
+          kv_tile<D, BF16, PRECISE>(kv, hl + j, rel, min(16, nv), st[j]);
+          if (nv > 16) kv_tile<D, BF16, PRECISE>(kv, hl + j, rel + 16, nv - 16, st[j]);
+        }
+      }
   }
   const int m = e - s;
   const int lg = 32 - __clz(m - 1);                       // ceil(log2 m), 0 for m = 1
   const float scale = __int_as_float((127 - lg) << 23);   // 2^-lg: keeps fp16 operands O(1)
-  OutOperands<D> oo;
-  make_out_operands<D, PRECISE>(st, scale, oo);
+  OutOperands<D> oo[C::HPW];
+#pragma unroll
+  for (int j = 0; j < C::HPW; ++j) make_out_operands<D, PRECISE>(st[j], scale, oo[j]);
   for (int r = s; r < e; r += 32) {
     const int nv = min(32, e - r), rel = r - S0;
     ring_release_below<C::SR>(qv, rel);
     ring_wait_upto(qv, (rel + nv - 1) / C::SR);
-    q_tile<D, BF16, PRECISE, T>(qv, hl, rel, min(16, nv), oo, out_head + (size_t)r * Ctot, Ctot);
-    if (nv > 16)
-      q_tile<D, BF16, PRECISE, T>(qv, hl, rel + 16, nv - 16, oo, out_head + (size_t)(r + 16) * Ctot, Ctot);
+#pragma unroll
+    for (int j = 0; j < C::HPW; ++j)
+      if (j < nh) {
+        T* oh = out_head + j * D;
+        if (nv == 32) {
+          q_tile<D, BF16, PRECISE, T, true>(qv, hl + j, rel, 16, oo[j], oh + (size_t)r * Ctot, Ctot);
+          q_tile<D, BF16, PRECISE, T, true>(qv, hl + j, rel + 16, 16, oo[j], oh + (size_t)(r + 16) * Ctot, Ctot);
+        } else {
+          q_tile<D, BF16, PRECISE, T>(qv, hl + j, rel, min(16, nv), oo[j], oh + (size_t)r * Ctot, Ctot);
+          if (nv > 16)
+            q_tile<D, BF16, PRECISE, T>(qv, hl + j, rel + 16, nv - 16, oo[j], oh + (size_t)(r + 16) * Ctot, Ctot);
+        }
+      }
   }
 }
 
 // The piece [ps,pe) of a split window: partial state -> workspace atomics.
 template <int D, bool BF16>
-__device__ __forceinline__ void process_piece(RingView& kv, int hl, int S0, int ps, int pe,
-                                              float* __restrict__ slot) {
+__device__ __forceinline__ void process_piece(RingView& kv, int hl, int nh, int S0, int ps, int pe,
+                                              float* __restrict__ slot /*slot of head hl*/) {
   using C = Cfg<D>;
   const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
-  State<D> st;
-  st.clear();
+  State<D> st[C::HPW];
+#pragma unroll
+  for (int j = 0; j < C::HPW; ++j) st[j].clear();
   for (int r = ps; r < pe; r += 32) {
     const int nv = min(32, pe - r), rel = r - S0;
     ring_release_below<C::SR>(kv, rel);
     ring_wait_upto(kv, (rel + nv - 1) / C::SR);
-    kv_tile<D, BF16, false>(kv, hl, rel, min(16, nv), st);
-    if (nv > 16) kv_tile<D, BF16, false>(kv, hl, rel + 16, nv - 16, st);
-  }
 #pragma unroll
-  for (int mt = 0; mt < D / 16; ++mt)
-#pragma unroll
-    for (int nt = 0; nt < D / 8; ++nt)
-#pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        const int r = 16 * mt + g + 8 * (c >> 1), p = 8 * nt + 2 * t + (c & 1);
-        atomicAdd(slot + p * D + r, st.ST[mt][nt][c]);
+    for (int j = 0; j < C::HPW; ++j)
+      if (j < nh) {
+        kv_tile<D, BF16, false>(kv, hl + j, rel, min(16, nv), st[j]);
+        if (nv > 16) kv_tile<D, BF16, false>(kv, hl + j, rel + 16, nv - 16, st[j]);
       }
-  if (g == 0) {
-#pragma unroll
-    for (int nt = 0; nt < D / 8; ++nt)
-#pragma unroll
-      for (int c = 0; c < 2; ++c) atomicAdd(slot + D * D + 8 * nt + 2 * t + c, st.Z[nt][c]);
   }
+#pragma unroll
+  for (int j = 0; j < C::HPW; ++j)
+    if (j < nh) {
+      float* sl = slot + j * (D + 1) * D;
+#pragma unroll
+      for (int mt = 0; mt < D / 16; ++mt)
+#pragma unroll
+        for (int nt = 0; nt < D / 8; ++nt)
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            const int r = 16 * mt + g + 8 * (c >> 1), p = 8 * nt + 2 * t + (c & 1);
+            atomicAdd(sl + p * D + r, st[j].ST[mt][nt][c]);
+          }
+      if (g == 0) {
+#pragma unroll
+        for (int nt = 0; nt < D / 8; ++nt)
+#pragma unroll
+          for (int c = 0; c < 2; ++c) atomicAdd(sl + D * D + 8 * nt + 2 * t + c, st[j].Z[nt][c]);
+      }
+    }
 }
 
 template <int D, bool BF16, typename T>
-__global__ void __launch_bounds__(TC_THREADS, (D == 16 ? 3 : 2))
+__global__ void __launch_bounds__(Cfg<D>::THREADS, (D == 16 ? SLA_MINB : 2))
 sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                   const __grid_constant__ CUtensorMap tmV, const int32_t* __restrict__ off,
                   T* __restrict__ out, float* __restrict__ ws, int N, int W, int H, int span, int dbg) {
@@ -569,9 +631,12 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int R0 = blockIdx.x * span, R1 = min(R0 + span, N);
   const int h0 = blockIdx.y * NW;
-  const int nact = min(NW, H - h0);
+  const int nheads = min(NW, H - h0);                       // heads of this slab
+  const int nact = (nheads + C::HPW - 1) / C::HPW;           // active consumer warps
   const int Ctot = H * D;
 
+  TRACE(0);
+  TRACE_SM();
   if (threadIdx.x == 0) {
     for (int i = 0; i < NST; ++i) {
       mbar_init(smem_u32(&ctrl.full_kv[i]), 1);
@@ -583,7 +648,7 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   }
   __syncthreads();
 
-  if (warp >= NW) {
+  if (warp >= C::NCW) {
     // ---------------- producer warp: lane 0 streams K,V; lane 1 streams Q ----------------
     const bool is_kv = (lane == 0);
     const uint32_t full = smem_u32(is_kv ? ctrl.full_kv : ctrl.full_q);
@@ -611,7 +676,7 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     __syncthreads();                                           // setup published (stream bounds)
     if (lane < 2) {
       S0 = ctrl.stream_begin;
-      const int total = (ctrl.stream_end - S0 + C::SR - 1) / C::SR;
+      const int total = (dbg & 8) ? 0 : (ctrl.stream_end - S0 + C::SR - 1) / C::SR;
       for (int st = 0; st < total; ++st) {
         if (st >= NST) mbar_wait(empty + 8u * (st % NST), (uint32_t)(((st / NST) - 1) & 1));
         issue(st);
@@ -640,13 +705,15 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     }
   }
   __syncthreads();
+  TRACE(1);
   if (warp >= nact) return;
 
-  const int hl = warp;
+  const int hl = warp * C::HPW;                              // first head (within the slab) of this warp
+  const int nh = min(C::HPW, nheads - hl);
   const int S0 = ctrl.stream_begin;
   const int total = (ctrl.stream_end - S0 + C::SR - 1) / C::SR;
-  RingView kv{kv_base, smem_u32(ctrl.full_kv), smem_u32(ctrl.empty_kv), 0, 0};
-  RingView qv{q_base, smem_u32(ctrl.full_q), smem_u32(ctrl.empty_q), 0, 0};
+  RingView kv{kv_base, smem_u32(ctrl.full_kv), smem_u32(ctrl.empty_kv), 0, 0, (dbg >> 3) & 1};
+  RingView qv{q_base, smem_u32(ctrl.full_q), smem_u32(ctrl.empty_q), 0, 0, (dbg >> 3) & 1};
   T* out_head = out + (size_t)(h0 + hl) * D;
   if (dbg & 1) {   // debug: stream only, no compute
     ring_release_below<C::SR>(kv, total * C::SR);
@@ -696,24 +763,26 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       ring_release_below<C::SR>(qv, rel);
       ring_wait_upto(kv, (rel + rows - 1) / C::SR);
       ring_wait_upto(qv, (rel + rows - 1) / C::SR);
-      quad_tile<D, BF16, T>(kv, qv, hl, rel, rows, wid, out_head + (size_t)s * Ctot, Ctot);
+#pragma unroll
+      for (int j = 0; j < C::HPW; ++j)
+        if (j < nh) quad_tile<D, BF16, T>(kv, qv, hl + j, rel, rows, wid, out_head + j * D + (size_t)s * Ctot, Ctot);
       ring_release_below<C::SR>(kv, rel + rows);
       ring_release_below<C::SR>(qv, rel + rows);
       continue;
     }
     if (m <= kFuseMax) {
-      if (m <= HL_MAX) process_window<D, BF16, true, T>(kv, qv, hl, S0, s, e, out_head, Ctot);
-      else process_window<D, BF16, false, T>(kv, qv, hl, S0, s, e, out_head, Ctot);
+      process_window<D, BF16, false, T>(kv, qv, hl, nh, S0, s, e, out_head, Ctot);
     } else {
       float* slot = ws + kWsHeaderFloats + ((size_t)(s / (kFuseMax + 1)) * H + (h0 + hl)) * (size_t)((D + 1) * D);
       if (hl == 0 && lane == 0) reinterpret_cast<volatile int*>(ws)[0] = 1;   // tell the output kernel
-      process_piece<D, BF16>(kv, hl, S0, max(s, R0), min(e, R1), slot);
+      process_piece<D, BF16>(kv, hl, nh, S0, max(s, R0), min(e, R1), slot);
     }
     ++w;
   }
   // hand back every remaining stage the producers will issue (rows of split windows' Q, tail rows)
   ring_release_below<C::SR>(kv, total * C::SR);
   ring_release_below<C::SR>(qv, total * C::SR);
+  TRACE(2);
 }
 
 // ---- host side -------------------------------------------------------------------------------------
@@ -786,11 +855,17 @@ cudaError_t tc_launch(const Problem& p, cudaStream_t st) {
   if (span < 32) span = 32;
   nx = (p.N + span - 1) / span;
   dim3 grid(nx, slabs);
-  kern<<<grid, TC_THREADS, C::SMEM_DYN, st>>>(tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H, span, dbg_env);
+  kern<<<grid, C::THREADS, C::SMEM_DYN, st>>>(tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H, span, dbg_env);
   return cudaGetLastError();
 }
 
 }  // namespace
+
+#ifdef SLA_TRACE
+extern "C" int sla_debug_read_trace(unsigned long long* host, int n) {
+  return (int)cudaMemcpyFromSymbol(host, g_trace, sizeof(unsigned long long) * n);
+}
+#endif
 
 bool forward_tc_supported(const Problem& p, int dt) {
   if (dt != SLA_F16 && dt != SLA_BF16) return false;
