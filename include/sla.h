@@ -74,6 +74,18 @@ int sla_forward(const void* q, const void* k, const void* v, const int32_t* wind
                 int64_t N, int32_t W, int32_t H, int32_t d_h, int dt, void* out,
                 void* workspace, size_t workspace_bytes, sla_stream_t stream);
 
+/* SLA forward when the caller knows an upper bound on the window length.  In ScatterFormer a window
+ * is a fixed block of BEV cells (12x12 on Waymo), so no window can hold more than 144
+ * voxels: that bound is a model constant.  With 1 <= max_window_len <= 256 every window is processed
+ * whole by one thread block, so the call is ONE kernel launch and needs no workspace.
+ *   max_window_len  every window must satisfy off[w+1]-off[w] <= max_window_len (not checked on the
+ *                   device; a longer window is undefined behaviour).  > 256 -> SLA_ERR_UNSUPPORTED
+ *                   (call sla_forward instead).
+ * Results are identical to sla_forward on the same inputs. */
+int sla_forward_bounded(const void* q, const void* k, const void* v, const int32_t* window_offsets,
+                        int64_t N, int32_t W, int32_t H, int32_t d_h, int dt, void* out,
+                        int32_t max_window_len, sla_stream_t stream);
+
 /* SLA backward: gradients of L = sum(d_out * SLA(q,k,v)) (the paper is silent on backward; these are
  * the analytic derivatives of Eq. 3):
  *   dnum_i = g_i/den_i, dden_i = -(g_i.o_i)/den_i, da_i = dnum_i S^T + dden_i z, dq_i = da_i*phi'(q_i)

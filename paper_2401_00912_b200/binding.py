@@ -18,7 +18,7 @@ SLA_F32, SLA_F16, SLA_BF16 = 0, 1, 2
 # Every symbol include/sla.h declares (tests check the library exports exactly these).
 SYMBOLS = (
     "sla_status_string", "sla_version", "sla_workspace_bytes", "sla_offsets_from_window_ids",
-    "sla_forward", "sla_backward", "sla_forward_host",
+    "sla_forward", "sla_forward_bounded", "sla_backward", "sla_forward_host",
 )
 
 _lib = None
@@ -49,6 +49,8 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     L.sla_offsets_from_window_ids.restype = ci
     L.sla_forward.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp, sz, vp]
     L.sla_forward.restype = ci
+    L.sla_forward_bounded.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, i32, vp]
+    L.sla_forward_bounded.restype = ci
     L.sla_backward.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp, vp, vp, vp, sz, vp]
     L.sla_backward.restype = ci
     L.sla_forward_host.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp]
@@ -112,8 +114,10 @@ def sla_offsets_from_window_ids(win_id, W: int, out=None, stream=None):
     return out
 
 
-def sla_forward(q, k, v, window_offsets, out=None, workspace=None, stream=None):
-    """q,k,v: CUDA [N,H,d_h] (fp32/fp16/bf16); window_offsets: CUDA int32[W+1] -> out [N,H,d_h]."""
+def sla_forward(q, k, v, window_offsets, out=None, workspace=None, stream=None, max_window_len=0):
+    """q,k,v: CUDA [N,H,d_h] (fp32/fp16/bf16); window_offsets: CUDA int32[W+1] -> out [N,H,d_h].
+    max_window_len > 0 (a promise that no window is longer; <= 256) takes sla_forward_bounded: one
+    kernel launch, no workspace."""
     import torch
     L = load_library()
     _chk_dev(q, k, v, window_offsets)
@@ -126,6 +130,11 @@ def sla_forward(q, k, v, window_offsets, out=None, workspace=None, stream=None):
     dt = _dt(q)
     if out is None:
         out = torch.empty_like(q)
+    if max_window_len:
+        _check(L.sla_forward_bounded(q.data_ptr(), k.data_ptr(), v.data_ptr(), window_offsets.data_ptr(), N, W,
+                                     H, d, dt, out.data_ptr(), int(max_window_len), _stream(stream)),
+               "sla_forward_bounded")
+        return out
     workspace, wsb = _workspace(q, N, W, H, d, dt, False, workspace)
     _check(L.sla_forward(q.data_ptr(), k.data_ptr(), v.data_ptr(), window_offsets.data_ptr(), N, W, H, d,
                          dt, out.data_ptr(), workspace.data_ptr(), wsb, _stream(stream)), "sla_forward")

@@ -78,6 +78,27 @@ int sla_forward(const void* q, const void* k, const void* v, const int32_t* wind
   return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
 }
 
+int sla_forward_bounded(const void* q, const void* k, const void* v, const int32_t* window_offsets,
+                        int64_t N, int32_t W, int32_t H, int32_t d_h, int dt, void* out,
+                        int32_t max_window_len, sla_stream_t stream) {
+  int rc = check_common(N, W, H, d_h, dt);
+  if (rc != SLA_OK) return rc;
+  if (max_window_len < 1) return SLA_ERR_INVALID_ARG;
+  if (max_window_len > sla::kFuseMax) return SLA_ERR_UNSUPPORTED;   // use sla_forward
+  if (N == 0 || W == 0) return SLA_OK;
+  if (!q || !k || !v || !window_offsets || !out) return SLA_ERR_INVALID_ARG;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out)) return SLA_ERR_UNSUPPORTED;
+  sla::Problem p{};
+  p.q = q; p.k = k; p.v = v; p.out = out; p.off = window_offsets;
+  p.N = (int)N; p.W = W; p.H = H; p.d = d_h;
+  p.bounded = true;                                           // one launch: no workspace, no split pass
+  const char* force = getenv("SLA_FORCE_GENERIC");
+  const bool tc = !(force && force[0] == '1') && sla::forward_tc_supported(p, dt);
+  cudaError_t e = tc ? sla::launch_forward_tc(p, dt, (cudaStream_t)stream)
+                     : sla::launch_forward_generic(p, dt, (cudaStream_t)stream);
+  return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
+}
+
 int sla_backward(const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
                  int32_t W, int32_t H, int32_t d_h, int dt, const void* d_out, void* dq, void* dk,
                  void* dv, void* workspace, size_t workspace_bytes, sla_stream_t stream) {

@@ -629,7 +629,15 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   const uint32_t ring = (smem_u32(dyn_smem) + 1023u) & ~1023u;
   const uint32_t kv_base = ring, q_base = ring + NST * C::KV_STAGE;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int R0 = blockIdx.x * span, R1 = min(R0 + span, N);
+  // CTAs are dispatched in blockIdx order; map them to spans middle-out so that, when the grid runs in
+  // several waves, the spans most likely to be heavy (LiDAR scenes are densest near the sensor, i.e.
+  // in the middle of the row-major window order) start first and light ones fill the tail.
+  const int nspan = gridDim.x, mid = nspan >> 1;
+  const int bx = blockIdx.x;
+  int sidx = (bx & 1) ? mid - 1 - (bx >> 1) : mid + (bx >> 1);
+  if (sidx < 0) sidx = bx;            // (odd counts: the far end is reached by the even branch only)
+  if (sidx >= nspan) sidx = nspan - 1 - bx;
+  const int R0 = (dbg & 16) ? bx * span : sidx * span, R1 = min(R0 + span, N);
   const int h0 = blockIdx.y * NW;
   const int nheads = min(NW, H - h0);                       // heads of this slab
   const int nact = (nheads + C::HPW - 1) / C::HPW;           // active consumer warps
@@ -877,7 +885,7 @@ cudaError_t launch_forward_tc(const Problem& p, int dt, cudaStream_t st) {
   cudaError_t e;
   if (p.d == 16) e = (dt == SLA_F16) ? tc_launch<16, false, __half>(p, st) : tc_launch<16, true, __nv_bfloat16>(p, st);
   else e = (dt == SLA_F16) ? tc_launch<32, false, __half>(p, st) : tc_launch<32, true, __nv_bfloat16>(p, st);
-  if (e != cudaSuccess) return e;
+  if (e != cudaSuccess || p.bounded) return e;
   return launch_forward_generic_split_only(p, dt, st);        // outputs of split windows
 }
 

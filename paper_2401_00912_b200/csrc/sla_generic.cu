@@ -486,8 +486,9 @@ cudaError_t fwd_launch(const Problem& p, cudaStream_t st) {
   dim3 grid((p.N + kTileRows - 1) / kTileRows, (p.H + HB - 1) / HB);
   sla_fwd_generic_kernel<T, D><<<grid, CB, 0, st>>>((const T*)p.q, (const T*)p.k, (const T*)p.v, p.off,
                                                     (T*)p.out, p.ws_state, p.N, p.W, p.H);
-  sla_fwd_generic_split_kernel<T, D><<<grid, CB, 0, st>>>((const T*)p.q, p.off, (T*)p.out, p.ws_state,
-                                                          p.N, p.W, p.H);
+  if (!p.bounded)
+    sla_fwd_generic_split_kernel<T, D><<<grid, CB, 0, st>>>((const T*)p.q, p.off, (T*)p.out, p.ws_state,
+                                                            p.N, p.W, p.H);
   return cudaGetLastError();
 }
 

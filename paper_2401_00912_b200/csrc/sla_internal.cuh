@@ -64,6 +64,7 @@ struct Problem {
   float* ws_state;   // [W,H,d+1,d] fp32 (S rows 0..d-1, z in row d) for split windows
   float* ws_dstate;  // [W,H,d+1,d] fp32 (dS, dz) for split windows (backward)
   int N, W, H, d;
+  bool bounded;      // caller guarantees every window has <= kFuseMax rows: no workspace, no split pass
 };
 
 // Launchers (defined in the .cu files); all enqueue on `st` and return the last CUDA error.

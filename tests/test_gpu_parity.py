@@ -201,3 +201,57 @@ def test_host_entry_matches_device_entry():
     off = torch.from_numpy(sc.offsets).cuda()
     out_d = pkg.sla_forward(q.cuda(), k.cuda(), v.cuda(), off)
     assert torch.equal(out_h, out_d.cpu())
+
+
+@pytest.mark.parametrize("c", [1, 4])
+def test_forward_bounded_entry_matches_general_and_oracle(c):
+    """sla_forward_bounded (one launch, no workspace; windows <= 144 rows by construction of the
+    12x12-window configs) must give exactly what sla_forward gives, and match the oracle."""
+    torch = _torch()
+    sc = wl.make_config(c)
+    assert int(sc.lengths.max()) <= 144
+    q, k, v = sc.tensor("q"), sc.tensor("k"), sc.tensor("v")
+    off = torch.from_numpy(sc.offsets).cuda()
+    tq, tk, tv = (to_dev(a, sc.dtype) for a in (q, k, v))
+    out_b = pkg.sla_forward(tq, tk, tv, off, max_window_len=144)
+    out_g = pkg.sla_forward(tq, tk, tv, off)
+    torch.cuda.synchronize()
+    assert torch.equal(out_b, out_g)
+    ref = sla_oracle.forward(q, k, v, sc.offsets, nthreads=8)
+    check(f"{sc.name}.bounded", out_b, ref, sc.dtype, sc.lengths)
+
+
+def test_forward_bounded_generic_path_and_errors():
+    torch = _torch()
+    sc = wl.make_scene([5, 1, 144, 33, 2, 100, 16, 17], 4, 32, "f32", seed=12)
+    q, k, v = sc.tensor("q"), sc.tensor("k"), sc.tensor("v")
+    off = torch.from_numpy(sc.offsets).cuda()
+    out = pkg.sla_forward(*(to_dev(a, "f32") for a in (q, k, v)), off, max_window_len=144)
+    check("bounded_f32.out", out, sla_oracle.forward(q, k, v, sc.offsets), "f32", sc.lengths)
+    with pytest.raises(pkg.SlaError, match="UNSUPPORTED"):
+        pkg.sla_forward(*(to_dev(a, "f32") for a in (q, k, v)), off, max_window_len=1000)
+
+
+def test_forward_under_cuda_graph_replay():
+    """The C-ABI calls are capturable: a graph of prep + forward replays to the same result."""
+    torch = _torch()
+    sc = wl.make_config(1)
+    q, k, v = (to_dev(sc.tensor(n), sc.dtype) for n in ("q", "k", "v"))
+    ids = torch.from_numpy(sc.window_ids).cuda()
+    off = torch.empty(sc.W + 1, dtype=torch.int32, device="cuda")
+    out = torch.empty_like(q)
+    ws = torch.empty(pkg.workspace_bytes(sc.N, sc.W, sc.H, sc.d_h, pkg.SLA_F16), dtype=torch.uint8, device="cuda")
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        pkg.sla_offsets_from_window_ids(ids, sc.W, out=off, stream=s)
+        pkg.sla_forward(q, k, v, off, out=out, workspace=ws, stream=s)
+        torch.cuda.synchronize()
+        want = out.clone()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            pkg.sla_offsets_from_window_ids(ids, sc.W, out=off, stream=s)
+            pkg.sla_forward(q, k, v, off, out=out, workspace=ws, stream=s)
+        out.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+    assert torch.equal(out, want)
