@@ -323,7 +323,7 @@ def run_ours(args):
                 "api": "sla_forward_host (pinned host buffers)"},
         "gpu_launches": args.steps * (2 if bounded else 3),   # prep + forward kernel(s); memset not counted
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES, "peak_source": peak_src,
+                     "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES if (args.config == 1 and bounded) else None, "peak_source": peak_src,
                      "kernel": "sla_fwd_tc_kernel (the single launch of sla_forward_bounded)" if bounded
                                else "sla_forward (all launches of one call)",
                      "algorithmic_bytes": alg_bytes, "bytes_per_voxel": alg_bytes / N,
@@ -345,8 +345,10 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel from profiles/ (None until captured)
-NCU_TRAFFIC_BYTES = None
+# dram__bytes_read.sum + dram__bytes_write.sum of sla_fwd_tc_kernel per launch, config 1, from
+# profiles/r01_fwd_tc_ncu_full.md (46.13 MB read + 0.19 MB written; the 15.36 MB of output is still dirty in
+# L2 when the kernel ends).  Only valid for the default workload.
+NCU_TRAFFIC_BYTES = 46127360 + 193536
 
 
 def run_reference(args):
