@@ -629,14 +629,14 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   const uint32_t ring = (smem_u32(dyn_smem) + 1023u) & ~1023u;
   const uint32_t kv_base = ring, q_base = ring + NST * C::KV_STAGE;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  // CTAs are dispatched in blockIdx order; map them to spans middle-out so that, when the grid runs in
-  // several waves, the spans most likely to be heavy (LiDAR scenes are densest near the sensor, i.e.
-  // in the middle of the row-major window order) start first and light ones fill the tail.
-  const int nspan = gridDim.x, mid = nspan >> 1;
+  // CTAs are dispatched in blockIdx order and the grid runs in several waves (spans are short).
+  // Map CTAs to spans outside-in: both ends of the row-major window order first.  In a LiDAR scene
+  // those are the far-range rows: sparse, many 1-4 voxel windows, the slowest spans per row (measured
+  // 6 rows/us against 11-12 for dense spans), so they get the head start and the fast dense spans of
+  // the middle fill the tail.  (dbg 16: natural order, for A/B measurements.)
+  const int nspan = gridDim.x;
   const int bx = blockIdx.x;
-  int sidx = (bx & 1) ? mid - 1 - (bx >> 1) : mid + (bx >> 1);
-  if (sidx < 0) sidx = bx;            // (odd counts: the far end is reached by the even branch only)
-  if (sidx >= nspan) sidx = nspan - 1 - bx;
+  const int sidx = (bx & 1) ? nspan - 1 - (bx >> 1) : (bx >> 1);
   const int R0 = (dbg & 16) ? bx * span : sidx * span, R1 = min(R0 + span, N);
   const int h0 = blockIdx.y * NW;
   const int nheads = min(NW, H - h0);                       // heads of this slab
@@ -702,10 +702,12 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     if (lane == 0) {
       const int sa = __ldg(off + wa), ea = __ldg(off + wa + 1);
       const int sl = __ldg(off + wl), el = __ldg(off + wl + 1);
-      // the window holding R0 belongs to an earlier CTA if it is fused and starts before R0
-      const int sb = (ea - sa <= kFuseMax && sa < R0) ? ea : R0;
+      // Ownership of a fused window (<= kFuseMax rows): the CTA whose span holds its MIDDLE row
+      // (rows owned = span +- half a window at each end instead of a whole one: better balance).
+      const int ma = sa + ((ea - sa) >> 1), ml = sl + ((el - sl) >> 1);
+      const int sb = (ea - sa <= kFuseMax) ? (ma >= R0 ? sa : ea) : R0;
       int se;
-      if (el - sl <= kFuseMax) se = (sl >= R0) ? el : sb;   // last window fused: owned iff it starts here
+      if (el - sl <= kFuseMax) se = (ml < R1) ? el : sl;    // last window fused: owned iff its middle is here
       else se = R1;                                         // split: this CTA's piece ends at R1
       ctrl.wa = wa;
       ctrl.stream_begin = sb;
@@ -714,6 +716,9 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   }
   __syncthreads();
   TRACE(1);
+#ifdef SLA_TRACE
+  if (threadIdx.x == 0 && blockIdx.x < 8192) g_trace[blockIdx.x * 4 + 3] |= ((unsigned long long)(ctrl.stream_end - ctrl.stream_begin)) << 16;
+#endif
   if (warp >= nact) return;
 
   const int hl = warp * C::HPW;                              // first head (within the slab) of this warp
@@ -750,7 +755,8 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     bounds(w, s, e);
     if (s >= R1) break;
     const int m = e - s;
-    if (m <= 0 || (m <= kFuseMax && s < R0)) { ++w; continue; }   // empty, or owned by an earlier CTA
+    if (m <= kFuseMax && s + (m >> 1) >= R1) break;               // middle beyond the span: a later CTA's
+    if (m <= 0 || (m <= kFuseMax && s + (m >> 1) < R0)) { ++w; continue; }   // empty, or an earlier CTA's
     if (m <= QUAD_MAX) {
       // pack following whole short windows (each <= QUAD_MAX rows, owned) into one 16-row tile
       int rows = 0, ord = 0, wid = -1;
@@ -759,7 +765,7 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
         bounds(w, s2, e2);
         const int m2 = e2 - s2;
         if (m2 > 0) {
-          if (m2 > QUAD_MAX || rows + m2 > 16 || s2 >= R1) break;
+          if (m2 > QUAD_MAX || rows + m2 > 16 || s2 + (m2 >> 1) >= R1) break;
           if (lane >= rows && lane < rows + m2) wid = ord;
           rows += m2;
           ++ord;
@@ -858,6 +864,7 @@ cudaError_t tc_launch(const Problem& p, cudaStream_t st) {
   int span = (p.N + nx - 1) / nx;
   static const int dbg_env = []() { const char* e = getenv("SLA_TC_DBG"); return e ? atoi(e) : 0; }();
   static const int span_env = []() { const char* e = getenv("SLA_TC_SPAN"); return e ? atoi(e) : 0; }();
+  if (span > 64) span = 64;             // short spans, several waves: dynamic balance across SMs
   if (span_env > 0) span = span_env;
   span = (span + 15) / 16 * 16;
   if (span < 32) span = 32;
