@@ -758,20 +758,21 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     if (m <= kFuseMax && s + (m >> 1) >= R1) break;               // middle beyond the span: a later CTA's
     if (m <= 0 || (m <= kFuseMax && s + (m >> 1) < R0)) { ++w; continue; }   // empty, or an earlier CTA's
     if (m <= QUAD_MAX) {
-      // pack following whole short windows (each <= QUAD_MAX rows, owned) into one 16-row tile
-      int rows = 0, ord = 0, wid = -1;
-      while (w < W) {
-        int s2, e2;
-        bounds(w, s2, e2);
-        const int m2 = e2 - s2;
-        if (m2 > 0) {
-          if (m2 > QUAD_MAX || rows + m2 > 16 || s2 + (m2 >> 1) >= R1) break;
-          if (lane >= rows && lane < rows + m2) wid = ord;
-          rows += m2;
-          ++ord;
-        }
-        ++w;
-      }
+      // Pack the following whole short windows (owned, together <= 16 rows) into one 16-row tile.
+      // Done for all cached windows at once: lane j holds off[wbase+j]; one ballot finds how many
+      // consecutive windows fit, one OR-reduction builds the bit mask of window starts inside the
+      // tile, and the window ordinal of tile row r is a popcount of that mask.
+      const int i0 = w - wbase;                                   // lane of the first window (<= 30)
+      const int e_j = __shfl_down_sync(0xffffffffu, cur, 1);      // off[wbase+lane+1]
+      const int mid_j = cur + ((e_j - cur) >> 1);
+      const bool fits = lane >= i0 && lane < 31 && (e_j - s) <= 16 && mid_j < R1;
+      const unsigned okm = __ballot_sync(0xffffffffu, fits) >> i0;
+      const int cnt = __ffs(~okm) - 1;                            // consecutive windows that fit (>= 1)
+      const int rows = __shfl_sync(0xffffffffu, cur, i0 + cnt) - s;
+      const unsigned startbit = (lane > i0 && lane < i0 + cnt) ? (1u << (cur - s)) : 0u;
+      const unsigned starts = __reduce_or_sync(0xffffffffu, startbit) & 0xFFFEu;   // bit r: a window starts at row r
+      const int wid = (lane < rows) ? __popc(starts & ((2u << lane) - 1u)) : -1;
+      w += cnt;
       const int rel = s - S0;
       ring_release_below<C::SR>(kv, rel);
       ring_release_below<C::SR>(qv, rel);
