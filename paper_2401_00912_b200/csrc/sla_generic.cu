@@ -367,8 +367,8 @@ sla_bwd_generic_kernel(const T* __restrict__ q, const T* __restrict__ k, const T
   float* bsB = sm + RB * 256;
   const Ctx cx = make_ctx(H, D);
   const int h = cx.c / D;
-  const int row0 = blockIdx.x * kTileRows;
-  const int row1 = min(row0 + kTileRows, N);
+  const int row0 = blockIdx.x * kBwdTileRows;
+  const int row1 = min(row0 + kBwdTileRows, N);
   for (int w = window_of_row(off, W, row0); w < W; ++w) {
     const int s = __ldg(off + w), e = __ldg(off + w + 1);
     if (s >= row1) break;
@@ -414,8 +414,8 @@ sla_bwd_generic_split_q_kernel(const T* __restrict__ q, const T* __restrict__ g,
   if (reinterpret_cast<const volatile int*>(ws)[0] == 0) return;   // no split window in this call
   const Ctx cx = make_ctx(H, D);
   const int h = cx.c / D;
-  const int row0 = blockIdx.x * kTileRows;
-  const int row1 = min(row0 + kTileRows, N);
+  const int row0 = blockIdx.x * kBwdTileRows;
+  const int row1 = min(row0 + kBwdTileRows, N);
   for (int w = window_of_row(off, W, row0); w < W; ++w) {
     const int s = __ldg(off + w), e = __ldg(off + w + 1);
     if (s >= row1) break;
@@ -453,8 +453,8 @@ sla_bwd_generic_split_kv_kernel(const T* __restrict__ k, const T* __restrict__ v
   if (reinterpret_cast<const volatile int*>(ws)[0] == 0) return;   // no split window in this call
   const Ctx cx = make_ctx(H, D);
   const int h = cx.c / D;
-  const int row0 = blockIdx.x * kTileRows;
-  const int row1 = min(row0 + kTileRows, N);
+  const int row0 = blockIdx.x * kBwdTileRows;
+  const int row1 = min(row0 + kBwdTileRows, N);
   for (int w = window_of_row(off, W, row0); w < W; ++w) {
     const int s = __ldg(off + w), e = __ldg(off + w + 1);
     if (s >= row1) break;
@@ -506,7 +506,7 @@ template <typename T, int D>
 cudaError_t bwd_launch(const Problem& p, cudaStream_t st) {
   const int CB = block_threads(p.H, D);
   const int HB = CB / D;
-  dim3 grid((p.N + kTileRows - 1) / kTileRows, (p.H + HB - 1) / HB);
+  dim3 grid((p.N + kBwdTileRows - 1) / kBwdTileRows, (p.H + HB - 1) / HB);
   sla_bwd_generic_kernel<T, D><<<grid, CB, 0, st>>>((const T*)p.q, (const T*)p.k, (const T*)p.v,
                                                     (const T*)p.g, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv,
                                                     p.ws_state, p.N, p.W, p.H);

@@ -51,6 +51,10 @@ __device__ __forceinline__ int window_of_row(const int32_t* __restrict__ off, in
 //              first row (state never leaves the SM); longer windows are split by tile and their
 //              partial states are reduced in global memory (workspace) with fp32 atomics.
 constexpr int kTileRows = 64;
+#ifndef SLA_BWD_TILE
+#define SLA_BWD_TILE 64
+#endif
+constexpr int kBwdTileRows = SLA_BWD_TILE;   // backward: rows per thread block
 constexpr int kFuseMax = 256;
 constexpr int kRowBatch = 8;  // rows staged per inner step
 // The workspace starts with a 16-byte header (int flag: 1 = some window was split in this call),
