@@ -4,10 +4,10 @@
 // Design:
 //   * The flat window-sorted matrix is cut into equal row spans, one per CTA
 //     (load balance by rows/chunks, not by window -- PAPER.md:93 Fig. 3a).  A CTA owns every window
-//     of <= FUSE_MAX rows whose first row lies in its span (processed whole, state never leaves the
+//     of <= FUSE_MAX rows whose middle row lies in its span (processed whole, state never leaves the
 //     SM) and, for longer windows, the piece that intersects its span (partial state -> fp32
-//     atomics into the workspace; outputs by the second kernel).
-//   * Memory streaming is decoupled from the window structure: two producer warps stream the CTA's
+//     atomics into the workspace; outputs by a second launch of this kernel in OUTPASS mode).
+//   * Memory streaming is decoupled from the window structure: two producer lanes stream the CTA's
 //     rows of K,V and of Q through two shared-memory rings with 2-D TMA (128-byte swizzle) and
 //     mbarriers, regardless of where windows begin and end.
 //   * Consumer warp h owns head h of the slab (8 heads).  Per 16-row tile it forms
@@ -15,9 +15,10 @@
 //       z   += 1^T phi(K)   (normaliser)
 //     with ldmatrix.trans operands, then per 16-row Q tile  O = phi(Q) S / (phi(Q) z).
 //     The accumulator fragment of S^T is exactly the B fragment of S for the output mma.
-//   * Precision: phi() in fp32; operands are fp16.  Windows of <= HL_MAX rows use split operands
-//     (x = hi + lo, both fp16) so that the products carry ~22 bits; long windows use one term with
-//     the state scaled by 2^-ceil(log2 m) (the ratio of Eq. 3 is scale invariant).
+//   * Precision: operands are fp16, accumulation fp32.  Windows of <= 16 rows are packed into 16-row
+//     tiles and evaluated in the quadratic form with phi() in fp32 and split operands (x = hi + lo,
+//     both fp16: ~22-bit products); longer windows use phi() in fp16x2, one term, and the state scaled
+//     by 2^-ceil(log2 m) (the ratio of Eq. 3 is scale invariant).
 #include <cuda.h>
 
 #include <cstdlib>
@@ -618,7 +619,51 @@ __device__ __forceinline__ void process_piece(RingView& kv, int hl, int nh, int 
     }
 }
 
+// Output pass for the piece [ps,pe) of a split window of m rows: the complete state is read from the
+// workspace slot (fp32 [d+1, d]: rows 0..d-1 = S, row d = z) into the mma fragment layout.
 template <int D, bool BF16, typename T>
+__device__ __forceinline__ void output_piece(RingView& qv, int hl, int S0, int ps, int pe, int m,
+                                             const float* __restrict__ slot, T* __restrict__ out_head,
+                                             int Ctot) {
+  using C = Cfg<D>;
+  const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  State<D> st;
+#pragma unroll
+  for (int mt = 0; mt < D / 16; ++mt)
+#pragma unroll
+    for (int nt = 0; nt < D / 8; ++nt)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const int r = 16 * mt + g + 8 * (c >> 1), p = 8 * nt + 2 * t + (c & 1);
+        st.ST[mt][nt][c] = slot[p * D + r];
+      }
+#pragma unroll
+  for (int nt = 0; nt < D / 8; ++nt)
+#pragma unroll
+    for (int c = 0; c < 4; ++c) st.Z[nt][c] = slot[D * D + 8 * nt + 2 * t + (c & 1)];
+  const int lg = 32 - __clz(m - 1);
+  const float scale = __int_as_float((127 - lg) << 23);
+  OutOperands<D> oo;
+  make_out_operands<D, false>(st, scale, oo);
+  for (int r = ps; r < pe; r += 32) {
+    const int nv = min(32, pe - r), rel = r - S0;
+    ring_release_below<C::SR>(qv, rel);
+    ring_wait_upto(qv, (rel + nv - 1) / C::SR);
+    if (nv == 32) {
+      q_tile<D, BF16, false, T, true>(qv, hl, rel, 16, oo, out_head + (size_t)r * Ctot, Ctot);
+      q_tile<D, BF16, false, T, true>(qv, hl, rel + 16, 16, oo, out_head + (size_t)(r + 16) * Ctot, Ctot);
+    } else {
+      q_tile<D, BF16, false, T>(qv, hl, rel, min(16, nv), oo, out_head + (size_t)r * Ctot, Ctot);
+      if (nv > 16)
+        q_tile<D, BF16, false, T>(qv, hl, rel + 16, nv - 16, oo, out_head + (size_t)(r + 16) * Ctot, Ctot);
+    }
+  }
+}
+
+// OUTPASS = false: the main kernel.  OUTPASS = true: the second pass of the general entry -- outputs of
+// the pieces of windows longer than kFuseMax, whose complete states the main kernel left in the
+// workspace; it streams only Q and exits at once if the main kernel met no such window.
+template <int D, bool BF16, typename T, bool OUTPASS>
 __global__ void __launch_bounds__(Cfg<D>::THREADS, (D == 16 ? SLA_MINB : 2))
 sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                   const __grid_constant__ CUtensorMap tmV, const int32_t* __restrict__ off,
@@ -626,6 +671,7 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   using C = Cfg<D>;
   extern __shared__ uint8_t dyn_smem[];
   __shared__ Ctrl ctrl;
+  if (OUTPASS && reinterpret_cast<const volatile int*>(ws)[0] == 0) return;   // no split window in this call
   const uint32_t ring = (smem_u32(dyn_smem) + 1023u) & ~1023u;
   const uint32_t kv_base = ring, q_base = ring + NST * C::KV_STAGE;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -684,7 +730,7 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     __syncthreads();                                           // setup published (stream bounds)
     if (lane < 2) {
       S0 = ctrl.stream_begin;
-      const int total = (dbg & 8) ? 0 : (ctrl.stream_end - S0 + C::SR - 1) / C::SR;
+      const int total = ((dbg & 8) || (OUTPASS && is_kv)) ? 0 : (ctrl.stream_end - S0 + C::SR - 1) / C::SR;
       for (int st = 0; st < total; ++st) {
         if (st >= NST) mbar_wait(empty + 8u * (st % NST), (uint32_t)(((st / NST) - 1) & 1));
         issue(st);
@@ -705,10 +751,16 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       // Ownership of a fused window (<= kFuseMax rows): the CTA whose span holds its MIDDLE row
       // (rows owned = span +- half a window at each end instead of a whole one: better balance).
       const int ma = sa + ((ea - sa) >> 1), ml = sl + ((el - sl) >> 1);
-      const int sb = (ea - sa <= kFuseMax) ? (ma >= R0 ? sa : ea) : R0;
+      int sb = (ea - sa <= kFuseMax) ? (ma >= R0 ? sa : ea) : R0;
       int se;
       if (el - sl <= kFuseMax) se = (ml < R1) ? el : sl;    // last window fused: owned iff its middle is here
       else se = R1;                                         // split: this CTA's piece ends at R1
+      if (OUTPASS) {
+        // span <= kFuseMax, so a split window that meets [R0,R1) holds R0 (window wa) or R1-1 (wl)
+        const bool A = ea - sa > kFuseMax, B = el - sl > kFuseMax;
+        sb = A ? R0 : (B ? max(sl, R0) : R0);
+        se = B ? R1 : (A ? min(ea, R1) : sb);
+      }
       ctrl.wa = wa;
       ctrl.stream_begin = sb;
       ctrl.stream_end = (dbg & 2) ? sb : max(se, sb);   // dbg 2: setup only, nothing streamed
@@ -750,6 +802,24 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     e = __shfl_sync(0xffffffffu, cur, i + 1);
   };
   int w = wbase;
+  if (OUTPASS) {
+    while (w < W) {
+      int s, e;
+      bounds(w, s, e);
+      if (s >= R1) break;
+      if (e - s > kFuseMax) {
+#pragma unroll
+        for (int j = 0; j < C::HPW; ++j)
+          if (j < nh) {
+            const float* slot = ws + kWsHeaderFloats +
+                                ((size_t)(s / (kFuseMax + 1)) * H + (h0 + hl + j)) * (size_t)((D + 1) * D);
+            output_piece<D, BF16, T>(qv, hl + j, S0, max(s, R0), min(e, R1), e - s, slot, out_head + j * D, Ctot);
+          }
+      }
+      ++w;
+    }
+    ring_release_below<C::SR>(qv, total * C::SR);
+  } else {
   while (w < W) {
     int s, e;
     bounds(w, s, e);
@@ -797,6 +867,7 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   // hand back every remaining stage the producers will issue (rows of split windows' Q, tail rows)
   ring_release_below<C::SR>(kv, total * C::SR);
   ring_release_below<C::SR>(qv, total * C::SR);
+  }
   TRACE(2);
 }
 
@@ -848,10 +919,13 @@ cudaError_t tc_launch(const Problem& p, cudaStream_t st) {
   if (!make_map(&tq, p.q, p.N, Ctot, C::SR) || !make_map(&tk, p.k, p.N, Ctot, C::SR) ||
       !make_map(&tv, p.v, p.N, Ctot, C::SR))
     return cudaErrorInvalidValue;
-  auto kern = sla_fwd_tc_kernel<D, BF16, T>;
+  auto kern = sla_fwd_tc_kernel<D, BF16, T, false>;
+  auto kern_out = sla_fwd_tc_kernel<D, BF16, T, true>;
   static bool attr_set = false;
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_DYN);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(kern_out, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_DYN);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
@@ -872,6 +946,13 @@ cudaError_t tc_launch(const Problem& p, cudaStream_t st) {
   nx = (p.N + span - 1) / span;
   dim3 grid(nx, slabs);
   kern<<<grid, C::THREADS, C::SMEM_DYN, st>>>(tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H, span, dbg_env);
+  if (!p.bounded) {
+    // second pass: outputs of windows longer than kFuseMax (exits at once if there were none)
+    const int span2 = span > kFuseMax ? kFuseMax / 16 * 16 : span;
+    dim3 grid2((p.N + span2 - 1) / span2, slabs);
+    kern_out<<<grid2, C::THREADS, C::SMEM_DYN, st>>>(tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H, span2,
+                                                     dbg_env);
+  }
   return cudaGetLastError();
 }
 
@@ -893,8 +974,7 @@ cudaError_t launch_forward_tc(const Problem& p, int dt, cudaStream_t st) {
   cudaError_t e;
   if (p.d == 16) e = (dt == SLA_F16) ? tc_launch<16, false, __half>(p, st) : tc_launch<16, true, __nv_bfloat16>(p, st);
   else e = (dt == SLA_F16) ? tc_launch<32, false, __half>(p, st) : tc_launch<32, true, __nv_bfloat16>(p, st);
-  if (e != cudaSuccess || p.bounded) return e;
-  return launch_forward_generic_split_only(p, dt, st);        // outputs of split windows
+  return e;
 }
 
 }  // namespace sla
