@@ -57,139 +57,7 @@ template <int D> struct Cfg {
   static constexpr int THREADS = (NCW + 1) * 32;          // + one producer warp
 };
 
-// ---- PTX wrappers ---------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
-}
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  uint32_t done;
-  do {
-    asm volatile(
-        "{\n\t.reg .pred P1;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2, %3;\n\t"
-        "selp.b32 %0, 1, 0, P1;\n\t}"
-        : "=r"(done) : "r"(bar), "r"(parity), "r"(20000u) : "memory");
-  } while (!done);
-}
-__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int x, int y) {
-  asm volatile(
-      "cp.async.bulk.tensor.2d.shared::cta.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
-      ::"r"(dst), "l"(tm), "r"(bar), "r"(x), "r"(y) : "memory");
-}
-__device__ __forceinline__ void ldsm_x4(uint32_t addr, uint32_t (&r)[4]) {
-  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
-               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
-}
-__device__ __forceinline__ void ldsm_x4_t(uint32_t addr, uint32_t (&r)[4]) {
-  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
-               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
-}
-// D(16x8,f32) += A(16x16,f16,row) * B(16x8,f16,col)
-__device__ __forceinline__ void mma16816(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
-                                         uint32_t b0, uint32_t b1) {
-  asm(
-      "mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
-      : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
-      : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
-}
-
-// ---- element helpers ------------------------------------------------------------------------------
-template <bool BF16>
-__device__ __forceinline__ float2 unpack2(uint32_t r) {   // two packed I/O elements -> fp32
-  if (BF16) return make_float2(__uint_as_float(r << 16), __uint_as_float(r & 0xffff0000u));
-  return __half22float2(*reinterpret_cast<const __half2*>(&r));
-}
-__device__ __forceinline__ uint32_t pack_h2(float lo, float hi) {
-  __half2 h = __floats2half2_rn(lo, hi);
-  return *reinterpret_cast<uint32_t*>(&h);
-}
-template <bool BF16>
-__device__ __forceinline__ uint32_t pack_out(float lo, float hi) {
-  if (BF16) {
-    __nv_bfloat162 b = __floats2bfloat162_rn(lo, hi);
-    return *reinterpret_cast<uint32_t*>(&b);
-  }
-  return pack_h2(lo, hi);
-}
-// phi(x) = elu(x)+1 (reading A1); fast exp (ex2.approx) -- relative error ~2^-21, far below fp16 operands
-__device__ __forceinline__ float phi_fast(float x) { return x > 0.f ? x + 1.f : __expf(x); }
-
-// phi on two packed I/O elements, evaluated in fp16x2 (long windows only: the operand is rounded to
-// fp16 anyway; x+1 is the same single rounding, exp(x) = ex2(x*log2e) costs ~2 extra fp16 ulps on
-// negative inputs, whose phi < 1).  Result: fp16x2 {phi(x0), phi(x1)}.
-template <bool BF16>
-__device__ __forceinline__ uint32_t phi_h2(uint32_t raw) {
-  uint32_t x = raw;
-  if (BF16) { float2 f = unpack2<true>(raw); x = pack_h2(f.x, f.y); }
-  uint32_t e, p1, m;
-  const uint32_t log2e = 0x3DC53DC5u, one = 0x3C003C00u, zero = 0u;   // fp16 1.4424, 1.0
-  asm("{\n\t.reg .b32 t;\n\tmul.f16x2 t, %1, %2;\n\tex2.approx.f16x2 %0, t;\n\t}" : "=r"(e) : "r"(x), "r"(log2e));
-  asm("add.f16x2 %0, %1, %2;" : "=r"(p1) : "r"(x), "r"(one));
-  asm("set.gt.u32.f16x2 %0, %1, %2;" : "=r"(m) : "r"(x), "r"(zero));     // 0xFFFF per lane where x > 0
-  return (p1 & m) | (e & ~m);
-}
-__device__ __forceinline__ float fast_rcp(float x) {
-  float r;
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-  return r;
-}
-
-// fp32 pair -> fp16x2 "hi" and the fp16x2 residual "lo"
-__device__ __forceinline__ void split_h2(float x0, float x1, uint32_t& hi, uint32_t& lo) {
-  __half2 h = __floats2half2_rn(x0, x1);
-  float2 hf = __half22float2(h);
-  hi = *reinterpret_cast<uint32_t*>(&h);
-  lo = pack_h2(x0 - hf.x, x1 - hf.y);
-}
-
-// ---- per-warp consumer view of one ring -----------------------------------------------------------
-// Stage st of a stream holds rows [R0 + st*SR, R0 + (st+1)*SR).  `waited` = stages whose full barrier
-// this warp has observed; `released` = stages this warp has handed back to the producer.
-struct RingView {
-  uint32_t base;      // shared address of slot 0
-  uint32_t full;      // shared address of full barriers [NST]
-  uint32_t empty;     // shared address of empty barriers [NST]
-  int waited;
-  int released;
-  int nowait;         // debug: pretend every stage has landed (timing experiments only)
-};
-
-__device__ __forceinline__ void ring_wait_upto(RingView& rv, int stage_last) {
-  while (rv.waited <= stage_last) {
-    if (!rv.nowait) mbar_wait(rv.full + 8u * (rv.waited % NST), (uint32_t)((rv.waited / NST) & 1));
-    ++rv.waited;
-  }
-}
-// Release every stage that lies entirely below relative row `rel` (rows are relative to R0).
-template <int SR>
-__device__ __forceinline__ void ring_release_below(RingView& rv, int rel) {
-  while ((rv.released + 1) * SR <= rel) {
-    ring_wait_upto(rv, rv.released);   // never release a stage before it has landed (phase pacing)
-    __syncwarp();
-    if ((threadIdx.x & 31) == 0 && !rv.nowait) mbar_arrive(rv.empty + 8u * (rv.released % NST));
-    ++rv.released;
-  }
-}
-
-// Shared address of (relative row rel, 16-byte chunk `chunk` of this slab row) inside a ring whose
-// slots are `slot_bytes` apart; the tensor's stage starts `toff` bytes into the slot.
-template <int D>
-__device__ __forceinline__ uint32_t ring_addr(uint32_t base, int slot_bytes, int toff, int rel, int chunk) {
-  using C = Cfg<D>;
-  const int st = rel / C::SR, r = rel % C::SR;
-  const int box = chunk >> 3, cib = chunk & 7;
-  return base + (uint32_t)((st % NST) * slot_bytes + toff + box * C::BOX_BYTES + r * 128 +
-                           ((cib ^ (r & 7)) << 4));
-}
+#include "sla_tc_common.cuh"
 
 // ---- state of one (window, head) in mma fragments --------------------------------------------------
 //   ST[mt][nt][c]: S^T[r][p], r = 16*mt + g + 8*(c/2), p = 8*nt + 2*t + (c%2)   (g = lane/4, t = lane%4)
@@ -495,34 +363,6 @@ struct Ctrl {
   int stream_begin;  // S0: first row any owned item touches
   int stream_end;    // one past the last row any owned item touches (>= S0)
 };
-
-// For two rows at once (independent probes in flight together): the largest w in [0,W) with
-// off[w] <= row (row < off[W] = N), found by one warp with 32-way probes per round.
-__device__ __forceinline__ void warp_windows_of_rows(const int32_t* __restrict__ off, int W, int rowa,
-                                                     int rowb, int& wa, int& wb) {
-  const int lane = threadIdx.x & 31;
-  int lo[2] = {0, 0}, hi[2] = {W, W};
-  const int row[2] = {rowa, rowb};
-  while (hi[0] - lo[0] > 1 || hi[1] - lo[1] > 1) {
-    int step[2], idx[2], val[2];
-#pragma unroll
-    for (int k = 0; k < 2; ++k) {
-      step[k] = max(1, (hi[k] - lo[k] + 31) / 32);
-      idx[k] = lo[k] + (lane + 1) * step[k];
-      val[k] = __ldg(off + min(idx[k], W));
-    }
-#pragma unroll
-    for (int k = 0; k < 2; ++k) {
-      const bool ok = idx[k] < hi[k] && val[k] <= row[k];
-      const int cnt = __popc(__ballot_sync(0xffffffffu, ok));
-      const int nlo = lo[k] + cnt * step[k];
-      hi[k] = min(hi[k], nlo + step[k]);
-      lo[k] = nlo;
-    }
-  }
-  wa = lo[0];
-  wb = lo[1];
-}
 
 // One whole (fused) window [s,e) for head slot hl: state pass over K,V then output pass over Q.
 // Rows are addressed relative to S0, the first row of this CTA's streams.  Two 16-row tiles per
@@ -871,46 +711,7 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   TRACE(2);
 }
 
-// ---- host side -------------------------------------------------------------------------------------
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
-                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
-                                  CUtensorMapFloatOOBfill);
-
-EncodeTiledFn encode_fn() {
-  static EncodeTiledFn fn = []() -> EncodeTiledFn {
-    void* p = nullptr;
-    cudaDriverEntryPointQueryResult q;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
-        q != cudaDriverEntryPointSuccess)
-      return nullptr;
-    return reinterpret_cast<EncodeTiledFn>(p);
-  }();
-  return fn;
-}
-
-// 2-D map over a row-major [N, C] 16-bit tensor; box = 64 columns (128 B) x box_rows, 128-B swizzle.
-bool make_map(CUtensorMap* tm, const void* base, int N, int C, int box_rows) {
-  EncodeTiledFn enc = encode_fn();
-  if (!enc) return false;
-  const cuuint64_t dims[2] = {(cuuint64_t)C, (cuuint64_t)N};
-  const cuuint64_t strides[1] = {(cuuint64_t)C * 2};
-  const cuuint32_t box[2] = {64u, (cuuint32_t)box_rows};
-  const cuuint32_t estr[2] = {1u, 1u};
-  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, const_cast<void*>(base), dims, strides, box, estr,
-             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
-}
-
-int sm_count() {
-  static int n = []() {
-    int dev = 0, v = 148;
-    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
-    return v > 0 ? v : 148;
-  }();
-  return n;
-}
-
+// ---- host side (tensor-map encoder, SM count: sla_tc_common.cuh) -----------------------------------
 template <int D, bool BF16, typename T>
 cudaError_t tc_launch(const Problem& p, cudaStream_t st) {
   using C = Cfg<D>;
