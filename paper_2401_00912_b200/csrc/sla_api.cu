@@ -118,7 +118,9 @@ int sla_backward(const void* q, const void* k, const void* v, const int32_t* win
   p.ws_state = static_cast<float*>(workspace);
   p.ws_dstate = reinterpret_cast<float*>(static_cast<char*>(workspace) + one);
   p.N = (int)N; p.W = W; p.H = H; p.d = d_h;
-  cudaError_t e = sla::launch_backward_generic(p, dt, st);
+  const char* force = getenv("SLA_FORCE_GENERIC");
+  const bool tc = !(force && force[0] == '1') && sla::backward_tc_supported(p, dt);
+  cudaError_t e = tc ? sla::launch_backward_tc(p, dt, st) : sla::launch_backward_generic(p, dt, st);
   return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
 }
 

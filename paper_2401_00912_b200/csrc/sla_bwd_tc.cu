@@ -1,0 +1,507 @@
+// sla_bwd_tc.cu -- SLA backward for fp16 / bf16 I/O, d_h = 16, on sm_100a: same skeleton as the
+// forward (sla_fwd_tc.cu): equal row spans per CTA, TMA + mbarrier rings, one consumer warp per head,
+// mma.sync m16n8k16 with fp32 accumulation, window state in registers.
+//
+// Gradients of Eq. 3 (the paper is silent on backward), per window
+// and head, a = phi(q), b = phi(k), g = dO:
+//   pass A (K,V):    S = sum_j b_j^T v_j (kept as S and S^T fragments), z = sum_j b_j
+//   pass B (Q,dO):   num = a S, den = a.z, o = num/den, dnum = g/den, dden = -(g.o)/den
+//                    dq = (dnum S^T + dden z) * phi'(q)
+//                    dS += a^T dnum (kept as dS and dS^T fragments), dz += dden a
+//   pass C (K,V):    dv = b dS,  dk = (v dS^T + dz) * phi'(k)
+// Three streams (K,V / Q,dO / K,V again) run through three shared-memory rings.
+//
+// Scaling: with m rows and s = 2^-ceil(log2 m), the operands use S' = s S, z' = s z, so den' = s den
+// and dnum' = g/den' = dnum/s stay O(1) in fp16; dS' = dS/s and dz' = dz/s are scaled back by s when
+// they become operands of pass C.  Windows of <= 32 rows use split fp16 operands (hi + lo).
+// Windows longer than kFuseMax rows are left to the generic kernels (a flag in the workspace header
+// tells them whether there is anything to do).
+#include <cuda.h>
+
+#include <cstdlib>
+
+#include "sla_internal.cuh"
+
+namespace sla {
+namespace {
+
+constexpr int NW = 8;     // consumer warps = heads per slab
+constexpr int NST = 2;    // ring stages per stream
+constexpr int BWD_PRECISE_MAX = 32;
+
+template <int D> struct Cfg {
+  static constexpr int SR = 32;                           // rows per ring stage
+  static constexpr int NBOX = NW * D / 64;                // 128-byte column boxes per slab row
+  static constexpr int BOX_BYTES = SR * 128;
+  static constexpr int T_STAGE = NBOX * BOX_BYTES;        // one tensor's stage (8 KB at d_h = 16)
+  static constexpr int KV_STAGE = 2 * T_STAGE;            // every ring stage holds two tensors
+  static constexpr int RING_BYTES = 3 * NST * KV_STAGE;   // K,V | Q,dO | K,V again
+  static constexpr int SMEM_DYN = RING_BYTES + 1024;
+  static constexpr int THREADS = (NW + 1) * 32;
+};
+
+#include "sla_tc_common.cuh"
+
+constexpr int D = 16;
+using C = Cfg<D>;
+
+// fragments of one (window, head); c index: rows g (c<2) / g+8 (c>=2), columns 2t + (c&1)
+struct BwdState {
+  float ST[2][4];    // S^T : rows r, column tile nt over p
+  float SS[2][4];    // S   : rows p, column tile nt over r
+  float Z[2][4];     // z[p] in columns p (same in every row)
+  float dST[2][4];   // dS^T (scaled by 1/s)
+  float dSS[2][4];   // dS   (scaled by 1/s)
+  float DZ[2][4];    // dz   (scaled by 1/s)
+  __device__ __forceinline__ void clear() {
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        ST[a][c] = 0.f; SS[a][c] = 0.f; Z[a][c] = 0.f; dST[a][c] = 0.f; dSS[a][c] = 0.f; DZ[a][c] = 0.f;
+      }
+  }
+};
+
+// B-operand pairs built from a 2-tile accumulator X[nt][c]:  op[n][b] = pack(X[b][2n], X[b][2n+1]) * scale
+struct OpPair { uint32_t hi[2][2], lo[2][2]; };
+template <bool PRECISE>
+__device__ __forceinline__ void make_ops(const float (&X)[2][4], float scale, OpPair& o) {
+#pragma unroll
+  for (int n = 0; n < 2; ++n)
+#pragma unroll
+    for (int b = 0; b < 2; ++b) {
+      const float x0 = X[b][2 * n] * scale, x1 = X[b][2 * n + 1] * scale;
+      if (PRECISE) split_h2(x0, x1, o.hi[n][b], o.lo[n][b]);
+      else { o.hi[n][b] = pack_h2(x0, x1); o.lo[n][b] = 0u; }
+    }
+}
+
+// phi of a packed pair in fp32 (a) and its derivative factor (x>0 ? 1 : phi(x))
+template <bool BF16>
+__device__ __forceinline__ void phi_pair(uint32_t raw, float2& a, float2& da) {
+  const float2 x = unpack2<BF16>(raw);
+  a.x = phi_fast(x.x); a.y = phi_fast(x.y);
+  da.x = x.x > 0.f ? 1.f : a.x; da.y = x.y > 0.f ? 1.f : a.y;
+}
+template <bool PRECISE>
+__device__ __forceinline__ void to_op(float x0, float x1, uint32_t& hi, uint32_t& lo) {
+  if (PRECISE) split_h2(x0, x1, hi, lo);
+  else { hi = pack_h2(x0, x1); lo = 0u; }
+}
+// a (hi,lo) x b (hi,lo): 1 term, or the 3 leading terms
+template <bool PRECISE>
+__device__ __forceinline__ void mma3(float (&c)[4], const uint32_t (&ah)[4], const uint32_t (&al)[4],
+                                     uint32_t bh0, uint32_t bh1, uint32_t bl0, uint32_t bl1) {
+  mma16816(c, ah[0], ah[1], ah[2], ah[3], bh0, bh1);
+  if (PRECISE) {
+    mma16816(c, al[0], al[1], al[2], al[3], bh0, bh1);
+    mma16816(c, ah[0], ah[1], ah[2], ah[3], bl0, bl1);
+  }
+}
+
+// lane -> (tile row, 16-byte chunk select) for the x4 ldmatrix pattern
+//   registers: (rows0-7,c0), (rows0-7,c1), (rows8-15,c0), (rows8-15,c1)
+__device__ __forceinline__ void lane_pattern(int nvalid, int& trow, int& csel) {
+  const int lane = threadIdx.x & 31, mi = lane >> 3;
+  trow = (lane & 7) + 8 * (mi >> 1);
+  if (trow >= nvalid) trow = 0;          // clamp: row 0 of the tile is always valid and loaded
+  csel = mi & 1;
+}
+
+// ---- pass A: one 16-row K/V tile -> S^T, S, z -------------------------------------------------------
+template <bool BF16, bool PRECISE>
+__device__ __forceinline__ void bwd_kv_tile(const RingView& rv, int hl, int rel0, int nvalid, BwdState& s) {
+  const int t = threadIdx.x & 3;
+  int trow, csel;
+  lane_pattern(nvalid, trow, csel);
+  const int chunk = hl * 2 + csel;
+  uint32_t kr[4], vr[4];
+  ldsm_x4_t(ring_addr<D>(rv.base, C::KV_STAGE, 0, rel0 + trow, chunk), kr);
+  ldsm_x4_t(ring_addr<D>(rv.base, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), vr);
+  // transposed loads: kr[i] = K[j = 2t,2t+1 (+8 for i>=2)][p = g (+8 for odd i)], same for vr with r
+  uint32_t bh[4], bl[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int j0 = 2 * t + 8 * (i >> 1);
+    const float2 x = unpack2<BF16>(kr[i]);
+    const float b0 = (j0 < nvalid) ? phi_fast(x.x) : 0.f;
+    const float b1 = (j0 + 1 < nvalid) ? phi_fast(x.y) : 0.f;
+    to_op<PRECISE>(b0, b1, bh[i], bl[i]);
+  }
+  if (BF16) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { const float2 x = unpack2<true>(vr[i]); vr[i] = pack_h2(x.x, x.y); }
+  }
+  const uint32_t ones = 0x3C003C00u;
+#pragma unroll
+  for (int nt = 0; nt < 2; ++nt) {
+    // S^T (rows r, cols p): A = V^T = (vr0..3), B = phi(K) tile nt = (b[nt], b[2+nt])
+    mma16816(s.ST[nt], vr[0], vr[1], vr[2], vr[3], bh[nt], bh[2 + nt]);
+    mma16816(s.Z[nt], ones, ones, ones, ones, bh[nt], bh[2 + nt]);
+    // S (rows p, cols r): A = phi(K)^T = (b0..3), B = V tile nt = (vr[nt], vr[2+nt])
+    mma16816(s.SS[nt], bh[0], bh[1], bh[2], bh[3], vr[nt], vr[2 + nt]);
+    if (PRECISE) {
+      mma16816(s.ST[nt], vr[0], vr[1], vr[2], vr[3], bl[nt], bl[2 + nt]);
+      mma16816(s.Z[nt], ones, ones, ones, ones, bl[nt], bl[2 + nt]);
+      mma16816(s.SS[nt], bl[0], bl[1], bl[2], bl[3], vr[nt], vr[2 + nt]);
+    }
+  }
+}
+
+struct PassBOps {
+  OpPair num;            // from S^T: B operand of num = a S
+  OpPair da;             // from S  : B operand of da = dnum S^T
+  uint32_t zh[2], zl[2]; // z as B operand of den
+  float zs[2][2];        // scaled z in columns p = 8*np + 2t + c
+};
+
+// ---- pass B: one 16-row Q/dO tile -> dq rows, dS^T, dS, dz accumulators ------------------------------
+template <bool BF16, bool PRECISE, typename T>
+__device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0, int nvalid,
+                                           const PassBOps& op, BwdState& s, T* __restrict__ dq_rows,
+                                           int C_total) {
+  const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  int trow, csel;
+  lane_pattern(nvalid, trow, csel);
+  const int chunk = hl * 2 + csel;
+  const int perm[4] = {0, 2, 1, 3};   // ldmatrix register order -> A-fragment order (a0..a3)
+  uint32_t qn[4], gn[4];
+  ldsm_x4(ring_addr<D>(rv.base, C::KV_STAGE, 0, rel0 + trow, chunk), qn);
+  ldsm_x4(ring_addr<D>(rv.base, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), gn);
+  // A fragments: index 0: (row g, cols 2t..), 1: (row g+8, cols 2t..), 2: (row g, cols 8+2t..), 3: (row g+8, 8+2t..)
+  uint32_t ah[4], al[4];
+  float2 dph[4], gv[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    float2 a;
+    phi_pair<BF16>(qn[perm[i]], a, dph[i]);
+    to_op<PRECISE>(a.x, a.y, ah[i], al[i]);
+    gv[i] = unpack2<BF16>(gn[perm[i]]);
+  }
+  float num[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}}, den[4] = {0.f, 0.f, 0.f, 0.f};
+  mma3<PRECISE>(den, ah, al, op.zh[0], op.zh[1], op.zl[0], op.zl[1]);
+#pragma unroll
+  for (int n = 0; n < 2; ++n) mma3<PRECISE>(num[n], ah, al, op.num.hi[n][0], op.num.hi[n][1], op.num.lo[n][0], op.num.lo[n][1]);
+  const float inv0 = fast_rcp(den[0]), inv1 = fast_rcp(den[2]);       // rows g, g+8
+  // g.o per row: this lane holds columns 2t,2t+1 (tile 0) and 8+2t.. (tile 1) of rows g and g+8
+  float go0 = gv[0].x * num[0][0] + gv[0].y * num[0][1] + gv[2].x * num[1][0] + gv[2].y * num[1][1];
+  float go1 = gv[1].x * num[0][2] + gv[1].y * num[0][3] + gv[3].x * num[1][2] + gv[3].y * num[1][3];
+  go0 += __shfl_xor_sync(0xffffffffu, go0, 1); go0 += __shfl_xor_sync(0xffffffffu, go0, 2);
+  go1 += __shfl_xor_sync(0xffffffffu, go1, 1); go1 += __shfl_xor_sync(0xffffffffu, go1, 2);
+  const float dden0 = -(go0 * inv0) * inv0, dden1 = -(go1 * inv1) * inv1;   // o = num*inv
+  // dnum as A fragment (rows g / g+8 scaled by their 1/den)
+  uint32_t dh[4], dl[4];
+  to_op<PRECISE>(gv[0].x * inv0, gv[0].y * inv0, dh[0], dl[0]);
+  to_op<PRECISE>(gv[1].x * inv1, gv[1].y * inv1, dh[1], dl[1]);
+  to_op<PRECISE>(gv[2].x * inv0, gv[2].y * inv0, dh[2], dl[2]);
+  to_op<PRECISE>(gv[3].x * inv1, gv[3].y * inv1, dh[3], dl[3]);
+  // da = dnum S^T + dden z ; dq = da * phi'(q)
+#pragma unroll
+  for (int np = 0; np < 2; ++np) {
+    float da[4] = {0.f, 0.f, 0.f, 0.f};
+    mma3<PRECISE>(da, dh, dl, op.da.hi[np][0], op.da.hi[np][1], op.da.lo[np][0], op.da.lo[np][1]);
+    // C fragment (np): c0,c1 = (row g, p = 8np+2t,+1) <-> A index 2*np ; c2,c3 = row g+8 <-> A index 2*np+1
+    const float q0 = (da[0] + dden0 * op.zs[np][0]) * dph[2 * np].x;
+    const float q1 = (da[1] + dden0 * op.zs[np][1]) * dph[2 * np].y;
+    const float q2 = (da[2] + dden1 * op.zs[np][0]) * dph[2 * np + 1].x;
+    const float q3 = (da[3] + dden1 * op.zs[np][1]) * dph[2 * np + 1].y;
+    uint32_t* p0 = reinterpret_cast<uint32_t*>(dq_rows + (size_t)g * C_total + 8 * np + 2 * t);
+    uint32_t* p1 = reinterpret_cast<uint32_t*>(dq_rows + (size_t)(g + 8) * C_total + 8 * np + 2 * t);
+    if (g < nvalid) *p0 = pack_out<BF16>(q0, q1);
+    if (g + 8 < nvalid) *p1 = pack_out<BF16>(q2, q3);
+  }
+  // ---- transposed operands (contraction over the rows i of the tile) ----
+  uint32_t qt[4], gt[4];
+  ldsm_x4_t(ring_addr<D>(rv.base, C::KV_STAGE, 0, rel0 + trow, chunk), qt);
+  ldsm_x4_t(ring_addr<D>(rv.base, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), gt);
+  // qt[i] = Q[i' = 2t,2t+1 (+8 for i>=2)][p = g (+8 for odd i)] ; gt[i] likewise with r
+  // 1/den and dden of rows 2t, 2t+1, 2t+8, 2t+9 live in the lanes whose g equals that row
+  const int l0 = 4 * (2 * t), l1 = 4 * (2 * t + 1);
+  const float ir0 = __shfl_sync(0xffffffffu, inv0, l0), ir1 = __shfl_sync(0xffffffffu, inv0, l1);
+  const float ir2 = __shfl_sync(0xffffffffu, inv1, l0), ir3 = __shfl_sync(0xffffffffu, inv1, l1);
+  float dd0 = __shfl_sync(0xffffffffu, dden0, l0), dd1 = __shfl_sync(0xffffffffu, dden0, l1);
+  float dd2 = __shfl_sync(0xffffffffu, dden1, l0), dd3 = __shfl_sync(0xffffffffu, dden1, l1);
+  uint32_t uh[4], ul[4], th[4], tl[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int i0 = 2 * t + 8 * (i >> 1);
+    const float2 x = unpack2<BF16>(qt[i]);
+    const float a0 = (i0 < nvalid) ? phi_fast(x.x) : 0.f;       // rows beyond the window contribute nothing
+    const float a1 = (i0 + 1 < nvalid) ? phi_fast(x.y) : 0.f;
+    to_op<PRECISE>(a0, a1, uh[i], ul[i]);
+    const float2 gg = unpack2<BF16>(gt[i]);
+    const float s0 = (i >> 1) ? ir2 : ir0, s1 = (i >> 1) ? ir3 : ir1;
+    to_op<PRECISE>(gg.x * s0, gg.y * s1, th[i], tl[i]);
+  }
+  uint32_t ddh[2], ddl[2];
+  to_op<PRECISE>(dd0, dd1, ddh[0], ddl[0]);
+  to_op<PRECISE>(dd2, dd3, ddh[1], ddl[1]);
+  const uint32_t dda_h[4] = {ddh[0], ddh[0], ddh[1], ddh[1]}, dda_l[4] = {ddl[0], ddl[0], ddl[1], ddl[1]};
+#pragma unroll
+  for (int nt = 0; nt < 2; ++nt) {
+    // dS^T (rows r, cols p): A = dnum^T = (t0..3), B = a tile nt over p = (u[nt], u[2+nt])
+    mma3<PRECISE>(s.dST[nt], th, tl, uh[nt], uh[2 + nt], ul[nt], ul[2 + nt]);
+    // dS (rows p, cols r): A = a^T = (u0..3), B = dnum tile nt over r = (t[nt], t[2+nt])
+    mma3<PRECISE>(s.dSS[nt], uh, ul, th[nt], th[2 + nt], tl[nt], tl[2 + nt]);
+    // dz[p] = sum_i dden_i a_i[p]: A rows all equal to dden over i, B = a tile nt
+    mma3<PRECISE>(s.DZ[nt], dda_h, dda_l, uh[nt], uh[2 + nt], ul[nt], ul[2 + nt]);
+  }
+}
+
+struct PassCOps {
+  OpPair dv;             // from dS^T: B operand of dv = b dS
+  OpPair db;             // from dS  : B operand of db = v dS^T
+  float dzs[2][2];       // dz in columns p = 8*np + 2t + c
+};
+
+// ---- pass C: one 16-row K/V tile -> dk, dv rows ------------------------------------------------------
+template <bool BF16, bool PRECISE, typename T>
+__device__ __forceinline__ void bwd_kv_out_tile(const RingView& rv, int hl, int rel0, int nvalid,
+                                                const PassCOps& op, T* __restrict__ dk_rows,
+                                                T* __restrict__ dv_rows, int C_total) {
+  const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  int trow, csel;
+  lane_pattern(nvalid, trow, csel);
+  const int chunk = hl * 2 + csel;
+  const int perm[4] = {0, 2, 1, 3};
+  uint32_t kn[4], vn[4];
+  ldsm_x4(ring_addr<D>(rv.base, C::KV_STAGE, 0, rel0 + trow, chunk), kn);
+  ldsm_x4(ring_addr<D>(rv.base, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), vn);
+  uint32_t bh[4], bl[4], vh[4];
+  const uint32_t vzero[4] = {0u, 0u, 0u, 0u};
+  float2 dph[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    float2 b;
+    phi_pair<BF16>(kn[perm[i]], b, dph[i]);
+    to_op<PRECISE>(b.x, b.y, bh[i], bl[i]);
+    if (BF16) { const float2 x = unpack2<true>(vn[perm[i]]); vh[i] = pack_h2(x.x, x.y); }
+    else vh[i] = vn[perm[i]];
+  }
+#pragma unroll
+  for (int n = 0; n < 2; ++n) {
+    float dv[4] = {0.f, 0.f, 0.f, 0.f}, db[4] = {0.f, 0.f, 0.f, 0.f};
+    mma3<PRECISE>(dv, bh, bl, op.dv.hi[n][0], op.dv.hi[n][1], op.dv.lo[n][0], op.dv.lo[n][1]);
+    mma16816(db, vh[0], vh[1], vh[2], vh[3], op.db.hi[n][0], op.db.hi[n][1]);
+    if (PRECISE) mma16816(db, vh[0], vh[1], vh[2], vh[3], op.db.lo[n][0], op.db.lo[n][1]);   // v is exact
+    (void)vzero;
+    const float k0 = (db[0] + op.dzs[n][0]) * dph[2 * n].x, k1 = (db[1] + op.dzs[n][1]) * dph[2 * n].y;
+    const float k2 = (db[2] + op.dzs[n][0]) * dph[2 * n + 1].x, k3 = (db[3] + op.dzs[n][1]) * dph[2 * n + 1].y;
+    const size_t o0 = (size_t)g * C_total + 8 * n + 2 * t, o1 = (size_t)(g + 8) * C_total + 8 * n + 2 * t;
+    if (g < nvalid) {
+      *reinterpret_cast<uint32_t*>(dv_rows + o0) = pack_out<BF16>(dv[0], dv[1]);
+      *reinterpret_cast<uint32_t*>(dk_rows + o0) = pack_out<BF16>(k0, k1);
+    }
+    if (g + 8 < nvalid) {
+      *reinterpret_cast<uint32_t*>(dv_rows + o1) = pack_out<BF16>(dv[2], dv[3]);
+      *reinterpret_cast<uint32_t*>(dk_rows + o1) = pack_out<BF16>(k2, k3);
+    }
+  }
+}
+
+// ---- one whole window: the three passes -------------------------------------------------------------
+template <bool BF16, bool PRECISE, typename T>
+__device__ __forceinline__ void bwd_window(RingView& kv, RingView& qg, RingView& kv2, int hl, int S0, int s,
+                                           int e, T* __restrict__ dq_head, T* __restrict__ dk_head,
+                                           T* __restrict__ dv_head, int Ctot) {
+  BwdState st;
+  st.clear();
+  for (int r = s; r < e; r += 16) {
+    const int nv = min(16, e - r), rel = r - S0;
+    ring_release_below<C::SR>(kv, rel);
+    ring_wait_upto(kv, (rel + nv - 1) / C::SR);
+    bwd_kv_tile<BF16, PRECISE>(kv, hl, rel, nv, st);
+  }
+  const int m = e - s;
+  const int lg = 32 - __clz(m - 1);
+  const float scale = __int_as_float((127 - lg) << 23);   // s = 2^-ceil(log2 m)
+  PassBOps ob;
+  make_ops<PRECISE>(st.ST, scale, ob.num);
+  make_ops<PRECISE>(st.SS, scale, ob.da);
+#pragma unroll
+  for (int b = 0; b < 2; ++b) {
+    ob.zs[b][0] = st.Z[b][0] * scale; ob.zs[b][1] = st.Z[b][1] * scale;
+    to_op<PRECISE>(ob.zs[b][0], ob.zs[b][1], ob.zh[b], ob.zl[b]);
+  }
+  for (int r = s; r < e; r += 16) {
+    const int nv = min(16, e - r), rel = r - S0;
+    ring_release_below<C::SR>(qg, rel);
+    ring_wait_upto(qg, (rel + nv - 1) / C::SR);
+    bwd_q_tile<BF16, PRECISE, T>(qg, hl, rel, nv, ob, st, dq_head + (size_t)r * Ctot, Ctot);
+  }
+  PassCOps oc;
+  make_ops<PRECISE>(st.dST, scale, oc.dv);
+  make_ops<PRECISE>(st.dSS, scale, oc.db);
+#pragma unroll
+  for (int b = 0; b < 2; ++b) { oc.dzs[b][0] = st.DZ[b][0] * scale; oc.dzs[b][1] = st.DZ[b][1] * scale; }
+  for (int r = s; r < e; r += 16) {
+    const int nv = min(16, e - r), rel = r - S0;
+    ring_release_below<C::SR>(kv2, rel);
+    ring_wait_upto(kv2, (rel + nv - 1) / C::SR);
+    bwd_kv_out_tile<BF16, PRECISE, T>(kv2, hl, rel, nv, oc, dk_head + (size_t)r * Ctot,
+                                      dv_head + (size_t)r * Ctot, Ctot);
+  }
+}
+
+struct Ctrl {
+  unsigned long long full[3][NST], empty[3][NST];
+  int wa, stream_begin, stream_end;
+};
+
+template <bool BF16, typename T>
+__global__ void __launch_bounds__(Cfg<D>::THREADS, 2)
+sla_bwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
+                  const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmG,
+                  const int32_t* __restrict__ off, T* __restrict__ dq, T* __restrict__ dk,
+                  T* __restrict__ dv, float* __restrict__ ws, int N, int W, int H, int span) {
+  extern __shared__ uint8_t dyn_smem[];
+  __shared__ Ctrl ctrl;
+  const uint32_t ring = (smem_u32(dyn_smem) + 1023u) & ~1023u;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int nspan = gridDim.x, bx = blockIdx.x;
+  const int sidx = (bx & 1) ? nspan - 1 - (bx >> 1) : (bx >> 1);     // outside-in, as the forward
+  const int R0 = sidx * span, R1 = min(R0 + span, N);
+  const int h0 = blockIdx.y * NW;
+  const int nheads = min(NW, H - h0);
+  const int Ctot = H * D;
+
+  if (threadIdx.x == 0) {
+    for (int r = 0; r < 3; ++r)
+      for (int i = 0; i < NST; ++i) {
+        mbar_init(smem_u32(&ctrl.full[r][i]), 1);
+        mbar_init(smem_u32(&ctrl.empty[r][i]), nheads);
+      }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  if (warp >= NW) {
+    // producer warp: lane 0 streams K,V (pass A); lane 1 streams Q,dO (pass B); lane 2 streams K,V (pass C)
+    const int r = lane;
+    __syncthreads();
+    if (lane < 3) {
+      const uint32_t full = smem_u32(ctrl.full[r]), empty = smem_u32(ctrl.empty[r]);
+      const uint32_t base = ring + r * NST * C::KV_STAGE;
+      const CUtensorMap* ma = (r == 1) ? &tmQ : &tmK;
+      const CUtensorMap* mb = (r == 1) ? &tmG : &tmV;
+      const int S0 = ctrl.stream_begin;
+      const int total = (ctrl.stream_end - S0 + C::SR - 1) / C::SR;
+      for (int st = 0; st < total; ++st) {
+        if (st >= NST) mbar_wait(empty + 8u * (st % NST), (uint32_t)(((st / NST) - 1) & 1));
+        const uint32_t bar = full + 8u * (st % NST);
+        const uint32_t dst = base + (st % NST) * C::KV_STAGE;
+        const int y = S0 + st * C::SR;
+        mbar_expect_tx(bar, (uint32_t)C::KV_STAGE);
+#pragma unroll
+        for (int b = 0; b < C::NBOX; ++b) {
+          const int x = h0 * D + 64 * b;
+          tma_load_2d(dst + b * C::BOX_BYTES, ma, bar, x, y);
+          tma_load_2d(dst + C::T_STAGE + b * C::BOX_BYTES, mb, bar, x, y);
+        }
+      }
+      for (int st = max(0, total - NST); st < total; ++st)      // no TMA may be in flight at exit
+        mbar_wait(full + 8u * (st % NST), (uint32_t)((st / NST) & 1));
+    }
+    return;
+  }
+
+  if (warp == 0) {
+    int wa, wl;
+    warp_windows_of_rows(off, W, R0, R1 - 1, wa, wl);
+    if (lane == 0) {
+      const int sa = __ldg(off + wa), ea = __ldg(off + wa + 1);
+      const int sl = __ldg(off + wl), el = __ldg(off + wl + 1);
+      const int ma = sa + ((ea - sa) >> 1), ml = sl + ((el - sl) >> 1);
+      // fused windows: owned by the CTA whose span holds the middle row; longer ones are not ours
+      const int sb = (ea - sa <= kFuseMax) ? (ma >= R0 ? sa : ea) : min(ea, R1);
+      const int se = (el - sl <= kFuseMax) ? ((ml < R1) ? el : sl) : max(sl, R0);
+      ctrl.wa = wa;
+      ctrl.stream_begin = sb;
+      ctrl.stream_end = max(se, sb);
+    }
+  }
+  __syncthreads();
+  if (warp >= nheads) return;
+
+  const int hl = warp;
+  const int S0 = ctrl.stream_begin;
+  const int total = (ctrl.stream_end - S0 + C::SR - 1) / C::SR;
+  RingView kv{ring, smem_u32(ctrl.full[0]), smem_u32(ctrl.empty[0]), 0, 0, 0};
+  RingView qg{ring + NST * C::KV_STAGE, smem_u32(ctrl.full[1]), smem_u32(ctrl.empty[1]), 0, 0, 0};
+  RingView kv2{ring + 2 * NST * C::KV_STAGE, smem_u32(ctrl.full[2]), smem_u32(ctrl.empty[2]), 0, 0, 0};
+  const size_t hcol = (size_t)(h0 + hl) * D;
+
+  int wbase = ctrl.wa;
+  int cur = __ldg(off + min(wbase + lane, W));
+  int nxt = __ldg(off + min(wbase + 31 + lane, W));
+  for (int w = wbase; w < W; ++w) {
+    int i = w - wbase;
+    if (i >= 31) {
+      wbase += 31;
+      cur = nxt;
+      nxt = __ldg(off + min(wbase + 31 + lane, W));
+      i = w - wbase;
+    }
+    const int s = __shfl_sync(0xffffffffu, cur, i), e = __shfl_sync(0xffffffffu, cur, i + 1);
+    if (s >= R1) break;
+    const int m = e - s;
+    if (m <= 0) continue;
+    if (m > kFuseMax) {                                   // left to the generic kernels
+      if (hl == 0 && lane == 0) reinterpret_cast<volatile int*>(ws)[0] = 1;
+      continue;
+    }
+    const int mid = s + (m >> 1);
+    if (mid >= R1) break;
+    if (mid < R0) continue;
+    if (m <= BWD_PRECISE_MAX)
+      bwd_window<BF16, true, T>(kv, qg, kv2, hl, S0, s, e, dq + hcol, dk + hcol, dv + hcol, Ctot);
+    else
+      bwd_window<BF16, false, T>(kv, qg, kv2, hl, S0, s, e, dq + hcol, dk + hcol, dv + hcol, Ctot);
+  }
+  ring_release_below<C::SR>(kv, total * C::SR);
+  ring_release_below<C::SR>(qg, total * C::SR);
+  ring_release_below<C::SR>(kv2, total * C::SR);
+}
+
+template <bool BF16, typename T>
+cudaError_t bwd_tc_launch(const Problem& p, cudaStream_t st) {
+  CUtensorMap tq, tk, tv, tg;
+  const int Ctot = p.H * D;
+  if (!make_map(&tq, p.q, p.N, Ctot, C::SR) || !make_map(&tk, p.k, p.N, Ctot, C::SR) ||
+      !make_map(&tv, p.v, p.N, Ctot, C::SR) || !make_map(&tg, p.g, p.N, Ctot, C::SR))
+    return cudaErrorInvalidValue;
+  auto kern = sla_bwd_tc_kernel<BF16, T>;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_DYN);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  static const int span_env = []() { const char* e = getenv("SLA_TC_BWD_SPAN"); return e ? atoi(e) : 0; }();
+  int span = span_env > 0 ? span_env : 64;
+  span = (span + 15) / 16 * 16;
+  if (span > kFuseMax) span = kFuseMax / 16 * 16;
+  dim3 grid((p.N + span - 1) / span, (p.H + NW - 1) / NW);
+  kern<<<grid, C::THREADS, C::SMEM_DYN, st>>>(tq, tk, tv, tg, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state,
+                                              p.N, p.W, p.H, span);
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+bool backward_tc_supported(const Problem& p, int dt) {
+  if (dt != SLA_F16 && dt != SLA_BF16) return false;
+  if (p.d != 16 || (p.H * p.d) % 64 != 0) return false;
+  return encode_fn() != nullptr;
+}
+
+// Fused windows (<= kFuseMax rows) by the tensor-core kernel; longer windows by the generic kernels in
+// split-only mode (they exit at once unless the tensor-core kernel raised the workspace flag).
+cudaError_t launch_backward_tc(const Problem& p, int dt, cudaStream_t st) {
+  cudaError_t e = (dt == SLA_F16) ? bwd_tc_launch<false, __half>(p, st) : bwd_tc_launch<true, __nv_bfloat16>(p, st);
+  if (e != cudaSuccess) return e;
+  return launch_backward_generic_split_only(p, dt, st);
+}
+
+}  // namespace sla

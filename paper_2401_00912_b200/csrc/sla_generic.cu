@@ -361,10 +361,13 @@ __global__ void __launch_bounds__(256)
 sla_bwd_generic_kernel(const T* __restrict__ q, const T* __restrict__ k, const T* __restrict__ v,
                        const T* __restrict__ g, const int32_t* __restrict__ off, T* __restrict__ dq,
                        T* __restrict__ dk, T* __restrict__ dv, float* __restrict__ ws, int N, int W,
-                       int H) {
+                       int H, int split_only) {
   __shared__ __align__(16) float sm[BwdSmem<D>::kFloats];
   float* bsA = sm;
   float* bsB = sm + RB * 256;
+  // split_only: the tensor-core kernel did every window <= kFuseMax rows and raised the workspace flag
+  // if it met a longer one; here only those longer windows are accumulated
+  if (split_only && reinterpret_cast<const volatile int*>(ws)[0] == 0) return;
   const Ctx cx = make_ctx(H, D);
   const int h = cx.c / D;
   const int row0 = blockIdx.x * kBwdTileRows;
@@ -378,7 +381,7 @@ sla_bwd_generic_kernel(const T* __restrict__ q, const T* __restrict__ k, const T
 #pragma unroll
     for (int p = 0; p < D; ++p) Scol[p] = 0.f;
     if (m <= kFuseMax) {
-      if (s < row0) continue;
+      if (s < row0 || split_only) continue;
       accumulate_state<T, D>(k, v, s, e, cx, bsA, Scol, z);
       float Srow[D], dScol[D], dz = 0.f;
       transpose_state<D>(Scol, Srow, cx, sm);
@@ -503,13 +506,13 @@ cudaError_t fwd_split_launch(const Problem& p, cudaStream_t st) {
 }
 
 template <typename T, int D>
-cudaError_t bwd_launch(const Problem& p, cudaStream_t st) {
+cudaError_t bwd_launch(const Problem& p, cudaStream_t st, int split_only = 0) {
   const int CB = block_threads(p.H, D);
   const int HB = CB / D;
   dim3 grid((p.N + kBwdTileRows - 1) / kBwdTileRows, (p.H + HB - 1) / HB);
   sla_bwd_generic_kernel<T, D><<<grid, CB, 0, st>>>((const T*)p.q, (const T*)p.k, (const T*)p.v,
                                                     (const T*)p.g, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv,
-                                                    p.ws_state, p.N, p.W, p.H);
+                                                    p.ws_state, p.N, p.W, p.H, split_only);
   sla_bwd_generic_split_q_kernel<T, D><<<grid, CB, 0, st>>>((const T*)p.q, (const T*)p.g, p.off,
                                                             (T*)p.dq, p.ws_state, p.ws_dstate, p.N, p.W,
                                                             p.H);
@@ -541,6 +544,15 @@ cudaError_t launch_forward_generic_split_only(const Problem& p, int dt, cudaStre
   if (dt == SLA_F32) return fwd_split_launch<float, 32>(p, st);
   if (dt == SLA_F16) return fwd_split_launch<__half, 32>(p, st);
   return fwd_split_launch<__nv_bfloat16, 32>(p, st);
+}
+
+cudaError_t launch_backward_generic_split_only(const Problem& p, int dt, cudaStream_t st) {
+  if (p.d == 16) {
+    if (dt == SLA_F16) return bwd_launch<__half, 16>(p, st, 1);
+    return bwd_launch<__nv_bfloat16, 16>(p, st, 1);
+  }
+  if (dt == SLA_F16) return bwd_launch<__half, 32>(p, st, 1);
+  return bwd_launch<__nv_bfloat16, 32>(p, st, 1);
 }
 
 cudaError_t launch_backward_generic(const Problem& p, int dt, cudaStream_t st) {
