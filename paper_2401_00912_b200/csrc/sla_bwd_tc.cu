@@ -479,7 +479,7 @@ cudaError_t bwd_tc_launch(const Problem& p, cudaStream_t st) {
     attr_set = true;
   }
   static const int span_env = []() { const char* e = getenv("SLA_TC_BWD_SPAN"); return e ? atoi(e) : 0; }();
-  int span = span_env > 0 ? span_env : 64;
+  int span = span_env > 0 ? span_env : 32;   // short spans: the grid runs in many waves (dynamic balance)
   span = (span + 15) / 16 * 16;
   if (span > kFuseMax) span = kFuseMax / 16 * 16;
   dim3 grid((p.N + span - 1) / span, (p.H + NW - 1) / NW);
