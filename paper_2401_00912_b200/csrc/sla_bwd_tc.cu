@@ -117,8 +117,8 @@ __device__ __forceinline__ void bwd_kv_tile(const RingView& rv, int hl, int rel0
   lane_pattern(nvalid, trow, csel);
   const int chunk = hl * 2 + csel;
   uint32_t kr[4], vr[4];
-  ldsm_x4_t(ring_addr<D>(rv.base, C::KV_STAGE, 0, rel0 + trow, chunk), kr);
-  ldsm_x4_t(ring_addr<D>(rv.base, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), vr);
+  ldsm_x4_t(ring_addr<D>(rv, C::KV_STAGE, 0, rel0 + trow, chunk), kr);
+  ldsm_x4_t(ring_addr<D>(rv, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), vr);
   // transposed loads: kr[i] = K[j = 2t,2t+1 (+8 for i>=2)][p = g (+8 for odd i)], same for vr with r
   uint32_t bh[4], bl[4];
 #pragma unroll
@@ -167,8 +167,8 @@ __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0,
   const int chunk = hl * 2 + csel;
   const int perm[4] = {0, 2, 1, 3};   // ldmatrix register order -> A-fragment order (a0..a3)
   uint32_t qn[4], gn[4];
-  ldsm_x4(ring_addr<D>(rv.base, C::KV_STAGE, 0, rel0 + trow, chunk), qn);
-  ldsm_x4(ring_addr<D>(rv.base, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), gn);
+  ldsm_x4(ring_addr<D>(rv, C::KV_STAGE, 0, rel0 + trow, chunk), qn);
+  ldsm_x4(ring_addr<D>(rv, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), gn);
   // A fragments: index 0: (row g, cols 2t..), 1: (row g+8, cols 2t..), 2: (row g, cols 8+2t..), 3: (row g+8, 8+2t..)
   uint32_t ah[4], al[4];
   float2 dph[4], gv[4];
@@ -213,8 +213,8 @@ __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0,
   }
   // ---- transposed operands (contraction over the rows i of the tile) ----
   uint32_t qt[4], gt[4];
-  ldsm_x4_t(ring_addr<D>(rv.base, C::KV_STAGE, 0, rel0 + trow, chunk), qt);
-  ldsm_x4_t(ring_addr<D>(rv.base, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), gt);
+  ldsm_x4_t(ring_addr<D>(rv, C::KV_STAGE, 0, rel0 + trow, chunk), qt);
+  ldsm_x4_t(ring_addr<D>(rv, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), gt);
   // qt[i] = Q[i' = 2t,2t+1 (+8 for i>=2)][p = g (+8 for odd i)] ; gt[i] likewise with r
   // 1/den and dden of rows 2t, 2t+1, 2t+8, 2t+9 live in the lanes whose g equals that row
   const int l0 = 4 * (2 * t), l1 = 4 * (2 * t + 1);
@@ -266,8 +266,8 @@ __device__ __forceinline__ void bwd_kv_out_tile(const RingView& rv, int hl, int 
   const int chunk = hl * 2 + csel;
   const int perm[4] = {0, 2, 1, 3};
   uint32_t kn[4], vn[4];
-  ldsm_x4(ring_addr<D>(rv.base, C::KV_STAGE, 0, rel0 + trow, chunk), kn);
-  ldsm_x4(ring_addr<D>(rv.base, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), vn);
+  ldsm_x4(ring_addr<D>(rv, C::KV_STAGE, 0, rel0 + trow, chunk), kn);
+  ldsm_x4(ring_addr<D>(rv, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), vn);
   uint32_t bh[4], bl[4], vh[4];
   const uint32_t vzero[4] = {0u, 0u, 0u, 0u};
   float2 dph[4];
@@ -427,9 +427,9 @@ sla_bwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   const int hl = warp;
   const int S0 = ctrl.stream_begin;
   const int total = (ctrl.stream_end - S0 + C::SR - 1) / C::SR;
-  RingView kv{ring, smem_u32(ctrl.full[0]), smem_u32(ctrl.empty[0]), 0, 0, 0};
-  RingView qg{ring + NST * C::KV_STAGE, smem_u32(ctrl.full[1]), smem_u32(ctrl.empty[1]), 0, 0, 0};
-  RingView kv2{ring + 2 * NST * C::KV_STAGE, smem_u32(ctrl.full[2]), smem_u32(ctrl.empty[2]), 0, 0, 0};
+  RingView kv = make_ring(ring, smem_u32(ctrl.full[0]), smem_u32(ctrl.empty[0]), 0);
+  RingView qg = make_ring(ring + NST * C::KV_STAGE, smem_u32(ctrl.full[1]), smem_u32(ctrl.empty[1]), 0);
+  RingView kv2 = make_ring(ring + 2 * NST * C::KV_STAGE, smem_u32(ctrl.full[2]), smem_u32(ctrl.empty[2]), 0);
   const size_t hcol = (size_t)(h0 + hl) * D;
 
   int wbase = ctrl.wa;

@@ -95,8 +95,8 @@ __device__ __forceinline__ void kv_tile(const RingView& rv, int hl, int rel0, in
   for (int cp = 0; cp < D / 16; ++cp) {            // 16-channel column pairs of the head
     const int chunk = hl * (D / 8) + 2 * cp + csel;
     uint32_t kr[4], vr[4];
-    ldsm_x4_t(ring_addr<D>(rv.base, C::KV_STAGE, 0, rel0 + trow, chunk), kr);
-    ldsm_x4_t(ring_addr<D>(rv.base, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), vr);
+    ldsm_x4_t(ring_addr<D>(rv, C::KV_STAGE, 0, rel0 + trow, chunk), kr);
+    ldsm_x4_t(ring_addr<D>(rv, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), vr);
     // phi(K) fragments: kr[0],kr[1] hold voxels j = 2t,2t+1; kr[2],kr[3] hold j = 2t+8,2t+9
     uint32_t bhi[4], blo[4];
     if (PRECISE) {
@@ -149,7 +149,7 @@ __device__ __forceinline__ void kv_tile(const RingView& rv, int hl, int rel0, in
         if (mt == cp) { va[0] = vr[0]; va[1] = vr[1]; va[2] = vr[2]; va[3] = vr[3]; }
         else {
           const int vchunk = hl * (D / 8) + 2 * mt + csel;
-          ldsm_x4_t(ring_addr<D>(rv.base, C::KV_STAGE, C::T_STAGE, rel0 + trow, vchunk), va);
+          ldsm_x4_t(ring_addr<D>(rv, C::KV_STAGE, C::T_STAGE, rel0 + trow, vchunk), va);
           if (BF16) {
 #pragma unroll
             for (int i = 0; i < 4; ++i) { float2 x = unpack2<true>(va[i]); va[i] = pack_h2(x.x, x.y); }
@@ -213,7 +213,7 @@ __device__ __forceinline__ void q_tile(const RingView& rv, int hl, int rel0, int
 #pragma unroll
   for (int ks = 0; ks < D / 16; ++ks) {
     uint32_t qr[4];
-    ldsm_x4(ring_addr<D>(rv.base, C::T_STAGE, 0, rel0 + trow, hl * (D / 8) + 2 * ks + csel), qr);
+    ldsm_x4(ring_addr<D>(rv, C::T_STAGE, 0, rel0 + trow, hl * (D / 8) + 2 * ks + csel), qr);
     // registers (rows0-7,c0),(rows0-7,c1),(rows8-15,c0),(rows8-15,c1) -> a0=r0, a1=r2, a2=r1, a3=r3
     const int perm[4] = {0, 2, 1, 3};
 #pragma unroll
@@ -278,8 +278,8 @@ __device__ __forceinline__ void quad_tile(const RingView& kv, const RingView& qv
   for (int ks = 0; ks < D / 16; ++ks) {
     const int chunk = hl * (D / 8) + 2 * ks + csel;
     uint32_t qr[4], kr[4];
-    ldsm_x4(ring_addr<D>(qv.base, C::T_STAGE, 0, rel0 + trow, chunk), qr);
-    ldsm_x4(ring_addr<D>(kv.base, C::KV_STAGE, 0, rel0 + trow, chunk), kr);
+    ldsm_x4(ring_addr<D>(qv, C::T_STAGE, 0, rel0 + trow, chunk), qr);
+    ldsm_x4(ring_addr<D>(kv, C::KV_STAGE, 0, rel0 + trow, chunk), kr);
     uint32_t ahi[4], alo[4], bhi[4], blo[4];
     const int perm[4] = {0, 2, 1, 3};   // (rows0-7,c0),(rows0-7,c1),(rows8-15,c0),(rows8-15,c1) -> a0..a3
 #pragma unroll
@@ -322,7 +322,7 @@ __device__ __forceinline__ void quad_tile(const RingView& kv, const RingView& qv
 #pragma unroll
   for (int cp = 0; cp < D / 16; ++cp) {
     uint32_t vr[4];
-    ldsm_x4_t(ring_addr<D>(kv.base, C::KV_STAGE, C::T_STAGE, rel0 + trow, hl * (D / 8) + 2 * cp + csel), vr);
+    ldsm_x4_t(ring_addr<D>(kv, C::KV_STAGE, C::T_STAGE, rel0 + trow, hl * (D / 8) + 2 * cp + csel), vr);
     if (BF16) {
 #pragma unroll
       for (int i = 0; i < 4; ++i) { float2 x = unpack2<true>(vr[i]); vr[i] = pack_h2(x.x, x.y); }
@@ -617,8 +617,8 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   const int nh = min(C::HPW, nheads - hl);
   const int S0 = ctrl.stream_begin;
   const int total = (ctrl.stream_end - S0 + C::SR - 1) / C::SR;
-  RingView kv{kv_base, smem_u32(ctrl.full_kv), smem_u32(ctrl.empty_kv), 0, 0, (dbg >> 3) & 1};
-  RingView qv{q_base, smem_u32(ctrl.full_q), smem_u32(ctrl.empty_q), 0, 0, (dbg >> 3) & 1};
+  RingView kv = make_ring(kv_base, smem_u32(ctrl.full_kv), smem_u32(ctrl.empty_kv), (dbg >> 3) & 1);
+  RingView qv = make_ring(q_base, smem_u32(ctrl.full_q), smem_u32(ctrl.empty_q), (dbg >> 3) & 1);
   T* out_head = out + (size_t)(h0 + hl) * D;
   if (dbg & 1) {   // debug: stream only, no compute
     ring_release_below<C::SR>(kv, total * C::SR);

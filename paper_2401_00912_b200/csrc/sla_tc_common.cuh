@@ -74,18 +74,25 @@ __device__ __forceinline__ uint32_t pack_out(float lo, float hi) {
 __device__ __forceinline__ float phi_fast(float x) { return x > 0.f ? x + 1.f : __expf(x); }
 
 // phi on two packed I/O elements, evaluated in fp16x2 (long windows only: the operand is rounded to
-// fp16 anyway; x+1 is the same single rounding, exp(x) = ex2(x*log2e) costs ~2 extra fp16 ulps on
-// negative inputs, whose phi < 1).  Result: fp16x2 {phi(x0), phi(x1)}.
+// fp16 anyway).  Branch-free on the FMA pipe (the ALU pipe is the busy one in these kernels):
+//   r = relu(x*log2e)            (fma.relu)
+//   t = x*log2e - r = min(x*log2e, 0)   (one fused rounding)
+//   phi = 2^t + r*ln2            x <= 0: r = 0, phi = 2^(x*log2e) = e^x
+//                                x  > 0: t is only the rounding residual of r, 2^t = 1 + t*ln2 + ..., so
+//                                        phi = 1 + x to first order in that residual (~1.5 fp16 ulp)
+// Result: fp16x2 {phi(x0), phi(x1)}.
 template <bool BF16>
 __device__ __forceinline__ uint32_t phi_h2(uint32_t raw) {
   uint32_t x = raw;
   if (BF16) { float2 f = unpack2<true>(raw); x = pack_h2(f.x, f.y); }
-  uint32_t e, p1, m;
-  const uint32_t log2e = 0x3DC53DC5u, one = 0x3C003C00u, zero = 0u;   // fp16 1.4424, 1.0
-  asm("{\n\t.reg .b32 t;\n\tmul.f16x2 t, %1, %2;\n\tex2.approx.f16x2 %0, t;\n\t}" : "=r"(e) : "r"(x), "r"(log2e));
-  asm("add.f16x2 %0, %1, %2;" : "=r"(p1) : "r"(x), "r"(one));
-  asm("set.gt.u32.f16x2 %0, %1, %2;" : "=r"(m) : "r"(x), "r"(zero));     // 0xFFFF per lane where x > 0
-  return (p1 & m) | (e & ~m);
+  uint32_t r, t, e, out;
+  const uint32_t log2e = 0x3DC53DC5u, ln2 = 0x398C398Cu, zero = 0u;   // fp16 1.4424, 0.6931
+  asm("fma.rn.relu.f16x2 %0, %1, %2, %3;" : "=r"(r) : "r"(x), "r"(log2e), "r"(zero));
+  asm("{\n\t.reg .b32 nr;\n\tneg.f16x2 nr, %3;\n\tfma.rn.f16x2 %0, %1, %2, nr;\n\t}"
+      : "=r"(t) : "r"(x), "r"(log2e), "r"(r));
+  asm("ex2.approx.f16x2 %0, %1;" : "=r"(e) : "r"(t));
+  asm("fma.rn.f16x2 %0, %1, %2, %3;" : "=r"(out) : "r"(r), "r"(ln2), "r"(e));
+  return out;
 }
 __device__ __forceinline__ float fast_rcp(float x) {
   float r;
@@ -103,7 +110,10 @@ __device__ __forceinline__ void split_h2(float x0, float x1, uint32_t& hi, uint3
 
 // ---- per-warp consumer view of one ring -----------------------------------------------------------
 // Stage st of a stream holds rows [R0 + st*SR, R0 + (st+1)*SR).  `waited` = stages whose full barrier
-// this warp has observed; `released` = stages this warp has handed back to the producer.
+// this warp has observed; `released` = stages this warp has handed back to the producer.  The ring slot
+// and barrier phase of the next stage to wait for / to release are tracked incrementally (no division
+// by the stage count in the hot loops): stage st lives in slot (st + bias) mod NST for every stage that
+// has not been released yet, with bias = r_slot - released.
 struct RingView {
   uint32_t base;      // shared address of slot 0
   uint32_t full;      // shared address of full barriers [NST]
@@ -111,12 +121,18 @@ struct RingView {
   int waited;
   int released;
   int nowait;         // debug: pretend every stage has landed (timing experiments only)
+  int w_slot, w_phase;   // slot and parity of stage `waited`
+  int r_slot, bias;      // slot of stage `released`; bias = r_slot - released
 };
+__device__ __forceinline__ RingView make_ring(uint32_t base, uint32_t full, uint32_t empty, int nowait = 0) {
+  return RingView{base, full, empty, 0, 0, nowait, 0, 0, 0, 0};
+}
 
 __device__ __forceinline__ void ring_wait_upto(RingView& rv, int stage_last) {
   while (rv.waited <= stage_last) {
-    if (!rv.nowait) mbar_wait(rv.full + 8u * (rv.waited % NST), (uint32_t)((rv.waited / NST) & 1));
+    if (!rv.nowait) mbar_wait(rv.full + 8u * rv.w_slot, (uint32_t)rv.w_phase);
     ++rv.waited;
+    if (++rv.w_slot == NST) { rv.w_slot = 0; rv.w_phase ^= 1; }
   }
 }
 // Release every stage that lies entirely below relative row `rel` (rows are relative to R0).
@@ -125,20 +141,24 @@ __device__ __forceinline__ void ring_release_below(RingView& rv, int rel) {
   while ((rv.released + 1) * SR <= rel) {
     ring_wait_upto(rv, rv.released);   // never release a stage before it has landed (phase pacing)
     __syncwarp();
-    if ((threadIdx.x & 31) == 0 && !rv.nowait) mbar_arrive(rv.empty + 8u * (rv.released % NST));
+    if ((threadIdx.x & 31) == 0 && !rv.nowait) mbar_arrive(rv.empty + 8u * rv.r_slot);
     ++rv.released;
+    if (++rv.r_slot == NST) { rv.r_slot = 0; rv.bias -= NST; }
   }
 }
 
 // Shared address of (relative row rel, 16-byte chunk `chunk` of this slab row) inside a ring whose
-// slots are `slot_bytes` apart; the tensor's stage starts `toff` bytes into the slot.
+// slots are `slot_bytes` apart; the tensor's stage starts `toff` bytes into the slot.  The row must
+// belong to a stage that has been waited for and not yet released.
 template <int D>
-__device__ __forceinline__ uint32_t ring_addr(uint32_t base, int slot_bytes, int toff, int rel, int chunk) {
+__device__ __forceinline__ uint32_t ring_addr(const RingView& rv, int slot_bytes, int toff, int rel, int chunk) {
   using C = Cfg<D>;
-  const int st = rel / C::SR, r = rel % C::SR;
+  const int st = (int)((unsigned)rel / (unsigned)C::SR), r = (int)((unsigned)rel % (unsigned)C::SR);   // rel >= 0
+  int slot = st + rv.bias;
+  if (slot >= NST) slot -= NST;
   const int box = chunk >> 3, cib = chunk & 7;
-  return base + (uint32_t)((st % NST) * slot_bytes + toff + box * C::BOX_BYTES + r * 128 +
-                           ((cib ^ (r & 7)) << 4));
+  return rv.base + (uint32_t)(slot * slot_bytes + toff + box * C::BOX_BYTES + r * 128 +
+                              ((cib ^ (r & 7)) << 4));
 }
 
 // For two rows at once (independent probes in flight together): the largest w in [0,W) with
