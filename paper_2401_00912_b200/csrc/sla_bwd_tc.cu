@@ -81,8 +81,8 @@ __device__ __forceinline__ void make_ops(const float (&X)[2][4], float scale, Op
 template <bool BF16>
 __device__ __forceinline__ void phi_pair(uint32_t raw, float2& a, float2& da) {
   const float2 x = unpack2<BF16>(raw);
-  a.x = phi_fast(x.x); a.y = phi_fast(x.y);
-  da.x = x.x > 0.f ? 1.f : a.x; da.y = x.y > 0.f ? 1.f : a.y;
+  da.x = dphi_fast(x.x); da.y = dphi_fast(x.y);
+  a.x = fmaxf(x.x, 0.f) + da.x; a.y = fmaxf(x.y, 0.f) + da.y;
 }
 template <bool PRECISE>
 __device__ __forceinline__ void to_op(float x0, float x1, uint32_t& hi, uint32_t& lo) {
