@@ -80,23 +80,40 @@ template <int D> struct State {
 };
 
 // One 16-row K/V tile starting at relative row `rel0` with `nvalid` rows of the current window.
+//
+// Shared addresses: the head's 16-byte chunks are hl*(D/8) + 2*cp + csel, all inside one 128-byte box
+// row, and chunk bit 1 = cp, so under the 128-byte swizzle (chunk ^ (row & 7)) the address of column
+// pair cp is the address of pair 0 with bit 5 flipped.  `a0` is that pair-0 address of this lane's
+// ldmatrix row in the K stage (V: + T_STAGE); full 32-row steps pass it in and advance it by one ring
+// slot per step instead of recomputing stage, slot and swizzle (process_window).
+template <int D>
+__device__ __forceinline__ uint32_t lane_tile_addr(const RingView& rv, int slot_bytes, int hl, int rel0, int nvalid) {
+  const int lane = threadIdx.x & 31;
+  const int mi = lane >> 3;
+  int trow = (lane & 7) + 8 * (mi >> 1);           // tile row this lane addresses for ldmatrix
+  if (trow >= nvalid) trow = 0;                    // clamp: row 0 of the tile is always valid
+  return ring_addr<D>(rv, slot_bytes, 0, rel0 + trow, hl * (D / 8) + (mi & 1));
+}
+// advance a lane address by one ring slot (the next stage), wrapping at the end of the ring
+__device__ __forceinline__ uint32_t ring_next_slot(uint32_t a, uint32_t ring_end, int slot_bytes) {
+  a += (uint32_t)slot_bytes;
+  return a >= ring_end ? a - (uint32_t)(NST * slot_bytes) : a;
+}
+
 template <int D, bool BF16, bool PRECISE, bool FULL = false>
-__device__ __forceinline__ void kv_tile(const RingView& rv, int hl, int rel0, int nvalid_in, State<D>& s) {
+__device__ __forceinline__ void kv_tile(const RingView& rv, int hl, int rel0, int nvalid_in, State<D>& s,
+                                        uint32_t a0_in = 0u) {
   const int nvalid = FULL ? 16 : nvalid_in;
   using C = Cfg<D>;
   const int lane = threadIdx.x & 31;
   const int t = lane & 3;
-  const int mi = lane >> 3;
-  int trow = (lane & 7) + 8 * (mi >> 1);           // tile row this lane addresses for ldmatrix
-  if (trow >= nvalid) trow = 0;                    // clamp: row 0 of the tile is always valid
-  const int csel = mi & 1;
+  const uint32_t a0 = FULL ? a0_in : lane_tile_addr<D>(rv, C::KV_STAGE, hl, rel0, nvalid);
   const uint32_t ones = 0x3C003C00u;               // fp16 {1,1}
 #pragma unroll
   for (int cp = 0; cp < D / 16; ++cp) {            // 16-channel column pairs of the head
-    const int chunk = hl * (D / 8) + 2 * cp + csel;
     uint32_t kr[4], vr[4];
-    ldsm_x4_t(ring_addr<D>(rv, C::KV_STAGE, 0, rel0 + trow, chunk), kr);
-    ldsm_x4_t(ring_addr<D>(rv, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), vr);
+    ldsm_x4_t(a0 ^ (uint32_t)(cp << 5), kr);
+    ldsm_x4_t((a0 ^ (uint32_t)(cp << 5)) + C::T_STAGE, vr);
     // phi(K) fragments: kr[0],kr[1] hold voxels j = 2t,2t+1; kr[2],kr[3] hold j = 2t+8,2t+9
     uint32_t bhi[4], blo[4];
     if (PRECISE) {
@@ -148,8 +165,7 @@ __device__ __forceinline__ void kv_tile(const RingView& rv, int hl, int rel0, in
         uint32_t va[4];
         if (mt == cp) { va[0] = vr[0]; va[1] = vr[1]; va[2] = vr[2]; va[3] = vr[3]; }
         else {
-          const int vchunk = hl * (D / 8) + 2 * mt + csel;
-          ldsm_x4_t(ring_addr<D>(rv, C::KV_STAGE, C::T_STAGE, rel0 + trow, vchunk), va);
+          ldsm_x4_t((a0 ^ (uint32_t)(mt << 5)) + C::T_STAGE, va);
           if (BF16) {
 #pragma unroll
             for (int i = 0; i < 4; ++i) { float2 x = unpack2<true>(va[i]); va[i] = pack_h2(x.x, x.y); }
@@ -196,24 +212,22 @@ __device__ __forceinline__ void make_out_operands(const State<D>& s, float scale
     }
 }
 
-// One 16-row Q tile: out rows [row0, row0+nvalid) of head h.
+// One 16-row Q tile: out rows [row0, row0+nvalid) of head h.  `lane_out` = this lane's first output
+// element (row0 + g, head column + 2t); `o8` = 8 rows in elements.
 template <int D, bool BF16, bool PRECISE, typename T, bool FULL = false>
 __device__ __forceinline__ void q_tile(const RingView& rv, int hl, int rel0, int nvalid_in,
-                                       const OutOperands<D>& o, T* __restrict__ out_rows /*row0, head col*/,
-                                       int C_total) {
+                                       const OutOperands<D>& o, T* __restrict__ lane_out, size_t o8,
+                                       uint32_t a0_in = 0u) {
   const int nvalid = FULL ? 16 : nvalid_in;
   using C = Cfg<D>;
   const int lane = threadIdx.x & 31;
-  const int g = lane >> 2, t = lane & 3;
-  const int mi = lane >> 3;
-  int trow = (lane & 7) + 8 * (mi >> 1);
-  if (trow >= nvalid) trow = 0;
-  const int csel = mi & 1;
+  const int g = lane >> 2;
+  const uint32_t a0 = FULL ? a0_in : lane_tile_addr<D>(rv, C::T_STAGE, hl, rel0, nvalid);
   uint32_t ahi[D / 16][4], alo[D / 16][4];
 #pragma unroll
   for (int ks = 0; ks < D / 16; ++ks) {
     uint32_t qr[4];
-    ldsm_x4(ring_addr<D>(rv, C::T_STAGE, 0, rel0 + trow, hl * (D / 8) + 2 * ks + csel), qr);
+    ldsm_x4(a0 ^ (uint32_t)(ks << 5), qr);
     // registers (rows0-7,c0),(rows0-7,c1),(rows8-15,c0),(rows8-15,c1) -> a0=r0, a1=r2, a2=r1, a3=r3
     const int perm[4] = {0, 2, 1, 3};
 #pragma unroll
@@ -248,10 +262,10 @@ __device__ __forceinline__ void q_tile(const RingView& rv, int hl, int rel0, int
         mma16816(acc, ahi[ks][0], ahi[ks][1], ahi[ks][2], ahi[ks][3], o.lo[n2][ks][0], o.lo[n2][ks][1]);
       }
     }
-    uint32_t* p0 = reinterpret_cast<uint32_t*>(out_rows + (size_t)g * C_total + 8 * n2 + 2 * t);
-    uint32_t* p1 = reinterpret_cast<uint32_t*>(out_rows + (size_t)(g + 8) * C_total + 8 * n2 + 2 * t);
-    if (g < nvalid) *p0 = pack_out<BF16>(acc[0] * inv0, acc[1] * inv0);
-    if (g + 8 < nvalid) *p1 = pack_out<BF16>(acc[2] * inv1, acc[3] * inv1);
+    uint32_t* p0 = reinterpret_cast<uint32_t*>(lane_out + 8 * n2);
+    uint32_t* p1 = reinterpret_cast<uint32_t*>(lane_out + o8 + 8 * n2);
+    if (FULL || g < nvalid) *p0 = pack_out<BF16>(acc[0] * inv0, acc[1] * inv0);
+    if (FULL || g + 8 < nvalid) *p1 = pack_out<BF16>(acc[2] * inv1, acc[3] * inv1);
   }
 }
 
@@ -375,6 +389,17 @@ __device__ __forceinline__ void process_window(RingView& kv, RingView& qv, int h
   State<D> st[C::HPW];
 #pragma unroll
   for (int j = 0; j < C::HPW; ++j) st[j].clear();
+  const int lane = threadIdx.x & 31;
+  // Lane addresses of the two 16-row tiles of a full 32-row step: computed once per pass, then moved
+  // to the next ring slot each step (a step is exactly one stage of rows).
+  uint32_t ak[C::HPW][2];
+  ring_release_below<C::SR>(kv, s - S0);   // ring_addr needs the stage within NST of `released`
+#pragma unroll
+  for (int j = 0; j < C::HPW; ++j) {
+    ak[j][0] = lane_tile_addr<D>(kv, C::KV_STAGE, hl + j, s - S0, 16);
+    ak[j][1] = lane_tile_addr<D>(kv, C::KV_STAGE, hl + j, s - S0 + 16, 16);
+  }
+  const uint32_t kv_end = kv.base + NST * C::KV_STAGE;
   for (int r = s; r < e; r += 32) {
     const int nv = min(32, e - r), rel = r - S0;
     ring_release_below<C::SR>(kv, rel);   // skipped rows first: a wait must never pin older stages
@@ -383,8 +408,10 @@ __device__ __forceinline__ void process_window(RingView& kv, RingView& qv, int h
     for (int j = 0; j < C::HPW; ++j)
       if (j < nh) {
         if (nv == 32) {   // two full tiles, one basic block: the two dependency chains interleave
-          kv_tile<D, BF16, PRECISE, true>(kv, hl + j, rel, 16, st[j]);
-          kv_tile<D, BF16, PRECISE, true>(kv, hl + j, rel + 16, 16, st[j]);
+          kv_tile<D, BF16, PRECISE, true>(kv, hl + j, rel, 16, st[j], ak[j][0]);
+          kv_tile<D, BF16, PRECISE, true>(kv, hl + j, rel + 16, 16, st[j], ak[j][1]);
+          ak[j][0] = ring_next_slot(ak[j][0], kv_end, C::KV_STAGE);
+          ak[j][1] = ring_next_slot(ak[j][1], kv_end, C::KV_STAGE);
         } else {
           kv_tile<D, BF16, PRECISE>(kv, hl + j, rel, min(16, nv), st[j]);
           if (nv > 16) kv_tile<D, BF16, PRECISE>(kv, hl + j, rel + 16, nv - 16, st[j]);
@@ -397,21 +424,33 @@ __device__ __forceinline__ void process_window(RingView& kv, RingView& qv, int h
   OutOperands<D> oo[C::HPW];
 #pragma unroll
   for (int j = 0; j < C::HPW; ++j) make_out_operands<D, PRECISE>(st[j], scale, oo[j]);
-  for (int r = s; r < e; r += 32) {
+  uint32_t aq[C::HPW][2];
+  ring_release_below<C::SR>(qv, s - S0);
+#pragma unroll
+  for (int j = 0; j < C::HPW; ++j) {
+    aq[j][0] = lane_tile_addr<D>(qv, C::T_STAGE, hl + j, s - S0, 16);
+    aq[j][1] = lane_tile_addr<D>(qv, C::T_STAGE, hl + j, s - S0 + 16, 16);
+  }
+  const uint32_t q_end = qv.base + NST * C::T_STAGE;
+  const size_t o8 = (size_t)8 * Ctot;
+  // this lane's first output element: row s + g, head column + 2t; 32 rows further every step
+  T* lp = out_head + (size_t)(s + (lane >> 2)) * Ctot + 2 * (lane & 3);
+  for (int r = s; r < e; r += 32, lp += 4 * o8) {
     const int nv = min(32, e - r), rel = r - S0;
     ring_release_below<C::SR>(qv, rel);
     ring_wait_upto(qv, (rel + nv - 1) / C::SR);
 #pragma unroll
     for (int j = 0; j < C::HPW; ++j)
       if (j < nh) {
-        T* oh = out_head + j * D;
+        T* oh = lp + j * D;
         if (nv == 32) {
-          q_tile<D, BF16, PRECISE, T, true>(qv, hl + j, rel, 16, oo[j], oh + (size_t)r * Ctot, Ctot);
-          q_tile<D, BF16, PRECISE, T, true>(qv, hl + j, rel + 16, 16, oo[j], oh + (size_t)(r + 16) * Ctot, Ctot);
+          q_tile<D, BF16, PRECISE, T, true>(qv, hl + j, rel, 16, oo[j], oh, o8, aq[j][0]);
+          q_tile<D, BF16, PRECISE, T, true>(qv, hl + j, rel + 16, 16, oo[j], oh + 2 * o8, o8, aq[j][1]);
+          aq[j][0] = ring_next_slot(aq[j][0], q_end, C::T_STAGE);
+          aq[j][1] = ring_next_slot(aq[j][1], q_end, C::T_STAGE);
         } else {
-          q_tile<D, BF16, PRECISE, T>(qv, hl + j, rel, min(16, nv), oo[j], oh + (size_t)r * Ctot, Ctot);
-          if (nv > 16)
-            q_tile<D, BF16, PRECISE, T>(qv, hl + j, rel + 16, nv - 16, oo[j], oh + (size_t)(r + 16) * Ctot, Ctot);
+          q_tile<D, BF16, PRECISE, T>(qv, hl + j, rel, min(16, nv), oo[j], oh, o8);
+          if (nv > 16) q_tile<D, BF16, PRECISE, T>(qv, hl + j, rel + 16, nv - 16, oo[j], oh + 2 * o8, o8);
         }
       }
   }
@@ -485,17 +524,25 @@ __device__ __forceinline__ void output_piece(RingView& qv, int hl, int S0, int p
   const float scale = __int_as_float((127 - lg) << 23);
   OutOperands<D> oo;
   make_out_operands<D, false>(st, scale, oo);
-  for (int r = ps; r < pe; r += 32) {
+  uint32_t aq[2];
+  ring_release_below<C::SR>(qv, ps - S0);
+  aq[0] = lane_tile_addr<D>(qv, C::T_STAGE, hl, ps - S0, 16);
+  aq[1] = lane_tile_addr<D>(qv, C::T_STAGE, hl, ps - S0 + 16, 16);
+  const uint32_t q_end = qv.base + NST * C::T_STAGE;
+  const size_t o8 = (size_t)8 * Ctot;
+  T* lp = out_head + (size_t)(ps + g) * Ctot + 2 * t;
+  for (int r = ps; r < pe; r += 32, lp += 4 * o8) {
     const int nv = min(32, pe - r), rel = r - S0;
     ring_release_below<C::SR>(qv, rel);
     ring_wait_upto(qv, (rel + nv - 1) / C::SR);
     if (nv == 32) {
-      q_tile<D, BF16, false, T, true>(qv, hl, rel, 16, oo, out_head + (size_t)r * Ctot, Ctot);
-      q_tile<D, BF16, false, T, true>(qv, hl, rel + 16, 16, oo, out_head + (size_t)(r + 16) * Ctot, Ctot);
+      q_tile<D, BF16, false, T, true>(qv, hl, rel, 16, oo, lp, o8, aq[0]);
+      q_tile<D, BF16, false, T, true>(qv, hl, rel + 16, 16, oo, lp + 2 * o8, o8, aq[1]);
+      aq[0] = ring_next_slot(aq[0], q_end, C::T_STAGE);
+      aq[1] = ring_next_slot(aq[1], q_end, C::T_STAGE);
     } else {
-      q_tile<D, BF16, false, T>(qv, hl, rel, min(16, nv), oo, out_head + (size_t)r * Ctot, Ctot);
-      if (nv > 16)
-        q_tile<D, BF16, false, T>(qv, hl, rel + 16, nv - 16, oo, out_head + (size_t)(r + 16) * Ctot, Ctot);
+      q_tile<D, BF16, false, T>(qv, hl, rel, min(16, nv), oo, lp, o8);
+      if (nv > 16) q_tile<D, BF16, false, T>(qv, hl, rel + 16, nv - 16, oo, lp + 2 * o8, o8);
     }
   }
 }
