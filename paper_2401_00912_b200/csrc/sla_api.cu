@@ -124,6 +124,35 @@ int sla_backward(const void* q, const void* k, const void* v, const int32_t* win
   return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
 }
 
+}  // extern "C"
+
+namespace {
+// Memory pool of the host-buffer entry, one per device, created on first use and kept for the life of
+// the process.  Its release threshold is unbounded, so the staging block of one call is reused by the
+// next instead of going back to the driver at every stream synchronisation (the default pool's
+// threshold is 0: a real allocation and free of ~80 MB per call, several ms).
+cudaMemPool_t host_entry_pool() {
+  static cudaMemPool_t pools[64] = {};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+  if (!pools[dev]) {
+    cudaMemPoolProps props = {};
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = dev;
+    cudaMemPool_t pool = nullptr;
+    if (cudaMemPoolCreate(&pool, &props) != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
+    unsigned long long thr = ~0ull;
+    cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+    pools[dev] = pool;
+  }
+  return pools[dev];
+}
+}  // namespace
+
+extern "C" {
+
 int sla_forward_host(const void* q, const void* k, const void* v, const int32_t* win_id, int64_t N,
                      int32_t W, int32_t H, int32_t d_h, int dt, void* out, sla_stream_t stream) {
   int rc = check_common(N, W, H, d_h, dt);
@@ -137,9 +166,11 @@ int sla_forward_host(const void* q, const void* k, const void* v, const int32_t*
   const size_t off_al = ((size_t)(W + 1) * 4 + 255) / 256 * 256;
   const size_t ws = state_bytes(N, H, d_h);
   char* base = nullptr;
-  if (cudaMallocAsync(reinterpret_cast<void**>(&base), 4 * tb_al + ids_al + off_al + ws, st) !=
-      cudaSuccess)
-    return SLA_ERR_CUDA;
+  cudaMemPool_t pool = host_entry_pool();
+  const size_t total = 4 * tb_al + ids_al + off_al + ws;
+  const cudaError_t ae = pool ? cudaMallocFromPoolAsync(reinterpret_cast<void**>(&base), total, pool, st)
+                              : cudaMallocAsync(reinterpret_cast<void**>(&base), total, st);
+  if (ae != cudaSuccess) return SLA_ERR_CUDA;
   char* dq_ = base; char* dk_ = base + tb_al; char* dv_ = base + 2 * tb_al; char* do_ = base + 3 * tb_al;
   int32_t* dids = reinterpret_cast<int32_t*>(base + 4 * tb_al);
   int32_t* doff = reinterpret_cast<int32_t*>(base + 4 * tb_al + ids_al);

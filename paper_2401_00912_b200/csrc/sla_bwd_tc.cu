@@ -427,9 +427,9 @@ sla_bwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   const int hl = warp;
   const int S0 = ctrl.stream_begin;
   const int total = (ctrl.stream_end - S0 + C::SR - 1) / C::SR;
-  RingView kv = make_ring(ring, smem_u32(ctrl.full[0]), smem_u32(ctrl.empty[0]), 0);
-  RingView qg = make_ring(ring + NST * C::KV_STAGE, smem_u32(ctrl.full[1]), smem_u32(ctrl.empty[1]), 0);
-  RingView kv2 = make_ring(ring + 2 * NST * C::KV_STAGE, smem_u32(ctrl.full[2]), smem_u32(ctrl.empty[2]), 0);
+  RingView kv = make_ring(ring, smem_u32(ctrl.full[0]), smem_u32(ctrl.empty[0]));
+  RingView qg = make_ring(ring + NST * C::KV_STAGE, smem_u32(ctrl.full[1]), smem_u32(ctrl.empty[1]));
+  RingView kv2 = make_ring(ring + 2 * NST * C::KV_STAGE, smem_u32(ctrl.full[2]), smem_u32(ctrl.empty[2]));
   const size_t hcol = (size_t)(h0 + hl) * D;
 
   int wbase = ctrl.wa;

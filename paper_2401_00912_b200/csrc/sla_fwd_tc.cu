@@ -402,7 +402,10 @@ __device__ __forceinline__ void process_window(RingView& kv, RingView& qv, int h
   const uint32_t kv_end = kv.base + NST * C::KV_STAGE;
   for (int r = s; r < e; r += 32) {
     const int nv = min(32, e - r), rel = r - S0;
-    ring_release_below<C::SR>(kv, rel);   // skipped rows first: a wait must never pin older stages
+    // stages entirely below this step go back to the producer first: a wait must never pin older
+    // stages.  The first step's were released above; every later step frees exactly one (SR = 32).
+    if (C::SR != 32) ring_release_below<C::SR>(kv, rel);
+    else if (r != s) ring_release_one(kv);
     ring_wait_upto(kv, (rel + nv - 1) / C::SR);
 #pragma unroll
     for (int j = 0; j < C::HPW; ++j)
@@ -437,7 +440,8 @@ __device__ __forceinline__ void process_window(RingView& kv, RingView& qv, int h
   T* lp = out_head + (size_t)(s + (lane >> 2)) * Ctot + 2 * (lane & 3);
   for (int r = s; r < e; r += 32, lp += 4 * o8) {
     const int nv = min(32, e - r), rel = r - S0;
-    ring_release_below<C::SR>(qv, rel);
+    if (C::SR != 32) ring_release_below<C::SR>(qv, rel);
+    else if (r != s) ring_release_one(qv);
     ring_wait_upto(qv, (rel + nv - 1) / C::SR);
 #pragma unroll
     for (int j = 0; j < C::HPW; ++j)
@@ -533,7 +537,8 @@ __device__ __forceinline__ void output_piece(RingView& qv, int hl, int S0, int p
   T* lp = out_head + (size_t)(ps + g) * Ctot + 2 * t;
   for (int r = ps; r < pe; r += 32, lp += 4 * o8) {
     const int nv = min(32, pe - r), rel = r - S0;
-    ring_release_below<C::SR>(qv, rel);
+    if (C::SR != 32) ring_release_below<C::SR>(qv, rel);
+    else if (r != ps) ring_release_one(qv);
     ring_wait_upto(qv, (rel + nv - 1) / C::SR);
     if (nv == 32) {
       q_tile<D, BF16, false, T, true>(qv, hl, rel, 16, oo, lp, o8, aq[0]);
@@ -617,7 +622,7 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     __syncthreads();                                           // setup published (stream bounds)
     if (lane < 2) {
       S0 = ctrl.stream_begin;
-      const int total = ((dbg & 8) || (OUTPASS && is_kv)) ? 0 : (ctrl.stream_end - S0 + C::SR - 1) / C::SR;
+      const int total = (OUTPASS && is_kv) ? 0 : (ctrl.stream_end - S0 + C::SR - 1) / C::SR;
       for (int st = 0; st < total; ++st) {
         if (st >= NST) mbar_wait(empty + 8u * (st % NST), (uint32_t)(((st / NST) - 1) & 1));
         issue(st);
@@ -664,8 +669,8 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   const int nh = min(C::HPW, nheads - hl);
   const int S0 = ctrl.stream_begin;
   const int total = (ctrl.stream_end - S0 + C::SR - 1) / C::SR;
-  RingView kv = make_ring(kv_base, smem_u32(ctrl.full_kv), smem_u32(ctrl.empty_kv), (dbg >> 3) & 1);
-  RingView qv = make_ring(q_base, smem_u32(ctrl.full_q), smem_u32(ctrl.empty_q), (dbg >> 3) & 1);
+  RingView kv = make_ring(kv_base, smem_u32(ctrl.full_kv), smem_u32(ctrl.empty_kv));
+  RingView qv = make_ring(q_base, smem_u32(ctrl.full_q), smem_u32(ctrl.empty_q));
   T* out_head = out + (size_t)(h0 + hl) * D;
   if (dbg & 1) {   // debug: stream only, no compute
     ring_release_below<C::SR>(kv, total * C::SR);

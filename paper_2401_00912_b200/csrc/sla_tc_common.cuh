@@ -129,17 +129,16 @@ struct RingView {
   uint32_t empty;     // shared address of empty barriers [NST]
   int waited;
   int released;
-  int nowait;         // debug: pretend every stage has landed (timing experiments only)
   int w_slot, w_phase;   // slot and parity of stage `waited`
   int r_slot, bias;      // slot of stage `released`; bias = r_slot - released
 };
-__device__ __forceinline__ RingView make_ring(uint32_t base, uint32_t full, uint32_t empty, int nowait = 0) {
-  return RingView{base, full, empty, 0, 0, nowait, 0, 0, 0, 0};
+__device__ __forceinline__ RingView make_ring(uint32_t base, uint32_t full, uint32_t empty) {
+  return RingView{base, full, empty, 0, 0, 0, 0, 0, 0};
 }
 
 __device__ __forceinline__ void ring_wait_upto(RingView& rv, int stage_last) {
   while (rv.waited <= stage_last) {
-    if (!rv.nowait) mbar_wait(rv.full + 8u * rv.w_slot, (uint32_t)rv.w_phase);
+    mbar_wait(rv.full + 8u * rv.w_slot, (uint32_t)rv.w_phase);
     ++rv.waited;
     if (++rv.w_slot == NST) { rv.w_slot = 0; rv.w_phase ^= 1; }
   }
@@ -150,10 +149,19 @@ __device__ __forceinline__ void ring_release_below(RingView& rv, int rel) {
   while ((rv.released + 1) * SR <= rel) {
     ring_wait_upto(rv, rv.released);   // never release a stage before it has landed (phase pacing)
     __syncwarp();
-    if ((threadIdx.x & 31) == 0 && !rv.nowait) mbar_arrive(rv.empty + 8u * rv.r_slot);
+    if ((threadIdx.x & 31) == 0) mbar_arrive(rv.empty + 8u * rv.r_slot);
     ++rv.released;
     if (++rv.r_slot == NST) { rv.r_slot = 0; rv.bias -= NST; }
   }
+}
+// Steady state of a loop whose step is exactly one stage of rows: after the first step of a pass,
+// every further step starts SR rows later, so exactly one more stage -- the oldest unreleased one, which
+// the previous step has read and therefore waited for -- lies entirely below it.
+__device__ __forceinline__ void ring_release_one(RingView& rv) {
+  __syncwarp();
+  if ((threadIdx.x & 31) == 0) mbar_arrive(rv.empty + 8u * rv.r_slot);
+  ++rv.released;
+  if (++rv.r_slot == NST) { rv.r_slot = 0; rv.bias -= NST; }
 }
 
 // Shared address of (relative row rel, 16-byte chunk `chunk` of this slab row) inside a ring whose
