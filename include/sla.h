@@ -101,8 +101,10 @@ int sla_backward(const void* q, const void* k, const void* v, const int32_t* win
 
 /* End-to-end host entry (what a user with host data calls): copies q,k,v (and win_id) from HOST
  * memory to the device, runs sla_offsets_from_window_ids + sla_forward, copies `out` back to HOST
- * memory and synchronises `stream` before returning.  Device scratch is taken from the stream-ordered
- * CUDA memory pool and returned to it before the call ends.
+ * memory and synchronises `stream` before returning.  Device scratch is taken from a stream-ordered
+ * CUDA memory pool that the library creates per device on first use (unbounded release threshold, so
+ * the block is reused by the next call instead of going back to the driver) and is returned to that
+ * pool before the call ends.  This is the only entry that owns device memory; it lives until exit.
  *   q,k,v   HOST [N,H,d_h] of dt (pinned memory recommended)      win_id  HOST int32[N]
  *   out     HOST [N,H,d_h] of dt */
 int sla_forward_host(const void* q, const void* k, const void* v, const int32_t* win_id,
