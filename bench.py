@@ -39,6 +39,8 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (bench line = 1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra", action="store_true",
+                    help="skip the extra legs (config-4 training step, batch-size sweep) of the default run")
     ap.add_argument("--launch", default="graph", choices=["graph", "eager"],
                     help="timed region replays CUDA graphs captured from the C-ABI calls (default) or calls eagerly")
     ap.add_argument("--entry", default="bounded", choices=["bounded", "general"],
@@ -172,6 +174,78 @@ def cpu_oracle_time(sc, reps: int = 3):
         sla_oracle.forward(q, k, v, ids_off, nthreads=cores)
         best = min(best, time.perf_counter() - t0)
     return best, cores
+
+
+def extra_legs(pkg, torch, dev, peak):
+    """Beyond the headline line (rank 0, N = 1, config 1 only): the training step of BASELINE.json config 4
+    (sla_forward_bounded + sla_backward, N = 120 000) and the forward kernel on batches of
+    config-1 scenes (the Fig. 4-style size sweep of SURVEY 8(d)(v)).  Every tensor set here is larger than
+    the 126 MB L2 or rotated; CUDA events around K back-to-back eager calls on the current stream."""
+    from paper_2401_00912_b200 import workloads as wl
+
+    def timed(fn, K=30):
+        for i in range(3):
+            fn(i)
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for i in range(K):
+            fn(i)
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / K * 1e3   # us
+
+    out = {}
+    sc = wl.make_config(4)
+    n_sets = 2                                            # 2 x 7 x 30.7 MB = 430 MB > 2 x L2
+    sets = []
+    for r in range(n_sets):
+        t = [torch.from_numpy(sc.tensor(n)).to(torch.float16).to(dev) for n in ("q", "k", "v", "do")]
+        if r:
+            t = [x.roll(17 * r, 0).contiguous() for x in t]
+        sets.append(t + [torch.empty_like(t[0]) for _ in range(4)])
+    off = torch.from_numpy(sc.offsets).to(dev)
+    N, W, H, d = sc.N, sc.W, sc.H, sc.d_h
+    ws = torch.empty(pkg.workspace_bytes(N, W, H, d, 1, True), dtype=torch.uint8, device=dev)
+    tb = N * H * d * 2
+
+    def fwd4(i):
+        q, k, v, g, o, dq, dk, dv = sets[i % n_sets]
+        pkg.sla_forward(q, k, v, off, out=o, max_window_len=144)
+
+    def bwd4(i):
+        q, k, v, g, o, dq, dk, dv = sets[i % n_sets]
+        pkg.sla_backward(q, k, v, off, g, dq=dq, dk=dk, dv=dv, workspace=ws)
+
+    uf, ub = timed(fwd4), timed(bwd4)
+    out["training_step_config4"] = {
+        "N": N, "W": W, "fwd_us": uf, "bwd_us": ub, "fwd_bwd_us": uf + ub,
+        "voxels_per_sec_fwd_bwd": N / ((uf + ub) * 1e-6),
+        "fwd_frac_of_peak": 4 * tb / (uf * 1e-6) / 1e9 / peak,
+        "bwd_frac_of_peak": 7 * tb / (ub * 1e-6) / 1e9 / peak,
+        "bwd_algorithmic_bytes": 7 * tb, "note": "eager C-ABI calls back to back; bwd = workspace memset + sla_bwd_tc_kernel"}
+    del sets
+    sweep = []
+    for frames in (1, 2, 4, 8, 16):
+        ln = [wl.lengths_waymo_like(wl.SEED_BASE + 1 + f, 60000) for f in range(frames)]
+        scb = wl.make_scene(__import__("numpy").concatenate(ln), 8, 16, "f16", wl.SEED_BASE + 50 + frames)
+        Nb = scb.N
+        n_sets = max(2, -(-2 * L2_BYTES // (4 * Nb * 256)) + 1)
+        base = [torch.from_numpy(scb.tensor(n)).to(torch.float16).to(dev) for n in ("q", "k", "v")]
+        bs = [[x.roll(17 * r, 0).contiguous() if r else x for x in base] + [torch.empty_like(base[0])]
+              for r in range(n_sets)]
+        offb = torch.from_numpy(scb.offsets).to(dev)
+
+        def fb(i):
+            q, k, v, o = bs[i % n_sets]
+            pkg.sla_forward(q, k, v, offb, out=o, max_window_len=144)
+
+        us = timed(fb)
+        sweep.append({"frames": frames, "N": Nb, "us": us, "voxels_per_sec": Nb / (us * 1e-6),
+                      "frac_of_peak": (4 * Nb * 256 + 4 * (scb.W + 1)) / (us * 1e-6) / 1e9 / peak})
+        del bs, base
+    out["fwd_batch_sweep"] = sweep
+    return out
 
 
 def run_ours(args):
@@ -340,6 +414,9 @@ def run_ours(args):
                      "us_per_launch_event_pair_median": fwd_ms[len(fwd_ms) // 2] * 1e3,
                      "frac_of_nominal_8TBs": achieved / 8000.0},
     }
+    if rank == 0 and world == 1 and args.config == 1 and not args.no_extra:
+        with torch.cuda.stream(side):
+            line.update(extra_legs(pkg, torch, dev, peak))
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         secs, cores = cpu_oracle_time(sc)
         line["cpu_baseline"] = {"value": N / secs, "unit": UNIT, "cores": cores, "kind": "oracle",
