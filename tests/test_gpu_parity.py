@@ -203,6 +203,22 @@ def test_host_entry_matches_device_entry():
     assert torch.equal(out_h, out_d.cpu())
 
 
+def test_host_entry_repeated_calls_reuse_the_pool():
+    """sla_forward_host takes its staging block from a library-owned memory pool that keeps the block
+    between calls: calls of different sizes, interleaved and repeated, must each match the device entry
+    bit for bit (a stale or too-small reused block would show here)."""
+    torch = _torch()
+    scenes = [wl.make_config(0), wl.make_config(1), wl.make_config(0), wl.make_config(1)]
+    for sc in scenes:
+        tdt = torch.float16 if sc.dtype == "f16" else torch.float32
+        q, k, v = (torch.from_numpy(sc.tensor(n)).to(tdt).pin_memory() for n in ("q", "k", "v"))
+        ids = torch.from_numpy(sc.window_ids).pin_memory()
+        out_h = pkg.sla_forward_host(q, k, v, ids, sc.W)
+        off = torch.from_numpy(sc.offsets).cuda()
+        out_d = pkg.sla_forward(q.cuda(), k.cuda(), v.cuda(), off)
+        assert torch.equal(out_h, out_d.cpu()), sc.name
+
+
 @pytest.mark.parametrize("c", [1, 4])
 def test_forward_bounded_entry_matches_general_and_oracle(c):
     """sla_forward_bounded (one launch, no workspace; windows <= 144 rows by construction of the
