@@ -354,6 +354,24 @@ def run_ours(args):
         e1.record(side)
         torch.cuda.synchronize()
         fwd_b2b_ms = e0.elapsed_time(e1) / args.steps
+        # the same kernel as a stream of dependent launches: one graph of 4R forward calls on rotating
+        # sets; inside a graph consecutive launches keep their programmatic (PDL) edges, so the ramp of
+        # launch i+1 overlaps the tail of launch i, as it does between the kernels of a real model step
+        fwd_stream_ms = None
+        if use_graph:
+            gs = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(gs, stream=side):
+                for i in range(4 * R):
+                    fwd(i)
+            gs.replay()
+            torch.cuda.synchronize()
+            reps = max(1, args.steps // (4 * R))
+            e0.record(side)
+            for _ in range(reps):
+                gs.replay()
+            e1.record(side)
+            torch.cuda.synchronize()
+            fwd_stream_ms = e0.elapsed_time(e1) / (reps * 4 * R)
         # the general entry (sla_forward: memset + main + split-window pass), for comparison
         e0.record(side)
         for i in range(args.steps):
@@ -409,6 +427,9 @@ def run_ours(args):
                      "us_per_launch": fwd_b2b_ms * 1e3,
                      "timing": "CUDA events around the region of K back-to-back launches of the kernel, cold L2",
                      "us_general_entry_eager": fwd_general_eager_ms * 1e3,
+                     "us_per_launch_in_stream_pdl": None if fwd_stream_ms is None else fwd_stream_ms * 1e3,
+                     "frac_in_stream_pdl": None if fwd_stream_ms is None
+                                           else alg_bytes / (fwd_stream_ms * 1e-3) / 1e9 / peak,
                      "copy_ceiling_note": "a cold torch copy of the same 61 MB takes 16.8 us = 0.56 of peak (DESIGN.md 7)",
                      "us_per_launch_event_pair_avg": fwd_ms_avg * 1e3,
                      "us_per_launch_event_pair_median": fwd_ms[len(fwd_ms) // 2] * 1e3,

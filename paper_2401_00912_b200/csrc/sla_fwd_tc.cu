@@ -563,7 +563,16 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   using C = Cfg<D>;
   extern __shared__ uint8_t dyn_smem[];
   __shared__ Ctrl ctrl;
-  if (OUTPASS && reinterpret_cast<const volatile int*>(ws)[0] == 0) return;   // no split window in this call
+  // Programmatic dependent launch (the host side opts in with the stream-serialisation attribute): this
+  // grid may become resident while the previous kernel of the stream is still in its tail.  Nothing that
+  // kernel may have written (offsets, tensors, workspace) is touched before griddepcontrol.wait, which
+  // returns once that whole grid has completed; only the barrier set-up runs ahead.  The next kernel is
+  // released at once: it can only become resident when every CTA of this grid has started.
+  asm volatile("griddepcontrol.launch_dependents;");
+  if (OUTPASS) {
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (reinterpret_cast<const volatile int*>(ws)[0] == 0) return;   // no split window in this call
+  }
   const uint32_t ring = (smem_u32(dyn_smem) + 1023u) & ~1023u;
   const uint32_t kv_base = ring, q_base = ring + NST * C::KV_STAGE;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -592,6 +601,7 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  if (!OUTPASS) asm volatile("griddepcontrol.wait;" ::: "memory");
   __syncthreads();
 
   if (warp >= C::NCW) {
@@ -798,7 +808,22 @@ cudaError_t tc_launch(const Problem& p, cudaStream_t st) {
   if (span < 32) span = 32;
   nx = (p.N + span - 1) / span;
   dim3 grid(nx, slabs);
-  kern<<<grid, C::THREADS, C::SMEM_DYN, st>>>(tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H, span, dbg_env);
+  // programmatic stream serialisation: see the note at the top of the kernel
+  cudaLaunchAttribute pdl[1];
+  pdl[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  pdl[0].val.programmaticStreamSerializationAllowed = (dbg_env & 32) ? 0 : 1;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = dim3(C::THREADS);
+  cfg.dynamicSmemBytes = C::SMEM_DYN;
+  cfg.stream = st;
+  cfg.attrs = pdl;
+  cfg.numAttrs = 1;
+  {
+    cudaError_t le = cudaLaunchKernelEx(&cfg, kern, tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H, span,
+                                        dbg_env);
+    if (le != cudaSuccess) return le;
+  }
   if (!p.bounded) {
     // second pass: outputs of windows longer than kFuseMax (exits at once if there were none)
     const int span2 = span > kFuseMax ? kFuseMax / 16 * 16 : span;

@@ -13,6 +13,9 @@ namespace {
 
 __global__ void __launch_bounds__(256)
 sla_offsets_kernel(const int32_t* __restrict__ win_id, int N, int W, int32_t* __restrict__ off) {
+  // Programmatic dependent launch: a following kernel that opted in (sla_fwd_tc_kernel) may become
+  // resident now; it still waits for this whole grid (griddepcontrol.wait) before it reads `off`.
+  asm volatile("griddepcontrol.launch_dependents;");
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i > N) return;
   const int lo = (i == 0) ? 0 : __ldg(win_id + i - 1) + 1;
