@@ -828,8 +828,10 @@ cudaError_t tc_launch(const Problem& p, cudaStream_t st) {
     // second pass: outputs of windows longer than kFuseMax (exits at once if there were none)
     const int span2 = span > kFuseMax ? kFuseMax / 16 * 16 : span;
     dim3 grid2((p.N + span2 - 1) / span2, slabs);
-    kern_out<<<grid2, C::THREADS, C::SMEM_DYN, st>>>(tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H, span2,
-                                                     dbg_env);
+    cfg.gridDim = grid2;   // same attribute: resident behind the main kernel's tail, waits for its states
+    cudaError_t le = cudaLaunchKernelEx(&cfg, kern_out, tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H,
+                                        span2, dbg_env);
+    if (le != cudaSuccess) return le;
   }
   return cudaGetLastError();
 }
