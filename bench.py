@@ -248,6 +248,88 @@ def extra_legs(pkg, torch, dev, peak):
     return out
 
 
+def other_config_legs(pkg, torch, dev, peak):
+    """Forward and backward of BASELINE.json configs 2 and 3 through the general entries (sla_forward /
+    sla_backward), eager C-ABI calls back to back, CUDA events; cold L2 by rotation where one tensor set is
+    smaller than 2x L2.  Fractions are of the measured HBM peak on the algorithmic bytes of SURVEY 8(d):
+    forward 4*N*C*esz + 4(W+1), backward 7*N*C*esz."""
+    from paper_2401_00912_b200 import workloads as wl
+    tdt = {"f32": torch.float32, "f16": torch.float16, "bf16": torch.bfloat16}
+    legs = {}
+    for c in (2, 3):
+        sc = wl.make_config(c)
+        N, W, H, d = sc.N, sc.W, sc.H, sc.d_h
+        tb = N * H * d * 2
+        n_sets = max(1, -(-2 * L2_BYTES // (7 * tb)))
+        base = [torch.from_numpy(sc.tensor(n)).to(tdt[sc.dtype]).to(dev) for n in ("q", "k", "v", "do")]
+        sets = []
+        for r in range(n_sets):
+            t = [x.roll(17 * r, 0).contiguous() for x in base] if r else base
+            sets.append(t + [torch.empty_like(t[0]) for _ in range(4)])
+        off = torch.from_numpy(sc.offsets).to(dev)
+        ws = torch.empty(pkg.workspace_bytes(N, W, H, d, pkg.binding._dt(base[0]), True), dtype=torch.uint8,
+                         device=dev)
+
+        def fwd(i):
+            q, k, v, g, o, dq, dk, dv = sets[i % n_sets]
+            pkg.sla_forward(q, k, v, off, out=o, workspace=ws)
+
+        def bwd(i):
+            q, k, v, g, o, dq, dk, dv = sets[i % n_sets]
+            pkg.sla_backward(q, k, v, off, g, dq=dq, dk=dk, dv=dv, workspace=ws)
+
+        res = {"N": N, "W": W, "H": H, "d_h": d, "dtype": sc.dtype,
+               "l2_protocol": f"{n_sets} rotating set(s) of {7 * tb / 1e6:.0f} MB"}
+        for name, fn, nb, K in (("fwd", fwd, 4 * tb + 4 * (W + 1), 20), ("bwd", bwd, 7 * tb, 8)):
+            for i in range(3):
+                fn(i)
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for i in range(K):
+                fn(i)
+            b.record()
+            torch.cuda.synchronize()
+            us = a.elapsed_time(b) / K * 1e3
+            res[name + "_us"] = us
+            res[name + "_algorithmic_bytes"] = nb
+            res[name + "_frac_of_peak"] = nb / (us * 1e-6) / 1e9 / peak
+        legs[f"config{c}"] = res
+        del sets, base, ws
+        torch.cuda.empty_cache()
+    return legs
+
+
+def ncu_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the forward kernel on config 1, as recorded
+    in the committed ncu summary of this round (a line `dram_bytes_per_launch: <int>`); None if absent."""
+    import re
+    for name in ("r02_fwd_ncu_full.md",):
+        p = os.path.join(ROOT, "profiles", name)
+        if os.path.exists(p):
+            m = re.search(r"dram_bytes_per_launch:\s*(\d+)", open(p).read())
+            if m:
+                return int(m.group(1)), "profiles/" + name
+    return None, None
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` without torchrun: start N ranks of this script (one per GPU) and wait."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    procs = []
+    for r in range(args.gpus):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE=str(args.gpus),
+                   MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, os.path.abspath(__file__)] + sys.argv[1:], env=env))
+    rc = 0
+    for pr in procs:
+        rc = rc or pr.wait()
+    sys.exit(rc)
+
+
 def run_ours(args):
     import torch
     import paper_2401_00912_b200 as pkg
@@ -380,6 +462,39 @@ def run_ours(args):
         e1.record(side)
         torch.cuda.synchronize()
         fwd_general_eager_ms = e0.elapsed_time(e1) / args.steps
+        # the whole step, one event pair per step (a spin kernel first so the host runs ahead): spread
+        sev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+               for _ in range(args.steps)]
+        for i, (a, b) in enumerate(sev):
+            torch.cuda._sleep(60000)
+            a.record(side)
+            run_step(i)
+            b.record(side)
+        torch.cuda.synchronize()
+        step_us = sorted(a.elapsed_time(b) * 1e3 for a, b in sev)
+        pct = lambda xs, f: xs[min(len(xs) - 1, int(f * len(xs)))]
+        # size-matched ceiling: a pure 128-bit streaming kernel, 3 tensors in and 1 out, on
+        # the same rotating cold sets under the same protocol (graph replays back to back)
+        ceil_graphs = []
+        for r in range(R):
+            q, k, v, o = sets[r]
+            pkg.sla_bench_stream_ceiling(q, k, v, o, stream=side)
+            if use_graph:
+                gc = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(gc, stream=side):
+                    pkg.sla_bench_stream_ceiling(q, k, v, o, stream=side)
+                ceil_graphs.append(gc)
+        run_ceil = (lambda i: ceil_graphs[i % R].replay()) if use_graph else \
+                   (lambda i: pkg.sla_bench_stream_ceiling(*sets[i % R], stream=side))
+        for i in range(R):
+            run_ceil(i)
+        torch.cuda.synchronize()
+        e0.record(side)
+        for i in range(args.steps):
+            run_ceil(i)
+        e1.record(side)
+        torch.cuda.synchronize()
+        ceil_ms = e0.elapsed_time(e1) / args.steps
     peak, peak_src = measured_peaks()
     # The kernel's average launch duration = CUDA events around the timed region of K back-to-back
     # launches of that kernel (cold L2: rotating sets).  It still contains the inter-launch gaps, so it
@@ -387,6 +502,7 @@ def run_ours(args):
     # (profiles/).  The event-pair-per-launch figure (each interval also holds one graph-launch latency)
     # is reported next to it.
     achieved = alg_bytes / (fwd_b2b_ms * 1e-3) / 1e9
+    traffic, traffic_src = ncu_traffic()
 
     # end to end through the host entry point (pinned host buffers; H2D + prep + forward + D2H inside)
     out_host = torch.empty_like(host[0]).pin_memory()
@@ -404,6 +520,7 @@ def run_ours(args):
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(3, args.warmup), "ms_per_step": ms_step, "us_per_scene": ms_step * 1e3,
+        "us_per_scene_p10_p50_p90": [pct(step_us, 0.1), pct(step_us, 0.5), pct(step_us, 0.9)],
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": sc.dtype,
         "data": "synthetic", "impl": "ours",
         "config": {"workload": WORKLOAD if args.config == 1 else sc.name, "N": N, "W": W, "H": H,
@@ -420,7 +537,11 @@ def run_ours(args):
                 "api": "sla_forward_host (pinned host buffers)"},
         "gpu_launches": args.steps * (2 if bounded else 3),   # prep + forward kernel(s); memset not counted
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES if (args.config == 1 and bounded) else None, "peak_source": peak_src,
+                     "frac": achieved / peak, "traffic": traffic if args.config == 1 else None,
+                     "traffic_source": traffic_src if args.config == 1 else None, "peak_source": peak_src,
+                     "ceiling_us": ceil_ms * 1e3, "ceiling_frac": 4 * tensor_bytes / (ceil_ms * 1e-3) / 1e9 / peak,
+                     "ceiling": "sla_bench_stream_ceiling: 128-bit loads of q,k,v + store of out (3:1 mix), same "
+                                "rotating cold sets, same event protocol as us_per_launch",
                      "kernel": "sla_fwd_tc_kernel (the single launch of sla_forward_bounded)" if bounded
                                else "sla_forward (all launches of one call)",
                      "algorithmic_bytes": alg_bytes, "bytes_per_voxel": alg_bytes / N,
@@ -430,7 +551,6 @@ def run_ours(args):
                      "us_per_launch_in_stream_pdl": None if fwd_stream_ms is None else fwd_stream_ms * 1e3,
                      "frac_in_stream_pdl": None if fwd_stream_ms is None
                                            else alg_bytes / (fwd_stream_ms * 1e-3) / 1e9 / peak,
-                     "copy_ceiling_note": "a cold torch copy of the same 61 MB takes 16.8 us = 0.56 of peak (DESIGN.md 7)",
                      "us_per_launch_event_pair_avg": fwd_ms_avg * 1e3,
                      "us_per_launch_event_pair_median": fwd_ms[len(fwd_ms) // 2] * 1e3,
                      "frac_of_nominal_8TBs": achieved / 8000.0},
@@ -438,6 +558,7 @@ def run_ours(args):
     if rank == 0 and world == 1 and args.config == 1 and not args.no_extra:
         with torch.cuda.stream(side):
             line.update(extra_legs(pkg, torch, dev, peak))
+            line["other_configs"] = other_config_legs(pkg, torch, dev, peak)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         secs, cores = cpu_oracle_time(sc)
         line["cpu_baseline"] = {"value": N / secs, "unit": UNIT, "cores": cores, "kind": "oracle",
@@ -448,12 +569,6 @@ def run_ours(args):
     if world > 1:
         import torch.distributed as dist
         dist.destroy_process_group()
-
-
-# dram__bytes_read.sum + dram__bytes_write.sum of sla_fwd_tc_kernel per launch, config 1, from
-# profiles/r01_fwd_tc_ncu_full.md (46.13 MB read + 0.23 MB written; the 15.36 MB of output is still dirty in
-# L2 when the kernel ends).  Only valid for the default workload.
-NCU_TRAFFIC_BYTES = 46127360 + 234752
 
 
 def run_reference(args):
@@ -488,5 +603,7 @@ if __name__ == "__main__":
     a = parse_args()
     if a.impl == "reference":
         run_reference(a)
+    elif a.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_ranks(a)
     else:
         run_ours(a)

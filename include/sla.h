@@ -111,6 +111,14 @@ int sla_forward_host(const void* q, const void* k, const void* v, const int32_t*
                      int64_t N, int32_t W, int32_t H, int32_t d_h, int dt, void* out,
                      sla_stream_t stream);
 
+/* Measurement aid, not a step of the SLA path ("a size-matched pure read+write kernel
+ * run beside config 1 as the practical ceiling").  Streams three tensors in and one out with 128-bit
+ * accesses -- the forward's 3:1 read:write mix -- and nothing else: out = a ^ b ^ c, bytewise.
+ *   a,b,c  DEV, `bytes` bytes each, 16-byte aligned (read-only)      out  DEV, `bytes` bytes
+ *   bytes  a multiple of 16.  Enqueues one kernel on `stream`; never synchronises. */
+int sla_bench_stream_ceiling(const void* a, const void* b, const void* c, void* out, size_t bytes,
+                             sla_stream_t stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -18,7 +18,7 @@ SLA_F32, SLA_F16, SLA_BF16 = 0, 1, 2
 # Every symbol include/sla.h declares (tests check the library exports exactly these).
 SYMBOLS = (
     "sla_status_string", "sla_version", "sla_workspace_bytes", "sla_offsets_from_window_ids",
-    "sla_forward", "sla_forward_bounded", "sla_backward", "sla_forward_host",
+    "sla_forward", "sla_forward_bounded", "sla_backward", "sla_forward_host", "sla_bench_stream_ceiling",
 )
 
 _lib = None
@@ -55,6 +55,8 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     L.sla_backward.restype = ci
     L.sla_forward_host.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp]
     L.sla_forward_host.restype = ci
+    L.sla_bench_stream_ceiling.argtypes = [vp, vp, vp, vp, sz, vp]
+    L.sla_bench_stream_ceiling.restype = ci
     if path is None:
         _lib = L
     return L
@@ -172,9 +174,26 @@ def sla_forward_host(q, k, v, win_id, W: int, out=None, stream=None):
     for t in (q, k, v, win_id):
         if t.is_cuda or not t.is_contiguous():
             raise SlaError("sla_forward_host takes contiguous host tensors")
+    if not (q.shape == k.shape == v.shape and q.dim() == 3 and q.dtype == k.dtype == v.dtype):
+        raise SlaError("q,k,v must share shape [N,H,d_h] and dtype")
+    if win_id.dtype != torch.int32 or win_id.numel() != q.shape[0]:
+        raise SlaError("win_id must be int32[N]")
     N, H, d = q.shape
     if out is None:
         out = torch.empty_like(q, pin_memory=q.is_pinned())
     _check(L.sla_forward_host(q.data_ptr(), k.data_ptr(), v.data_ptr(), win_id.data_ptr(), N, W, H, d,
                               _dt(q), out.data_ptr(), _stream(stream)), "sla_forward_host")
+    return out
+
+
+def sla_bench_stream_ceiling(a, b, c, out, stream=None):
+    """Measurement aid (include/sla.h): out = a ^ b ^ c bytewise, 128-bit streaming accesses."""
+    L = load_library()
+    _chk_dev(a, b, c, out)
+    nbytes = a.numel() * a.element_size()
+    for t in (b, c, out):
+        if t.numel() * t.element_size() != nbytes:
+            raise SlaError("a, b, c, out must have the same size in bytes")
+    _check(L.sla_bench_stream_ceiling(a.data_ptr(), b.data_ptr(), c.data_ptr(), out.data_ptr(), nbytes,
+                                      _stream(stream)), "sla_bench_stream_ceiling")
     return out

@@ -1,6 +1,6 @@
 // sla_api.cu -- the extern "C" boundary declared in include/sla.h: argument validation, workspace
 // carving and kernel dispatch.  No torch types; plain pointers and sizes.
-#include <cstdlib>
+#include <mutex>
 
 #include "sla_internal.cuh"
 
@@ -56,6 +56,14 @@ int sla_offsets_from_window_ids(const int32_t* win_id, int64_t N, int32_t W, int
   return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
 }
 
+int sla_bench_stream_ceiling(const void* a, const void* b, const void* c, void* out, size_t bytes,
+                             sla_stream_t stream) {
+  if (!a || !b || !c || !out) return SLA_ERR_INVALID_ARG;
+  if (bytes % 16 != 0 || !aligned16(a) || !aligned16(b) || !aligned16(c) || !aligned16(out)) return SLA_ERR_UNSUPPORTED;
+  cudaError_t e = sla::launch_stream_ceiling(a, b, c, out, bytes, (cudaStream_t)stream);
+  return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
+}
+
 int sla_forward(const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
                 int32_t W, int32_t H, int32_t d_h, int dt, void* out, void* workspace,
                 size_t workspace_bytes, sla_stream_t stream) {
@@ -72,8 +80,7 @@ int sla_forward(const void* q, const void* k, const void* v, const int32_t* wind
   p.q = q; p.k = k; p.v = v; p.out = out; p.off = window_offsets;
   p.ws_state = static_cast<float*>(workspace);
   p.N = (int)N; p.W = W; p.H = H; p.d = d_h;
-  const char* force = getenv("SLA_FORCE_GENERIC");            // debugging/A-B switch, not a fallback
-  const bool tc = !(force && force[0] == '1') && sla::forward_tc_supported(p, dt);
+  const bool tc = sla::forward_tc_supported(p, dt);
   cudaError_t e = tc ? sla::launch_forward_tc(p, dt, st) : sla::launch_forward_generic(p, dt, st);
   return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
 }
@@ -92,8 +99,7 @@ int sla_forward_bounded(const void* q, const void* k, const void* v, const int32
   p.q = q; p.k = k; p.v = v; p.out = out; p.off = window_offsets;
   p.N = (int)N; p.W = W; p.H = H; p.d = d_h;
   p.bounded = true;                                           // one launch: no workspace, no split pass
-  const char* force = getenv("SLA_FORCE_GENERIC");
-  const bool tc = !(force && force[0] == '1') && sla::forward_tc_supported(p, dt);
+  const bool tc = sla::forward_tc_supported(p, dt);
   cudaError_t e = tc ? sla::launch_forward_tc(p, dt, (cudaStream_t)stream)
                      : sla::launch_forward_generic(p, dt, (cudaStream_t)stream);
   return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
@@ -118,8 +124,7 @@ int sla_backward(const void* q, const void* k, const void* v, const int32_t* win
   p.ws_state = static_cast<float*>(workspace);
   p.ws_dstate = reinterpret_cast<float*>(static_cast<char*>(workspace) + one);
   p.N = (int)N; p.W = W; p.H = H; p.d = d_h;
-  const char* force = getenv("SLA_FORCE_GENERIC");
-  const bool tc = !(force && force[0] == '1') && sla::backward_tc_supported(p, dt);
+  const bool tc = sla::backward_tc_supported(p, dt);
   cudaError_t e = tc ? sla::launch_backward_tc(p, dt, st) : sla::launch_backward_generic(p, dt, st);
   return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
 }
@@ -133,8 +138,10 @@ namespace {
 // threshold is 0: a real allocation and free of ~80 MB per call, several ms).
 cudaMemPool_t host_entry_pool() {
   static cudaMemPool_t pools[64] = {};
+  static std::mutex mu;
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+  std::lock_guard<std::mutex> lock(mu);
   if (!pools[dev]) {
     cudaMemPoolProps props = {};
     props.allocType = cudaMemAllocationTypePinned;

@@ -18,7 +18,7 @@
 // tells them whether there is anything to do).
 #include <cuda.h>
 
-#include <cstdlib>
+#include <atomic>
 
 #include "sla_internal.cuh"
 
@@ -472,16 +472,14 @@ cudaError_t bwd_tc_launch(const Problem& p, cudaStream_t st) {
       !make_map(&tv, p.v, p.N, Ctot, C::SR) || !make_map(&tg, p.g, p.N, Ctot, C::SR))
     return cudaErrorInvalidValue;
   auto kern = sla_bwd_tc_kernel<BF16, T>;
-  static bool attr_set = false;
-  if (!attr_set) {
+  static std::atomic<bool> attr_set[kMaxDevices];         // the smem opt-in is per device
+  const int dev = current_device();
+  if (!attr_set[dev].load(std::memory_order_acquire)) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_DYN);
     if (e != cudaSuccess) return e;
-    attr_set = true;
+    attr_set[dev].store(true, std::memory_order_release);
   }
-  static const int span_env = []() { const char* e = getenv("SLA_TC_BWD_SPAN"); return e ? atoi(e) : 0; }();
-  int span = span_env > 0 ? span_env : 32;   // short spans: the grid runs in many waves (dynamic balance)
-  span = (span + 15) / 16 * 16;
-  if (span > kFuseMax) span = kFuseMax / 16 * 16;
+  const int span = 32;   // short spans: the grid runs in many waves (dynamic balance)
   dim3 grid((p.N + span - 1) / span, (p.H + NW - 1) / NW);
   kern<<<grid, C::THREADS, C::SMEM_DYN, st>>>(tq, tk, tv, tg, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state,
                                               p.N, p.W, p.H, span);

@@ -21,7 +21,7 @@
 //     by 2^-ceil(log2 m) (the ratio of Eq. 3 is scale invariant).
 #include <cuda.h>
 
-#include <cstdlib>
+#include <atomic>
 
 #include "sla_internal.cuh"
 
@@ -356,20 +356,6 @@ __device__ __forceinline__ void quad_tile(const RingView& kv, const RingView& qv
   }
 }
 
-#ifdef SLA_TRACE
-__device__ unsigned long long g_trace[8192 * 4];
-__device__ __forceinline__ unsigned long long gtime() {
-  unsigned long long t;
-  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
-  return t;
-}
-#define TRACE(slot) do { if (threadIdx.x == 0 && blockIdx.x < 8192) g_trace[blockIdx.x * 4 + (slot)] = gtime(); } while (0)
-#define TRACE_SM() do { if (threadIdx.x == 0 && blockIdx.x < 8192) { unsigned sm; asm("mov.u32 %0, %smid;" : "=r"(sm)); g_trace[blockIdx.x * 4 + 3] = sm; } } while (0)
-#else
-#define TRACE(slot) do {} while (0)
-#define TRACE_SM() do {} while (0)
-#endif
-
 // ---- CTA-level shared control block ----------------------------------------------------------------
 struct Ctrl {
   unsigned long long full_kv[NST], empty_kv[NST], full_q[NST], empty_q[NST];
@@ -559,7 +545,7 @@ template <int D, bool BF16, typename T, bool OUTPASS>
 __global__ void __launch_bounds__(Cfg<D>::THREADS, (D == 16 ? SLA_MINB : 2))
 sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                   const __grid_constant__ CUtensorMap tmV, const int32_t* __restrict__ off,
-                  T* __restrict__ out, float* __restrict__ ws, int N, int W, int H, int span, int dbg) {
+                  T* __restrict__ out, float* __restrict__ ws, int N, int W, int H, int span) {
   using C = Cfg<D>;
   extern __shared__ uint8_t dyn_smem[];
   __shared__ Ctrl ctrl;
@@ -580,18 +566,16 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   // Map CTAs to spans outside-in: both ends of the row-major window order first.  In a LiDAR scene
   // those are the far-range rows: sparse, many 1-4 voxel windows, the slowest spans per row (measured
   // 6 rows/us against 11-12 for dense spans), so they get the head start and the fast dense spans of
-  // the middle fill the tail.  (dbg 16: natural order, for A/B measurements.)
+  // the middle fill the tail.
   const int nspan = gridDim.x;
   const int bx = blockIdx.x;
   const int sidx = (bx & 1) ? nspan - 1 - (bx >> 1) : (bx >> 1);
-  const int R0 = (dbg & 16) ? bx * span : sidx * span, R1 = min(R0 + span, N);
+  const int R0 = sidx * span, R1 = min(R0 + span, N);
   const int h0 = blockIdx.y * NW;
   const int nheads = min(NW, H - h0);                       // heads of this slab
   const int nact = (nheads + C::HPW - 1) / C::HPW;           // active consumer warps
   const int Ctot = H * D;
 
-  TRACE(0);
-  TRACE_SM();
   if (threadIdx.x == 0) {
     for (int i = 0; i < NST; ++i) {
       mbar_init(smem_u32(&ctrl.full_kv[i]), 1);
@@ -665,14 +649,10 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       }
       ctrl.wa = wa;
       ctrl.stream_begin = sb;
-      ctrl.stream_end = (dbg & 2) ? sb : max(se, sb);   // dbg 2: setup only, nothing streamed
+      ctrl.stream_end = max(se, sb);
     }
   }
   __syncthreads();
-  TRACE(1);
-#ifdef SLA_TRACE
-  if (threadIdx.x == 0 && blockIdx.x < 8192) g_trace[blockIdx.x * 4 + 3] |= ((unsigned long long)(ctrl.stream_end - ctrl.stream_begin)) << 16;
-#endif
   if (warp >= nact) return;
 
   const int hl = warp * C::HPW;                              // first head (within the slab) of this warp
@@ -682,11 +662,6 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   RingView kv = make_ring(kv_base, smem_u32(ctrl.full_kv), smem_u32(ctrl.empty_kv));
   RingView qv = make_ring(q_base, smem_u32(ctrl.full_q), smem_u32(ctrl.empty_q));
   T* out_head = out + (size_t)(h0 + hl) * D;
-  if (dbg & 1) {   // debug: stream only, no compute
-    ring_release_below<C::SR>(kv, total * C::SR);
-    ring_release_below<C::SR>(qv, total * C::SR);
-    return;
-  }
 
   // window walk with a 32-entry register cache of the offsets (one global round trip per 31 windows)
   int wbase = ctrl.wa;
@@ -759,7 +734,7 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     }
     if (m <= kFuseMax) {
       process_window<D, BF16, false, T>(kv, qv, hl, nh, S0, s, e, out_head, Ctot);
-    } else {
+    } else if (ws != nullptr) {   // bounded entry (no workspace): a window that breaks the caller's promise is skipped
       float* slot = ws + kWsHeaderFloats + ((size_t)(s / (kFuseMax + 1)) * H + (h0 + hl)) * (size_t)((D + 1) * D);
       if (hl == 0 && lane == 0) reinterpret_cast<volatile int*>(ws)[0] = 1;   // tell the output kernel
       process_piece<D, BF16>(kv, hl, nh, S0, max(s, R0), min(e, R1), slot);
@@ -770,7 +745,6 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   ring_release_below<C::SR>(kv, total * C::SR);
   ring_release_below<C::SR>(qv, total * C::SR);
   }
-  TRACE(2);
 }
 
 // ---- host side (tensor-map encoder, SM count: sla_tc_common.cuh) -----------------------------------
@@ -784,26 +758,21 @@ cudaError_t tc_launch(const Problem& p, cudaStream_t st) {
     return cudaErrorInvalidValue;
   auto kern = sla_fwd_tc_kernel<D, BF16, T, false>;
   auto kern_out = sla_fwd_tc_kernel<D, BF16, T, true>;
-  static bool attr_set = false;
-  if (!attr_set) {
+  // the dynamic shared-memory opt-in is per device: set it once for every device this process uses
+  static std::atomic<bool> attr_set[kMaxDevices];
+  const int dev = current_device();
+  if (!attr_set[dev].load(std::memory_order_acquire)) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_DYN);
     if (e == cudaSuccess)
       e = cudaFuncSetAttribute(kern_out, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_DYN);
     if (e != cudaSuccess) return e;
-    attr_set = true;
+    attr_set[dev].store(true, std::memory_order_release);
   }
   const int slabs = (p.H + NW - 1) / NW;
-  static const int per_sm = []() {                          // resident CTAs per SM the grid is sized for
-    const char* e = getenv("SLA_TC_CTAS_PER_SM");
-    const int v = e ? atoi(e) : 0;
-    return v > 0 ? v : (D == 16 ? 3 : 2);
-  }();
+  const int per_sm = (D == 16 ? 3 : 2);                     // resident CTAs per SM the grid is sized for
   int nx = (per_sm * sm_count() + slabs - 1) / slabs;
   int span = (p.N + nx - 1) / nx;
-  static const int dbg_env = []() { const char* e = getenv("SLA_TC_DBG"); return e ? atoi(e) : 0; }();
-  static const int span_env = []() { const char* e = getenv("SLA_TC_SPAN"); return e ? atoi(e) : 0; }();
   if (span > 64) span = 64;             // short spans, several waves: dynamic balance across SMs
-  if (span_env > 0) span = span_env;
   span = (span + 15) / 16 * 16;
   if (span < 32) span = 32;
   nx = (p.N + span - 1) / span;
@@ -811,7 +780,7 @@ cudaError_t tc_launch(const Problem& p, cudaStream_t st) {
   // programmatic stream serialisation: see the note at the top of the kernel
   cudaLaunchAttribute pdl[1];
   pdl[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  pdl[0].val.programmaticStreamSerializationAllowed = (dbg_env & 32) ? 0 : 1;
+  pdl[0].val.programmaticStreamSerializationAllowed = 1;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = grid;
   cfg.blockDim = dim3(C::THREADS);
@@ -820,8 +789,7 @@ cudaError_t tc_launch(const Problem& p, cudaStream_t st) {
   cfg.attrs = pdl;
   cfg.numAttrs = 1;
   {
-    cudaError_t le = cudaLaunchKernelEx(&cfg, kern, tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H, span,
-                                        dbg_env);
+    cudaError_t le = cudaLaunchKernelEx(&cfg, kern, tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H, span);
     if (le != cudaSuccess) return le;
   }
   if (!p.bounded) {
@@ -830,19 +798,13 @@ cudaError_t tc_launch(const Problem& p, cudaStream_t st) {
     dim3 grid2((p.N + span2 - 1) / span2, slabs);
     cfg.gridDim = grid2;   // same attribute: resident behind the main kernel's tail, waits for its states
     cudaError_t le = cudaLaunchKernelEx(&cfg, kern_out, tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H,
-                                        span2, dbg_env);
+                                        span2);
     if (le != cudaSuccess) return le;
   }
   return cudaGetLastError();
 }
 
 }  // namespace
-
-#ifdef SLA_TRACE
-extern "C" int sla_debug_read_trace(unsigned long long* host, int n) {
-  return (int)cudaMemcpyFromSymbol(host, g_trace, sizeof(unsigned long long) * n);
-}
-#endif
 
 bool forward_tc_supported(const Problem& p, int dt) {
   if (dt != SLA_F16 && dt != SLA_BF16) return false;

@@ -157,7 +157,7 @@ sla_fwd_generic_kernel(const T* __restrict__ q, const T* __restrict__ k, const T
       for (int p = 0; p < D; ++p) S[p] = 0.f;
       accumulate_state<T, D>(k, v, s, e, cx, bs, S, z);
       emit_output<T, D>(q, out, s, e, cx, bs, S, z);
-    } else {
+    } else if (ws != nullptr) {   // bounded entry (no workspace): a window that breaks the caller's promise is skipped
       float S[D], z = 0.f;
 #pragma unroll
       for (int p = 0; p < D; ++p) S[p] = 0.f;
@@ -496,16 +496,6 @@ cudaError_t fwd_launch(const Problem& p, cudaStream_t st) {
 }
 
 template <typename T, int D>
-cudaError_t fwd_split_launch(const Problem& p, cudaStream_t st) {
-  const int CB = block_threads(p.H, D);
-  const int HB = CB / D;
-  dim3 grid((p.N + kTileRows - 1) / kTileRows, (p.H + HB - 1) / HB);
-  sla_fwd_generic_split_kernel<T, D><<<grid, CB, 0, st>>>((const T*)p.q, p.off, (T*)p.out, p.ws_state,
-                                                          p.N, p.W, p.H);
-  return cudaGetLastError();
-}
-
-template <typename T, int D>
 cudaError_t bwd_launch(const Problem& p, cudaStream_t st, int split_only = 0) {
   const int CB = block_threads(p.H, D);
   const int HB = CB / D;
@@ -533,17 +523,6 @@ cudaError_t launch_forward_generic(const Problem& p, int dt, cudaStream_t st) {
   if (dt == SLA_F32) return fwd_launch<float, 32>(p, st);
   if (dt == SLA_F16) return fwd_launch<__half, 32>(p, st);
   return fwd_launch<__nv_bfloat16, 32>(p, st);
-}
-
-cudaError_t launch_forward_generic_split_only(const Problem& p, int dt, cudaStream_t st) {
-  if (p.d == 16) {
-    if (dt == SLA_F32) return fwd_split_launch<float, 16>(p, st);
-    if (dt == SLA_F16) return fwd_split_launch<__half, 16>(p, st);
-    return fwd_split_launch<__nv_bfloat16, 16>(p, st);
-  }
-  if (dt == SLA_F32) return fwd_split_launch<float, 32>(p, st);
-  if (dt == SLA_F16) return fwd_split_launch<__half, 32>(p, st);
-  return fwd_split_launch<__nv_bfloat16, 32>(p, st);
 }
 
 cudaError_t launch_backward_generic_split_only(const Problem& p, int dt, cudaStream_t st) {

@@ -75,14 +75,14 @@ struct Problem {
 cudaError_t launch_offsets(const int32_t* win_id, int N, int W, int32_t* off, cudaStream_t st);
 cudaError_t launch_forward_generic(const Problem& p, int dt, cudaStream_t st);
 cudaError_t launch_backward_generic(const Problem& p, int dt, cudaStream_t st);
-// second kernel of the forward only: outputs of windows longer than kFuseMax (state from ws_state)
-cudaError_t launch_forward_generic_split_only(const Problem& p, int dt, cudaStream_t st);
-// tensor-core forward (fp16/bf16): main TMA/mma kernel + the split-window output kernel
 // backward of windows longer than kFuseMax only (needs the workspace flag set by the tensor-core kernel)
 cudaError_t launch_backward_generic_split_only(const Problem& p, int dt, cudaStream_t st);
 bool backward_tc_supported(const Problem& p, int dt);
 cudaError_t launch_backward_tc(const Problem& p, int dt, cudaStream_t st);
 bool forward_tc_supported(const Problem& p, int dt);
 cudaError_t launch_forward_tc(const Problem& p, int dt, cudaStream_t st);
+// measurement aid (sla_bench_stream_ceiling): out = a ^ b ^ c over `bytes` bytes per tensor, 128-bit accesses
+cudaError_t launch_stream_ceiling(const void* a, const void* b, const void* c, void* out, size_t bytes,
+                                  cudaStream_t st);
 
 }  // namespace sla

@@ -1,7 +1,10 @@
 """GPU parity: the CUDA path (through the C ABI) against the fp64 CPU oracle, element by element on
 the same seeded inputs.  Tolerances (BASELINE.json north_star; reading A11):
   |gpu - ref| <= atol + rtol*|ref|,  fp32: rtol 1e-5, atol 1e-6;  fp16/bf16: rtol 2e-2, atol 1e-3.
-Gradients additionally: relative L2 error <= 1e-2 (fp16/bf16), 1e-5 (fp32)."""
+Gradients additionally: relative L2 error <= 1e-2 (fp16/bf16), 1e-5 (fp32), taken over the rows
+of windows with >= 2 voxels and, separately, over the rows of windows longer than 256 voxels (whose small
+gradients would pass the atol of the elementwise check trivially).  Rows of length-1 windows (dq = dk = 0
+exactly, so a relative norm is ill-posed there) keep the elementwise check only."""
 import numpy as np
 import pytest
 
@@ -63,13 +66,20 @@ def run_backward(sc):
 
 
 def check_grads(grads, ref, sc):
+    lengths = np.asarray(sc.lengths)
+    row_len = np.repeat(lengths, lengths)                 # window length of every row
+    groups = [("windows>=2", row_len >= 2), ("windows>256", row_len > 256)]
     for name, got, want in zip(("dq", "dk", "dv"), grads, ref):
         check(f"{sc.name}.{name}", got, want, sc.dtype, sc.lengths)
         gotd = got.double().cpu().numpy()
-        # mixed criterion: ||diff|| <= REL_L2*||want|| + atol*sqrt(n)  (length-1 windows have dq = dk = 0
-        # exactly, so a purely relative norm is meaningless there)
-        bound = REL_L2[sc.dtype] * np.linalg.norm(want) + TOL[sc.dtype][1] * np.sqrt(want.size)
-        assert np.linalg.norm(gotd - want) <= bound, f"{sc.name}.{name}: L2 error {np.linalg.norm(gotd - want):.3e} > {bound:.3e}"
+        for gname, rows in groups:
+            if not rows.any():
+                continue
+            den = np.linalg.norm(want[rows])
+            if den == 0.0:
+                continue
+            rel = np.linalg.norm(gotd[rows] - want[rows]) / den
+            assert rel <= REL_L2[sc.dtype], f"{sc.name}.{name} [{gname}]: relative L2 error {rel:.3e} > {REL_L2[sc.dtype]:.0e}"
 
 
 # ---- prep kernel: bit-exact ----------------------------------------------------------------------
@@ -159,6 +169,13 @@ def test_large_magnitude_inputs(dtype):
     out = pkg.sla_forward(to_dev(q, dtype), to_dev(k, dtype), to_dev(v, dtype), off)
     ref = sla_oracle.forward(q, k, v, sc.offsets)
     check("large_magnitude.out", out, ref, dtype, sc.lengths)
+    # backward on the same inputs: phi' spans e^-20 .. 1, den spans orders of magnitude
+    g = sc.tensor("do")
+    grads = pkg.sla_backward(to_dev(q, dtype), to_dev(k, dtype), to_dev(v, dtype), off, to_dev(g, dtype))
+    torch.cuda.synchronize()
+    gref = sla_oracle.backward(q, k, v, g, sc.offsets)
+    for name, got, want in zip(("dq", "dk", "dv"), grads, gref):
+        check(f"large_magnitude.{name}", got, want, dtype, sc.lengths)
 
 
 def test_n0_w0_and_errors():
