@@ -269,91 +269,16 @@ __device__ __forceinline__ void q_tile(const RingView& rv, int hl, int rel0, int
   }
 }
 
-// ---- packed short windows: masked quadratic form inside one 16-row tile -----------------------------
-// Several WHOLE windows of <= 16 rows each are packed into one tile of <= 16 consecutive rows and
-// evaluated in the (mathematically identical) quadratic form
-//   P = phi(Q) phi(K)^T  masked to same-window pairs,   O = (P / rowsum P) V
-// so a 1-voxel window costs 1/16 of a tile instead of a whole one.  phi(Q), phi(K) and the normalised
-// P are split into fp16 hi+lo operands (~22-bit products).  `wid` = window ordinal of tile row `lane`
-// (lanes >= nvalid hold -1).
+// packed short windows (quad_tile_core, sla_tc_base.cuh) on rows rel0.. of this CTA's K/V and Q rings
 template <int D, bool BF16, typename T>
 __device__ __forceinline__ void quad_tile(const RingView& kv, const RingView& qv, int hl, int rel0,
                                           int nvalid, int wid, T* __restrict__ out_rows, int C_total) {
   using C = Cfg<D>;
-  const int lane = threadIdx.x & 31;
-  const int g = lane >> 2, t = lane & 3;
-  const int mi = lane >> 3;
-  int trow = (lane & 7) + 8 * (mi >> 1);
-  if (trow >= nvalid) trow = 0;
-  const int csel = mi & 1;
-  // P[jt][c]: rows i = g (c<2) / g+8 (c>=2), cols j = 8*jt + 2t + (c&1)
-  float P[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
-#pragma unroll
-  for (int ks = 0; ks < D / 16; ++ks) {
-    const int chunk = hl * (D / 8) + 2 * ks + csel;
-    uint32_t qr[4], kr[4];
-    ldsm_x4(ring_addr<D>(qv, C::T_STAGE, 0, rel0 + trow, chunk), qr);
-    ldsm_x4(ring_addr<D>(kv, C::KV_STAGE, 0, rel0 + trow, chunk), kr);
-    uint32_t ahi[4], alo[4], bhi[4], blo[4];
-    const int perm[4] = {0, 2, 1, 3};   // (rows0-7,c0),(rows0-7,c1),(rows8-15,c0),(rows8-15,c1) -> a0..a3
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      float2 x = unpack2<BF16>(qr[perm[i]]);
-      split_h2(phi_fast(x.x), phi_fast(x.y), ahi[i], alo[i]);
-      float2 y = unpack2<BF16>(kr[i]);
-      split_h2(phi_fast(y.x), phi_fast(y.y), bhi[i], blo[i]);
-    }
-    // K (non-transposed) as B operand: j-tile 0 -> (b0,b1) = (r0,r1); j-tile 1 -> (r2,r3)
-#pragma unroll
-    for (int jt = 0; jt < 2; ++jt) {
-      mma16816(P[jt], ahi[0], ahi[1], ahi[2], ahi[3], bhi[2 * jt], bhi[2 * jt + 1]);
-      mma16816(P[jt], alo[0], alo[1], alo[2], alo[3], bhi[2 * jt], bhi[2 * jt + 1]);
-      mma16816(P[jt], ahi[0], ahi[1], ahi[2], ahi[3], blo[2 * jt], blo[2 * jt + 1]);
-    }
-  }
-  // same-window mask and row sums
-  const int wi0 = __shfl_sync(0xffffffffu, wid, g), wi1 = __shfl_sync(0xffffffffu, wid, g + 8);
-  float rs0 = 0.f, rs1 = 0.f;
-#pragma unroll
-  for (int jt = 0; jt < 2; ++jt)
-#pragma unroll
-    for (int c = 0; c < 2; ++c) {
-      const int wj = __shfl_sync(0xffffffffu, wid, 8 * jt + 2 * t + c);
-      P[jt][c] = (wj == wi0 && wj >= 0) ? P[jt][c] : 0.f;
-      P[jt][2 + c] = (wj == wi1 && wj >= 0) ? P[jt][2 + c] : 0.f;
-      rs0 += P[jt][c];
-      rs1 += P[jt][2 + c];
-    }
-  rs0 += __shfl_xor_sync(0xffffffffu, rs0, 1); rs0 += __shfl_xor_sync(0xffffffffu, rs0, 2);
-  rs1 += __shfl_xor_sync(0xffffffffu, rs1, 1); rs1 += __shfl_xor_sync(0xffffffffu, rs1, 2);
-  const float inv0 = (g < nvalid) ? fast_rcp(rs0) : 0.f, inv1 = (g + 8 < nvalid) ? fast_rcp(rs1) : 0.f;
-  // normalised weights as A operand (k = j): a0=(g,2t..) a1=(g+8,2t..) a2=(g,2t+8..) a3=(g+8,2t+8..)
-  uint32_t phi_[4], plo_[4];
-  split_h2(P[0][0] * inv0, P[0][1] * inv0, phi_[0], plo_[0]);
-  split_h2(P[0][2] * inv1, P[0][3] * inv1, phi_[1], plo_[1]);
-  split_h2(P[1][0] * inv0, P[1][1] * inv0, phi_[2], plo_[2]);
-  split_h2(P[1][2] * inv1, P[1][3] * inv1, phi_[3], plo_[3]);
-#pragma unroll
-  for (int cp = 0; cp < D / 16; ++cp) {
-    uint32_t vr[4];
-    ldsm_x4_t(ring_addr<D>(kv, C::KV_STAGE, C::T_STAGE, rel0 + trow, hl * (D / 8) + 2 * cp + csel), vr);
-    if (BF16) {
-#pragma unroll
-      for (int i = 0; i < 4; ++i) { float2 x = unpack2<true>(vr[i]); vr[i] = pack_h2(x.x, x.y); }
-    }
-    // V (transposed) as B operand: n-tile 2cp -> (r0,r2); n-tile 2cp+1 -> (r1,r3)
-#pragma unroll
-    for (int half = 0; half < 2; ++half) {
-      const int nt = 2 * cp + half;
-      float acc[4] = {0.f, 0.f, 0.f, 0.f};
-      mma16816(acc, phi_[0], phi_[1], phi_[2], phi_[3], vr[half], vr[2 + half]);
-      mma16816(acc, plo_[0], plo_[1], plo_[2], plo_[3], vr[half], vr[2 + half]);
-      uint32_t* p0 = reinterpret_cast<uint32_t*>(out_rows + (size_t)g * C_total + 8 * nt + 2 * t);
-      uint32_t* p1 = reinterpret_cast<uint32_t*>(out_rows + (size_t)(g + 8) * C_total + 8 * nt + 2 * t);
-      if (g < nvalid) *p0 = pack_out<BF16>(acc[0], acc[1]);
-      if (g + 8 < nvalid) *p1 = pack_out<BF16>(acc[2], acc[3]);
-    }
-  }
+  quad_tile_core<D, BF16, T>(
+      [&](int r, int c) { return ring_addr<D>(qv, C::T_STAGE, 0, rel0 + r, c); },
+      [&](int r, int c) { return ring_addr<D>(kv, C::KV_STAGE, 0, rel0 + r, c); },
+      [&](int r, int c) { return ring_addr<D>(kv, C::KV_STAGE, C::T_STAGE, rel0 + r, c); }, hl, nvalid, wid,
+      out_rows, C_total);
 }
 
 // ---- CTA-level shared control block ----------------------------------------------------------------
@@ -748,8 +673,10 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
 }
 
 // ---- host side (tensor-map encoder, SM count: sla_tc_common.cuh) -----------------------------------
+// `main_pass` = false: only the OUTPASS launch (the main pass was done by the tcgen05 kernel, sla_fwd_umma.cu,
+// which follows the same workspace protocol).
 template <int D, bool BF16, typename T>
-cudaError_t tc_launch(const Problem& p, cudaStream_t st) {
+cudaError_t tc_launch(const Problem& p, cudaStream_t st, bool main_pass) {
   using C = Cfg<D>;
   CUtensorMap tq, tk, tv;
   const int Ctot = p.H * D;
@@ -788,7 +715,7 @@ cudaError_t tc_launch(const Problem& p, cudaStream_t st) {
   cfg.stream = st;
   cfg.attrs = pdl;
   cfg.numAttrs = 1;
-  {
+  if (main_pass) {
     cudaError_t le = cudaLaunchKernelEx(&cfg, kern, tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H, span);
     if (le != cudaSuccess) return le;
   }
@@ -813,9 +740,20 @@ bool forward_tc_supported(const Problem& p, int dt) {
 }
 
 cudaError_t launch_forward_tc(const Problem& p, int dt, cudaStream_t st) {
+  bool main_pass = true;
+#ifndef SLA_NO_UMMA
+  if (forward_umma_supported(p, dt)) {   // main pass on tcgen05 (sla_fwd_umma.cu); long windows' outputs below
+    cudaError_t e = launch_forward_umma_main(p, dt, st);
+    if (e != cudaSuccess) return e;
+    if (p.bounded) return cudaSuccess;
+    main_pass = false;
+  }
+#endif
   cudaError_t e;
-  if (p.d == 16) e = (dt == SLA_F16) ? tc_launch<16, false, __half>(p, st) : tc_launch<16, true, __nv_bfloat16>(p, st);
-  else e = (dt == SLA_F16) ? tc_launch<32, false, __half>(p, st) : tc_launch<32, true, __nv_bfloat16>(p, st);
+  if (p.d == 16)
+    e = (dt == SLA_F16) ? tc_launch<16, false, __half>(p, st, main_pass) : tc_launch<16, true, __nv_bfloat16>(p, st, main_pass);
+  else
+    e = (dt == SLA_F16) ? tc_launch<32, false, __half>(p, st, main_pass) : tc_launch<32, true, __nv_bfloat16>(p, st, main_pass);
   return e;
 }
 

@@ -81,6 +81,9 @@ bool backward_tc_supported(const Problem& p, int dt);
 cudaError_t launch_backward_tc(const Problem& p, int dt, cudaStream_t st);
 bool forward_tc_supported(const Problem& p, int dt);
 cudaError_t launch_forward_tc(const Problem& p, int dt, cudaStream_t st);
+// tcgen05 main pass of the forward (sla_fwd_umma.cu): fused windows + partial states of long windows
+bool forward_umma_supported(const Problem& p, int dt);
+cudaError_t launch_forward_umma_main(const Problem& p, int dt, cudaStream_t st);
 // measurement aid (sla_bench_stream_ceiling): out = a ^ b ^ c over `bytes` bytes per tensor, 128-bit accesses
 cudaError_t launch_stream_ceiling(const void* a, const void* b, const void* c, void* out, size_t bytes,
                                   cudaStream_t st);

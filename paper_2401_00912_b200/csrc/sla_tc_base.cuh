@@ -1,0 +1,287 @@
+// sla_tc_base.cuh -- helpers shared by every tensor-core kernel of the library: PTX wrappers (mbarrier, TMA,
+// ldmatrix, mma.sync), element / feature-map helpers, the warp-wide window search, the packed
+// short-window tile (masked quadratic form) and the host-side tensor-map encoder.
+//
+// Include it INSIDE the translation unit's `namespace sla { namespace { ... } }`.
+#ifndef SLA_TC_BASE_INCLUDED
+#define SLA_TC_BASE_INCLUDED
+
+// ---- PTX wrappers ---------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred P1;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2, %3;\n\t"
+        "selp.b32 %0, 1, 0, P1;\n\t}"
+        : "=r"(done) : "r"(bar), "r"(parity), "r"(20000u) : "memory");
+  } while (!done);
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int x, int y) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cta.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+      ::"r"(dst), "l"(tm), "r"(bar), "r"(x), "r"(y) : "memory");
+}
+__device__ __forceinline__ void ldsm_x4(uint32_t addr, uint32_t (&r)[4]) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void ldsm_x4_t(uint32_t addr, uint32_t (&r)[4]) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+// D(16x8,f32) += A(16x16,f16,row) * B(16x8,f16,col)
+__device__ __forceinline__ void mma16816(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
+                                         uint32_t b0, uint32_t b1) {
+  asm(
+      "mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+      : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+      : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+
+// ---- element helpers ------------------------------------------------------------------------------
+template <bool BF16>
+__device__ __forceinline__ float2 unpack2(uint32_t r) {   // two packed I/O elements -> fp32
+  if (BF16) return make_float2(__uint_as_float(r << 16), __uint_as_float(r & 0xffff0000u));
+  return __half22float2(*reinterpret_cast<const __half2*>(&r));
+}
+__device__ __forceinline__ uint32_t pack_h2(float lo, float hi) {
+  __half2 h = __floats2half2_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&h);
+}
+template <bool BF16>
+__device__ __forceinline__ uint32_t pack_out(float lo, float hi) {
+  if (BF16) {
+    __nv_bfloat162 b = __floats2bfloat162_rn(lo, hi);
+    return *reinterpret_cast<uint32_t*>(&b);
+  }
+  return pack_h2(lo, hi);
+}
+// phi(x) = elu(x)+1 (reading A1); fast exp (ex2.approx) -- relative error ~2^-21, far below fp16 operands
+// Branch-free: phi = max(x,0) + 2^min(x*log2e, 0)  (x > 0: x + 2^0 = x + 1 exactly; x <= 0: e^x), and the
+// second term alone is phi'(x) = (x > 0 ? 1 : e^x).  One ex2.approx.ftz (relative error 2^-22) instead of
+// __expf's range-checked sequence: 5 instructions per element.
+__device__ __forceinline__ float ex2_fast(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float dphi_fast(float x) { return ex2_fast(fminf(x * 1.4426950408889634f, 0.f)); }
+__device__ __forceinline__ float phi_fast(float x) { return fmaxf(x, 0.f) + dphi_fast(x); }
+
+// phi on two packed I/O elements, evaluated in fp16x2 (long windows only: the operand is rounded to
+// fp16 anyway).  Branch-free on the FMA pipe (the ALU pipe is the busy one in these kernels):
+//   r = relu(x*log2e)            (fma.relu)
+//   t = x*log2e - r = min(x*log2e, 0)   (one fused rounding)
+//   phi = 2^t + r*ln2            x <= 0: r = 0, phi = 2^(x*log2e) = e^x
+//                                x  > 0: t is only the rounding residual of r, 2^t = 1 + t*ln2 + ..., so
+//                                        phi = 1 + x to first order in that residual (~1.5 fp16 ulp)
+// Result: fp16x2 {phi(x0), phi(x1)}.
+template <bool BF16>
+__device__ __forceinline__ uint32_t phi_h2(uint32_t raw) {
+  uint32_t x = raw;
+  if (BF16) { float2 f = unpack2<true>(raw); x = pack_h2(f.x, f.y); }
+  uint32_t r, t, e, out;
+  const uint32_t log2e = 0x3DC53DC5u, ln2 = 0x398C398Cu, zero = 0u;   // fp16 1.4424, 0.6931
+  asm("fma.rn.relu.f16x2 %0, %1, %2, %3;" : "=r"(r) : "r"(x), "r"(log2e), "r"(zero));
+  asm("{\n\t.reg .b32 nr;\n\tneg.f16x2 nr, %3;\n\tfma.rn.f16x2 %0, %1, %2, nr;\n\t}"
+      : "=r"(t) : "r"(x), "r"(log2e), "r"(r));
+  asm("ex2.approx.f16x2 %0, %1;" : "=r"(e) : "r"(t));
+  asm("fma.rn.f16x2 %0, %1, %2, %3;" : "=r"(out) : "r"(r), "r"(ln2), "r"(e));
+  return out;
+}
+__device__ __forceinline__ float fast_rcp(float x) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+
+// fp32 pair -> fp16x2 "hi" and the fp16x2 residual "lo"
+__device__ __forceinline__ void split_h2(float x0, float x1, uint32_t& hi, uint32_t& lo) {
+  __half2 h = __floats2half2_rn(x0, x1);
+  float2 hf = __half22float2(h);
+  hi = *reinterpret_cast<uint32_t*>(&h);
+  lo = pack_h2(x0 - hf.x, x1 - hf.y);
+}
+
+// ---- packed short windows: masked quadratic form inside one 16-row tile -----------------------------
+// Several WHOLE windows of <= 16 rows each are packed into one tile of <= 16 consecutive rows and
+// evaluated in the (mathematically identical) quadratic form
+//   P = phi(Q) phi(K)^T  masked to same-window pairs,   O = (P / rowsum P) V
+// so a 1-voxel window costs 1/16 of a tile instead of a whole one.  phi(Q), phi(K) and the normalised
+// P are split into fp16 hi+lo operands (~22-bit products).  `wid` = window ordinal of tile row `lane`
+// (lanes >= nvalid hold -1).
+//
+// The tile's rows live in shared memory in the 128-byte-swizzled layout the TMA boxes have; the three
+// functors return the shared address of (tile row, 16-byte chunk of the slab row) of Q, K and V.
+template <int D, bool BF16, typename T, typename QA, typename KA, typename VA>
+__device__ __forceinline__ void quad_tile_core(QA qaddr, KA kaddr, VA vaddr, int hl, int nvalid, int wid,
+                                               T* __restrict__ out_rows, int C_total) {
+  const int lane = threadIdx.x & 31;
+  const int g = lane >> 2, t = lane & 3;
+  const int mi = lane >> 3;
+  int trow = (lane & 7) + 8 * (mi >> 1);
+  if (trow >= nvalid) trow = 0;
+  const int csel = mi & 1;
+  // P[jt][c]: rows i = g (c<2) / g+8 (c>=2), cols j = 8*jt + 2t + (c&1)
+  float P[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+#pragma unroll
+  for (int ks = 0; ks < D / 16; ++ks) {
+    const int chunk = hl * (D / 8) + 2 * ks + csel;
+    uint32_t qr[4], kr[4];
+    ldsm_x4(qaddr(trow, chunk), qr);
+    ldsm_x4(kaddr(trow, chunk), kr);
+    uint32_t ahi[4], alo[4], bhi[4], blo[4];
+    const int perm[4] = {0, 2, 1, 3};   // (rows0-7,c0),(rows0-7,c1),(rows8-15,c0),(rows8-15,c1) -> a0..a3
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      float2 x = unpack2<BF16>(qr[perm[i]]);
+      split_h2(phi_fast(x.x), phi_fast(x.y), ahi[i], alo[i]);
+      float2 y = unpack2<BF16>(kr[i]);
+      split_h2(phi_fast(y.x), phi_fast(y.y), bhi[i], blo[i]);
+    }
+    // K (non-transposed) as B operand: j-tile 0 -> (b0,b1) = (r0,r1); j-tile 1 -> (r2,r3)
+#pragma unroll
+    for (int jt = 0; jt < 2; ++jt) {
+      mma16816(P[jt], ahi[0], ahi[1], ahi[2], ahi[3], bhi[2 * jt], bhi[2 * jt + 1]);
+      mma16816(P[jt], alo[0], alo[1], alo[2], alo[3], bhi[2 * jt], bhi[2 * jt + 1]);
+      mma16816(P[jt], ahi[0], ahi[1], ahi[2], ahi[3], blo[2 * jt], blo[2 * jt + 1]);
+    }
+  }
+  // same-window mask and row sums
+  const int wi0 = __shfl_sync(0xffffffffu, wid, g), wi1 = __shfl_sync(0xffffffffu, wid, g + 8);
+  float rs0 = 0.f, rs1 = 0.f;
+#pragma unroll
+  for (int jt = 0; jt < 2; ++jt)
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+      const int wj = __shfl_sync(0xffffffffu, wid, 8 * jt + 2 * t + c);
+      P[jt][c] = (wj == wi0 && wj >= 0) ? P[jt][c] : 0.f;
+      P[jt][2 + c] = (wj == wi1 && wj >= 0) ? P[jt][2 + c] : 0.f;
+      rs0 += P[jt][c];
+      rs1 += P[jt][2 + c];
+    }
+  rs0 += __shfl_xor_sync(0xffffffffu, rs0, 1); rs0 += __shfl_xor_sync(0xffffffffu, rs0, 2);
+  rs1 += __shfl_xor_sync(0xffffffffu, rs1, 1); rs1 += __shfl_xor_sync(0xffffffffu, rs1, 2);
+  const float inv0 = (g < nvalid) ? fast_rcp(rs0) : 0.f, inv1 = (g + 8 < nvalid) ? fast_rcp(rs1) : 0.f;
+  // normalised weights as A operand (k = j): a0=(g,2t..) a1=(g+8,2t..) a2=(g,2t+8..) a3=(g+8,2t+8..)
+  uint32_t phi_[4], plo_[4];
+  split_h2(P[0][0] * inv0, P[0][1] * inv0, phi_[0], plo_[0]);
+  split_h2(P[0][2] * inv1, P[0][3] * inv1, phi_[1], plo_[1]);
+  split_h2(P[1][0] * inv0, P[1][1] * inv0, phi_[2], plo_[2]);
+  split_h2(P[1][2] * inv1, P[1][3] * inv1, phi_[3], plo_[3]);
+#pragma unroll
+  for (int cp = 0; cp < D / 16; ++cp) {
+    uint32_t vr[4];
+    ldsm_x4_t(vaddr(trow, hl * (D / 8) + 2 * cp + csel), vr);
+    if (BF16) {
+#pragma unroll
+      for (int i = 0; i < 4; ++i) { float2 x = unpack2<true>(vr[i]); vr[i] = pack_h2(x.x, x.y); }
+    }
+    // V (transposed) as B operand: n-tile 2cp -> (r0,r2); n-tile 2cp+1 -> (r1,r3)
+#pragma unroll
+    for (int half = 0; half < 2; ++half) {
+      const int nt = 2 * cp + half;
+      float acc[4] = {0.f, 0.f, 0.f, 0.f};
+      mma16816(acc, phi_[0], phi_[1], phi_[2], phi_[3], vr[half], vr[2 + half]);
+      mma16816(acc, plo_[0], plo_[1], plo_[2], plo_[3], vr[half], vr[2 + half]);
+      uint32_t* p0 = reinterpret_cast<uint32_t*>(out_rows + (size_t)g * C_total + 8 * nt + 2 * t);
+      uint32_t* p1 = reinterpret_cast<uint32_t*>(out_rows + (size_t)(g + 8) * C_total + 8 * nt + 2 * t);
+      if (g < nvalid) *p0 = pack_out<BF16>(acc[0], acc[1]);
+      if (g + 8 < nvalid) *p1 = pack_out<BF16>(acc[2], acc[3]);
+    }
+  }
+}
+
+// For two rows at once (independent probes in flight together): the largest w in [0,W) with
+// off[w] <= row (row < off[W] = N), found by one warp with 32-way probes per round.
+__device__ __forceinline__ void warp_windows_of_rows(const int32_t* __restrict__ off, int W, int rowa,
+                                                     int rowb, int& wa, int& wb) {
+  const int lane = threadIdx.x & 31;
+  int lo[2] = {0, 0}, hi[2] = {W, W};
+  const int row[2] = {rowa, rowb};
+  while (hi[0] - lo[0] > 1 || hi[1] - lo[1] > 1) {
+    int step[2], idx[2], val[2];
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      step[k] = max(1, (hi[k] - lo[k] + 31) / 32);
+      idx[k] = lo[k] + (lane + 1) * step[k];
+      val[k] = __ldg(off + min(idx[k], W));
+    }
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const bool ok = idx[k] < hi[k] && val[k] <= row[k];
+      const int cnt = __popc(__ballot_sync(0xffffffffu, ok));
+      const int nlo = lo[k] + cnt * step[k];
+      hi[k] = min(hi[k], nlo + step[k]);
+      lo[k] = nlo;
+    }
+  }
+  wa = lo[0];
+  wb = lo[1];
+}
+
+// ---- host side -------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
+                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                  CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = []() -> EncodeTiledFn {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      return nullptr;
+    return reinterpret_cast<EncodeTiledFn>(p);
+  }();
+  return fn;
+}
+
+// 2-D map over a row-major [N, C] 16-bit tensor; box = 64 columns (128 B) x box_rows, 128-B swizzle.
+bool make_map(CUtensorMap* tm, const void* base, int N, int C, int box_rows) {
+  EncodeTiledFn enc = encode_fn();
+  if (!enc) return false;
+  const cuuint64_t dims[2] = {(cuuint64_t)C, (cuuint64_t)N};
+  const cuuint64_t strides[1] = {(cuuint64_t)C * 2};
+  const cuuint32_t box[2] = {64u, (cuuint32_t)box_rows};
+  const cuuint32_t estr[2] = {1u, 1u};
+  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// Per-device caches (a process may drive several GPUs): index = current CUDA device.
+constexpr int kMaxDevices = 64;
+int current_device() {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) dev = 0;
+  return dev;
+}
+int sm_count() {
+  static std::atomic<int> cache[kMaxDevices];
+  const int dev = current_device();
+  int v = cache[dev].load(std::memory_order_relaxed);
+  if (v <= 0) {
+    v = 148;
+    cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
+    if (v <= 0) v = 148;
+    cache[dev].store(v, std::memory_order_relaxed);
+  }
+  return v;
+}
+
+#endif  // SLA_TC_BASE_INCLUDED
