@@ -1,5 +1,5 @@
 // sla_fwd_umma.cu -- SLA forward on the 5th-generation tensor cores (tcgen05.mma, accumulators in TMEM), all heads
-// of a 128-channel slab at once.  fp16 / bf16 I/O, d_h = 16, H*d_h a multiple of 128.
+// of a 128-channel slab at once.  fp16 I/O, d_h = 16, H*d_h a multiple of 128.
 //
 // What is computed (Eq. 2-3): per window w and head h
 //     S = sum_j phi(k_j)^T v_j,   z = sum_j phi(k_j),   o_i = phi(q_i) S / (phi(q_i) . z).
@@ -9,33 +9,34 @@
 //     (load balance by rows, Fig. 3a).  A CTA owns every window of <= kFuseMax rows whose middle
 //     row lies in its span, and the pieces of longer windows that intersect it (partial state -> fp32 atomics
 //     into the workspace; their outputs come from the OUTPASS launch of sla_fwd_tc.cu).
-//   * A producer warp walks the window offsets and turns them into ITEMS (a descriptor ring in shared memory):
+//   * The walk warp turns the window offsets into ITEMS (a descriptor ring in shared memory):
 //       PACK   consecutive whole windows of <= 16 rows, together <= 16 rows: one packed tile, masked quadratic
 //              form on mma.sync with split operands (quad_tile_core) -- the fp16-operand linear form does not
 //              meet the tolerance on windows this short;
 //       WIN    one window of 17..kFuseMax rows;
 //       PIECE  the part of a longer window inside this span (state only).
-//     For every item it issues 2-D TMA loads (box 64 channels x 16 rows, 128-byte swizzle) of exactly that
-//     item's rows: K,V tiles of 16 rows into a ring, Q blocks of up to 128 rows into block buffers.
-//   * K-group warps apply phi to each K tile IN PLACE (rows past the window end are zeroed: the contraction of
-//     the state MMA runs over rows); the MMA warp then issues, per 16 rows,
+//     Rows travel in CHUNKS of up to 8 tiles of 16 rows (one chunk = one MMA block of up to 128 rows of one
+//     item): the walk warp loads K,V chunks, a second loader warp Q chunks, with 2-D TMA boxes of 64 channels
+//     x 16/32/64/128 rows (128-byte swizzle) into tile rings; a chunk never wraps around its ring.
+//   * phi warps (one whole 16-row tile per warp, tiles dealt round-robin) apply phi to K and Q tiles IN PLACE
+//     (K rows past the window end are zeroed: the contraction of the state MMA runs over rows).
+//   * Two issuer warps then run, per 16 rows and straight from the TMA tiles,
 //         D[r][p]  += sum_j V[j][r] phi(K)[j][p]      tcgen05.mma M=128 N=128 K=16, both operands MN-major,
-//         Z[p][.]  += sum_j phi(K)[j][p] * 1          tcgen05.mma M=128 N=16  K=16 against a tile of ones,
-//     straight from the TMA tiles.  The 16x16 diagonal blocks of D are the per-head states S_h^T; the
-//     off-diagonal blocks (7/8 of the tensor work, ~64 cycles per 16 rows) are ignored.
-//   * When a window's state is complete the K-group reads its diagonal blocks and z from TMEM, scales them by
-//     2^-ceil(log2 m) (Eq. 3 is a ratio) and writes them as fp16 B operands: per head a [16 x 16] K-major tile
-//     (row r = S_h[.][r]) and one [8 x 128] tile of the z_h.
-//   * Q-group warps apply phi to the Q block in place; the MMA warp issues per head
-//         O[i][16h..16h+15] = phi(Q)[i][16h..16h+15] . B_h^T    M=128 N=16 K=16
-//     and the denominators  O[i][128+h] = phi(Q)[i][:] . Bden[h][:]   M=128 N=16 K=128,
-//     into the TMEM columns the state occupied; the Q-group reads its rows back (one thread per row), divides and
-//     stores 32 contiguous bytes per head with 128-bit stores.
-//   * Precision: operands fp16 (bf16 inputs: V is consumed as bf16 by the tensor core, K and Q are converted
-//     when phi is applied), accumulation fp32.
+//         Z[p][.]  += sum_j phi(K)[j][p] * 1          tcgen05.mma M=128 N=16  K=16 against a tile of ones.
+//     The 16x16 diagonal blocks of D are the per-head states S_h^T; the off-diagonal blocks (7/8 of the tensor
+//     work, ~64 cycles per 16 rows) are ignored.
+//   * When a window's state is complete the convert warps read its diagonal blocks and z from TMEM, scale them by
+//     2^-ceil(log2 m) (Eq. 3 is a ratio) and write them as fp16 B operands: per head a [32 x 16] K-major tile,
+//     rows 0..15 = S_h[.][r], row 16 = z_h.
+//   * The output issuer runs per head  O[i][32h..32h+31] = phi(Q)[i][16h..16h+15] . B_h^T  (M=128 N=32 K=16):
+//     columns 32h..32h+15 are the numerators, column 32h+16 the denominator, in the TMEM columns the state
+//     occupied.  Epilogue warps read their rows back (one thread per row), divide, stage the fp16 rows in the
+//     (now dead) Q tiles and store them with fully coalesced 128-bit stores.
+//   * Precision: operands fp16, accumulation fp32.
 #include <cuda.h>
 
 #include <atomic>
+#include <cstdio>
 
 #include "sla_internal.cuh"
 
@@ -46,39 +47,65 @@ namespace {
 
 constexpr int D = 16;                       // head dim of this kernel
 constexpr int HS = 128 / D;                 // heads per 128-channel slab
-constexpr int NKV = 6;                      // K/V tile ring: slots of [K 16x128 | V 16x128] fp16 = 8 KB
-constexpr int NQB = 3;                      // Q block buffers: [128 rows x 128 ch] fp16 = 32 KB
-constexpr int NSL = 3;                      // TMEM regions of 144 columns (state, then output, of one item)
-constexpr int NB = 2;                       // B operand buffers (8 head tiles of 2 KB + 4 KB of z)
-constexpr int NPK = 2;                      // packed-tile slots [K | V | Q] 16 rows each = 12 KB
-constexpr int NIT = 8;                      // item descriptor ring
-constexpr int KG_WARPS = 8, QG_WARPS = 8;
-constexpr int WARP_PROD = 0, WARP_MMA = 1, WARP_KG0 = 2, WARP_QG0 = WARP_KG0 + KG_WARPS;
-constexpr int THREADS = (2 + KG_WARPS + QG_WARPS) * 32;
-constexpr int TILE_BYTES = 4096;            // 16 rows x 128 channels fp16 (two 64-channel boxes of 2 KB)
-constexpr int KV_SLOT = 2 * TILE_BYTES, Q_BUF = 8 * TILE_BYTES, PK_SLOT = 3 * TILE_BYTES;
-constexpr int BH_BYTES = 2048, B_BUF = HS * BH_BYTES + 4096, ONES_BYTES = 2048;
-constexpr int OFF_KV = 0, OFF_Q = OFF_KV + NKV * KV_SLOT, OFF_B = OFF_Q + NQB * Q_BUF,
-              OFF_PK = OFF_B + NB * B_BUF, OFF_ONES = OFF_PK + NPK * PK_SLOT;
-constexpr int SMEM_DYN = OFF_ONES + ONES_BYTES + 1024;      // + alignment slack (swizzle needs 1 KB)
-constexpr int REGION_COLS = 144, TMEM_COLS = 512;
-constexpr int PF_AHEAD = 512, PF_CHUNK = 64;                // L2 prefetch distance / granularity in rows
+constexpr int NKV = 14;                     // K/V tile ring (tiles of 16 rows: K 4 KB + V 4 KB, as four 64-channel box regions)
+constexpr int NQT = 18;                     // Q tile ring (4 KB per tile, as two box regions)
+constexpr int NSL = 2;                      // TMEM regions of 256 columns (state, then output, of one item)
+constexpr int NB = 3;                       // B operand buffers (2 tiles of 4 heads x 32 rows = 8 KB)
+constexpr int NIT = 16;                     // item descriptor ring
+constexpr int KVC = 4;                      // tiles per K/V chunk (Q chunks are MMA blocks of up to 8 tiles)
+constexpr int NPHI = 8, NCONV = 4, NEPI = 8;
+constexpr int WARP_WALK = 0, WARP_QLOAD = 1, WARP_SMMA = 2, WARP_ZMMA = 3, WARP_OMMA = 4, WARP_PHI0 = 5,
+              WARP_CONV0 = WARP_PHI0 + NPHI, WARP_EPI0 = WARP_CONV0 + NCONV, NWARPS = WARP_EPI0 + NEPI;
+constexpr int THREADS = NWARPS * 32;
+constexpr int NREADERS = NWARPS - 1;        // every warp but the walk warp reads the item ring
+constexpr int KV_REG = NKV * 2048, Q_REG = NQT * 2048;          // one 64-channel box region of a ring
+constexpr int B_BUF = 2 * 4096, ONES_BYTES = 2048;
+constexpr int OFF_K = 0, OFF_V = 2 * KV_REG, OFF_Q = 4 * KV_REG, OFF_B = OFF_Q + 2 * Q_REG, OFF_ONES = OFF_B + NB * B_BUF;
+constexpr int SMEM_DYN = OFF_ONES + ONES_BYTES + 1024;          // + alignment slack (swizzle needs 1 KB)
+constexpr int REGION_COLS = 256, TMEM_COLS = 512;
+constexpr int PF_FIRST = 1024, PF_CHUNK = 32;                   // L2 prefetch: rows requested up front / per request
+static_assert(NB * B_BUF >= 7 * 2048, "an M=128 Q block starting at the last ring tile reads 7 tiles past the ring");
+static_assert(NKV <= 32 && NQT <= 32, "one parity bit per ring tile");
+
+#ifdef SLA_DEVEL_TRACE   // development only (never defined in the product build)
+__device__ unsigned long long g_trace[512 * 64];
+__device__ __forceinline__ void trace_at(int slot) {
+  if (blockIdx.x < 512 && slot < 64) {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    g_trace[blockIdx.x * 64 + slot] = t;
+  }
+}
+#define TR(cond, slot) do { if (cond) trace_at(slot); } while (0)
+// fine-grained event log of two CTAs: per warp (lane 0) a private list of (code, id, SM clock); plain stores only
+__device__ int g_log_cta[2] = {40, 10};
+__device__ int4 g_log[2][32][512];
+#define LOG_DECL int lg_n = 0; const int lg_which = (int)blockIdx.x == g_log_cta[0] ? 0 : ((int)blockIdx.x == g_log_cta[1] ? 1 : -1);
+#define LOG(code, id) do { if (lg_which >= 0 && (threadIdx.x & 31) == 0 && lg_n < 511) { \
+    g_log[lg_which][threadIdx.x >> 5][++lg_n] = make_int4(code, id, (int)clock64(), 0); \
+    g_log[lg_which][threadIdx.x >> 5][0].x = lg_n; } } while (0)
+#else
+#define TR(cond, slot) do {} while (0)
+#define LOG_DECL
+#define LOG(code, id) do {} while (0)
+#endif
 
 enum ItemType { IT_END = 0, IT_PACK = 1, IT_WIN = 2, IT_PIECE = 3 };
 
+// Barriers.  Ring barriers are indexed by the FIRST tile of a chunk and complete one phase per use of that index.
 struct Ctrl {
   unsigned long long item_full[NIT], item_empty[NIT];
   unsigned long long kv_full[NKV], kphi[NKV], kv_empty[NKV];
-  unsigned long long q_full[NQB], qphi[NQB], q_empty[NQB];
+  unsigned long long q_full[NQT], qphi[NQT], q_empty[NQT];
   unsigned long long state_full[NSL], region_free[NSL], o_full[NSL], o_drained[NSL];
   unsigned long long b_full[NB], b_empty[NB];
-  unsigned long long pk_full[NPK], pk_empty[NPK];
   int4 items[NIT];
   uint32_t tmem_base;
+  int search_lo;
+  int kv_owner[NKV], q_owner[NQT];         // loader-private: the chunk (first tile) that last used each tile, or -1
 };
 
-// ring cursor: slot index and the parity of the current use of that slot
-struct Cur {
+struct Cur {                                 // ring cursor: slot and the parity of the current use of that slot
   int slot;
   uint32_t phase;
 };
@@ -86,6 +113,23 @@ template <int N>
 __device__ __forceinline__ void advance(Cur& c) {
   if (++c.slot == N) { c.slot = 0; c.phase ^= 1u; }
 }
+// Tile ring with contiguous chunk allocation: a chunk of n tiles never wraps (its tiles are one MMA operand); tiles
+// skipped at the end of the ring are not used in that round.  Every role keeps one parity bit per chunk barrier index.
+template <int N>
+struct TileRing {
+  int pos;
+  uint32_t bits;
+  __device__ __forceinline__ int alloc(int n) {
+    if (pos + n > N) pos = 0;
+    const int first = pos;
+    pos += n;
+    return first;
+  }
+  __device__ __forceinline__ uint32_t parity(int t) const { return (bits >> t) & 1u; }
+  __device__ __forceinline__ void used(int t) { bits ^= 1u << t; }
+};
+
+struct Maps { CUtensorMap m[3][4]; };        // [q, k, v][box rows 16, 32, 64, 128]
 
 // ---- tcgen05 wrappers --------------------------------------------------------------------------------
 // shared-memory matrix descriptor, 128-byte swizzle, Blackwell descriptor version 1
@@ -126,10 +170,6 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
         "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
       : "r"(taddr));
 }
-__device__ __forceinline__ void tmem_ld4(uint32_t taddr, uint32_t (&r)[4]) {
-  asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
-               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(taddr));
-}
 __device__ __forceinline__ void tmem_ld1(uint32_t taddr, uint32_t& r) {
   asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(r) : "r"(taddr));
 }
@@ -148,6 +188,9 @@ __device__ __forceinline__ void l2_prefetch(const void* p, uint32_t bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 // mbarrier wait with a watchdog: a protocol error traps instead of hanging the device
+#ifdef SLA_DEVEL_TRACE
+__device__ int g_abort[8];   // development build: the first wait that times out records itself, every wait then gives up
+#endif
 __device__ __forceinline__ void mbar_wait_wd(uint32_t bar, uint32_t parity) {
   uint32_t done, spins = 0;
   do {
@@ -156,33 +199,79 @@ __device__ __forceinline__ void mbar_wait_wd(uint32_t bar, uint32_t parity) {
         "mbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2, %3;\n\t"
         "selp.b32 %0, 1, 0, P1;\n\t}"
         : "=r"(done) : "r"(bar), "r"(parity), "r"(100000u) : "memory");
+#ifdef SLA_DEVEL_TRACE
+    if (!done) {
+      if (*reinterpret_cast<volatile int*>(&g_abort[0])) return;
+      if (++spins > (1u << 14)) {
+        if (atomicCAS(&g_abort[0], 0, 1) == 0) {
+          g_abort[1] = blockIdx.x; g_abort[2] = threadIdx.x >> 5; g_abort[3] = (int)bar; g_abort[4] = (int)parity;
+          g_abort[5] = threadIdx.x & 31;
+          __threadfence();
+        }
+        return;
+      }
+    }
+#else
     if (!done && ++spins > (1u << 16)) __trap();
+#endif
   } while (!done);
 }
 
-// phi on one 16-byte chunk (8 elements) in place; `keep` = false zeroes it (rows past the window end)
-template <bool BF16>
-__device__ __forceinline__ void phi_chunk(uint32_t addr, bool keep) {
-  uint4 x = lds128(addr);
-  x.x = phi_h2<BF16>(x.x); x.y = phi_h2<BF16>(x.y); x.z = phi_h2<BF16>(x.z); x.w = phi_h2<BF16>(x.w);
-  if (!keep) x = make_uint4(0u, 0u, 0u, 0u);
-  sts128(addr, x);
+__device__ __forceinline__ void mbar_arrive_relaxed(uint32_t bar) {
+  asm volatile("mbarrier.arrive.relaxed.cta.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_n(uint32_t bar, uint32_t n) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(n) : "memory");
 }
 
-// shared address of (row, 16-byte chunk of the 128-channel slab row) in a 16-row tile of two swizzled boxes
-__device__ __forceinline__ uint32_t tile_addr(uint32_t base, int row, int chunk) {
-  return base + (uint32_t)(((chunk >> 3) << 11) + row * 128 + (((chunk & 7) ^ (row & 7)) << 4));
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+      : "r"(taddr));
+}
+
+// phi in place on the 8 sixteen-byte chunks a lane owns of one tile (chunk c at addr[c]); keep_mask bit c = 0 zeroes
+// chunk c (rows past the window end).  All loads are issued before the first use.
+template <bool BF16>
+__device__ __forceinline__ void phi_tile_lane(const uint32_t (&addr)[8], uint32_t keep_mask) {
+  uint4 x[8];
+#pragma unroll
+  for (int c = 0; c < 8; ++c) x[c] = lds128(addr[c]);
+#pragma unroll
+  for (int c = 0; c < 8; ++c) {
+    x[c].x = phi_h2<BF16>(x[c].x); x[c].y = phi_h2<BF16>(x[c].y);
+    x[c].z = phi_h2<BF16>(x[c].z); x[c].w = phi_h2<BF16>(x[c].w);
+    if (!((keep_mask >> c) & 1u)) x[c] = make_uint4(0u, 0u, 0u, 0u);
+    sts128(addr[c], x[c]);
+  }
+}
+// the 8 chunk addresses of a lane in ring tile t (box regions box0, box0 + reg): chunk c -> region c/4, chunk
+// (lane + 32 (c%4)) of the 2 KB box tile, i.e. tile row (lane/8) + 4 (c%4)
+__device__ __forceinline__ void lane_chunks(uint32_t box0, int reg, int t, uint32_t (&addr)[8]) {
+  const uint32_t a = box0 + (uint32_t)(t * 2048 + (threadIdx.x & 31) * 16);
+#pragma unroll
+  for (int c = 0; c < 8; ++c) addr[c] = a + (uint32_t)((c >> 2) * reg + (c & 3) * 512);
+}
+// shared address of (row, 16-byte chunk of the 128-channel slab row) in a 16-row tile whose two swizzled
+// 64-channel boxes start at box0 and box1
+__device__ __forceinline__ uint32_t tile_addr(uint32_t box0, uint32_t box1, int row, int chunk) {
+  return ((chunk >> 3) ? box1 : box0) + (uint32_t)(row * 128 + (((chunk & 7) ^ (row & 7)) << 4));
 }
 
 template <bool BF16, typename T>
 __global__ void __launch_bounds__(THREADS, 1)
-sla_fwd_umma_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
-                    const __grid_constant__ CUtensorMap tmV, const T* __restrict__ qg, const T* __restrict__ kg_,
+sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg, const T* __restrict__ kg_,
                     const T* __restrict__ vg, const int32_t* __restrict__ off, T* __restrict__ out,
                     float* __restrict__ ws, int N, int W, int H, int span) {
   extern __shared__ uint8_t dyn_smem[];
   __shared__ Ctrl ctrl;
   asm volatile("griddepcontrol.launch_dependents;");
+  TR(threadIdx.x == 0, 0);
+#ifdef SLA_DEVEL_TRACE
+  if (threadIdx.x == 0 && blockIdx.x == 0) g_abort[6] = (int)smem_u32(&ctrl);
+#endif
   const uint32_t sbase = (smem_u32(dyn_smem) + 1023u) & ~1023u;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int Ctot = H * D;
@@ -191,38 +280,92 @@ sla_fwd_umma_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
   const int R0 = blockIdx.x * span, R1 = min(R0 + span, N);
 
   // ---- set-up: barriers, TMEM, constant operands -------------------------------------------------------
-  if (threadIdx.x == 0) {
-    for (int i = 0; i < NIT; ++i) { mbar_init(smem_u32(&ctrl.item_full[i]), 1); mbar_init(smem_u32(&ctrl.item_empty[i]), 1 + KG_WARPS + QG_WARPS); }
-    for (int i = 0; i < NKV; ++i) { mbar_init(smem_u32(&ctrl.kv_full[i]), 1); mbar_init(smem_u32(&ctrl.kphi[i]), KG_WARPS); mbar_init(smem_u32(&ctrl.kv_empty[i]), 1); }
-    for (int i = 0; i < NQB; ++i) { mbar_init(smem_u32(&ctrl.q_full[i]), 1); mbar_init(smem_u32(&ctrl.qphi[i]), QG_WARPS); mbar_init(smem_u32(&ctrl.q_empty[i]), 1); }
-    for (int i = 0; i < NSL; ++i) {
-      mbar_init(smem_u32(&ctrl.state_full[i]), 1); mbar_init(smem_u32(&ctrl.region_free[i]), 8);
-      mbar_init(smem_u32(&ctrl.o_full[i]), 1); mbar_init(smem_u32(&ctrl.o_drained[i]), QG_WARPS);
+  {
+    const int t = threadIdx.x;
+    if (t < NIT) { mbar_init(smem_u32(&ctrl.item_full[t]), 1); mbar_init(smem_u32(&ctrl.item_empty[t]), NREADERS); }
+    if (t < NKV) {
+      mbar_init(smem_u32(&ctrl.kv_full[t]), 1); mbar_init(smem_u32(&ctrl.kphi[t]), 8); mbar_init(smem_u32(&ctrl.kv_empty[t]), 2);
+      ctrl.kv_owner[t] = -1;
     }
-    for (int i = 0; i < NB; ++i) { mbar_init(smem_u32(&ctrl.b_full[i]), 4); mbar_init(smem_u32(&ctrl.b_empty[i]), 1); }
-    for (int i = 0; i < NPK; ++i) { mbar_init(smem_u32(&ctrl.pk_full[i]), 1); mbar_init(smem_u32(&ctrl.pk_empty[i]), 8); }
+    if (t < NQT) {
+      mbar_init(smem_u32(&ctrl.q_full[t]), 1); mbar_init(smem_u32(&ctrl.qphi[t]), 8); mbar_init(smem_u32(&ctrl.q_empty[t]), NEPI);
+      ctrl.q_owner[t] = -1;
+    }
+    if (t < NSL) {
+      mbar_init(smem_u32(&ctrl.state_full[t]), 2); mbar_init(smem_u32(&ctrl.region_free[t]), NEPI);
+      mbar_init(smem_u32(&ctrl.o_full[t]), 1); mbar_init(smem_u32(&ctrl.o_drained[t]), NEPI);
+    }
+    if (t < NB) { mbar_init(smem_u32(&ctrl.b_full[t]), NCONV); mbar_init(smem_u32(&ctrl.b_empty[t]), 1); }
+    if (t == 0) ctrl.search_lo = 0;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == WARP_MMA) {
+  if (warp == WARP_SMMA) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&ctrl.tmem_base)), "n"(TMEM_COLS));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
-  // ones tile (B operand of the z MMA) and zeroed z tiles of the B buffers
+  if (warp == WARP_WALK && lane < 12)
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.m[lane >> 2][lane & 3]) : "memory");
+  // ones tile (B operand of the z MMA)
   for (int i = threadIdx.x; i < ONES_BYTES / 16; i += THREADS)
     sts128(sbase + OFF_ONES + i * 16, make_uint4(0x3C003C00u, 0x3C003C00u, 0x3C003C00u, 0x3C003C00u));
-  for (int i = threadIdx.x; i < NB * (4096 / 16); i += THREADS)
-    sts128(sbase + OFF_B + (i / 256) * B_BUF + HS * BH_BYTES + (i % 256) * 16, make_uint4(0u, 0u, 0u, 0u));
   proxy_fence();
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = ctrl.tmem_base;
+  TR(threadIdx.x == 0, 1);
   // nothing a previous kernel of the stream may have written (offsets, tensors, workspace, out) is touched before
   asm volatile("griddepcontrol.wait;" ::: "memory");
+  TR(threadIdx.x == 0, 2);
+  // the rows of this span go to L2 now, in the order they will be needed (whole rows of k, v, q)
+  if (warp == WARP_WALK && lane < 3 && R0 < R1) {
+    const T* base = lane == 0 ? kg_ : (lane == 1 ? vg : qg);
+    const int lo = max(0, R0 - 64), hi = min(N, min(R1 + 128, lo + PF_FIRST));
+    for (int r = lo; r < hi; r += PF_CHUNK)
+      l2_prefetch(base + (size_t)r * Ctot, (uint32_t)(min(PF_CHUNK, hi - r) * Ctot * 2));
+  }
+  // first round of the window search by the whole CTA: the largest probe idx with off[idx] <= R0
+  const int sstep = (W + THREADS - 1) / THREADS;
+  if (R0 < R1) {
+    const long long idx = (long long)(threadIdx.x + 1) * sstep;
+    if (idx < W && __ldg(off + idx) <= R0) atomicMax(&ctrl.search_lo, (int)idx);
+  }
+  __syncthreads();
+  LOG_DECL
 
-  if (warp == WARP_PROD) {
-    // =========================== producer: window walk -> items -> TMA ===========================
-    Cur it{0, 0}, kv{0, 0}, qb{0, 0}, pk{0, 0};
+  // every consumer role reads the item ring in order
+  auto next_item = [&](Cur& it) -> int4 {
+    mbar_wait_wd(smem_u32(&ctrl.item_full[it.slot]), it.phase);
+    const int4 d = ctrl.items[it.slot];
+    __syncwarp();
+    if (lane == 0) mbar_arrive(smem_u32(&ctrl.item_empty[it.slot]));
+    advance<NIT>(it);
+    return d;
+  };
+  // Loader side of a tile ring (lane 0): make tiles [first, first+n) reusable.  A tile is guarded by the empty barrier
+  // of the chunk that last used it (indexed by that chunk's first tile); its parity is that of the index's last use.
+  auto claim_tiles = [&](int* owner, unsigned long long* empty, int ntiles, uint32_t bits, int first, int n) {
+    for (int t = first; t < first + n; ++t) {
+      const int o = owner[t];
+      if (o >= 0) {
+        mbar_wait_wd(smem_u32(&empty[o]), ((bits >> o) & 1u) ^ 1u);
+        for (int u = 0; u < ntiles; ++u)
+          if (owner[u] == o) owner[u] = -1;
+      }
+    }
+    for (int t = first; t < first + n; ++t) owner[t] = first;
+  };
+  // a chunk of n tiles as boxes of 8 / 4 / 2 / 1 tiles: op(map index, first row, first tile)
+  auto for_pieces = [&](int n, int y, int tile, auto&& op) {
+#pragma unroll
+    for (int k = 3; k >= 0; --k)
+      if (n & (1 << k)) { op(k, y, tile); y += 16 << k; tile += 1 << k; }
+  };
+
+  if (warp == WARP_WALK) {
+    // =========================== walk: window offsets -> items; K,V chunk loads ===========================
+    Cur it{0, 0};
+    TileRing<NKV> kr{0, 0u};
     auto emit = [&](int type, int s, int m, int aux) {
       if (lane == 0) {
         mbar_wait_wd(smem_u32(&ctrl.item_empty[it.slot]), it.phase ^ 1u);
@@ -232,12 +375,21 @@ sla_fwd_umma_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
       advance<NIT>(it);
     };
     if (R0 < R1) {
-      int wa, wl;
-      warp_windows_of_rows(off, W, R0, R1 - 1, wa, wl);
-      // L2 prefetch cursor over the rows this CTA is about to load (whole rows of q, k, v)
-      int pf_row = max(0, R0 - 64);
+      // second round of the search: off[lo] <= R0 < off[min(W, lo + sstep)]
+      int lo = ctrl.search_lo, hi = min(W, lo + sstep);
+      while (hi - lo > 1) {
+        const int step = max(1, (hi - lo + 31) / 32);
+        const int idx = lo + (lane + 1) * step;
+        const bool ok = idx < hi && __ldg(off + min(idx, W)) <= R0;
+        const int cnt = __popc(__ballot_sync(0xffffffffu, ok));
+        lo += cnt * step;
+        hi = min(hi, lo + step);
+      }
+      const int wa = lo;
+      TR(lane == 0, 3);
+      int pf_row = min(N, min(R1 + 128, max(0, R0 - 64) + PF_FIRST));
       const int pf_end = min(N, R1 + 128);
-      auto prefetch_to = [&](int row) {
+      auto prefetch_to = [&](int row) {       // rows beyond the first PF_FIRST: requested as the walk advances
         row = min(row, pf_end);
         while (pf_row < row) {
           const int n = min(PF_CHUNK, pf_end - pf_row);
@@ -248,7 +400,6 @@ sla_fwd_umma_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
           pf_row += n;
         }
       };
-      prefetch_to(R0 + PF_AHEAD);
       // window walk with a 32-entry register cache of the offsets
       int wbase = wa;
       int cur = __ldg(off + min(wbase + lane, W));
@@ -264,27 +415,26 @@ sla_fwd_umma_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
         s = __shfl_sync(0xffffffffu, cur, i);
         e = __shfl_sync(0xffffffffu, cur, i + 1);
       };
-      auto load_kv = [&](int y) {   // one K/V tile of 16 rows starting at row y (lane 0)
-        mbar_wait_wd(smem_u32(&ctrl.kv_empty[kv.slot]), kv.phase ^ 1u);
-        const uint32_t bar = smem_u32(&ctrl.kv_full[kv.slot]);
-        const uint32_t dst = sbase + OFF_KV + kv.slot * KV_SLOT;
-        mbar_expect_tx(bar, KV_SLOT);
-        tma_load_2d(dst, &tmK, bar, col0, y);
-        tma_load_2d(dst + 2048, &tmK, bar, col0 + 64, y);
-        tma_load_2d(dst + 4096, &tmV, bar, col0, y);
-        tma_load_2d(dst + 6144, &tmV, bar, col0 + 64, y);
-        advance<NKV>(kv);
-      };
-      auto load_q = [&](int y, int tiles) {   // one Q block: `tiles` tiles of 16 rows starting at row y (lane 0)
-        mbar_wait_wd(smem_u32(&ctrl.q_empty[qb.slot]), qb.phase ^ 1u);
-        const uint32_t bar = smem_u32(&ctrl.q_full[qb.slot]);
-        const uint32_t dst = sbase + OFF_Q + qb.slot * Q_BUF;
-        mbar_expect_tx(bar, (uint32_t)(tiles * TILE_BYTES));
-        for (int j = 0; j < tiles; ++j) {
-          tma_load_2d(dst + j * 2048, &tmQ, bar, col0, y + 16 * j);
-          tma_load_2d(dst + 16384 + j * 2048, &tmQ, bar, col0 + 64, y + 16 * j);
+      auto load_kv = [&](int y, int T16) {   // the K,V tiles of rows [y, y + 16 T16) in chunks of <= KVC tiles
+        for (int c = 0; c * KVC < T16; ++c) {
+          const int n = min(KVC, T16 - KVC * c);
+          const int first = kr.alloc(n);
+          if (lane == 0) {
+            LOG(10, y + 16 * KVC * c);
+            claim_tiles(ctrl.kv_owner, ctrl.kv_empty, NKV, kr.bits, first, n);
+            const uint32_t bar = smem_u32(&ctrl.kv_full[first]);
+            mbar_expect_tx(bar, (uint32_t)(n * 8192));
+            for_pieces(n, y + 16 * KVC * c, first, [&](int mi, int yy, int tile) {
+              const uint32_t dk = sbase + OFF_K + tile * 2048, dv = sbase + OFF_V + tile * 2048;
+              tma_load_2d(dk, &maps.m[1][mi], bar, col0, yy);
+              tma_load_2d(dk + KV_REG, &maps.m[1][mi], bar, col0 + 64, yy);
+              tma_load_2d(dv, &maps.m[2][mi], bar, col0, yy);
+              tma_load_2d(dv + KV_REG, &maps.m[2][mi], bar, col0 + 64, yy);
+            });
+            LOG(11, y + 16 * KVC * c);
+          }
+          kr.used(first);
         }
-        advance<NQB>(qb);
       };
       int w = wa;
       while (w < W) {
@@ -294,7 +444,7 @@ sla_fwd_umma_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
         const int m = e - s;
         if (m <= kFuseMax && s + (m >> 1) >= R1) break;                          // middle beyond the span: a later CTA's
         if (m <= 0 || (m <= kFuseMax && s + (m >> 1) < R0)) { ++w; continue; }   // empty, or an earlier CTA's
-        prefetch_to(min(e, R1) + PF_AHEAD);
+        prefetch_to(min(e, R1) + PF_FIRST / 2);
         if (m <= 16) {
           // pack the following whole short windows (owned, together <= 16 rows) into one tile
           const int i0 = w - wbase;
@@ -308,303 +458,362 @@ sla_fwd_umma_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
           const unsigned starts = __reduce_or_sync(0xffffffffu, startbit) & 0xFFFEu;
           w += cnt;
           emit(IT_PACK, s, rows, (int)starts);
-          if (lane == 0) {
-            mbar_wait_wd(smem_u32(&ctrl.pk_empty[pk.slot]), pk.phase ^ 1u);
-            const uint32_t bar = smem_u32(&ctrl.pk_full[pk.slot]);
-            const uint32_t dst = sbase + OFF_PK + pk.slot * PK_SLOT;
-            mbar_expect_tx(bar, PK_SLOT);
-            tma_load_2d(dst, &tmK, bar, col0, s);
-            tma_load_2d(dst + 2048, &tmK, bar, col0 + 64, s);
-            tma_load_2d(dst + 4096, &tmV, bar, col0, s);
-            tma_load_2d(dst + 6144, &tmV, bar, col0 + 64, s);
-            tma_load_2d(dst + 8192, &tmQ, bar, col0, s);
-            tma_load_2d(dst + 10240, &tmQ, bar, col0 + 64, s);
-          }
-          advance<NPK>(pk);
+          load_kv(s, 1);
           continue;
         }
         if (m <= kFuseMax) {
           emit(IT_WIN, s, m, 0);
-          const int T16 = (m + 15) >> 4;
-          if (lane == 0) {
-            const int first = min(T16, 4);             // a few K/V tiles, then Q (never queued behind a full ring)
-            for (int t = 0; t < first; ++t) load_kv(s + 16 * t);
-            for (int b = 0; b * 8 < T16; ++b) load_q(s + 128 * b, min(8, T16 - 8 * b));
-            for (int t = first; t < T16; ++t) load_kv(s + 16 * t);
-          } else {
-            for (int t = 0; t < T16; ++t) advance<NKV>(kv);
-            for (int b = 0; b * 8 < T16; ++b) advance<NQB>(qb);
-          }
+          load_kv(s, (m + 15) >> 4);
         } else if (ws != nullptr) {   // bounded entry (no workspace): a window that breaks the promise is skipped
           const int ps = max(s, R0), pe = min(e, R1);
           if (lane == 0) reinterpret_cast<volatile int*>(ws)[0] = 1;             // tell the output kernel
           emit(IT_PIECE, ps, pe - ps, s);
-          const int T16 = (pe - ps + 15) >> 4;
-          if (lane == 0) {
-            for (int t = 0; t < T16; ++t) load_kv(ps + 16 * t);
-          } else {
-            for (int t = 0; t < T16; ++t) advance<NKV>(kv);
-          }
+          load_kv(ps, (pe - ps + 15) >> 4);
         }
         ++w;
       }
     }
     emit(IT_END, 0, 0, 0);
-  } else if (warp == WARP_MMA) {
-    // =========================== MMA issuer ===========================
-    Cur it{0, 0}, kv{0, 0}, qb{0, 0}, rg{0, 0}, bb{0, 0};
-    uint32_t od_ph = 0;                                  // parity of the next o_drained completion, per region
+    TR(lane == 0, 4);
+  } else if (warp == WARP_QLOAD) {
+    // =========================== Q chunk loads ===========================
+    Cur it{0, 0};
+    TileRing<NQT> qr{0, 0u};
+    while (true) {
+      const int4 d = next_item(it);
+      if (d.x == IT_END) break;
+      if (d.x == IT_PIECE) continue;
+      const int T16 = d.x == IT_PACK ? 1 : (d.z + 15) >> 4;
+      for (int c = 0; c * 8 < T16; ++c) {
+        const int n = min(8, T16 - 8 * c);
+        const int first = qr.alloc(n);
+        if (lane == 0) {
+          LOG(12, d.y + 128 * c);
+          claim_tiles(ctrl.q_owner, ctrl.q_empty, NQT, qr.bits, first, n);
+          const uint32_t bar = smem_u32(&ctrl.q_full[first]);
+          mbar_expect_tx(bar, (uint32_t)(n * 4096));
+          for_pieces(n, d.y + 128 * c, first, [&](int mi, int yy, int tile) {
+            const uint32_t dq = sbase + OFF_Q + tile * 2048;
+            tma_load_2d(dq, &maps.m[0][mi], bar, col0, yy);
+            tma_load_2d(dq + Q_REG, &maps.m[0][mi], bar, col0 + 64, yy);
+          });
+          LOG(13, d.y + 128 * c);
+        }
+        qr.used(first);
+      }
+    }
+  } else if (warp == WARP_SMMA || warp == WARP_ZMMA) {
+    // =========================== state MMA issuers: D += V^T phi(K)  |  Z += phi(K)^T 1 ===========================
+    const bool zrole = warp == WARP_ZMMA;
+    Cur it{0, 0}, rg{0, 0};
+    TileRing<NKV> kr{0, 0u};
     constexpr uint32_t ID_STATE = make_idesc(128, 128, true, true, BF16, false);   // A = V (I/O dtype), B = phi(K) fp16
     constexpr uint32_t ID_Z = make_idesc(128, 16, true, false, false, false);      // A = phi(K), B = ones
-    constexpr uint32_t ID_OUT = make_idesc(128, 16, false, false, false, false);
-    const uint32_t ones = sbase + OFF_ONES;
+    const uint64_t dones = make_desc(sbase + OFF_ONES, 16, 1024);
+    uint32_t kphi_bits = 0;   // kphi completes a phase only for chunks that pass through the MMA: its own parity bits
     while (true) {
-      mbar_wait_wd(smem_u32(&ctrl.item_full[it.slot]), it.phase);
-      const int4 d = ctrl.items[it.slot];
-      __syncwarp();
-      if (lane == 0) mbar_arrive(smem_u32(&ctrl.item_empty[it.slot]));
-      advance<NIT>(it);
+      const int4 d = next_item(it);
       if (d.x == IT_END) break;
-      if (d.x == IT_PACK) continue;
+      if (d.x == IT_PACK) { kr.alloc(1); continue; }     // a packed tile passes through no MMA: ring position only
       const int T16 = (d.z + 15) >> 4;
       const uint32_t region = tmem + (uint32_t)(rg.slot * REGION_COLS);
       mbar_wait_wd(smem_u32(&ctrl.region_free[rg.slot]), rg.phase ^ 1u);
-      for (int t = 0; t < T16; ++t) {
-        mbar_wait_wd(smem_u32(&ctrl.kphi[kv.slot]), kv.phase);
+      for (int c = 0; c * KVC < T16; ++c) {
+        const int n = min(KVC, T16 - KVC * c);
+        const int first = kr.alloc(n);
+        LOG(20, d.y + 16 * KVC * c);
+        mbar_wait_wd(smem_u32(&ctrl.kphi[first]), (kphi_bits >> first) & 1u);
+        kphi_bits ^= 1u << first;
         tc_fence_after();
+        LOG(21, d.y + 16 * KVC * c);
         if (lane == 0) {
-          const uint32_t ks = sbase + OFF_KV + kv.slot * KV_SLOT;
-          const uint64_t dk = make_desc(ks, 2048, 1024), dv = make_desc(ks + 4096, 2048, 1024);
-          umma(region, dv, dk, ID_STATE, t > 0 ? 1u : 0u);
-          umma(region + 128, dk, make_desc(ones, 16, 1024), ID_Z, t > 0 ? 1u : 0u);
-          umma_commit(smem_u32(&ctrl.kv_empty[kv.slot]));
+          for (int j = 0; j < n; ++j) {
+            const uint32_t kt = sbase + OFF_K + (first + j) * 2048;
+            const uint64_t dk = make_desc(kt, KV_REG, 1024);
+            const uint32_t acc = (c | j) ? 1u : 0u;
+            if (zrole) umma(region + 128, dk, dones, ID_Z, acc);
+            else umma(region, make_desc(kt + (OFF_V - OFF_K), KV_REG, 1024), dk, ID_STATE, acc);
+          }
+          umma_commit(smem_u32(&ctrl.kv_empty[first]));
         }
         __syncwarp();
-        advance<NKV>(kv);
       }
       if (lane == 0) umma_commit(smem_u32(&ctrl.state_full[rg.slot]));
       __syncwarp();
-      if (d.x == IT_WIN) {
-        const uint32_t bbuf = sbase + OFF_B + bb.slot * B_BUF;
-        mbar_wait_wd(smem_u32(&ctrl.b_full[bb.slot]), bb.phase);
-        for (int b = 0; b * 8 < T16; ++b) {
-          mbar_wait_wd(smem_u32(&ctrl.qphi[qb.slot]), qb.phase);
-          if (b > 0) {
-            mbar_wait_wd(smem_u32(&ctrl.o_drained[rg.slot]), (od_ph >> rg.slot) & 1u);
-            od_ph ^= 1u << rg.slot;
-          }
-          tc_fence_after();
-          if (lane == 0) {
-            const uint32_t qs = sbase + OFF_Q + qb.slot * Q_BUF;
-#pragma unroll
-            for (int h = 0; h < HS; ++h)
-              umma(region + 16 * h, make_desc(qs + (h >> 2) * 16384 + (h & 3) * 32, 16, 1024),
-                   make_desc(bbuf + h * BH_BYTES, 16, 1024), ID_OUT, 0u);
-#pragma unroll
-            for (int ks = 0; ks < 8; ++ks)
-              umma(region + 128, make_desc(qs + (ks >> 2) * 16384 + (ks & 3) * 32, 16, 1024),
-                   make_desc(bbuf + HS * BH_BYTES + (ks >> 2) * 2048 + (ks & 3) * 32, 16, 1024), ID_OUT,
-                   ks > 0 ? 1u : 0u);
-            umma_commit(smem_u32(&ctrl.q_empty[qb.slot]));
-            umma_commit(smem_u32(&ctrl.o_full[rg.slot]));
-          }
-          __syncwarp();
-          advance<NQB>(qb);
-        }
-        if (lane == 0) umma_commit(smem_u32(&ctrl.b_empty[bb.slot]));
-        __syncwarp();
-        advance<NB>(bb);
-      }
+      LOG(22, d.y);
       advance<NSL>(rg);
     }
-  } else if (warp < WARP_QG0) {
-    // =========================== K group: phi(K) in place, state -> B operands ===========================
-    const int kgw = warp - WARP_KG0;                     // 0..7
-    const int tid_g = kgw * 32 + lane;                   // 0..255: one 16-byte chunk of a K tile each
-    const int quad = warp & 3;                           // TMEM lane quadrant of this warp
-    Cur it{0, 0}, kv{0, 0}, rg{0, 0}, bb{0, 0}, pk{0, 0};
-    int npack = 0;
+  } else if (warp == WARP_OMMA) {
+    // =========================== output MMA issuer ===========================
+    Cur it{0, 0}, rg{0, 0}, bb{0, 0};
+    TileRing<NQT> qr{0, 0u};
+    uint32_t od_ph = 0;                                  // parity of the next o_drained completion, per region
+    uint32_t qphi_bits = 0;                              // qphi completes a phase only for chunks of WIN items
+    constexpr uint32_t ID_OUT = make_idesc(128, 32, false, false, false, false);
     while (true) {
-      mbar_wait_wd(smem_u32(&ctrl.item_full[it.slot]), it.phase);
-      const int4 d = ctrl.items[it.slot];
+      const int4 d = next_item(it);
+      if (d.x == IT_END) break;
+      if (d.x == IT_PACK) { qr.alloc(1); continue; }
+      if (d.x == IT_PIECE) { advance<NSL>(rg); continue; }
+      const int T16 = (d.z + 15) >> 4;
+      const uint32_t region = tmem + (uint32_t)(rg.slot * REGION_COLS);
+      const uint32_t bbuf = sbase + OFF_B + bb.slot * B_BUF;
+      LOG(30, d.y);
+      mbar_wait_wd(smem_u32(&ctrl.b_full[bb.slot]), bb.phase);
+      LOG(31, d.y);
+      for (int b = 0; b * 8 < T16; ++b) {
+        const int n = min(8, T16 - 8 * b);
+        const int first = qr.alloc(n);
+        mbar_wait_wd(smem_u32(&ctrl.qphi[first]), (qphi_bits >> first) & 1u);
+        qphi_bits ^= 1u << first;
+        if (b > 0) {
+          mbar_wait_wd(smem_u32(&ctrl.o_drained[rg.slot]), (od_ph >> rg.slot) & 1u);
+          od_ph ^= 1u << rg.slot;
+        }
+        tc_fence_after();
+        LOG(32, d.y + 128 * b);
+        if (lane == 0) {
+          const uint32_t qs0 = sbase + OFF_Q + first * 2048;
+#pragma unroll
+          for (int h = 0; h < HS; ++h)
+            umma(region + 32 * h, make_desc(qs0 + (h >> 2) * Q_REG + (h & 3) * 32, 16, 1024),
+                 make_desc(bbuf + (h >> 2) * 4096 + (h & 3) * 32, 16, 1024), ID_OUT, 0u);
+          umma_commit(smem_u32(&ctrl.o_full[rg.slot]));
+        }
+        __syncwarp();
+        LOG(33, d.y + 128 * b);
+      }
+      if (lane == 0) umma_commit(smem_u32(&ctrl.b_empty[bb.slot]));
       __syncwarp();
-      if (lane == 0) mbar_arrive(smem_u32(&ctrl.item_empty[it.slot]));
-      advance<NIT>(it);
+      advance<NB>(bb);
+      advance<NSL>(rg);
+    }
+  } else if (warp < WARP_CONV0) {
+    // =========================== phi warps: all 256 threads on every chunk, one 16-byte chunk of each tile per thread ===========
+    const int pw = warp - WARP_PHI0;
+    const int tid_g = pw * 32 + lane;                    // 16-byte chunk of a 4 KB tile: box region tid_g/128, row (tid_g%128)/8
+    const uint32_t coff = (uint32_t)((tid_g & 127) * 16);
+    const int crow = (tid_g & 127) >> 3;
+    Cur it{0, 0};
+    TileRing<NKV> kr{0, 0u};
+    TileRing<NQT> qr{0, 0u};
+    // phi in place on this thread's chunk of tiles first .. first+n-1 (n <= 4 at a time: the loads go out together)
+    auto phi_chunk = [&](uint32_t base, int first, int n, int row0, int m) {
+      for (int j0 = 0; j0 < n; j0 += 4) {
+        uint4 x[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+          if (j0 + j < n) x[j] = lds128(base + (first + j0 + j) * 2048 + coff);
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+          if (j0 + j < n) {
+            x[j].x = phi_h2<BF16>(x[j].x); x[j].y = phi_h2<BF16>(x[j].y);
+            x[j].z = phi_h2<BF16>(x[j].z); x[j].w = phi_h2<BF16>(x[j].w);
+            if (row0 + 16 * (j0 + j) + crow >= m) x[j] = make_uint4(0u, 0u, 0u, 0u);   // rows past the window end
+            sts128(base + (first + j0 + j) * 2048 + coff, x[j]);
+          }
+      }
+    };
+    while (true) {
+      const int4 d = next_item(it);
       if (d.x == IT_END) break;
       if (d.x == IT_PACK) {
-        if ((npack++ & 1) == 0) {                        // even packed tiles: this group; odd: the Q group
-          mbar_wait_wd(smem_u32(&ctrl.pk_full[pk.slot]), pk.phase);
-          const uint32_t pb = sbase + OFF_PK + pk.slot * PK_SLOT;
-          const int wid = (lane < d.z) ? __popc((unsigned)d.w & ((2u << lane) - 1u)) : -1;
-          if (kgw < HS)
-            quad_tile_core<D, BF16, T>([&](int r, int c) { return tile_addr(pb + 8192, r, c); },
-                                       [&](int r, int c) { return tile_addr(pb, r, c); },
-                                       [&](int r, int c) { return tile_addr(pb + 4096, r, c); }, kgw, d.z, wid,
-                                       out + (size_t)d.y * Ctot + col0 + kgw * D, Ctot);
-          __syncwarp();
-          if (lane == 0) mbar_arrive(smem_u32(&ctrl.pk_empty[pk.slot]));
+        const int kt = kr.alloc(1), qt = qr.alloc(1);
+        mbar_wait_wd(smem_u32(&ctrl.kv_full[kt]), kr.parity(kt));
+        mbar_wait_wd(smem_u32(&ctrl.q_full[qt]), qr.parity(qt));
+        const uint32_t kb = sbase + OFF_K + kt * 2048, vb = sbase + OFF_V + kt * 2048, qb = sbase + OFF_Q + qt * 2048;
+        const int wid = (lane < d.z) ? __popc((unsigned)d.w & ((2u << lane) - 1u)) : -1;
+        if (pw < HS)                                     // warp pw = head pw of the slab
+          quad_tile_core<D, BF16, T>([&](int r, int c) { return tile_addr(qb, qb + Q_REG, r, c); },
+                                     [&](int r, int c) { return tile_addr(kb, kb + KV_REG, r, c); },
+                                     [&](int r, int c) { return tile_addr(vb, vb + KV_REG, r, c); }, pw, d.z, wid,
+                                     out + (size_t)d.y * Ctot + col0 + pw * D, Ctot);
+        asm volatile("bar.sync 1, %0;" ::"n"(NPHI * 32) : "memory");   // every head is done with the tiles
+        if (tid_g == 0) {
+          mbar_arrive_n(smem_u32(&ctrl.kv_empty[kt]), 2);
+          mbar_arrive_n(smem_u32(&ctrl.q_empty[qt]), NEPI);
         }
-        advance<NPK>(pk);
+        kr.used(kt);
+        qr.used(qt);
         continue;
       }
       const int m = d.z, T16 = (m + 15) >> 4;
-      for (int t = 0; t < T16; ++t) {
-        mbar_wait_wd(smem_u32(&ctrl.kv_full[kv.slot]), kv.phase);
-        const int row = (tid_g & 127) >> 3;
-        phi_chunk<BF16>(sbase + OFF_KV + kv.slot * KV_SLOT + tid_g * 16, 16 * t + row < m);
+      for (int c = 0; c * KVC < T16; ++c) {
+        const int n = min(KVC, T16 - KVC * c);
+        const int first = kr.alloc(n);
+        LOG(40, d.y + 16 * KVC * c);
+        mbar_wait_wd(smem_u32(&ctrl.kv_full[first]), kr.parity(first));
+        LOG(41, d.y + 16 * KVC * c);
+        phi_chunk(sbase + OFF_K + (tid_g >> 7) * KV_REG, first, n, 16 * KVC * c, m);
         proxy_fence();
         __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&ctrl.kphi[kv.slot]));
-        advance<NKV>(kv);
-      }
-      // the state of this item is complete when the MMA warp's commit lands
-      const uint32_t region = tmem + (uint32_t)(rg.slot * REGION_COLS);
-      if (kgw < 4) {
-        mbar_wait_wd(smem_u32(&ctrl.state_full[rg.slot]), rg.phase);
-        tc_fence_after();
-        uint32_t v[32], zr;
-        const uint32_t lane_base = (uint32_t)(32 * quad) << 16;
-        tmem_ld32(region + lane_base + 32 * quad, v);     // columns 32q..32q+31: the diagonal blocks of heads 2q, 2q+1
-        tmem_ld1(region + lane_base + 128, zr);
-        tmem_wait_ld();
-        const int h = 2 * quad + (lane >> 4), r = lane & 15;   // this lane = channel (h, r) of the slab
-        float x[16];
-#pragma unroll
-        for (int p = 0; p < 16; ++p) x[p] = __uint_as_float((lane & 16) ? v[16 + p] : v[p]);   // S_h[p][r]
-        const float zv = __uint_as_float(zr);                                                   // z_h[r]
-        if (d.x == IT_WIN) {
-          const int lg = 32 - __clz(m - 1);
-          const float scale = __int_as_float((127 - lg) << 23);   // 2^-ceil(log2 m): fp16 operands stay O(1)
-          mbar_wait_wd(smem_u32(&ctrl.b_empty[bb.slot]), bb.phase ^ 1u);
-          const uint32_t bbuf = sbase + OFF_B + bb.slot * B_BUF;
-          uint4 c0, c1;
-          c0.x = pack_h2(x[0] * scale, x[1] * scale);   c0.y = pack_h2(x[2] * scale, x[3] * scale);
-          c0.z = pack_h2(x[4] * scale, x[5] * scale);   c0.w = pack_h2(x[6] * scale, x[7] * scale);
-          c1.x = pack_h2(x[8] * scale, x[9] * scale);   c1.y = pack_h2(x[10] * scale, x[11] * scale);
-          c1.z = pack_h2(x[12] * scale, x[13] * scale); c1.w = pack_h2(x[14] * scale, x[15] * scale);
-          const uint32_t rowa = bbuf + h * BH_BYTES + r * 128;
-          sts128(rowa + ((0 ^ (r & 7)) << 4), c0);        // B_h[n = r][k = 0..7]
-          sts128(rowa + ((1 ^ (r & 7)) << 4), c1);        // B_h[n = r][k = 8..15]
-          // Bden[n = h][k = 16h + r] = z_h[r]
-          const __half zh = __float2half_rn(zv * scale);
-          sts16(bbuf + HS * BH_BYTES + (h >> 2) * 2048 + h * 128 + (((2 * (h & 3) + (r >> 3)) ^ (h & 7)) << 4) + (r & 7) * 2,
-                __half_as_ushort(zh));
-          proxy_fence();
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(smem_u32(&ctrl.b_full[bb.slot]));
-        } else {
-          // piece of a long window: partial state -> workspace slot of the window (fp32 atomics)
-          float* slot = ws + kWsHeaderFloats +
-                        ((size_t)(d.w / (kFuseMax + 1)) * H + (h0 + h)) * (size_t)((D + 1) * D);
-#pragma unroll
-          for (int p = 0; p < 16; ++p) atomicAdd(slot + p * D + r, x[p]);
-          atomicAdd(slot + D * D + r, zv);
-          tc_fence_before();
-        }
+        if (lane == 0) mbar_arrive(smem_u32(&ctrl.kphi[first]));
+        LOG(42, d.y + 16 * KVC * c);
+        kr.used(first);
       }
       if (d.x == IT_WIN) {
+        for (int b = 0; b * 8 < T16; ++b) {
+          const int n = min(8, T16 - 8 * b);
+          const int first = qr.alloc(n);
+          LOG(43, d.y + 128 * b);
+          mbar_wait_wd(smem_u32(&ctrl.q_full[first]), qr.parity(first));
+          LOG(44, d.y + 128 * b);
+          phi_chunk(sbase + OFF_Q + (tid_g >> 7) * Q_REG, first, n, 0, 1 << 30);
+          proxy_fence();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(smem_u32(&ctrl.qphi[first]));
+          LOG(45, d.y + 128 * b);
+          qr.used(first);
+        }
+      }
+    }
+  } else if (warp < WARP_EPI0) {
+    // =========================== state -> B operands (or workspace atomics for pieces) ===========================
+    const int quad = warp & 3;                           // TMEM lane quadrant of this warp
+    Cur it{0, 0}, rg{0, 0}, bb{0, 0};
+    while (true) {
+      const int4 d = next_item(it);
+      if (d.x == IT_END) break;
+      if (d.x == IT_PACK) continue;
+      const int m = d.z;
+      const uint32_t region = tmem + (uint32_t)(rg.slot * REGION_COLS);
+      LOG(50, d.y);
+      mbar_wait_wd(smem_u32(&ctrl.state_full[rg.slot]), rg.phase);
+      tc_fence_after();
+      LOG(51, d.y);
+      uint32_t v[32], zr;
+      const uint32_t lane_base = (uint32_t)(32 * quad) << 16;
+      tmem_ld32(region + lane_base + 32 * quad, v);       // columns 32q..32q+31: the diagonal blocks of heads 2q, 2q+1
+      tmem_ld1(region + lane_base + 128, zr);
+      tmem_wait_ld();
+      LOG(53, 0);
+      const int h = 2 * quad + (lane >> 4), r = lane & 15;     // this lane = channel (h, r) of the slab
+      float x[16];
+#pragma unroll
+      for (int p = 0; p < 16; ++p) x[p] = __uint_as_float((lane & 16) ? v[16 + p] : v[p]);   // S_h[p][r]
+      const float zv = __uint_as_float(zr);                                                   // z_h[r]
+      if (d.x == IT_WIN) {
+        const int lg = 32 - __clz(m - 1);
+        const float scale = __int_as_float((127 - lg) << 23);   // 2^-ceil(log2 m): fp16 operands stay O(1)
+        mbar_wait_wd(smem_u32(&ctrl.b_empty[bb.slot]), bb.phase ^ 1u);
+        LOG(54, 0);
+        uint4 c0, c1;
+        c0.x = pack_h2(x[0] * scale, x[1] * scale);   c0.y = pack_h2(x[2] * scale, x[3] * scale);
+        c0.z = pack_h2(x[4] * scale, x[5] * scale);   c0.w = pack_h2(x[6] * scale, x[7] * scale);
+        c1.x = pack_h2(x[8] * scale, x[9] * scale);   c1.y = pack_h2(x[10] * scale, x[11] * scale);
+        c1.z = pack_h2(x[12] * scale, x[13] * scale); c1.w = pack_h2(x[14] * scale, x[15] * scale);
+        // B tile of heads 4g..4g+3 ([32 rows x 64 k], K-major, 128-byte swizzle): head h at k = 16 (h & 3) .. +15;
+        // row n = r < 16 holds S_h[.][r], row 16 holds z_h
+        const uint32_t tile = sbase + OFF_B + bb.slot * B_BUF + (h >> 2) * 4096;
+        const int lc = 2 * (h & 3);                       // first logical 16-byte chunk of the head
+        sts128(tile + r * 128 + ((lc ^ (r & 7)) << 4), c0);
+        sts128(tile + r * 128 + (((lc + 1) ^ (r & 7)) << 4), c1);
+        sts16(tile + 16 * 128 + ((lc + (r >> 3)) << 4) + (r & 7) * 2, __half_as_ushort(__float2half_rn(zv * scale)));
+        LOG(55, 0);
+        proxy_fence();
+        tc_fence_before();
+        __syncwarp();
+        LOG(56, 0);
+        if (lane == 0) mbar_arrive(smem_u32(&ctrl.b_full[bb.slot]));
         advance<NB>(bb);
       } else {
+        // piece of a long window: partial state -> workspace slot of the window (fp32 atomics)
+        float* slot = ws + kWsHeaderFloats + ((size_t)(d.w / (kFuseMax + 1)) * H + (h0 + h)) * (size_t)((D + 1) * D);
+#pragma unroll
+        for (int p = 0; p < 16; ++p) atomicAdd(slot + p * D + r, x[p]);
+        atomicAdd(slot + D * D + r, zv);
+        tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&ctrl.region_free[rg.slot]));   // all 8 K warps: the region is free again
+        if (lane == 0) mbar_arrive_n(smem_u32(&ctrl.region_free[rg.slot]), NEPI / NCONV);
       }
+      LOG(52, d.y);
       advance<NSL>(rg);
     }
   } else {
-    // =========================== Q group: phi(Q) in place, epilogue ===========================
-    const int qgw = warp - WARP_QG0;                     // 0..7
-    const int tid_g = qgw * 32 + lane;
-    const int quad = warp & 3, half = qgw >> 2;          // TMEM lane quadrant; which 4 heads this warp stores
-    Cur it{0, 0}, qb{0, 0}, rg{0, 0}, pk{0, 0};
+    // =========================== epilogue: one thread per output row ===========================
+    const int ew = warp - WARP_EPI0;
+    const int quad = warp & 3, half = ew >> 2;           // TMEM lane quadrant; which 4 heads (64 channels) this warp stores
+    Cur it{0, 0}, rg{0, 0};
+    TileRing<NQT> qr{0, 0u};
     uint32_t of_ph = 0;                                  // parity of the next o_full completion, per region
-    int npack = 0;
+    const uint32_t stage0 = sbase + OFF_Q + half * Q_REG;   // this warp stages its rows in its half of the dead Q tiles
     while (true) {
-      mbar_wait_wd(smem_u32(&ctrl.item_full[it.slot]), it.phase);
-      const int4 d = ctrl.items[it.slot];
-      __syncwarp();
-      if (lane == 0) mbar_arrive(smem_u32(&ctrl.item_empty[it.slot]));
-      advance<NIT>(it);
+      const int4 d = next_item(it);
       if (d.x == IT_END) break;
-      if (d.x == IT_PACK) {
-        if ((npack++ & 1) == 1) {
-          mbar_wait_wd(smem_u32(&ctrl.pk_full[pk.slot]), pk.phase);
-          const uint32_t pb = sbase + OFF_PK + pk.slot * PK_SLOT;
-          const int wid = (lane < d.z) ? __popc((unsigned)d.w & ((2u << lane) - 1u)) : -1;
-          if (qgw < HS)
-            quad_tile_core<D, BF16, T>([&](int r, int c) { return tile_addr(pb + 8192, r, c); },
-                                       [&](int r, int c) { return tile_addr(pb, r, c); },
-                                       [&](int r, int c) { return tile_addr(pb + 4096, r, c); }, qgw, d.z, wid,
-                                       out + (size_t)d.y * Ctot + col0 + qgw * D, Ctot);
-          __syncwarp();
-          if (lane == 0) mbar_arrive(smem_u32(&ctrl.pk_empty[pk.slot]));
-        }
-        advance<NPK>(pk);
-        continue;
-      }
+      if (d.x == IT_PACK) { qr.alloc(1); continue; }
       if (d.x == IT_PIECE) { advance<NSL>(rg); continue; }
-      const int s = d.y, m = d.z, T16 = (m + 15) >> 4;
-      const int nblk = (T16 + 7) >> 3;
-      for (int b = 0; b < nblk; ++b) {
-        const int tiles = min(8, T16 - 8 * b);
-        mbar_wait_wd(smem_u32(&ctrl.q_full[qb.slot]), qb.phase);
-        const uint32_t a0 = sbase + OFF_Q + qb.slot * Q_BUF + (tid_g >> 7) * 16384 + (tid_g & 127) * 16;
-        int j = 0;
-        for (; j + 1 < tiles; j += 2) {
-          phi_chunk<BF16>(a0 + j * 2048, true);
-          phi_chunk<BF16>(a0 + (j + 1) * 2048, true);
-        }
-        if (j < tiles) phi_chunk<BF16>(a0 + j * 2048, true);
-        proxy_fence();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&ctrl.qphi[qb.slot]));
-        advance<NQB>(qb);
-      }
+      const int s = d.y, m = d.z;
+      const int T16 = (m + 15) >> 4;
       const uint32_t region = tmem + (uint32_t)(rg.slot * REGION_COLS);
-      for (int b = 0; b < nblk; ++b) {
+      for (int b = 0; b * 8 < T16; ++b) {
+        const int first = qr.alloc(min(8, T16 - 8 * b));
         const int rows = min(128, m - 128 * b);          // valid rows of this block
+        LOG(60, s + 128 * b);
         mbar_wait_wd(smem_u32(&ctrl.o_full[rg.slot]), (of_ph >> rg.slot) & 1u);
         of_ph ^= 1u << rg.slot;
         tc_fence_after();
+        LOG(61, s + 128 * b);
         if (32 * quad < rows) {
-          const uint32_t taddr = region + ((uint32_t)(32 * quad) << 16);
-          uint32_t dn[4];
-          tmem_ld4(taddr + 128 + 4 * half, dn);
+          const uint32_t taddr = region + ((uint32_t)(32 * quad) << 16) + 128 * half;
           const int rib = 32 * quad + lane;              // row of the block this thread owns
-          T* orow = out + (size_t)(s + 128 * b + rib) * Ctot + col0 + 64 * half;
+          const uint32_t srow = stage0 + (first + (rib >> 4)) * 2048 + (rib & 15) * 128;
 #pragma unroll
-          for (int hp = 0; hp < 2; ++hp) {               // two heads per 32-column load
-            uint32_t v[32];
-            tmem_ld32(taddr + 64 * half + 32 * hp, v);
+          for (int hp = 0; hp < 2; ++hp) {               // two heads at a time
+            uint32_t va[16], vb[16], da, db;
+            tmem_ld16(taddr + 64 * hp, va);
+            tmem_ld1(taddr + 64 * hp + 16, da);
+            tmem_ld16(taddr + 64 * hp + 32, vb);
+            tmem_ld1(taddr + 64 * hp + 48, db);
             tmem_wait_ld();
-            const float i0 = fast_rcp(__uint_as_float(dn[2 * hp])), i1 = fast_rcp(__uint_as_float(dn[2 * hp + 1]));
+            LOG(63, hp);
+            const float ia = fast_rcp(__uint_as_float(da)), ib = fast_rcp(__uint_as_float(db));
+            uint4 o[4];
+#pragma unroll
+            for (int c = 0; c < 2; ++c) {
+              o[c].x = pack_out<BF16>(__uint_as_float(va[8 * c + 0]) * ia, __uint_as_float(va[8 * c + 1]) * ia);
+              o[c].y = pack_out<BF16>(__uint_as_float(va[8 * c + 2]) * ia, __uint_as_float(va[8 * c + 3]) * ia);
+              o[c].z = pack_out<BF16>(__uint_as_float(va[8 * c + 4]) * ia, __uint_as_float(va[8 * c + 5]) * ia);
+              o[c].w = pack_out<BF16>(__uint_as_float(va[8 * c + 6]) * ia, __uint_as_float(va[8 * c + 7]) * ia);
+              o[2 + c].x = pack_out<BF16>(__uint_as_float(vb[8 * c + 0]) * ib, __uint_as_float(vb[8 * c + 1]) * ib);
+              o[2 + c].y = pack_out<BF16>(__uint_as_float(vb[8 * c + 2]) * ib, __uint_as_float(vb[8 * c + 3]) * ib);
+              o[2 + c].z = pack_out<BF16>(__uint_as_float(vb[8 * c + 4]) * ib, __uint_as_float(vb[8 * c + 5]) * ib);
+              o[2 + c].w = pack_out<BF16>(__uint_as_float(vb[8 * c + 6]) * ib, __uint_as_float(vb[8 * c + 7]) * ib);
+            }
             if (rib < rows) {
-              uint4 o0, o1, o2, o3;
-              o0.x = pack_out<BF16>(__uint_as_float(v[0]) * i0, __uint_as_float(v[1]) * i0);
-              o0.y = pack_out<BF16>(__uint_as_float(v[2]) * i0, __uint_as_float(v[3]) * i0);
-              o0.z = pack_out<BF16>(__uint_as_float(v[4]) * i0, __uint_as_float(v[5]) * i0);
-              o0.w = pack_out<BF16>(__uint_as_float(v[6]) * i0, __uint_as_float(v[7]) * i0);
-              o1.x = pack_out<BF16>(__uint_as_float(v[8]) * i0, __uint_as_float(v[9]) * i0);
-              o1.y = pack_out<BF16>(__uint_as_float(v[10]) * i0, __uint_as_float(v[11]) * i0);
-              o1.z = pack_out<BF16>(__uint_as_float(v[12]) * i0, __uint_as_float(v[13]) * i0);
-              o1.w = pack_out<BF16>(__uint_as_float(v[14]) * i0, __uint_as_float(v[15]) * i0);
-              o2.x = pack_out<BF16>(__uint_as_float(v[16]) * i1, __uint_as_float(v[17]) * i1);
-              o2.y = pack_out<BF16>(__uint_as_float(v[18]) * i1, __uint_as_float(v[19]) * i1);
-              o2.z = pack_out<BF16>(__uint_as_float(v[20]) * i1, __uint_as_float(v[21]) * i1);
-              o2.w = pack_out<BF16>(__uint_as_float(v[22]) * i1, __uint_as_float(v[23]) * i1);
-              o3.x = pack_out<BF16>(__uint_as_float(v[24]) * i1, __uint_as_float(v[25]) * i1);
-              o3.y = pack_out<BF16>(__uint_as_float(v[26]) * i1, __uint_as_float(v[27]) * i1);
-              o3.z = pack_out<BF16>(__uint_as_float(v[28]) * i1, __uint_as_float(v[29]) * i1);
-              o3.w = pack_out<BF16>(__uint_as_float(v[30]) * i1, __uint_as_float(v[31]) * i1);
-              uint4* op = reinterpret_cast<uint4*>(orow + 32 * hp);
-              op[0] = o0; op[1] = o1; op[2] = o2; op[3] = o3;
+#pragma unroll
+              for (int c = 0; c < 4; ++c) sts128(srow + (((4 * hp + c) ^ (rib & 7)) << 4), o[c]);
             }
           }
+          __syncwarp();
+          LOG(64, 0);
+          // coalesced copy-out: per instruction 4 rows x 128 bytes (lane -> row 4 it + lane/8, chunk lane%8)
+          const int nr = min(32, rows - 32 * quad);
+          T* obase = out + (size_t)(s + 128 * b + 32 * quad) * Ctot + col0 + 64 * half + (lane & 7) * 8;
+          uint4 x[8];
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const int row = 4 * i + (lane >> 3), rb = 32 * quad + row;
+            if (row < nr)
+              x[i] = lds128(stage0 + (first + (rb >> 4)) * 2048 + (rb & 15) * 128 + (((lane & 7) ^ (rb & 7)) << 4));
+          }
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const int row = 4 * i + (lane >> 3);
+            if (row < nr) *reinterpret_cast<uint4*>(obase + (size_t)row * Ctot) = x[i];
+          }
+          LOG(65, 0);
+          proxy_fence();
+          LOG(66, 0);                                 // the tiles go back to the TMA loader
         }
         tc_fence_before();
         __syncwarp();
-        if (lane == 0)
-          mbar_arrive(smem_u32(b + 1 < nblk ? &ctrl.o_drained[rg.slot] : &ctrl.region_free[rg.slot]));
+        if (lane == 0) {
+          // relaxed: what these arrivals publish (TMEM reads, shared-memory reads of the staging tiles) is complete;
+          // a releasing arrive would also wait for the global stores above to be acknowledged
+          mbar_arrive_relaxed(smem_u32(&ctrl.q_empty[first]));
+          mbar_arrive_relaxed(smem_u32((b + 1) * 8 < T16 ? &ctrl.o_drained[rg.slot] : &ctrl.region_free[rg.slot]));
+        }
+        LOG(62, s + 128 * b);
       }
       advance<NSL>(rg);
     }
@@ -613,19 +822,21 @@ sla_fwd_umma_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
   // ---- teardown ---------------------------------------------------------------------------------------
   tc_fence_before();
   __syncthreads();
-  if (warp == WARP_MMA) {
+  TR(threadIdx.x == 0, 5);
+  if (warp == WARP_SMMA) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(TMEM_COLS));
   }
 }
 
-// 2-D map over a row-major [N, C] 16-bit tensor; box = 64 columns (128 B) x 16 rows, 128-byte swizzle
 template <bool BF16, typename T>
 cudaError_t umma_launch(const Problem& p, cudaStream_t st) {
-  CUtensorMap tq, tk, tv;
+  Maps maps;
   const int Ctot = p.H * D;
-  if (!make_map(&tq, p.q, p.N, Ctot, 16) || !make_map(&tk, p.k, p.N, Ctot, 16) || !make_map(&tv, p.v, p.N, Ctot, 16))
-    return cudaErrorInvalidValue;
+  const void* base[3] = {p.q, p.k, p.v};
+  for (int t = 0; t < 3; ++t)
+    for (int k = 0; k < 4; ++k)
+      if (!make_map(&maps.m[t][k], base[t], p.N, Ctot, 16 << k)) return cudaErrorInvalidValue;
   auto kern = sla_fwd_umma_kernel<BF16, T>;
   static std::atomic<bool> attr_set[kMaxDevices];         // the smem opt-in is per device
   const int dev = current_device();
@@ -650,11 +861,32 @@ cudaError_t umma_launch(const Problem& p, cudaStream_t st) {
   cfg.stream = st;
   cfg.attrs = pdl;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, kern, tq, tk, tv, (const T*)p.q, (const T*)p.k, (const T*)p.v, p.off, (T*)p.out,
+  return cudaLaunchKernelEx(&cfg, kern, maps, (const T*)p.q, (const T*)p.k, (const T*)p.v, p.off, (T*)p.out,
                             p.ws_state, p.N, p.W, p.H, span);
 }
 
 }  // namespace
+
+#ifdef SLA_DEVEL_TRACE
+extern "C" int sla_debug_read_trace(unsigned long long* host, int n) {
+  return (int)cudaMemcpyFromSymbol(host, g_trace, sizeof(unsigned long long) * n);
+}
+extern "C" int sla_debug_read_log(int* host_int4, int cta0, int cta1) {   // host: 2*32*512 int4; then re-arms
+  cudaError_t e = cudaMemcpyFromSymbol(host_int4, g_log, sizeof(int4) * 2 * 32 * 512);
+  void* p = nullptr;
+  cudaGetSymbolAddress(&p, g_log);
+  cudaMemset(p, 0, sizeof(int4) * 2 * 32 * 512);
+  int c[2] = {cta0, cta1};
+  cudaMemcpyToSymbol(g_log_cta, c, sizeof(c));
+  return (int)e;
+}
+extern "C" int sla_debug_read_abort(int* host) {   // host[0..7]; also clears the flag
+  cudaError_t e = cudaMemcpyFromSymbol(host, g_abort, sizeof(int) * 8);
+  int z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  cudaMemcpyToSymbol(g_abort, z, sizeof(z));
+  return (int)e;
+}
+#endif
 
 bool forward_umma_supported(const Problem& p, int dt) {
   if (dt != SLA_F16) return false;
@@ -664,7 +896,11 @@ bool forward_umma_supported(const Problem& p, int dt) {
 
 cudaError_t launch_forward_umma_main(const Problem& p, int dt, cudaStream_t st) {
   (void)dt;
-  return umma_launch<false, __half>(p, st);
+  cudaError_t e = umma_launch<false, __half>(p, st);
+#ifdef SLA_DEVEL_TRACE
+  if (e != cudaSuccess) fprintf(stderr, "umma_launch: %s\n", cudaGetErrorString(e));
+#endif
+  return e;
 }
 
 }  // namespace sla
