@@ -43,8 +43,8 @@ def parse_args():
                     help="skip the extra legs (config-4 training step, batch-size sweep) of the default run")
     ap.add_argument("--launch", default="graph", choices=["graph", "eager"],
                     help="timed region replays CUDA graphs captured from the C-ABI calls (default) or calls eagerly")
-    ap.add_argument("--entry", default="bounded", choices=["bounded", "general"],
-                    help="sla_forward_bounded(max_window_len=144) for the 12x12-window configs, or sla_forward")
+    ap.add_argument("--entry", default="general", choices=["general", "bounded"],
+                    help="sla_forward (the entry north_star names; default) or sla_forward_bounded(max_window_len=144)")
     return ap.parse_args()
 
 
@@ -462,6 +462,36 @@ def run_ours(args):
         e1.record(side)
         torch.cuda.synchronize()
         fwd_general_eager_ms = e0.elapsed_time(e1) / args.steps
+
+        def graph_leg(call):
+            """us per call of `call(set_index)`: one graph per rotating set, replayed back to back (cold L2)."""
+            if not use_graph:
+                return None
+            gl = []
+            for r in range(R):
+                call(r)
+                gg = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(gg, stream=side):
+                    call(r)
+                gl.append(gg)
+            for r in range(R):
+                gl[r].replay()
+            torch.cuda.synchronize()
+            e0.record(side)
+            for i in range(args.steps):
+                gl[i % R].replay()
+            e1.record(side)
+            torch.cuda.synchronize()
+            return e0.elapsed_time(e1) / args.steps * 1e3
+
+        # the other forward entries on the same sets under the same protocol
+        us_bounded = us_tcgen05 = None
+        if max_len <= 144:
+            us_bounded = graph_leg(lambda r: pkg.sla_forward(*sets[r][:3], off, out=sets[r][3], stream=side,
+                                                             max_window_len=144))
+        if sc.dtype == "f16" and d == 16 and (H * d) % 128 == 0:
+            us_tcgen05 = graph_leg(lambda r: pkg.sla_forward(*sets[r][:3], off, out=sets[r][3], workspace=ws,
+                                                             stream=side, tcgen05=True))
         # the whole step, one event pair per step (a spin kernel first so the host runs ahead): spread
         sev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
                for _ in range(args.steps)]
@@ -535,7 +565,7 @@ def run_ours(args):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 3 * tensor_bytes + 4 * N,
                 "d2h_bytes_per_step": tensor_bytes, "ms_per_step": e2e_s * 1e3,
                 "api": "sla_forward_host (pinned host buffers)"},
-        "gpu_launches": args.steps * (2 if bounded else 3),   # prep + forward kernel(s); memset not counted
+        "gpu_launches": args.steps * (2 if bounded else 4),   # prep + (zero +) forward kernel (+ split-window pass)
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": traffic if args.config == 1 else None,
                      "traffic_source": traffic_src if args.config == 1 else None, "peak_source": peak_src,
@@ -543,11 +573,12 @@ def run_ours(args):
                      "ceiling": "sla_bench_stream_ceiling: 128-bit loads of q,k,v + store of out (3:1 mix), same "
                                 "rotating cold sets, same event protocol as us_per_launch",
                      "kernel": "sla_fwd_tc_kernel (the single launch of sla_forward_bounded)" if bounded
-                               else "sla_forward (all launches of one call)",
+                               else "sla_forward: sla_zero_kernel + sla_fwd_tc_kernel + its split-window pass (all launches of one call)",
                      "algorithmic_bytes": alg_bytes, "bytes_per_voxel": alg_bytes / N,
                      "us_per_launch": fwd_b2b_ms * 1e3,
                      "timing": "CUDA events around the region of K back-to-back launches of the kernel, cold L2",
                      "us_general_entry_eager": fwd_general_eager_ms * 1e3,
+                     "us_sla_forward_bounded": us_bounded, "us_sla_forward_tcgen05": us_tcgen05,
                      "us_per_launch_in_stream_pdl": None if fwd_stream_ms is None else fwd_stream_ms * 1e3,
                      "frac_in_stream_pdl": None if fwd_stream_ms is None
                                            else alg_bytes / (fwd_stream_ms * 1e-3) / 1e9 / peak,

@@ -18,7 +18,8 @@ SLA_F32, SLA_F16, SLA_BF16 = 0, 1, 2
 # Every symbol include/sla.h declares (tests check the library exports exactly these).
 SYMBOLS = (
     "sla_status_string", "sla_version", "sla_workspace_bytes", "sla_offsets_from_window_ids",
-    "sla_forward", "sla_forward_bounded", "sla_backward", "sla_forward_host", "sla_bench_stream_ceiling",
+    "sla_forward", "sla_forward_tcgen05", "sla_forward_bounded", "sla_backward", "sla_forward_host",
+    "sla_bench_stream_ceiling",
 )
 
 _lib = None
@@ -49,6 +50,8 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     L.sla_offsets_from_window_ids.restype = ci
     L.sla_forward.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp, sz, vp]
     L.sla_forward.restype = ci
+    L.sla_forward_tcgen05.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp, sz, vp]
+    L.sla_forward_tcgen05.restype = ci
     L.sla_forward_bounded.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, i32, vp]
     L.sla_forward_bounded.restype = ci
     L.sla_backward.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp, vp, vp, vp, sz, vp]
@@ -116,10 +119,10 @@ def sla_offsets_from_window_ids(win_id, W: int, out=None, stream=None):
     return out
 
 
-def sla_forward(q, k, v, window_offsets, out=None, workspace=None, stream=None, max_window_len=0):
+def sla_forward(q, k, v, window_offsets, out=None, workspace=None, stream=None, max_window_len=0, tcgen05=False):
     """q,k,v: CUDA [N,H,d_h] (fp32/fp16/bf16); window_offsets: CUDA int32[W+1] -> out [N,H,d_h].
     max_window_len > 0 (a promise that no window is longer; <= 256) takes sla_forward_bounded: one
-    kernel launch, no workspace."""
+    kernel launch, no workspace.  tcgen05=True takes sla_forward_tcgen05 (fp16, d_h = 16, H*d_h % 128 == 0)."""
     import torch
     L = load_library()
     _chk_dev(q, k, v, window_offsets)
@@ -138,8 +141,9 @@ def sla_forward(q, k, v, window_offsets, out=None, workspace=None, stream=None, 
                "sla_forward_bounded")
         return out
     workspace, wsb = _workspace(q, N, W, H, d, dt, False, workspace)
-    _check(L.sla_forward(q.data_ptr(), k.data_ptr(), v.data_ptr(), window_offsets.data_ptr(), N, W, H, d,
-                         dt, out.data_ptr(), workspace.data_ptr(), wsb, _stream(stream)), "sla_forward")
+    fn, name = (L.sla_forward_tcgen05, "sla_forward_tcgen05") if tcgen05 else (L.sla_forward, "sla_forward")
+    _check(fn(q.data_ptr(), k.data_ptr(), v.data_ptr(), window_offsets.data_ptr(), N, W, H, d,
+              dt, out.data_ptr(), workspace.data_ptr(), wsb, _stream(stream)), name)
     return out
 
 

@@ -64,9 +64,9 @@ int sla_bench_stream_ceiling(const void* a, const void* b, const void* c, void* 
   return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
 }
 
-int sla_forward(const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
-                int32_t W, int32_t H, int32_t d_h, int dt, void* out, void* workspace,
-                size_t workspace_bytes, sla_stream_t stream) {
+static int forward_impl(bool tcgen05, const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
+                        int32_t W, int32_t H, int32_t d_h, int dt, void* out, void* workspace,
+                        size_t workspace_bytes, sla_stream_t stream) {
   int rc = check_common(N, W, H, d_h, dt);
   if (rc != SLA_OK) return rc;
   if (N == 0 || W == 0) return SLA_OK;
@@ -75,14 +75,28 @@ int sla_forward(const void* q, const void* k, const void* v, const int32_t* wind
   const size_t need = state_bytes(N, H, d_h);
   if (!workspace || workspace_bytes < need || !aligned16(workspace)) return SLA_ERR_WORKSPACE;
   cudaStream_t st = (cudaStream_t)stream;
-  if (cudaMemsetAsync(workspace, 0, need, st) != cudaSuccess) return SLA_ERR_CUDA;
+  if (sla::launch_zero(workspace, need, st) != cudaSuccess) return SLA_ERR_CUDA;
   sla::Problem p{};
   p.q = q; p.k = k; p.v = v; p.out = out; p.off = window_offsets;
   p.ws_state = static_cast<float*>(workspace);
   p.N = (int)N; p.W = W; p.H = H; p.d = d_h;
+  p.tcgen05 = tcgen05;
+  if (tcgen05 && !sla::forward_umma_supported(p, dt)) return SLA_ERR_UNSUPPORTED;
   const bool tc = sla::forward_tc_supported(p, dt);
   cudaError_t e = tc ? sla::launch_forward_tc(p, dt, st) : sla::launch_forward_generic(p, dt, st);
   return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
+}
+
+int sla_forward(const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
+                int32_t W, int32_t H, int32_t d_h, int dt, void* out, void* workspace,
+                size_t workspace_bytes, sla_stream_t stream) {
+  return forward_impl(false, q, k, v, window_offsets, N, W, H, d_h, dt, out, workspace, workspace_bytes, stream);
+}
+
+int sla_forward_tcgen05(const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
+                        int32_t W, int32_t H, int32_t d_h, int dt, void* out, void* workspace,
+                        size_t workspace_bytes, sla_stream_t stream) {
+  return forward_impl(true, q, k, v, window_offsets, N, W, H, d_h, dt, out, workspace, workspace_bytes, stream);
 }
 
 int sla_forward_bounded(const void* q, const void* k, const void* v, const int32_t* window_offsets,
@@ -118,7 +132,7 @@ int sla_backward(const void* q, const void* k, const void* v, const int32_t* win
   const size_t one = state_bytes(N, H, d_h);
   if (!workspace || workspace_bytes < 2 * one || !aligned16(workspace)) return SLA_ERR_WORKSPACE;
   cudaStream_t st = (cudaStream_t)stream;
-  if (cudaMemsetAsync(workspace, 0, 2 * one, st) != cudaSuccess) return SLA_ERR_CUDA;
+  if (sla::launch_zero(workspace, 2 * one, st) != cudaSuccess) return SLA_ERR_CUDA;
   sla::Problem p{};
   p.q = q; p.k = k; p.v = v; p.g = d_out; p.dq = dq; p.dk = dk; p.dv = dv; p.off = window_offsets;
   p.ws_state = static_cast<float*>(workspace);

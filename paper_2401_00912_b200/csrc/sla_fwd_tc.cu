@@ -721,7 +721,7 @@ cudaError_t tc_launch(const Problem& p, cudaStream_t st, bool main_pass) {
   }
   if (!p.bounded) {
     // second pass: outputs of windows longer than kFuseMax (exits at once if there were none)
-    const int span2 = span > kFuseMax ? kFuseMax / 16 * 16 : span;
+    const int span2 = kFuseMax / 16 * 16;   // the largest span OUTPASS handles: fewer CTAs to start and retire when nothing was split
     dim3 grid2((p.N + span2 - 1) / span2, slabs);
     cfg.gridDim = grid2;   // same attribute: resident behind the main kernel's tail, waits for its states
     cudaError_t le = cudaLaunchKernelEx(&cfg, kern_out, tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H,
@@ -741,14 +741,12 @@ bool forward_tc_supported(const Problem& p, int dt) {
 
 cudaError_t launch_forward_tc(const Problem& p, int dt, cudaStream_t st) {
   bool main_pass = true;
-#ifndef SLA_NO_UMMA
-  if (forward_umma_supported(p, dt)) {   // main pass on tcgen05 (sla_fwd_umma.cu); long windows' outputs below
+  if (p.tcgen05) {   // main pass on tcgen05 (sla_fwd_umma.cu, same workspace protocol); long windows' outputs below
     cudaError_t e = launch_forward_umma_main(p, dt, st);
     if (e != cudaSuccess) return e;
     if (p.bounded) return cudaSuccess;
     main_pass = false;
   }
-#endif
   cudaError_t e;
   if (p.d == 16)
     e = (dt == SLA_F16) ? tc_launch<16, false, __half>(p, st, main_pass) : tc_launch<16, true, __nv_bfloat16>(p, st, main_pass);

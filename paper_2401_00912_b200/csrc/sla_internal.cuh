@@ -69,9 +69,12 @@ struct Problem {
   float* ws_dstate;  // [W,H,d+1,d] fp32 (dS, dz) for split windows (backward)
   int N, W, H, d;
   bool bounded;      // caller guarantees every window has <= kFuseMax rows: no workspace, no split pass
+  bool tcgen05;      // main pass on the tcgen05 kernel (sla_fwd_umma.cu) instead of the mma.sync kernel
 };
 
 // Launchers (defined in the .cu files); all enqueue on `st` and return the last CUDA error.
+// zero `bytes` bytes (16-byte aligned) with a kernel that takes part in programmatic dependent launch
+cudaError_t launch_zero(void* p, size_t bytes, cudaStream_t st);
 cudaError_t launch_offsets(const int32_t* win_id, int N, int W, int32_t* off, cudaStream_t st);
 cudaError_t launch_forward_generic(const Problem& p, int dt, cudaStream_t st);
 cudaError_t launch_backward_generic(const Problem& p, int dt, cudaStream_t st);

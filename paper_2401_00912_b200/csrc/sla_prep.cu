@@ -57,7 +57,34 @@ sla_stream_ceiling_kernel(const uint4* __restrict__ a, const uint4* __restrict__
   }
 }
 
+// Zero the fp32 state slots of the workspace.  A kernel rather than a memset node so that it can sit in the chain of
+// programmatic dependent launches: the forward/backward kernel behind it becomes resident and sets itself up while
+// this one runs, and this one does the same behind whatever precedes it in the stream.
+__global__ void __launch_bounds__(256) sla_zero_kernel(uint4* __restrict__ p, size_t n16) {
+  asm volatile("griddepcontrol.launch_dependents;");
+  asm volatile("griddepcontrol.wait;" ::: "memory");   // a previous call's kernels may still be reading the workspace
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += (size_t)gridDim.x * blockDim.x)
+    p[i] = make_uint4(0u, 0u, 0u, 0u);
+}
+
 }  // namespace
+
+cudaError_t launch_zero(void* p, size_t bytes, cudaStream_t st) {
+  const size_t n16 = (bytes + 15) / 16;                    // the workspace size is a multiple of 16
+  if (n16 == 0) return cudaSuccess;
+  unsigned blocks = (unsigned)((n16 + 1023) / 1024);
+  if (blocks > 592) blocks = 592;
+  cudaLaunchAttribute pdl[1];
+  pdl[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  pdl[0].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(blocks);
+  cfg.blockDim = dim3(256);
+  cfg.stream = st;
+  cfg.attrs = pdl;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, sla_zero_kernel, (uint4*)p, n16);
+}
 
 cudaError_t launch_stream_ceiling(const void* a, const void* b, const void* c, void* out, size_t bytes,
                                   cudaStream_t st) {

@@ -178,6 +178,43 @@ def test_large_magnitude_inputs(dtype):
         check(f"large_magnitude.{name}", got, want, dtype, sc.lengths)
 
 
+# ---- the tcgen05 forward (sla_forward_tcgen05): same oracle, same tolerance --------------------------
+TCGEN05_LAYOUTS = dict(EDGE_LAYOUTS, mixed_pack_wrap=[2, 6, 3, 15, 8, 53, 88, 53, 76, 107, 121, 144, 144] * 40,
+                       dense_144=[144] * 400, tiny_3=[3] * 3000)
+
+
+@pytest.mark.parametrize("c", [1, 3, 4])
+def test_forward_tcgen05_configs(c):
+    torch = _torch()
+    sc = wl.make_config(c)
+    q, k, v = sc.tensor("q"), sc.tensor("k"), sc.tensor("v")
+    off = torch.from_numpy(sc.offsets).cuda()
+    out = pkg.sla_forward(to_dev(q, sc.dtype), to_dev(k, sc.dtype), to_dev(v, sc.dtype), off, tcgen05=True)
+    torch.cuda.synchronize()
+    check(f"{sc.name}.tcgen05", out, sla_oracle.forward(q, k, v, sc.offsets, nthreads=8), sc.dtype, sc.lengths)
+
+
+@pytest.mark.parametrize("layout", sorted(TCGEN05_LAYOUTS))
+@pytest.mark.parametrize("H", [8, 16])
+def test_forward_tcgen05_edge_layouts(layout, H):
+    torch = _torch()
+    sc = wl.make_scene(TCGEN05_LAYOUTS[layout], H, 16, "f16", seed=177 + len(layout), name=layout)
+    q, k, v = sc.tensor("q"), sc.tensor("k"), sc.tensor("v")
+    off = torch.from_numpy(sc.offsets).cuda()
+    out = pkg.sla_forward(to_dev(q, "f16"), to_dev(k, "f16"), to_dev(v, "f16"), off, tcgen05=True)
+    torch.cuda.synchronize()
+    check(f"{layout}.tcgen05", out, sla_oracle.forward(q, k, v, sc.offsets, nthreads=8), "f16", sc.lengths)
+
+
+def test_forward_tcgen05_unsupported_shapes():
+    torch = _torch()
+    off = torch.tensor([0, 4], dtype=torch.int32, device="cuda")
+    for shape, dt in (((4, 4, 16), torch.float16), ((4, 8, 32), torch.float16), ((4, 8, 16), torch.bfloat16)):
+        q = torch.zeros(*shape, dtype=dt, device="cuda")
+        with pytest.raises(pkg.SlaError, match="UNSUPPORTED"):
+            pkg.sla_forward(q, q, q, off, tcgen05=True)
+
+
 def test_n0_w0_and_errors():
     torch = _torch()
     q = torch.empty(0, 8, 16, dtype=torch.float16, device="cuda")
