@@ -33,9 +33,9 @@ def _load():
         p = ctypes.c_void_p
         i = ctypes.c_int
         for suf in ("f32", "f64"):
-            getattr(L, f"sla_oracle_forward_{suf}").argtypes = [p, p, p, p, i, i, i, p, p, p, i]
+            getattr(L, f"sla_oracle_forward_{suf}").argtypes = [p, p, p, p, i, i, i, p, p, p, i, i, ctypes.c_double]
             getattr(L, f"sla_oracle_forward_{suf}").restype = None
-            getattr(L, f"sla_oracle_backward_{suf}").argtypes = [p, p, p, p, p, i, i, i, p, p, p, i]
+            getattr(L, f"sla_oracle_backward_{suf}").argtypes = [p, p, p, p, p, i, i, i, p, p, p, i, i, ctypes.c_double]
             getattr(L, f"sla_oracle_backward_{suf}").restype = None
         L.sla_oracle_offsets.argtypes = [p, ctypes.c_int64, i, p]
         L.sla_oracle_offsets.restype = None
@@ -55,9 +55,13 @@ def _prep(x):
     return np.ascontiguousarray(x)
 
 
-def forward(q, k, v, offsets, *, return_state: bool = False, nthreads: int = 1):
+PHI_KINDS = {"elu1": 0, "relu": 1}
+
+
+def forward(q, k, v, offsets, *, return_state: bool = False, nthreads: int = 1, phi: str = "elu1", eps: float = 0.0):
     """q,k,v: [N,H,d] float32 or float64 numpy; offsets int32[W+1].  Returns float64 out [N,H,d]
-    (and S [W,H,d,d], z [W,H,d] if return_state)."""
+    (and S [W,H,d,d], z [W,H,d] if return_state).  phi: "elu1" (default, eps 0) or "relu" (epsilon `eps` in the
+    denominator, reading A15)."""
     L = _load()
     q, k, v = _prep(q), _prep(k), _prep(v)
     assert q.dtype == k.dtype == v.dtype and q.shape == k.shape == v.shape and q.ndim == 3
@@ -69,11 +73,12 @@ def forward(q, k, v, offsets, *, return_state: bool = False, nthreads: int = 1):
     S = np.zeros((W, H, d, d), dtype=np.float64) if return_state else None
     z = np.zeros((W, H, d), dtype=np.float64) if return_state else None
     fn = L.sla_oracle_forward_f32 if q.dtype == np.float32 else L.sla_oracle_forward_f64
-    fn(_ptr(q), _ptr(k), _ptr(v), _ptr(off), W, H, d, _ptr(out), _ptr(S), _ptr(z), int(nthreads))
+    fn(_ptr(q), _ptr(k), _ptr(v), _ptr(off), W, H, d, _ptr(out), _ptr(S), _ptr(z), int(nthreads), PHI_KINDS[phi],
+       float(eps))
     return (out, S, z) if return_state else out
 
 
-def backward(q, k, v, d_out, offsets, *, nthreads: int = 1):
+def backward(q, k, v, d_out, offsets, *, nthreads: int = 1, phi: str = "elu1", eps: float = 0.0):
     """Analytic gradients of L = sum(d_out * SLA(q,k,v)).  Returns float64 dq, dk, dv."""
     L = _load()
     q, k, v, g = _prep(q), _prep(k), _prep(v), _prep(d_out)
@@ -86,7 +91,8 @@ def backward(q, k, v, d_out, offsets, *, nthreads: int = 1):
     dk = np.full((N, H, d), np.nan, dtype=np.float64)
     dv = np.full((N, H, d), np.nan, dtype=np.float64)
     fn = L.sla_oracle_backward_f32 if q.dtype == np.float32 else L.sla_oracle_backward_f64
-    fn(_ptr(q), _ptr(k), _ptr(v), _ptr(g), _ptr(off), W, H, d, _ptr(dq), _ptr(dk), _ptr(dv), int(nthreads))
+    fn(_ptr(q), _ptr(k), _ptr(v), _ptr(g), _ptr(off), W, H, d, _ptr(dq), _ptr(dk), _ptr(dv), int(nthreads),
+       PHI_KINDS[phi], float(eps))
     return dq, dk, dv
 
 

@@ -360,3 +360,116 @@ def test_offsets_against_searchsorted_and_bruteforce():
         assert off[0] == 0 and off[-1] == N
     s = wl.make_config(3)
     np.testing.assert_array_equal(orc.offsets_from_window_ids(s.window_ids, s.W), s.offsets)
+
+
+# ---------------------------------------------------------------- ReLU feature map with eps (reading A15)
+GOLD_RELU = os.path.join(os.path.dirname(__file__), "golden", "sla_golden_relu_d2.txt")
+
+
+def quadratic_window_relu(q, k, v, eps):
+    """(relu(Q) relu(K)^T) V / (rowsum + eps) for ONE window (numpy restatement, PAPER.md:73 with reading A15)."""
+    a, b = np.maximum(q, 0.0), np.maximum(k, 0.0)
+    A = np.einsum("ihp,jhp->hij", a, b)
+    return np.einsum("hij,jhr->ihr", A, v) / (A.sum(axis=2).T[:, :, None] + eps)
+
+
+def test_relu_golden_hand_example():
+    global GOLD
+    saved, GOLD = GOLD, GOLD_RELU
+    try:
+        g = load_golden()
+    finally:
+        GOLD = saved
+    q, k, v = (g[n][:, None, :] for n in ("q", "k", "v"))
+    eps = float(g["eps"][0, 0])
+    out, S, z = orc.forward(q, k, v, offsets_of([3]), return_state=True, phi="relu", eps=eps)
+    np.testing.assert_allclose(S[0, 0], g["S"], rtol=0, atol=1e-15)
+    np.testing.assert_allclose(z[0, 0], g["z"][0], rtol=0, atol=1e-15)
+    np.testing.assert_allclose(out[:, 0, :], g["o"], rtol=1e-15, atol=1e-16)
+    # the first two rows at eps = 0: (1,5)/6 and (0,1)
+    out0 = orc.forward(q[:2], k[:2], v[:2], offsets_of([2]), phi="relu", eps=0.0)
+    np.testing.assert_allclose(out0[:, 0, :], [[1 / 6, 5 / 6], [0.0, 1.0]], rtol=1e-15)
+
+
+@pytest.mark.parametrize("H,d", [(1, 1), (2, 4), (3, 16), (2, 32)])
+def test_relu_linear_equals_quadratic_with_eps(H, d):
+    rng = np.random.default_rng(100 + d)
+    lengths = [1, 2, 3, 7, 16, 33, 64]
+    q, k, v = rand_qkv(rng, sum(lengths), H, d)
+    off = offsets_of(lengths)
+    for eps in (1e-6, 0.25):
+        out = orc.forward(q, k, v, off, phi="relu", eps=eps)
+        for w in range(len(lengths)):
+            s, e = off[w], off[w + 1]
+            np.testing.assert_allclose(out[s:e], quadratic_window_relu(q[s:e], k[s:e], v[s:e], eps), rtol=1e-12, atol=1e-14)
+
+
+def test_relu_homogeneity_and_eps_closed_form():
+    """relu(c x) = c relu(x) for c > 0: at eps = 0 the output is invariant to a positive scaling of q and of all k
+    of a window (SURVEY f1's pin); and o(eps) = o(0) den / (den + eps) wherever den > 0."""
+    rng = np.random.default_rng(7)
+    lengths = [5, 40, 9]
+    q, k, v = rand_qkv(rng, sum(lengths), 2, 8)
+    off = offsets_of(lengths)
+    o0, S, z = orc.forward(q, k, v, off, return_state=True, phi="relu", eps=0.0)
+    assert np.isfinite(o0).all()                    # d = 8, windows >= 5 rows: den > 0 on this draw
+    np.testing.assert_allclose(orc.forward(3.7 * q, k, v, off, phi="relu", eps=0.0), o0, rtol=1e-12, atol=1e-14)
+    np.testing.assert_allclose(orc.forward(q, 0.2 * k, v, off, phi="relu", eps=0.0), o0, rtol=1e-12, atol=1e-14)
+    eps = 0.3
+    oe = orc.forward(q, k, v, off, phi="relu", eps=eps)
+    for w in range(len(lengths)):
+        s, e = off[w], off[w + 1]
+        den = np.einsum("ihp,hp->ih", np.maximum(q[s:e], 0.0), z[w])[:, :, None]
+        np.testing.assert_allclose(oe[s:e], o0[s:e] * den / (den + eps), rtol=1e-12, atol=1e-14)
+
+
+def test_relu_length_one_windows():
+    """m = 1: o = v (a.b)/(a.b + eps); exactly 0 when a.b = 0 (probability (3/4)^d per head)."""
+    rng = np.random.default_rng(8)
+    q, k, v = rand_qkv(rng, 400, 3, 4)
+    off = offsets_of([1] * 400)
+    eps = 1e-3
+    out = orc.forward(q, k, v, off, phi="relu", eps=eps)
+    ab = (np.maximum(q, 0.0) * np.maximum(k, 0.0)).sum(-1, keepdims=True)
+    np.testing.assert_allclose(out, v * ab / (ab + eps), rtol=1e-13, atol=0)
+    assert (ab == 0).any() and np.all(out[np.broadcast_to(ab == 0, out.shape)] == 0.0)
+
+
+def test_relu_backward_autograd_and_finite_differences():
+    rng = np.random.default_rng(21)
+    lengths = (2, 9, 1, 14)
+    N, H, d = sum(lengths), 3, 4
+    q, k, v = rand_qkv(rng, N, H, d)
+    # keep every input away from the kink of relu so that derivatives (and central differences) are well defined
+    q = np.where(np.abs(q) < 0.05, 0.05 * np.sign(q) + (q == 0) * 0.05, q)
+    k = np.where(np.abs(k) < 0.05, 0.05 * np.sign(k) + (k == 0) * 0.05, k)
+    g = rng.standard_normal((N, H, d))
+    off = offsets_of(lengths)
+    eps = 1e-2
+    dq, dk, dv = orc.backward(q, k, v, g, off, phi="relu", eps=eps)
+    tq, tk, tv = (torch.tensor(x, dtype=torch.float64, requires_grad=True) for x in (q, k, v))
+    tg = torch.tensor(g)
+    loss = 0.0
+    for w in range(len(lengths)):
+        s, e = int(off[w]), int(off[w + 1])
+        A = torch.einsum("ihp,jhp->hij", torch.relu(tq[s:e]), torch.relu(tk[s:e]))
+        o = torch.einsum("hij,jhr->ihr", A, tv[s:e]) / (A.sum(-1).transpose(0, 1)[..., None] + eps)
+        loss = loss + (o * tg[s:e]).sum()
+    loss.backward()
+    np.testing.assert_allclose(dq, tq.grad.numpy(), rtol=1e-10, atol=1e-12)
+    np.testing.assert_allclose(dk, tk.grad.numpy(), rtol=1e-10, atol=1e-12)
+    np.testing.assert_allclose(dv, tv.grad.numpy(), rtol=1e-10, atol=1e-12)
+    # central differences of L = sum(g * forward) on a few scalars of each tensor
+    def L(qq, kk, vv):
+        return float((g * orc.forward(qq, kk, vv, off, phi="relu", eps=eps)).sum())
+    h = 1e-6
+    for name, x, grad in (("q", q, dq), ("k", k, dk), ("v", v, dv)):
+        for _ in range(12):
+            idx = tuple(rng.integers(0, n) for n in x.shape)
+            xp, xm = x.copy(), x.copy()
+            xp[idx] += h
+            xm[idx] -= h
+            args_p = {"q": (xp, k, v), "k": (q, xp, v), "v": (q, k, xp)}[name]
+            args_m = {"q": (xm, k, v), "k": (q, xm, v), "v": (q, k, xm)}[name]
+            fd = (L(*args_p) - L(*args_m)) / (2 * h)
+            assert abs(fd - grad[idx]) <= 1e-6 * max(1.0, abs(grad[idx])), (name, idx, fd, grad[idx])
