@@ -489,6 +489,9 @@ def run_ours(args):
         if max_len <= 144:
             us_bounded = graph_leg(lambda r: pkg.sla_forward(*sets[r][:3], off, out=sets[r][3], stream=side,
                                                              max_window_len=144))
+        # the second feature map (ReLU with eps) through sla_forward_phi
+        us_relu = graph_leg(lambda r: pkg.sla_forward(*sets[r][:3], off, out=sets[r][3], workspace=ws, stream=side,
+                                                      phi="relu", eps=1e-6))
         if sc.dtype == "f16" and d == 16 and (H * d) % 128 == 0:
             us_tcgen05 = graph_leg(lambda r: pkg.sla_forward(*sets[r][:3], off, out=sets[r][3], workspace=ws,
                                                              stream=side, tcgen05=True))
@@ -584,6 +587,7 @@ def run_ours(args):
                      "timing": "CUDA events around the region of K back-to-back launches of the kernel, cold L2",
                      "us_general_entry_eager": fwd_general_eager_ms * 1e3,
                      "us_sla_forward_bounded": us_bounded, "us_sla_forward_tcgen05": us_tcgen05,
+                     "us_sla_forward_phi_relu": us_relu,
                      "us_per_launch_in_stream_pdl": None if fwd_stream_ms is None else fwd_stream_ms * 1e3,
                      "frac_in_stream_pdl": None if fwd_stream_ms is None
                                            else alg_bytes / (fwd_stream_ms * 1e-3) / 1e9 / peak,

@@ -42,6 +42,14 @@ typedef enum {
 
 typedef enum { SLA_F32 = 0, SLA_F16 = 1, SLA_BF16 = 2 } sla_dtype_t;
 
+/* Feature map phi of Eq. 3 ("phi(x) is the kernel function"; the paper never writes it out):
+ *   SLA_PHI_ELU1  phi(x) = elu(x)+1, the map of the linear attention [17] that Eq. 3 cites; strictly
+ *                 positive, so the denominator needs no epsilon.  What sla_forward / sla_backward compute.
+ *   SLA_PHI_RELU  phi(x) = max(x, 0), the "Efficient Attn [3]" kernel that labels Table 7's default row
+ *                 (PAPER.md:277, 296), with an epsilon added to the denominator (which can otherwise be exactly 0):
+ *                 o_i = phi(q_i) S / (phi(q_i) . z + eps).  Entry points sla_forward_phi / sla_backward_phi. */
+typedef enum { SLA_PHI_ELU1 = 0, SLA_PHI_RELU = 1 } sla_feature_map_t;
+
 /* Opaque CUDA stream handle (a cudaStream_t / CUstream); NULL = the legacy default stream. */
 typedef struct CUstream_st* sla_stream_t;
 
@@ -73,6 +81,19 @@ int sla_offsets_from_window_ids(const int32_t* win_id, int64_t N, int32_t W,
 int sla_forward(const void* q, const void* k, const void* v, const int32_t* window_offsets,
                 int64_t N, int32_t W, int32_t H, int32_t d_h, int dt, void* out,
                 void* workspace, size_t workspace_bytes, sla_stream_t stream);
+
+/* sla_forward / sla_backward with the feature map chosen by the caller (sla_feature_map_t) and `eps` added to the
+ * denominator of Eq. 3 (eps >= 0; must be 0 for SLA_PHI_ELU1, > 0 recommended for SLA_PHI_RELU, e.g. 1e-6).  All other
+ * arguments, the workspace size and the error behaviour are those of sla_forward / sla_backward, which are these
+ * calls with (SLA_PHI_ELU1, 0).  Unknown map or eps < 0 -> SLA_ERR_INVALID_ARG.  Backward of the ReLU map:
+ * phi'(x) = 1 for x > 0, else 0. */
+int sla_forward_phi(const void* q, const void* k, const void* v, const int32_t* window_offsets,
+                    int64_t N, int32_t W, int32_t H, int32_t d_h, int dt, int feature_map, float eps, void* out,
+                    void* workspace, size_t workspace_bytes, sla_stream_t stream);
+int sla_backward_phi(const void* q, const void* k, const void* v, const int32_t* window_offsets,
+                     int64_t N, int32_t W, int32_t H, int32_t d_h, int dt, int feature_map, float eps,
+                     const void* d_out, void* dq, void* dk, void* dv,
+                     void* workspace, size_t workspace_bytes, sla_stream_t stream);
 
 /* The same operation as sla_forward, same arguments and results within the same tolerance, with the main pass on
  * the 5th-generation tensor cores (tcgen05.mma, accumulators in tensor memory; csrc/sla_fwd_umma.cu): all heads of a

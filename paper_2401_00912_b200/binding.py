@@ -14,11 +14,13 @@ LIB_PATH = os.path.join(_HERE, "libsla_b200.so")
 
 SLA_OK = 0
 SLA_F32, SLA_F16, SLA_BF16 = 0, 1, 2
+SLA_PHI_ELU1, SLA_PHI_RELU = 0, 1
+_PHI = {"elu1": SLA_PHI_ELU1, "relu": SLA_PHI_RELU}
 
 # Every symbol include/sla.h declares (tests check the library exports exactly these).
 SYMBOLS = (
     "sla_status_string", "sla_version", "sla_workspace_bytes", "sla_offsets_from_window_ids",
-    "sla_forward", "sla_forward_tcgen05", "sla_forward_bounded", "sla_backward", "sla_forward_host",
+    "sla_forward", "sla_forward_phi", "sla_backward_phi", "sla_forward_tcgen05", "sla_forward_bounded", "sla_backward", "sla_forward_host",
     "sla_bench_stream_ceiling",
 )
 
@@ -50,6 +52,10 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     L.sla_offsets_from_window_ids.restype = ci
     L.sla_forward.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp, sz, vp]
     L.sla_forward.restype = ci
+    L.sla_forward_phi.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, ci, ctypes.c_float, vp, vp, sz, vp]
+    L.sla_forward_phi.restype = ci
+    L.sla_backward_phi.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, ci, ctypes.c_float, vp, vp, vp, vp, vp, sz, vp]
+    L.sla_backward_phi.restype = ci
     L.sla_forward_tcgen05.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp, sz, vp]
     L.sla_forward_tcgen05.restype = ci
     L.sla_forward_bounded.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, i32, vp]
@@ -119,10 +125,12 @@ def sla_offsets_from_window_ids(win_id, W: int, out=None, stream=None):
     return out
 
 
-def sla_forward(q, k, v, window_offsets, out=None, workspace=None, stream=None, max_window_len=0, tcgen05=False):
+def sla_forward(q, k, v, window_offsets, out=None, workspace=None, stream=None, max_window_len=0, tcgen05=False,
+                phi="elu1", eps=0.0):
     """q,k,v: CUDA [N,H,d_h] (fp32/fp16/bf16); window_offsets: CUDA int32[W+1] -> out [N,H,d_h].
     max_window_len > 0 (a promise that no window is longer; <= 256) takes sla_forward_bounded: one
-    kernel launch, no workspace.  tcgen05=True takes sla_forward_tcgen05 (fp16, d_h = 16, H*d_h % 128 == 0)."""
+    kernel launch, no workspace.  tcgen05=True takes sla_forward_tcgen05 (fp16, d_h = 16, H*d_h % 128 == 0).
+    phi="relu" (with eps > 0 in the denominator) takes sla_forward_phi."""
     import torch
     L = load_library()
     _chk_dev(q, k, v, window_offsets)
@@ -141,13 +149,19 @@ def sla_forward(q, k, v, window_offsets, out=None, workspace=None, stream=None, 
                "sla_forward_bounded")
         return out
     workspace, wsb = _workspace(q, N, W, H, d, dt, False, workspace)
+    if phi != "elu1":
+        _check(L.sla_forward_phi(q.data_ptr(), k.data_ptr(), v.data_ptr(), window_offsets.data_ptr(), N, W, H, d, dt,
+                                 _PHI[phi], float(eps), out.data_ptr(), workspace.data_ptr(), wsb, _stream(stream)),
+               "sla_forward_phi")
+        return out
     fn, name = (L.sla_forward_tcgen05, "sla_forward_tcgen05") if tcgen05 else (L.sla_forward, "sla_forward")
     _check(fn(q.data_ptr(), k.data_ptr(), v.data_ptr(), window_offsets.data_ptr(), N, W, H, d,
               dt, out.data_ptr(), workspace.data_ptr(), wsb, _stream(stream)), name)
     return out
 
 
-def sla_backward(q, k, v, window_offsets, d_out, dq=None, dk=None, dv=None, workspace=None, stream=None):
+def sla_backward(q, k, v, window_offsets, d_out, dq=None, dk=None, dv=None, workspace=None, stream=None,
+                 phi="elu1", eps=0.0):
     """Gradients of sum(d_out * SLA(q,k,v)) -> (dq, dk, dv), each [N,H,d_h] of the input dtype."""
     import torch
     L = load_library()
@@ -164,6 +178,11 @@ def sla_backward(q, k, v, window_offsets, d_out, dq=None, dk=None, dv=None, work
     dk = torch.empty_like(q) if dk is None else dk
     dv = torch.empty_like(q) if dv is None else dv
     workspace, wsb = _workspace(q, N, W, H, d, dt, True, workspace)
+    if phi != "elu1":
+        _check(L.sla_backward_phi(q.data_ptr(), k.data_ptr(), v.data_ptr(), window_offsets.data_ptr(), N, W, H, d, dt,
+                                  _PHI[phi], float(eps), d_out.data_ptr(), dq.data_ptr(), dk.data_ptr(), dv.data_ptr(),
+                                  workspace.data_ptr(), wsb, _stream(stream)), "sla_backward_phi")
+        return dq, dk, dv
     _check(L.sla_backward(q.data_ptr(), k.data_ptr(), v.data_ptr(), window_offsets.data_ptr(), N, W, H, d,
                           dt, d_out.data_ptr(), dq.data_ptr(), dk.data_ptr(), dv.data_ptr(),
                           workspace.data_ptr(), wsb, _stream(stream)), "sla_backward")

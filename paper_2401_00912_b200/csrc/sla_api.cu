@@ -64,7 +64,7 @@ int sla_bench_stream_ceiling(const void* a, const void* b, const void* c, void* 
   return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
 }
 
-static int forward_impl(bool tcgen05, const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
+static int forward_impl(bool tcgen05, int phi, float eps, const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
                         int32_t W, int32_t H, int32_t d_h, int dt, void* out, void* workspace,
                         size_t workspace_bytes, sla_stream_t stream) {
   int rc = check_common(N, W, H, d_h, dt);
@@ -81,6 +81,7 @@ static int forward_impl(bool tcgen05, const void* q, const void* k, const void* 
   p.ws_state = static_cast<float*>(workspace);
   p.N = (int)N; p.W = W; p.H = H; p.d = d_h;
   p.tcgen05 = tcgen05;
+  p.phi = phi; p.eps = eps;
   if (tcgen05 && !sla::forward_umma_supported(p, dt)) return SLA_ERR_UNSUPPORTED;
   const bool tc = sla::forward_tc_supported(p, dt);
   cudaError_t e = tc ? sla::launch_forward_tc(p, dt, st) : sla::launch_forward_generic(p, dt, st);
@@ -90,13 +91,29 @@ static int forward_impl(bool tcgen05, const void* q, const void* k, const void* 
 int sla_forward(const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
                 int32_t W, int32_t H, int32_t d_h, int dt, void* out, void* workspace,
                 size_t workspace_bytes, sla_stream_t stream) {
-  return forward_impl(false, q, k, v, window_offsets, N, W, H, d_h, dt, out, workspace, workspace_bytes, stream);
+  return forward_impl(false, SLA_PHI_ELU1, 0.f, q, k, v, window_offsets, N, W, H, d_h, dt, out, workspace, workspace_bytes, stream);
+}
+
+// feature map / epsilon arguments of the *_phi entries
+static int check_phi(int phi, float eps) {
+  if (phi != SLA_PHI_ELU1 && phi != SLA_PHI_RELU) return SLA_ERR_INVALID_ARG;
+  if (!(eps >= 0.f) || (phi == SLA_PHI_ELU1 && eps != 0.f)) return SLA_ERR_INVALID_ARG;
+  return SLA_OK;
+}
+
+int sla_forward_phi(const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
+                    int32_t W, int32_t H, int32_t d_h, int dt, int feature_map, float eps, void* out,
+                    void* workspace, size_t workspace_bytes, sla_stream_t stream) {
+  const int rc = check_phi(feature_map, eps);
+  if (rc != SLA_OK) return rc;
+  return forward_impl(false, feature_map, eps, q, k, v, window_offsets, N, W, H, d_h, dt, out, workspace,
+                      workspace_bytes, stream);
 }
 
 int sla_forward_tcgen05(const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
                         int32_t W, int32_t H, int32_t d_h, int dt, void* out, void* workspace,
                         size_t workspace_bytes, sla_stream_t stream) {
-  return forward_impl(true, q, k, v, window_offsets, N, W, H, d_h, dt, out, workspace, workspace_bytes, stream);
+  return forward_impl(true, SLA_PHI_ELU1, 0.f, q, k, v, window_offsets, N, W, H, d_h, dt, out, workspace, workspace_bytes, stream);
 }
 
 int sla_forward_bounded(const void* q, const void* k, const void* v, const int32_t* window_offsets,
@@ -119,7 +136,7 @@ int sla_forward_bounded(const void* q, const void* k, const void* v, const int32
   return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
 }
 
-int sla_backward(const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
+static int backward_impl(int phi, float eps, const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
                  int32_t W, int32_t H, int32_t d_h, int dt, const void* d_out, void* dq, void* dk,
                  void* dv, void* workspace, size_t workspace_bytes, sla_stream_t stream) {
   int rc = check_common(N, W, H, d_h, dt);
@@ -138,9 +155,26 @@ int sla_backward(const void* q, const void* k, const void* v, const int32_t* win
   p.ws_state = static_cast<float*>(workspace);
   p.ws_dstate = reinterpret_cast<float*>(static_cast<char*>(workspace) + one);
   p.N = (int)N; p.W = W; p.H = H; p.d = d_h;
+  p.phi = phi; p.eps = eps;
   const bool tc = sla::backward_tc_supported(p, dt);
   cudaError_t e = tc ? sla::launch_backward_tc(p, dt, st) : sla::launch_backward_generic(p, dt, st);
   return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
+}
+
+int sla_backward(const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
+                 int32_t W, int32_t H, int32_t d_h, int dt, const void* d_out, void* dq, void* dk,
+                 void* dv, void* workspace, size_t workspace_bytes, sla_stream_t stream) {
+  return backward_impl(SLA_PHI_ELU1, 0.f, q, k, v, window_offsets, N, W, H, d_h, dt, d_out, dq, dk, dv, workspace,
+                       workspace_bytes, stream);
+}
+
+int sla_backward_phi(const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
+                     int32_t W, int32_t H, int32_t d_h, int dt, int feature_map, float eps, const void* d_out,
+                     void* dq, void* dk, void* dv, void* workspace, size_t workspace_bytes, sla_stream_t stream) {
+  const int rc = check_phi(feature_map, eps);
+  if (rc != SLA_OK) return rc;
+  return backward_impl(feature_map, eps, q, k, v, window_offsets, N, W, H, d_h, dt, d_out, dq, dk, dv, workspace,
+                       workspace_bytes, stream);
 }
 
 }  // extern "C"

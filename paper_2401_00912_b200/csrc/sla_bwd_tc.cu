@@ -491,6 +491,7 @@ cudaError_t bwd_tc_launch(const Problem& p, cudaStream_t st) {
 bool backward_tc_supported(const Problem& p, int dt) {
   if (dt != SLA_F16 && dt != SLA_BF16) return false;
   if (p.d != 16 || (p.H * p.d) % 64 != 0) return false;
+  if (p.phi != SLA_PHI_ELU1) return false;                     // the ReLU map's backward runs on the generic kernels
   return encode_fn() != nullptr;
 }
 

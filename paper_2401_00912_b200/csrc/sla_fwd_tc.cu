@@ -100,9 +100,12 @@ __device__ __forceinline__ uint32_t ring_next_slot(uint32_t a, uint32_t ring_end
   return a >= ring_end ? a - (uint32_t)(NST * slot_bytes) : a;
 }
 
-template <int D, bool BF16, bool PRECISE, bool FULL = false>
+template <int D, int MODE, bool PRECISE, bool FULL = false>
 __device__ __forceinline__ void kv_tile(const RingView& rv, int hl, int rel0, int nvalid_in, State<D>& s,
                                         uint32_t a0_in = 0u) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   const int nvalid = FULL ? 16 : nvalid_in;
   using C = Cfg<D>;
   const int lane = threadIdx.x & 31;
@@ -121,13 +124,13 @@ __device__ __forceinline__ void kv_tile(const RingView& rv, int hl, int rel0, in
       for (int i = 0; i < 4; ++i) {
         const int j0 = 2 * t + 8 * (i >> 1);
         float2 x = unpack2<BF16>(kr[i]);
-        float b0 = (j0 < nvalid) ? phi_fast(x.x) : 0.f;
-        float b1 = (j0 + 1 < nvalid) ? phi_fast(x.y) : 0.f;
+        float b0 = (j0 < nvalid) ? phi_fast<PHI>(x.x) : 0.f;
+        float b1 = (j0 + 1 < nvalid) ? phi_fast<PHI>(x.y) : 0.f;
         split_h2(b0, b1, bhi[i], blo[i]);
       }
     } else {
 #pragma unroll
-      for (int i = 0; i < 4; ++i) { bhi[i] = phi_h2<BF16>(kr[i]); blo[i] = 0u; }
+      for (int i = 0; i < 4; ++i) { bhi[i] = phi_h2<BF16, PHI>(kr[i]); blo[i] = 0u; }
       if (nvalid < 16) {                            // ragged last tile of the window: zero phi(K) rows
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
@@ -187,10 +190,12 @@ __device__ __forceinline__ void kv_tile(const RingView& rv, int hl, int rel0, in
 template <int D> struct OutOperands {
   uint32_t hi[D / 8][D / 16][2], lo[D / 8][D / 16][2];
   uint32_t zhi[D / 16][2], zlo[D / 16][2];
+  float eps;   // epsilon of the denominator on the scale of the operands (eps * scale)
 };
 
 template <int D, bool PRECISE>
-__device__ __forceinline__ void make_out_operands(const State<D>& s, float scale, OutOperands<D>& o) {
+__device__ __forceinline__ void make_out_operands(const State<D>& s, float scale, float eps, OutOperands<D>& o) {
+  o.eps = eps * scale;
 #pragma unroll
   for (int n2 = 0; n2 < D / 8; ++n2)
 #pragma unroll
@@ -214,10 +219,13 @@ __device__ __forceinline__ void make_out_operands(const State<D>& s, float scale
 
 // One 16-row Q tile: out rows [row0, row0+nvalid) of head h.  `lane_out` = this lane's first output
 // element (row0 + g, head column + 2t); `o8` = 8 rows in elements.
-template <int D, bool BF16, bool PRECISE, typename T, bool FULL = false>
+template <int D, int MODE, bool PRECISE, typename T, bool FULL = false>
 __device__ __forceinline__ void q_tile(const RingView& rv, int hl, int rel0, int nvalid_in,
                                        const OutOperands<D>& o, T* __restrict__ lane_out, size_t o8,
                                        uint32_t a0_in = 0u) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   const int nvalid = FULL ? 16 : nvalid_in;
   using C = Cfg<D>;
   const int lane = threadIdx.x & 31;
@@ -234,9 +242,9 @@ __device__ __forceinline__ void q_tile(const RingView& rv, int hl, int rel0, int
     for (int i = 0; i < 4; ++i) {
       if (PRECISE) {
         float2 x = unpack2<BF16>(qr[perm[i]]);
-        split_h2(phi_fast(x.x), phi_fast(x.y), ahi[ks][i], alo[ks][i]);
+        split_h2(phi_fast<PHI>(x.x), phi_fast<PHI>(x.y), ahi[ks][i], alo[ks][i]);
       } else {
-        ahi[ks][i] = phi_h2<BF16>(qr[perm[i]]);
+        ahi[ks][i] = phi_h2<BF16, PHI>(qr[perm[i]]);
         alo[ks][i] = 0u;
       }
     }
@@ -250,7 +258,7 @@ __device__ __forceinline__ void q_tile(const RingView& rv, int hl, int rel0, int
       mma16816(den, ahi[ks][0], ahi[ks][1], ahi[ks][2], ahi[ks][3], o.zlo[ks][0], o.zlo[ks][1]);
     }
   }
-  const float inv0 = fast_rcp(den[0]), inv1 = fast_rcp(den[2]);
+  const float inv0 = fast_rcp(den[0] + o.eps), inv1 = fast_rcp(den[2] + o.eps);
 #pragma unroll
   for (int n2 = 0; n2 < D / 8; ++n2) {
     float acc[4] = {0.f, 0.f, 0.f, 0.f};
@@ -270,15 +278,18 @@ __device__ __forceinline__ void q_tile(const RingView& rv, int hl, int rel0, int
 }
 
 // packed short windows (quad_tile_core, sla_tc_base.cuh) on rows rel0.. of this CTA's K/V and Q rings
-template <int D, bool BF16, typename T>
+template <int D, int MODE, typename T>
 __device__ __forceinline__ void quad_tile(const RingView& kv, const RingView& qv, int hl, int rel0,
-                                          int nvalid, int wid, T* __restrict__ out_rows, int C_total) {
+                                          int nvalid, int wid, T* __restrict__ out_rows, int C_total, float eps) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   using C = Cfg<D>;
-  quad_tile_core<D, BF16, T>(
+  quad_tile_core<D, BF16, T, PHI>(
       [&](int r, int c) { return ring_addr<D>(qv, C::T_STAGE, 0, rel0 + r, c); },
       [&](int r, int c) { return ring_addr<D>(kv, C::KV_STAGE, 0, rel0 + r, c); },
       [&](int r, int c) { return ring_addr<D>(kv, C::KV_STAGE, C::T_STAGE, rel0 + r, c); }, hl, nvalid, wid,
-      out_rows, C_total);
+      out_rows, C_total, eps);
 }
 
 // ---- CTA-level shared control block ----------------------------------------------------------------
@@ -292,10 +303,13 @@ struct Ctrl {
 // One whole (fused) window [s,e) for head slot hl: state pass over K,V then output pass over Q.
 // Rows are addressed relative to S0, the first row of this CTA's streams.  Two 16-row tiles per
 // iteration: one wait/release bookkeeping step per 32 rows and two independent dependency chains.
-template <int D, bool BF16, bool PRECISE, typename T>
+template <int D, int MODE, bool PRECISE, typename T>
 __device__ __forceinline__ void process_window(RingView& kv, RingView& qv, int hl, int nh, int S0, int s,
                                                int e, T* __restrict__ out_head /*out + head column*/,
-                                               int Ctot) {
+                                               int Ctot, float eps) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   using C = Cfg<D>;
   State<D> st[C::HPW];
 #pragma unroll
@@ -322,13 +336,13 @@ __device__ __forceinline__ void process_window(RingView& kv, RingView& qv, int h
     for (int j = 0; j < C::HPW; ++j)
       if (j < nh) {
         if (nv == 32) {   // two full tiles, one basic block: the two dependency chains interleave
-          kv_tile<D, BF16, PRECISE, true>(kv, hl + j, rel, 16, st[j], ak[j][0]);
-          kv_tile<D, BF16, PRECISE, true>(kv, hl + j, rel + 16, 16, st[j], ak[j][1]);
+          kv_tile<D, MODE, PRECISE, true>(kv, hl + j, rel, 16, st[j], ak[j][0]);
+          kv_tile<D, MODE, PRECISE, true>(kv, hl + j, rel + 16, 16, st[j], ak[j][1]);
           ak[j][0] = ring_next_slot(ak[j][0], kv_end, C::KV_STAGE);
           ak[j][1] = ring_next_slot(ak[j][1], kv_end, C::KV_STAGE);
         } else {
-          kv_tile<D, BF16, PRECISE>(kv, hl + j, rel, min(16, nv), st[j]);
-          if (nv > 16) kv_tile<D, BF16, PRECISE>(kv, hl + j, rel + 16, nv - 16, st[j]);
+          kv_tile<D, MODE, PRECISE>(kv, hl + j, rel, min(16, nv), st[j]);
+          if (nv > 16) kv_tile<D, MODE, PRECISE>(kv, hl + j, rel + 16, nv - 16, st[j]);
         }
       }
   }
@@ -337,7 +351,7 @@ __device__ __forceinline__ void process_window(RingView& kv, RingView& qv, int h
   const float scale = __int_as_float((127 - lg) << 23);   // 2^-lg: keeps fp16 operands O(1)
   OutOperands<D> oo[C::HPW];
 #pragma unroll
-  for (int j = 0; j < C::HPW; ++j) make_out_operands<D, PRECISE>(st[j], scale, oo[j]);
+  for (int j = 0; j < C::HPW; ++j) make_out_operands<D, PRECISE>(st[j], scale, eps, oo[j]);
   uint32_t aq[C::HPW][2];
   ring_release_below<C::SR>(qv, s - S0);
 #pragma unroll
@@ -359,22 +373,25 @@ __device__ __forceinline__ void process_window(RingView& kv, RingView& qv, int h
       if (j < nh) {
         T* oh = lp + j * D;
         if (nv == 32) {
-          q_tile<D, BF16, PRECISE, T, true>(qv, hl + j, rel, 16, oo[j], oh, o8, aq[j][0]);
-          q_tile<D, BF16, PRECISE, T, true>(qv, hl + j, rel + 16, 16, oo[j], oh + 2 * o8, o8, aq[j][1]);
+          q_tile<D, MODE, PRECISE, T, true>(qv, hl + j, rel, 16, oo[j], oh, o8, aq[j][0]);
+          q_tile<D, MODE, PRECISE, T, true>(qv, hl + j, rel + 16, 16, oo[j], oh + 2 * o8, o8, aq[j][1]);
           aq[j][0] = ring_next_slot(aq[j][0], q_end, C::T_STAGE);
           aq[j][1] = ring_next_slot(aq[j][1], q_end, C::T_STAGE);
         } else {
-          q_tile<D, BF16, PRECISE, T>(qv, hl + j, rel, min(16, nv), oo[j], oh, o8);
-          if (nv > 16) q_tile<D, BF16, PRECISE, T>(qv, hl + j, rel + 16, nv - 16, oo[j], oh + 2 * o8, o8);
+          q_tile<D, MODE, PRECISE, T>(qv, hl + j, rel, min(16, nv), oo[j], oh, o8);
+          if (nv > 16) q_tile<D, MODE, PRECISE, T>(qv, hl + j, rel + 16, nv - 16, oo[j], oh + 2 * o8, o8);
         }
       }
   }
 }
 
 // The piece [ps,pe) of a split window: partial state -> workspace atomics.
-template <int D, bool BF16>
+template <int D, int MODE>
 __device__ __forceinline__ void process_piece(RingView& kv, int hl, int nh, int S0, int ps, int pe,
                                               float* __restrict__ slot /*slot of head hl*/) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   using C = Cfg<D>;
   const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   State<D> st[C::HPW];
@@ -387,8 +404,8 @@ __device__ __forceinline__ void process_piece(RingView& kv, int hl, int nh, int 
 #pragma unroll
     for (int j = 0; j < C::HPW; ++j)
       if (j < nh) {
-        kv_tile<D, BF16, false>(kv, hl + j, rel, min(16, nv), st[j]);
-        if (nv > 16) kv_tile<D, BF16, false>(kv, hl + j, rel + 16, nv - 16, st[j]);
+        kv_tile<D, MODE, false>(kv, hl + j, rel, min(16, nv), st[j]);
+        if (nv > 16) kv_tile<D, MODE, false>(kv, hl + j, rel + 16, nv - 16, st[j]);
       }
   }
 #pragma unroll
@@ -415,10 +432,13 @@ __device__ __forceinline__ void process_piece(RingView& kv, int hl, int nh, int 
 
 // Output pass for the piece [ps,pe) of a split window of m rows: the complete state is read from the
 // workspace slot (fp32 [d+1, d]: rows 0..d-1 = S, row d = z) into the mma fragment layout.
-template <int D, bool BF16, typename T>
+template <int D, int MODE, typename T>
 __device__ __forceinline__ void output_piece(RingView& qv, int hl, int S0, int ps, int pe, int m,
                                              const float* __restrict__ slot, T* __restrict__ out_head,
-                                             int Ctot) {
+                                             int Ctot, float eps) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   using C = Cfg<D>;
   const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   State<D> st;
@@ -438,7 +458,7 @@ __device__ __forceinline__ void output_piece(RingView& qv, int hl, int S0, int p
   const int lg = 32 - __clz(m - 1);
   const float scale = __int_as_float((127 - lg) << 23);
   OutOperands<D> oo;
-  make_out_operands<D, false>(st, scale, oo);
+  make_out_operands<D, false>(st, scale, eps, oo);
   uint32_t aq[2];
   ring_release_below<C::SR>(qv, ps - S0);
   aq[0] = lane_tile_addr<D>(qv, C::T_STAGE, hl, ps - S0, 16);
@@ -452,13 +472,13 @@ __device__ __forceinline__ void output_piece(RingView& qv, int hl, int S0, int p
     else if (r != ps) ring_release_one(qv);
     ring_wait_upto(qv, (rel + nv - 1) / C::SR);
     if (nv == 32) {
-      q_tile<D, BF16, false, T, true>(qv, hl, rel, 16, oo, lp, o8, aq[0]);
-      q_tile<D, BF16, false, T, true>(qv, hl, rel + 16, 16, oo, lp + 2 * o8, o8, aq[1]);
+      q_tile<D, MODE, false, T, true>(qv, hl, rel, 16, oo, lp, o8, aq[0]);
+      q_tile<D, MODE, false, T, true>(qv, hl, rel + 16, 16, oo, lp + 2 * o8, o8, aq[1]);
       aq[0] = ring_next_slot(aq[0], q_end, C::T_STAGE);
       aq[1] = ring_next_slot(aq[1], q_end, C::T_STAGE);
     } else {
-      q_tile<D, BF16, false, T>(qv, hl, rel, min(16, nv), oo, lp, o8);
-      if (nv > 16) q_tile<D, BF16, false, T>(qv, hl, rel + 16, nv - 16, oo, lp + 2 * o8, o8);
+      q_tile<D, MODE, false, T>(qv, hl, rel, min(16, nv), oo, lp, o8);
+      if (nv > 16) q_tile<D, MODE, false, T>(qv, hl, rel + 16, nv - 16, oo, lp + 2 * o8, o8);
     }
   }
 }
@@ -466,11 +486,11 @@ __device__ __forceinline__ void output_piece(RingView& qv, int hl, int S0, int p
 // OUTPASS = false: the main kernel.  OUTPASS = true: the second pass of the general entry -- outputs of
 // the pieces of windows longer than kFuseMax, whose complete states the main kernel left in the
 // workspace; it streams only Q and exits at once if the main kernel met no such window.
-template <int D, bool BF16, typename T, bool OUTPASS>
+template <int D, int MODE, typename T, bool OUTPASS>
 __global__ void __launch_bounds__(Cfg<D>::THREADS, (D == 16 ? SLA_MINB : 2))
 sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                   const __grid_constant__ CUtensorMap tmV, const int32_t* __restrict__ off,
-                  T* __restrict__ out, float* __restrict__ ws, int N, int W, int H, int span) {
+                  T* __restrict__ out, float* __restrict__ ws, int N, int W, int H, int span, float eps) {
   using C = Cfg<D>;
   extern __shared__ uint8_t dyn_smem[];
   __shared__ Ctrl ctrl;
@@ -615,7 +635,7 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
           if (j < nh) {
             const float* slot = ws + kWsHeaderFloats +
                                 ((size_t)(s / (kFuseMax + 1)) * H + (h0 + hl + j)) * (size_t)((D + 1) * D);
-            output_piece<D, BF16, T>(qv, hl + j, S0, max(s, R0), min(e, R1), e - s, slot, out_head + j * D, Ctot);
+            output_piece<D, MODE, T>(qv, hl + j, S0, max(s, R0), min(e, R1), e - s, slot, out_head + j * D, Ctot, eps);
           }
       }
       ++w;
@@ -652,17 +672,17 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       ring_wait_upto(qv, (rel + rows - 1) / C::SR);
 #pragma unroll
       for (int j = 0; j < C::HPW; ++j)
-        if (j < nh) quad_tile<D, BF16, T>(kv, qv, hl + j, rel, rows, wid, out_head + j * D + (size_t)s * Ctot, Ctot);
+        if (j < nh) quad_tile<D, MODE, T>(kv, qv, hl + j, rel, rows, wid, out_head + j * D + (size_t)s * Ctot, Ctot, eps);
       ring_release_below<C::SR>(kv, rel + rows);
       ring_release_below<C::SR>(qv, rel + rows);
       continue;
     }
     if (m <= kFuseMax) {
-      process_window<D, BF16, false, T>(kv, qv, hl, nh, S0, s, e, out_head, Ctot);
+      process_window<D, MODE, false, T>(kv, qv, hl, nh, S0, s, e, out_head, Ctot, eps);
     } else if (ws != nullptr) {   // bounded entry (no workspace): a window that breaks the caller's promise is skipped
       float* slot = ws + kWsHeaderFloats + ((size_t)(s / (kFuseMax + 1)) * H + (h0 + hl)) * (size_t)((D + 1) * D);
       if (hl == 0 && lane == 0) reinterpret_cast<volatile int*>(ws)[0] = 1;   // tell the output kernel
-      process_piece<D, BF16>(kv, hl, nh, S0, max(s, R0), min(e, R1), slot);
+      process_piece<D, MODE>(kv, hl, nh, S0, max(s, R0), min(e, R1), slot);
     }
     ++w;
   }
@@ -675,7 +695,7 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
 // ---- host side (tensor-map encoder, SM count: sla_tc_common.cuh) -----------------------------------
 // `main_pass` = false: only the OUTPASS launch (the main pass was done by the tcgen05 kernel, sla_fwd_umma.cu,
 // which follows the same workspace protocol).
-template <int D, bool BF16, typename T>
+template <int D, int MODE, typename T>
 cudaError_t tc_launch(const Problem& p, cudaStream_t st, bool main_pass) {
   using C = Cfg<D>;
   CUtensorMap tq, tk, tv;
@@ -683,8 +703,8 @@ cudaError_t tc_launch(const Problem& p, cudaStream_t st, bool main_pass) {
   if (!make_map(&tq, p.q, p.N, Ctot, C::SR) || !make_map(&tk, p.k, p.N, Ctot, C::SR) ||
       !make_map(&tv, p.v, p.N, Ctot, C::SR))
     return cudaErrorInvalidValue;
-  auto kern = sla_fwd_tc_kernel<D, BF16, T, false>;
-  auto kern_out = sla_fwd_tc_kernel<D, BF16, T, true>;
+  auto kern = sla_fwd_tc_kernel<D, MODE, T, false>;
+  auto kern_out = sla_fwd_tc_kernel<D, MODE, T, true>;
   // the dynamic shared-memory opt-in is per device: set it once for every device this process uses
   static std::atomic<bool> attr_set[kMaxDevices];
   const int dev = current_device();
@@ -716,7 +736,7 @@ cudaError_t tc_launch(const Problem& p, cudaStream_t st, bool main_pass) {
   cfg.attrs = pdl;
   cfg.numAttrs = 1;
   if (main_pass) {
-    cudaError_t le = cudaLaunchKernelEx(&cfg, kern, tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H, span);
+    cudaError_t le = cudaLaunchKernelEx(&cfg, kern, tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H, span, p.eps);
     if (le != cudaSuccess) return le;
   }
   if (!p.bounded) {
@@ -725,7 +745,7 @@ cudaError_t tc_launch(const Problem& p, cudaStream_t st, bool main_pass) {
     dim3 grid2((p.N + span2 - 1) / span2, slabs);
     cfg.gridDim = grid2;   // same attribute: resident behind the main kernel's tail, waits for its states
     cudaError_t le = cudaLaunchKernelEx(&cfg, kern_out, tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H,
-                                        span2);
+                                        span2, p.eps);
     if (le != cudaSuccess) return le;
   }
   return cudaGetLastError();
@@ -747,12 +767,14 @@ cudaError_t launch_forward_tc(const Problem& p, int dt, cudaStream_t st) {
     if (p.bounded) return cudaSuccess;
     main_pass = false;
   }
-  cudaError_t e;
-  if (p.d == 16)
-    e = (dt == SLA_F16) ? tc_launch<16, false, __half>(p, st, main_pass) : tc_launch<16, true, __nv_bfloat16>(p, st, main_pass);
-  else
-    e = (dt == SLA_F16) ? tc_launch<32, false, __half>(p, st, main_pass) : tc_launch<32, true, __nv_bfloat16>(p, st, main_pass);
-  return e;
+  // MODE = (bf16 ? 1 : 0) | (feature map << 1)
+  const bool relu = p.phi == SLA_PHI_RELU;
+  if (p.d == 16) {
+    if (dt == SLA_F16) return relu ? tc_launch<16, 2, __half>(p, st, main_pass) : tc_launch<16, 0, __half>(p, st, main_pass);
+    return relu ? tc_launch<16, 3, __nv_bfloat16>(p, st, main_pass) : tc_launch<16, 1, __nv_bfloat16>(p, st, main_pass);
+  }
+  if (dt == SLA_F16) return relu ? tc_launch<32, 2, __half>(p, st, main_pass) : tc_launch<32, 0, __half>(p, st, main_pass);
+  return relu ? tc_launch<32, 3, __nv_bfloat16>(p, st, main_pass) : tc_launch<32, 1, __nv_bfloat16>(p, st, main_pass);
 }
 
 }  // namespace sla

@@ -889,7 +889,7 @@ extern "C" int sla_debug_read_abort(int* host) {   // host[0..7]; also clears th
 #endif
 
 bool forward_umma_supported(const Problem& p, int dt) {
-  if (dt != SLA_F16) return false;
+  if (dt != SLA_F16 || p.phi != SLA_PHI_ELU1) return false;
   if (p.d != D || (p.H * p.d) % 128 != 0) return false;
   return encode_fn() != nullptr;
 }

@@ -36,6 +36,8 @@ struct Ctx {
   int x;       // channel inside the head
   int CB;      // threads per block
   bool active; // h < H
+  bool relu;   // feature map: false = elu(x)+1, true = max(x,0)
+  float eps;   // added to the denominator of Eq. 3 (0 for elu+1)
 };
 
 // S[p] += sum_j phi(k_j[h][p]) * v_j[h][x] ; z += sum_j phi(k_j[h][x])   over rows [r0,r1)
@@ -51,7 +53,7 @@ __device__ __forceinline__ void accumulate_state(const T* __restrict__ k, const 
       vv[i] = 0.f;
       if (i < nb && cx.active) {
         const size_t idx = (size_t)(base + i) * cx.C + cx.c;
-        const float b = phi_f32(Elem<T>::ld(k + idx));
+        const float b = phi_f32(Elem<T>::ld(k + idx), cx.relu);
         vv[i] = Elem<T>::ld(v + idx);
         bs[i * cx.CB + threadIdx.x] = b;
         z += b;
@@ -88,7 +90,7 @@ __device__ __forceinline__ void emit_output(const T* __restrict__ q, T* __restri
     for (int i = 0; i < RB; ++i) {
       aown[i] = 0.f;
       if (i < nb && cx.active) {
-        aown[i] = phi_f32(Elem<T>::ld(q + (size_t)(base + i) * cx.C + cx.c));
+        aown[i] = phi_f32(Elem<T>::ld(q + (size_t)(base + i) * cx.C + cx.c), cx.relu);
         bs[i * cx.CB + threadIdx.x] = aown[i];
       }
     }
@@ -106,7 +108,7 @@ __device__ __forceinline__ void emit_output(const T* __restrict__ q, T* __restri
           num = fmaf(a4.z, S[4 * p4 + 2], num);
           num = fmaf(a4.w, S[4 * p4 + 3], num);
         }
-        const float den = reduce_head<D>(aown[i] * z);
+        const float den = reduce_head<D>(aown[i] * z) + cx.eps;
         if (cx.active) Elem<T>::st(out + (size_t)(base + i) * cx.C + cx.c, num / den);
       }
     }
@@ -120,8 +122,10 @@ __device__ __forceinline__ float* state_slot(float* ws, int s, int H, int h) {
   return ws + kWsHeaderFloats + ((size_t)(s / (kFuseMax + 1)) * H + h) * (size_t)((D + 1) * D);
 }
 
-__device__ __forceinline__ Ctx make_ctx(int H, int D) {
+__device__ __forceinline__ Ctx make_ctx(int H, int D, int phi, float eps) {
   Ctx cx;
+  cx.relu = phi == SLA_PHI_RELU;
+  cx.eps = eps;
   cx.CB = blockDim.x;
   const int HB = cx.CB / D;
   cx.hl = threadIdx.x / D;
@@ -139,9 +143,9 @@ template <typename T, int D>
 __global__ void __launch_bounds__(256)
 sla_fwd_generic_kernel(const T* __restrict__ q, const T* __restrict__ k, const T* __restrict__ v,
                        const int32_t* __restrict__ off, T* __restrict__ out, float* __restrict__ ws,
-                       int N, int W, int H) {
+                       int N, int W, int H, int phi, float eps) {
   __shared__ __align__(16) float bs[RB * 256];
-  const Ctx cx = make_ctx(H, D);
+  const Ctx cx = make_ctx(H, D, phi, eps);
   const int h = cx.c / D;
   const int row0 = blockIdx.x * kTileRows;
   const int row1 = min(row0 + kTileRows, N);
@@ -177,10 +181,10 @@ sla_fwd_generic_kernel(const T* __restrict__ q, const T* __restrict__ k, const T
 template <typename T, int D>
 __global__ void __launch_bounds__(256)
 sla_fwd_generic_split_kernel(const T* __restrict__ q, const int32_t* __restrict__ off,
-                             T* __restrict__ out, const float* __restrict__ ws, int N, int W, int H) {
+                             T* __restrict__ out, const float* __restrict__ ws, int N, int W, int H, int phi, float eps) {
   __shared__ __align__(16) float bs[RB * 256];
   if (reinterpret_cast<const volatile int*>(ws)[0] == 0) return;   // no split window in this call
-  const Ctx cx = make_ctx(H, D);
+  const Ctx cx = make_ctx(H, D, phi, eps);
   const int h = cx.c / D;
   const int row0 = blockIdx.x * kTileRows;
   const int row1 = min(row0 + kTileRows, N);
@@ -240,7 +244,7 @@ __device__ __forceinline__ void backward_query_pass(const T* __restrict__ q, con
         const size_t idx = (size_t)(base + i) * cx.C + cx.c;
         qv[i] = Elem<T>::ld(q + idx);
         gv[i] = Elem<T>::ld(g + idx);
-        aown[i] = phi_f32(qv[i]);
+        aown[i] = phi_f32(qv[i], cx.relu);
         bsA[i * cx.CB + threadIdx.x] = aown[i];
       }
     }
@@ -259,7 +263,7 @@ __device__ __forceinline__ void backward_query_pass(const T* __restrict__ q, con
           num = fmaf(a4.z, Scol[4 * p4 + 2], num);
           num = fmaf(a4.w, Scol[4 * p4 + 3], num);
         }
-        const float den = reduce_head<D>(aown[i] * z);
+        const float den = reduce_head<D>(aown[i] * z) + cx.eps;
         const float inv = 1.f / den;
         const float o = num * inv;
         const float go = reduce_head<D>(gv[i] * o);
@@ -290,7 +294,7 @@ __device__ __forceinline__ void backward_query_pass(const T* __restrict__ q, con
         }
         dz = fmaf(dden[i], aown[i], dz);
         if (cx.active)
-          Elem<T>::st(dq + (size_t)(base + i) * cx.C + cx.c, da * dphi_f32(qv[i]));
+          Elem<T>::st(dq + (size_t)(base + i) * cx.C + cx.c, da * dphi_f32(qv[i], cx.relu));
       }
     }
     __syncthreads();
@@ -314,7 +318,7 @@ __device__ __forceinline__ void backward_key_pass(const T* __restrict__ k, const
       if (i < nb && cx.active) {
         const size_t idx = (size_t)(base + i) * cx.C + cx.c;
         kv[i] = Elem<T>::ld(k + idx);
-        bsA[i * cx.CB + threadIdx.x] = phi_f32(kv[i]);
+        bsA[i * cx.CB + threadIdx.x] = phi_f32(kv[i], cx.relu);
         bsB[i * cx.CB + threadIdx.x] = Elem<T>::ld(v + idx);
       }
     }
@@ -341,7 +345,7 @@ __device__ __forceinline__ void backward_key_pass(const T* __restrict__ k, const
         if (cx.active) {
           const size_t idx = (size_t)(base + i) * cx.C + cx.c;
           Elem<T>::st(dv + idx, dvx);
-          Elem<T>::st(dk + idx, db * dphi_f32(kv[i]));
+          Elem<T>::st(dk + idx, db * dphi_f32(kv[i], cx.relu));
         }
       }
     }
@@ -361,14 +365,14 @@ __global__ void __launch_bounds__(256)
 sla_bwd_generic_kernel(const T* __restrict__ q, const T* __restrict__ k, const T* __restrict__ v,
                        const T* __restrict__ g, const int32_t* __restrict__ off, T* __restrict__ dq,
                        T* __restrict__ dk, T* __restrict__ dv, float* __restrict__ ws, int N, int W,
-                       int H, int split_only) {
+                       int H, int split_only, int phi, float eps) {
   __shared__ __align__(16) float sm[BwdSmem<D>::kFloats];
   float* bsA = sm;
   float* bsB = sm + RB * 256;
   // split_only: the tensor-core kernel did every window <= kFuseMax rows and raised the workspace flag
   // if it met a longer one; here only those longer windows are accumulated
   if (split_only && reinterpret_cast<const volatile int*>(ws)[0] == 0) return;
-  const Ctx cx = make_ctx(H, D);
+  const Ctx cx = make_ctx(H, D, phi, eps);
   const int h = cx.c / D;
   const int row0 = blockIdx.x * kBwdTileRows;
   const int row1 = min(row0 + kBwdTileRows, N);
@@ -410,12 +414,12 @@ __global__ void __launch_bounds__(256)
 sla_bwd_generic_split_q_kernel(const T* __restrict__ q, const T* __restrict__ g,
                                const int32_t* __restrict__ off, T* __restrict__ dq,
                                const float* __restrict__ ws, float* __restrict__ wd, int N, int W,
-                               int H) {
+                               int H, int phi, float eps) {
   __shared__ __align__(16) float sm[2 * RB * 256];
   float* bsA = sm;
   float* bsB = sm + RB * 256;
   if (reinterpret_cast<const volatile int*>(ws)[0] == 0) return;   // no split window in this call
-  const Ctx cx = make_ctx(H, D);
+  const Ctx cx = make_ctx(H, D, phi, eps);
   const int h = cx.c / D;
   const int row0 = blockIdx.x * kBwdTileRows;
   const int row1 = min(row0 + kBwdTileRows, N);
@@ -449,12 +453,12 @@ __global__ void __launch_bounds__(256)
 sla_bwd_generic_split_kv_kernel(const T* __restrict__ k, const T* __restrict__ v,
                                 const int32_t* __restrict__ off, T* __restrict__ dk,
                                 T* __restrict__ dv, const float* __restrict__ wd,
-                                const float* __restrict__ ws, int N, int W, int H) {
+                                const float* __restrict__ ws, int N, int W, int H, int phi, float eps) {
   __shared__ __align__(16) float sm[2 * RB * 256];
   float* bsA = sm;
   float* bsB = sm + RB * 256;
   if (reinterpret_cast<const volatile int*>(ws)[0] == 0) return;   // no split window in this call
-  const Ctx cx = make_ctx(H, D);
+  const Ctx cx = make_ctx(H, D, phi, eps);
   const int h = cx.c / D;
   const int row0 = blockIdx.x * kBwdTileRows;
   const int row1 = min(row0 + kBwdTileRows, N);
@@ -488,10 +492,10 @@ cudaError_t fwd_launch(const Problem& p, cudaStream_t st) {
   const int HB = CB / D;
   dim3 grid((p.N + kTileRows - 1) / kTileRows, (p.H + HB - 1) / HB);
   sla_fwd_generic_kernel<T, D><<<grid, CB, 0, st>>>((const T*)p.q, (const T*)p.k, (const T*)p.v, p.off,
-                                                    (T*)p.out, p.ws_state, p.N, p.W, p.H);
+                                                    (T*)p.out, p.ws_state, p.N, p.W, p.H, p.phi, p.eps);
   if (!p.bounded)
     sla_fwd_generic_split_kernel<T, D><<<grid, CB, 0, st>>>((const T*)p.q, p.off, (T*)p.out, p.ws_state,
-                                                            p.N, p.W, p.H);
+                                                            p.N, p.W, p.H, p.phi, p.eps);
   return cudaGetLastError();
 }
 
@@ -502,13 +506,13 @@ cudaError_t bwd_launch(const Problem& p, cudaStream_t st, int split_only = 0) {
   dim3 grid((p.N + kBwdTileRows - 1) / kBwdTileRows, (p.H + HB - 1) / HB);
   sla_bwd_generic_kernel<T, D><<<grid, CB, 0, st>>>((const T*)p.q, (const T*)p.k, (const T*)p.v,
                                                     (const T*)p.g, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv,
-                                                    p.ws_state, p.N, p.W, p.H, split_only);
+                                                    p.ws_state, p.N, p.W, p.H, split_only, p.phi, p.eps);
   sla_bwd_generic_split_q_kernel<T, D><<<grid, CB, 0, st>>>((const T*)p.q, (const T*)p.g, p.off,
                                                             (T*)p.dq, p.ws_state, p.ws_dstate, p.N, p.W,
-                                                            p.H);
+                                                            p.H, p.phi, p.eps);
   sla_bwd_generic_split_kv_kernel<T, D><<<grid, CB, 0, st>>>((const T*)p.k, (const T*)p.v, p.off,
                                                              (T*)p.dk, (T*)p.dv, p.ws_dstate, p.ws_state, p.N,
-                                                             p.W, p.H);
+                                                             p.W, p.H, p.phi, p.eps);
   return cudaGetLastError();
 }
 

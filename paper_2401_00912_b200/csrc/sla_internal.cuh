@@ -32,8 +32,13 @@ template <> struct Elem<__nv_bfloat16> {
 
 // ---- feature map phi(x) = elu(x)+1 (reading A1; Eq. 3 cites [17]) and its derivative --
 // fp32 path: full-precision expf (the fp32 tolerance is 1e-5 relative).
-__device__ __forceinline__ float phi_f32(float x) { return x > 0.f ? x + 1.f : expf(x); }
-__device__ __forceinline__ float dphi_f32(float x) { return x > 0.f ? 1.f : expf(x); }
+// `relu` selects the second map ("Efficient Attn [3]"): phi(x) = max(x, 0).
+__device__ __forceinline__ float phi_f32(float x, bool relu) {
+  return relu ? fmaxf(x, 0.f) : (x > 0.f ? x + 1.f : expf(x));
+}
+__device__ __forceinline__ float dphi_f32(float x, bool relu) {
+  return relu ? (x > 0.f ? 1.f : 0.f) : (x > 0.f ? 1.f : expf(x));
+}
 
 // ---- window search: largest w in [0,W) with off[w] <= row  (off[0]=0 <= row < off[W]) -------------
 __device__ __forceinline__ int window_of_row(const int32_t* __restrict__ off, int W, int row) {
@@ -68,6 +73,8 @@ struct Problem {
   float* ws_state;   // [W,H,d+1,d] fp32 (S rows 0..d-1, z in row d) for split windows
   float* ws_dstate;  // [W,H,d+1,d] fp32 (dS, dz) for split windows (backward)
   int N, W, H, d;
+  int phi;           // sla_feature_map_t
+  float eps;         // added to the denominator (0 for SLA_PHI_ELU1)
   bool bounded;      // caller guarantees every window has <= kFuseMax rows: no workspace, no split pass
   bool tcgen05;      // main pass on the tcgen05 kernel (sla_fwd_umma.cu) instead of the mma.sync kernel
 };

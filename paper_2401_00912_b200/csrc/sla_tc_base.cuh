@@ -79,7 +79,9 @@ __device__ __forceinline__ float ex2_fast(float x) {
   return y;
 }
 __device__ __forceinline__ float dphi_fast(float x) { return ex2_fast(fminf(x * 1.4426950408889634f, 0.f)); }
-__device__ __forceinline__ float phi_fast(float x) { return fmaxf(x, 0.f) + dphi_fast(x); }
+// PHI = 0: elu(x)+1; PHI = 1: max(x, 0) (SLA_PHI_RELU)
+template <int PHI = 0>
+__device__ __forceinline__ float phi_fast(float x) { return PHI ? fmaxf(x, 0.f) : fmaxf(x, 0.f) + dphi_fast(x); }
 
 // phi on two packed I/O elements, evaluated in fp16x2 (long windows only: the operand is rounded to
 // fp16 anyway).  Branch-free on the FMA pipe (the ALU pipe is the busy one in these kernels):
@@ -89,10 +91,16 @@ __device__ __forceinline__ float phi_fast(float x) { return fmaxf(x, 0.f) + dphi
 //                                x  > 0: t is only the rounding residual of r, 2^t = 1 + t*ln2 + ..., so
 //                                        phi = 1 + x to first order in that residual (~1.5 fp16 ulp)
 // Result: fp16x2 {phi(x0), phi(x1)}.
-template <bool BF16>
+template <bool BF16, int PHI = 0>
 __device__ __forceinline__ uint32_t phi_h2(uint32_t raw) {
   uint32_t x = raw;
   if (BF16) { float2 f = unpack2<true>(raw); x = pack_h2(f.x, f.y); }
+  if (PHI) {   // max(x, 0): one fma.relu on the FMA pipe, no MUFU
+    uint32_t m;
+    const uint32_t one = 0x3C003C00u, zero = 0u;
+    asm("fma.rn.relu.f16x2 %0, %1, %2, %3;" : "=r"(m) : "r"(x), "r"(one), "r"(zero));
+    return m;
+  }
   uint32_t r, t, e, out;
   const uint32_t log2e = 0x3DC53DC5u, ln2 = 0x398C398Cu, zero = 0u;   // fp16 1.4424, 0.6931
   asm("fma.rn.relu.f16x2 %0, %1, %2, %3;" : "=r"(r) : "r"(x), "r"(log2e), "r"(zero));
@@ -126,9 +134,9 @@ __device__ __forceinline__ void split_h2(float x0, float x1, uint32_t& hi, uint3
 //
 // The tile's rows live in shared memory in the 128-byte-swizzled layout the TMA boxes have; the three
 // functors return the shared address of (tile row, 16-byte chunk of the slab row) of Q, K and V.
-template <int D, bool BF16, typename T, typename QA, typename KA, typename VA>
+template <int D, bool BF16, typename T, int PHI = 0, typename QA, typename KA, typename VA>
 __device__ __forceinline__ void quad_tile_core(QA qaddr, KA kaddr, VA vaddr, int hl, int nvalid, int wid,
-                                               T* __restrict__ out_rows, int C_total) {
+                                               T* __restrict__ out_rows, int C_total, float eps = 0.f) {
   const int lane = threadIdx.x & 31;
   const int g = lane >> 2, t = lane & 3;
   const int mi = lane >> 3;
@@ -148,9 +156,9 @@ __device__ __forceinline__ void quad_tile_core(QA qaddr, KA kaddr, VA vaddr, int
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
       float2 x = unpack2<BF16>(qr[perm[i]]);
-      split_h2(phi_fast(x.x), phi_fast(x.y), ahi[i], alo[i]);
+      split_h2(phi_fast<PHI>(x.x), phi_fast<PHI>(x.y), ahi[i], alo[i]);
       float2 y = unpack2<BF16>(kr[i]);
-      split_h2(phi_fast(y.x), phi_fast(y.y), bhi[i], blo[i]);
+      split_h2(phi_fast<PHI>(y.x), phi_fast<PHI>(y.y), bhi[i], blo[i]);
     }
     // K (non-transposed) as B operand: j-tile 0 -> (b0,b1) = (r0,r1); j-tile 1 -> (r2,r3)
 #pragma unroll
@@ -175,7 +183,7 @@ __device__ __forceinline__ void quad_tile_core(QA qaddr, KA kaddr, VA vaddr, int
     }
   rs0 += __shfl_xor_sync(0xffffffffu, rs0, 1); rs0 += __shfl_xor_sync(0xffffffffu, rs0, 2);
   rs1 += __shfl_xor_sync(0xffffffffu, rs1, 1); rs1 += __shfl_xor_sync(0xffffffffu, rs1, 2);
-  const float inv0 = (g < nvalid) ? fast_rcp(rs0) : 0.f, inv1 = (g + 8 < nvalid) ? fast_rcp(rs1) : 0.f;
+  const float inv0 = (g < nvalid) ? fast_rcp(rs0 + eps) : 0.f, inv1 = (g + 8 < nvalid) ? fast_rcp(rs1 + eps) : 0.f;
   // normalised weights as A operand (k = j): a0=(g,2t..) a1=(g+8,2t..) a2=(g,2t+8..) a3=(g+8,2t+8..)
   uint32_t phi_[4], plo_[4];
   split_h2(P[0][0] * inv0, P[0][1] * inv0, phi_[0], plo_[0]);

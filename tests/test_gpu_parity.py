@@ -215,6 +215,90 @@ def test_forward_tcgen05_unsupported_shapes():
             pkg.sla_forward(q, q, q, off, tcgen05=True)
 
 
+# ---- ReLU feature map with eps (sla_forward_phi / sla_backward_phi) ------------------
+RELU_EPS = 1e-6
+
+
+UNIT = {"f32": 2.0 ** -24, "f16": 2.0 ** -11, "bf16": 2.0 ** -8}
+
+
+def _relu_grad_amplification(q, k, v, g, offsets, eps):
+    """Forward-error scale of the ReLU map's gradients.  With max(x,0) the denominator a.z + eps can be arbitrarily
+    small, and dq = (dnum S^T + dden z) phi'(q) is then a difference of two large terms (for a length-1 window they
+    cancel to O(eps)): any arithmetic with unit roundoff u has an error of order u times the sum of the ABSOLUTE
+    values of the terms.  This returns that sum per element for dq, dk, dv (numpy, from the definition)."""
+    a, b = np.maximum(q, 0.0), np.maximum(k, 0.0)
+    amp_q, amp_k, amp_v = np.zeros_like(q), np.zeros_like(q), np.zeros_like(q)
+    for w in range(len(offsets) - 1):
+        s, e = int(offsets[w]), int(offsets[w + 1])
+        if e == s:
+            continue
+        S = np.einsum("jhp,jhr->hpr", b[s:e], np.abs(v[s:e]))        # |S| (b >= 0)
+        z = b[s:e].sum(0)                                             # [H,d]
+        Sv = np.einsum("jhp,jhr->hpr", b[s:e], v[s:e])
+        den = np.einsum("ihp,hp->ih", a[s:e], z) + eps                # [m,H]
+        o = np.einsum("ihp,hpr->ihr", a[s:e], Sv) / den[..., None]
+        dnum = np.abs(g[s:e]) / den[..., None]                        # |dnum|
+        dden = np.abs((g[s:e] * o).sum(-1)) / den                     # |dden|
+        amp_q[s:e] = np.einsum("ihr,hpr->ihp", dnum, S) + dden[..., None] * z[None]
+        dS = np.einsum("ihp,ihr->hpr", a[s:e], dnum)                  # |dS|
+        dz = np.einsum("ih,ihp->hp", dden, a[s:e])                    # |dz|
+        amp_k[s:e] = np.einsum("jhr,hpr->jhp", np.abs(v[s:e]), dS) + dz[None]
+        amp_v[s:e] = np.einsum("jhp,hpr->jhr", b[s:e], dS)
+    return amp_q, amp_k, amp_v
+
+
+def _relu_case(sc, backward=True):
+    torch = _torch()
+    q, k, v, g = sc.tensor("q"), sc.tensor("k"), sc.tensor("v"), sc.tensor("do")
+    off = torch.from_numpy(sc.offsets).cuda()
+    tq, tk, tv, tg = (to_dev(a, sc.dtype) for a in (q, k, v, g))
+    out = pkg.sla_forward(tq, tk, tv, off, phi="relu", eps=RELU_EPS)
+    torch.cuda.synchronize()
+    ref = sla_oracle.forward(q, k, v, sc.offsets, nthreads=8, phi="relu", eps=RELU_EPS)
+    check(f"{sc.name}.relu.out", out, ref, sc.dtype, sc.lengths)
+    if backward:
+        grads = pkg.sla_backward(tq, tk, tv, off, tg, phi="relu", eps=RELU_EPS)
+        torch.cuda.synchronize()
+        gref = sla_oracle.backward(q, k, v, g, sc.offsets, nthreads=8, phi="relu", eps=RELU_EPS)
+        amps = _relu_grad_amplification(*(x.astype(np.float64) for x in (q, k, v, g)), sc.offsets, RELU_EPS)
+        rtol, atol = TOL[sc.dtype]
+        for name, got, want, amp in zip(("dq", "dk", "dv"), grads, gref, amps):
+            gotd = got.double().cpu().numpy()
+            assert np.isfinite(gotd).all(), f"{sc.name}.relu.{name}: non-finite"
+            # the north-star tolerance plus the conditioning of the element itself (see _relu_grad_amplification)
+            err = np.abs(gotd - want) / (atol + rtol * np.abs(want) + 16 * UNIT[sc.dtype] * amp)
+            worst = np.unravel_index(np.argmax(err), err.shape)
+            assert err.max() <= 1.0, f"{sc.name}.relu.{name}: worst err/tol {err.max():.3f} at {worst} got {gotd[worst]} want {want[worst]} amp {amp[worst]}"
+
+
+@pytest.mark.parametrize("c", [0, 1, 3])
+def test_relu_forward_configs(c):
+    _relu_case(wl.make_config(c), backward=False)
+
+
+@pytest.mark.parametrize("layout", sorted(EDGE_LAYOUTS))
+@pytest.mark.parametrize("dtype,H,d", [("f32", 4, 32), ("f16", 8, 16), ("bf16", 8, 32), ("f16", 3, 16)])
+def test_relu_edge_layouts_forward_backward(layout, dtype, H, d):
+    _relu_case(wl.make_scene(EDGE_LAYOUTS[layout], H, d, dtype, seed=277 + len(layout), name=layout))
+
+
+def test_relu_zero_denominator_rows_and_errors():
+    """A query whose every channel is negative has phi(q) = 0: the output row is 0/(0+eps) = 0, finite."""
+    torch = _torch()
+    sc = wl.make_scene([1, 5, 40], 8, 16, "f16", seed=9)
+    q, k, v = sc.tensor("q").copy(), sc.tensor("k"), sc.tensor("v")
+    q[3] = -np.abs(q[3]) - 0.5
+    q[20] = -np.abs(q[20]) - 0.5
+    off = torch.from_numpy(sc.offsets).cuda()
+    out = pkg.sla_forward(to_dev(q, "f16"), to_dev(k, "f16"), to_dev(v, "f16"), off, phi="relu", eps=RELU_EPS)
+    assert torch.all(out[3] == 0) and torch.all(out[20] == 0) and torch.isfinite(out).all()
+    check("relu.zero_den", out, sla_oracle.forward(q, k, v, sc.offsets, phi="relu", eps=RELU_EPS), "f16", sc.lengths)
+    t = to_dev(q, "f16")
+    with pytest.raises(pkg.SlaError, match="INVALID_ARG"):
+        pkg.sla_forward(t, t, t, off, phi="relu", eps=-1.0)
+
+
 def test_n0_w0_and_errors():
     torch = _torch()
     q = torch.empty(0, 8, 16, dtype=torch.float16, device="cuda")
