@@ -14,8 +14,8 @@
 // Scaling: with m rows and s = 2^-ceil(log2 m), the operands use S' = s S, z' = s z, so den' = s den
 // and dnum' = g/den' = dnum/s stay O(1) in fp16; dS' = dS/s and dz' = dz/s are scaled back by s when
 // they become operands of pass C.  Windows of <= 32 rows use split fp16 operands (hi + lo).
-// Windows longer than kFuseMax rows are left to the generic kernels (a flag in the workspace header
-// tells them whether there is anything to do).
+// Windows longer than kFuseMax rows are left to the three split passes at the end of this file (a flag in the
+// workspace header tells them whether there is anything to do).
 #include <cuda.h>
 
 #include <atomic>
@@ -300,6 +300,140 @@ __device__ __forceinline__ void bwd_kv_out_tile(const RingView& rv, int hl, int 
   }
 }
 
+// ---- packed short windows: the backward of the masked quadratic form inside one 16-row tile ---------------------
+// Several WHOLE windows of <= 16 rows each, together <= 16 consecutive rows (the forward's packing).  With
+// P_ij = a_i.b_j masked to same-window pairs, r_i = sum_j P_ij, W = P / r, o_i = sum_j W_ij v_j (the
+// same function as Eq. 3) and g = dO:
+//   X_ij = g_i.v_j,   g_i.o_i = sum_j W_ij X_ij,   dP_ij = (X_ij - g_i.o_i) / r_i  (masked)
+//   dv_j = sum_i W_ij g_i,   da_i = sum_j dP_ij b_j,   db_j = sum_i dP_ij a_i,   dq = da phi'(q),  dk = db phi'(k)
+// a, b, W and dP are split into fp16 hi+lo operands (as in the forward's packed tiles); g and v are exact.
+// `wid` = window ordinal of tile row `lane` (lanes >= nvalid hold -1).
+__device__ __forceinline__ uint32_t movm_t(uint32_t x) {   // transpose of one 8x8 block of 16-bit elements
+  uint32_t y;
+  asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(y) : "r"(x));
+  return y;
+}
+template <bool BF16, typename T>
+__device__ __forceinline__ void bwd_quad_tile(const RingView& kv, const RingView& qg, int hl, int rel0, int nvalid,
+                                              int wid, T* __restrict__ dq_rows, T* __restrict__ dk_rows,
+                                              T* __restrict__ dv_rows, int C_total) {
+  const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+  int trow, csel;
+  lane_pattern(nvalid, trow, csel);
+  const int chunk = hl * 2 + csel;
+  const int perm[4] = {0, 2, 1, 3};   // ldmatrix register order -> A-fragment order
+  uint32_t rq[4], rk[4], rg[4], rv[4], tq[4], tk[4], tg[4];
+  ldsm_x4(ring_addr<D>(qg, C::KV_STAGE, 0, rel0 + trow, chunk), rq);
+  ldsm_x4(ring_addr<D>(qg, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), rg);
+  ldsm_x4(ring_addr<D>(kv, C::KV_STAGE, 0, rel0 + trow, chunk), rk);
+  ldsm_x4(ring_addr<D>(kv, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), rv);
+  ldsm_x4_t(ring_addr<D>(qg, C::KV_STAGE, 0, rel0 + trow, chunk), tq);
+  ldsm_x4_t(ring_addr<D>(qg, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), tg);
+  ldsm_x4_t(ring_addr<D>(kv, C::KV_STAGE, 0, rel0 + trow, chunk), tk);
+  // operands: a (A of P), b (B of P), aT (B of db), bT (B of da); derivative factors in the ldmatrix block order
+  uint32_t ah[4], al[4], bh[4], bl[4], ath[4], atl[4], bth[4], btl[4], gh[4], vh[4], gth[4];
+  float2 dpq[4], dpk[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    float2 a, b, x, da_, db_;
+    phi_pair<BF16>(rq[i], a, dpq[i]);
+    phi_pair<BF16>(rk[i], b, dpk[i]);
+    split_h2(a.x, a.y, ah[i], al[i]);
+    split_h2(b.x, b.y, bh[i], bl[i]);
+    phi_pair<BF16>(tq[i], x, da_);
+    split_h2(x.x, x.y, ath[i], atl[i]);
+    phi_pair<BF16>(tk[i], x, db_);
+    split_h2(x.x, x.y, bth[i], btl[i]);
+    if (BF16) {
+      float2 y = unpack2<true>(rg[i]); gh[i] = pack_h2(y.x, y.y);
+      y = unpack2<true>(rv[i]); vh[i] = pack_h2(y.x, y.y);
+      y = unpack2<true>(tg[i]); gth[i] = pack_h2(y.x, y.y);
+    } else { gh[i] = rg[i]; vh[i] = rv[i]; gth[i] = tg[i]; }
+  }
+  const uint32_t aH[4] = {ah[0], ah[2], ah[1], ah[3]}, aL[4] = {al[0], al[2], al[1], al[3]};
+  const uint32_t gA[4] = {gh[perm[0]], gh[perm[1]], gh[perm[2]], gh[perm[3]]};
+  // P[jt][c] and X[jt][c]: rows i = g (c<2) / g+8 (c>=2), columns j = 8 jt + 2t + (c&1)
+  float P[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}}, X[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+#pragma unroll
+  for (int jt = 0; jt < 2; ++jt) {
+    mma3<true>(P[jt], aH, aL, bh[2 * jt], bh[2 * jt + 1], bl[2 * jt], bl[2 * jt + 1]);
+    mma16816(X[jt], gA[0], gA[1], gA[2], gA[3], vh[2 * jt], vh[2 * jt + 1]);
+  }
+  const int wi0 = __shfl_sync(0xffffffffu, wid, g), wi1 = __shfl_sync(0xffffffffu, wid, g + 8);
+  float rs0 = 0.f, rs1 = 0.f;
+#pragma unroll
+  for (int jt = 0; jt < 2; ++jt)
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+      const int wj = __shfl_sync(0xffffffffu, wid, 8 * jt + 2 * t + c);
+      const bool m0 = wj == wi0 && wj >= 0, m1 = wj == wi1 && wj >= 0;
+      P[jt][c] = m0 ? P[jt][c] : 0.f;          X[jt][c] = m0 ? X[jt][c] : 0.f;
+      P[jt][2 + c] = m1 ? P[jt][2 + c] : 0.f;  X[jt][2 + c] = m1 ? X[jt][2 + c] : 0.f;
+      rs0 += P[jt][c];
+      rs1 += P[jt][2 + c];
+    }
+  rs0 += __shfl_xor_sync(0xffffffffu, rs0, 1); rs0 += __shfl_xor_sync(0xffffffffu, rs0, 2);
+  rs1 += __shfl_xor_sync(0xffffffffu, rs1, 1); rs1 += __shfl_xor_sync(0xffffffffu, rs1, 2);
+  const float inv0 = (g < nvalid) ? fast_rcp(rs0) : 0.f, inv1 = (g + 8 < nvalid) ? fast_rcp(rs1) : 0.f;
+  float go0 = 0.f, go1 = 0.f;                 // g_i . o_i = sum_j W_ij X_ij
+#pragma unroll
+  for (int jt = 0; jt < 2; ++jt)
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+      P[jt][c] *= inv0; P[jt][2 + c] *= inv1;             // W
+      go0 += P[jt][c] * X[jt][c];
+      go1 += P[jt][2 + c] * X[jt][2 + c];
+    }
+  go0 += __shfl_xor_sync(0xffffffffu, go0, 1); go0 += __shfl_xor_sync(0xffffffffu, go0, 2);
+  go1 += __shfl_xor_sync(0xffffffffu, go1, 1); go1 += __shfl_xor_sync(0xffffffffu, go1, 2);
+#pragma unroll
+  for (int jt = 0; jt < 2; ++jt)
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {               // dP (zero where W is zero: masked pairs)
+      X[jt][c] = (P[jt][c] != 0.f) ? (X[jt][c] - go0) * inv0 : 0.f;
+      X[jt][2 + c] = (P[jt][2 + c] != 0.f) ? (X[jt][2 + c] - go1) * inv1 : 0.f;
+    }
+  // A operands (k = j) of W and dP, and their transposes (m = j, k = i) by 8x8 block transposes
+  uint32_t wh[4], wl[4], ph[4], pl[4], wth[4], wtl[4], pth[4], ptl[4];
+#pragma unroll
+  for (int jt = 0; jt < 2; ++jt)
+#pragma unroll
+    for (int ib = 0; ib < 2; ++ib) {
+      split_h2(P[jt][2 * ib], P[jt][2 * ib + 1], wh[2 * jt + ib], wl[2 * jt + ib]);   // A index: a0=(g,jt0) a1=(g+8,jt0) a2=(g,jt1) a3=(g+8,jt1)
+      split_h2(X[jt][2 * ib], X[jt][2 * ib + 1], ph[2 * jt + ib], pl[2 * jt + ib]);
+    }
+  // block (ib, jt) sits at A index 2 jt + ib; its transpose is the block (jt, ib) of the transposed operand: index 2 ib + jt
+#pragma unroll
+  for (int jt = 0; jt < 2; ++jt)
+#pragma unroll
+    for (int ib = 0; ib < 2; ++ib) {
+      wth[2 * ib + jt] = movm_t(wh[2 * jt + ib]); wtl[2 * ib + jt] = movm_t(wl[2 * jt + ib]);
+      pth[2 * ib + jt] = movm_t(ph[2 * jt + ib]); ptl[2 * ib + jt] = movm_t(pl[2 * jt + ib]);
+    }
+#pragma unroll
+  for (int nt = 0; nt < 2; ++nt) {
+    // dv (rows j, cols r): A = W^T, B = g over rows i (transposed load): exact operand
+    float dv[4] = {0.f, 0.f, 0.f, 0.f}, da[4] = {0.f, 0.f, 0.f, 0.f}, db[4] = {0.f, 0.f, 0.f, 0.f};
+    mma16816(dv, wth[0], wth[1], wth[2], wth[3], gth[nt], gth[2 + nt]);
+    mma16816(dv, wtl[0], wtl[1], wtl[2], wtl[3], gth[nt], gth[2 + nt]);
+    // da (rows i, cols p): A = dP, B = b over rows j ; db (rows j, cols p): A = dP^T, B = a over rows i
+    mma3<true>(da, ph, pl, bth[nt], bth[2 + nt], btl[nt], btl[2 + nt]);
+    mma3<true>(db, pth, ptl, ath[nt], ath[2 + nt], atl[nt], atl[2 + nt]);
+    // derivative factors at (row g / g+8, channels 8 nt + 2t..): ldmatrix blocks (rowhalf, chalf = nt) = index 2*rowhalf + nt
+    const size_t o0 = (size_t)g * C_total + 8 * nt + 2 * t, o1 = (size_t)(g + 8) * C_total + 8 * nt + 2 * t;
+    if (g < nvalid) {
+      *reinterpret_cast<uint32_t*>(dv_rows + o0) = pack_out<BF16>(dv[0], dv[1]);
+      *reinterpret_cast<uint32_t*>(dq_rows + o0) = pack_out<BF16>(da[0] * dpq[nt].x, da[1] * dpq[nt].y);
+      *reinterpret_cast<uint32_t*>(dk_rows + o0) = pack_out<BF16>(db[0] * dpk[nt].x, db[1] * dpk[nt].y);
+    }
+    if (g + 8 < nvalid) {
+      *reinterpret_cast<uint32_t*>(dv_rows + o1) = pack_out<BF16>(dv[2], dv[3]);
+      *reinterpret_cast<uint32_t*>(dq_rows + o1) = pack_out<BF16>(da[2] * dpq[2 + nt].x, da[3] * dpq[2 + nt].y);
+      *reinterpret_cast<uint32_t*>(dk_rows + o1) = pack_out<BF16>(db[2] * dpk[2 + nt].x, db[3] * dpk[2 + nt].y);
+    }
+  }
+}
+
 // ---- one whole window: the three passes -------------------------------------------------------------
 template <bool BF16, bool PRECISE, typename T>
 __device__ __forceinline__ void bwd_window(RingView& kv, RingView& qg, RingView& kv2, int hl, int S0, int s,
@@ -435,7 +569,8 @@ sla_bwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   int wbase = ctrl.wa;
   int cur = __ldg(off + min(wbase + lane, W));
   int nxt = __ldg(off + min(wbase + 31 + lane, W));
-  for (int w = wbase; w < W; ++w) {
+  int w = wbase;
+  while (w < W) {
     int i = w - wbase;
     if (i >= 31) {
       wbase += 31;
@@ -446,22 +581,217 @@ sla_bwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     const int s = __shfl_sync(0xffffffffu, cur, i), e = __shfl_sync(0xffffffffu, cur, i + 1);
     if (s >= R1) break;
     const int m = e - s;
-    if (m <= 0) continue;
-    if (m > kFuseMax) {                                   // left to the generic kernels
+    if (m <= 0) { ++w; continue; }
+    if (m > kFuseMax) {                                   // left to the split passes
       if (hl == 0 && lane == 0) reinterpret_cast<volatile int*>(ws)[0] = 1;
+      ++w;
       continue;
     }
     const int mid = s + (m >> 1);
     if (mid >= R1) break;
-    if (mid < R0) continue;
+    if (mid < R0) { ++w; continue; }
+    if (m <= 16) {
+      // Pack the following whole short windows (owned, together <= 16 rows) into one 16-row tile, as the forward does:
+      // lane j holds off[wbase+j]; one ballot finds how many consecutive windows fit, one OR-reduction the bit mask of
+      // window starts inside the tile; the window ordinal of tile row r is a popcount of that mask.
+      const int e_j = __shfl_down_sync(0xffffffffu, cur, 1);      // off[wbase+lane+1]
+      const int mid_j = cur + ((e_j - cur) >> 1);
+      const bool fits = lane >= i && lane < 31 && (e_j - s) <= 16 && mid_j < R1;
+      const unsigned okm = __ballot_sync(0xffffffffu, fits) >> i;
+      const int cnt = __ffs(~okm) - 1;                            // consecutive windows that fit (>= 1)
+      const int rows = __shfl_sync(0xffffffffu, cur, i + cnt) - s;
+      const unsigned startbit = (lane > i && lane < i + cnt) ? (1u << (cur - s)) : 0u;
+      const unsigned starts = __reduce_or_sync(0xffffffffu, startbit) & 0xFFFEu;
+      const int wid = (lane < rows) ? __popc(starts & ((2u << lane) - 1u)) : -1;
+      w += cnt;
+      const int rel = s - S0;
+      ring_release_below<C::SR>(kv, rel);
+      ring_release_below<C::SR>(qg, rel);
+      ring_wait_upto(kv, (rel + rows - 1) / C::SR);
+      ring_wait_upto(qg, (rel + rows - 1) / C::SR);
+      bwd_quad_tile<BF16, T>(kv, qg, hl, rel, rows, wid, dq + hcol + (size_t)s * Ctot, dk + hcol + (size_t)s * Ctot,
+                             dv + hcol + (size_t)s * Ctot, Ctot);
+      ring_release_below<C::SR>(kv, rel + rows);
+      ring_release_below<C::SR>(qg, rel + rows);
+      ring_release_below<C::SR>(kv2, rel + rows);                 // the third stream carries these rows too
+      continue;
+    }
     if (m <= BWD_PRECISE_MAX)
       bwd_window<BF16, true, T>(kv, qg, kv2, hl, S0, s, e, dq + hcol, dk + hcol, dv + hcol, Ctot);
     else
       bwd_window<BF16, false, T>(kv, qg, kv2, hl, S0, s, e, dq + hcol, dk + hcol, dv + hcol, Ctot);
+    ++w;
   }
   ring_release_below<C::SR>(kv, total * C::SR);
   ring_release_below<C::SR>(qg, total * C::SR);
   ring_release_below<C::SR>(kv2, total * C::SR);
+}
+
+// ---- windows longer than kFuseMax rows: three stream-ordered passes over their pieces ----------------------------
+// A piece = the intersection of such a window with one row span.  PASS 0: partial S, z of the piece -> fp32 atomics into
+// the window's slot of ws_state.  PASS 1 (states complete): dq rows of the piece, partial dS, dz -> atomics into
+// ws_dstate.  PASS 2: dk, dv rows.  Same tiles as the fused windows (single fp16 operand: these windows are long), one
+// ring, one consumer warp per head.  A pass exits at once when the main kernel met no long window (workspace flag).
+__device__ __forceinline__ float* split_slot(float* ws, int s, int H, int h) {
+  return ws + kWsHeaderFloats + ((size_t)(s / (kFuseMax + 1)) * H + h) * (size_t)((D + 1) * D);
+}
+
+template <bool BF16, typename T, int PASS>
+__global__ void __launch_bounds__(Cfg<D>::THREADS, 2)
+sla_bwd_tc_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+                        const int32_t* __restrict__ off, T* __restrict__ dq, T* __restrict__ dk, T* __restrict__ dv,
+                        float* __restrict__ ws, float* __restrict__ wd, int N, int W, int H, int span) {
+  extern __shared__ uint8_t dyn_smem[];
+  __shared__ Ctrl ctrl;
+  if (reinterpret_cast<const volatile int*>(ws)[0] == 0) return;   // no long window in this call
+  const uint32_t ring = (smem_u32(dyn_smem) + 1023u) & ~1023u;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int R0 = blockIdx.x * span, R1 = min(R0 + span, N);
+  const int h0 = blockIdx.y * NW;
+  const int nheads = min(NW, H - h0);
+  const int Ctot = H * D;
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < NST; ++i) {
+      mbar_init(smem_u32(&ctrl.full[0][i]), 1);
+      mbar_init(smem_u32(&ctrl.empty[0][i]), nheads);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (warp >= NW) {   // producer: lane 0 streams the two tensors of this pass over the rows of the pieces
+    __syncthreads();
+    if (lane == 0) {
+      const uint32_t full = smem_u32(ctrl.full[0]), empty = smem_u32(ctrl.empty[0]);
+      const int S0 = ctrl.stream_begin;
+      const int total = (ctrl.stream_end - S0 + C::SR - 1) / C::SR;
+      for (int st = 0; st < total; ++st) {
+        if (st >= NST) mbar_wait(empty + 8u * (st % NST), (uint32_t)(((st / NST) - 1) & 1));
+        const uint32_t bar = full + 8u * (st % NST);
+        const uint32_t dst = ring + (st % NST) * C::KV_STAGE;
+        const int y = S0 + st * C::SR;
+        mbar_expect_tx(bar, (uint32_t)C::KV_STAGE);
+#pragma unroll
+        for (int b = 0; b < C::NBOX; ++b) {
+          const int x = h0 * D + 64 * b;
+          tma_load_2d(dst + b * C::BOX_BYTES, &tmA, bar, x, y);
+          tma_load_2d(dst + C::T_STAGE + b * C::BOX_BYTES, &tmB, bar, x, y);
+        }
+      }
+      for (int st = max(0, total - NST); st < total; ++st)
+        mbar_wait(full + 8u * (st % NST), (uint32_t)((st / NST) & 1));
+    }
+    return;
+  }
+  if (warp == 0) {
+    int wa, wl;
+    warp_windows_of_rows(off, W, R0, R1 - 1, wa, wl);
+    if (lane == 0) {
+      const int sa = __ldg(off + wa), ea = __ldg(off + wa + 1);
+      const int sl = __ldg(off + wl), el = __ldg(off + wl + 1);
+      // span <= kFuseMax: a long window that meets [R0,R1) holds R0 (window wa) or R1-1 (window wl)
+      const bool A = ea - sa > kFuseMax, B = el - sl > kFuseMax;
+      const int sb = A ? R0 : (B ? max(sl, R0) : R0);
+      const int se = B ? R1 : (A ? min(ea, R1) : sb);
+      ctrl.wa = wa;
+      ctrl.stream_begin = sb;
+      ctrl.stream_end = max(se, sb);
+    }
+  }
+  __syncthreads();
+  if (warp >= nheads) return;
+  const int hl = warp, g = lane >> 2, t = lane & 3;
+  const int S0 = ctrl.stream_begin;
+  const int total = (ctrl.stream_end - S0 + C::SR - 1) / C::SR;
+  RingView rv = make_ring(ring, smem_u32(ctrl.full[0]), smem_u32(ctrl.empty[0]));
+  const size_t hcol = (size_t)(h0 + hl) * D;
+  for (int w = ctrl.wa; w < W; ++w) {
+    const int s = __ldg(off + w), e = __ldg(off + w + 1);
+    if (s >= R1) break;
+    const int m = e - s;
+    if (m <= kFuseMax) continue;
+    const int ps = max(s, R0), pe = min(e, R1);
+    float* slot = split_slot(ws, s, H, h0 + hl);
+    float* dslot = split_slot(wd, s, H, h0 + hl);
+    const int lg = 32 - __clz(m - 1);
+    const float scale = __int_as_float((127 - lg) << 23);
+    BwdState st;
+    st.clear();
+    if (PASS == 0) {
+      for (int r = ps; r < pe; r += 16) {
+        const int nv = min(16, pe - r), rel = r - S0;
+        ring_release_below<C::SR>(rv, rel);
+        ring_wait_upto(rv, (rel + nv - 1) / C::SR);
+        bwd_kv_tile<BF16, false>(rv, hl, rel, nv, st);
+      }
+#pragma unroll
+      for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+        for (int c = 0; c < 4; ++c)      // S^T fragment: row r = g + 8 (c/2), column p = 8 nt + 2t + (c%2)
+          atomicAdd(slot + (8 * nt + 2 * t + (c & 1)) * D + g + 8 * (c >> 1), st.ST[nt][c]);
+      if (g == 0) {
+#pragma unroll
+        for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+          for (int c = 0; c < 2; ++c) atomicAdd(slot + D * D + 8 * nt + 2 * t + c, st.Z[nt][c]);
+      }
+    } else if (PASS == 1) {
+#pragma unroll
+      for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          st.ST[nt][c] = slot[(8 * nt + 2 * t + (c & 1)) * D + g + 8 * (c >> 1)];     // S^T[r][p] = S[p][r]
+          st.SS[nt][c] = slot[(g + 8 * (c >> 1)) * D + 8 * nt + 2 * t + (c & 1)];     // S[p][r]
+          st.Z[nt][c] = slot[D * D + 8 * nt + 2 * t + (c & 1)];
+        }
+      PassBOps ob;
+      make_ops<false>(st.ST, scale, ob.num);
+      make_ops<false>(st.SS, scale, ob.da);
+#pragma unroll
+      for (int b = 0; b < 2; ++b) {
+        ob.zs[b][0] = st.Z[b][0] * scale; ob.zs[b][1] = st.Z[b][1] * scale;
+        to_op<false>(ob.zs[b][0], ob.zs[b][1], ob.zh[b], ob.zl[b]);
+      }
+      for (int r = ps; r < pe; r += 16) {
+        const int nv = min(16, pe - r), rel = r - S0;
+        ring_release_below<C::SR>(rv, rel);
+        ring_wait_upto(rv, (rel + nv - 1) / C::SR);
+        bwd_q_tile<BF16, false, T>(rv, hl, rel, nv, ob, st, dq + hcol + (size_t)r * Ctot, Ctot);
+      }
+#pragma unroll
+      for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+        for (int c = 0; c < 4; ++c)      // dS fragment (scaled by 1/s): row p = g + 8 (c/2), column r = 8 nt + 2t + (c%2)
+          atomicAdd(dslot + (g + 8 * (c >> 1)) * D + 8 * nt + 2 * t + (c & 1), st.dSS[nt][c]);
+      if (g == 0) {
+#pragma unroll
+        for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+          for (int c = 0; c < 2; ++c) atomicAdd(dslot + D * D + 8 * nt + 2 * t + c, st.DZ[nt][c]);
+      }
+    } else {
+      PassCOps oc;
+#pragma unroll
+      for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          st.dST[nt][c] = dslot[(8 * nt + 2 * t + (c & 1)) * D + g + 8 * (c >> 1)];   // dS^T[r][p]
+          st.dSS[nt][c] = dslot[(g + 8 * (c >> 1)) * D + 8 * nt + 2 * t + (c & 1)];   // dS[p][r]
+          st.DZ[nt][c] = dslot[D * D + 8 * nt + 2 * t + (c & 1)];
+        }
+      make_ops<false>(st.dST, scale, oc.dv);
+      make_ops<false>(st.dSS, scale, oc.db);
+#pragma unroll
+      for (int b = 0; b < 2; ++b) { oc.dzs[b][0] = st.DZ[b][0] * scale; oc.dzs[b][1] = st.DZ[b][1] * scale; }
+      for (int r = ps; r < pe; r += 16) {
+        const int nv = min(16, pe - r), rel = r - S0;
+        ring_release_below<C::SR>(rv, rel);
+        ring_wait_upto(rv, (rel + nv - 1) / C::SR);
+        bwd_kv_out_tile<BF16, false, T>(rv, hl, rel, nv, oc, dk + hcol + (size_t)r * Ctot,
+                                        dv + hcol + (size_t)r * Ctot, Ctot);
+      }
+    }
+  }
+  ring_release_below<C::SR>(rv, total * C::SR);
 }
 
 template <bool BF16, typename T>
@@ -483,6 +813,26 @@ cudaError_t bwd_tc_launch(const Problem& p, cudaStream_t st) {
   dim3 grid((p.N + span - 1) / span, (p.H + NW - 1) / NW);
   kern<<<grid, C::THREADS, C::SMEM_DYN, st>>>(tq, tk, tv, tg, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state,
                                               p.N, p.W, p.H, span);
+  // windows longer than kFuseMax rows: three passes over their pieces (each exits at once if there is none)
+  auto k0 = sla_bwd_tc_split_kernel<BF16, T, 0>;
+  auto k1 = sla_bwd_tc_split_kernel<BF16, T, 1>;
+  auto k2 = sla_bwd_tc_split_kernel<BF16, T, 2>;
+  static std::atomic<bool> attr2_set[kMaxDevices];
+  if (!attr2_set[dev].load(std::memory_order_acquire)) {
+    cudaError_t e = cudaFuncSetAttribute(k0, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_DYN);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_DYN);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k2, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_DYN);
+    if (e != cudaSuccess) return e;
+    attr2_set[dev].store(true, std::memory_order_release);
+  }
+  const int span2 = 128;                                   // <= kFuseMax; few pieces per window = few atomics per slot
+  dim3 grid2((p.N + span2 - 1) / span2, (p.H + NW - 1) / NW);
+  k0<<<grid2, C::THREADS, C::SMEM_DYN, st>>>(tk, tv, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state, p.ws_dstate,
+                                             p.N, p.W, p.H, span2);
+  k1<<<grid2, C::THREADS, C::SMEM_DYN, st>>>(tq, tg, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state, p.ws_dstate,
+                                             p.N, p.W, p.H, span2);
+  k2<<<grid2, C::THREADS, C::SMEM_DYN, st>>>(tk, tv, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state, p.ws_dstate,
+                                             p.N, p.W, p.H, span2);
   return cudaGetLastError();
 }
 
@@ -495,12 +845,10 @@ bool backward_tc_supported(const Problem& p, int dt) {
   return encode_fn() != nullptr;
 }
 
-// Fused windows (<= kFuseMax rows) by the tensor-core kernel; longer windows by the generic kernels in
-// split-only mode (they exit at once unless the tensor-core kernel raised the workspace flag).
+// Fused windows (<= kFuseMax rows) by sla_bwd_tc_kernel; longer windows by the three sla_bwd_tc_split_kernel passes
+// (they exit at once unless the first kernel raised the workspace flag).
 cudaError_t launch_backward_tc(const Problem& p, int dt, cudaStream_t st) {
-  cudaError_t e = (dt == SLA_F16) ? bwd_tc_launch<false, __half>(p, st) : bwd_tc_launch<true, __nv_bfloat16>(p, st);
-  if (e != cudaSuccess) return e;
-  return launch_backward_generic_split_only(p, dt, st);
+  return (dt == SLA_F16) ? bwd_tc_launch<false, __half>(p, st) : bwd_tc_launch<true, __nv_bfloat16>(p, st);
 }
 
 }  // namespace sla

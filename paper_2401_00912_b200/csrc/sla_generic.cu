@@ -529,15 +529,6 @@ cudaError_t launch_forward_generic(const Problem& p, int dt, cudaStream_t st) {
   return fwd_launch<__nv_bfloat16, 32>(p, st);
 }
 
-cudaError_t launch_backward_generic_split_only(const Problem& p, int dt, cudaStream_t st) {
-  if (p.d == 16) {
-    if (dt == SLA_F16) return bwd_launch<__half, 16>(p, st, 1);
-    return bwd_launch<__nv_bfloat16, 16>(p, st, 1);
-  }
-  if (dt == SLA_F16) return bwd_launch<__half, 32>(p, st, 1);
-  return bwd_launch<__nv_bfloat16, 32>(p, st, 1);
-}
-
 cudaError_t launch_backward_generic(const Problem& p, int dt, cudaStream_t st) {
   if (p.d == 16) {
     if (dt == SLA_F32) return bwd_launch<float, 16>(p, st);

@@ -85,8 +85,6 @@ cudaError_t launch_zero(void* p, size_t bytes, cudaStream_t st);
 cudaError_t launch_offsets(const int32_t* win_id, int N, int W, int32_t* off, cudaStream_t st);
 cudaError_t launch_forward_generic(const Problem& p, int dt, cudaStream_t st);
 cudaError_t launch_backward_generic(const Problem& p, int dt, cudaStream_t st);
-// backward of windows longer than kFuseMax only (needs the workspace flag set by the tensor-core kernel)
-cudaError_t launch_backward_generic_split_only(const Problem& p, int dt, cudaStream_t st);
 bool backward_tc_supported(const Problem& p, int dt);
 cudaError_t launch_backward_tc(const Problem& p, int dt, cudaStream_t st);
 bool forward_tc_supported(const Problem& p, int dt);
