@@ -122,9 +122,9 @@ __device__ __forceinline__ float* state_slot(float* ws, int s, int H, int h) {
   return ws + kWsHeaderFloats + ((size_t)(s / (kFuseMax + 1)) * H + h) * (size_t)((D + 1) * D);
 }
 
-__device__ __forceinline__ Ctx make_ctx(int H, int D, int phi, float eps) {
+__device__ __forceinline__ Ctx make_ctx(int H, int D, bool relu, float eps) {
   Ctx cx;
-  cx.relu = phi == SLA_PHI_RELU;
+  cx.relu = relu;   // a compile-time constant of the calling kernel: the feature-map branches fold away
   cx.eps = eps;
   cx.CB = blockDim.x;
   const int HB = cx.CB / D;
@@ -139,13 +139,13 @@ __device__ __forceinline__ Ctx make_ctx(int H, int D, int phi, float eps) {
 
 // ------------------------------------------------------------------------------------------------
 // Forward, main kernel: fused whole windows + partial states of split windows.
-template <typename T, int D>
+template <typename T, int D, bool RELU>
 __global__ void __launch_bounds__(256)
 sla_fwd_generic_kernel(const T* __restrict__ q, const T* __restrict__ k, const T* __restrict__ v,
                        const int32_t* __restrict__ off, T* __restrict__ out, float* __restrict__ ws,
-                       int N, int W, int H, int phi, float eps) {
+                       int N, int W, int H, float eps) {
   __shared__ __align__(16) float bs[RB * 256];
-  const Ctx cx = make_ctx(H, D, phi, eps);
+  const Ctx cx = make_ctx(H, D, RELU, eps);
   const int h = cx.c / D;
   const int row0 = blockIdx.x * kTileRows;
   const int row1 = min(row0 + kTileRows, N);
@@ -178,13 +178,13 @@ sla_fwd_generic_kernel(const T* __restrict__ q, const T* __restrict__ k, const T
 }
 
 // Forward, second kernel: outputs of the pieces of split windows (state read from the workspace).
-template <typename T, int D>
+template <typename T, int D, bool RELU>
 __global__ void __launch_bounds__(256)
 sla_fwd_generic_split_kernel(const T* __restrict__ q, const int32_t* __restrict__ off,
-                             T* __restrict__ out, const float* __restrict__ ws, int N, int W, int H, int phi, float eps) {
+                             T* __restrict__ out, const float* __restrict__ ws, int N, int W, int H, float eps) {
   __shared__ __align__(16) float bs[RB * 256];
   if (reinterpret_cast<const volatile int*>(ws)[0] == 0) return;   // no split window in this call
-  const Ctx cx = make_ctx(H, D, phi, eps);
+  const Ctx cx = make_ctx(H, D, RELU, eps);
   const int h = cx.c / D;
   const int row0 = blockIdx.x * kTileRows;
   const int row1 = min(row0 + kTileRows, N);
@@ -360,19 +360,19 @@ template <int D> struct BwdSmem {
 };
 
 // Backward kernel 1: whole (fused) windows completely; partial states of split windows.
-template <typename T, int D>
+template <typename T, int D, bool RELU>
 __global__ void __launch_bounds__(256)
 sla_bwd_generic_kernel(const T* __restrict__ q, const T* __restrict__ k, const T* __restrict__ v,
                        const T* __restrict__ g, const int32_t* __restrict__ off, T* __restrict__ dq,
                        T* __restrict__ dk, T* __restrict__ dv, float* __restrict__ ws, int N, int W,
-                       int H, int split_only, int phi, float eps) {
+                       int H, int split_only, float eps) {
   __shared__ __align__(16) float sm[BwdSmem<D>::kFloats];
   float* bsA = sm;
   float* bsB = sm + RB * 256;
   // split_only: the tensor-core kernel did every window <= kFuseMax rows and raised the workspace flag
   // if it met a longer one; here only those longer windows are accumulated
   if (split_only && reinterpret_cast<const volatile int*>(ws)[0] == 0) return;
-  const Ctx cx = make_ctx(H, D, phi, eps);
+  const Ctx cx = make_ctx(H, D, RELU, eps);
   const int h = cx.c / D;
   const int row0 = blockIdx.x * kBwdTileRows;
   const int row1 = min(row0 + kBwdTileRows, N);
@@ -409,17 +409,17 @@ sla_bwd_generic_kernel(const T* __restrict__ q, const T* __restrict__ k, const T
 }
 
 // Backward kernel 2 (split windows only): dq of each piece, dS/dz partials into the workspace.
-template <typename T, int D>
+template <typename T, int D, bool RELU>
 __global__ void __launch_bounds__(256)
 sla_bwd_generic_split_q_kernel(const T* __restrict__ q, const T* __restrict__ g,
                                const int32_t* __restrict__ off, T* __restrict__ dq,
                                const float* __restrict__ ws, float* __restrict__ wd, int N, int W,
-                               int H, int phi, float eps) {
+                               int H, float eps) {
   __shared__ __align__(16) float sm[2 * RB * 256];
   float* bsA = sm;
   float* bsB = sm + RB * 256;
   if (reinterpret_cast<const volatile int*>(ws)[0] == 0) return;   // no split window in this call
-  const Ctx cx = make_ctx(H, D, phi, eps);
+  const Ctx cx = make_ctx(H, D, RELU, eps);
   const int h = cx.c / D;
   const int row0 = blockIdx.x * kBwdTileRows;
   const int row1 = min(row0 + kBwdTileRows, N);
@@ -448,17 +448,17 @@ sla_bwd_generic_split_q_kernel(const T* __restrict__ q, const T* __restrict__ g,
 }
 
 // Backward kernel 3 (split windows only): dk, dv of each piece.
-template <typename T, int D>
+template <typename T, int D, bool RELU>
 __global__ void __launch_bounds__(256)
 sla_bwd_generic_split_kv_kernel(const T* __restrict__ k, const T* __restrict__ v,
                                 const int32_t* __restrict__ off, T* __restrict__ dk,
                                 T* __restrict__ dv, const float* __restrict__ wd,
-                                const float* __restrict__ ws, int N, int W, int H, int phi, float eps) {
+                                const float* __restrict__ ws, int N, int W, int H, float eps) {
   __shared__ __align__(16) float sm[2 * RB * 256];
   float* bsA = sm;
   float* bsB = sm + RB * 256;
   if (reinterpret_cast<const volatile int*>(ws)[0] == 0) return;   // no split window in this call
-  const Ctx cx = make_ctx(H, D, phi, eps);
+  const Ctx cx = make_ctx(H, D, RELU, eps);
   const int h = cx.c / D;
   const int row0 = blockIdx.x * kBwdTileRows;
   const int row1 = min(row0 + kBwdTileRows, N);
@@ -486,33 +486,33 @@ inline int block_threads(int H, int D) {
   return c < 256 ? c : 256;
 }
 
-template <typename T, int D>
+template <typename T, int D, bool RELU>
 cudaError_t fwd_launch(const Problem& p, cudaStream_t st) {
   const int CB = block_threads(p.H, D);
   const int HB = CB / D;
   dim3 grid((p.N + kTileRows - 1) / kTileRows, (p.H + HB - 1) / HB);
-  sla_fwd_generic_kernel<T, D><<<grid, CB, 0, st>>>((const T*)p.q, (const T*)p.k, (const T*)p.v, p.off,
-                                                    (T*)p.out, p.ws_state, p.N, p.W, p.H, p.phi, p.eps);
+  sla_fwd_generic_kernel<T, D, RELU><<<grid, CB, 0, st>>>((const T*)p.q, (const T*)p.k, (const T*)p.v, p.off,
+                                                    (T*)p.out, p.ws_state, p.N, p.W, p.H, p.eps);
   if (!p.bounded)
-    sla_fwd_generic_split_kernel<T, D><<<grid, CB, 0, st>>>((const T*)p.q, p.off, (T*)p.out, p.ws_state,
-                                                            p.N, p.W, p.H, p.phi, p.eps);
+    sla_fwd_generic_split_kernel<T, D, RELU><<<grid, CB, 0, st>>>((const T*)p.q, p.off, (T*)p.out, p.ws_state,
+                                                            p.N, p.W, p.H, p.eps);
   return cudaGetLastError();
 }
 
-template <typename T, int D>
+template <typename T, int D, bool RELU>
 cudaError_t bwd_launch(const Problem& p, cudaStream_t st, int split_only = 0) {
   const int CB = block_threads(p.H, D);
   const int HB = CB / D;
   dim3 grid((p.N + kBwdTileRows - 1) / kBwdTileRows, (p.H + HB - 1) / HB);
-  sla_bwd_generic_kernel<T, D><<<grid, CB, 0, st>>>((const T*)p.q, (const T*)p.k, (const T*)p.v,
+  sla_bwd_generic_kernel<T, D, RELU><<<grid, CB, 0, st>>>((const T*)p.q, (const T*)p.k, (const T*)p.v,
                                                     (const T*)p.g, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv,
-                                                    p.ws_state, p.N, p.W, p.H, split_only, p.phi, p.eps);
-  sla_bwd_generic_split_q_kernel<T, D><<<grid, CB, 0, st>>>((const T*)p.q, (const T*)p.g, p.off,
+                                                    p.ws_state, p.N, p.W, p.H, split_only, p.eps);
+  sla_bwd_generic_split_q_kernel<T, D, RELU><<<grid, CB, 0, st>>>((const T*)p.q, (const T*)p.g, p.off,
                                                             (T*)p.dq, p.ws_state, p.ws_dstate, p.N, p.W,
-                                                            p.H, p.phi, p.eps);
-  sla_bwd_generic_split_kv_kernel<T, D><<<grid, CB, 0, st>>>((const T*)p.k, (const T*)p.v, p.off,
+                                                            p.H, p.eps);
+  sla_bwd_generic_split_kv_kernel<T, D, RELU><<<grid, CB, 0, st>>>((const T*)p.k, (const T*)p.v, p.off,
                                                              (T*)p.dk, (T*)p.dv, p.ws_dstate, p.ws_state, p.N,
-                                                             p.W, p.H, p.phi, p.eps);
+                                                             p.W, p.H, p.eps);
   return cudaGetLastError();
 }
 
@@ -520,24 +520,24 @@ cudaError_t bwd_launch(const Problem& p, cudaStream_t st, int split_only = 0) {
 
 cudaError_t launch_forward_generic(const Problem& p, int dt, cudaStream_t st) {
   if (p.d == 16) {
-    if (dt == SLA_F32) return fwd_launch<float, 16>(p, st);
-    if (dt == SLA_F16) return fwd_launch<__half, 16>(p, st);
-    return fwd_launch<__nv_bfloat16, 16>(p, st);
+    if (dt == SLA_F32) return p.phi == SLA_PHI_RELU ? fwd_launch<float, 16, true>(p, st) : fwd_launch<float, 16, false>(p, st);
+    if (dt == SLA_F16) return p.phi == SLA_PHI_RELU ? fwd_launch<__half, 16, true>(p, st) : fwd_launch<__half, 16, false>(p, st);
+    return p.phi == SLA_PHI_RELU ? fwd_launch<__nv_bfloat16, 16, true>(p, st) : fwd_launch<__nv_bfloat16, 16, false>(p, st);
   }
-  if (dt == SLA_F32) return fwd_launch<float, 32>(p, st);
-  if (dt == SLA_F16) return fwd_launch<__half, 32>(p, st);
-  return fwd_launch<__nv_bfloat16, 32>(p, st);
+  if (dt == SLA_F32) return p.phi == SLA_PHI_RELU ? fwd_launch<float, 32, true>(p, st) : fwd_launch<float, 32, false>(p, st);
+  if (dt == SLA_F16) return p.phi == SLA_PHI_RELU ? fwd_launch<__half, 32, true>(p, st) : fwd_launch<__half, 32, false>(p, st);
+  return p.phi == SLA_PHI_RELU ? fwd_launch<__nv_bfloat16, 32, true>(p, st) : fwd_launch<__nv_bfloat16, 32, false>(p, st);
 }
 
 cudaError_t launch_backward_generic(const Problem& p, int dt, cudaStream_t st) {
   if (p.d == 16) {
-    if (dt == SLA_F32) return bwd_launch<float, 16>(p, st);
-    if (dt == SLA_F16) return bwd_launch<__half, 16>(p, st);
-    return bwd_launch<__nv_bfloat16, 16>(p, st);
+    if (dt == SLA_F32) return p.phi == SLA_PHI_RELU ? bwd_launch<float, 16, true>(p, st) : bwd_launch<float, 16, false>(p, st);
+    if (dt == SLA_F16) return p.phi == SLA_PHI_RELU ? bwd_launch<__half, 16, true>(p, st) : bwd_launch<__half, 16, false>(p, st);
+    return p.phi == SLA_PHI_RELU ? bwd_launch<__nv_bfloat16, 16, true>(p, st) : bwd_launch<__nv_bfloat16, 16, false>(p, st);
   }
-  if (dt == SLA_F32) return bwd_launch<float, 32>(p, st);
-  if (dt == SLA_F16) return bwd_launch<__half, 32>(p, st);
-  return bwd_launch<__nv_bfloat16, 32>(p, st);
+  if (dt == SLA_F32) return p.phi == SLA_PHI_RELU ? bwd_launch<float, 32, true>(p, st) : bwd_launch<float, 32, false>(p, st);
+  if (dt == SLA_F16) return p.phi == SLA_PHI_RELU ? bwd_launch<__half, 32, true>(p, st) : bwd_launch<__half, 32, false>(p, st);
+  return p.phi == SLA_PHI_RELU ? bwd_launch<__nv_bfloat16, 32, true>(p, st) : bwd_launch<__nv_bfloat16, 32, false>(p, st);
 }
 
 }  // namespace sla
