@@ -134,7 +134,10 @@ int sla_backward(const void* q, const void* k, const void* v, const int32_t* win
  * memory and synchronises `stream` before returning.  Device scratch is taken from a stream-ordered
  * CUDA memory pool that the library creates per device on first use (unbounded release threshold, so
  * the block is reused by the next call instead of going back to the driver) and is returned to that
- * pool before the call ends.  This is the only entry that owns device memory; it lives until exit.
+ * pool before the call ends.  The scene is cut at window boundaries into up to four chunks; chunk c+1 is copied in while
+ * chunk c is computed and chunk c-1 is copied out, on two copy streams the library creates per device on first use
+ * (ordered against `stream` with events).  This is the only entry that owns device memory and streams; they live until
+ * exit.  win_id must be non-decreasing with every id in [0, W) (checked at the chunk boundaries only).
  *   q,k,v   HOST [N,H,d_h] of dt (pinned memory recommended)      win_id  HOST int32[N]
  *   out     HOST [N,H,d_h] of dt */
 int sla_forward_host(const void* q, const void* k, const void* v, const int32_t* win_id,

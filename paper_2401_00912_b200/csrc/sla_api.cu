@@ -204,6 +204,26 @@ cudaMemPool_t host_entry_pool() {
   }
   return pools[dev];
 }
+// Two copy streams per device for the host entry (host -> device, device -> host), created on first use and kept for the
+// life of the process like the pool.  Work on them is ordered against the caller's stream with events only.
+struct HostLanes { cudaStream_t in, out; };
+HostLanes* host_entry_lanes() {
+  static HostLanes lanes[64] = {};
+  static bool made[64] = {};
+  static std::mutex mu;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+  std::lock_guard<std::mutex> lock(mu);
+  if (!made[dev]) {
+    if (cudaStreamCreateWithFlags(&lanes[dev].in, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaStreamCreateWithFlags(&lanes[dev].out, cudaStreamNonBlocking) != cudaSuccess) {
+      (void)cudaGetLastError();
+      return nullptr;
+    }
+    made[dev] = true;
+  }
+  return &lanes[dev];
+}
 }  // namespace
 
 extern "C" {
@@ -215,33 +235,91 @@ int sla_forward_host(const void* q, const void* k, const void* v, const int32_t*
   if (N == 0 || W == 0) return SLA_OK;
   if (!q || !k || !v || !win_id || !out) return SLA_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
-  const size_t tb = (size_t)N * H * d_h * esize(dt);           // bytes per tensor
+  const size_t row = (size_t)H * d_h * esize(dt);              // bytes per row of one tensor
+  const size_t tb = (size_t)N * row;
   const size_t tb_al = (tb + 255) / 256 * 256;
   const size_t ids_al = ((size_t)N * 4 + 255) / 256 * 256;
-  const size_t off_al = ((size_t)(W + 1) * 4 + 255) / 256 * 256;
+  // The scene is cut at window boundaries into up to kHostChunks chunks of about equal row count (host-side scan of the
+  // ids, integers only).  Chunk c+1 travels host -> device while chunk c is computed and chunk c-1 travels back: the two
+  // directions of the link are independent, so the copy out hides behind the copy in.
+  constexpr int kHostChunks = 4;
+  int64_t cut[kHostChunks + 1];
+  int nch = 0;
+  cut[0] = 0;
+  const int want = N >= 16384 ? kHostChunks : 1;
+  for (int c = 1; c < want; ++c) {
+    int64_t r = N * c / want;
+    if (r <= cut[nch]) continue;
+    while (r < N && win_id[r] == win_id[r - 1]) ++r;           // move the cut to the next window boundary
+    if (r >= N) break;
+    cut[++nch] = r;
+  }
+  cut[++nch] = N;
+  size_t off_al = 0;                                           // local offsets of all chunks, back to back
+  int32_t w0[kHostChunks], wc[kHostChunks];
+  for (int c = 0; c < nch; ++c) {
+    w0[c] = win_id[cut[c]];
+    wc[c] = win_id[cut[c + 1] - 1] - w0[c] + 1;
+    if (w0[c] < 0 || wc[c] < 1 || (int64_t)w0[c] + wc[c] > W) return SLA_ERR_INVALID_ARG;   // ids not sorted in [0, W)
+    off_al += ((size_t)(wc[c] + 1) * 4 + 255) / 256 * 256;
+  }
   const size_t ws = state_bytes(N, H, d_h);
-  char* base = nullptr;
+  HostLanes* lanes = host_entry_lanes();
   cudaMemPool_t pool = host_entry_pool();
+  if (!lanes) return SLA_ERR_CUDA;
+  char* base = nullptr;
   const size_t total = 4 * tb_al + ids_al + off_al + ws;
   const cudaError_t ae = pool ? cudaMallocFromPoolAsync(reinterpret_cast<void**>(&base), total, pool, st)
                               : cudaMallocAsync(reinterpret_cast<void**>(&base), total, st);
   if (ae != cudaSuccess) return SLA_ERR_CUDA;
   char* dq_ = base; char* dk_ = base + tb_al; char* dv_ = base + 2 * tb_al; char* do_ = base + 3 * tb_al;
   int32_t* dids = reinterpret_cast<int32_t*>(base + 4 * tb_al);
-  int32_t* doff = reinterpret_cast<int32_t*>(base + 4 * tb_al + ids_al);
+  char* doff = base + 4 * tb_al + ids_al;
   void* dws = base + 4 * tb_al + ids_al + off_al;
-  bool ok = true;
-  ok = ok && cudaMemcpyAsync(dids, win_id, (size_t)N * 4, cudaMemcpyHostToDevice, st) == cudaSuccess;
-  ok = ok && cudaMemcpyAsync(dk_, k, tb, cudaMemcpyHostToDevice, st) == cudaSuccess;
-  ok = ok && cudaMemcpyAsync(dv_, v, tb, cudaMemcpyHostToDevice, st) == cudaSuccess;
-  ok = ok && cudaMemcpyAsync(dq_, q, tb, cudaMemcpyHostToDevice, st) == cudaSuccess;
-  if (ok) rc = sla_offsets_from_window_ids(dids, N, W, doff, stream);
-  if (ok && rc == SLA_OK)
-    rc = sla_forward(dq_, dk_, dv_, doff, N, W, H, d_h, dt, do_, dws, ws, stream);
-  ok = ok && rc == SLA_OK;
-  ok = ok && cudaMemcpyAsync(out, do_, tb, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+  cudaEvent_t ev_start = nullptr, ev_in[kHostChunks] = {}, ev_done[kHostChunks] = {}, ev_out = nullptr;
+  bool ok = cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming) == cudaSuccess &&
+            cudaEventCreateWithFlags(&ev_out, cudaEventDisableTiming) == cudaSuccess;
+  for (int c = 0; c < nch && ok; ++c)
+    ok = cudaEventCreateWithFlags(&ev_in[c], cudaEventDisableTiming) == cudaSuccess &&
+         cudaEventCreateWithFlags(&ev_done[c], cudaEventDisableTiming) == cudaSuccess;
+  // the copy lanes start after whatever precedes this call on the caller's stream (and after the allocation)
+  ok = ok && cudaEventRecord(ev_start, st) == cudaSuccess && cudaStreamWaitEvent(lanes->in, ev_start, 0) == cudaSuccess &&
+       cudaStreamWaitEvent(lanes->out, ev_start, 0) == cudaSuccess;
+  for (int c = 0; c < nch && ok; ++c) {                        // lane "in": host -> device, chunk by chunk
+    const int64_t r0 = cut[c], n = cut[c + 1] - cut[c];
+    ok = ok && cudaMemcpyAsync(dids + r0, win_id + r0, (size_t)n * 4, cudaMemcpyHostToDevice, lanes->in) == cudaSuccess;
+    ok = ok && cudaMemcpyAsync(dk_ + r0 * row, (const char*)k + r0 * row, n * row, cudaMemcpyHostToDevice, lanes->in) == cudaSuccess;
+    ok = ok && cudaMemcpyAsync(dv_ + r0 * row, (const char*)v + r0 * row, n * row, cudaMemcpyHostToDevice, lanes->in) == cudaSuccess;
+    ok = ok && cudaMemcpyAsync(dq_ + r0 * row, (const char*)q + r0 * row, n * row, cudaMemcpyHostToDevice, lanes->in) == cudaSuccess;
+    ok = ok && cudaEventRecord(ev_in[c], lanes->in) == cudaSuccess;
+  }
+  size_t off_pos = 0;
+  for (int c = 0; c < nch && ok && rc == SLA_OK; ++c) {        // caller's stream: prep + forward of chunk c
+    const int64_t r0 = cut[c], n = cut[c + 1] - cut[c];
+    int32_t* off_c = reinterpret_cast<int32_t*>(doff + off_pos);
+    off_pos += ((size_t)(wc[c] + 1) * 4 + 255) / 256 * 256;
+    ok = ok && cudaStreamWaitEvent(st, ev_in[c], 0) == cudaSuccess;
+    ok = ok && sla::launch_offsets(dids + r0, (int)n, wc[c], off_c, st, w0[c]) == cudaSuccess;
+    if (ok) rc = sla_forward(dq_ + r0 * row, dk_ + r0 * row, dv_ + r0 * row, off_c, n, wc[c], H, d_h, dt, do_ + r0 * row,
+                             dws, ws, stream);
+    ok = ok && cudaEventRecord(ev_done[c], st) == cudaSuccess;
+    // lane "out": device -> host as soon as the chunk is done
+    ok = ok && cudaStreamWaitEvent(lanes->out, ev_done[c], 0) == cudaSuccess;
+    ok = ok && cudaMemcpyAsync((char*)out + r0 * row, do_ + r0 * row, n * row, cudaMemcpyDeviceToHost, lanes->out) == cudaSuccess;
+  }
+  // join the lanes back into the caller's stream before the block goes back to the pool
+  if (ev_out && cudaEventRecord(ev_out, lanes->out) == cudaSuccess) cudaStreamWaitEvent(st, ev_out, 0);
+  else cudaStreamSynchronize(lanes->out);
+  if (ev_start && cudaEventRecord(ev_start, lanes->in) == cudaSuccess) cudaStreamWaitEvent(st, ev_start, 0);
+  else cudaStreamSynchronize(lanes->in);
   cudaFreeAsync(base, st);
   if (cudaStreamSynchronize(st) != cudaSuccess) ok = false;
+  if (ev_start) cudaEventDestroy(ev_start);
+  if (ev_out) cudaEventDestroy(ev_out);
+  for (int c = 0; c < kHostChunks; ++c) {
+    if (ev_in[c]) cudaEventDestroy(ev_in[c]);
+    if (ev_done[c]) cudaEventDestroy(ev_done[c]);
+  }
   if (rc != SLA_OK) return rc;
   return ok ? SLA_OK : SLA_ERR_CUDA;
 }

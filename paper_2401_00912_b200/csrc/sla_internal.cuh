@@ -82,7 +82,7 @@ struct Problem {
 // Launchers (defined in the .cu files); all enqueue on `st` and return the last CUDA error.
 // zero `bytes` bytes (16-byte aligned) with a kernel that takes part in programmatic dependent launch
 cudaError_t launch_zero(void* p, size_t bytes, cudaStream_t st);
-cudaError_t launch_offsets(const int32_t* win_id, int N, int W, int32_t* off, cudaStream_t st);
+cudaError_t launch_offsets(const int32_t* win_id, int N, int W, int32_t* off, cudaStream_t st, int id_base = 0);
 cudaError_t launch_forward_generic(const Problem& p, int dt, cudaStream_t st);
 cudaError_t launch_backward_generic(const Problem& p, int dt, cudaStream_t st);
 bool backward_tc_supported(const Problem& p, int dt);

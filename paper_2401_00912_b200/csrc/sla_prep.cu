@@ -12,7 +12,7 @@ namespace sla {
 namespace {
 
 __global__ void __launch_bounds__(256)
-sla_offsets_kernel(const int32_t* __restrict__ win_id, int N, int W, int32_t* __restrict__ off) {
+sla_offsets_kernel(const int32_t* __restrict__ win_id, int N, int W, int32_t* __restrict__ off, int id_base) {
   // Programmatic dependent launch: a following kernel that opted in (sla_fwd_tc_kernel) may become
   // resident now; it still waits for this whole grid (griddepcontrol.wait) before it reads `off`.
   asm volatile("griddepcontrol.launch_dependents;");
@@ -20,8 +20,9 @@ sla_offsets_kernel(const int32_t* __restrict__ win_id, int N, int W, int32_t* __
   if (i64 > N) return;
   const int i = (int)i64;
   // ids outside [0, W) violate the precondition; clamp so that they can never write out of bounds
-  const int lo = (i == 0) ? 0 : max(0, min(W, __ldg(win_id + i - 1)) + 1);
-  const int hi = (i == N) ? W : min(W, __ldg(win_id + i));
+  // id_base: the ids are window indices of a longer scene; this call covers windows id_base .. id_base+W-1 of it
+  const int lo = (i == 0) ? 0 : max(0, min(W, __ldg(win_id + i - 1) - id_base) + 1);
+  const int hi = (i == N) ? W : max(-1, min(W, __ldg(win_id + i) - id_base));
   for (int w = lo; w <= hi; ++w) off[w] = i;
 }
 
@@ -97,10 +98,10 @@ cudaError_t launch_stream_ceiling(const void* a, const void* b, const void* c, v
   return cudaGetLastError();
 }
 
-cudaError_t launch_offsets(const int32_t* win_id, int N, int W, int32_t* off, cudaStream_t st) {
+cudaError_t launch_offsets(const int32_t* win_id, int N, int W, int32_t* off, cudaStream_t st, int id_base) {
   const int threads = 256;
   const unsigned blocks = (unsigned)(((long long)N + 1 + threads - 1) / threads);
-  sla_offsets_kernel<<<blocks, threads, 0, st>>>(win_id, N, W, off);
+  sla_offsets_kernel<<<blocks, threads, 0, st>>>(win_id, N, W, off, id_base);
   return cudaGetLastError();
 }
 
