@@ -53,8 +53,12 @@ constexpr int NSL = 2;                      // TMEM regions of 256 columns (stat
 constexpr int NB = 3;                       // B operand buffers (2 tiles of 4 heads x 32 rows = 8 KB)
 constexpr int NIT = 16;                     // item descriptor ring
 constexpr int KVC = 4;                      // tiles per K/V chunk (Q chunks are MMA blocks of up to 8 tiles)
-constexpr int NPHI = 8, NCONV = 4, NEPI = 8;
-constexpr int WARP_WALK = 0, WARP_QLOAD = 1, WARP_SMMA = 2, WARP_ZMMA = 3, WARP_OMMA = 4, WARP_PHI0 = 5,
+#ifndef SLA_NEPI
+#define SLA_NEPI 4
+#endif
+constexpr int NPHI = 8, NCONV = 4, NEPI = SLA_NEPI;      // NEPI = 4: each epilogue warp stores all 8 heads of its 32 rows
+constexpr int EPI_HALVES = 8 / NEPI;
+constexpr int WARP_WALK = 0, WARP_QLOAD = 1, WARP_SMMA = 2, WARP_OMMA = 3, WARP_PHI0 = 4,
               WARP_CONV0 = WARP_PHI0 + NPHI, WARP_EPI0 = WARP_CONV0 + NCONV, NWARPS = WARP_EPI0 + NEPI;
 constexpr int THREADS = NWARPS * 32;
 constexpr int NREADERS = NWARPS - 1;        // every warp but the walk warp reads the item ring
@@ -284,7 +288,7 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
     const int t = threadIdx.x;
     if (t < NIT) { mbar_init(smem_u32(&ctrl.item_full[t]), 1); mbar_init(smem_u32(&ctrl.item_empty[t]), NREADERS); }
     if (t < NKV) {
-      mbar_init(smem_u32(&ctrl.kv_full[t]), 1); mbar_init(smem_u32(&ctrl.kphi[t]), 8); mbar_init(smem_u32(&ctrl.kv_empty[t]), 2);
+      mbar_init(smem_u32(&ctrl.kv_full[t]), 1); mbar_init(smem_u32(&ctrl.kphi[t]), 8); mbar_init(smem_u32(&ctrl.kv_empty[t]), 1);
       ctrl.kv_owner[t] = -1;
     }
     if (t < NQT) {
@@ -292,7 +296,7 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
       ctrl.q_owner[t] = -1;
     }
     if (t < NSL) {
-      mbar_init(smem_u32(&ctrl.state_full[t]), 2); mbar_init(smem_u32(&ctrl.region_free[t]), NEPI);
+      mbar_init(smem_u32(&ctrl.state_full[t]), 1); mbar_init(smem_u32(&ctrl.region_free[t]), NEPI);
       mbar_init(smem_u32(&ctrl.o_full[t]), 1); mbar_init(smem_u32(&ctrl.o_drained[t]), NEPI);
     }
     if (t < NB) { mbar_init(smem_u32(&ctrl.b_full[t]), NCONV); mbar_init(smem_u32(&ctrl.b_empty[t]), 1); }
@@ -502,9 +506,8 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
         qr.used(first);
       }
     }
-  } else if (warp == WARP_SMMA || warp == WARP_ZMMA) {
+  } else if (warp == WARP_SMMA) {
     // =========================== state MMA issuers: D += V^T phi(K)  |  Z += phi(K)^T 1 ===========================
-    const bool zrole = warp == WARP_ZMMA;
     Cur it{0, 0}, rg{0, 0};
     TileRing<NKV> kr{0, 0u};
     constexpr uint32_t ID_STATE = make_idesc(128, 128, true, true, BF16, false);   // A = V (I/O dtype), B = phi(K) fp16
@@ -531,8 +534,8 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
             const uint32_t kt = sbase + OFF_K + (first + j) * 2048;
             const uint64_t dk = make_desc(kt, KV_REG, 1024);
             const uint32_t acc = (c | j) ? 1u : 0u;
-            if (zrole) umma(region + 128, dk, dones, ID_Z, acc);
-            else umma(region, make_desc(kt + (OFF_V - OFF_K), KV_REG, 1024), dk, ID_STATE, acc);
+            umma(region, make_desc(kt + (OFF_V - OFF_K), KV_REG, 1024), dk, ID_STATE, acc);
+            umma(region + 128, dk, dones, ID_Z, acc);
           }
           umma_commit(smem_u32(&ctrl.kv_empty[first]));
         }
@@ -630,7 +633,7 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
                                      out + (size_t)d.y * Ctot + col0 + pw * D, Ctot);
         asm volatile("bar.sync 1, %0;" ::"n"(NPHI * 32) : "memory");   // every head is done with the tiles
         if (tid_g == 0) {
-          mbar_arrive_n(smem_u32(&ctrl.kv_empty[kt]), 2);
+          mbar_arrive_n(smem_u32(&ctrl.kv_empty[kt]), 1);
           mbar_arrive_n(smem_u32(&ctrl.q_empty[qt]), NEPI);
         }
         kr.used(kt);
@@ -732,11 +735,10 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
   } else {
     // =========================== epilogue: one thread per output row ===========================
     const int ew = warp - WARP_EPI0;
-    const int quad = warp & 3, half = ew >> 2;           // TMEM lane quadrant; which 4 heads (64 channels) this warp stores
+    const int quad = warp & 3;                           // TMEM lane quadrant of this warp
     Cur it{0, 0}, rg{0, 0};
     TileRing<NQT> qr{0, 0u};
     uint32_t of_ph = 0;                                  // parity of the next o_full completion, per region
-    const uint32_t stage0 = sbase + OFF_Q + half * Q_REG;   // this warp stages its rows in its half of the dead Q tiles
     while (true) {
       const int4 d = next_item(it);
       if (d.x == IT_END) break;
@@ -754,6 +756,10 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
         tc_fence_after();
         LOG(61, s + 128 * b);
         if (32 * quad < rows) {
+#pragma unroll 1
+         for (int hf = 0; hf < EPI_HALVES; ++hf) {
+          const int half = EPI_HALVES == 2 ? hf : (ew >> 2);   // which 4 heads (64 channels)
+          const uint32_t stage0 = sbase + OFF_Q + half * Q_REG;   // staging: this half of the (now dead) Q tiles
           const uint32_t taddr = region + ((uint32_t)(32 * quad) << 16) + 128 * half;
           const int rib = 32 * quad + lane;              // row of the block this thread owns
           const uint32_t srow = stage0 + (first + (rib >> 4)) * 2048 + (rib & 15) * 128;
@@ -802,6 +808,7 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
             if (row < nr) *reinterpret_cast<uint4*>(obase + (size_t)row * Ctot) = x[i];
           }
           LOG(65, 0);
+         }
           proxy_fence();
           LOG(66, 0);                                 // the tiles go back to the TMA loader
         }
