@@ -99,7 +99,7 @@ int sla_backward_phi(const void* q, const void* k, const void* v, const int32_t*
  * the 5th-generation tensor cores (tcgen05.mma, accumulators in tensor memory; csrc/sla_fwd_umma.cu): all heads of a
  * 128-channel slab in one MMA per 16 rows.  Supported: dt = SLA_F16, d_h = 16, H*d_h a multiple of 128; anything
  * else -> SLA_ERR_UNSUPPORTED.  It is parity-tested like sla_forward but slower on the measured scenes (DESIGN.md
- * 5.8), so sla_forward does not route to it. */
+ * 5.7), so sla_forward does not route to it. */
 int sla_forward_tcgen05(const void* q, const void* k, const void* v, const int32_t* window_offsets,
                         int64_t N, int32_t W, int32_t H, int32_t d_h, int dt, void* out,
                         void* workspace, size_t workspace_bytes, sla_stream_t stream);

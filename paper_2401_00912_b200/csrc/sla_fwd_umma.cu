@@ -4,7 +4,7 @@
 // What is computed (Eq. 2-3): per window w and head h
 //     S = sum_j phi(k_j)^T v_j,   z = sum_j phi(k_j),   o_i = phi(q_i) S / (phi(q_i) . z).
 //
-// Design:
+// Design (parity-tested entry sla_forward_tcgen05, not the default path):
 //   * One persistent CTA per SM; the flat window-sorted matrix is cut into one row span per CTA
 //     (load balance by rows, Fig. 3a).  A CTA owns every window of <= kFuseMax rows whose middle
 //     row lies in its span, and the pieces of longer windows that intersect it (partial state -> fp32 atomics
@@ -15,12 +15,12 @@
 //              meet the tolerance on windows this short;
 //       WIN    one window of 17..kFuseMax rows;
 //       PIECE  the part of a longer window inside this span (state only).
-//     Rows travel in CHUNKS of up to 8 tiles of 16 rows (one chunk = one MMA block of up to 128 rows of one
-//     item): the walk warp loads K,V chunks, a second loader warp Q chunks, with 2-D TMA boxes of 64 channels
-//     x 16/32/64/128 rows (128-byte swizzle) into tile rings; a chunk never wraps around its ring.
-//   * phi warps (one whole 16-row tile per warp, tiles dealt round-robin) apply phi to K and Q tiles IN PLACE
+//     Rows travel in CHUNKS of one item: the walk warp loads K,V chunks of <= 4 tiles of 16 rows, a second loader
+//     warp Q chunks of <= 8 tiles (one MMA block of up to 128 rows), with 2-D TMA boxes of 64 channels x
+//     16/32/64/128 rows (128-byte swizzle) into tile rings; a chunk never wraps around its ring.
+//   * 8 phi warps (one 16-byte chunk of every tile of the chunk per thread) apply phi to K and Q tiles IN PLACE
 //     (K rows past the window end are zeroed: the contraction of the state MMA runs over rows).
-//   * Two issuer warps then run, per 16 rows and straight from the TMA tiles,
+//   * The state issuer warp then runs, per 16 rows and straight from the TMA tiles,
 //         D[r][p]  += sum_j V[j][r] phi(K)[j][p]      tcgen05.mma M=128 N=128 K=16, both operands MN-major,
 //         Z[p][.]  += sum_j phi(K)[j][p] * 1          tcgen05.mma M=128 N=16  K=16 against a tile of ones.
 //     The 16x16 diagonal blocks of D are the per-head states S_h^T; the off-diagonal blocks (7/8 of the tensor
@@ -32,6 +32,10 @@
 //     columns 32h..32h+15 are the numerators, column 32h+16 the denominator, in the TMEM columns the state
 //     occupied.  Epilogue warps read their rows back (one thread per row), divide, stage the fp16 rows in the
 //     (now dead) Q tiles and store them with fully coalesced 128-bit stores.
+//   * Barrier discipline: ring barriers are indexed by the first tile of a chunk; a role that waits on a barrier
+//     family waits on it at every use (a role that only toggled a parity could run a phase ahead and pass a
+//     try_wait.parity on the wrong phase), and barriers that complete only for some item types (kphi, qphi) have their
+//     own parity bits.
 //   * Precision: operands fp16, accumulation fp32.
 #include <cuda.h>
 
