@@ -41,7 +41,7 @@ constexpr int NW = 8;                       // consumer warps = heads per slab
 #ifndef SLA_SR
 #define SLA_SR 32
 #endif
-constexpr int NST = SLA_NST;                // ring stages per stream (power of two)
+constexpr int NST = SLA_NST;                // ring stages per stream at d_h = 16 (and the size of the barrier arrays)
 constexpr int QUAD_MAX = 16;                // windows up to this length are packed into quadratic-form tiles
 
 template <int D> struct Cfg {
@@ -50,7 +50,9 @@ template <int D> struct Cfg {
   static constexpr int BOX_BYTES = SR * 128;
   static constexpr int T_STAGE = NBOX * BOX_BYTES;        // bytes of one tensor's stage (4 / 8 KB)
   static constexpr int KV_STAGE = 2 * T_STAGE;
-  static constexpr int RING_BYTES = NST * (KV_STAGE + T_STAGE);
+  // d_h = 32: a stage is twice as large; two stages instead of three let two CTAs share an SM (config 2: 188 -> 147 us)
+  static constexpr int NSTG = (D == 32 && NST > 2) ? 2 : NST;
+  static constexpr int RING_BYTES = NSTG * (KV_STAGE + T_STAGE);
   static constexpr int SMEM_DYN = RING_BYTES + 1024;      // + alignment slack (swizzle needs 1 KB)
   static constexpr int HPW = (D == 16) ? SLA_HPW : 1;     // heads per consumer warp (ILP, shared bookkeeping)
   static constexpr int NCW = NW / HPW;                    // consumer warps per CTA
@@ -95,9 +97,9 @@ __device__ __forceinline__ uint32_t lane_tile_addr(const RingView& rv, int slot_
   return ring_addr<D>(rv, slot_bytes, 0, rel0 + trow, hl * (D / 8) + (mi & 1));
 }
 // advance a lane address by one ring slot (the next stage), wrapping at the end of the ring
-__device__ __forceinline__ uint32_t ring_next_slot(uint32_t a, uint32_t ring_end, int slot_bytes) {
+__device__ __forceinline__ uint32_t ring_next_slot(uint32_t a, uint32_t ring_end, int slot_bytes, int nst) {
   a += (uint32_t)slot_bytes;
-  return a >= ring_end ? a - (uint32_t)(NST * slot_bytes) : a;
+  return a >= ring_end ? a - (uint32_t)(nst * slot_bytes) : a;
 }
 
 template <int D, int MODE, bool PRECISE, bool FULL = false>
@@ -324,7 +326,7 @@ __device__ __forceinline__ void process_window(RingView& kv, RingView& qv, int h
     ak[j][0] = lane_tile_addr<D>(kv, C::KV_STAGE, hl + j, s - S0, 16);
     ak[j][1] = lane_tile_addr<D>(kv, C::KV_STAGE, hl + j, s - S0 + 16, 16);
   }
-  const uint32_t kv_end = kv.base + NST * C::KV_STAGE;
+  const uint32_t kv_end = kv.base + C::NSTG * C::KV_STAGE;
   for (int r = s; r < e; r += 32) {
     const int nv = min(32, e - r), rel = r - S0;
     // stages entirely below this step go back to the producer first: a wait must never pin older
@@ -338,8 +340,8 @@ __device__ __forceinline__ void process_window(RingView& kv, RingView& qv, int h
         if (nv == 32) {   // two full tiles, one basic block: the two dependency chains interleave
           kv_tile<D, MODE, PRECISE, true>(kv, hl + j, rel, 16, st[j], ak[j][0]);
           kv_tile<D, MODE, PRECISE, true>(kv, hl + j, rel + 16, 16, st[j], ak[j][1]);
-          ak[j][0] = ring_next_slot(ak[j][0], kv_end, C::KV_STAGE);
-          ak[j][1] = ring_next_slot(ak[j][1], kv_end, C::KV_STAGE);
+          ak[j][0] = ring_next_slot(ak[j][0], kv_end, C::KV_STAGE, C::NSTG);
+          ak[j][1] = ring_next_slot(ak[j][1], kv_end, C::KV_STAGE, C::NSTG);
         } else {
           kv_tile<D, MODE, PRECISE>(kv, hl + j, rel, min(16, nv), st[j]);
           if (nv > 16) kv_tile<D, MODE, PRECISE>(kv, hl + j, rel + 16, nv - 16, st[j]);
@@ -359,7 +361,7 @@ __device__ __forceinline__ void process_window(RingView& kv, RingView& qv, int h
     aq[j][0] = lane_tile_addr<D>(qv, C::T_STAGE, hl + j, s - S0, 16);
     aq[j][1] = lane_tile_addr<D>(qv, C::T_STAGE, hl + j, s - S0 + 16, 16);
   }
-  const uint32_t q_end = qv.base + NST * C::T_STAGE;
+  const uint32_t q_end = qv.base + C::NSTG * C::T_STAGE;
   const size_t o8 = (size_t)8 * Ctot;
   // this lane's first output element: row s + g, head column + 2t; 32 rows further every step
   T* lp = out_head + (size_t)(s + (lane >> 2)) * Ctot + 2 * (lane & 3);
@@ -375,8 +377,8 @@ __device__ __forceinline__ void process_window(RingView& kv, RingView& qv, int h
         if (nv == 32) {
           q_tile<D, MODE, PRECISE, T, true>(qv, hl + j, rel, 16, oo[j], oh, o8, aq[j][0]);
           q_tile<D, MODE, PRECISE, T, true>(qv, hl + j, rel + 16, 16, oo[j], oh + 2 * o8, o8, aq[j][1]);
-          aq[j][0] = ring_next_slot(aq[j][0], q_end, C::T_STAGE);
-          aq[j][1] = ring_next_slot(aq[j][1], q_end, C::T_STAGE);
+          aq[j][0] = ring_next_slot(aq[j][0], q_end, C::T_STAGE, C::NSTG);
+          aq[j][1] = ring_next_slot(aq[j][1], q_end, C::T_STAGE, C::NSTG);
         } else {
           q_tile<D, MODE, PRECISE, T>(qv, hl + j, rel, min(16, nv), oo[j], oh, o8);
           if (nv > 16) q_tile<D, MODE, PRECISE, T>(qv, hl + j, rel + 16, nv - 16, oo[j], oh + 2 * o8, o8);
@@ -463,7 +465,7 @@ __device__ __forceinline__ void output_piece(RingView& qv, int hl, int S0, int p
   ring_release_below<C::SR>(qv, ps - S0);
   aq[0] = lane_tile_addr<D>(qv, C::T_STAGE, hl, ps - S0, 16);
   aq[1] = lane_tile_addr<D>(qv, C::T_STAGE, hl, ps - S0 + 16, 16);
-  const uint32_t q_end = qv.base + NST * C::T_STAGE;
+  const uint32_t q_end = qv.base + C::NSTG * C::T_STAGE;
   const size_t o8 = (size_t)8 * Ctot;
   T* lp = out_head + (size_t)(ps + g) * Ctot + 2 * t;
   for (int r = ps; r < pe; r += 32, lp += 4 * o8) {
@@ -474,8 +476,8 @@ __device__ __forceinline__ void output_piece(RingView& qv, int hl, int S0, int p
     if (nv == 32) {
       q_tile<D, MODE, false, T, true>(qv, hl, rel, 16, oo, lp, o8, aq[0]);
       q_tile<D, MODE, false, T, true>(qv, hl, rel + 16, 16, oo, lp + 2 * o8, o8, aq[1]);
-      aq[0] = ring_next_slot(aq[0], q_end, C::T_STAGE);
-      aq[1] = ring_next_slot(aq[1], q_end, C::T_STAGE);
+      aq[0] = ring_next_slot(aq[0], q_end, C::T_STAGE, C::NSTG);
+      aq[1] = ring_next_slot(aq[1], q_end, C::T_STAGE, C::NSTG);
     } else {
       q_tile<D, MODE, false, T>(qv, hl, rel, min(16, nv), oo, lp, o8);
       if (nv > 16) q_tile<D, MODE, false, T>(qv, hl, rel + 16, nv - 16, oo, lp + 2 * o8, o8);
@@ -505,7 +507,7 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     if (reinterpret_cast<const volatile int*>(ws)[0] == 0) return;   // no split window in this call
   }
   const uint32_t ring = (smem_u32(dyn_smem) + 1023u) & ~1023u;
-  const uint32_t kv_base = ring, q_base = ring + NST * C::KV_STAGE;
+  const uint32_t kv_base = ring, q_base = ring + C::NSTG * C::KV_STAGE;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   // CTAs are dispatched in blockIdx order and the grid runs in several waves (spans are short).
   // Map CTAs to spans outside-in: both ends of the row-major window order first.  In a LiDAR scene
@@ -522,7 +524,7 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   const int Ctot = H * D;
 
   if (threadIdx.x == 0) {
-    for (int i = 0; i < NST; ++i) {
+    for (int i = 0; i < C::NSTG; ++i) {
       mbar_init(smem_u32(&ctrl.full_kv[i]), 1);
       mbar_init(smem_u32(&ctrl.empty_kv[i]), nact);
       mbar_init(smem_u32(&ctrl.full_q[i]), 1);
@@ -542,7 +544,7 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     const int slot_bytes = is_kv ? C::KV_STAGE : C::T_STAGE;
     int S0 = R0;
     auto issue = [&](int st) {
-      const int slot = st % NST;
+      const int slot = st % C::NSTG;
       const uint32_t bar = full + 8u * slot;
       const uint32_t dst = base + slot * slot_bytes;
       const int y = S0 + st * C::SR;
@@ -563,11 +565,11 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       S0 = ctrl.stream_begin;
       const int total = (OUTPASS && is_kv) ? 0 : (ctrl.stream_end - S0 + C::SR - 1) / C::SR;
       for (int st = 0; st < total; ++st) {
-        if (st >= NST) mbar_wait(empty + 8u * (st % NST), (uint32_t)(((st / NST) - 1) & 1));
+        if (st >= C::NSTG) mbar_wait(empty + 8u * (st % C::NSTG), (uint32_t)(((st / C::NSTG) - 1) & 1));
         issue(st);
       }
-      for (int st = max(0, total - NST); st < total; ++st)      // no TMA may be in flight at exit
-        mbar_wait(full + 8u * (st % NST), (uint32_t)((st / NST) & 1));
+      for (int st = max(0, total - C::NSTG); st < total; ++st)      // no TMA may be in flight at exit
+        mbar_wait(full + 8u * (st % C::NSTG), (uint32_t)((st / C::NSTG) & 1));
     }
     return;
   }
@@ -604,8 +606,8 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   const int nh = min(C::HPW, nheads - hl);
   const int S0 = ctrl.stream_begin;
   const int total = (ctrl.stream_end - S0 + C::SR - 1) / C::SR;
-  RingView kv = make_ring(kv_base, smem_u32(ctrl.full_kv), smem_u32(ctrl.empty_kv));
-  RingView qv = make_ring(q_base, smem_u32(ctrl.full_q), smem_u32(ctrl.empty_q));
+  RingView kv = make_ring(kv_base, smem_u32(ctrl.full_kv), smem_u32(ctrl.empty_kv), C::NSTG);
+  RingView qv = make_ring(q_base, smem_u32(ctrl.full_q), smem_u32(ctrl.empty_q), C::NSTG);
   T* out_head = out + (size_t)(h0 + hl) * D;
 
   // window walk with a 32-entry register cache of the offsets (one global round trip per 31 windows)

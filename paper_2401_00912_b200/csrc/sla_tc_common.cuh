@@ -22,16 +22,17 @@ struct RingView {
   int released;
   int w_slot, w_phase;   // slot and parity of stage `waited`
   int r_slot, bias;      // slot of stage `released`; bias = r_slot - released
+  int nst;               // stages of this ring (a compile-time constant of the caller: folds after inlining)
 };
-__device__ __forceinline__ RingView make_ring(uint32_t base, uint32_t full, uint32_t empty) {
-  return RingView{base, full, empty, 0, 0, 0, 0, 0, 0};
+__device__ __forceinline__ RingView make_ring(uint32_t base, uint32_t full, uint32_t empty, int nst = NST) {
+  return RingView{base, full, empty, 0, 0, 0, 0, 0, 0, nst};
 }
 
 __device__ __forceinline__ void ring_wait_upto(RingView& rv, int stage_last) {
   while (rv.waited <= stage_last) {
     mbar_wait(rv.full + 8u * rv.w_slot, (uint32_t)rv.w_phase);
     ++rv.waited;
-    if (++rv.w_slot == NST) { rv.w_slot = 0; rv.w_phase ^= 1; }
+    if (++rv.w_slot == rv.nst) { rv.w_slot = 0; rv.w_phase ^= 1; }
   }
 }
 // Release every stage that lies entirely below relative row `rel` (rows are relative to R0).
@@ -42,7 +43,7 @@ __device__ __forceinline__ void ring_release_below(RingView& rv, int rel) {
     __syncwarp();
     if ((threadIdx.x & 31) == 0) mbar_arrive(rv.empty + 8u * rv.r_slot);
     ++rv.released;
-    if (++rv.r_slot == NST) { rv.r_slot = 0; rv.bias -= NST; }
+    if (++rv.r_slot == rv.nst) { rv.r_slot = 0; rv.bias -= rv.nst; }
   }
 }
 // Steady state of a loop whose step is exactly one stage of rows: after the first step of a pass,
@@ -52,7 +53,7 @@ __device__ __forceinline__ void ring_release_one(RingView& rv) {
   __syncwarp();
   if ((threadIdx.x & 31) == 0) mbar_arrive(rv.empty + 8u * rv.r_slot);
   ++rv.released;
-  if (++rv.r_slot == NST) { rv.r_slot = 0; rv.bias -= NST; }
+  if (++rv.r_slot == rv.nst) { rv.r_slot = 0; rv.bias -= rv.nst; }
 }
 
 // Shared address of (relative row rel, 16-byte chunk `chunk` of this slab row) inside a ring whose
@@ -63,7 +64,7 @@ __device__ __forceinline__ uint32_t ring_addr(const RingView& rv, int slot_bytes
   using C = Cfg<D>;
   const int st = (int)((unsigned)rel / (unsigned)C::SR), r = (int)((unsigned)rel % (unsigned)C::SR);   // rel >= 0
   int slot = st + rv.bias;
-  if (slot >= NST) slot -= NST;
+  if (slot >= rv.nst) slot -= rv.nst;
   const int box = chunk >> 3, cib = chunk & 7;
   return rv.base + (uint32_t)(slot * slot_bytes + toff + box * C::BOX_BYTES + r * 128 +
                               ((cib ^ (r & 7)) << 4));
