@@ -66,7 +66,8 @@ const char* sla_version(void);
 size_t sla_workspace_bytes(int64_t N, int32_t W, int32_t H, int32_t d_h, int dt, int for_backward);
 
 /* Offsets prep ("offsets generation", Fig. 5; flat window-sorted layout PAPER.md:77).
- *   win_id          DEV int32[N]   window index of each voxel, non-decreasing, each in [0, W)
+ *   win_id          DEV int32[N]   window index of each voxel, non-decreasing, each in [0, W); a tail of ids
+ *                                  equal to W ("no window", see sla_window_keys) is accepted
  *   window_offsets  DEV int32[W+1] out: off[w] = #{ i : win_id[i] < w }   (bit-exact integer result)
  * Gaps in the ids give zero-length windows (reading A10). */
 int sla_offsets_from_window_ids(const int32_t* win_id, int64_t N, int32_t W,
@@ -143,6 +144,55 @@ int sla_backward(const void* q, const void* k, const void* v, const int32_t* win
 int sla_forward_host(const void* q, const void* k, const void* v, const int32_t* win_id,
                      int64_t N, int32_t W, int32_t H, int32_t d_h, int dt, void* out,
                      sla_stream_t stream);
+
+/* ---- Sequence preparation ------------------------------------------------------------------
+ * "we arrange the voxels of the entire scene into a single flattened matrix ... ordered based on their window
+ * coordinates, ensuring that voxels from the same window form a sub-matrix in contiguous memory";
+ * windows are S_h x S_w cells of the ground plane.  Integer and byte work: every result below is
+ * unique and bit-exact.  What the paper leaves open is fixed by DESIGN.md reading A16:
+ *   - coords is int32[N,4], one row (b, z, y, x) per voxel: sample in the batch, then the cell, slowest axis first;
+ *     z takes no part.  The key of a voxel is the row-major index of (b, y / S_h, x / S_w) among the
+ *     W = batch * ceil(grid_h / S_h) * ceil(grid_w / S_w) windows; a voxel with b, y or x outside
+ *     [0,batch) x [0,grid_h) x [0,grid_w) gets the key W ("no window"; it sorts behind every window).
+ *   - The window-sorted order is the STABLE sort by key (voxels of one window keep their input order);
+ *     perm[j] is the input position of the voxel at sorted position j.
+ * All pointers DEV; every entry only enqueues kernels on `stream`.  N < 2^31, W < 2^31 - 1. */
+
+/* W for this grid and window shape; -1 if an argument is < 1 or W does not fit. */
+int64_t sla_window_count(int32_t batch, int32_t grid_h, int32_t grid_w, int32_t S_h, int32_t S_w);
+
+/*   coords  DEV int32[N,4], 16-byte aligned (read-only)        key  DEV int32[N] out, each in [0, W] */
+int sla_window_keys(const int32_t* coords, int64_t N, int32_t batch, int32_t grid_h, int32_t grid_w,
+                    int32_t S_h, int32_t S_w, int32_t* key, sla_stream_t stream);
+
+/* Bytes of device workspace sla_sort_by_window needs for N keys (0 on invalid N). */
+size_t sla_sort_workspace_bytes(int64_t N);
+
+/* Stable sort of the voxels by key (least-significant-digit radix sort, 8 bits per pass over the bits of W).
+ *   key         DEV int32[N], each in [0, W] (read-only; a key outside that range is undefined behaviour)
+ *   perm        DEV int32[N] out: a permutation of 0..N-1, key[perm[j]] non-decreasing in j, ties in input order
+ *   key_sorted  DEV int32[N] out: key[perm[j]]; must not be `key`.  Feed it to sla_offsets_from_window_ids
+ *               (which accepts the trailing keys equal to W: off[W] is then the number of voxels inside the grid).
+ *   workspace   DEV, >= sla_sort_workspace_bytes(N) bytes, 16-byte aligned, scratch */
+int sla_sort_by_window(const int32_t* key, int64_t N, int32_t W, int32_t* perm, int32_t* key_sorted,
+                       void* workspace, size_t workspace_bytes, sla_stream_t stream);
+
+/* dst[j] = src[perm[j]] for j in [0,N): input-order rows -> the window-sorted matrix.  Rows are `row_bytes` bytes,
+ * a multiple of 4 (copied 16 bytes at a time when rows and both base pointers allow); src and dst 4-byte aligned and
+ * distinct.  A row whose perm entry lies outside [0,N) is skipped (never read or written out of bounds). */
+int sla_gather_rows(const void* src, const int32_t* perm, int64_t N, size_t row_bytes, void* dst, sla_stream_t stream);
+
+/* dst[perm[j]] = src[j]: window-sorted rows (the op's output) back to input order; undoes sla_gather_rows. */
+int sla_scatter_rows(const void* src, const int32_t* perm, int64_t N, size_t row_bytes, void* dst, sla_stream_t stream);
+
+/* The three steps in one call: keys -> stable sort -> offsets.
+ *   perm, key_sorted  DEV int32[N] out (as above)        window_offsets  DEV int32[W+1] out, W = sla_window_count(...)
+ *   workspace         DEV, >= sla_sequence_workspace_bytes(N) bytes, 16-byte aligned, scratch
+ * off[W] is the number of voxels inside the grid: pass that as N to sla_forward when some voxels lie outside. */
+size_t sla_sequence_workspace_bytes(int64_t N);
+int sla_sequence_from_coords(const int32_t* coords, int64_t N, int32_t batch, int32_t grid_h, int32_t grid_w,
+                             int32_t S_h, int32_t S_w, int32_t* perm, int32_t* key_sorted, int32_t* window_offsets,
+                             void* workspace, size_t workspace_bytes, sla_stream_t stream);
 
 /* Measurement aid, not a step of the SLA path ("a size-matched pure read+write kernel
  * run beside config 1 as the practical ceiling").  Streams three tensors in and one out with 128-bit

@@ -22,6 +22,8 @@ SYMBOLS = (
     "sla_status_string", "sla_version", "sla_workspace_bytes", "sla_offsets_from_window_ids",
     "sla_forward", "sla_forward_phi", "sla_backward_phi", "sla_forward_tcgen05", "sla_forward_bounded", "sla_backward", "sla_forward_host",
     "sla_bench_stream_ceiling",
+    "sla_window_count", "sla_window_keys", "sla_sort_workspace_bytes", "sla_sort_by_window", "sla_gather_rows",
+    "sla_scatter_rows", "sla_sequence_workspace_bytes", "sla_sequence_from_coords",
 )
 
 _lib = None
@@ -66,6 +68,22 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     L.sla_forward_host.restype = ci
     L.sla_bench_stream_ceiling.argtypes = [vp, vp, vp, vp, sz, vp]
     L.sla_bench_stream_ceiling.restype = ci
+    L.sla_window_count.argtypes = [i32, i32, i32, i32, i32]
+    L.sla_window_count.restype = i64
+    L.sla_window_keys.argtypes = [vp, i64, i32, i32, i32, i32, i32, vp, vp]
+    L.sla_window_keys.restype = ci
+    L.sla_sort_workspace_bytes.argtypes = [i64]
+    L.sla_sort_workspace_bytes.restype = sz
+    L.sla_sort_by_window.argtypes = [vp, i64, i32, vp, vp, vp, sz, vp]
+    L.sla_sort_by_window.restype = ci
+    L.sla_gather_rows.argtypes = [vp, vp, i64, sz, vp, vp]
+    L.sla_gather_rows.restype = ci
+    L.sla_scatter_rows.argtypes = [vp, vp, i64, sz, vp, vp]
+    L.sla_scatter_rows.restype = ci
+    L.sla_sequence_workspace_bytes.argtypes = [i64]
+    L.sla_sequence_workspace_bytes.restype = sz
+    L.sla_sequence_from_coords.argtypes = [vp, i64, i32, i32, i32, i32, i32, vp, vp, vp, vp, sz, vp]
+    L.sla_sequence_from_coords.restype = ci
     if path is None:
         _lib = L
     return L
@@ -220,3 +238,94 @@ def sla_bench_stream_ceiling(a, b, c, out, stream=None):
     _check(L.sla_bench_stream_ceiling(a.data_ptr(), b.data_ptr(), c.data_ptr(), out.data_ptr(), nbytes,
                                       _stream(stream)), "sla_bench_stream_ceiling")
     return out
+
+
+# ---- sequence preparation (include/sla.h) ----
+
+def sla_window_count(batch: int, grid_h: int, grid_w: int, S_h: int, S_w: int) -> int:
+    W = int(load_library().sla_window_count(batch, grid_h, grid_w, S_h, S_w))
+    if W < 0:
+        raise SlaError("sla_window_count: arguments must be >= 1 and W must fit in int32")
+    return W
+
+
+def _chk_i32(t, what):
+    import torch
+    _chk_dev(t)
+    if t.dtype != torch.int32:
+        raise SlaError(f"{what} must be int32")
+
+
+def sla_window_keys(coords, batch: int, grid_h: int, grid_w: int, S_h: int, S_w: int, out=None, stream=None):
+    """coords: CUDA int32[N,4] rows (b, z, y, x) -> CUDA int32[N] window keys in [0, W]."""
+    import torch
+    _chk_i32(coords, "coords")
+    if coords.dim() != 2 or coords.shape[1] != 4:
+        raise SlaError("coords must be [N,4]")
+    N = coords.shape[0]
+    if out is None:
+        out = torch.empty(N, dtype=torch.int32, device=coords.device)
+    _check(load_library().sla_window_keys(coords.data_ptr(), N, batch, grid_h, grid_w, S_h, S_w, out.data_ptr(),
+                                          _stream(stream)), "sla_window_keys")
+    return out
+
+
+def sla_sort_by_window(key, W: int, workspace=None, stream=None):
+    """key: CUDA int32[N] in [0, W] -> (perm, key_sorted), the stable sort by key."""
+    import torch
+    L = load_library()
+    _chk_i32(key, "key")
+    N = key.numel()
+    perm = torch.empty(N, dtype=torch.int32, device=key.device)
+    ks = torch.empty(N, dtype=torch.int32, device=key.device)
+    if workspace is None:
+        workspace = torch.empty(max(int(L.sla_sort_workspace_bytes(N)), 16), dtype=torch.uint8, device=key.device)
+    _check(L.sla_sort_by_window(key.data_ptr(), N, W, perm.data_ptr(), ks.data_ptr(), workspace.data_ptr(),
+                                workspace.numel(), _stream(stream)), "sla_sort_by_window")
+    return perm, ks
+
+
+def _permute_rows(fn, name, src, perm, out, stream):
+    import torch
+    _chk_dev(src)
+    _chk_i32(perm, "perm")
+    N = perm.numel()
+    if src.shape[0] != N:
+        raise SlaError("src must have one row per entry of perm")
+    if out is None:
+        out = torch.empty_like(src)
+    row_bytes = (src.numel() // N) * src.element_size() if N else 0
+    _check(fn(src.data_ptr(), perm.data_ptr(), N, row_bytes, out.data_ptr(), _stream(stream)), name)
+    return out
+
+
+def sla_gather_rows(src, perm, out=None, stream=None):
+    """out[j] = src[perm[j]] (rows of any shape and dtype whose size is a multiple of 4 bytes)."""
+    return _permute_rows(load_library().sla_gather_rows, "sla_gather_rows", src, perm, out, stream)
+
+
+def sla_scatter_rows(src, perm, out=None, stream=None):
+    """out[perm[j]] = src[j]: undoes sla_gather_rows."""
+    return _permute_rows(load_library().sla_scatter_rows, "sla_scatter_rows", src, perm, out, stream)
+
+
+def sla_sequence_from_coords(coords, batch: int, grid_h: int, grid_w: int, S_h: int, S_w: int, workspace=None,
+                             stream=None):
+    """coords: CUDA int32[N,4] -> (perm int32[N], key_sorted int32[N], window_offsets int32[W+1]) in one C call."""
+    import torch
+    L = load_library()
+    _chk_i32(coords, "coords")
+    if coords.dim() != 2 or coords.shape[1] != 4:
+        raise SlaError("coords must be [N,4]")
+    N = coords.shape[0]
+    W = sla_window_count(batch, grid_h, grid_w, S_h, S_w)
+    dev = coords.device
+    perm = torch.empty(N, dtype=torch.int32, device=dev)
+    ks = torch.empty(N, dtype=torch.int32, device=dev)
+    off = torch.empty(W + 1, dtype=torch.int32, device=dev)
+    if workspace is None:
+        workspace = torch.empty(max(int(L.sla_sequence_workspace_bytes(N)), 16), dtype=torch.uint8, device=dev)
+    _check(L.sla_sequence_from_coords(coords.data_ptr(), N, batch, grid_h, grid_w, S_h, S_w, perm.data_ptr(),
+                                      ks.data_ptr(), off.data_ptr(), workspace.data_ptr(), workspace.numel(),
+                                      _stream(stream)), "sla_sequence_from_coords")
+    return perm, ks, off

@@ -1,5 +1,6 @@
 // sla_api.cu -- the extern "C" boundary declared in include/sla.h: argument validation, workspace
 // carving and kernel dispatch.  No torch types; plain pointers and sizes.
+#include <cstdint>
 #include <mutex>
 
 #include "sla_internal.cuh"
@@ -54,6 +55,90 @@ int sla_offsets_from_window_ids(const int32_t* win_id, int64_t N, int32_t W, int
   if (N > 0 && W == 0) return SLA_ERR_INVALID_ARG;
   cudaError_t e = sla::launch_offsets(win_id, (int)N, W, window_offsets, (cudaStream_t)stream);
   return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
+}
+
+// ---- sequence preparation ----
+static int64_t count_windows(int32_t batch, int32_t grid_h, int32_t grid_w, int32_t S_h, int32_t S_w) {
+  if (batch < 1 || grid_h < 1 || grid_w < 1 || S_h < 1 || S_w < 1) return -1;
+  const int64_t nwy = ((int64_t)grid_h + S_h - 1) / S_h, nwx = ((int64_t)grid_w + S_w - 1) / S_w;
+  const int64_t W = (int64_t)batch * nwy * nwx;
+  return W < (int64_t(1) << 31) - 1 ? W : -1;
+}
+
+int64_t sla_window_count(int32_t batch, int32_t grid_h, int32_t grid_w, int32_t S_h, int32_t S_w) {
+  return count_windows(batch, grid_h, grid_w, S_h, S_w);
+}
+
+int sla_window_keys(const int32_t* coords, int64_t N, int32_t batch, int32_t grid_h, int32_t grid_w, int32_t S_h,
+                    int32_t S_w, int32_t* key, sla_stream_t stream) {
+  if (N < 0 || N >= (int64_t(1) << 31) || count_windows(batch, grid_h, grid_w, S_h, S_w) < 0) return SLA_ERR_INVALID_ARG;
+  if (N == 0) return SLA_OK;
+  if (!coords || !key) return SLA_ERR_INVALID_ARG;
+  if (!aligned16(coords)) return SLA_ERR_UNSUPPORTED;
+  cudaError_t e = sla::launch_window_keys(coords, (int)N, batch, grid_h, grid_w, S_h, S_w, key, (cudaStream_t)stream);
+  return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
+}
+
+size_t sla_sort_workspace_bytes(int64_t N) {
+  if (N < 0 || N >= (int64_t(1) << 31)) return 0;
+  return sla::sort_workspace_bytes(N);
+}
+
+int sla_sort_by_window(const int32_t* key, int64_t N, int32_t W, int32_t* perm, int32_t* key_sorted,
+                       void* workspace, size_t workspace_bytes, sla_stream_t stream) {
+  if (N < 0 || N >= (int64_t(1) << 31) || W < 0 || W == INT32_MAX) return SLA_ERR_INVALID_ARG;
+  if (N == 0) return SLA_OK;
+  if (!key || !perm || !key_sorted || key == key_sorted) return SLA_ERR_INVALID_ARG;
+  if (!workspace || workspace_bytes < sla::sort_workspace_bytes(N) || !aligned16(workspace)) return SLA_ERR_WORKSPACE;
+  cudaError_t e = sla::launch_sort_by_key(key, (int)N, W, perm, key_sorted, workspace, (cudaStream_t)stream);
+  return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
+}
+
+static int permute_rows(const void* src, const int32_t* perm, int64_t N, size_t row_bytes, void* dst, bool scatter,
+                        sla_stream_t stream) {
+  if (N < 0 || N >= (int64_t(1) << 31)) return SLA_ERR_INVALID_ARG;
+  if (N == 0 || row_bytes == 0) return SLA_OK;
+  if (!src || !perm || !dst || src == dst) return SLA_ERR_INVALID_ARG;
+  if (row_bytes % 4 != 0 || ((reinterpret_cast<uintptr_t>(src) | reinterpret_cast<uintptr_t>(dst)) & 3u) != 0 ||
+      row_bytes / 4 > (size_t)INT32_MAX)
+    return SLA_ERR_UNSUPPORTED;
+  cudaError_t e = sla::launch_permute_rows(src, perm, N, row_bytes, dst, scatter, (cudaStream_t)stream);
+  return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
+}
+
+int sla_gather_rows(const void* src, const int32_t* perm, int64_t N, size_t row_bytes, void* dst, sla_stream_t stream) {
+  return permute_rows(src, perm, N, row_bytes, dst, false, stream);
+}
+
+int sla_scatter_rows(const void* src, const int32_t* perm, int64_t N, size_t row_bytes, void* dst, sla_stream_t stream) {
+  return permute_rows(src, perm, N, row_bytes, dst, true, stream);
+}
+
+int sla_sequence_from_coords(const int32_t* coords, int64_t N, int32_t batch, int32_t grid_h, int32_t grid_w,
+                             int32_t S_h, int32_t S_w, int32_t* perm, int32_t* key_sorted, int32_t* window_offsets,
+                             void* workspace, size_t workspace_bytes, sla_stream_t stream) {
+  const int64_t W = count_windows(batch, grid_h, grid_w, S_h, S_w);
+  if (N < 0 || N >= (int64_t(1) << 31) || W < 0) return SLA_ERR_INVALID_ARG;
+  if (!window_offsets || (N > 0 && (!coords || !perm || !key_sorted))) return SLA_ERR_INVALID_ARG;
+  if (N > 0 && !aligned16(coords)) return SLA_ERR_UNSUPPORTED;
+  const size_t key_bytes = ((size_t)N * 4 + 15) / 16 * 16;
+  if (N > 0 && (!workspace || workspace_bytes < key_bytes + sla::sort_workspace_bytes(N) || !aligned16(workspace)))
+    return SLA_ERR_WORKSPACE;
+  cudaStream_t st = (cudaStream_t)stream;
+  int32_t* key = static_cast<int32_t*>(workspace);
+  if (N > 0) {
+    if (sla::launch_window_keys(coords, (int)N, batch, grid_h, grid_w, S_h, S_w, key, st) != cudaSuccess) return SLA_ERR_CUDA;
+    if (sla::launch_sort_by_key(key, (int)N, (int)W, perm, key_sorted, static_cast<char*>(workspace) + key_bytes, st) != cudaSuccess)
+      return SLA_ERR_CUDA;
+  }
+  // keys equal to W (voxels outside the grid) sort behind every window: off[W] = number of voxels inside
+  cudaError_t e = sla::launch_offsets(key_sorted, (int)N, (int)W, window_offsets, st);
+  return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
+}
+
+size_t sla_sequence_workspace_bytes(int64_t N) {
+  if (N < 0 || N >= (int64_t(1) << 31)) return 0;
+  return ((size_t)N * 4 + 15) / 16 * 16 + sla::sort_workspace_bytes(N);
 }
 
 int sla_bench_stream_ceiling(const void* a, const void* b, const void* c, void* out, size_t bytes,

@@ -93,6 +93,14 @@ cudaError_t launch_forward_tc(const Problem& p, int dt, cudaStream_t st);
 bool forward_umma_supported(const Problem& p, int dt);
 cudaError_t launch_forward_umma_main(const Problem& p, int dt, cudaStream_t st);
 // measurement aid (sla_bench_stream_ceiling): out = a ^ b ^ c over `bytes` bytes per tensor, 128-bit accesses
+// sequence preparation (sla_seq.cu)
+size_t sort_workspace_bytes(long long N);
+cudaError_t launch_window_keys(const int32_t* coords, int N, int batch, int grid_h, int grid_w, int S_h, int S_w,
+                               int32_t* key, cudaStream_t st);
+cudaError_t launch_sort_by_key(const int32_t* key, int N, int W, int32_t* perm, int32_t* key_sorted, void* ws,
+                               cudaStream_t st);
+cudaError_t launch_permute_rows(const void* src, const int32_t* perm, long long N, size_t row_bytes, void* dst,
+                                bool scatter, cudaStream_t st);
 cudaError_t launch_stream_ceiling(const void* a, const void* b, const void* c, void* out, size_t bytes,
                                   cudaStream_t st);
 

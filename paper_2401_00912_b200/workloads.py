@@ -155,6 +155,42 @@ def lengths_waymo_like(seed: int, N: int = 60000, grid: int = 39, cap: int = 144
     return ln
 
 
+def coords_waymo_like(seed: int, N: int = 60000, batch: int = 1, grid_hw: int = 468, win: int = 12, nz: int = 32,
+                      r0: float = 2.6, sigma: float = 0.5, n_outside: int = 0) -> np.ndarray:
+    """Voxel coordinates int32[N,4], rows (b, z, y, x), for the sequence preparation: per
+    sample, N/batch distinct cells of a grid_hw x grid_hw ground-plane grid, drawn without replacement with
+    probability ~ exp(-r/r0) (r = distance of the cell's win x win window from the centre, in windows) times a
+    lognormal jitter per window -- the density model of lengths_waymo_like -- then shuffled: a voxeliser emits
+    voxels in no particular order.  z is uniform in [0, nz).  The last n_outside rows are moved off the grid
+    (b, y or x out of range, both sides), then everything is shuffled again."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    g = -(-grid_hw // win)
+    c = (g - 1) / 2.0
+    yy, xx = np.meshgrid(np.arange(grid_hw), np.arange(grid_hw), indexing="ij")
+    wy, wx = yy // win, xx // win
+    out = []
+    per = [N // batch + (1 if b < N % batch else 0) for b in range(batch)]
+    for b in range(batch):
+        jitter = np.exp(sigma * rng.standard_normal((g, g)))
+        r = np.sqrt((wy - c) ** 2 + (wx - c) ** 2)
+        p = (np.exp(-r / r0) * jitter[wy, wx]).ravel()
+        p /= p.sum()
+        cells = rng.choice(grid_hw * grid_hw, size=per[b], replace=False, p=p)
+        co = np.empty((per[b], 4), dtype=np.int32)
+        co[:, 0] = b
+        co[:, 1] = rng.integers(0, nz, per[b])
+        co[:, 2] = cells // grid_hw
+        co[:, 3] = cells % grid_hw
+        out.append(co)
+    co = np.concatenate(out, axis=0) if out else np.empty((0, 4), np.int32)
+    co = co[rng.permutation(co.shape[0])]
+    for j in range(min(n_outside, co.shape[0])):
+        row = co.shape[0] - 1 - j
+        col, val = [(0, batch), (0, -1), (2, grid_hw), (2, -1), (3, grid_hw + 7), (3, -2)][j % 6]
+        co[row, col] = val
+    return np.ascontiguousarray(co[rng.permutation(co.shape[0])])
+
+
 def lengths_config2(seed: int = SEED_BASE + 2, N: int = 200000, W: int = 4000) -> np.ndarray:
     """Lognormal(3.5, 1.2) lengths clipped to [1,2000], rescaled to sum N."""
     rng = np.random.Generator(np.random.PCG64(seed))
