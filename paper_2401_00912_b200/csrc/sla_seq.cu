@@ -6,25 +6,40 @@
 //
 // The sort is a least-significant-digit radix sort, 8 bits per pass, ceil(bits(W) / 8) passes (two for the
 // 3042 windows of a Waymo-like batch).  One pass is three kernels:
-//   hist     a warp owns a tile of 512 consecutive keys and counts its digits            cnt[tile][digit]
-//   scan     one block turns the counts into start positions in digit-major order        pre[tile][digit]
-//   scatter  the warp walks its tile again 32 keys at a time, in order; match_any groups the lanes of equal
-//            digit, a lane's rank in its group is its place behind the keys the warp already placed
+//   hist     a warp owns a tile of 128 (512 beyond 2^18 keys) consecutive keys and counts its digits; the 8 warps
+//            of a block add their counts, so global memory sees one row per block                 cnt[block][digit]
+//   scan     one block turns the counts into start positions in digit-major order        pre[block][digit]
+//            (up to 128 blocks there is no such kernel: every scatter block sums the rows it needs itself)
+//   scatter  the warps count again, take their start behind the warps before them, then walk their tile
+//            32 keys at a time, in order; match_any groups the lanes of equal digit, a lane's rank in its
+//            group is its place behind the keys the warp already placed
 // Equal digits keep their order inside a warp step (rank by lane), across the steps of a tile (running
-// start position) and across tiles (scan order), so every pass is stable and so is the whole sort.
+// start position), across the warps of a block and across blocks (scan order), so every pass is stable and
+// so is the whole sort.  The kernels of a call form one chain of programmatic dependent launches: each lets
+// its successor become resident at once and waits for its predecessor before it touches global memory.
 #include "sla_internal.cuh"
 
 namespace sla {
 namespace {
 
 constexpr int kDigitBits = 8, kBins = 1 << kDigitBits;
-constexpr int kTileSteps = 16, kTile = 32 * kTileSteps;   // keys per warp
-constexpr int kSortWarps = 4;                            // warps (tiles) per block
+constexpr int kSortWarps = 8;                            // warps per block
+// A warp walks STEPS x 32 keys in order, one dependent step after the other, so a short tile means a short
+// kernel and more blocks to spread over the SMs; a long tile means fewer rows of counts for the one-block scan.
+constexpr int kStepsSmall = 4, kStepsLarge = 16;
+constexpr long long kSmallSortMax = 1 << 18;             // up to here: 4 steps (1024 keys per block)
+constexpr int kOwnScanMax = 128;                         // up to this many blocks the scatter kernel scans for itself
 constexpr int kScanGroups = 4;                           // scan block = kScanGroups x kBins threads
+static_assert(32 * kSortWarps == kBins, "one thread per digit when the warps' counts are combined");
+
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 __global__ void __launch_bounds__(256)
 sla_window_key_kernel(const int4* __restrict__ coords, int N, int batch, int grid_h, int grid_w, int S_h,
                       int S_w, int nwy, int nwx, int W, int32_t* __restrict__ key) {
+  pdl_launch_dependents();
+  pdl_wait();
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= N) return;
   const int4 c = __ldg(coords + i);                      // (b, z, y, x); z takes no part
@@ -38,40 +53,70 @@ __device__ __forceinline__ int digit_of(int key, int shift, bool valid) {
   return valid ? ((key >> shift) & (kBins - 1)) : kBins;
 }
 
-__global__ void __launch_bounds__(32 * kSortWarps)
-sla_sort_hist_kernel(const int32_t* __restrict__ key_in, int N, int shift, int T, uint32_t* __restrict__ cnt) {
-  __shared__ uint32_t h[kSortWarps][kBins];
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int t = blockIdx.x * kSortWarps + warp;
-  if (t >= T) return;
+// The warp's 512 keys -> registers, and their digit counts -> h[0..255] (the warp's own row of shared memory).
+template <int STEPS>
+__device__ __forceinline__ void load_and_count(const int32_t* __restrict__ key_in, long long base, int N, int shift,
+                                               int lane, int (&key)[STEPS], uint32_t* h) {
 #pragma unroll
-  for (int j = 0; j < kBins / 32; ++j) h[warp][lane + 32 * j] = 0;
-  __syncwarp();
-  const long long base = (long long)t * kTile;
-  int key[kTileSteps];
+  for (int j = 0; j < kBins / 32; ++j) h[lane + 32 * j] = 0;
 #pragma unroll
-  for (int s = 0; s < kTileSteps; ++s) {
+  for (int s = 0; s < STEPS; ++s) {
     const long long i = base + s * 32 + lane;
-    key[s] = i < N ? __ldg(key_in + i) : 0;
+    key[s] = i < N ? key_in[i] : 0;                      // plain loads: the predecessor kernel wrote them
   }
+  __syncwarp();
 #pragma unroll
-  for (int s = 0; s < kTileSteps; ++s) {
+  for (int s = 0; s < STEPS; ++s) {
     const bool valid = base + s * 32 + lane < N;
     const int d = digit_of(key[s], shift, valid);
     const unsigned grp = __match_any_sync(0xffffffffu, d);
-    if (valid && lane == __ffs(grp) - 1) h[warp][d] += __popc(grp);   // one writer per digit and step
+    if (valid && lane == __ffs(grp) - 1) h[d] += __popc(grp);   // one writer per digit and step
     __syncwarp();
   }
-#pragma unroll
-  for (int j = 0; j < kBins / 32; ++j) cnt[(size_t)t * kBins + lane + 32 * j] = h[warp][lane + 32 * j];
 }
 
-// pre[t][d] = #keys with a smaller digit + #keys with digit d in tiles before t.  Thread (g, d) owns digit d
-// of the g-th quarter of the tiles; consecutive threads read consecutive digits, so the walks are coalesced.
+template <int STEPS>
+__global__ void __launch_bounds__(32 * kSortWarps)
+sla_sort_hist_kernel(const int32_t* __restrict__ key_in, int N, int shift, uint32_t* __restrict__ cnt) {
+  __shared__ uint32_t h[kSortWarps][kBins];
+  pdl_launch_dependents();
+  pdl_wait();
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  int key[STEPS];
+  load_and_count<STEPS>(key_in, ((long long)blockIdx.x * kSortWarps + warp) * (32 * STEPS), N, shift, lane, key, h[warp]);
+  __syncthreads();
+  uint32_t tot = 0;
+#pragma unroll
+  for (int w = 0; w < kSortWarps; ++w) tot += h[w][threadIdx.x];
+  cnt[(size_t)blockIdx.x * kBins + threadIdx.x] = tot;
+}
+
+// exclusive scan of tot[0..255] in place, by the first warp of the block (the caller syncs before and after)
+__device__ __forceinline__ void scan_digits(uint32_t* tot) {
+  if (threadIdx.x < 32) {
+    uint32_t v[kBins / 32], run = 0;
+#pragma unroll
+    for (int j = 0; j < kBins / 32; ++j) { v[j] = tot[threadIdx.x * (kBins / 32) + j]; run += v[j]; }
+    uint32_t inc = run;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t up = __shfl_up_sync(0xffffffffu, inc, o);
+      if ((int)threadIdx.x >= o) inc += up;
+    }
+    uint32_t ex = inc - run;
+#pragma unroll
+    for (int j = 0; j < kBins / 32; ++j) { tot[threadIdx.x * (kBins / 32) + j] = ex; ex += v[j]; }
+  }
+}
+
+// pre[t][d] = #keys with a smaller digit + #keys with digit d in blocks before t.  Thread (g, d) owns digit d
+// of the g-th quarter of the rows; consecutive threads read consecutive digits, so the walks are coalesced.
 __global__ void __launch_bounds__(kScanGroups * kBins)
 sla_sort_scan_kernel(uint32_t* __restrict__ cnt, int T) {
   __shared__ uint32_t part[kScanGroups][kBins];
   __shared__ uint32_t digit_base[kBins];
+  pdl_launch_dependents();
+  pdl_wait();
   const int g = threadIdx.x / kBins, d = threadIdx.x % kBins;
   const int per = (T + kScanGroups - 1) / kScanGroups;
   const int t0 = min(T, g * per), t1 = min(T, t0 + per);
@@ -86,20 +131,7 @@ sla_sort_scan_kernel(uint32_t* __restrict__ cnt, int T) {
     digit_base[d] = tot;
   }
   __syncthreads();
-  if (threadIdx.x < 32) {                                 // exclusive scan of the 256 digit totals by one warp
-    uint32_t v[kBins / 32], run = 0;
-#pragma unroll
-    for (int j = 0; j < kBins / 32; ++j) { v[j] = digit_base[threadIdx.x * (kBins / 32) + j]; run += v[j]; }
-    uint32_t inc = run;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const uint32_t up = __shfl_up_sync(0xffffffffu, inc, o);
-      if ((int)threadIdx.x >= o) inc += up;
-    }
-    uint32_t ex = inc - run;
-#pragma unroll
-    for (int j = 0; j < kBins / 32; ++j) { digit_base[threadIdx.x * (kBins / 32) + j] = ex; ex += v[j]; }
-  }
+  scan_digits(digit_base);
   __syncthreads();
   uint32_t run = digit_base[d];
   for (int j = 0; j < g; ++j) run += part[j][d];
@@ -111,29 +143,53 @@ sla_sort_scan_kernel(uint32_t* __restrict__ cnt, int T) {
   }
 }
 
-template <bool FIRST>
+// OWN_SCAN: `pre` holds the raw counts of all T blocks and every block works out its own start positions (few
+// blocks: T rows of 1 KB out of L2 cost less than a kernel in between); else sla_sort_scan_kernel has run.
+template <int STEPS, bool FIRST, bool OWN_SCAN>
 __global__ void __launch_bounds__(32 * kSortWarps)
 sla_sort_scatter_kernel(const int32_t* __restrict__ key_in, const int32_t* __restrict__ val_in, int N, int shift,
                         int T, const uint32_t* __restrict__ pre, int32_t* __restrict__ key_out,
                         int32_t* __restrict__ val_out) {
   __shared__ uint32_t start[kSortWarps][kBins];
+  __shared__ uint32_t digit_base[kBins];
+  pdl_launch_dependents();
+  pdl_wait();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int t = blockIdx.x * kSortWarps + warp;
-  if (t >= T) return;
+  const long long base = ((long long)blockIdx.x * kSortWarps + warp) * (32 * STEPS);
+  int key[STEPS], val[STEPS];
+  load_and_count<STEPS>(key_in, base, N, shift, lane, key, start[warp]);
 #pragma unroll
-  for (int j = 0; j < kBins / 32; ++j) start[warp][lane + 32 * j] = __ldg(pre + (size_t)t * kBins + lane + 32 * j);
-  const long long base = (long long)t * kTile;
-  int key[kTileSteps], val[kTileSteps];
-#pragma unroll
-  for (int s = 0; s < kTileSteps; ++s) {
+  for (int s = 0; s < STEPS; ++s) {
     const long long i = base + s * 32 + lane;
-    key[s] = i < N ? __ldg(key_in + i) : 0;
-    val[s] = FIRST ? (int)i : (i < N ? __ldg(val_in + i) : 0);   // first pass: the value is the input position
+    val[s] = FIRST ? (int)i : (i < N ? val_in[i] : 0);    // first pass: the value is the input position
   }
-  __syncwarp();
+  uint32_t run;
+  if (OWN_SCAN) {
+    uint32_t before = 0, all = 0;                         // thread d: digit d in the blocks before this one / in all
+    for (int t = 0; t < T; ++t) {
+      const uint32_t c = pre[(size_t)t * kBins + threadIdx.x];
+      all += c;
+      if (t < (int)blockIdx.x) before += c;
+    }
+    digit_base[threadIdx.x] = all;
+    __syncthreads();
+    scan_digits(digit_base);
+    __syncthreads();
+    run = digit_base[threadIdx.x] + before;
+  } else {
+    run = pre[(size_t)blockIdx.x * kBins + threadIdx.x];
+    __syncthreads();
+  }
+#pragma unroll
+  for (int w = 0; w < kSortWarps; ++w) {                  // counts -> starts, warp by warp behind the block's start
+    const uint32_t c = start[w][threadIdx.x];
+    start[w][threadIdx.x] = run;
+    run += c;
+  }
+  __syncthreads();
   const unsigned below = (1u << lane) - 1u;
 #pragma unroll
-  for (int s = 0; s < kTileSteps; ++s) {
+  for (int s = 0; s < STEPS; ++s) {
     const bool valid = base + s * 32 + lane < N;
     const int d = digit_of(key[s], shift, valid);
     const unsigned grp = __match_any_sync(0xffffffffu, d);
@@ -148,36 +204,88 @@ sla_sort_scatter_kernel(const int32_t* __restrict__ key_in, const int32_t* __res
 
 // dst[j] = src[perm[j]] (gather) or dst[perm[j]] = src[j] (scatter), rows of `vpr` vectors of type V.  A row
 // whose perm entry lies outside [0, N) is skipped, so a bad permutation cannot reach outside the buffers.
+// A thread moves kPermUnroll vectors, 256 apart, and has all its loads in flight before the first store.
+constexpr int kPermUnroll = 4;
 template <typename V, bool SCATTER>
 __global__ void __launch_bounds__(256)
 sla_permute_rows_kernel(const V* __restrict__ src, const int32_t* __restrict__ perm, long long N, int vpr,
                         V* __restrict__ dst) {
-  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  const long long row = idx / vpr;
-  if (row >= N) return;
-  const int col = (int)(idx - row * vpr);
-  const long long p = __ldg(perm + row);
-  if (p < 0 || p >= N) return;
-  if (SCATTER) dst[p * vpr + col] = src[row * vpr + col];
-  else         dst[row * vpr + col] = src[p * vpr + col];
+  pdl_launch_dependents();
+  pdl_wait();
+  const long long total = N * vpr;
+  const long long first = (long long)blockIdx.x * (256 * kPermUnroll) + threadIdx.x;
+  long long from[kPermUnroll], to[kPermUnroll];
+  V x[kPermUnroll];
+#pragma unroll
+  for (int u = 0; u < kPermUnroll; ++u) {
+    const long long idx = first + u * 256;
+    from[u] = -1;
+    if (idx < total) {
+      const long long row = idx / vpr;
+      const int col = (int)(idx - row * vpr);
+      const long long p = perm[row];
+      if (p >= 0 && p < N) {
+        from[u] = (SCATTER ? row : p) * vpr + col;
+        to[u] = (SCATTER ? p : row) * vpr + col;
+      }
+    }
+  }
+#pragma unroll
+  for (int u = 0; u < kPermUnroll; ++u)
+    if (from[u] >= 0) x[u] = src[from[u]];
+#pragma unroll
+  for (int u = 0; u < kPermUnroll; ++u)
+    if (from[u] >= 0) dst[to[u]] = x[u];
+}
+
+// One link of a chain of programmatic dependent launches (see the kernels: launch_dependents, then wait).
+template <typename... KArgs, typename... Args>
+cudaError_t launch_chained(void (*kernel)(KArgs...), unsigned blocks, unsigned threads, cudaStream_t st, Args... args) {
+  cudaLaunchAttribute pdl[1];
+  pdl[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  pdl[0].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(blocks);
+  cfg.blockDim = dim3(threads);
+  cfg.stream = st;
+  cfg.attrs = pdl;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
 }  // namespace
 
-int sort_tiles(long long N) { return (int)((N + kTile - 1) / kTile); }
+static int sort_steps(long long N) { return N <= kSmallSortMax ? kStepsSmall : kStepsLarge; }
+static int sort_blocks(long long N) {
+  const long long tile = (long long)kSortWarps * 32 * sort_steps(N);
+  return (int)((N + tile - 1) / tile);
+}
+
+template <int STEPS>
+static cudaError_t sort_pass(const int32_t* kin, const int32_t* vin, int N, int shift, int T, uint32_t* cnt,
+                             int32_t* kout, int32_t* vout, bool first, cudaStream_t st) {
+  cudaError_t e = launch_chained(sla_sort_hist_kernel<STEPS>, T, 32 * kSortWarps, st, kin, N, shift, cnt);
+  if (e != cudaSuccess) return e;
+  if (T <= kOwnScanMax)
+    return first ? launch_chained(sla_sort_scatter_kernel<STEPS, true, true>, T, 32 * kSortWarps, st, kin, vin, N, shift, T, cnt, kout, vout)
+                 : launch_chained(sla_sort_scatter_kernel<STEPS, false, true>, T, 32 * kSortWarps, st, kin, vin, N, shift, T, cnt, kout, vout);
+  e = launch_chained(sla_sort_scan_kernel, 1, kScanGroups * kBins, st, cnt, T);
+  if (e != cudaSuccess) return e;
+  return first ? launch_chained(sla_sort_scatter_kernel<STEPS, true, false>, T, 32 * kSortWarps, st, kin, vin, N, shift, T, cnt, kout, vout)
+               : launch_chained(sla_sort_scatter_kernel<STEPS, false, false>, T, 32 * kSortWarps, st, kin, vin, N, shift, T, cnt, kout, vout);
+}
 
 size_t sort_workspace_bytes(long long N) {
   const size_t n4 = ((size_t)N * 4 + 15) / 16 * 16;
-  return 2 * n4 + (size_t)sort_tiles(N) * kBins * sizeof(uint32_t);
+  return 2 * n4 + (size_t)sort_blocks(N) * kBins * sizeof(uint32_t);
 }
 
 cudaError_t launch_window_keys(const int32_t* coords, int N, int batch, int grid_h, int grid_w, int S_h, int S_w,
                                int32_t* key, cudaStream_t st) {
   const int nwy = (grid_h + S_h - 1) / S_h, nwx = (grid_w + S_w - 1) / S_w;
   const unsigned blocks = (unsigned)(((long long)N + 255) / 256);
-  sla_window_key_kernel<<<blocks, 256, 0, st>>>((const int4*)coords, N, batch, grid_h, grid_w, S_h, S_w, nwy, nwx,
-                                                batch * nwy * nwx, key);
-  return cudaGetLastError();
+  return launch_chained(sla_window_key_kernel, blocks, 256, st, (const int4*)coords, N, batch, grid_h, grid_w, S_h,
+                        S_w, nwy, nwx, batch * nwy * nwx, key);
 }
 
 cudaError_t launch_sort_by_key(const int32_t* key, int N, int W, int32_t* perm, int32_t* key_sorted, void* ws,
@@ -186,26 +294,24 @@ cudaError_t launch_sort_by_key(const int32_t* key, int N, int W, int32_t* perm, 
   int32_t* key_tmp = (int32_t*)ws;
   int32_t* val_tmp = (int32_t*)((char*)ws + n4);
   uint32_t* cnt = (uint32_t*)((char*)ws + 2 * n4);
-  const int T = sort_tiles(N);
+  const int T = sort_blocks(N);
   int bits = 0;
   while (bits < 31 && (W >> bits) != 0) ++bits;           // keys lie in [0, W]
   const int passes = bits == 0 ? 1 : (bits + kDigitBits - 1) / kDigitBits;
-  const unsigned blocks = (unsigned)((T + kSortWarps - 1) / kSortWarps);
   const int32_t* kin = key;
   const int32_t* vin = nullptr;
-  for (int p = 0; p < passes; ++p) {
+  cudaError_t e = cudaSuccess;
+  for (int p = 0; p < passes && e == cudaSuccess; ++p) {
     const bool to_user = ((passes - 1 - p) & 1) == 0;      // ping-pong so that the last pass lands in the outputs
     int32_t* kout = to_user ? key_sorted : key_tmp;
     int32_t* vout = to_user ? perm : val_tmp;
     const int shift = p * kDigitBits;
-    sla_sort_hist_kernel<<<blocks, 32 * kSortWarps, 0, st>>>(kin, N, shift, T, cnt);
-    sla_sort_scan_kernel<<<1, kScanGroups * kBins, 0, st>>>(cnt, T);
-    if (p == 0) sla_sort_scatter_kernel<true><<<blocks, 32 * kSortWarps, 0, st>>>(kin, vin, N, shift, T, cnt, kout, vout);
-    else        sla_sort_scatter_kernel<false><<<blocks, 32 * kSortWarps, 0, st>>>(kin, vin, N, shift, T, cnt, kout, vout);
+    e = sort_steps(N) == kStepsSmall ? sort_pass<kStepsSmall>(kin, vin, N, shift, T, cnt, kout, vout, p == 0, st)
+                                     : sort_pass<kStepsLarge>(kin, vin, N, shift, T, cnt, kout, vout, p == 0, st);
     kin = kout;
     vin = vout;
   }
-  return cudaGetLastError();
+  return e;
 }
 
 cudaError_t launch_permute_rows(const void* src, const int32_t* perm, long long N, size_t row_bytes, void* dst,
@@ -214,16 +320,14 @@ cudaError_t launch_permute_rows(const void* src, const int32_t* perm, long long 
   const size_t vec = wide ? 16 : 4;
   const int vpr = (int)(row_bytes / vec);
   const unsigned long long total = (unsigned long long)N * (unsigned long long)vpr;
-  const unsigned blocks = (unsigned)((total + 255) / 256);
+  const unsigned long long per_block = 256ull * kPermUnroll;
+  const unsigned blocks = (unsigned)((total + per_block - 1) / per_block);
   if (blocks == 0) return cudaSuccess;
-  if (wide) {
-    if (scatter) sla_permute_rows_kernel<uint4, true><<<blocks, 256, 0, st>>>((const uint4*)src, perm, N, vpr, (uint4*)dst);
-    else         sla_permute_rows_kernel<uint4, false><<<blocks, 256, 0, st>>>((const uint4*)src, perm, N, vpr, (uint4*)dst);
-  } else {
-    if (scatter) sla_permute_rows_kernel<uint32_t, true><<<blocks, 256, 0, st>>>((const uint32_t*)src, perm, N, vpr, (uint32_t*)dst);
-    else         sla_permute_rows_kernel<uint32_t, false><<<blocks, 256, 0, st>>>((const uint32_t*)src, perm, N, vpr, (uint32_t*)dst);
-  }
-  return cudaGetLastError();
+  if (wide)
+    return scatter ? launch_chained(sla_permute_rows_kernel<uint4, true>, blocks, 256, st, (const uint4*)src, perm, N, vpr, (uint4*)dst)
+                   : launch_chained(sla_permute_rows_kernel<uint4, false>, blocks, 256, st, (const uint4*)src, perm, N, vpr, (uint4*)dst);
+  return scatter ? launch_chained(sla_permute_rows_kernel<uint32_t, true>, blocks, 256, st, (const uint32_t*)src, perm, N, vpr, (uint32_t*)dst)
+                 : launch_chained(sla_permute_rows_kernel<uint32_t, false>, blocks, 256, st, (const uint32_t*)src, perm, N, vpr, (uint32_t*)dst);
 }
 
 }  // namespace sla

@@ -71,6 +71,21 @@ def test_sort_by_window(W, n):
         assert np.array_equal(perm.cpu().numpy(), perm_w), (kind, "perm")
 
 
+@pytest.mark.parametrize("n", [131072, 131073, 200001, 262144, 262145, 300001, 524289])
+def test_sort_by_window_kernel_variants(n):
+    """Sizes on both sides of the library's switches (short/long warp tiles, scan inside the scatter kernel or
+    as a kernel of its own), two and three passes."""
+    torch = _torch()
+    for W in (3042, 70000):
+        rng = np.random.default_rng(n + W)
+        key = _keys("uniform", n, W, rng)
+        perm_w, ks_w = P.sort_by_window(key)
+        perm, ks = pkg.sla_sort_by_window(_dev(key), W)
+        torch.cuda.synchronize()
+        assert np.array_equal(ks.cpu().numpy(), ks_w)
+        assert np.array_equal(perm.cpu().numpy(), perm_w)
+
+
 def test_sort_empty_and_errors():
     torch = _torch()
     perm, ks = pkg.sla_sort_by_window(torch.empty(0, dtype=torch.int32, device="cuda"), 10)
