@@ -300,6 +300,42 @@ def other_config_legs(pkg, torch, dev, peak):
     return legs
 
 
+def sequence_prep_leg(pkg, torch, dev, peak):
+    """The sequence preparation on a config-1-sized scene: voxel coordinates in voxeliser order ->
+    keys + stable sort + offsets (one C call), then one gather of a [N,8,16] fp16 tensor.  Eager C-ABI calls, CUDA
+    events, cold L2 (a 256 MB buffer is overwritten before every call)."""
+    from paper_2401_00912_b200 import workloads as wl
+    N, batch, grid, win = 60000, 1, 468, 12
+    coords = torch.from_numpy(wl.coords_waymo_like(wl.SEED_BASE + 70, N=N, batch=batch)).to(dev)
+    x = torch.randn(N, 8, 16, device=dev, dtype=torch.float16)
+    y = torch.empty_like(x)
+    ws = torch.empty(int(pkg.load_library().sla_sequence_workspace_bytes(N)) + 16, dtype=torch.uint8, device=dev)
+    flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=dev)
+    perm = pkg.sla_sequence_from_coords(coords, batch, grid, grid, win, win, workspace=ws)[0]
+
+    def timed(fn, K=40):
+        ts = []
+        for i in range(K + 5):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fn()
+            b.record()
+            torch.cuda.synchronize()
+            if i >= 5:
+                ts.append(a.elapsed_time(b) * 1e3)
+        return sorted(ts)[len(ts) // 2]
+
+    seq_us = timed(lambda: pkg.sla_sequence_from_coords(coords, batch, grid, grid, win, win, workspace=ws))
+    gather_us = timed(lambda: pkg.sla_gather_rows(x, perm, out=y))
+    nb = 2 * x.numel() * 2 + 4 * N
+    return {"N": N, "W": pkg.sla_window_count(batch, grid, grid, win, win),
+            "sequence_from_coords_us": seq_us, "kernels_per_call": 6,
+            "gather_rows_us": gather_us, "gather_algorithmic_bytes": nb,
+            "gather_frac_of_peak": nb / (gather_us * 1e-6) / 1e9 / peak,
+            "timing": "median of 40 eager calls, one event pair per call (includes the binding's launch path), cold L2"}
+
+
 def ncu_traffic():
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the forward kernel on config 1, as recorded
     in the committed ncu summary of this round (a line `dram_bytes_per_launch: <int>`); None if absent."""
@@ -599,6 +635,7 @@ def run_ours(args):
         with torch.cuda.stream(side):
             line.update(extra_legs(pkg, torch, dev, peak))
             line["other_configs"] = other_config_legs(pkg, torch, dev, peak)
+            line["sequence_prep"] = sequence_prep_leg(pkg, torch, dev, peak)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         secs, cores = cpu_oracle_time(sc)
         line["cpu_baseline"] = {"value": N / secs, "unit": UNIT, "cores": cores, "kind": "oracle",
