@@ -361,7 +361,7 @@ template <int D> struct BwdSmem {
 
 // Backward kernel 1: whole (fused) windows completely; partial states of split windows.
 template <typename T, int D, bool RELU>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 2)
 sla_bwd_generic_kernel(const T* __restrict__ q, const T* __restrict__ k, const T* __restrict__ v,
                        const T* __restrict__ g, const int32_t* __restrict__ off, T* __restrict__ dq,
                        T* __restrict__ dk, T* __restrict__ dv, float* __restrict__ ws, int N, int W,
