@@ -130,6 +130,15 @@ int sla_backward(const void* q, const void* k, const void* v, const int32_t* win
                  void* dq, void* dk, void* dv,
                  void* workspace, size_t workspace_bytes, sla_stream_t stream);
 
+/* sla_backward when the caller knows an upper bound on the window length (see sla_forward_bounded): with
+ * 1 <= max_window_len <= 256 every window is differentiated whole by one thread block, so the call is ONE kernel
+ * launch and needs no workspace.  A window longer than the promise is undefined behaviour (not checked on the device);
+ * max_window_len > 256 -> SLA_ERR_UNSUPPORTED (call sla_backward).  Results are identical to sla_backward. */
+int sla_backward_bounded(const void* q, const void* k, const void* v, const int32_t* window_offsets,
+                         int64_t N, int32_t W, int32_t H, int32_t d_h, int dt,
+                         const void* d_out, void* dq, void* dk, void* dv,
+                         int32_t max_window_len, sla_stream_t stream);
+
 /* End-to-end host entry (what a user with host data calls): copies q,k,v (and win_id) from HOST
  * memory to the device, runs sla_offsets_from_window_ids + sla_forward, copies `out` back to HOST
  * memory and synchronises `stream` before returning.  Device scratch is taken from a stream-ordered

@@ -20,7 +20,7 @@ _PHI = {"elu1": SLA_PHI_ELU1, "relu": SLA_PHI_RELU}
 # Every symbol include/sla.h declares (tests check the library exports exactly these).
 SYMBOLS = (
     "sla_status_string", "sla_version", "sla_workspace_bytes", "sla_offsets_from_window_ids",
-    "sla_forward", "sla_forward_phi", "sla_backward_phi", "sla_forward_tcgen05", "sla_forward_bounded", "sla_backward", "sla_forward_host",
+    "sla_forward", "sla_forward_phi", "sla_backward_phi", "sla_forward_tcgen05", "sla_forward_bounded", "sla_backward", "sla_backward_bounded", "sla_forward_host",
     "sla_bench_stream_ceiling",
     "sla_window_count", "sla_window_keys", "sla_sort_workspace_bytes", "sla_sort_by_window", "sla_gather_rows",
     "sla_scatter_rows", "sla_sequence_workspace_bytes", "sla_sequence_from_coords",
@@ -64,6 +64,8 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     L.sla_forward_bounded.restype = ci
     L.sla_backward.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp, vp, vp, vp, sz, vp]
     L.sla_backward.restype = ci
+    L.sla_backward_bounded.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp, vp, vp, i32, vp]
+    L.sla_backward_bounded.restype = ci
     L.sla_forward_host.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp]
     L.sla_forward_host.restype = ci
     L.sla_bench_stream_ceiling.argtypes = [vp, vp, vp, vp, sz, vp]
@@ -179,8 +181,10 @@ def sla_forward(q, k, v, window_offsets, out=None, workspace=None, stream=None, 
 
 
 def sla_backward(q, k, v, window_offsets, d_out, dq=None, dk=None, dv=None, workspace=None, stream=None,
-                 phi="elu1", eps=0.0):
-    """Gradients of sum(d_out * SLA(q,k,v)) -> (dq, dk, dv), each [N,H,d_h] of the input dtype."""
+                 phi="elu1", eps=0.0, max_window_len=0):
+    """Gradients of sum(d_out * SLA(q,k,v)) -> (dq, dk, dv), each [N,H,d_h] of the input dtype.
+    max_window_len > 0 (a promise that no window is longer; <= 256) takes sla_backward_bounded: one kernel
+    launch, no workspace."""
     import torch
     L = load_library()
     _chk_dev(q, k, v, window_offsets, d_out)
@@ -195,6 +199,13 @@ def sla_backward(q, k, v, window_offsets, d_out, dq=None, dk=None, dv=None, work
     dq = torch.empty_like(q) if dq is None else dq
     dk = torch.empty_like(q) if dk is None else dk
     dv = torch.empty_like(q) if dv is None else dv
+    if max_window_len:
+        if phi != "elu1":
+            raise SlaError("sla_backward_bounded computes the elu+1 map only")
+        _check(L.sla_backward_bounded(q.data_ptr(), k.data_ptr(), v.data_ptr(), window_offsets.data_ptr(), N, W, H, d,
+                                      dt, d_out.data_ptr(), dq.data_ptr(), dk.data_ptr(), dv.data_ptr(),
+                                      int(max_window_len), _stream(stream)), "sla_backward_bounded")
+        return dq, dk, dv
     workspace, wsb = _workspace(q, N, W, H, d, dt, True, workspace)
     if phi != "elu1":
         _check(L.sla_backward_phi(q.data_ptr(), k.data_ptr(), v.data_ptr(), window_offsets.data_ptr(), N, W, H, d, dt,

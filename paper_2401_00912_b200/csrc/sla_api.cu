@@ -253,6 +253,29 @@ int sla_backward(const void* q, const void* k, const void* v, const int32_t* win
                        workspace_bytes, stream);
 }
 
+int sla_backward_bounded(const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
+                         int32_t W, int32_t H, int32_t d_h, int dt, const void* d_out, void* dq, void* dk, void* dv,
+                         int32_t max_window_len, sla_stream_t stream) {
+  int rc = check_common(N, W, H, d_h, dt);
+  if (rc != SLA_OK) return rc;
+  if (max_window_len < 1) return SLA_ERR_INVALID_ARG;
+  if (max_window_len > sla::kFuseMax) return SLA_ERR_UNSUPPORTED;   // use sla_backward
+  if (N == 0 || W == 0) return SLA_OK;
+  if (!q || !k || !v || !window_offsets || !d_out || !dq || !dk || !dv) return SLA_ERR_INVALID_ARG;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(d_out) || !aligned16(dq) ||
+      !aligned16(dk) || !aligned16(dv))
+    return SLA_ERR_UNSUPPORTED;
+  sla::Problem p{};
+  p.q = q; p.k = k; p.v = v; p.g = d_out; p.dq = dq; p.dk = dk; p.dv = dv; p.off = window_offsets;
+  p.N = (int)N; p.W = W; p.H = H; p.d = d_h;
+  p.phi = SLA_PHI_ELU1; p.eps = 0.f;
+  p.bounded = true;                                           // one launch: no workspace, no split passes
+  const bool tc = sla::backward_tc_supported(p, dt);
+  cudaError_t e = tc ? sla::launch_backward_tc(p, dt, (cudaStream_t)stream)
+                     : sla::launch_backward_generic(p, dt, (cudaStream_t)stream);
+  return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
+}
+
 int sla_backward_phi(const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
                      int32_t W, int32_t H, int32_t d_h, int dt, int feature_map, float eps, const void* d_out,
                      void* dq, void* dk, void* dv, void* workspace, size_t workspace_bytes, sla_stream_t stream) {

@@ -491,6 +491,9 @@ sla_bwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
                   T* __restrict__ dv, float* __restrict__ ws, int N, int W, int H, int span) {
   extern __shared__ uint8_t dyn_smem[];
   __shared__ Ctrl ctrl;
+  // programmatic dependent launch, as the forward: resident behind the previous kernel's tail, barrier set-up runs
+  // ahead, nothing that kernel may have written is touched before griddepcontrol.wait
+  asm volatile("griddepcontrol.launch_dependents;");
   const uint32_t ring = (smem_u32(dyn_smem) + 1023u) & ~1023u;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int nspan = gridDim.x, bx = blockIdx.x;
@@ -508,6 +511,7 @@ sla_bwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   __syncthreads();
 
   if (warp >= NW) {
@@ -583,7 +587,8 @@ sla_bwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
     const int m = e - s;
     if (m <= 0) { ++w; continue; }
     if (m > kFuseMax) {                                   // left to the split passes
-      if (hl == 0 && lane == 0) reinterpret_cast<volatile int*>(ws)[0] = 1;
+      // bounded entry (no workspace): a window that breaks the caller's promise is skipped
+      if (ws != nullptr && hl == 0 && lane == 0) reinterpret_cast<volatile int*>(ws)[0] = 1;
       ++w;
       continue;
     }
@@ -643,6 +648,8 @@ sla_bwd_tc_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_co
                         float* __restrict__ ws, float* __restrict__ wd, int N, int W, int H, int span) {
   extern __shared__ uint8_t dyn_smem[];
   __shared__ Ctrl ctrl;
+  asm volatile("griddepcontrol.launch_dependents;");
+  asm volatile("griddepcontrol.wait;" ::: "memory");               // every CTA waits, so completion is transitive
   if (reinterpret_cast<const volatile int*>(ws)[0] == 0) return;   // no long window in this call
   const uint32_t ring = (smem_u32(dyn_smem) + 1023u) & ~1023u;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -810,9 +817,21 @@ cudaError_t bwd_tc_launch(const Problem& p, cudaStream_t st) {
     attr_set[dev].store(true, std::memory_order_release);
   }
   const int span = 32;   // short spans: the grid runs in many waves (dynamic balance)
-  dim3 grid((p.N + span - 1) / span, (p.H + NW - 1) / NW);
-  kern<<<grid, C::THREADS, C::SMEM_DYN, st>>>(tq, tk, tv, tg, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state,
-                                              p.N, p.W, p.H, span);
+  const int slabs = (p.H + NW - 1) / NW;
+  // one chain of programmatic dependent launches: zeroing kernel -> main -> the three split passes
+  cudaLaunchAttribute pdl[1];
+  pdl[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  pdl[0].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((p.N + span - 1) / span, slabs);
+  cfg.blockDim = dim3(C::THREADS);
+  cfg.dynamicSmemBytes = C::SMEM_DYN;
+  cfg.stream = st;
+  cfg.attrs = pdl;
+  cfg.numAttrs = 1;
+  cudaError_t le = cudaLaunchKernelEx(&cfg, kern, tq, tk, tv, tg, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state,
+                                      p.N, p.W, p.H, span);
+  if (le != cudaSuccess || p.bounded) return le;   // bounded entry: no window is left to the split passes
   // windows longer than kFuseMax rows: three passes over their pieces (each exits at once if there is none)
   auto k0 = sla_bwd_tc_split_kernel<BF16, T, 0>;
   auto k1 = sla_bwd_tc_split_kernel<BF16, T, 1>;
@@ -826,14 +845,16 @@ cudaError_t bwd_tc_launch(const Problem& p, cudaStream_t st) {
     attr2_set[dev].store(true, std::memory_order_release);
   }
   const int span2 = 128;                                   // <= kFuseMax; few pieces per window = few atomics per slot
-  dim3 grid2((p.N + span2 - 1) / span2, (p.H + NW - 1) / NW);
-  k0<<<grid2, C::THREADS, C::SMEM_DYN, st>>>(tk, tv, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state, p.ws_dstate,
-                                             p.N, p.W, p.H, span2);
-  k1<<<grid2, C::THREADS, C::SMEM_DYN, st>>>(tq, tg, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state, p.ws_dstate,
-                                             p.N, p.W, p.H, span2);
-  k2<<<grid2, C::THREADS, C::SMEM_DYN, st>>>(tk, tv, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state, p.ws_dstate,
-                                             p.N, p.W, p.H, span2);
-  return cudaGetLastError();
+  cfg.gridDim = dim3((p.N + span2 - 1) / span2, slabs);
+  le = cudaLaunchKernelEx(&cfg, k0, tk, tv, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state, p.ws_dstate, p.N, p.W,
+                          p.H, span2);
+  if (le == cudaSuccess)
+    le = cudaLaunchKernelEx(&cfg, k1, tq, tg, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state, p.ws_dstate, p.N, p.W,
+                            p.H, span2);
+  if (le == cudaSuccess)
+    le = cudaLaunchKernelEx(&cfg, k2, tk, tv, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state, p.ws_dstate, p.N, p.W,
+                            p.H, span2);
+  return le;
 }
 
 }  // namespace

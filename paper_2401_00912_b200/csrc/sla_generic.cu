@@ -396,6 +396,7 @@ sla_bwd_generic_kernel(const T* __restrict__ q, const T* __restrict__ k, const T
       transpose_state<D>(dScol, dSrow, cx, sm);
       backward_key_pass<T, D>(k, v, dk, dv, s, e, cx, bsA, bsB, dScol, dSrow, dz);
     } else {
+      if (ws == nullptr) continue;   // bounded entry (no workspace): a window that breaks the caller's promise is skipped
       accumulate_state<T, D>(k, v, max(s, row0), min(e, row1), cx, bsA, Scol, z);
       if (threadIdx.x == 0) reinterpret_cast<volatile int*>(ws)[0] = 1;
       if (cx.active) {
@@ -507,6 +508,7 @@ cudaError_t bwd_launch(const Problem& p, cudaStream_t st, int split_only = 0) {
   sla_bwd_generic_kernel<T, D, RELU><<<grid, CB, 0, st>>>((const T*)p.q, (const T*)p.k, (const T*)p.v,
                                                     (const T*)p.g, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv,
                                                     p.ws_state, p.N, p.W, p.H, split_only, p.eps);
+  if (p.bounded) return cudaGetLastError();   // no window is left to the split kernels
   sla_bwd_generic_split_q_kernel<T, D, RELU><<<grid, CB, 0, st>>>((const T*)p.q, (const T*)p.g, p.off,
                                                             (T*)p.dq, p.ws_state, p.ws_dstate, p.N, p.W,
                                                             p.H, p.eps);

@@ -409,6 +409,40 @@ def test_forward_bounded_generic_path_and_errors():
         pkg.sla_forward(*(to_dev(a, "f32") for a in (q, k, v)), off, max_window_len=1000)
 
 
+@pytest.mark.parametrize("c", [1, 4])
+def test_backward_bounded_entry_matches_general_and_oracle(c):
+    """sla_backward_bounded (one launch, no workspace) must give exactly what sla_backward gives, and pass the
+    gradient criterion against the oracle."""
+    torch = _torch()
+    sc = wl.make_config(c)
+    assert int(sc.lengths.max()) <= 144
+    q, k, v, g = (sc.tensor(n) for n in ("q", "k", "v", "do"))
+    off = torch.from_numpy(sc.offsets).cuda()
+    tq, tk, tv, tg = (to_dev(a, sc.dtype) for a in (q, k, v, g))
+    gb = pkg.sla_backward(tq, tk, tv, off, tg, max_window_len=144)
+    gg = pkg.sla_backward(tq, tk, tv, off, tg)
+    torch.cuda.synchronize()
+    for a, b in zip(gb, gg):
+        assert torch.equal(a, b)
+    check_grads(gb, sla_oracle.backward(q, k, v, g, sc.offsets, nthreads=8), sc)
+
+
+@pytest.mark.parametrize("dtype,d", [("f32", 32), ("bf16", 32), ("f32", 16)])
+def test_backward_bounded_generic_path_and_errors(dtype, d):
+    torch = _torch()
+    sc = wl.make_scene([5, 1, 144, 33, 2, 100, 16, 17, 256], 4, d, dtype, seed=13)
+    q, k, v, g = (sc.tensor(n) for n in ("q", "k", "v", "do"))
+    off = torch.from_numpy(sc.offsets).cuda()
+    dev = [to_dev(a, dtype) for a in (q, k, v)]
+    grads = pkg.sla_backward(*dev, off, to_dev(g, dtype), max_window_len=256)
+    torch.cuda.synchronize()
+    check_grads(grads, sla_oracle.backward(q, k, v, g, sc.offsets), sc)
+    with pytest.raises(pkg.SlaError, match="UNSUPPORTED"):
+        pkg.sla_backward(*dev, off, to_dev(g, dtype), max_window_len=257)
+    with pytest.raises(pkg.SlaError):
+        pkg.sla_backward(*dev, off, to_dev(g, dtype), max_window_len=16, phi="relu", eps=1e-6)
+
+
 def test_forward_under_cuda_graph_replay():
     """The C-ABI calls are capturable: a graph of prep + forward replays to the same result."""
     torch = _torch()
