@@ -124,10 +124,16 @@ __device__ __forceinline__ void bwd_kv_tile(const RingView& rv, int hl, int rel0
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
     const int j0 = 2 * t + 8 * (i >> 1);
-    const float2 x = unpack2<BF16>(kr[i]);
-    const float b0 = (j0 < nvalid) ? phi_fast(x.x) : 0.f;
-    const float b1 = (j0 + 1 < nvalid) ? phi_fast(x.y) : 0.f;
-    to_op<PRECISE>(b0, b1, bh[i], bl[i]);
+    if (PRECISE) {
+      const float2 x = unpack2<BF16>(kr[i]);
+      const float b0 = (j0 < nvalid) ? phi_fast(x.x) : 0.f;
+      const float b1 = (j0 + 1 < nvalid) ? phi_fast(x.y) : 0.f;
+      to_op<true>(b0, b1, bh[i], bl[i]);
+    } else {   // long window: phi in fp16x2 (the operand is a single fp16 anyway), rows beyond the window zeroed
+      bh[i] = phi_h2<BF16>(kr[i]);
+      if (nvalid < 16) bh[i] &= pair_mask(j0, nvalid);
+      bl[i] = 0u;
+    }
   }
   if (BF16) {
 #pragma unroll
@@ -170,13 +176,18 @@ __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0,
   ldsm_x4(ring_addr<D>(rv, C::KV_STAGE, 0, rel0 + trow, chunk), qn);
   ldsm_x4(ring_addr<D>(rv, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), gn);
   // A fragments: index 0: (row g, cols 2t..), 1: (row g+8, cols 2t..), 2: (row g, cols 8+2t..), 3: (row g+8, 8+2t..)
-  uint32_t ah[4], al[4];
+  uint32_t ah[4], al[4], dph2[4];   // dph2: phi'(q) as fp16x2 (long windows)
   float2 dph[4], gv[4];
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
-    float2 a;
-    phi_pair<BF16>(qn[perm[i]], a, dph[i]);
-    to_op<PRECISE>(a.x, a.y, ah[i], al[i]);
+    if (PRECISE) {
+      float2 a;
+      phi_pair<BF16>(qn[perm[i]], a, dph[i]);
+      to_op<true>(a.x, a.y, ah[i], al[i]);
+    } else {
+      phi_dphi_h2<BF16>(qn[perm[i]], ah[i], dph2[i]);
+      al[i] = 0u;
+    }
     gv[i] = unpack2<BF16>(gn[perm[i]]);
   }
   float num[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}}, den[4] = {0.f, 0.f, 0.f, 0.f};
@@ -192,24 +203,34 @@ __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0,
   const float dden0 = -(go0 * inv0) * inv0, dden1 = -(go1 * inv1) * inv1;   // o = num*inv
   // dnum as A fragment (rows g / g+8 scaled by their 1/den)
   uint32_t dh[4], dl[4];
-  to_op<PRECISE>(gv[0].x * inv0, gv[0].y * inv0, dh[0], dl[0]);
-  to_op<PRECISE>(gv[1].x * inv1, gv[1].y * inv1, dh[1], dl[1]);
-  to_op<PRECISE>(gv[2].x * inv0, gv[2].y * inv0, dh[2], dl[2]);
-  to_op<PRECISE>(gv[3].x * inv1, gv[3].y * inv1, dh[3], dl[3]);
+  if (PRECISE || BF16) {
+    to_op<PRECISE>(gv[0].x * inv0, gv[0].y * inv0, dh[0], dl[0]);
+    to_op<PRECISE>(gv[1].x * inv1, gv[1].y * inv1, dh[1], dl[1]);
+    to_op<PRECISE>(gv[2].x * inv0, gv[2].y * inv0, dh[2], dl[2]);
+    to_op<PRECISE>(gv[3].x * inv1, gv[3].y * inv1, dh[3], dl[3]);
+  } else {   // fp16 dO, long window: scale the packed pairs directly
+    const uint32_t i0h = pack_h2(inv0, inv0), i1h = pack_h2(inv1, inv1);
+    dh[0] = hmul2_u32(gn[perm[0]], i0h); dh[1] = hmul2_u32(gn[perm[1]], i1h);
+    dh[2] = hmul2_u32(gn[perm[2]], i0h); dh[3] = hmul2_u32(gn[perm[3]], i1h);
+    dl[0] = dl[1] = dl[2] = dl[3] = 0u;
+  }
   // da = dnum S^T + dden z ; dq = da * phi'(q)
 #pragma unroll
   for (int np = 0; np < 2; ++np) {
     float da[4] = {0.f, 0.f, 0.f, 0.f};
     mma3<PRECISE>(da, dh, dl, op.da.hi[np][0], op.da.hi[np][1], op.da.lo[np][0], op.da.lo[np][1]);
     // C fragment (np): c0,c1 = (row g, p = 8np+2t,+1) <-> A index 2*np ; c2,c3 = row g+8 <-> A index 2*np+1
-    const float q0 = (da[0] + dden0 * op.zs[np][0]) * dph[2 * np].x;
-    const float q1 = (da[1] + dden0 * op.zs[np][1]) * dph[2 * np].y;
-    const float q2 = (da[2] + dden1 * op.zs[np][0]) * dph[2 * np + 1].x;
-    const float q3 = (da[3] + dden1 * op.zs[np][1]) * dph[2 * np + 1].y;
+    const float q0 = da[0] + dden0 * op.zs[np][0], q1 = da[1] + dden0 * op.zs[np][1];
+    const float q2 = da[2] + dden1 * op.zs[np][0], q3 = da[3] + dden1 * op.zs[np][1];
     uint32_t* p0 = reinterpret_cast<uint32_t*>(dq_rows + (size_t)g * C_total + 8 * np + 2 * t);
     uint32_t* p1 = reinterpret_cast<uint32_t*>(dq_rows + (size_t)(g + 8) * C_total + 8 * np + 2 * t);
-    if (g < nvalid) *p0 = pack_out<BF16>(q0, q1);
-    if (g + 8 < nvalid) *p1 = pack_out<BF16>(q2, q3);
+    if (PRECISE) {
+      if (g < nvalid) *p0 = pack_out<BF16>(q0 * dph[2 * np].x, q1 * dph[2 * np].y);
+      if (g + 8 < nvalid) *p1 = pack_out<BF16>(q2 * dph[2 * np + 1].x, q3 * dph[2 * np + 1].y);
+    } else {
+      if (g < nvalid) *p0 = pack_out_times_h2<BF16>(q0, q1, dph2[2 * np]);
+      if (g + 8 < nvalid) *p1 = pack_out_times_h2<BF16>(q2, q3, dph2[2 * np + 1]);
+    }
   }
   // ---- transposed operands (contraction over the rows i of the tile) ----
   uint32_t qt[4], gt[4];
@@ -226,13 +247,24 @@ __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0,
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
     const int i0 = 2 * t + 8 * (i >> 1);
-    const float2 x = unpack2<BF16>(qt[i]);
-    const float a0 = (i0 < nvalid) ? phi_fast(x.x) : 0.f;       // rows beyond the window contribute nothing
-    const float a1 = (i0 + 1 < nvalid) ? phi_fast(x.y) : 0.f;
-    to_op<PRECISE>(a0, a1, uh[i], ul[i]);
-    const float2 gg = unpack2<BF16>(gt[i]);
     const float s0 = (i >> 1) ? ir2 : ir0, s1 = (i >> 1) ? ir3 : ir1;
-    to_op<PRECISE>(gg.x * s0, gg.y * s1, th[i], tl[i]);
+    if (PRECISE) {
+      const float2 x = unpack2<BF16>(qt[i]);
+      const float a0 = (i0 < nvalid) ? phi_fast(x.x) : 0.f;       // rows beyond the window contribute nothing
+      const float a1 = (i0 + 1 < nvalid) ? phi_fast(x.y) : 0.f;
+      to_op<true>(a0, a1, uh[i], ul[i]);
+    } else {
+      uh[i] = phi_h2<BF16>(qt[i]);
+      if (nvalid < 16) uh[i] &= pair_mask(i0, nvalid);
+      ul[i] = 0u;
+    }
+    if (PRECISE || BF16) {
+      const float2 gg = unpack2<BF16>(gt[i]);
+      to_op<PRECISE>(gg.x * s0, gg.y * s1, th[i], tl[i]);
+    } else {
+      th[i] = hmul2_u32(gt[i], pack_h2(s0, s1));
+      tl[i] = 0u;
+    }
   }
   uint32_t ddh[2], ddl[2];
   to_op<PRECISE>(dd0, dd1, ddh[0], ddl[0]);
@@ -268,14 +300,18 @@ __device__ __forceinline__ void bwd_kv_out_tile(const RingView& rv, int hl, int 
   uint32_t kn[4], vn[4];
   ldsm_x4(ring_addr<D>(rv, C::KV_STAGE, 0, rel0 + trow, chunk), kn);
   ldsm_x4(ring_addr<D>(rv, C::KV_STAGE, C::T_STAGE, rel0 + trow, chunk), vn);
-  uint32_t bh[4], bl[4], vh[4];
-  const uint32_t vzero[4] = {0u, 0u, 0u, 0u};
+  uint32_t bh[4], bl[4], vh[4], dph2[4];
   float2 dph[4];
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
-    float2 b;
-    phi_pair<BF16>(kn[perm[i]], b, dph[i]);
-    to_op<PRECISE>(b.x, b.y, bh[i], bl[i]);
+    if (PRECISE) {
+      float2 b;
+      phi_pair<BF16>(kn[perm[i]], b, dph[i]);
+      to_op<true>(b.x, b.y, bh[i], bl[i]);
+    } else {
+      phi_dphi_h2<BF16>(kn[perm[i]], bh[i], dph2[i]);
+      bl[i] = 0u;
+    }
     if (BF16) { const float2 x = unpack2<true>(vn[perm[i]]); vh[i] = pack_h2(x.x, x.y); }
     else vh[i] = vn[perm[i]];
   }
@@ -285,17 +321,18 @@ __device__ __forceinline__ void bwd_kv_out_tile(const RingView& rv, int hl, int 
     mma3<PRECISE>(dv, bh, bl, op.dv.hi[n][0], op.dv.hi[n][1], op.dv.lo[n][0], op.dv.lo[n][1]);
     mma16816(db, vh[0], vh[1], vh[2], vh[3], op.db.hi[n][0], op.db.hi[n][1]);
     if (PRECISE) mma16816(db, vh[0], vh[1], vh[2], vh[3], op.db.lo[n][0], op.db.lo[n][1]);   // v is exact
-    (void)vzero;
-    const float k0 = (db[0] + op.dzs[n][0]) * dph[2 * n].x, k1 = (db[1] + op.dzs[n][1]) * dph[2 * n].y;
-    const float k2 = (db[2] + op.dzs[n][0]) * dph[2 * n + 1].x, k3 = (db[3] + op.dzs[n][1]) * dph[2 * n + 1].y;
+    const float k0 = db[0] + op.dzs[n][0], k1 = db[1] + op.dzs[n][1];
+    const float k2 = db[2] + op.dzs[n][0], k3 = db[3] + op.dzs[n][1];
     const size_t o0 = (size_t)g * C_total + 8 * n + 2 * t, o1 = (size_t)(g + 8) * C_total + 8 * n + 2 * t;
     if (g < nvalid) {
       *reinterpret_cast<uint32_t*>(dv_rows + o0) = pack_out<BF16>(dv[0], dv[1]);
-      *reinterpret_cast<uint32_t*>(dk_rows + o0) = pack_out<BF16>(k0, k1);
+      *reinterpret_cast<uint32_t*>(dk_rows + o0) = PRECISE ? pack_out<BF16>(k0 * dph[2 * n].x, k1 * dph[2 * n].y)
+                                                           : pack_out_times_h2<BF16>(k0, k1, dph2[2 * n]);
     }
     if (g + 8 < nvalid) {
       *reinterpret_cast<uint32_t*>(dv_rows + o1) = pack_out<BF16>(dv[2], dv[3]);
-      *reinterpret_cast<uint32_t*>(dk_rows + o1) = pack_out<BF16>(k2, k3);
+      *reinterpret_cast<uint32_t*>(dk_rows + o1) = PRECISE ? pack_out<BF16>(k2 * dph[2 * n + 1].x, k3 * dph[2 * n + 1].y)
+                                                           : pack_out_times_h2<BF16>(k2, k3, dph2[2 * n + 1]);
     }
   }
 }
@@ -816,7 +853,10 @@ cudaError_t bwd_tc_launch(const Problem& p, cudaStream_t st) {
     if (e != cudaSuccess) return e;
     attr_set[dev].store(true, std::memory_order_release);
   }
-  const int span = 32;   // short spans: the grid runs in many waves (dynamic balance)
+#ifndef SLA_BWD_SPAN
+#define SLA_BWD_SPAN 64
+#endif
+  const int span = SLA_BWD_SPAN;   // short spans: the grid runs in many waves (dynamic balance)
   const int slabs = (p.H + NW - 1) / NW;
   // one chain of programmatic dependent launches: zeroing kernel -> main -> the three split passes
   cudaLaunchAttribute pdl[1];

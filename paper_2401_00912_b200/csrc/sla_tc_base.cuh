@@ -110,6 +110,38 @@ __device__ __forceinline__ uint32_t phi_h2(uint32_t raw) {
   asm("fma.rn.f16x2 %0, %1, %2, %3;" : "=r"(out) : "r"(r), "r"(ln2), "r"(e));
   return out;
 }
+// elu+1 and its derivative on two packed I/O elements in fp16x2 (the backward's long windows): the same four
+// instructions as phi_h2; 2^t is phi'(x) = (x > 0 ? 1 : e^x) (for x > 0, t is the rounding residual: 1 +- 1.5 ulp).
+template <bool BF16>
+__device__ __forceinline__ void phi_dphi_h2(uint32_t raw, uint32_t& phi, uint32_t& dphi) {
+  uint32_t x = raw;
+  if (BF16) { float2 f = unpack2<true>(raw); x = pack_h2(f.x, f.y); }
+  uint32_t r, t;
+  const uint32_t log2e = 0x3DC53DC5u, ln2 = 0x398C398Cu, zero = 0u;
+  asm("fma.rn.relu.f16x2 %0, %1, %2, %3;" : "=r"(r) : "r"(x), "r"(log2e), "r"(zero));
+  asm("{\n\t.reg .b32 nr;\n\tneg.f16x2 nr, %3;\n\tfma.rn.f16x2 %0, %1, %2, nr;\n\t}"
+      : "=r"(t) : "r"(x), "r"(log2e), "r"(r));
+  asm("ex2.approx.f16x2 %0, %1;" : "=r"(dphi) : "r"(t));
+  asm("fma.rn.f16x2 %0, %1, %2, %3;" : "=r"(phi) : "r"(r), "r"(ln2), "r"(dphi));
+}
+// (v0, v1) * f (fp16x2) -> two packed output elements
+template <bool BF16>
+__device__ __forceinline__ uint32_t pack_out_times_h2(float v0, float v1, uint32_t f) {
+  if (BF16) {
+    const float2 ff = __half22float2(*reinterpret_cast<const __half2*>(&f));
+    return pack_out<true>(v0 * ff.x, v1 * ff.y);
+  }
+  __half2 r = __hmul2(__floats2half2_rn(v0, v1), *reinterpret_cast<const __half2*>(&f));
+  return *reinterpret_cast<uint32_t*>(&r);
+}
+__device__ __forceinline__ uint32_t hmul2_u32(uint32_t a, uint32_t b) {
+  __half2 r = __hmul2(*reinterpret_cast<const __half2*>(&a), *reinterpret_cast<const __half2*>(&b));
+  return *reinterpret_cast<uint32_t*>(&r);
+}
+// mask of the packed pair (j0, j0+1): keeps the elements whose index is below nvalid
+__device__ __forceinline__ uint32_t pair_mask(int j0, int nvalid) {
+  return ((j0 < nvalid) ? 0x0000FFFFu : 0u) | ((j0 + 1 < nvalid) ? 0xFFFF0000u : 0u);
+}
 __device__ __forceinline__ float fast_rcp(float x) {
   float r;
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
