@@ -37,7 +37,8 @@ typedef enum {
   SLA_ERR_INVALID_ARG = 1,  /* NULL pointer, negative size, N >= 2^31 */
   SLA_ERR_UNSUPPORTED = 2,  /* d_h not in {16,32}, misaligned pointer, bad dtype */
   SLA_ERR_WORKSPACE = 3,    /* workspace NULL or smaller than sla_workspace_bytes() */
-  SLA_ERR_CUDA = 4          /* a CUDA runtime call failed (sticky error left for the caller) */
+  SLA_ERR_CUDA = 4,         /* a CUDA runtime call failed (sticky error left for the caller) */
+  SLA_ERR_TOO_LARGE = 5     /* sla_forward_static: the problem needs more than SLA_STATIC_WORKSPACE_BYTES of scratch */
 } sla_status_t;
 
 typedef enum { SLA_F32 = 0, SLA_F16 = 1, SLA_BF16 = 2 } sla_dtype_t;
@@ -104,6 +105,22 @@ int sla_backward_phi(const void* q, const void* k, const void* v, const int32_t*
 int sla_forward_tcgen05(const void* q, const void* k, const void* v, const int32_t* window_offsets,
                         int64_t N, int32_t W, int32_t H, int32_t d_h, int dt, void* out,
                         void* workspace, size_t workspace_bytes, sla_stream_t stream);
+
+/* sla_forward for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): the same operation, arguments, kernels and results as sla_forward, but the workspace is a
+ * static device array inside the library, so the caller passes none and the call allocates nothing -- no cudaMalloc,
+ * cudaFree or allocating library routine, in the library or asked of the caller.
+ *   - The array has SLA_STATIC_WORKSPACE_BYTES (4 MiB); every GPU that loads the library holds it until exit.
+ *   - A problem fits iff sla_workspace_bytes(N, W, H, d_h, dt, 0) <= SLA_STATIC_WORKSPACE_BYTES, i.e. about
+ *     N * H * (d_h + 1) * d_h * 4 / 257 bytes: N up to ~123 000 voxels at H = 8, d_h = 16 (configs 1 and 4 fit, config 2
+ *     does not).  Anything larger -> SLA_ERR_TOO_LARGE, nothing launched; call sla_forward with your own workspace.
+ *   - All calls on one device share the array, and it keeps the previous call's contents: each call zeroes the part
+ *     it uses on `stream` before its kernels run.  Calls that may overlap on the GPU (different streams, or graphs
+ *     replayed concurrently) RACE on it; serialise them, or use sla_forward with one workspace per stream.
+ *   - The array's device address is looked up once per device (cudaGetSymbolAddress) on the first call there. */
+#define SLA_STATIC_WORKSPACE_BYTES (4u << 20)
+int sla_forward_static(const void* q, const void* k, const void* v, const int32_t* window_offsets,
+                       int64_t N, int32_t W, int32_t H, int32_t d_h, int dt, void* out, sla_stream_t stream);
 
 /* SLA forward when the caller knows an upper bound on the window length.  In ScatterFormer a window
  * is a fixed block of BEV cells (12x12 on Waymo), so no window can hold more than 144

@@ -20,7 +20,7 @@ _PHI = {"elu1": SLA_PHI_ELU1, "relu": SLA_PHI_RELU}
 # Every symbol include/sla.h declares (tests check the library exports exactly these).
 SYMBOLS = (
     "sla_status_string", "sla_version", "sla_workspace_bytes", "sla_offsets_from_window_ids",
-    "sla_forward", "sla_forward_phi", "sla_backward_phi", "sla_forward_tcgen05", "sla_forward_bounded", "sla_backward", "sla_backward_bounded", "sla_forward_host",
+    "sla_forward", "sla_forward_phi", "sla_backward_phi", "sla_forward_tcgen05", "sla_forward_static", "sla_forward_bounded", "sla_backward", "sla_backward_bounded", "sla_forward_host",
     "sla_bench_stream_ceiling",
     "sla_window_count", "sla_window_keys", "sla_sort_workspace_bytes", "sla_sort_by_window", "sla_gather_rows",
     "sla_scatter_rows", "sla_sequence_workspace_bytes", "sla_sequence_from_coords",
@@ -60,6 +60,8 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     L.sla_backward_phi.restype = ci
     L.sla_forward_tcgen05.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp, sz, vp]
     L.sla_forward_tcgen05.restype = ci
+    L.sla_forward_static.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp]
+    L.sla_forward_static.restype = ci
     L.sla_forward_bounded.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, i32, vp]
     L.sla_forward_bounded.restype = ci
     L.sla_backward.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp, vp, vp, vp, sz, vp]
@@ -340,3 +342,23 @@ def sla_sequence_from_coords(coords, batch: int, grid_h: int, grid_w: int, S_h: 
                                       ks.data_ptr(), off.data_ptr(), workspace.data_ptr(), workspace.numel(),
                                       _stream(stream)), "sla_sequence_from_coords")
     return perm, ks, off
+
+
+def sla_forward_static(q, k, v, window_offsets, out=None, stream=None):
+    """sla_forward with the workspace in the library's static device array (include/sla.h): the C call allocates
+    nothing; problems whose workspace exceeds 4 MiB raise SLA_ERR_TOO_LARGE.  `out` may be passed in so that this
+    wrapper allocates nothing either."""
+    import torch
+    L = load_library()
+    _chk_dev(q, k, v, window_offsets)
+    if not (q.shape == k.shape == v.shape and q.dim() == 3 and q.dtype == k.dtype == v.dtype):
+        raise SlaError("q,k,v must share shape [N,H,d_h] and dtype")
+    if window_offsets.dtype != torch.int32:
+        raise SlaError("window_offsets must be int32")
+    N, H, d = q.shape
+    if out is None:
+        out = torch.empty_like(q)
+    _check(L.sla_forward_static(q.data_ptr(), k.data_ptr(), v.data_ptr(), window_offsets.data_ptr(), N,
+                                window_offsets.numel() - 1, H, d, _dt(q), out.data_ptr(), _stream(stream)),
+           "sla_forward_static")
+    return out

@@ -25,6 +25,28 @@ int check_common(int64_t N, int32_t W, int32_t H, int32_t d_h, int dt) {
   return SLA_OK;
 }
 
+// ---- sla_forward_static: the forward's workspace in a file-scope device array, so the call allocates nothing ----
+// One array per GPU that loads the library, held until exit.  Every sla_forward_static call on a device shares it.
+static __device__ __align__(256) unsigned char g_static_workspace[SLA_STATIC_WORKSPACE_BYTES];
+
+// In host code `g_static_workspace` is only a handle for the symbol, not a device address: the address a kernel may
+// use comes from cudaGetSymbolAddress, asked once per device with that device current, here in the array's own file.
+int static_workspace(void** ptr) {
+  static std::mutex mu;
+  static void* addr[64] = {};
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) return SLA_ERR_CUDA;
+  if (dev < 0 || dev >= 64) return SLA_ERR_UNSUPPORTED;
+  std::lock_guard<std::mutex> lock(mu);
+  if (!addr[dev]) {
+    void* p = nullptr;
+    if (cudaGetSymbolAddress(&p, g_static_workspace) != cudaSuccess || !p) return SLA_ERR_CUDA;
+    addr[dev] = p;
+  }
+  *ptr = addr[dev];
+  return SLA_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -36,6 +58,7 @@ const char* sla_status_string(int status) {
     case SLA_ERR_UNSUPPORTED: return "SLA_ERR_UNSUPPORTED";
     case SLA_ERR_WORKSPACE: return "SLA_ERR_WORKSPACE";
     case SLA_ERR_CUDA: return "SLA_ERR_CUDA";
+    case SLA_ERR_TOO_LARGE: return "SLA_ERR_TOO_LARGE";
     default: return "SLA_ERR_UNKNOWN";
   }
 }
@@ -199,6 +222,22 @@ int sla_forward_tcgen05(const void* q, const void* k, const void* v, const int32
                         int32_t W, int32_t H, int32_t d_h, int dt, void* out, void* workspace,
                         size_t workspace_bytes, sla_stream_t stream) {
   return forward_impl(true, SLA_PHI_ELU1, 0.f, q, k, v, window_offsets, N, W, H, d_h, dt, out, workspace, workspace_bytes, stream);
+}
+
+int sla_forward_static(const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
+                       int32_t W, int32_t H, int32_t d_h, int dt, void* out, sla_stream_t stream) {
+  const int rc = check_common(N, W, H, d_h, dt);
+  if (rc != SLA_OK) return rc;
+  if (N == 0 || W == 0) return SLA_OK;
+  // what sla_forward would ask the caller for must fit the static array; checked before anything is launched
+  if (state_bytes(N, H, d_h) > (size_t)SLA_STATIC_WORKSPACE_BYTES) return SLA_ERR_TOO_LARGE;
+  void* ws = nullptr;
+  const int rs = static_workspace(&ws);
+  if (rs != SLA_OK) return rs;
+  // from here on the general entry's own path (it zeroes the part of the workspace it uses on `stream` first): the
+  // array keeps the previous call's contents, and two calls that overlap on the GPU would race on it
+  return forward_impl(false, SLA_PHI_ELU1, 0.f, q, k, v, window_offsets, N, W, H, d_h, dt, out, ws,
+                      (size_t)SLA_STATIC_WORKSPACE_BYTES, stream);
 }
 
 int sla_forward_bounded(const void* q, const void* k, const void* v, const int32_t* window_offsets,
