@@ -901,7 +901,7 @@ cudaError_t bwd_tc_launch(const Problem& p, cudaStream_t st) {
 
 bool backward_tc_supported(const Problem& p, int dt) {
   if (dt != SLA_F16 && dt != SLA_BF16) return false;
-  if (p.d != 16 || (p.H * p.d) % 64 != 0) return false;
+  if ((p.d != 16 && p.d != 32) || (p.H * p.d) % 64 != 0) return false;     // d_h = 32: sla_bwd_tc32.cu
   if (p.phi != SLA_PHI_ELU1) return false;                     // the ReLU map's backward runs on the generic kernels
   return encode_fn() != nullptr;
 }
@@ -909,6 +909,7 @@ bool backward_tc_supported(const Problem& p, int dt) {
 // Fused windows (<= kFuseMax rows) by sla_bwd_tc_kernel; longer windows by the three sla_bwd_tc_split_kernel passes
 // (they exit at once unless the first kernel raised the workspace flag).
 cudaError_t launch_backward_tc(const Problem& p, int dt, cudaStream_t st) {
+  if (p.d == 32) return launch_backward_tc32(p, dt, st);
   return (dt == SLA_F16) ? bwd_tc_launch<false, __half>(p, st) : bwd_tc_launch<true, __nv_bfloat16>(p, st);
 }
 

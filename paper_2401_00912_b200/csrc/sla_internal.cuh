@@ -87,6 +87,7 @@ cudaError_t launch_forward_generic(const Problem& p, int dt, cudaStream_t st);
 cudaError_t launch_backward_generic(const Problem& p, int dt, cudaStream_t st);
 bool backward_tc_supported(const Problem& p, int dt);
 cudaError_t launch_backward_tc(const Problem& p, int dt, cudaStream_t st);
+cudaError_t launch_backward_tc32(const Problem& p, int dt, cudaStream_t st);   // d_h = 32 (sla_bwd_tc32.cu)
 bool forward_tc_supported(const Problem& p, int dt);
 cudaError_t launch_forward_tc(const Problem& p, int dt, cudaStream_t st);
 // tcgen05 main pass of the forward (sla_fwd_umma.cu): fused windows + partial states of long windows
