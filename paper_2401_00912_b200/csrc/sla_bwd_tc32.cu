@@ -756,7 +756,7 @@ cudaError_t bwd_tc32_launch(const Problem& p, cudaStream_t st) {
   cudaError_t le = cudaLaunchKernelEx(&cfg, kern, tq, tk, tv, tg, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state,
                                       p.N, p.W, p.H, span);
   if (le != cudaSuccess || p.bounded) return le;   // bounded entry: no window is left to the split passes
-  const int span2 = 128;                           // <= kFuseMax; few pieces per window = few atomics per slot
+  const int span2 = kFuseMax / 16 * 16;            // the largest span the split passes handle: 33 x 32 atomics per piece and head
   cfg.gridDim = dim3((p.N + span2 - 1) / span2, slabs);
   le = cudaLaunchKernelEx(&cfg, k0, tk, tv, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state, p.ws_dstate, p.N, p.W,
                           p.H, span2);
