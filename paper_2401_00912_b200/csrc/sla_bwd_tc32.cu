@@ -740,7 +740,10 @@ cudaError_t bwd_tc32_launch(const Problem& p, cudaStream_t st) {
     if (e != cudaSuccess) return e;
     attr_set[dev].store(true, std::memory_order_release);
   }
-  const int span = 64;
+#ifndef SLA_BWD32_SPAN
+#define SLA_BWD32_SPAN 64
+#endif
+  const int span = SLA_BWD32_SPAN;
   const int slabs = (p.H + NW - 1) / NW;
   // one chain of programmatic dependent launches: zeroing kernel -> main -> the three split passes
   cudaLaunchAttribute pdl[1];
