@@ -35,10 +35,10 @@ def project_qkv(x, w, bias=None):
     return y[:, :C].copy(), y[:, C:2 * C].copy(), y[:, 2 * C:].copy()
 
 
-def error_bound(x, w, unit_roundoff: float, bias=None):
-    """Elementwise bound on |fl(y) - y| for a product accumulated in fp32 in any order and rounded once to a format of
-    unit roundoff `unit_roundoff`: K * 2^-24 * sum_k |x_k w_k| (accumulation, Higham 3.5 to first order, the bias term
-    included in the sum) + unit_roundoff * |y| (final rounding) + one subnormal spacing of fp16/bf16 storage."""
+def accumulation_bound(x, w, bias=None):
+    """(bound, mag): mag = sum_k |x_k w_k| (+ |bias|), and bound = (K + 1) * 2^-24 * mag, which covers the error of
+    accumulating the K products (and the bias) in fp32 in any order (Higham, Accuracy and Stability, 3.5, to first
+    order in 2^-24).  The parity test adds the final rounding to the storage format on top of it."""
     x = np.abs(np.asarray(x, dtype=np.float64))
     w = np.abs(np.asarray(w, dtype=np.float64))
     K = x.shape[1]

@@ -76,8 +76,9 @@ def test_linearity_and_bound():
     y1 = np.concatenate(P.project_qkv(x1, w), axis=1)
     y2 = np.concatenate(P.project_qkv(x2, w), axis=1)
     assert np.allclose(y12, a * y1 + b * y2, rtol=1e-12, atol=1e-12)
-    # the accumulation bound covers an fp32 evaluation of the same product
-    acc, mag = P.error_bound(x1, w, 2.0 ** -11)
-    y32 = (x1.astype(np.float32) @ w.T.astype(np.float32)).astype(np.float64)
-    yex = (x1.astype(np.float32).astype(np.float64)) @ (w.T.astype(np.float32).astype(np.float64))
-    assert np.all(np.abs(y32 - yex) <= acc + 1e-30) and np.all(mag >= np.abs(yex) - 1e-12)
+    # the accumulation bound covers an fp32 evaluation of the same product (inputs exactly representable in fp32)
+    xf, wf = x1.astype(np.float32), w.astype(np.float32)
+    acc, mag = P.accumulation_bound(xf, wf)
+    y32 = (xf @ wf.T).astype(np.float64)
+    yex = xf.astype(np.float64) @ wf.T.astype(np.float64)
+    assert np.all(np.abs(y32 - yex) <= acc) and np.all(mag >= np.abs(yex) * (1 - 1e-12))
