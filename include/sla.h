@@ -220,6 +220,30 @@ int sla_sequence_from_coords(const int32_t* coords, int64_t N, int32_t batch, in
                              int32_t S_h, int32_t S_w, int32_t* perm, int32_t* key_sorted, int32_t* window_offsets,
                              void* workspace, size_t workspace_bytes, sla_stream_t stream);
 
+/* ---- The shared Q/K/V projection around the op ------------------------------------------------
+ * "Self-attention first linearly projects the input to queries, keys, and values ... Q = x W_Q, K = x W_K, V = x W_V"
+ * (PAPER.md:71); "we use a shared projection layer to map all the voxels in the scene to query, key, and value
+ * representations".  One GEMM y[N, 3C] = x[N, C] . w_qkv[3C, C]^T (+ bias) on the tensor cores
+ * (tcgen05.mma, fp32 accumulation, one rounding to `dt`), written to three tensors (reading A17):
+ *   x      DEV [N, C] of dt, C = H * d_h (read-only)
+ *   w_qkv  DEV [3C, C] of dt: row j holds the weights of output feature j (the layout of a linear layer's weight);
+ *          rows 0..C-1 give Q (W_Q of the paper is their transpose), C..2C-1 give K, 2C..3C-1 give V (read-only)
+ *   bias   DEV fp32 [3C], 16-byte aligned, added before the rounding; NULL = none (the paper's formula has none)
+ *   q,k,v  DEV [N, C] of dt out; as [N, H, d_h] they are what sla_forward takes
+ * Supported: dt = SLA_F16 / SLA_BF16 and C in {128, 256}; anything else -> SLA_ERR_UNSUPPORTED.  All base pointers
+ * 16-byte aligned.  Enqueues one kernel on `stream`; no workspace. */
+int sla_qkv_projection(const void* x, const void* w_qkv, const float* bias, int64_t N, int32_t C, int dt,
+                       void* q, void* k, void* v, sla_stream_t stream);
+
+/* The module of PAPER.md:77: projection, then SLA(Q, K, V) (Eq. 2-3): sla_qkv_projection followed by sla_forward on
+ * the same stream (one chain of programmatic dependent launches; q, k, v stay in L2 between the two when 3 N C
+ * elements fit there).  q, k, v are caller-owned outputs as well (a training step needs them for sla_backward);
+ * workspace as for sla_forward.  Errors: those of the two calls. */
+int sla_module_forward(const void* x, const void* w_qkv, const float* bias, const int32_t* window_offsets,
+                       int64_t N, int32_t W, int32_t H, int32_t d_h, int dt,
+                       void* q, void* k, void* v, void* out,
+                       void* workspace, size_t workspace_bytes, sla_stream_t stream);
+
 /* Measurement aid, not a step of the SLA path ("a size-matched pure read+write kernel
  * run beside config 1 as the practical ceiling").  Streams three tensors in and one out with 128-bit
  * accesses -- the forward's 3:1 read:write mix -- and nothing else: out = a ^ b ^ c, bytewise.

@@ -24,6 +24,7 @@ SYMBOLS = (
     "sla_bench_stream_ceiling",
     "sla_window_count", "sla_window_keys", "sla_sort_workspace_bytes", "sla_sort_by_window", "sla_gather_rows",
     "sla_scatter_rows", "sla_sequence_workspace_bytes", "sla_sequence_from_coords",
+    "sla_qkv_projection", "sla_module_forward",
 )
 
 _lib = None
@@ -88,6 +89,10 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     L.sla_sequence_workspace_bytes.restype = sz
     L.sla_sequence_from_coords.argtypes = [vp, i64, i32, i32, i32, i32, i32, vp, vp, vp, vp, sz, vp]
     L.sla_sequence_from_coords.restype = ci
+    L.sla_qkv_projection.argtypes = [vp, vp, vp, i64, i32, ci, vp, vp, vp, vp]
+    L.sla_qkv_projection.restype = ci
+    L.sla_module_forward.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp, vp, vp, vp, sz, vp]
+    L.sla_module_forward.restype = ci
     if path is None:
         _lib = L
     return L
@@ -362,3 +367,54 @@ def sla_forward_static(q, k, v, window_offsets, out=None, stream=None):
                                 window_offsets.numel() - 1, H, d, _dt(q), out.data_ptr(), _stream(stream)),
            "sla_forward_static")
     return out
+
+
+# ---- shared Q/K/V projection and the module (include/sla.h) ----
+
+def _chk_proj(x, w, bias):
+    import torch
+    _chk_dev(x, w)
+    if x.dim() != 2 or w.dim() != 2 or w.shape != (3 * x.shape[1], x.shape[1]) or w.dtype != x.dtype:
+        raise SlaError("x must be [N, C] and w_qkv [3C, C] of the same dtype")
+    if bias is not None:
+        _chk_dev(bias)
+        if bias.dtype != torch.float32 or bias.numel() != 3 * x.shape[1]:
+            raise SlaError("bias must be fp32 [3C]")
+
+
+def sla_qkv_projection(x, w_qkv, bias=None, q=None, k=None, v=None, stream=None):
+    """x: CUDA [N, C] fp16/bf16, w_qkv: [3C, C] (row j = weights of output feature j; Q, K, V blocks) -> (q, k, v),
+    each [N, C]: y = x w^T (+ bias) on tcgen05."""
+    import torch
+    L = load_library()
+    _chk_proj(x, w_qkv, bias)
+    N, C = x.shape
+    q, k, v = (torch.empty_like(x) if t is None else t for t in (q, k, v))
+    _check(L.sla_qkv_projection(x.data_ptr(), w_qkv.data_ptr(), bias.data_ptr() if bias is not None else None, N, C,
+                                _dt(x), q.data_ptr(), k.data_ptr(), v.data_ptr(), _stream(stream)),
+           "sla_qkv_projection")
+    return q, k, v
+
+
+def sla_module_forward(x, w_qkv, window_offsets, H: int, bias=None, q=None, k=None, v=None, out=None, workspace=None,
+                       stream=None):
+    """Projection, then SLA on its results, in one C call -> (out [N, H, d_h], q, k, v)."""
+    import torch
+    L = load_library()
+    _chk_proj(x, w_qkv, bias)
+    _chk_dev(window_offsets)
+    if window_offsets.dtype != torch.int32:
+        raise SlaError("window_offsets must be int32")
+    N, C = x.shape
+    if C % H:
+        raise SlaError("C must be H * d_h")
+    d = C // H
+    W = window_offsets.numel() - 1
+    dt = _dt(x)
+    q, k, v = (torch.empty(N, H, d, dtype=x.dtype, device=x.device) if t is None else t for t in (q, k, v))
+    out = torch.empty(N, H, d, dtype=x.dtype, device=x.device) if out is None else out
+    workspace, wsb = _workspace(x, N, W, H, d, dt, False, workspace)
+    _check(L.sla_module_forward(x.data_ptr(), w_qkv.data_ptr(), bias.data_ptr() if bias is not None else None,
+                                window_offsets.data_ptr(), N, W, H, d, dt, q.data_ptr(), k.data_ptr(), v.data_ptr(),
+                                out.data_ptr(), workspace.data_ptr(), wsb, _stream(stream)), "sla_module_forward")
+    return out, q, k, v

@@ -164,6 +164,19 @@ size_t sla_sequence_workspace_bytes(int64_t N) {
   return ((size_t)N * 4 + 15) / 16 * 16 + sla::sort_workspace_bytes(N);
 }
 
+// ---- shared Q/K/V projection ----
+int sla_qkv_projection(const void* x, const void* w_qkv, const float* bias, int64_t N, int32_t C, int dt, void* q,
+                       void* k, void* v, sla_stream_t stream) {
+  if (N < 0 || N >= (int64_t(1) << 31) || C < 1) return SLA_ERR_INVALID_ARG;
+  if (!sla::qkv_projection_supported(C, dt)) return SLA_ERR_UNSUPPORTED;
+  if (N == 0) return SLA_OK;
+  if (!x || !w_qkv || !q || !k || !v) return SLA_ERR_INVALID_ARG;
+  if (!aligned16(x) || !aligned16(w_qkv) || !aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(bias))
+    return SLA_ERR_UNSUPPORTED;
+  cudaError_t e = sla::launch_qkv_projection(x, w_qkv, bias, (int)N, C, dt, q, k, v, (cudaStream_t)stream);
+  return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
+}
+
 int sla_bench_stream_ceiling(const void* a, const void* b, const void* c, void* out, size_t bytes,
                              sla_stream_t stream) {
   if (!a || !b || !c || !out) return SLA_ERR_INVALID_ARG;
@@ -200,6 +213,19 @@ int sla_forward(const void* q, const void* k, const void* v, const int32_t* wind
                 int32_t W, int32_t H, int32_t d_h, int dt, void* out, void* workspace,
                 size_t workspace_bytes, sla_stream_t stream) {
   return forward_impl(false, SLA_PHI_ELU1, 0.f, q, k, v, window_offsets, N, W, H, d_h, dt, out, workspace, workspace_bytes, stream);
+}
+
+int sla_module_forward(const void* x, const void* w_qkv, const float* bias, const int32_t* window_offsets, int64_t N,
+                       int32_t W, int32_t H, int32_t d_h, int dt, void* q, void* k, void* v, void* out,
+                       void* workspace, size_t workspace_bytes, sla_stream_t stream) {
+  int rc = check_common(N, W, H, d_h, dt);
+  if (rc != SLA_OK) return rc;
+  // projection, then the op on its results: the kernels follow each other on `stream` as one chain of programmatic
+  // dependent launches, and q, k, v (3 N C elements) are still in L2 when the op reads them if they fit there
+  rc = sla_qkv_projection(x, w_qkv, bias, N, H * d_h, dt, q, k, v, stream);
+  if (rc != SLA_OK) return rc;
+  return forward_impl(false, SLA_PHI_ELU1, 0.f, q, k, v, window_offsets, N, W, H, d_h, dt, out, workspace,
+                      workspace_bytes, stream);
 }
 
 // feature map / epsilon arguments of the *_phi entries

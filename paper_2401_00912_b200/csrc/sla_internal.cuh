@@ -102,6 +102,10 @@ cudaError_t launch_sort_by_key(const int32_t* key, int N, int W, int32_t* perm, 
                                cudaStream_t st);
 cudaError_t launch_permute_rows(const void* src, const int32_t* perm, long long N, size_t row_bytes, void* dst,
                                 bool scatter, cudaStream_t st);
+// shared Q/K/V projection (sla_proj.cu): y = x w^T (+ bias) on tcgen05, split into q, k, v
+bool qkv_projection_supported(int C, int dt);
+cudaError_t launch_qkv_projection(const void* x, const void* w, const float* bias, int N, int C, int dt, void* q,
+                                  void* k, void* v, cudaStream_t st);
 cudaError_t launch_stream_ceiling(const void* a, const void* b, const void* c, void* out, size_t bytes,
                                   cudaStream_t st);
 
