@@ -125,7 +125,11 @@ sla_qkv_proj_kernel(const __grid_constant__ Maps maps, const float* __restrict__
   asm volatile("griddepcontrol.launch_dependents;");
   const uint32_t sbase = (smem_u32(dyn_smem) + 1023u) & ~1023u;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int ntiles = (N + TILE_M - 1) / TILE_M;
+  // Work unit = (128-row tile, 128-feature chunk).  Every CTA takes one contiguous range of units, so the ranges differ
+  // by at most one chunk (a third of a tile at C = 128) where whole tiles would differ by one tile in ~3; a tile that
+  // straddles two ranges is loaded by both CTAs (the second time out of L2).
+  const long long units = (long long)((N + TILE_M - 1) / TILE_M) * G::NCH;
+  const int u0 = (int)(units * blockIdx.x / gridDim.x), u1 = (int)(units * (blockIdx.x + 1) / gridDim.x);
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < 2; ++i) {
@@ -154,51 +158,53 @@ sla_qkv_proj_kernel(const __grid_constant__ Maps maps, const float* __restrict__
   if (warp == WARP_PRODUCER) {
     if (lane == 0) {
       Cur a{0, 0}, w{0, 0};
-      for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        mbar_wait_wd(smem_u32(&ctrl.a_empty[a.s]), a.ph ^ 1u);     // passes at once on a stage never used
-        const uint32_t abar = smem_u32(&ctrl.a_full[a.s]);
-        mbar_expect_tx(abar, (uint32_t)G::OPERAND_BYTES);
-#pragma unroll
-        for (int b = 0; b < G::KB; ++b)
-          tma_load_2d(sbase + G::OFF_A + a.s * G::OPERAND_BYTES + b * BOX_BYTES, &maps.x, abar, 64 * b, tile * TILE_M);
-        advance<G::NA>(a);
-        for (int j = 0; j < G::NCH; ++j) {
-          mbar_wait_wd(smem_u32(&ctrl.w_empty[w.s]), w.ph ^ 1u);
-          const uint32_t wbar = smem_u32(&ctrl.w_full[w.s]);
-          mbar_expect_tx(wbar, (uint32_t)G::OPERAND_BYTES);
+      for (int u = u0; u < u1; ++u) {
+        const int tile = u / G::NCH, j = u % G::NCH;
+        if (j == 0 || u == u0) {                                     // first unit of a tile in this range: its x rows
+          mbar_wait_wd(smem_u32(&ctrl.a_empty[a.s]), a.ph ^ 1u);     // passes at once on a stage never used
+          const uint32_t abar = smem_u32(&ctrl.a_full[a.s]);
+          mbar_expect_tx(abar, (uint32_t)G::OPERAND_BYTES);
 #pragma unroll
           for (int b = 0; b < G::KB; ++b)
-            tma_load_2d(sbase + G::OFF_W + w.s * G::OPERAND_BYTES + b * BOX_BYTES, &maps.w, wbar, 64 * b, CHUNK_N * j);
-          advance<G::NWS>(w);
+            tma_load_2d(sbase + G::OFF_A + a.s * G::OPERAND_BYTES + b * BOX_BYTES, &maps.x, abar, 64 * b, tile * TILE_M);
+          advance<G::NA>(a);
         }
+        mbar_wait_wd(smem_u32(&ctrl.w_empty[w.s]), w.ph ^ 1u);
+        const uint32_t wbar = smem_u32(&ctrl.w_full[w.s]);
+        mbar_expect_tx(wbar, (uint32_t)G::OPERAND_BYTES);
+#pragma unroll
+        for (int b = 0; b < G::KB; ++b)
+          tma_load_2d(sbase + G::OFF_W + w.s * G::OPERAND_BYTES + b * BOX_BYTES, &maps.w, wbar, 64 * b, CHUNK_N * j);
+        advance<G::NWS>(w);
       }
     }
   } else if (warp == WARP_MMA) {
     if (lane == 0) {
       constexpr uint32_t IDESC = make_idesc(TILE_M, CHUNK_N, BF16);
       Cur a{0, 0}, w{0, 0}, acc{0, 0};
-      for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        mbar_wait_wd(smem_u32(&ctrl.a_full[a.s]), a.ph);
+      for (int u = u0; u < u1; ++u) {
+        const int j = u % G::NCH;
+        if (j == 0 || u == u0) mbar_wait_wd(smem_u32(&ctrl.a_full[a.s]), a.ph);
         const uint32_t abase = sbase + G::OFF_A + a.s * G::OPERAND_BYTES;
-        for (int j = 0; j < G::NCH; ++j) {
-          mbar_wait_wd(smem_u32(&ctrl.w_full[w.s]), w.ph);
-          mbar_wait_wd(smem_u32(&ctrl.acc_empty[acc.s]), acc.ph ^ 1u);
-          tc_fence_after();
-          const uint32_t wbase = sbase + G::OFF_W + w.s * G::OPERAND_BYTES;
+        mbar_wait_wd(smem_u32(&ctrl.w_full[w.s]), w.ph);
+        mbar_wait_wd(smem_u32(&ctrl.acc_empty[acc.s]), acc.ph ^ 1u);
+        tc_fence_after();
+        const uint32_t wbase = sbase + G::OFF_W + w.s * G::OPERAND_BYTES;
 #pragma unroll
-          for (int ks = 0; ks < G::KSTEPS; ++ks) {
-            // k-step ks = 16 columns = 32 bytes inside the 128-byte row of box ks/4
-            const uint32_t koff = (uint32_t)((ks >> 2) * BOX_BYTES + (ks & 3) * 32);
-            umma(tmem + (uint32_t)(acc.s * CHUNK_N), make_desc(abase + koff), make_desc(wbase + koff), IDESC,
-                 ks > 0 ? 1u : 0u);
-          }
-          umma_commit(smem_u32(&ctrl.w_empty[w.s]));       // the w stage may be overwritten once these MMAs have read it
-          umma_commit(smem_u32(&ctrl.acc_full[acc.s]));
-          advance<G::NWS>(w);
-          advance<2>(acc);
+        for (int ks = 0; ks < G::KSTEPS; ++ks) {
+          // k-step ks = 16 columns = 32 bytes inside the 128-byte row of box ks/4
+          const uint32_t koff = (uint32_t)((ks >> 2) * BOX_BYTES + (ks & 3) * 32);
+          umma(tmem + (uint32_t)(acc.s * CHUNK_N), make_desc(abase + koff), make_desc(wbase + koff), IDESC,
+               ks > 0 ? 1u : 0u);
         }
-        umma_commit(smem_u32(&ctrl.a_empty[a.s]));
-        advance<G::NA>(a);
+        umma_commit(smem_u32(&ctrl.w_empty[w.s]));       // the w stage may be overwritten once these MMAs have read it
+        umma_commit(smem_u32(&ctrl.acc_full[acc.s]));
+        advance<G::NWS>(w);
+        advance<2>(acc);
+        if (j == G::NCH - 1 || u == u1 - 1) {             // last unit of the tile in this range: hand the x stage back
+          umma_commit(smem_u32(&ctrl.a_empty[a.s]));
+          advance<G::NA>(a);
+        }
       }
     }
   } else {
@@ -208,8 +214,9 @@ sla_qkv_proj_kernel(const __grid_constant__ Maps maps, const float* __restrict__
     const int et = threadIdx.x - WARP_EPI0 * 32;            // 0..127
     Cur acc{0, 0};
     int os = 0;                                              // staging buffer of the next chunk
-    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-      for (int j = 0; j < G::NCH; ++j) {
+    {
+      for (int u = u0; u < u1; ++u) {
+        const int tile = u / G::NCH, j = u % G::NCH;
         // the staging buffer must have been read by the bulk store of the chunk that used it last
         if (et == 0) bulk_wait_read<G::NOS - 1>();
         asm volatile("bar.sync 1, 128;" ::: "memory");
