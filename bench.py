@@ -345,6 +345,68 @@ def sequence_prep_leg(pkg, torch, dev, peak):
             "timing": "median of 40 eager calls, one event pair per call (includes the binding's launch path), cold L2"}
 
 
+def projection_leg(pkg, torch, dev, peak):
+    """The shared Q/K/V projection at the shape of config 1 (N = 60 000, C = 128, fp16) and the module
+    (projection + sla_forward in one C call).  Projection: eager calls back to back on rotating cold sets, CUDA events
+    around the region; HBM-bound, algorithmic bytes = x + w + q,k,v.  Module: one event pair per call, cold L2 (a 256 MB
+    buffer is overwritten before every call), against the two calls timed the same way on cold inputs."""
+    from paper_2401_00912_b200 import workloads as wl
+    sc = wl.make_config(1)
+    N, H, d = sc.N, sc.H, sc.d_h
+    C = H * d
+    n_sets = 6                                            # 6 x 61 MB > 2 x L2
+    xs = [torch.randn(N, C, device=dev, dtype=torch.float16) for _ in range(n_sets)]
+    w = (torch.randn(3 * C, C, device=dev) / C ** 0.5).to(torch.float16)
+    outs = [[torch.empty(N, H, d, device=dev, dtype=torch.float16) for _ in range(3)] for _ in range(n_sets)]
+
+    def proj(i):
+        q, k, v = outs[i % n_sets]
+        pkg.sla_qkv_projection(xs[i % n_sets], w, q=q.view(N, C), k=k.view(N, C), v=v.view(N, C))
+
+    for i in range(5):
+        proj(i)
+    torch.cuda.synchronize()
+    K = 60
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for i in range(K):
+        proj(i)
+    b.record()
+    torch.cuda.synchronize()
+    us = a.elapsed_time(b) / K * 1e3
+    nb = 4 * N * C * 2 + 3 * C * C * 2
+    off = torch.from_numpy(sc.offsets).to(dev)
+    o = torch.empty(N, H, d, device=dev, dtype=torch.float16)
+    ws = torch.empty(pkg.workspace_bytes(N, sc.W, H, d, 1), dtype=torch.uint8, device=dev)
+    flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=dev)
+    q, k, v = outs[0]
+
+    def cold(fn, reps=30):
+        ts = []
+        for i in range(reps + 5):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fn()
+            b.record()
+            torch.cuda.synchronize()
+            if i >= 5:
+                ts.append(a.elapsed_time(b) * 1e3)
+        return sorted(ts)[len(ts) // 2]
+
+    mod = cold(lambda: pkg.sla_module_forward(xs[0], w, off, H, q=q, k=k, v=v, out=o, workspace=ws))
+    sep_p = cold(lambda: pkg.sla_qkv_projection(xs[0], w, q=q.view(N, C), k=k.view(N, C), v=v.view(N, C)))
+    sep_f = cold(lambda: pkg.sla_forward(q, k, v, off, out=o, workspace=ws))
+    return {"N": N, "C": C, "dtype": "f16", "kernel": "sla_qkv_proj_kernel (tcgen05.mma, TMEM accumulators, TMA in and out)",
+            "us": us, "algorithmic_bytes": nb, "frac_of_peak": nb / (us * 1e-6) / 1e9 / peak, "bound": "hbm",
+            "tflops": 2.0 * N * C * 3 * C / (us * 1e-6) / 1e12,
+            "module_us_cold_single_call": mod, "projection_us_cold_single_call": sep_p,
+            "sla_forward_us_cold_single_call": sep_f,
+            "module_algorithmic_bytes_x_in_out_out": 2 * N * C * 2 + 3 * C * C * 2 + 4 * (sc.W + 1),
+            "timing": "us: CUDA events around 60 back-to-back calls on 6 rotating sets (cold L2); *_single_call: median "
+                      "of 30, one event pair per call, L2 flushed before each"}
+
+
 def ncu_traffic():
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the forward kernel on config 1, as recorded
     in the committed ncu summary of this round (a line `dram_bytes_per_launch: <int>`); None if absent."""
@@ -645,6 +707,7 @@ def run_ours(args):
             line.update(extra_legs(pkg, torch, dev, peak))
             line["other_configs"] = other_config_legs(pkg, torch, dev, peak)
             line["sequence_prep"] = sequence_prep_leg(pkg, torch, dev, peak)
+            line["qkv_projection"] = projection_leg(pkg, torch, dev, peak)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         secs, cores = cpu_oracle_time(sc)
         line["cpu_baseline"] = {"value": N / secs, "unit": UNIT, "cores": cores, "kind": "oracle",
