@@ -244,6 +244,32 @@ int sla_module_forward(const void* x, const void* w_qkv, const float* bias, cons
                        void* q, void* k, void* v, void* out,
                        void* workspace, size_t workspace_bytes, sla_stream_t stream);
 
+/* ---- Cross-Window Interaction (Eq. 4-7) --------------------------------------
+ * "the input features are divided along the channel dimension and processed through multiple branches using
+ * group-wise convolutions ... a (S_h+1) x 1 x 1 convolution in one branch and a 1 x (S_w+1) x 1 convolution in another
+ * ... a standard 3 x 3 x 3 convolution in one branch ... while another branch performs an identity mapping":
+ *   X' = Concat(DWConv_{S_h+1 along y}(X[:, 0:c]), DWConv_{S_w+1 along x}(X[:, c:2c]), DWConv_{3x3x3}(X[:, 2c:3c]), X[:, 3c:4c])
+ * with C = 4c and depth-wise (per-channel) kernels.  DESIGN.md reading A18 fixes what the paper leaves open:
+ *   - voxels are sparse: coords is int32[N,4], rows (b, z, y, x), all DISTINCT and inside
+ *     [0,batch) x [0,grid_z) x [0,grid_h) x [0,grid_w); outputs live on the same voxels (row i of out <-> row i of x);
+ *     a tap that lands on a cell without a voxel, outside the grid or in another sample contributes nothing.
+ *     A voxel outside the grid is seen by nobody and gets zeros in the three convolution branches; duplicated
+ *     coordinates give an unspecified one of the duplicates to their neighbours.  Nothing is read or written out of
+ *     bounds either way.
+ *   - S_h, S_w even (the window size): kernels of S+1 taps, centred, offsets -S/2..+S/2; 3x3x3 tap index
+ *     (dz+1)*9 + (dy+1)*3 + (dx+1); cross-correlation: out[i] = sum_t w[t] * x[voxel at coords[i] + offset(t)].
+ *   x, out   DEV [N, C] of dt (fp32 / fp16 / bf16), distinct buffers        coords  DEV int32[N,4], 16-byte aligned
+ *   w_h      DEV fp32 [c, S_h+1]     w_w  DEV fp32 [c, S_w+1]     w_3  DEV fp32 [c, 27]     (no bias)
+ *   workspace DEV, >= sla_cwi_workspace_bytes(batch, grid_z, grid_h, grid_w) = 4 bytes per grid cell (the dense
+ *            voxel-index grid, rebuilt by every call), 16-byte aligned, scratch
+ * fp32 accumulation in tap order (deterministic), one rounding to dt.  C % 4 == 0, C <= 512, S_h + S_w <= 99, fewer
+ * than 2^31 grid cells; otherwise SLA_ERR_UNSUPPORTED / SLA_ERR_INVALID_ARG.  Enqueues three kernels on `stream`. */
+size_t sla_cwi_workspace_bytes(int32_t batch, int32_t grid_z, int32_t grid_h, int32_t grid_w);
+int sla_cwi_forward(const void* x, const int32_t* coords, int64_t N, int32_t C, int dt,
+                    int32_t batch, int32_t grid_z, int32_t grid_h, int32_t grid_w, int32_t S_h, int32_t S_w,
+                    const float* w_h, const float* w_w, const float* w_3, void* out,
+                    void* workspace, size_t workspace_bytes, sla_stream_t stream);
+
 /* Measurement aid, not a step of the SLA path ("a size-matched pure read+write kernel
  * run beside config 1 as the practical ceiling").  Streams three tensors in and one out with 128-bit
  * accesses -- the forward's 3:1 read:write mix -- and nothing else: out = a ^ b ^ c, bytewise.

@@ -24,7 +24,7 @@ SYMBOLS = (
     "sla_bench_stream_ceiling",
     "sla_window_count", "sla_window_keys", "sla_sort_workspace_bytes", "sla_sort_by_window", "sla_gather_rows",
     "sla_scatter_rows", "sla_sequence_workspace_bytes", "sla_sequence_from_coords",
-    "sla_qkv_projection", "sla_module_forward",
+    "sla_qkv_projection", "sla_module_forward", "sla_cwi_workspace_bytes", "sla_cwi_forward",
 )
 
 _lib = None
@@ -93,6 +93,10 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     L.sla_qkv_projection.restype = ci
     L.sla_module_forward.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp, vp, vp, vp, sz, vp]
     L.sla_module_forward.restype = ci
+    L.sla_cwi_workspace_bytes.argtypes = [i32, i32, i32, i32]
+    L.sla_cwi_workspace_bytes.restype = sz
+    L.sla_cwi_forward.argtypes = [vp, vp, i64, i32, ci, i32, i32, i32, i32, i32, i32, vp, vp, vp, vp, vp, sz, vp]
+    L.sla_cwi_forward.restype = ci
     if path is None:
         _lib = L
     return L
@@ -418,3 +422,34 @@ def sla_module_forward(x, w_qkv, window_offsets, H: int, bias=None, q=None, k=No
                                 window_offsets.data_ptr(), N, W, H, d, dt, q.data_ptr(), k.data_ptr(), v.data_ptr(),
                                 out.data_ptr(), workspace.data_ptr(), wsb, _stream(stream)), "sla_module_forward")
     return out, q, k, v
+
+
+# ---- Cross-Window Interaction (include/sla.h) ----
+
+def sla_cwi_forward(x, coords, grid, S_h: int, S_w: int, w_h, w_w, w_3, out=None, workspace=None, stream=None):
+    """x: CUDA [N, 4c]; coords: CUDA int32 [N,4] rows (b, z, y, x); grid = (batch, grid_z, grid_h, grid_w);
+    w_h [c, S_h+1], w_w [c, S_w+1], w_3 [c, 27] fp32 -> out [N, 4c] (Eq. 4-7)."""
+    import torch
+    L = load_library()
+    _chk_dev(x, w_h, w_w, w_3)
+    _chk_i32(coords, "coords")
+    if x.dim() != 2 or coords.shape != (x.shape[0], 4):
+        raise SlaError("x must be [N, C] and coords [N, 4]")
+    N, C = x.shape
+    c = C // 4
+    for w, taps in ((w_h, S_h + 1), (w_w, S_w + 1), (w_3, 27)):
+        if w.dtype != torch.float32 or tuple(w.shape) != (c, taps):
+            raise SlaError("weights must be fp32 [c, taps]")
+    batch, gz, gh, gw = (int(v) for v in grid)
+    need = int(L.sla_cwi_workspace_bytes(batch, gz, gh, gw))
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=x.device)
+    if out is None:
+        out = torch.empty_like(x)
+    dt = {torch.float32: SLA_F32, torch.float16: SLA_F16, torch.bfloat16: SLA_BF16}.get(x.dtype)
+    if dt is None:
+        raise SlaError(f"unsupported dtype {x.dtype}")
+    _check(L.sla_cwi_forward(x.data_ptr(), coords.data_ptr(), N, C, dt, batch, gz, gh, gw, S_h, S_w, w_h.data_ptr(),
+                             w_w.data_ptr(), w_3.data_ptr(), out.data_ptr(), workspace.data_ptr(), workspace.numel(),
+                             _stream(stream)), "sla_cwi_forward")
+    return out

@@ -13,7 +13,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libsla_b200.so")
-SOURCES = ["sla_api.cu", "sla_prep.cu", "sla_generic.cu", "sla_fwd_tc.cu", "sla_fwd_umma.cu", "sla_seq.cu", "sla_bwd_tc.cu", "sla_bwd_tc32.cu", "sla_proj.cu"]
+SOURCES = ["sla_api.cu", "sla_prep.cu", "sla_generic.cu", "sla_fwd_tc.cu", "sla_fwd_umma.cu", "sla_seq.cu", "sla_bwd_tc.cu", "sla_bwd_tc32.cu", "sla_proj.cu", "sla_cwi.cu"]
 HEADERS = ["sla_internal.cuh", "sla_tc_common.cuh", "sla_tc_base.cuh", os.path.join("..", "..", "include", "sla.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -177,6 +177,37 @@ int sla_qkv_projection(const void* x, const void* w_qkv, const float* bias, int6
   return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
 }
 
+// ---- Cross-Window Interaction ----
+static int64_t cwi_cells(int32_t batch, int32_t gz, int32_t gh, int32_t gw) {
+  if (batch < 1 || gz < 1 || gh < 1 || gw < 1) return -1;
+  const int64_t a = (int64_t)batch * gz, b = (int64_t)gh * gw;
+  if (a > (int64_t(1) << 31) / b) return -1;
+  return a * b < (int64_t(1) << 31) ? a * b : -1;
+}
+
+size_t sla_cwi_workspace_bytes(int32_t batch, int32_t grid_z, int32_t grid_h, int32_t grid_w) {
+  const int64_t cells = cwi_cells(batch, grid_z, grid_h, grid_w);
+  return cells < 0 ? 0 : ((size_t)cells * 4 + 15) / 16 * 16;
+}
+
+int sla_cwi_forward(const void* x, const int32_t* coords, int64_t N, int32_t C, int dt, int32_t batch, int32_t grid_z,
+                    int32_t grid_h, int32_t grid_w, int32_t S_h, int32_t S_w, const float* w_h, const float* w_w,
+                    const float* w_3, void* out, void* workspace, size_t workspace_bytes, sla_stream_t stream) {
+  if (N < 0 || N >= (int64_t(1) << 31) || C < 4 || cwi_cells(batch, grid_z, grid_h, grid_w) < 0)
+    return SLA_ERR_INVALID_ARG;
+  if (S_h < 0 || S_w < 0 || (S_h & 1) || (S_w & 1)) return SLA_ERR_INVALID_ARG;   // even windows: odd, centred kernels
+  if (dt != SLA_F32 && dt != SLA_F16 && dt != SLA_BF16) return SLA_ERR_UNSUPPORTED;
+  if (C % 4 != 0 || C > 512 || S_h + S_w + 29 > 128) return SLA_ERR_UNSUPPORTED;
+  if (N == 0) return SLA_OK;
+  if (!x || !coords || !w_h || !w_w || !w_3 || !out || x == out) return SLA_ERR_INVALID_ARG;
+  if (!aligned16(coords)) return SLA_ERR_UNSUPPORTED;
+  if (!workspace || workspace_bytes < sla_cwi_workspace_bytes(batch, grid_z, grid_h, grid_w) || !aligned16(workspace))
+    return SLA_ERR_WORKSPACE;
+  cudaError_t e = sla::launch_cwi(x, coords, (int)N, C, dt, batch, grid_z, grid_h, grid_w, S_h, S_w, w_h, w_w, w_3, out,
+                                  static_cast<int32_t*>(workspace), (cudaStream_t)stream);
+  return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
+}
+
 int sla_bench_stream_ceiling(const void* a, const void* b, const void* c, void* out, size_t bytes,
                              sla_stream_t stream) {
   if (!a || !b || !c || !out) return SLA_ERR_INVALID_ARG;
