@@ -407,6 +407,39 @@ def projection_leg(pkg, torch, dev, peak):
                       "of 30, one event pair per call, L2 flushed before each"}
 
 
+def cwi_leg(pkg, torch, dev, peak):
+    """Cross-Window Interaction on a config-1-sized scene: 60 000 voxels of a 468 x 468 x 32 grid,
+    C = 128 fp16, 12 x 12 windows (13-tap kernels).  Eager C-ABI calls back to back, CUDA events around the region;
+    the call rebuilds its 28 MB index grid every time, so nothing of it survives in L2 between calls by design."""
+    from paper_2401_00912_b200 import workloads as wl
+    N, C, grid = 60000, 128, (1, 32, 468, 468)
+    coords = torch.from_numpy(wl.coords_waymo_like(wl.SEED_BASE + 80, N=N, batch=1, nz=32)).to(dev)
+    x = torch.randn(N, C, device=dev, dtype=torch.float16)
+    out = torch.empty_like(x)
+    w = [torch.randn(C // 4, t, device=dev) / t ** 0.5 for t in (13, 13, 27)]
+    ws = torch.empty(int(pkg.load_library().sla_cwi_workspace_bytes(*grid)), dtype=torch.uint8, device=dev)
+
+    def call():
+        pkg.sla_cwi_forward(x, coords, grid, 12, 12, *w, out=out, workspace=ws)
+
+    for _ in range(5):
+        call()
+    torch.cuda.synchronize()
+    K = 40
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(K):
+        call()
+    b.record()
+    torch.cuda.synchronize()
+    us = a.elapsed_time(b) / K * 1e3
+    cells = grid[0] * grid[1] * grid[2] * grid[3]
+    nb = 2 * N * C * 2 + 16 * N + 4 * cells + 4 * N
+    return {"N": N, "C": C, "grid": list(grid), "window": [12, 12], "dtype": "f16", "us": us, "kernels_per_call": 3,
+            "algorithmic_bytes": nb, "frac_of_peak": nb / (us * 1e-6) / 1e9 / peak, "bound": "hbm",
+            "note": "algorithmic bytes = x in + out + coords + the index grid written once (4 B per cell) + its N entries"}
+
+
 def ncu_traffic():
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the forward kernel on config 1, as recorded
     in the committed ncu summary of this round (a line `dram_bytes_per_launch: <int>`); None if absent."""
@@ -708,6 +741,7 @@ def run_ours(args):
             line["other_configs"] = other_config_legs(pkg, torch, dev, peak)
             line["sequence_prep"] = sequence_prep_leg(pkg, torch, dev, peak)
             line["qkv_projection"] = projection_leg(pkg, torch, dev, peak)
+            line["cross_window_interaction"] = cwi_leg(pkg, torch, dev, peak)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         secs, cores = cpu_oracle_time(sc)
         line["cpu_baseline"] = {"value": N / secs, "unit": UNIT, "cores": cores, "kind": "oracle",

@@ -55,7 +55,7 @@ template <> __device__ __forceinline__ float to_elem<float>(float v) { return v;
 template <> __device__ __forceinline__ __half to_elem<__half>(float v) { return __float2half_rn(v); }
 template <> __device__ __forceinline__ __nv_bfloat16 to_elem<__nv_bfloat16>(float v) { return __float2bfloat16_rn(v); }
 
-constexpr int kCwiWarps = 8;
+constexpr int kCwiWarps = 16;
 constexpr int kMaxTapSlots = 4;    // taps per lane: S_h + S_w + 29 <= 128
 
 // CPL = channels of a branch per lane = ceil(c / 32)
@@ -80,64 +80,95 @@ sla_cwi_conv_kernel(const T* __restrict__ x, const int4* __restrict__ coords, in
   pdl_wait();
   __syncthreads();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const long long i = (long long)blockIdx.x * kCwiWarps + warp;
-  if (i >= N) return;
-  const int4 me = __ldg(coords + i);                     // (b, z, y, x)
-  // every lane looks up the taps it owns: tap t -> offset (dz, dy, dx)
-  int idx[kMaxTapSlots];
+  // the taps a lane owns (tap t = lane + 32 s) and their offsets do not depend on the voxel
+  int tdz[kMaxTapSlots], tdy[kMaxTapSlots], tdx[kMaxTapSlots], tdelta[kMaxTapSlots];
 #pragma unroll
   for (int s = 0; s < kMaxTapSlots; ++s) {
     const int t = lane + 32 * s;
-    idx[s] = -1;
-    if (t < Tall) {
-      int dz = 0, dy = 0, dx = 0;
-      if (t < Th) dy = t - (S_h >> 1);
-      else if (t < Th + Tw) dx = t - Th - (S_w >> 1);
-      else { const int u = t - Th - Tw; dz = u / 9 - 1; dy = (u / 3) % 3 - 1; dx = u % 3 - 1; }
-      const long long cell = cell_of(g, me.x, me.y + dz, me.z + dy, me.w + dx);
-      if (cell >= 0) idx[s] = grid[cell];
-    }
+    int dz = 0, dy = 0, dx = 0;
+    if (t < Th) dy = t - (S_h >> 1);
+    else if (t < Th + Tw) dx = t - Th - (S_w >> 1);
+    else if (t < Tall) { const int u = t - Th - Tw; dz = u / 9 - 1; dy = (u / 3) % 3 - 1; dx = u % 3 - 1; }
+    else dz = 1 << 20;                                     // no such tap: always outside the grid
+    tdz[s] = dz; tdy[s] = dy; tdx[s] = dx;
+    tdelta[s] = (dz * g.gh + dy) * g.gw + dx;              // |.| < 2^31 cells
   }
-  float acc[3][CPL];
-#pragma unroll
-  for (int br = 0; br < 3; ++br)
-#pragma unroll
-    for (int k = 0; k < CPL; ++k) acc[br][k] = 0.f;
+  // bit masks of the taps of each branch inside each 32-tap slot
+  unsigned bmask[3][kMaxTapSlots];
 #pragma unroll
   for (int s = 0; s < kMaxTapSlots; ++s) {
-    if (32 * s >= Tall) break;
-    unsigned present = __ballot_sync(0xffffffffu, idx[s] >= 0);        // taps of this slot that hit a voxel
-    while (present) {                                                  // ascending tap order: deterministic sums
-      const int l = __ffs(present) - 1;
-      present &= present - 1;
-      const int t = l + 32 * s;
-      const int j = __shfl_sync(0xffffffffu, idx[s], l);
-      const int br = (t < Th) ? 0 : (t < Th + Tw ? 1 : 2);
-      const T* row = x + (size_t)j * C + br * c;
-      const float* wt = s_w + t * c;
+    const int lo = 32 * s;
+    auto range_mask = [&](int a, int b) -> unsigned {      // taps [a, b) intersected with [lo, lo + 32)
+      const int x0 = max(a, lo) - lo, x1 = min(b, lo + 32) - lo;
+      if (x1 <= x0) return 0u;
+      return (x1 - x0 == 32) ? 0xffffffffu : (((1u << (x1 - x0)) - 1u) << x0);
+    };
+    bmask[0][s] = range_mask(0, Th);
+    bmask[1][s] = range_mask(Th, Th + Tw);
+    bmask[2][s] = range_mask(Th + Tw, Tall);
+  }
+  // the grid cells of the taps this lane owns around voxel `me` -> idx[] (-1: no voxel there)
+  auto lookups = [&](const int4& me, int (&idx)[kMaxTapSlots]) {
+    const bool me_in = (unsigned)me.x < (unsigned)g.batch && (unsigned)me.y < (unsigned)g.gz &&
+                       (unsigned)me.z < (unsigned)g.gh && (unsigned)me.w < (unsigned)g.gw;
+    const long long cell0 = (((long long)me.x * g.gz + me.y) * g.gh + me.z) * g.gw + me.w;
 #pragma unroll
-      for (int k = 0; k < CPL; ++k) {
-        const int ch = lane + 32 * k;
-        if (ch < c) {
-          const float v = wt[ch] * ld_elem<T>(row + ch);
-          if (br == 0) acc[0][k] += v;
-          else if (br == 1) acc[1][k] += v;
-          else acc[2][k] += v;
+    for (int s = 0; s < kMaxTapSlots; ++s) {
+      const bool inside = me_in && (unsigned)(me.y + tdz[s]) < (unsigned)g.gz &&
+                          (unsigned)(me.z + tdy[s]) < (unsigned)g.gh && (unsigned)(me.w + tdx[s]) < (unsigned)g.gw;
+      idx[s] = inside ? grid[cell0 + tdelta[s]] : -1;
+    }
+  };
+  // Persistent warps (the weights are staged once per block, the tap set-up done once per warp), software-pipelined:
+  // while voxel i is processed, the look-ups of the warp's next voxel and the coordinates of the one after are in flight.
+  const long long stride = (long long)gridDim.x * kCwiWarps;
+  long long i = (long long)blockIdx.x * kCwiWarps + warp;
+  const int4 none = make_int4(-1, -1, -1, -1);             // outside every grid: all look-ups give -1 without a load
+  int idx[kMaxTapSlots];
+  lookups(i < N ? __ldg(coords + i) : none, idx);
+  int4 me_next = (i + stride < N) ? __ldg(coords + i + stride) : none;
+  for (; i < N; i += stride) {
+    int idx_next[kMaxTapSlots];
+    lookups(me_next, idx_next);
+    me_next = (i + 2 * stride < N) ? __ldg(coords + i + 2 * stride) : none;
+    float acc[3][CPL];
+#pragma unroll
+    for (int br = 0; br < 3; ++br) {
+#pragma unroll
+      for (int k = 0; k < CPL; ++k) acc[br][k] = 0.f;
+      const T* xb = x + br * c;
+#pragma unroll
+      for (int s = 0; s < kMaxTapSlots; ++s) {
+        if (32 * s >= Tall) break;
+        unsigned present = __ballot_sync(0xffffffffu, idx[s] >= 0) & bmask[br][s];   // this branch's taps that hit a voxel
+        while (present) {                                                            // ascending: deterministic sums
+          const int l = __ffs(present) - 1;
+          present &= present - 1;
+          const int j = __shfl_sync(0xffffffffu, idx[s], l);
+          const T* row = xb + (size_t)j * C;
+          const float* wt = s_w + (l + 32 * s) * c;
+#pragma unroll
+          for (int k = 0; k < CPL; ++k) {
+            const int ch = lane + 32 * k;
+            if (ch < c) acc[br][k] += wt[ch] * ld_elem<T>(row + ch);
+          }
         }
       }
     }
-  }
-  T* orow = out + (size_t)i * C;
-  const T* xrow = x + (size_t)i * C;
+    T* orow = out + (size_t)i * C;
+    const T* xrow = x + (size_t)i * C;
 #pragma unroll
-  for (int k = 0; k < CPL; ++k) {
-    const int ch = lane + 32 * k;
-    if (ch < c) {
-      orow[ch] = to_elem<T>(acc[0][k]);
-      orow[c + ch] = to_elem<T>(acc[1][k]);
-      orow[2 * c + ch] = to_elem<T>(acc[2][k]);
-      orow[3 * c + ch] = xrow[3 * c + ch];               // Eq. 4: identity branch
+    for (int k = 0; k < CPL; ++k) {
+      const int ch = lane + 32 * k;
+      if (ch < c) {
+        orow[ch] = to_elem<T>(acc[0][k]);
+        orow[c + ch] = to_elem<T>(acc[1][k]);
+        orow[2 * c + ch] = to_elem<T>(acc[2][k]);
+        orow[3 * c + ch] = xrow[3 * c + ch];               // Eq. 4: identity branch
+      }
     }
+#pragma unroll
+    for (int s = 0; s < kMaxTapSlots; ++s) idx[s] = idx_next[s];
   }
 }
 
@@ -170,7 +201,9 @@ cudaError_t cwi_launch(const void* x, const int32_t* coords, int N, int C, Geom 
   if (e != cudaSuccess) return e;
   const int c = C / 4;
   const size_t smem = (size_t)(S_h + S_w + 29) * c * sizeof(float);
-  const unsigned blocks = (unsigned)((N + kCwiWarps - 1) / kCwiWarps);
+  unsigned blocks = (unsigned)((N + kCwiWarps - 1) / kCwiWarps);
+  if (blocks > 592) blocks = 592;                        // 4 x 148 blocks of 16 warps: every warp walks ~6 voxels per 60 000,
+                                                         // so the per-block weight staging and per-warp tap set-up are amortised
   const int cpl = (c + 31) / 32;
 #define SLA_CWI_LAUNCH(CPL)                                                                                         \
   launch_chained(sla_cwi_conv_kernel<T, CPL>, blocks, 32 * kCwiWarps, smem, st, (const T*)x, (const int4*)coords, N, \
