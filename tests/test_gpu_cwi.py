@@ -100,6 +100,33 @@ def test_cwi_waymo_like_scene_two_calls():
         _check(out, x, coords, 12, 12, ws, "f16")
 
 
+def test_cwi_writes_nothing_beyond_n_and_ignores_voxels_off_the_grid():
+    torch = _torch()
+    rng = np.random.Generator(np.random.PCG64(77))
+    grid = (1, 2, 16, 16)
+    coords = _dense_scene(rng, 200, *grid)
+    x = wl.round_to_dtype(rng.standard_normal((200, 64)).astype(np.float32), "f16")
+    ws = _weights(rng, 16, 4, 4)
+    buf = torch.full((264, 64), 5.0, dtype=torch.float16, device="cuda")
+    pkg.sla_cwi_forward(torch.from_numpy(x).cuda().half(), torch.from_numpy(coords).cuda(), grid, 4, 4,
+                        *(torch.from_numpy(w).cuda() for w in ws), out=buf[:200])
+    torch.cuda.synchronize()
+    assert bool((buf[200:] == 5.0).all())
+    _check(buf[:200], x, coords, 4, 4, ws, "f16")
+    # a voxel off the grid: nobody sees it, its own convolution branches are zero, its identity branch is copied
+    co2 = coords.copy()
+    co2[7] = (0, 0, 16, 3)
+    out = pkg.sla_cwi_forward(torch.from_numpy(x).cuda().half(), torch.from_numpy(co2).cuda(), grid, 4, 4,
+                              *(torch.from_numpy(w).cuda() for w in ws))
+    torch.cuda.synchronize()
+    keep = np.ones(200, bool)
+    keep[7] = False
+    ref = O.cwi_forward(x[keep], co2[keep], 4, 4, *ws)
+    got = out.double().cpu().numpy()
+    assert np.allclose(got[keep], ref, rtol=2e-3, atol=2e-3)
+    assert np.all(got[7, :48] == 0) and np.array_equal(got[7, 48:], x[7, 48:].astype(np.float64))
+
+
 def test_cwi_errors():
     torch = _torch()
     x = torch.zeros(10, 128, dtype=torch.float16, device="cuda")

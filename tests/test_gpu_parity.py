@@ -444,6 +444,23 @@ def test_backward_bounded_generic_path_and_errors(dtype, d):
         pkg.sla_backward(*dev, off, to_dev(g, dtype), max_window_len=16, phi="relu", eps=1e-6)
 
 
+@pytest.mark.parametrize("dtype,H,d", [("f16", 8, 16), ("bf16", 8, 32), ("f16", 2, 32)])
+def test_backward_writes_nothing_beyond_n(dtype, H, d):
+    """Guard rows behind dq, dk, dv keep their sentinel (ragged last tiles, split windows, partial slabs)."""
+    torch = _torch()
+    sc = wl.make_scene([13, 300, 1, 29, 257, 7], H, d, dtype, seed=91)
+    q, k, v, g = (to_dev(sc.tensor(n), dtype) for n in ("q", "k", "v", "do"))
+    off = torch.from_numpy(sc.offsets).cuda()
+    pad = 64
+    bufs = [torch.full((sc.N + pad, H, d), 3.0, dtype=q.dtype, device="cuda") for _ in range(3)]
+    pkg.sla_backward(q, k, v, off, g, dq=bufs[0][:sc.N], dk=bufs[1][:sc.N], dv=bufs[2][:sc.N])
+    torch.cuda.synchronize()
+    for b in bufs:
+        assert bool((b[sc.N:] == 3.0).all())
+    ref = sla_oracle.backward(sc.tensor("q"), sc.tensor("k"), sc.tensor("v"), sc.tensor("do"), sc.offsets)
+    check_grads([b[:sc.N] for b in bufs], ref, sc)
+
+
 def test_forward_under_cuda_graph_replay():
     """The C-ABI calls are capturable: a graph of prep + forward replays to the same result."""
     torch = _torch()

@@ -97,6 +97,20 @@ def test_projection_full_size_configs():
             assert torch.equal(a, c)                      # deterministic: no atomics, fixed accumulation order
 
 
+@pytest.mark.parametrize("N", [1, 129, 300])
+def test_projection_writes_nothing_beyond_n(N):
+    """The last tile is clipped by the TMA unit: rows N.. of larger output buffers keep their sentinel."""
+    torch = _torch()
+    x, w, _ = _inputs(N, 128, "f16", 40 + N, False)
+    pad = 200
+    bufs = [torch.full((N + pad, 128), 7.0, dtype=torch.float16, device="cuda") for _ in range(3)]
+    pkg.sla_qkv_projection(_dev(x, "f16"), _dev(w, "f16"), q=bufs[0][:N], k=bufs[1][:N], v=bufs[2][:N])
+    torch.cuda.synchronize()
+    for b in bufs:
+        assert bool((b[N:] == 7.0).all())
+    _check_proj([b[:N] for b in bufs], x, w, None, "f16")
+
+
 def test_projection_errors_and_empty():
     torch = _torch()
     x = torch.zeros(10, 64, dtype=torch.float16, device="cuda")
