@@ -56,10 +56,9 @@ template <> __device__ __forceinline__ __half to_elem<__half>(float v) { return 
 template <> __device__ __forceinline__ __nv_bfloat16 to_elem<__nv_bfloat16>(float v) { return __float2bfloat16_rn(v); }
 
 constexpr int kCwiWarps = 16;
-constexpr int kMaxTapSlots = 4;    // taps per lane: S_h + S_w + 29 <= 128
 
-// CPL = channels of a branch per lane = ceil(c / 32)
-template <typename T, int CPL>
+// CPL = channels of a branch per lane = ceil(c / 32); NS = 32-tap slots = ceil((S_h + S_w + 29) / 32)
+template <typename T, int CPL, int NS>
 __global__ void __launch_bounds__(32 * kCwiWarps)
 sla_cwi_conv_kernel(const T* __restrict__ x, const int4* __restrict__ coords, int N, int C, Geom g, int S_h, int S_w,
                     const float* __restrict__ w_h, const float* __restrict__ w_w, const float* __restrict__ w_3,
@@ -81,9 +80,9 @@ sla_cwi_conv_kernel(const T* __restrict__ x, const int4* __restrict__ coords, in
   __syncthreads();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   // the taps a lane owns (tap t = lane + 32 s) and their offsets do not depend on the voxel
-  int tdz[kMaxTapSlots], tdy[kMaxTapSlots], tdx[kMaxTapSlots], tdelta[kMaxTapSlots];
+  int tdz[NS], tdy[NS], tdx[NS], tdelta[NS];
 #pragma unroll
-  for (int s = 0; s < kMaxTapSlots; ++s) {
+  for (int s = 0; s < NS; ++s) {
     const int t = lane + 32 * s;
     int dz = 0, dy = 0, dx = 0;
     if (t < Th) dy = t - (S_h >> 1);
@@ -94,9 +93,9 @@ sla_cwi_conv_kernel(const T* __restrict__ x, const int4* __restrict__ coords, in
     tdelta[s] = (dz * g.gh + dy) * g.gw + dx;              // |.| < 2^31 cells
   }
   // bit masks of the taps of each branch inside each 32-tap slot
-  unsigned bmask[3][kMaxTapSlots];
+  unsigned bmask[3][NS];
 #pragma unroll
-  for (int s = 0; s < kMaxTapSlots; ++s) {
+  for (int s = 0; s < NS; ++s) {
     const int lo = 32 * s;
     auto range_mask = [&](int a, int b) -> unsigned {      // taps [a, b) intersected with [lo, lo + 32)
       const int x0 = max(a, lo) - lo, x1 = min(b, lo + 32) - lo;
@@ -107,39 +106,50 @@ sla_cwi_conv_kernel(const T* __restrict__ x, const int4* __restrict__ coords, in
     bmask[1][s] = range_mask(Th, Th + Tw);
     bmask[2][s] = range_mask(Th + Tw, Tall);
   }
+  // the centre tap of every branch is the voxel itself: no look-up, no shuffle; taken out of the masks
+  const int tc[3] = {S_h >> 1, Th + (S_w >> 1), Th + Tw + 13};
+#pragma unroll
+  for (int br = 0; br < 3; ++br)
+#pragma unroll
+    for (int s = 0; s < NS; ++s)
+      if ((tc[br] >> 5) == s) bmask[br][s] &= ~(1u << (tc[br] & 31));
   // the grid cells of the taps this lane owns around voxel `me` -> idx[] (-1: no voxel there)
-  auto lookups = [&](const int4& me, int (&idx)[kMaxTapSlots]) {
+  auto lookups = [&](const int4& me, int (&idx)[NS]) -> bool {
     const bool me_in = (unsigned)me.x < (unsigned)g.batch && (unsigned)me.y < (unsigned)g.gz &&
                        (unsigned)me.z < (unsigned)g.gh && (unsigned)me.w < (unsigned)g.gw;
     const long long cell0 = (((long long)me.x * g.gz + me.y) * g.gh + me.z) * g.gw + me.w;
 #pragma unroll
-    for (int s = 0; s < kMaxTapSlots; ++s) {
+    for (int s = 0; s < NS; ++s) {
       const bool inside = me_in && (unsigned)(me.y + tdz[s]) < (unsigned)g.gz &&
                           (unsigned)(me.z + tdy[s]) < (unsigned)g.gh && (unsigned)(me.w + tdx[s]) < (unsigned)g.gw;
       idx[s] = inside ? grid[cell0 + tdelta[s]] : -1;
     }
+    return me_in;
   };
   // Persistent warps (the weights are staged once per block, the tap set-up done once per warp), software-pipelined:
   // while voxel i is processed, the look-ups of the warp's next voxel and the coordinates of the one after are in flight.
   const long long stride = (long long)gridDim.x * kCwiWarps;
   long long i = (long long)blockIdx.x * kCwiWarps + warp;
   const int4 none = make_int4(-1, -1, -1, -1);             // outside every grid: all look-ups give -1 without a load
-  int idx[kMaxTapSlots];
-  lookups(i < N ? __ldg(coords + i) : none, idx);
+  int idx[NS];
+  bool in_grid = lookups(i < N ? __ldg(coords + i) : none, idx);
   int4 me_next = (i + stride < N) ? __ldg(coords + i + stride) : none;
   for (; i < N; i += stride) {
-    int idx_next[kMaxTapSlots];
-    lookups(me_next, idx_next);
+    int idx_next[NS];
+    const bool in_grid_next = lookups(me_next, idx_next);
     me_next = (i + 2 * stride < N) ? __ldg(coords + i + 2 * stride) : none;
+    const T* xrow = x + (size_t)i * C;
     float acc[3][CPL];
 #pragma unroll
     for (int br = 0; br < 3; ++br) {
 #pragma unroll
-      for (int k = 0; k < CPL; ++k) acc[br][k] = 0.f;
+      for (int k = 0; k < CPL; ++k) {                      // centre tap (a voxel off the grid gets zeros here)
+        const int ch = lane + 32 * k;
+        acc[br][k] = (in_grid && ch < c) ? s_w[tc[br] * c + ch] * ld_elem<T>(xrow + br * c + ch) : 0.f;
+      }
       const T* xb = x + br * c;
 #pragma unroll
-      for (int s = 0; s < kMaxTapSlots; ++s) {
-        if (32 * s >= Tall) break;
+      for (int s = 0; s < NS; ++s) {
         unsigned present = __ballot_sync(0xffffffffu, idx[s] >= 0) & bmask[br][s];   // this branch's taps that hit a voxel
         while (present) {                                                            // ascending: deterministic sums
           const int l = __ffs(present) - 1;
@@ -156,7 +166,6 @@ sla_cwi_conv_kernel(const T* __restrict__ x, const int4* __restrict__ coords, in
       }
     }
     T* orow = out + (size_t)i * C;
-    const T* xrow = x + (size_t)i * C;
 #pragma unroll
     for (int k = 0; k < CPL; ++k) {
       const int ch = lane + 32 * k;
@@ -168,7 +177,8 @@ sla_cwi_conv_kernel(const T* __restrict__ x, const int4* __restrict__ coords, in
       }
     }
 #pragma unroll
-    for (int s = 0; s < kMaxTapSlots; ++s) idx[s] = idx_next[s];
+    for (int s = 0; s < NS; ++s) idx[s] = idx_next[s];
+    in_grid = in_grid_next;
   }
 }
 
@@ -205,15 +215,24 @@ cudaError_t cwi_launch(const void* x, const int32_t* coords, int N, int C, Geom 
   if (blocks > 592) blocks = 592;                        // 4 x 148 blocks of 16 warps: every warp walks ~6 voxels per 60 000,
                                                          // so the per-block weight staging and per-warp tap set-up are amortised
   const int cpl = (c + 31) / 32;
-#define SLA_CWI_LAUNCH(CPL)                                                                                         \
-  launch_chained(sla_cwi_conv_kernel<T, CPL>, blocks, 32 * kCwiWarps, smem, st, (const T*)x, (const int4*)coords, N, \
-                 C, g, S_h, S_w, w_h, w_w, w_3, (const int32_t*)grid, (T*)out)
-  switch (cpl) {
-    case 1: return SLA_CWI_LAUNCH(1);
-    case 2: return SLA_CWI_LAUNCH(2);
-    case 3: return SLA_CWI_LAUNCH(3);
-    default: return SLA_CWI_LAUNCH(4);
+#define SLA_CWI_LAUNCH(CPL, NS)                                                                                    \
+  launch_chained(sla_cwi_conv_kernel<T, CPL, NS>, blocks, 32 * kCwiWarps, smem, st, (const T*)x, (const int4*)coords, \
+                 N, C, g, S_h, S_w, w_h, w_w, w_3, (const int32_t*)grid, (T*)out)
+#define SLA_CWI_SLOTS(CPL)                     \
+  switch (ns) {                                \
+    case 1: return SLA_CWI_LAUNCH(CPL, 1);     \
+    case 2: return SLA_CWI_LAUNCH(CPL, 2);     \
+    case 3: return SLA_CWI_LAUNCH(CPL, 3);     \
+    default: return SLA_CWI_LAUNCH(CPL, 4);    \
   }
+  const int ns = (S_h + S_w + 29 + 31) / 32;
+  switch (cpl) {
+    case 1: SLA_CWI_SLOTS(1)
+    case 2: SLA_CWI_SLOTS(2)
+    case 3: SLA_CWI_SLOTS(3)
+    default: SLA_CWI_SLOTS(4)
+  }
+#undef SLA_CWI_SLOTS
 #undef SLA_CWI_LAUNCH
 }
 
