@@ -235,6 +235,12 @@ int sla_sequence_from_coords(const int32_t* coords, int64_t N, int32_t batch, in
 int sla_qkv_projection(const void* x, const void* w_qkv, const float* bias, int64_t N, int32_t C, int dt,
                        void* q, void* k, void* v, sla_stream_t stream);
 
+/* One linear layer with the same kernel: y[N, C] = x[N, C] . w[C, C]^T (+ bias), e.g. the output projection that follows
+ * the attention in a transformer block (the paper's module implies one; it prints no formula for it).  w is [C, C], row j =
+ * weights of output feature j; bias fp32 [C] or NULL; same support and alignment rules as sla_qkv_projection; x != y. */
+int sla_linear(const void* x, const void* w, const float* bias, int64_t N, int32_t C, int dt, void* y,
+               sla_stream_t stream);
+
 /* The module of PAPER.md:77: projection, then SLA(Q, K, V) (Eq. 2-3): sla_qkv_projection followed by sla_forward on
  * the same stream (one chain of programmatic dependent launches; q, k, v stay in L2 between the two when 3 N C
  * elements fit there).  q, k, v are caller-owned outputs as well (a training step needs them for sla_backward);

@@ -24,7 +24,7 @@ SYMBOLS = (
     "sla_bench_stream_ceiling",
     "sla_window_count", "sla_window_keys", "sla_sort_workspace_bytes", "sla_sort_by_window", "sla_gather_rows",
     "sla_scatter_rows", "sla_sequence_workspace_bytes", "sla_sequence_from_coords",
-    "sla_qkv_projection", "sla_module_forward", "sla_cwi_workspace_bytes", "sla_cwi_forward",
+    "sla_qkv_projection", "sla_linear", "sla_module_forward", "sla_cwi_workspace_bytes", "sla_cwi_forward",
 )
 
 _lib = None
@@ -91,6 +91,8 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     L.sla_sequence_from_coords.restype = ci
     L.sla_qkv_projection.argtypes = [vp, vp, vp, i64, i32, ci, vp, vp, vp, vp]
     L.sla_qkv_projection.restype = ci
+    L.sla_linear.argtypes = [vp, vp, vp, i64, i32, ci, vp, vp]
+    L.sla_linear.restype = ci
     L.sla_module_forward.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp, vp, vp, vp, sz, vp]
     L.sla_module_forward.restype = ci
     L.sla_cwi_workspace_bytes.argtypes = [i32, i32, i32, i32]
@@ -398,6 +400,23 @@ def sla_qkv_projection(x, w_qkv, bias=None, q=None, k=None, v=None, stream=None)
                                 _dt(x), q.data_ptr(), k.data_ptr(), v.data_ptr(), _stream(stream)),
            "sla_qkv_projection")
     return q, k, v
+
+
+def sla_linear(x, w, bias=None, out=None, stream=None):
+    """y = x w^T (+ bias): x CUDA [N, C] fp16/bf16, w [C, C] (row j = weights of output feature j), bias fp32 [C]."""
+    import torch
+    L = load_library()
+    _chk_dev(x, w)
+    if x.dim() != 2 or tuple(w.shape) != (x.shape[1], x.shape[1]) or w.dtype != x.dtype:
+        raise SlaError("x must be [N, C] and w [C, C] of the same dtype")
+    if bias is not None:
+        _chk_dev(bias)
+        if bias.dtype != torch.float32 or bias.numel() != x.shape[1]:
+            raise SlaError("bias must be fp32 [C]")
+    out = torch.empty_like(x) if out is None else out
+    _check(L.sla_linear(x.data_ptr(), w.data_ptr(), bias.data_ptr() if bias is not None else None, x.shape[0],
+                        x.shape[1], _dt(x), out.data_ptr(), _stream(stream)), "sla_linear")
+    return out
 
 
 def sla_module_forward(x, w_qkv, window_offsets, H: int, bias=None, q=None, k=None, v=None, out=None, workspace=None,

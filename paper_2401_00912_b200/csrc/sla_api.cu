@@ -173,7 +173,18 @@ int sla_qkv_projection(const void* x, const void* w_qkv, const float* bias, int6
   if (!x || !w_qkv || !q || !k || !v) return SLA_ERR_INVALID_ARG;
   if (!aligned16(x) || !aligned16(w_qkv) || !aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(bias))
     return SLA_ERR_UNSUPPORTED;
-  cudaError_t e = sla::launch_qkv_projection(x, w_qkv, bias, (int)N, C, dt, q, k, v, (cudaStream_t)stream);
+  cudaError_t e = sla::launch_qkv_projection(x, w_qkv, bias, (int)N, C, dt, 3, q, k, v, (cudaStream_t)stream);
+  return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
+}
+
+int sla_linear(const void* x, const void* w, const float* bias, int64_t N, int32_t C, int dt, void* y,
+               sla_stream_t stream) {
+  if (N < 0 || N >= (int64_t(1) << 31) || C < 1) return SLA_ERR_INVALID_ARG;
+  if (!sla::qkv_projection_supported(C, dt)) return SLA_ERR_UNSUPPORTED;
+  if (N == 0) return SLA_OK;
+  if (!x || !w || !y || x == y) return SLA_ERR_INVALID_ARG;
+  if (!aligned16(x) || !aligned16(w) || !aligned16(y) || !aligned16(bias)) return SLA_ERR_UNSUPPORTED;
+  cudaError_t e = sla::launch_qkv_projection(x, w, bias, (int)N, C, dt, 1, y, nullptr, nullptr, (cudaStream_t)stream);
   return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
 }
 

@@ -104,8 +104,9 @@ cudaError_t launch_permute_rows(const void* src, const int32_t* perm, long long 
                                 bool scatter, cudaStream_t st);
 // shared Q/K/V projection (sla_proj.cu): y = x w^T (+ bias) on tcgen05, split into q, k, v
 bool qkv_projection_supported(int C, int dt);
-cudaError_t launch_qkv_projection(const void* x, const void* w, const float* bias, int N, int C, int dt, void* q,
-                                  void* k, void* v, cudaStream_t st);
+// n_out = 3: w [3C, C] -> q, k, v; n_out = 1: w [C, C] -> q only (a plain linear layer, e.g. the output projection)
+cudaError_t launch_qkv_projection(const void* x, const void* w, const float* bias, int N, int C, int dt, int n_out,
+                                  void* q, void* k, void* v, cudaStream_t st);
 // Cross-Window Interaction (sla_cwi.cu): depth-wise sparse convolutions on the active voxels
 cudaError_t launch_cwi(const void* x, const int32_t* coords, int N, int C, int dt, int batch, int gz, int gh, int gw,
                        int S_h, int S_w, const float* w_h, const float* w_w, const float* w_3, void* out,

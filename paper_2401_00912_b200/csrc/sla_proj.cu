@@ -32,7 +32,6 @@ constexpr int THREADS = (WARP_EPI0 + NUM_EPI_WARPS) * 32;
 template <int C> struct Cfg {
   static constexpr int KB = C / 64;                       // 64-column boxes along K
   static constexpr int KSTEPS = C / 16;
-  static constexpr int NCH = 3 * C / CHUNK_N;             // chunks of output features
   static constexpr int OPERAND_BYTES = KB * BOX_BYTES;    // a 128 x C operand tile
   static constexpr int NA = (C <= 128) ? 2 : 1;           // x-tile stages
   static constexpr int NWS = 2;                           // w-chunk stages
@@ -118,7 +117,8 @@ template <int N> __device__ __forceinline__ void advance(Cur& c) { if (++c.s == 
 
 template <int C, bool BF16, typename T>
 __global__ void __launch_bounds__(THREADS, 1)
-sla_qkv_proj_kernel(const __grid_constant__ Maps maps, const float* __restrict__ bias, int N) {
+sla_qkv_proj_kernel(const __grid_constant__ Maps maps, const float* __restrict__ bias, int N, int nch) {
+  // nch = chunks of 128 output features = (number of [N, C] output tensors: 3 for q, k, v; 1 for a plain layer) * C / 128
   using G = Cfg<C>;
   extern __shared__ uint8_t dyn_smem[];
   __shared__ Ctrl ctrl;
@@ -128,7 +128,7 @@ sla_qkv_proj_kernel(const __grid_constant__ Maps maps, const float* __restrict__
   // Work unit = (128-row tile, 128-feature chunk).  Every CTA takes one contiguous range of units, so the ranges differ
   // by at most one chunk (a third of a tile at C = 128) where whole tiles would differ by one tile in ~3; a tile that
   // straddles two ranges is loaded by both CTAs (the second time out of L2).
-  const long long units = (long long)((N + TILE_M - 1) / TILE_M) * G::NCH;
+  const long long units = (long long)((N + TILE_M - 1) / TILE_M) * nch;
   const int u0 = (int)(units * blockIdx.x / gridDim.x), u1 = (int)(units * (blockIdx.x + 1) / gridDim.x);
 
   if (threadIdx.x == 0) {
@@ -159,7 +159,7 @@ sla_qkv_proj_kernel(const __grid_constant__ Maps maps, const float* __restrict__
     if (lane == 0) {
       Cur a{0, 0}, w{0, 0};
       for (int u = u0; u < u1; ++u) {
-        const int tile = u / G::NCH, j = u % G::NCH;
+        const int tile = u / nch, j = u % nch;
         if (j == 0 || u == u0) {                                     // first unit of a tile in this range: its x rows
           mbar_wait_wd(smem_u32(&ctrl.a_empty[a.s]), a.ph ^ 1u);     // passes at once on a stage never used
           const uint32_t abar = smem_u32(&ctrl.a_full[a.s]);
@@ -183,7 +183,7 @@ sla_qkv_proj_kernel(const __grid_constant__ Maps maps, const float* __restrict__
       constexpr uint32_t IDESC = make_idesc(TILE_M, CHUNK_N, BF16);
       Cur a{0, 0}, w{0, 0}, acc{0, 0};
       for (int u = u0; u < u1; ++u) {
-        const int j = u % G::NCH;
+        const int j = u % nch;
         if (j == 0 || u == u0) mbar_wait_wd(smem_u32(&ctrl.a_full[a.s]), a.ph);
         const uint32_t abase = sbase + G::OFF_A + a.s * G::OPERAND_BYTES;
         mbar_wait_wd(smem_u32(&ctrl.w_full[w.s]), w.ph);
@@ -201,7 +201,7 @@ sla_qkv_proj_kernel(const __grid_constant__ Maps maps, const float* __restrict__
         umma_commit(smem_u32(&ctrl.acc_full[acc.s]));
         advance<G::NWS>(w);
         advance<2>(acc);
-        if (j == G::NCH - 1 || u == u1 - 1) {             // last unit of the tile in this range: hand the x stage back
+        if (j == nch - 1 || u == u1 - 1) {             // last unit of the tile in this range: hand the x stage back
           umma_commit(smem_u32(&ctrl.a_empty[a.s]));
           advance<G::NA>(a);
         }
@@ -216,7 +216,7 @@ sla_qkv_proj_kernel(const __grid_constant__ Maps maps, const float* __restrict__
     int os = 0;                                              // staging buffer of the next chunk
     {
       for (int u = u0; u < u1; ++u) {
-        const int tile = u / G::NCH, j = u % G::NCH;
+        const int tile = u / nch, j = u % nch;
         // the staging buffer must have been read by the bulk store of the chunk that used it last
         if (et == 0) bulk_wait_read<G::NOS - 1>();
         asm volatile("bar.sync 1, 128;" ::: "memory");
@@ -274,14 +274,18 @@ sla_qkv_proj_kernel(const __grid_constant__ Maps maps, const float* __restrict__
   }
 }
 
+// n_out = 3: w is [3C, C], outputs q, k, v; n_out = 1: w is [C, C], one output (k and v unused)
 template <int C, bool BF16, typename T>
-cudaError_t proj_launch(const void* x, const void* w, const float* bias, int N, void* q, void* k, void* v,
+cudaError_t proj_launch(const void* x, const void* w, const float* bias, int N, int n_out, void* q, void* k, void* v,
                         cudaStream_t st) {
   using G = Cfg<C>;
   Maps maps;
-  if (!make_map(&maps.x, x, N, C, TILE_M) || !make_map(&maps.w, w, 3 * C, C, CHUNK_N) ||
-      !make_map(&maps.out[0], q, N, C, TILE_M) || !make_map(&maps.out[1], k, N, C, TILE_M) ||
-      !make_map(&maps.out[2], v, N, C, TILE_M))
+  if (!make_map(&maps.x, x, N, C, TILE_M) || !make_map(&maps.w, w, n_out * C, C, CHUNK_N) ||
+      !make_map(&maps.out[0], q, N, C, TILE_M))
+    return cudaErrorInvalidValue;
+  maps.out[1] = maps.out[0];
+  maps.out[2] = maps.out[0];
+  if (n_out == 3 && (!make_map(&maps.out[1], k, N, C, TILE_M) || !make_map(&maps.out[2], v, N, C, TILE_M)))
     return cudaErrorInvalidValue;
   auto kern = sla_qkv_proj_kernel<C, BF16, T>;
   static std::atomic<bool> attr_set[kMaxDevices];         // the smem opt-in is per device
@@ -302,7 +306,7 @@ cudaError_t proj_launch(const void* x, const void* w, const float* bias, int N, 
   cfg.stream = st;
   cfg.attrs = pdl;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, kern, maps, bias, N);
+  return cudaLaunchKernelEx(&cfg, kern, maps, bias, N, n_out * C / CHUNK_N);
 }
 
 }  // namespace
@@ -313,13 +317,13 @@ bool qkv_projection_supported(int C, int dt) {
   return encode_fn() != nullptr;
 }
 
-cudaError_t launch_qkv_projection(const void* x, const void* w, const float* bias, int N, int C, int dt, void* q,
-                                  void* k, void* v, cudaStream_t st) {
+cudaError_t launch_qkv_projection(const void* x, const void* w, const float* bias, int N, int C, int dt, int n_out,
+                                  void* q, void* k, void* v, cudaStream_t st) {
   if (C == 128)
-    return dt == SLA_F16 ? proj_launch<128, false, __half>(x, w, bias, N, q, k, v, st)
-                         : proj_launch<128, true, __nv_bfloat16>(x, w, bias, N, q, k, v, st);
-  return dt == SLA_F16 ? proj_launch<256, false, __half>(x, w, bias, N, q, k, v, st)
-                       : proj_launch<256, true, __nv_bfloat16>(x, w, bias, N, q, k, v, st);
+    return dt == SLA_F16 ? proj_launch<128, false, __half>(x, w, bias, N, n_out, q, k, v, st)
+                         : proj_launch<128, true, __nv_bfloat16>(x, w, bias, N, n_out, q, k, v, st);
+  return dt == SLA_F16 ? proj_launch<256, false, __half>(x, w, bias, N, n_out, q, k, v, st)
+                       : proj_launch<256, true, __nv_bfloat16>(x, w, bias, N, n_out, q, k, v, st);
 }
 
 }  // namespace sla

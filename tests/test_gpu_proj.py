@@ -111,6 +111,25 @@ def test_projection_writes_nothing_beyond_n(N):
     _check_proj([b[:N] for b in bufs], x, w, None, "f16")
 
 
+@pytest.mark.parametrize("N,C,dtype,bias", [(1000, 128, "f16", True), (333, 256, "bf16", False), (60000, 128, "f16", False)])
+def test_linear_against_oracle(N, C, dtype, bias):
+    """sla_linear (one [C, C] layer, e.g. the output projection) = the first block of the projection oracle."""
+    torch = _torch()
+    rng = np.random.Generator(np.random.PCG64(N + C))
+    x = wl.round_to_dtype(rng.standard_normal((N, C)).astype(np.float32), dtype)
+    w = wl.round_to_dtype((rng.standard_normal((C, C)) / np.sqrt(C)).astype(np.float32), dtype)
+    b = rng.standard_normal(C).astype(np.float32) if bias else None
+    got = pkg.sla_linear(_dev(x, dtype), _dev(w, dtype), _dev(b) if bias else None)
+    torch.cuda.synchronize()
+    w3 = np.concatenate([w, np.zeros((2 * C, C), np.float32)], axis=0)
+    b3 = np.concatenate([b, np.zeros(2 * C, np.float32)]) if bias else None
+    ref = P.project_qkv(x, w3, b3)[0]
+    acc = P.accumulation_bound(x, w3, b3)[0][:, :C]
+    allowed = acc + UNIT[dtype] * (np.abs(ref) + acc) + 2.0 ** -24
+    g = got.double().cpu().numpy()
+    assert np.isfinite(g).all() and (np.abs(g - ref) / allowed).max() <= 1.0
+
+
 def test_projection_errors_and_empty():
     torch = _torch()
     x = torch.zeros(10, 64, dtype=torch.float16, device="cuda")
