@@ -77,12 +77,20 @@ __device__ __forceinline__ void make_ops(const float (&X)[2][4], float scale, Op
     }
 }
 
-// phi of a packed pair in fp32 (a) and its derivative factor (x>0 ? 1 : phi(x))
-template <bool BF16>
+// phi of a packed pair in fp32 (a) and its derivative factor: elu+1: (x>0 ? 1 : phi(x)); ReLU: [x > 0]
+template <int MODE>
 __device__ __forceinline__ void phi_pair(uint32_t raw, float2& a, float2& da) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   const float2 x = unpack2<BF16>(raw);
-  da.x = dphi_fast(x.x); da.y = dphi_fast(x.y);
-  a.x = fmaxf(x.x, 0.f) + da.x; a.y = fmaxf(x.y, 0.f) + da.y;
+  if (PHI) {   // max(x, 0): phi' = [x > 0]
+    da.x = x.x > 0.f ? 1.f : 0.f; da.y = x.y > 0.f ? 1.f : 0.f;
+    a.x = fmaxf(x.x, 0.f); a.y = fmaxf(x.y, 0.f);
+  } else {
+    da.x = dphi_fast(x.x); da.y = dphi_fast(x.y);
+    a.x = fmaxf(x.x, 0.f) + da.x; a.y = fmaxf(x.y, 0.f) + da.y;
+  }
 }
 template <bool PRECISE>
 __device__ __forceinline__ void to_op(float x0, float x1, uint32_t& hi, uint32_t& lo) {
@@ -100,6 +108,26 @@ __device__ __forceinline__ void mma3(float (&c)[4], const uint32_t (&ah)[4], con
   }
 }
 
+// ReLU map only: with max(x, 0) a row's denominator can be eps alone, and g/den, dden reach 1/eps.  Every product that
+// survives in the result then meets a zero factor (phi or phi' vanishes wherever the row's a.b did), so such
+// intermediates only have to stay finite as fp16 operands: clamp them instead of letting them overflow to inf (0 * inf).
+template <int PHI>
+__device__ __forceinline__ float sat_h(float x) { return PHI ? fminf(fmaxf(x, -60000.f), 60000.f) : x; }
+
+// ReLU map only: power-of-two rescaling of a tile's large intermediates.  `mx` = this lane's largest magnitude; returns k
+// such that the warp-wide maximum times 2^-k is below 2^15 (k = 0 for the elu+1 map and for ordinary tiles), at most
+// 10 so that the partner operand, phi(q) * 2^k, stays inside fp16.  The operand that carries 1/den is multiplied by
+// 2^-k and its partner (or the fresh accumulator) by 2^k: exact.  What is still above fp16 after that belongs to rows
+// whose denominator is eps alone (sat_h above).
+template <int PHI>
+__device__ __forceinline__ int tile_shift(float mx) {
+  if (!PHI) return 0;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  return min(10, max(0, (int)((__float_as_uint(mx) >> 23) & 0xffu) - 127 - 14));
+}
+__device__ __forceinline__ float pow2f(int k) { return __uint_as_float((uint32_t)(127 + k) << 23); }
+
 // lane -> (tile row, 16-byte chunk select) for the x4 ldmatrix pattern
 //   registers: (rows0-7,c0), (rows0-7,c1), (rows8-15,c0), (rows8-15,c1)
 __device__ __forceinline__ void lane_pattern(int nvalid, int& trow, int& csel) {
@@ -110,8 +138,11 @@ __device__ __forceinline__ void lane_pattern(int nvalid, int& trow, int& csel) {
 }
 
 // ---- pass A: one 16-row K/V tile -> S^T, S, z -------------------------------------------------------
-template <bool BF16, bool PRECISE>
+template <int MODE, bool PRECISE>
 __device__ __forceinline__ void bwd_kv_tile(const RingView& rv, int hl, int rel0, int nvalid, BwdState& s) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   const int t = threadIdx.x & 3;
   int trow, csel;
   lane_pattern(nvalid, trow, csel);
@@ -126,11 +157,11 @@ __device__ __forceinline__ void bwd_kv_tile(const RingView& rv, int hl, int rel0
     const int j0 = 2 * t + 8 * (i >> 1);
     if (PRECISE) {
       const float2 x = unpack2<BF16>(kr[i]);
-      const float b0 = (j0 < nvalid) ? phi_fast(x.x) : 0.f;
-      const float b1 = (j0 + 1 < nvalid) ? phi_fast(x.y) : 0.f;
+      const float b0 = (j0 < nvalid) ? phi_fast<PHI>(x.x) : 0.f;
+      const float b1 = (j0 + 1 < nvalid) ? phi_fast<PHI>(x.y) : 0.f;
       to_op<true>(b0, b1, bh[i], bl[i]);
     } else {   // long window: phi in fp16x2 (the operand is a single fp16 anyway), rows beyond the window zeroed
-      bh[i] = phi_h2<BF16>(kr[i]);
+      bh[i] = phi_h2<BF16, PHI>(kr[i]);
       if (nvalid < 16) bh[i] &= pair_mask(j0, nvalid);
       bl[i] = 0u;
     }
@@ -160,13 +191,17 @@ struct PassBOps {
   OpPair da;             // from S  : B operand of da = dnum S^T
   uint32_t zh[2], zl[2]; // z as B operand of den
   float zs[2][2];        // scaled z in columns p = 8*np + 2t + c
+  float eps;             // epsilon of the denominator on the scale of the operands (eps * s); 0 for elu+1
 };
 
 // ---- pass B: one 16-row Q/dO tile -> dq rows, dS^T, dS, dz accumulators ------------------------------
-template <bool BF16, bool PRECISE, typename T>
+template <int MODE, bool PRECISE, typename T>
 __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0, int nvalid,
                                            const PassBOps& op, BwdState& s, T* __restrict__ dq_rows,
                                            int C_total) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   int trow, csel;
   lane_pattern(nvalid, trow, csel);
@@ -182,10 +217,10 @@ __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0,
   for (int i = 0; i < 4; ++i) {
     if (PRECISE) {
       float2 a;
-      phi_pair<BF16>(qn[perm[i]], a, dph[i]);
+      phi_pair<MODE>(qn[perm[i]], a, dph[i]);
       to_op<true>(a.x, a.y, ah[i], al[i]);
     } else {
-      phi_dphi_h2<BF16>(qn[perm[i]], ah[i], dph2[i]);
+      phi_dphi_h2<BF16, PHI>(qn[perm[i]], ah[i], dph2[i]);
       al[i] = 0u;
     }
     gv[i] = unpack2<BF16>(gn[perm[i]]);
@@ -194,20 +229,30 @@ __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0,
   mma3<PRECISE>(den, ah, al, op.zh[0], op.zh[1], op.zl[0], op.zl[1]);
 #pragma unroll
   for (int n = 0; n < 2; ++n) mma3<PRECISE>(num[n], ah, al, op.num.hi[n][0], op.num.hi[n][1], op.num.lo[n][0], op.num.lo[n][1]);
-  const float inv0 = fast_rcp(den[0]), inv1 = fast_rcp(den[2]);       // rows g, g+8
+  const float inv0 = fast_rcp(PHI ? den[0] + op.eps : den[0]), inv1 = fast_rcp(PHI ? den[2] + op.eps : den[2]);   // rows g, g+8
   // g.o per row: this lane holds columns 2t,2t+1 (tile 0) and 8+2t.. (tile 1) of rows g and g+8
   float go0 = gv[0].x * num[0][0] + gv[0].y * num[0][1] + gv[2].x * num[1][0] + gv[2].y * num[1][1];
   float go1 = gv[1].x * num[0][2] + gv[1].y * num[0][3] + gv[3].x * num[1][2] + gv[3].y * num[1][3];
   go0 += __shfl_xor_sync(0xffffffffu, go0, 1); go0 += __shfl_xor_sync(0xffffffffu, go0, 2);
   go1 += __shfl_xor_sync(0xffffffffu, go1, 1); go1 += __shfl_xor_sync(0xffffffffu, go1, 2);
   const float dden0 = -(go0 * inv0) * inv0, dden1 = -(go1 * inv1) * inv1;   // o = num*inv
+  // ReLU: rows whose denominator is almost eps alone make g/den and dden huge; rescale the tile by a power of two
+  float gmax = 0.f;
+  if (PHI) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) gmax = fmaxf(gmax, fmaxf(fabsf(gv[i].x), fabsf(gv[i].y)) * ((i & 1) ? inv1 : inv0));
+    gmax = fmaxf(gmax, fmaxf(fabsf(dden0), fabsf(dden1)));
+  }
+  const int ksh = tile_shift<PHI>(gmax);
+  const float dn = pow2f(-ksh), up = pow2f(ksh);        // both 1 unless ReLU and an ill-conditioned row
   // dnum as A fragment (rows g / g+8 scaled by their 1/den)
   uint32_t dh[4], dl[4];
-  if (PRECISE || BF16) {
-    to_op<PRECISE>(gv[0].x * inv0, gv[0].y * inv0, dh[0], dl[0]);
-    to_op<PRECISE>(gv[1].x * inv1, gv[1].y * inv1, dh[1], dl[1]);
-    to_op<PRECISE>(gv[2].x * inv0, gv[2].y * inv0, dh[2], dl[2]);
-    to_op<PRECISE>(gv[3].x * inv1, gv[3].y * inv1, dh[3], dl[3]);
+  if (PRECISE || BF16 || PHI) {
+    const float i0 = PHI ? inv0 * dn : inv0, i1 = PHI ? inv1 * dn : inv1;
+    to_op<PRECISE>(sat_h<PHI>(gv[0].x * i0), sat_h<PHI>(gv[0].y * i0), dh[0], dl[0]);
+    to_op<PRECISE>(sat_h<PHI>(gv[1].x * i1), sat_h<PHI>(gv[1].y * i1), dh[1], dl[1]);
+    to_op<PRECISE>(sat_h<PHI>(gv[2].x * i0), sat_h<PHI>(gv[2].y * i0), dh[2], dl[2]);
+    to_op<PRECISE>(sat_h<PHI>(gv[3].x * i1), sat_h<PHI>(gv[3].y * i1), dh[3], dl[3]);
   } else {   // fp16 dO, long window: scale the packed pairs directly
     const uint32_t i0h = pack_h2(inv0, inv0), i1h = pack_h2(inv1, inv1);
     dh[0] = hmul2_u32(gn[perm[0]], i0h); dh[1] = hmul2_u32(gn[perm[1]], i1h);
@@ -220,6 +265,7 @@ __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0,
     float da[4] = {0.f, 0.f, 0.f, 0.f};
     mma3<PRECISE>(da, dh, dl, op.da.hi[np][0], op.da.hi[np][1], op.da.lo[np][0], op.da.lo[np][1]);
     // C fragment (np): c0,c1 = (row g, p = 8np+2t,+1) <-> A index 2*np ; c2,c3 = row g+8 <-> A index 2*np+1
+    if (PHI) { da[0] *= up; da[1] *= up; da[2] *= up; da[3] *= up; }
     const float q0 = da[0] + dden0 * op.zs[np][0], q1 = da[1] + dden0 * op.zs[np][1];
     const float q2 = da[2] + dden1 * op.zs[np][0], q3 = da[3] + dden1 * op.zs[np][1];
     uint32_t* p0 = reinterpret_cast<uint32_t*>(dq_rows + (size_t)g * C_total + 8 * np + 2 * t);
@@ -228,8 +274,8 @@ __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0,
       if (g < nvalid) *p0 = pack_out<BF16>(q0 * dph[2 * np].x, q1 * dph[2 * np].y);
       if (g + 8 < nvalid) *p1 = pack_out<BF16>(q2 * dph[2 * np + 1].x, q3 * dph[2 * np + 1].y);
     } else {
-      if (g < nvalid) *p0 = pack_out_times_h2<BF16>(q0, q1, dph2[2 * np]);
-      if (g + 8 < nvalid) *p1 = pack_out_times_h2<BF16>(q2, q3, dph2[2 * np + 1]);
+      if (g < nvalid) *p0 = pack_out_times_h2<BF16, PHI != 0>(q0, q1, dph2[2 * np]);
+      if (g + 8 < nvalid) *p1 = pack_out_times_h2<BF16, PHI != 0>(q2, q3, dph2[2 * np + 1]);
     }
   }
   // ---- transposed operands (contraction over the rows i of the tile) ----
@@ -247,28 +293,29 @@ __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0,
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
     const int i0 = 2 * t + 8 * (i >> 1);
-    const float s0 = (i >> 1) ? ir2 : ir0, s1 = (i >> 1) ? ir3 : ir1;
+    const float s0 = ((i >> 1) ? ir2 : ir0) * dn, s1 = ((i >> 1) ? ir3 : ir1) * dn;   // dn = 1 unless ReLU
     if (PRECISE) {
       const float2 x = unpack2<BF16>(qt[i]);
-      const float a0 = (i0 < nvalid) ? phi_fast(x.x) : 0.f;       // rows beyond the window contribute nothing
-      const float a1 = (i0 + 1 < nvalid) ? phi_fast(x.y) : 0.f;
-      to_op<true>(a0, a1, uh[i], ul[i]);
+      const float a0 = (i0 < nvalid) ? phi_fast<PHI>(x.x) : 0.f;       // rows beyond the window contribute nothing
+      const float a1 = (i0 + 1 < nvalid) ? phi_fast<PHI>(x.y) : 0.f;
+      to_op<true>(sat_h<PHI>(a0 * up), sat_h<PHI>(a1 * up), uh[i], ul[i]);
     } else {
-      uh[i] = phi_h2<BF16>(qt[i]);
+      uh[i] = phi_h2<BF16, PHI>(qt[i]);
       if (nvalid < 16) uh[i] &= pair_mask(i0, nvalid);
+      if (PHI) uh[i] = hmul2_u32(uh[i], pack_h2(up, up));
       ul[i] = 0u;
     }
-    if (PRECISE || BF16) {
+    if (PRECISE || BF16 || PHI) {
       const float2 gg = unpack2<BF16>(gt[i]);
-      to_op<PRECISE>(gg.x * s0, gg.y * s1, th[i], tl[i]);
+      to_op<PRECISE>(sat_h<PHI>(gg.x * s0), sat_h<PHI>(gg.y * s1), th[i], tl[i]);
     } else {
       th[i] = hmul2_u32(gt[i], pack_h2(s0, s1));
       tl[i] = 0u;
     }
   }
   uint32_t ddh[2], ddl[2];
-  to_op<PRECISE>(dd0, dd1, ddh[0], ddl[0]);
-  to_op<PRECISE>(dd2, dd3, ddh[1], ddl[1]);
+  to_op<PRECISE>(sat_h<PHI>(dd0 * dn), sat_h<PHI>(dd1 * dn), ddh[0], ddl[0]);
+  to_op<PRECISE>(sat_h<PHI>(dd2 * dn), sat_h<PHI>(dd3 * dn), ddh[1], ddl[1]);
   const uint32_t dda_h[4] = {ddh[0], ddh[0], ddh[1], ddh[1]}, dda_l[4] = {ddl[0], ddl[0], ddl[1], ddl[1]};
 #pragma unroll
   for (int nt = 0; nt < 2; ++nt) {
@@ -288,10 +335,13 @@ struct PassCOps {
 };
 
 // ---- pass C: one 16-row K/V tile -> dk, dv rows ------------------------------------------------------
-template <bool BF16, bool PRECISE, typename T>
+template <int MODE, bool PRECISE, typename T>
 __device__ __forceinline__ void bwd_kv_out_tile(const RingView& rv, int hl, int rel0, int nvalid,
                                                 const PassCOps& op, T* __restrict__ dk_rows,
                                                 T* __restrict__ dv_rows, int C_total) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   int trow, csel;
   lane_pattern(nvalid, trow, csel);
@@ -306,10 +356,10 @@ __device__ __forceinline__ void bwd_kv_out_tile(const RingView& rv, int hl, int 
   for (int i = 0; i < 4; ++i) {
     if (PRECISE) {
       float2 b;
-      phi_pair<BF16>(kn[perm[i]], b, dph[i]);
+      phi_pair<MODE>(kn[perm[i]], b, dph[i]);
       to_op<true>(b.x, b.y, bh[i], bl[i]);
     } else {
-      phi_dphi_h2<BF16>(kn[perm[i]], bh[i], dph2[i]);
+      phi_dphi_h2<BF16, PHI>(kn[perm[i]], bh[i], dph2[i]);
       bl[i] = 0u;
     }
     if (BF16) { const float2 x = unpack2<true>(vn[perm[i]]); vh[i] = pack_h2(x.x, x.y); }
@@ -327,12 +377,12 @@ __device__ __forceinline__ void bwd_kv_out_tile(const RingView& rv, int hl, int 
     if (g < nvalid) {
       *reinterpret_cast<uint32_t*>(dv_rows + o0) = pack_out<BF16>(dv[0], dv[1]);
       *reinterpret_cast<uint32_t*>(dk_rows + o0) = PRECISE ? pack_out<BF16>(k0 * dph[2 * n].x, k1 * dph[2 * n].y)
-                                                           : pack_out_times_h2<BF16>(k0, k1, dph2[2 * n]);
+                                                           : pack_out_times_h2<BF16, PHI != 0>(k0, k1, dph2[2 * n]);
     }
     if (g + 8 < nvalid) {
       *reinterpret_cast<uint32_t*>(dv_rows + o1) = pack_out<BF16>(dv[2], dv[3]);
       *reinterpret_cast<uint32_t*>(dk_rows + o1) = PRECISE ? pack_out<BF16>(k2 * dph[2 * n + 1].x, k3 * dph[2 * n + 1].y)
-                                                           : pack_out_times_h2<BF16>(k2, k3, dph2[2 * n + 1]);
+                                                           : pack_out_times_h2<BF16, PHI != 0>(k2, k3, dph2[2 * n + 1]);
     }
   }
 }
@@ -350,10 +400,13 @@ __device__ __forceinline__ uint32_t movm_t(uint32_t x) {   // transpose of one 8
   asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(y) : "r"(x));
   return y;
 }
-template <bool BF16, typename T>
+template <int MODE, typename T>
 __device__ __forceinline__ void bwd_quad_tile(const RingView& kv, const RingView& qg, int hl, int rel0, int nvalid,
                                               int wid, T* __restrict__ dq_rows, T* __restrict__ dk_rows,
-                                              T* __restrict__ dv_rows, int C_total) {
+                                              T* __restrict__ dv_rows, int C_total, float eps) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   int trow, csel;
   lane_pattern(nvalid, trow, csel);
@@ -373,13 +426,13 @@ __device__ __forceinline__ void bwd_quad_tile(const RingView& kv, const RingView
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
     float2 a, b, x, da_, db_;
-    phi_pair<BF16>(rq[i], a, dpq[i]);
-    phi_pair<BF16>(rk[i], b, dpk[i]);
+    phi_pair<MODE>(rq[i], a, dpq[i]);
+    phi_pair<MODE>(rk[i], b, dpk[i]);
     split_h2(a.x, a.y, ah[i], al[i]);
     split_h2(b.x, b.y, bh[i], bl[i]);
-    phi_pair<BF16>(tq[i], x, da_);
+    phi_pair<MODE>(tq[i], x, da_);
     split_h2(x.x, x.y, ath[i], atl[i]);
-    phi_pair<BF16>(tk[i], x, db_);
+    phi_pair<MODE>(tk[i], x, db_);
     split_h2(x.x, x.y, bth[i], btl[i]);
     if (BF16) {
       float2 y = unpack2<true>(rg[i]); gh[i] = pack_h2(y.x, y.y);
@@ -398,12 +451,14 @@ __device__ __forceinline__ void bwd_quad_tile(const RingView& kv, const RingView
   }
   const int wi0 = __shfl_sync(0xffffffffu, wid, g), wi1 = __shfl_sync(0xffffffffu, wid, g + 8);
   float rs0 = 0.f, rs1 = 0.f;
+  unsigned same = 0u;                         // bit 2 jt + c: pair (row g, column j) in one window; bit 4 + ..: row g+8
 #pragma unroll
   for (int jt = 0; jt < 2; ++jt)
 #pragma unroll
     for (int c = 0; c < 2; ++c) {
       const int wj = __shfl_sync(0xffffffffu, wid, 8 * jt + 2 * t + c);
       const bool m0 = wj == wi0 && wj >= 0, m1 = wj == wi1 && wj >= 0;
+      same |= (m0 ? 1u : 0u) << (2 * jt + c) | (m1 ? 1u : 0u) << (4 + 2 * jt + c);
       P[jt][c] = m0 ? P[jt][c] : 0.f;          X[jt][c] = m0 ? X[jt][c] : 0.f;
       P[jt][2 + c] = m1 ? P[jt][2 + c] : 0.f;  X[jt][2 + c] = m1 ? X[jt][2 + c] : 0.f;
       rs0 += P[jt][c];
@@ -411,7 +466,8 @@ __device__ __forceinline__ void bwd_quad_tile(const RingView& kv, const RingView
     }
   rs0 += __shfl_xor_sync(0xffffffffu, rs0, 1); rs0 += __shfl_xor_sync(0xffffffffu, rs0, 2);
   rs1 += __shfl_xor_sync(0xffffffffu, rs1, 1); rs1 += __shfl_xor_sync(0xffffffffu, rs1, 2);
-  const float inv0 = (g < nvalid) ? fast_rcp(rs0) : 0.f, inv1 = (g + 8 < nvalid) ? fast_rcp(rs1) : 0.f;
+  const float inv0 = (g < nvalid) ? fast_rcp(PHI ? rs0 + eps : rs0) : 0.f;
+  const float inv1 = (g + 8 < nvalid) ? fast_rcp(PHI ? rs1 + eps : rs1) : 0.f;
   float go0 = 0.f, go1 = 0.f;                 // g_i . o_i = sum_j W_ij X_ij
 #pragma unroll
   for (int jt = 0; jt < 2; ++jt)
@@ -426,10 +482,27 @@ __device__ __forceinline__ void bwd_quad_tile(const RingView& kv, const RingView
 #pragma unroll
   for (int jt = 0; jt < 2; ++jt)
 #pragma unroll
-    for (int c = 0; c < 2; ++c) {               // dP (zero where W is zero: masked pairs)
-      X[jt][c] = (P[jt][c] != 0.f) ? (X[jt][c] - go0) * inv0 : 0.f;
-      X[jt][2 + c] = (P[jt][2 + c] != 0.f) ? (X[jt][2 + c] - go1) * inv1 : 0.f;
+    for (int c = 0; c < 2; ++c) {               // dP, zero on masked pairs (a ReLU weight can be 0 on an unmasked one)
+      X[jt][c] = ((same >> (2 * jt + c)) & 1u) ? (X[jt][c] - go0) * inv0 : 0.f;
+      X[jt][2 + c] = ((same >> (4 + 2 * jt + c)) & 1u) ? (X[jt][2 + c] - go1) * inv1 : 0.f;
     }
+  // ReLU: a row whose weights sum to almost eps alone has dP of the order 1/eps; rescale the tile by a power of two
+  float pmax = 0.f;
+  if (PHI) {
+#pragma unroll
+    for (int jt = 0; jt < 2; ++jt)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) pmax = fmaxf(pmax, fabsf(X[jt][c]));
+  }
+  const int ksh = tile_shift<PHI>(pmax);
+  const float up = pow2f(ksh);
+  if (PHI) {
+    const float dn = pow2f(-ksh);
+#pragma unroll
+    for (int jt = 0; jt < 2; ++jt)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) X[jt][c] = sat_h<PHI>(X[jt][c] * dn);
+  }
   // A operands (k = j) of W and dP, and their transposes (m = j, k = i) by 8x8 block transposes
   uint32_t wh[4], wl[4], ph[4], pl[4], wth[4], wtl[4], pth[4], ptl[4];
 #pragma unroll
@@ -456,6 +529,10 @@ __device__ __forceinline__ void bwd_quad_tile(const RingView& kv, const RingView
     // da (rows i, cols p): A = dP, B = b over rows j ; db (rows j, cols p): A = dP^T, B = a over rows i
     mma3<true>(da, ph, pl, bth[nt], bth[2 + nt], btl[nt], btl[2 + nt]);
     mma3<true>(db, pth, ptl, ath[nt], ath[2 + nt], atl[nt], atl[2 + nt]);
+    if (PHI) {
+#pragma unroll
+      for (int c = 0; c < 4; ++c) { da[c] *= up; db[c] *= up; }
+    }
     // derivative factors at (row g / g+8, channels 8 nt + 2t..): ldmatrix blocks (rowhalf, chalf = nt) = index 2*rowhalf + nt
     const size_t o0 = (size_t)g * C_total + 8 * nt + 2 * t, o1 = (size_t)(g + 8) * C_total + 8 * nt + 2 * t;
     if (g < nvalid) {
@@ -472,22 +549,26 @@ __device__ __forceinline__ void bwd_quad_tile(const RingView& kv, const RingView
 }
 
 // ---- one whole window: the three passes -------------------------------------------------------------
-template <bool BF16, bool PRECISE, typename T>
+template <int MODE, bool PRECISE, typename T>
 __device__ __forceinline__ void bwd_window(RingView& kv, RingView& qg, RingView& kv2, int hl, int S0, int s,
                                            int e, T* __restrict__ dq_head, T* __restrict__ dk_head,
-                                           T* __restrict__ dv_head, int Ctot) {
+                                           T* __restrict__ dv_head, int Ctot, float eps) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   BwdState st;
   st.clear();
   for (int r = s; r < e; r += 16) {
     const int nv = min(16, e - r), rel = r - S0;
     ring_release_below<C::SR>(kv, rel);
     ring_wait_upto(kv, (rel + nv - 1) / C::SR);
-    bwd_kv_tile<BF16, PRECISE>(kv, hl, rel, nv, st);
+    bwd_kv_tile<MODE, PRECISE>(kv, hl, rel, nv, st);
   }
   const int m = e - s;
   const int lg = 32 - __clz(m - 1);
   const float scale = __int_as_float((127 - lg) << 23);   // s = 2^-ceil(log2 m)
   PassBOps ob;
+  ob.eps = eps * scale;
   make_ops<PRECISE>(st.ST, scale, ob.num);
   make_ops<PRECISE>(st.SS, scale, ob.da);
 #pragma unroll
@@ -499,7 +580,7 @@ __device__ __forceinline__ void bwd_window(RingView& kv, RingView& qg, RingView&
     const int nv = min(16, e - r), rel = r - S0;
     ring_release_below<C::SR>(qg, rel);
     ring_wait_upto(qg, (rel + nv - 1) / C::SR);
-    bwd_q_tile<BF16, PRECISE, T>(qg, hl, rel, nv, ob, st, dq_head + (size_t)r * Ctot, Ctot);
+    bwd_q_tile<MODE, PRECISE, T>(qg, hl, rel, nv, ob, st, dq_head + (size_t)r * Ctot, Ctot);
   }
   PassCOps oc;
   make_ops<PRECISE>(st.dST, scale, oc.dv);
@@ -510,7 +591,7 @@ __device__ __forceinline__ void bwd_window(RingView& kv, RingView& qg, RingView&
     const int nv = min(16, e - r), rel = r - S0;
     ring_release_below<C::SR>(kv2, rel);
     ring_wait_upto(kv2, (rel + nv - 1) / C::SR);
-    bwd_kv_out_tile<BF16, PRECISE, T>(kv2, hl, rel, nv, oc, dk_head + (size_t)r * Ctot,
+    bwd_kv_out_tile<MODE, PRECISE, T>(kv2, hl, rel, nv, oc, dk_head + (size_t)r * Ctot,
                                       dv_head + (size_t)r * Ctot, Ctot);
   }
 }
@@ -520,12 +601,15 @@ struct Ctrl {
   int wa, stream_begin, stream_end;
 };
 
-template <bool BF16, typename T>
+template <int MODE, typename T>
 __global__ void __launch_bounds__(Cfg<D>::THREADS, 2)
 sla_bwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                   const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmG,
                   const int32_t* __restrict__ off, T* __restrict__ dq, T* __restrict__ dk,
-                  T* __restrict__ dv, float* __restrict__ ws, int N, int W, int H, int span) {
+                  T* __restrict__ dv, float* __restrict__ ws, int N, int W, int H, int span, float eps) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   extern __shared__ uint8_t dyn_smem[];
   __shared__ Ctrl ctrl;
   // programmatic dependent launch, as the forward: resident behind the previous kernel's tail, barrier set-up runs
@@ -651,17 +735,17 @@ sla_bwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
       ring_release_below<C::SR>(qg, rel);
       ring_wait_upto(kv, (rel + rows - 1) / C::SR);
       ring_wait_upto(qg, (rel + rows - 1) / C::SR);
-      bwd_quad_tile<BF16, T>(kv, qg, hl, rel, rows, wid, dq + hcol + (size_t)s * Ctot, dk + hcol + (size_t)s * Ctot,
-                             dv + hcol + (size_t)s * Ctot, Ctot);
+      bwd_quad_tile<MODE, T>(kv, qg, hl, rel, rows, wid, dq + hcol + (size_t)s * Ctot, dk + hcol + (size_t)s * Ctot,
+                             dv + hcol + (size_t)s * Ctot, Ctot, eps);
       ring_release_below<C::SR>(kv, rel + rows);
       ring_release_below<C::SR>(qg, rel + rows);
       ring_release_below<C::SR>(kv2, rel + rows);                 // the third stream carries these rows too
       continue;
     }
     if (m <= BWD_PRECISE_MAX)
-      bwd_window<BF16, true, T>(kv, qg, kv2, hl, S0, s, e, dq + hcol, dk + hcol, dv + hcol, Ctot);
+      bwd_window<MODE, true, T>(kv, qg, kv2, hl, S0, s, e, dq + hcol, dk + hcol, dv + hcol, Ctot, eps);
     else
-      bwd_window<BF16, false, T>(kv, qg, kv2, hl, S0, s, e, dq + hcol, dk + hcol, dv + hcol, Ctot);
+      bwd_window<MODE, false, T>(kv, qg, kv2, hl, S0, s, e, dq + hcol, dk + hcol, dv + hcol, Ctot, eps);
     ++w;
   }
   ring_release_below<C::SR>(kv, total * C::SR);
@@ -678,11 +762,14 @@ __device__ __forceinline__ float* split_slot(float* ws, int s, int H, int h) {
   return ws + kWsHeaderFloats + ((size_t)(s / (kFuseMax + 1)) * H + h) * (size_t)((D + 1) * D);
 }
 
-template <bool BF16, typename T, int PASS>
+template <int MODE, typename T, int PASS>
 __global__ void __launch_bounds__(Cfg<D>::THREADS, 2)
 sla_bwd_tc_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                         const int32_t* __restrict__ off, T* __restrict__ dq, T* __restrict__ dk, T* __restrict__ dv,
-                        float* __restrict__ ws, float* __restrict__ wd, int N, int W, int H, int span) {
+                        float* __restrict__ ws, float* __restrict__ wd, int N, int W, int H, int span, float eps) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   extern __shared__ uint8_t dyn_smem[];
   __shared__ Ctrl ctrl;
   asm volatile("griddepcontrol.launch_dependents;");
@@ -765,7 +852,7 @@ sla_bwd_tc_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_co
         const int nv = min(16, pe - r), rel = r - S0;
         ring_release_below<C::SR>(rv, rel);
         ring_wait_upto(rv, (rel + nv - 1) / C::SR);
-        bwd_kv_tile<BF16, false>(rv, hl, rel, nv, st);
+        bwd_kv_tile<MODE, false>(rv, hl, rel, nv, st);
       }
 #pragma unroll
       for (int nt = 0; nt < 2; ++nt)
@@ -788,6 +875,7 @@ sla_bwd_tc_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_co
           st.Z[nt][c] = slot[D * D + 8 * nt + 2 * t + (c & 1)];
         }
       PassBOps ob;
+      ob.eps = eps * scale;
       make_ops<false>(st.ST, scale, ob.num);
       make_ops<false>(st.SS, scale, ob.da);
 #pragma unroll
@@ -799,7 +887,7 @@ sla_bwd_tc_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_co
         const int nv = min(16, pe - r), rel = r - S0;
         ring_release_below<C::SR>(rv, rel);
         ring_wait_upto(rv, (rel + nv - 1) / C::SR);
-        bwd_q_tile<BF16, false, T>(rv, hl, rel, nv, ob, st, dq + hcol + (size_t)r * Ctot, Ctot);
+        bwd_q_tile<MODE, false, T>(rv, hl, rel, nv, ob, st, dq + hcol + (size_t)r * Ctot, Ctot);
       }
 #pragma unroll
       for (int nt = 0; nt < 2; ++nt)
@@ -830,7 +918,7 @@ sla_bwd_tc_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_co
         const int nv = min(16, pe - r), rel = r - S0;
         ring_release_below<C::SR>(rv, rel);
         ring_wait_upto(rv, (rel + nv - 1) / C::SR);
-        bwd_kv_out_tile<BF16, false, T>(rv, hl, rel, nv, oc, dk + hcol + (size_t)r * Ctot,
+        bwd_kv_out_tile<MODE, false, T>(rv, hl, rel, nv, oc, dk + hcol + (size_t)r * Ctot,
                                         dv + hcol + (size_t)r * Ctot, Ctot);
       }
     }
@@ -838,14 +926,17 @@ sla_bwd_tc_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_co
   ring_release_below<C::SR>(rv, total * C::SR);
 }
 
-template <bool BF16, typename T>
+template <int MODE, typename T>
 cudaError_t bwd_tc_launch(const Problem& p, cudaStream_t st) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   CUtensorMap tq, tk, tv, tg;
   const int Ctot = p.H * D;
   if (!make_map(&tq, p.q, p.N, Ctot, C::SR) || !make_map(&tk, p.k, p.N, Ctot, C::SR) ||
       !make_map(&tv, p.v, p.N, Ctot, C::SR) || !make_map(&tg, p.g, p.N, Ctot, C::SR))
     return cudaErrorInvalidValue;
-  auto kern = sla_bwd_tc_kernel<BF16, T>;
+  auto kern = sla_bwd_tc_kernel<MODE, T>;
   static std::atomic<bool> attr_set[kMaxDevices];         // the smem opt-in is per device
   const int dev = current_device();
   if (!attr_set[dev].load(std::memory_order_acquire)) {
@@ -870,12 +961,12 @@ cudaError_t bwd_tc_launch(const Problem& p, cudaStream_t st) {
   cfg.attrs = pdl;
   cfg.numAttrs = 1;
   cudaError_t le = cudaLaunchKernelEx(&cfg, kern, tq, tk, tv, tg, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state,
-                                      p.N, p.W, p.H, span);
+                                      p.N, p.W, p.H, span, p.eps);
   if (le != cudaSuccess || p.bounded) return le;   // bounded entry: no window is left to the split passes
   // windows longer than kFuseMax rows: three passes over their pieces (each exits at once if there is none)
-  auto k0 = sla_bwd_tc_split_kernel<BF16, T, 0>;
-  auto k1 = sla_bwd_tc_split_kernel<BF16, T, 1>;
-  auto k2 = sla_bwd_tc_split_kernel<BF16, T, 2>;
+  auto k0 = sla_bwd_tc_split_kernel<MODE, T, 0>;
+  auto k1 = sla_bwd_tc_split_kernel<MODE, T, 1>;
+  auto k2 = sla_bwd_tc_split_kernel<MODE, T, 2>;
   static std::atomic<bool> attr2_set[kMaxDevices];
   if (!attr2_set[dev].load(std::memory_order_acquire)) {
     cudaError_t e = cudaFuncSetAttribute(k0, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_DYN);
@@ -887,13 +978,13 @@ cudaError_t bwd_tc_launch(const Problem& p, cudaStream_t st) {
   const int span2 = 128;                                   // <= kFuseMax; few pieces per window = few atomics per slot
   cfg.gridDim = dim3((p.N + span2 - 1) / span2, slabs);
   le = cudaLaunchKernelEx(&cfg, k0, tk, tv, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state, p.ws_dstate, p.N, p.W,
-                          p.H, span2);
+                          p.H, span2, p.eps);
   if (le == cudaSuccess)
     le = cudaLaunchKernelEx(&cfg, k1, tq, tg, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state, p.ws_dstate, p.N, p.W,
-                            p.H, span2);
+                            p.H, span2, p.eps);
   if (le == cudaSuccess)
     le = cudaLaunchKernelEx(&cfg, k2, tk, tv, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state, p.ws_dstate, p.N, p.W,
-                            p.H, span2);
+                            p.H, span2, p.eps);
   return le;
 }
 
@@ -902,7 +993,6 @@ cudaError_t bwd_tc_launch(const Problem& p, cudaStream_t st) {
 bool backward_tc_supported(const Problem& p, int dt) {
   if (dt != SLA_F16 && dt != SLA_BF16) return false;
   if ((p.d != 16 && p.d != 32) || (p.H * p.d) % 64 != 0) return false;     // d_h = 32: sla_bwd_tc32.cu
-  if (p.phi != SLA_PHI_ELU1) return false;                     // the ReLU map's backward runs on the generic kernels
   return encode_fn() != nullptr;
 }
 
@@ -910,7 +1000,10 @@ bool backward_tc_supported(const Problem& p, int dt) {
 // (they exit at once unless the first kernel raised the workspace flag).
 cudaError_t launch_backward_tc(const Problem& p, int dt, cudaStream_t st) {
   if (p.d == 32) return launch_backward_tc32(p, dt, st);
-  return (dt == SLA_F16) ? bwd_tc_launch<false, __half>(p, st) : bwd_tc_launch<true, __nv_bfloat16>(p, st);
+  // MODE = (bf16 ? 1 : 0) | (feature map << 1)
+  const bool relu = p.phi == SLA_PHI_RELU;
+  if (dt == SLA_F16) return relu ? bwd_tc_launch<2, __half>(p, st) : bwd_tc_launch<0, __half>(p, st);
+  return relu ? bwd_tc_launch<3, __nv_bfloat16>(p, st) : bwd_tc_launch<1, __nv_bfloat16>(p, st);
 }
 
 }  // namespace sla

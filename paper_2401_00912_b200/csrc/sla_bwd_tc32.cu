@@ -1,4 +1,4 @@
-// sla_bwd_tc32.cu -- SLA backward for fp16 / bf16 I/O, d_h = 32, phi = elu+1, on the tensor cores.
+// sla_bwd_tc32.cu -- SLA backward for fp16 / bf16 I/O, d_h = 32, both feature maps, on the tensor cores.
 //
 // The d_h = 16 kernel (sla_bwd_tc.cu) written out for a head of KS = d_h/16 column groups: the same skeleton
 // (equal row spans per CTA, three TMA + mbarrier rings, one consumer warp per head, mma.sync m16n8k16 with fp32
@@ -90,12 +90,20 @@ __device__ __forceinline__ void make_ops(const float (&X)[KS][NT][4], float scal
                        o.hi[n][ks][b], o.lo[n][ks][b]);
 }
 
-// phi of a packed pair in fp32 (a) and its derivative factor (x > 0 ? 1 : phi(x))
-template <bool BF16>
+// phi of a packed pair in fp32 (a) and its derivative factor: elu+1: (x > 0 ? 1 : phi(x)); ReLU: [x > 0]
+template <int MODE>
 __device__ __forceinline__ void phi_pair(uint32_t raw, float2& a, float2& da) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   const float2 x = unpack2<BF16>(raw);
-  da.x = dphi_fast(x.x); da.y = dphi_fast(x.y);
-  a.x = fmaxf(x.x, 0.f) + da.x; a.y = fmaxf(x.y, 0.f) + da.y;
+  if (PHI) {   // max(x, 0): phi' = [x > 0]
+    da.x = x.x > 0.f ? 1.f : 0.f; da.y = x.y > 0.f ? 1.f : 0.f;
+    a.x = fmaxf(x.x, 0.f); a.y = fmaxf(x.y, 0.f);
+  } else {
+    da.x = dphi_fast(x.x); da.y = dphi_fast(x.y);
+    a.x = fmaxf(x.x, 0.f) + da.x; a.y = fmaxf(x.y, 0.f) + da.y;
+  }
 }
 // a (hi,lo) x b (hi,lo): 1 term, or the 3 leading terms
 template <bool PRECISE>
@@ -107,6 +115,26 @@ __device__ __forceinline__ void mma3(float (&c)[4], const uint32_t (&ah)[4], con
     mma16816(c, ah[0], ah[1], ah[2], ah[3], bl0, bl1);
   }
 }
+
+// ReLU map only: with max(x, 0) a row's denominator can be eps alone, and g/den, dden reach 1/eps.  Every product that
+// survives in the result then meets a zero factor (phi or phi' vanishes wherever the row's a.b did), so such
+// intermediates only have to stay finite as fp16 operands: clamp them instead of letting them overflow to inf (0 * inf).
+template <int PHI>
+__device__ __forceinline__ float sat_h(float x) { return PHI ? fminf(fmaxf(x, -60000.f), 60000.f) : x; }
+
+// ReLU map only: power-of-two rescaling of a tile's large intermediates.  `mx` = this lane's largest magnitude; returns k
+// such that the warp-wide maximum times 2^-k is below 2^15 (k = 0 for the elu+1 map and for ordinary tiles), at most
+// 10 so that the partner operand, phi(q) * 2^k, stays inside fp16.  The operand that carries 1/den is multiplied by
+// 2^-k and its partner (or the fresh accumulator) by 2^k: exact.  What is still above fp16 after that belongs to rows
+// whose denominator is eps alone (sat_h above).
+template <int PHI>
+__device__ __forceinline__ int tile_shift(float mx) {
+  if (!PHI) return 0;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  return min(10, max(0, (int)((__float_as_uint(mx) >> 23) & 0xffu) - 127 - 14));
+}
+__device__ __forceinline__ float pow2f(int k) { return __uint_as_float((uint32_t)(127 + k) << 23); }
 
 // lane -> (tile row, 16-byte chunk select) for the x4 ldmatrix pattern
 //   registers: (rows0-7,c0), (rows0-7,c1), (rows8-15,c0), (rows8-15,c1)
@@ -120,8 +148,11 @@ __device__ __forceinline__ void lane_pattern(int nvalid, int& trow, int& csel) {
 __device__ __forceinline__ int head_chunk(int hl, int ks, int csel) { return hl * (D / 8) + 2 * ks + csel; }
 
 // ---- pass A: one 16-row K/V tile -> S^T, S, z -------------------------------------------------------
-template <bool BF16, bool PRECISE>
+template <int MODE, bool PRECISE>
 __device__ __forceinline__ void bwd_kv_tile(const RingView& rv, int hl, int rel0, int nvalid, BwdState& s) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   const int t = threadIdx.x & 3;
   int trow, csel;
   lane_pattern(nvalid, trow, csel);
@@ -137,11 +168,11 @@ __device__ __forceinline__ void bwd_kv_tile(const RingView& rv, int hl, int rel0
       const int j0 = 2 * t + 8 * (i >> 1);
       if (PRECISE) {
         const float2 x = unpack2<BF16>(kr[i]);
-        const float b0 = (j0 < nvalid) ? phi_fast(x.x) : 0.f;
-        const float b1 = (j0 + 1 < nvalid) ? phi_fast(x.y) : 0.f;
+        const float b0 = (j0 < nvalid) ? phi_fast<PHI>(x.x) : 0.f;
+        const float b1 = (j0 + 1 < nvalid) ? phi_fast<PHI>(x.y) : 0.f;
         to_op<true>(b0, b1, bh[ks][i], bl[ks][i]);
       } else {   // long window: phi in fp16x2 (the operand is a single fp16 anyway), rows beyond the window zeroed
-        bh[ks][i] = phi_h2<BF16>(kr[i]);
+        bh[ks][i] = phi_h2<BF16, PHI>(kr[i]);
         if (nvalid < 16) bh[ks][i] &= pair_mask(j0, nvalid);
         bl[ks][i] = 0u;
       }
@@ -176,13 +207,17 @@ struct PassBOps {
   Ops da;                    // from S  : B operand of da = dnum S^T
   uint32_t zh[KS][2], zl[KS][2];   // z as B operand of den
   float zs[NT][2];           // scaled z in columns p = 8 np + 2t + c
+  float eps;                 // epsilon of the denominator on the scale of the operands (eps * s); 0 for elu+1
 };
 
 // ---- pass B: one 16-row Q/dO tile -> dq rows, dS^T, dS, dz accumulators ------------------------------
-template <bool BF16, bool PRECISE, typename T>
+template <int MODE, bool PRECISE, typename T>
 __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0, int nvalid,
                                            const PassBOps& op, BwdState& s, T* __restrict__ dq_rows,
                                            int C_total) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   int trow, csel;
   lane_pattern(nvalid, trow, csel);
@@ -199,10 +234,10 @@ __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0,
     for (int i = 0; i < 4; ++i) {
       if (PRECISE) {
         float2 a;
-        phi_pair<BF16>(qn[perm[i]], a, dph[ks][i]);
+        phi_pair<MODE>(qn[perm[i]], a, dph[ks][i]);
         to_op<true>(a.x, a.y, ah[ks][i], al[ks][i]);
       } else {
-        phi_dphi_h2<BF16>(qn[perm[i]], ah[ks][i], dph2[ks][i]);
+        phi_dphi_h2<BF16, PHI>(qn[perm[i]], ah[ks][i], dph2[ks][i]);
         al[ks][i] = 0u;
       }
       graw[ks][i] = gn[perm[i]];
@@ -220,7 +255,7 @@ __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0,
     for (int ks = 0; ks < KS; ++ks)
       mma3<PRECISE>(num[n], ah[ks], al[ks], op.num.hi[n][ks][0], op.num.hi[n][ks][1], op.num.lo[n][ks][0], op.num.lo[n][ks][1]);
   }
-  const float inv0 = fast_rcp(den[0]), inv1 = fast_rcp(den[2]);       // rows g, g+8
+  const float inv0 = fast_rcp(PHI ? den[0] + op.eps : den[0]), inv1 = fast_rcp(PHI ? den[2] + op.eps : den[2]);   // rows g, g+8
   // g.o per row: this lane holds columns 8n + 2t, +1 of rows g and g+8 for every tile n
   float go0 = 0.f, go1 = 0.f;
 #pragma unroll
@@ -232,14 +267,27 @@ __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0,
   go0 += __shfl_xor_sync(0xffffffffu, go0, 1); go0 += __shfl_xor_sync(0xffffffffu, go0, 2);
   go1 += __shfl_xor_sync(0xffffffffu, go1, 1); go1 += __shfl_xor_sync(0xffffffffu, go1, 2);
   const float dden0 = -(go0 * inv0) * inv0, dden1 = -(go1 * inv1) * inv1;   // o = num*inv
+  // ReLU: rows whose denominator is almost eps alone make g/den and dden huge; rescale the tile by a power of two
+  float gmax = 0.f;
+  if (PHI) {
+#pragma unroll
+    for (int ks = 0; ks < KS; ++ks)
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+        gmax = fmaxf(gmax, fmaxf(fabsf(gv[ks][i].x), fabsf(gv[ks][i].y)) * ((i & 1) ? inv1 : inv0));
+    gmax = fmaxf(gmax, fmaxf(fabsf(dden0), fabsf(dden1)));
+  }
+  const int ksh = tile_shift<PHI>(gmax);
+  const float dn = pow2f(-ksh), up = pow2f(ksh);        // both 1 unless ReLU and an ill-conditioned row
   // dnum as A fragments (rows g / g+8 scaled by their 1/den)
   uint32_t dh[KS][4], dl[KS][4];
 #pragma unroll
   for (int ks = 0; ks < KS; ++ks)
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-      const float iv = (i & 1) ? inv1 : inv0;
-      if (PRECISE || BF16) to_op<PRECISE>(gv[ks][i].x * iv, gv[ks][i].y * iv, dh[ks][i], dl[ks][i]);
+      const float iv = ((i & 1) ? inv1 : inv0) * dn;
+      if (PRECISE || BF16 || PHI)
+        to_op<PRECISE>(sat_h<PHI>(gv[ks][i].x * iv), sat_h<PHI>(gv[ks][i].y * iv), dh[ks][i], dl[ks][i]);
       else { dh[ks][i] = hmul2_u32(graw[ks][i], pack_h2(iv, iv)); dl[ks][i] = 0u; }
     }
   // da = dnum S^T + dden z ; dq = da * phi'(q)
@@ -250,6 +298,7 @@ __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0,
     for (int ks = 0; ks < KS; ++ks)
       mma3<PRECISE>(da, dh[ks], dl[ks], op.da.hi[np][ks][0], op.da.hi[np][ks][1], op.da.lo[np][ks][0], op.da.lo[np][ks][1]);
     // C fragment (np): c0,c1 = (row g, p = 8np+2t,+1) <-> A index 2 (np%2) of group np/2 ; c2,c3 = row g+8 <-> A index + 1
+    if (PHI) { da[0] *= up; da[1] *= up; da[2] *= up; da[3] *= up; }
     const float q0 = da[0] + dden0 * op.zs[np][0], q1 = da[1] + dden0 * op.zs[np][1];
     const float q2 = da[2] + dden1 * op.zs[np][0], q3 = da[3] + dden1 * op.zs[np][1];
     uint32_t* p0 = reinterpret_cast<uint32_t*>(dq_rows + (size_t)g * C_total + 8 * np + 2 * t);
@@ -259,8 +308,8 @@ __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0,
       if (g < nvalid) *p0 = pack_out<BF16>(q0 * dph[kg][ai].x, q1 * dph[kg][ai].y);
       if (g + 8 < nvalid) *p1 = pack_out<BF16>(q2 * dph[kg][ai + 1].x, q3 * dph[kg][ai + 1].y);
     } else {
-      if (g < nvalid) *p0 = pack_out_times_h2<BF16>(q0, q1, dph2[kg][ai]);
-      if (g + 8 < nvalid) *p1 = pack_out_times_h2<BF16>(q2, q3, dph2[kg][ai + 1]);
+      if (g < nvalid) *p0 = pack_out_times_h2<BF16, PHI != 0>(q0, q1, dph2[kg][ai]);
+      if (g + 8 < nvalid) *p1 = pack_out_times_h2<BF16, PHI != 0>(q2, q3, dph2[kg][ai + 1]);
     }
   }
   // ---- transposed operands (contraction over the rows i of the tile) ----
@@ -280,20 +329,21 @@ __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0,
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
       const int i0 = 2 * t + 8 * (i >> 1);
-      const float s0 = (i >> 1) ? ir2 : ir0, s1 = (i >> 1) ? ir3 : ir1;
+      const float s0 = ((i >> 1) ? ir2 : ir0) * dn, s1 = ((i >> 1) ? ir3 : ir1) * dn;   // dn = 1 unless ReLU
       if (PRECISE) {
         const float2 x = unpack2<BF16>(qt[i]);
-        const float a0 = (i0 < nvalid) ? phi_fast(x.x) : 0.f;       // rows beyond the window contribute nothing
-        const float a1 = (i0 + 1 < nvalid) ? phi_fast(x.y) : 0.f;
-        to_op<true>(a0, a1, uh[ks][i], ul[ks][i]);
+        const float a0 = (i0 < nvalid) ? phi_fast<PHI>(x.x) : 0.f;       // rows beyond the window contribute nothing
+        const float a1 = (i0 + 1 < nvalid) ? phi_fast<PHI>(x.y) : 0.f;
+        to_op<true>(sat_h<PHI>(a0 * up), sat_h<PHI>(a1 * up), uh[ks][i], ul[ks][i]);
       } else {
-        uh[ks][i] = phi_h2<BF16>(qt[i]);
+        uh[ks][i] = phi_h2<BF16, PHI>(qt[i]);
         if (nvalid < 16) uh[ks][i] &= pair_mask(i0, nvalid);
+        if (PHI) uh[ks][i] = hmul2_u32(uh[ks][i], pack_h2(up, up));
         ul[ks][i] = 0u;
       }
-      if (PRECISE || BF16) {
+      if (PRECISE || BF16 || PHI) {
         const float2 gg = unpack2<BF16>(gt[i]);
-        to_op<PRECISE>(gg.x * s0, gg.y * s1, th[ks][i], tl[ks][i]);
+        to_op<PRECISE>(sat_h<PHI>(gg.x * s0), sat_h<PHI>(gg.y * s1), th[ks][i], tl[ks][i]);
       } else {
         th[ks][i] = hmul2_u32(gt[i], pack_h2(s0, s1));
         tl[ks][i] = 0u;
@@ -301,8 +351,8 @@ __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0,
     }
   }
   uint32_t ddh[2], ddl[2];
-  to_op<PRECISE>(dd0, dd1, ddh[0], ddl[0]);
-  to_op<PRECISE>(dd2, dd3, ddh[1], ddl[1]);
+  to_op<PRECISE>(sat_h<PHI>(dd0 * dn), sat_h<PHI>(dd1 * dn), ddh[0], ddl[0]);
+  to_op<PRECISE>(sat_h<PHI>(dd2 * dn), sat_h<PHI>(dd3 * dn), ddh[1], ddl[1]);
   const uint32_t dda_h[4] = {ddh[0], ddh[0], ddh[1], ddh[1]}, dda_l[4] = {ddl[0], ddl[0], ddl[1], ddl[1]};
 #pragma unroll
   for (int nt = 0; nt < NT; ++nt) {
@@ -326,10 +376,13 @@ struct PassCOps {
 };
 
 // ---- pass C: one 16-row K/V tile -> dk, dv rows ------------------------------------------------------
-template <bool BF16, bool PRECISE, typename T>
+template <int MODE, bool PRECISE, typename T>
 __device__ __forceinline__ void bwd_kv_out_tile(const RingView& rv, int hl, int rel0, int nvalid,
                                                 const PassCOps& op, T* __restrict__ dk_rows,
                                                 T* __restrict__ dv_rows, int C_total) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
   int trow, csel;
   lane_pattern(nvalid, trow, csel);
@@ -345,10 +398,10 @@ __device__ __forceinline__ void bwd_kv_out_tile(const RingView& rv, int hl, int 
     for (int i = 0; i < 4; ++i) {
       if (PRECISE) {
         float2 b;
-        phi_pair<BF16>(kn[perm[i]], b, dph[ks][i]);
+        phi_pair<MODE>(kn[perm[i]], b, dph[ks][i]);
         to_op<true>(b.x, b.y, bh[ks][i], bl[ks][i]);
       } else {
-        phi_dphi_h2<BF16>(kn[perm[i]], bh[ks][i], dph2[ks][i]);
+        phi_dphi_h2<BF16, PHI>(kn[perm[i]], bh[ks][i], dph2[ks][i]);
         bl[ks][i] = 0u;
       }
       if (BF16) { const float2 x = unpack2<true>(vn[perm[i]]); vh[ks][i] = pack_h2(x.x, x.y); }
@@ -372,19 +425,20 @@ __device__ __forceinline__ void bwd_kv_out_tile(const RingView& rv, int hl, int 
     if (g < nvalid) {
       *reinterpret_cast<uint32_t*>(dv_rows + o0) = pack_out<BF16>(dv[0], dv[1]);
       *reinterpret_cast<uint32_t*>(dk_rows + o0) = PRECISE ? pack_out<BF16>(k0 * dph[kg][ai].x, k1 * dph[kg][ai].y)
-                                                           : pack_out_times_h2<BF16>(k0, k1, dph2[kg][ai]);
+                                                           : pack_out_times_h2<BF16, PHI != 0>(k0, k1, dph2[kg][ai]);
     }
     if (g + 8 < nvalid) {
       *reinterpret_cast<uint32_t*>(dv_rows + o1) = pack_out<BF16>(dv[2], dv[3]);
       *reinterpret_cast<uint32_t*>(dk_rows + o1) = PRECISE ? pack_out<BF16>(k2 * dph[kg][ai + 1].x, k3 * dph[kg][ai + 1].y)
-                                                           : pack_out_times_h2<BF16>(k2, k3, dph2[kg][ai + 1]);
+                                                           : pack_out_times_h2<BF16, PHI != 0>(k2, k3, dph2[kg][ai + 1]);
     }
   }
 }
 
 // operands of pass B from the complete state, and of pass C from the complete dS, dz (both on the window's scale)
 template <bool PRECISE>
-__device__ __forceinline__ void make_pass_b_ops(const BwdState& st, float scale, PassBOps& ob) {
+__device__ __forceinline__ void make_pass_b_ops(const BwdState& st, float scale, float eps, PassBOps& ob) {
+  ob.eps = eps * scale;
   make_ops<PRECISE>(st.ST, scale, ob.num);
   make_ops<PRECISE>(st.SS, scale, ob.da);
 #pragma unroll
@@ -404,29 +458,32 @@ __device__ __forceinline__ void make_pass_c_ops(const BwdState& st, float scale,
 }
 
 // ---- one whole window: the three passes -------------------------------------------------------------
-template <bool BF16, bool PRECISE, typename T>
+template <int MODE, bool PRECISE, typename T>
 __device__ __forceinline__ void bwd_window(RingView& kv, RingView& qg, RingView& kv2, int hl, int S0, int s,
                                         int e, T* __restrict__ dq_head, T* __restrict__ dk_head,
-                                        T* __restrict__ dv_head, int Ctot) {
+                                        T* __restrict__ dv_head, int Ctot, float eps) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   BwdState st;
   st.clear();
   for (int r = s; r < e; r += 16) {
     const int nv = min(16, e - r), rel = r - S0;
     ring_release_below<C::SR>(kv, rel);
     ring_wait_upto(kv, (rel + nv - 1) / C::SR);
-    bwd_kv_tile<BF16, PRECISE>(kv, hl, rel, nv, st);
+    bwd_kv_tile<MODE, PRECISE>(kv, hl, rel, nv, st);
   }
   const int m = e - s;
   const int lg = 32 - __clz(m - 1);
   const float scale = __int_as_float((127 - lg) << 23);   // s = 2^-ceil(log2 m)
   {
     PassBOps ob;
-    make_pass_b_ops<PRECISE>(st, scale, ob);
+    make_pass_b_ops<PRECISE>(st, scale, eps, ob);
     for (int r = s; r < e; r += 16) {
       const int nv = min(16, e - r), rel = r - S0;
       ring_release_below<C::SR>(qg, rel);
       ring_wait_upto(qg, (rel + nv - 1) / C::SR);
-      bwd_q_tile<BF16, PRECISE, T>(qg, hl, rel, nv, ob, st, dq_head + (size_t)r * Ctot, Ctot);
+      bwd_q_tile<MODE, PRECISE, T>(qg, hl, rel, nv, ob, st, dq_head + (size_t)r * Ctot, Ctot);
     }
   }
   PassCOps oc;
@@ -435,7 +492,7 @@ __device__ __forceinline__ void bwd_window(RingView& kv, RingView& qg, RingView&
     const int nv = min(16, e - r), rel = r - S0;
     ring_release_below<C::SR>(kv2, rel);
     ring_wait_upto(kv2, (rel + nv - 1) / C::SR);
-    bwd_kv_out_tile<BF16, PRECISE, T>(kv2, hl, rel, nv, oc, dk_head + (size_t)r * Ctot,
+    bwd_kv_out_tile<MODE, PRECISE, T>(kv2, hl, rel, nv, oc, dk_head + (size_t)r * Ctot,
                                       dv_head + (size_t)r * Ctot, Ctot);
   }
 }
@@ -465,12 +522,15 @@ __device__ __forceinline__ void produce_ring(uint32_t base, uint32_t full, uint3
 }
 
 // Fused windows (<= kFuseMax rows): every CTA owns the windows whose middle row lies in its span.
-template <bool BF16, typename T>
+template <int MODE, typename T>
 __global__ void __launch_bounds__(C::THREADS, 1)
 sla_bwd_tc32_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                     const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmG,
                     const int32_t* __restrict__ off, T* __restrict__ dq, T* __restrict__ dk,
-                    T* __restrict__ dv, float* __restrict__ ws, int N, int W, int H, int span) {
+                    T* __restrict__ dv, float* __restrict__ ws, int N, int W, int H, int span, float eps) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   extern __shared__ uint8_t dyn_smem[];
   __shared__ Ctrl ctrl;
   // programmatic dependent launch: resident behind the previous kernel's tail; the barrier set-up runs ahead,
@@ -548,9 +608,9 @@ sla_bwd_tc32_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_consta
     if (mid >= R1) break;
     if (mid < R0) continue;
     if (m <= BWD_PRECISE_MAX)
-      bwd_window<BF16, true, T>(kv, qg, kv2, hl, S0, s, e, dq + hcol, dk + hcol, dv + hcol, Ctot);
+      bwd_window<MODE, true, T>(kv, qg, kv2, hl, S0, s, e, dq + hcol, dk + hcol, dv + hcol, Ctot, eps);
     else
-      bwd_window<BF16, false, T>(kv, qg, kv2, hl, S0, s, e, dq + hcol, dk + hcol, dv + hcol, Ctot);
+      bwd_window<MODE, false, T>(kv, qg, kv2, hl, S0, s, e, dq + hcol, dk + hcol, dv + hcol, Ctot, eps);
   }
   ring_release_below<C::SR>(kv, total * C::SR);
   ring_release_below<C::SR>(qg, total * C::SR);
@@ -566,11 +626,14 @@ __device__ __forceinline__ float* split_slot(float* ws, int s, int H, int h) {
   return ws + kWsHeaderFloats + ((size_t)(s / (kFuseMax + 1)) * H + h) * (size_t)((D + 1) * D);
 }
 
-template <bool BF16, typename T, int PASS>
+template <int MODE, typename T, int PASS>
 __global__ void __launch_bounds__(C::THREADS, 1)
 sla_bwd_tc32_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                           const int32_t* __restrict__ off, T* __restrict__ dq, T* __restrict__ dk, T* __restrict__ dv,
-                          float* __restrict__ ws, float* __restrict__ wd, int N, int W, int H, int span) {
+                          float* __restrict__ ws, float* __restrict__ wd, int N, int W, int H, int span, float eps) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   extern __shared__ uint8_t dyn_smem[];
   __shared__ Ctrl ctrl;
   asm volatile("griddepcontrol.launch_dependents;");
@@ -639,7 +702,7 @@ sla_bwd_tc32_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_
         const int nv = min(16, pe - r), rel = r - S0;
         ring_release_below<C::SR>(rv, rel);
         ring_wait_upto(rv, (rel + nv - 1) / C::SR);
-        bwd_kv_tile<BF16, false>(rv, hl, rel, nv, st);
+        bwd_kv_tile<MODE, false>(rv, hl, rel, nv, st);
       }
 #pragma unroll
       for (int mt = 0; mt < KS; ++mt)
@@ -670,12 +733,12 @@ sla_bwd_tc32_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_
 #pragma unroll
         for (int c = 0; c < 4; ++c) st.Z[nt][c] = slot[D * D + 8 * nt + 2 * t + (c & 1)];
       PassBOps ob;
-      make_pass_b_ops<false>(st, scale, ob);
+      make_pass_b_ops<false>(st, scale, eps, ob);
       for (int r = ps; r < pe; r += 16) {
         const int nv = min(16, pe - r), rel = r - S0;
         ring_release_below<C::SR>(rv, rel);
         ring_wait_upto(rv, (rel + nv - 1) / C::SR);
-        bwd_q_tile<BF16, false, T>(rv, hl, rel, nv, ob, st, dq + hcol + (size_t)r * Ctot, Ctot);
+        bwd_q_tile<MODE, false, T>(rv, hl, rel, nv, ob, st, dq + hcol + (size_t)r * Ctot, Ctot);
       }
 #pragma unroll
       for (int mt = 0; mt < KS; ++mt)
@@ -711,7 +774,7 @@ sla_bwd_tc32_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_
         const int nv = min(16, pe - r), rel = r - S0;
         ring_release_below<C::SR>(rv, rel);
         ring_wait_upto(rv, (rel + nv - 1) / C::SR);
-        bwd_kv_out_tile<BF16, false, T>(rv, hl, rel, nv, oc, dk + hcol + (size_t)r * Ctot,
+        bwd_kv_out_tile<MODE, false, T>(rv, hl, rel, nv, oc, dk + hcol + (size_t)r * Ctot,
                                         dv + hcol + (size_t)r * Ctot, Ctot);
       }
     }
@@ -719,17 +782,20 @@ sla_bwd_tc32_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_
   ring_release_below<C::SR>(rv, total * C::SR);
 }
 
-template <bool BF16, typename T>
+template <int MODE, typename T>
 cudaError_t bwd_tc32_launch(const Problem& p, cudaStream_t st) {
+  constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
+  constexpr int PHI = MODE >> 1;            // feature map (sla_feature_map_t)
+  (void)BF16; (void)PHI;
   CUtensorMap tq, tk, tv, tg;
   const int Ctot = p.H * D;
   if (!make_map(&tq, p.q, p.N, Ctot, C::SR) || !make_map(&tk, p.k, p.N, Ctot, C::SR) ||
       !make_map(&tv, p.v, p.N, Ctot, C::SR) || !make_map(&tg, p.g, p.N, Ctot, C::SR))
     return cudaErrorInvalidValue;
-  auto kern = sla_bwd_tc32_kernel<BF16, T>;
-  auto k0 = sla_bwd_tc32_split_kernel<BF16, T, 0>;
-  auto k1 = sla_bwd_tc32_split_kernel<BF16, T, 1>;
-  auto k2 = sla_bwd_tc32_split_kernel<BF16, T, 2>;
+  auto kern = sla_bwd_tc32_kernel<MODE, T>;
+  auto k0 = sla_bwd_tc32_split_kernel<MODE, T, 0>;
+  auto k1 = sla_bwd_tc32_split_kernel<MODE, T, 1>;
+  auto k2 = sla_bwd_tc32_split_kernel<MODE, T, 2>;
   static std::atomic<bool> attr_set[kMaxDevices];         // the smem opt-in is per device
   const int dev = current_device();
   if (!attr_set[dev].load(std::memory_order_acquire)) {
@@ -757,25 +823,28 @@ cudaError_t bwd_tc32_launch(const Problem& p, cudaStream_t st) {
   cfg.attrs = pdl;
   cfg.numAttrs = 1;
   cudaError_t le = cudaLaunchKernelEx(&cfg, kern, tq, tk, tv, tg, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state,
-                                      p.N, p.W, p.H, span);
+                                      p.N, p.W, p.H, span, p.eps);
   if (le != cudaSuccess || p.bounded) return le;   // bounded entry: no window is left to the split passes
   const int span2 = kFuseMax / 16 * 16;            // the largest span the split passes handle: 33 x 32 atomics per piece and head
   cfg.gridDim = dim3((p.N + span2 - 1) / span2, slabs);
   le = cudaLaunchKernelEx(&cfg, k0, tk, tv, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state, p.ws_dstate, p.N, p.W,
-                          p.H, span2);
+                          p.H, span2, p.eps);
   if (le == cudaSuccess)
     le = cudaLaunchKernelEx(&cfg, k1, tq, tg, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state, p.ws_dstate, p.N, p.W,
-                            p.H, span2);
+                            p.H, span2, p.eps);
   if (le == cudaSuccess)
     le = cudaLaunchKernelEx(&cfg, k2, tk, tv, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state, p.ws_dstate, p.N, p.W,
-                            p.H, span2);
+                            p.H, span2, p.eps);
   return le;
 }
 
 }  // namespace
 
 cudaError_t launch_backward_tc32(const Problem& p, int dt, cudaStream_t st) {
-  return (dt == SLA_F16) ? bwd_tc32_launch<false, __half>(p, st) : bwd_tc32_launch<true, __nv_bfloat16>(p, st);
+  // MODE = (bf16 ? 1 : 0) | (feature map << 1)
+  const bool relu = p.phi == SLA_PHI_RELU;
+  if (dt == SLA_F16) return relu ? bwd_tc32_launch<2, __half>(p, st) : bwd_tc32_launch<0, __half>(p, st);
+  return relu ? bwd_tc32_launch<3, __nv_bfloat16>(p, st) : bwd_tc32_launch<1, __nv_bfloat16>(p, st);
 }
 
 }  // namespace sla

@@ -112,10 +112,16 @@ __device__ __forceinline__ uint32_t phi_h2(uint32_t raw) {
 }
 // elu+1 and its derivative on two packed I/O elements in fp16x2 (the backward's long windows): the same four
 // instructions as phi_h2; 2^t is phi'(x) = (x > 0 ? 1 : e^x) (for x > 0, t is the rounding residual: 1 +- 1.5 ulp).
-template <bool BF16>
+template <bool BF16, int PHI = 0>
 __device__ __forceinline__ void phi_dphi_h2(uint32_t raw, uint32_t& phi, uint32_t& dphi) {
   uint32_t x = raw;
   if (BF16) { float2 f = unpack2<true>(raw); x = pack_h2(f.x, f.y); }
+  if (PHI) {   // max(x, 0) and [x > 0] (1.0 / 0.0 per half)
+    const uint32_t one = 0x3C003C00u, zero = 0u;
+    asm("fma.rn.relu.f16x2 %0, %1, %2, %3;" : "=r"(phi) : "r"(x), "r"(one), "r"(zero));
+    asm("set.gt.f16x2.f16x2 %0, %1, %2;" : "=r"(dphi) : "r"(x), "r"(zero));
+    return;
+  }
   uint32_t r, t;
   const uint32_t log2e = 0x3DC53DC5u, ln2 = 0x398C398Cu, zero = 0u;
   asm("fma.rn.relu.f16x2 %0, %1, %2, %3;" : "=r"(r) : "r"(x), "r"(log2e), "r"(zero));
@@ -125,11 +131,12 @@ __device__ __forceinline__ void phi_dphi_h2(uint32_t raw, uint32_t& phi, uint32_
   asm("fma.rn.f16x2 %0, %1, %2, %3;" : "=r"(phi) : "r"(r), "r"(ln2), "r"(dphi));
 }
 // (v0, v1) * f (fp16x2) -> two packed output elements
-template <bool BF16>
+// F32: multiply in fp32 (needed when v may exceed fp16 while f is exactly 0: the ReLU map's phi')
+template <bool BF16, bool F32 = false>
 __device__ __forceinline__ uint32_t pack_out_times_h2(float v0, float v1, uint32_t f) {
-  if (BF16) {
+  if (BF16 || F32) {
     const float2 ff = __half22float2(*reinterpret_cast<const __half2*>(&f));
-    return pack_out<true>(v0 * ff.x, v1 * ff.y);
+    return pack_out<BF16>(v0 * ff.x, v1 * ff.y);
   }
   __half2 r = __hmul2(__floats2half2_rn(v0, v1), *reinterpret_cast<const __half2*>(&f));
   return *reinterpret_cast<uint32_t*>(&r);

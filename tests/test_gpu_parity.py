@@ -278,6 +278,13 @@ def test_relu_forward_configs(c):
     _relu_case(wl.make_config(c), backward=False)
 
 
+@pytest.mark.parametrize("c", [4, 2, 3])
+def test_relu_backward_configs(c):
+    """The ReLU map's backward at full size: config 4 (d_h = 16) and config 2 (d_h = 32) on the tensor-core kernels,
+    config 3 (tiny windows packed into quadratic tiles + four windows of 27 500 rows through the split passes)."""
+    _relu_case(wl.make_config(c))
+
+
 @pytest.mark.parametrize("layout", sorted(EDGE_LAYOUTS))
 @pytest.mark.parametrize("dtype,H,d", [("f32", 4, 32), ("f16", 8, 16), ("bf16", 8, 32), ("f16", 3, 16)])
 def test_relu_edge_layouts_forward_backward(layout, dtype, H, d):
