@@ -221,14 +221,18 @@ def extra_legs(pkg, torch, dev, peak):
         q, k, v, g, o, dq, dk, dv = sets[i % n_sets]
         pkg.sla_backward(q, k, v, off, g, dq=dq, dk=dk, dv=dv, max_window_len=144)
 
-    uf, ub, ubb = timed(fwd4), timed(bwd4), timed(bwd4b)
+    def bwd4r(i):
+        q, k, v, g, o, dq, dk, dv = sets[i % n_sets]
+        pkg.sla_backward(q, k, v, off, g, dq=dq, dk=dk, dv=dv, workspace=ws, phi="relu", eps=1e-6)
+
+    uf, ub, ubb, ubr = timed(fwd4), timed(bwd4), timed(bwd4b), timed(bwd4r)
     out["training_step_config4"] = {
         "N": N, "W": W, "fwd_us": uf, "bwd_us": ub, "fwd_bwd_us": uf + ub,
         "voxels_per_sec_fwd_bwd": N / ((uf + ub) * 1e-6),
         "fwd_frac_of_peak": 4 * tb / (uf * 1e-6) / 1e9 / peak,
         "bwd_frac_of_peak": 7 * tb / (ub * 1e-6) / 1e9 / peak,
         "bwd_bounded_us": ubb, "bwd_bounded_frac_of_peak": 7 * tb / (ubb * 1e-6) / 1e9 / peak,
-        "fwd_bwd_bounded_us": uf + ubb,
+        "fwd_bwd_bounded_us": uf + ubb, "bwd_phi_relu_us": ubr,
         "bwd_algorithmic_bytes": 7 * tb,
         "note": "eager C-ABI calls back to back; fwd = sla_forward_bounded; bwd = sla_backward (zeroing kernel + "
                 "sla_bwd_tc_kernel + three split passes that exit at once, one PDL chain); bwd_bounded = "
