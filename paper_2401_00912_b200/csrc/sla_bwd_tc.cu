@@ -975,7 +975,8 @@ cudaError_t bwd_tc_launch(const Problem& p, cudaStream_t st) {
     if (e != cudaSuccess) return e;
     attr2_set[dev].store(true, std::memory_order_release);
   }
-  const int span2 = 128;                                   // <= kFuseMax; few pieces per window = few atomics per slot
+  const int span2 = kFuseMax / 16 * 16;                    // the largest span the split passes handle: few pieces per window (few atomics
+                                                           // per slot) and few blocks to start and retire when there is no long window
   cfg.gridDim = dim3((p.N + span2 - 1) / span2, slabs);
   le = cudaLaunchKernelEx(&cfg, k0, tk, tv, p.off, (T*)p.dq, (T*)p.dk, (T*)p.dv, p.ws_state, p.ws_dstate, p.N, p.W,
                           p.H, span2, p.eps);
