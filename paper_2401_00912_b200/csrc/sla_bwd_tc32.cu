@@ -4,11 +4,11 @@
 // (equal row spans per CTA, three TMA + mbarrier rings, one consumer warp per head, mma.sync m16n8k16 with fp32
 // accumulation, window state in registers), the same three passes per window and the same gradients of Eq. 3
 // (reading A14):
-//   pass A (K,V):    S = sum_j b_j^T v_j (kept as S and S^T fragments), z = sum_j b_j
+//   pass A (K,V):    S = sum_j b_j^T v_j (kept as S^T fragments), z = sum_j b_j
 //   pass B (Q,dO):   num = a S, den = a.z, dnum = g/den, dden = -(g.o)/den
 //                    dq = (dnum S^T + dden z) * phi'(q);  dS += a^T dnum;  dz += dden a
 //   pass C (K,V):    dv = b dS,  dk = (v dS^T + dz) * phi'(k)
-// A 32 x 32 state is four times the registers of a 16 x 16 one (S, S^T, dS, dS^T, z, dz: 160 fp32 per lane), so one
+// A 32 x 32 state is four times the registers of a 16 x 16 one (S^T, dS^T, z, dz: 96 fp32 per lane), so one
 // CTA of 8 head warps is resident per SM; short windows are not packed into shared tiles here (the d_h = 32 workload,
 // BASELINE.json config 2, has few rows in them).  Windows longer than kFuseMax rows go through three split passes
 // with their states in the fp32 workspace, as in the d_h = 16 file.
@@ -47,12 +47,12 @@ constexpr int KS = D / 16;   // 16-wide column groups of a head = k-steps of a c
 constexpr int NT = D / 8;    // 8-wide column tiles of a head
 using C = Cfg<D>;
 
+// Only the transposed forms S^T and dS^T are accumulated: the operands that need S and dS themselves are the 8 x 8
+// block transposes (movmatrix) of the operands built from S^T and dS^T (make_pass_b_ops / make_pass_c_ops).
 struct BwdState {
   float ST[KS][NT][4];    // S^T : rows r, columns p
-  float SS[KS][NT][4];    // S   : rows p, columns r
   float Z[NT][4];         // z[p] in columns p (same in every row)
   float dST[KS][NT][4];   // dS^T (scaled by 1/s)
-  float dSS[KS][NT][4];   // dS   (scaled by 1/s)
   float DZ[NT][4];        // dz   (scaled by 1/s)
   __device__ __forceinline__ void clear() {
 #pragma unroll
@@ -60,7 +60,7 @@ struct BwdState {
 #pragma unroll
       for (int b = 0; b < NT; ++b)
 #pragma unroll
-        for (int c = 0; c < 4; ++c) { ST[a][b][c] = 0.f; SS[a][b][c] = 0.f; dST[a][b][c] = 0.f; dSS[a][b][c] = 0.f; }
+        for (int c = 0; c < 4; ++c) { ST[a][b][c] = 0.f; dST[a][b][c] = 0.f; }
 #pragma unroll
     for (int b = 0; b < NT; ++b)
 #pragma unroll
@@ -88,6 +88,27 @@ __device__ __forceinline__ void make_ops(const float (&X)[KS][NT][4], float scal
       for (int b = 0; b < 2; ++b)
         to_op<PRECISE>(X[n / 2][2 * ks + b][2 * (n & 1)] * scale, X[n / 2][2 * ks + b][2 * (n & 1) + 1] * scale,
                        o.hi[n][ks][b], o.lo[n][ks][b]);
+}
+
+__device__ __forceinline__ uint32_t movm_t(uint32_t x) {   // transpose of one 8x8 block of 16-bit elements
+  uint32_t y;
+  asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(y) : "r"(x));
+  return y;
+}
+// Operands of the transposed matrix: o holds the 8 x 8 blocks (output block n, contraction block 2 ks + b) of X; the
+// same blocks of X^T are the transposes of the blocks (2 ks + b, n) of X.
+template <bool PRECISE>
+__device__ __forceinline__ void transpose_ops(const Ops& o, Ops& t) {
+#pragma unroll
+  for (int n = 0; n < NT; ++n)
+#pragma unroll
+    for (int ks = 0; ks < KS; ++ks)
+#pragma unroll
+      for (int b = 0; b < 2; ++b) {
+        const int m = 2 * ks + b;                      // contraction block of t = output block of o
+        t.hi[n][ks][b] = movm_t(o.hi[m][n >> 1][n & 1]);
+        t.lo[n][ks][b] = PRECISE ? movm_t(o.lo[m][n >> 1][n & 1]) : 0u;
+      }
 }
 
 // phi of a packed pair in fp32 (a) and its derivative factor: elu+1: (x > 0 ? 1 : phi(x)); ReLU: [x > 0]
@@ -147,7 +168,7 @@ __device__ __forceinline__ void lane_pattern(int nvalid, int& trow, int& csel) {
 // 16-byte chunk of column group ks of head hl inside the slab row (a head is D/8 chunks)
 __device__ __forceinline__ int head_chunk(int hl, int ks, int csel) { return hl * (D / 8) + 2 * ks + csel; }
 
-// ---- pass A: one 16-row K/V tile -> S^T, S, z -------------------------------------------------------
+// ---- pass A: one 16-row K/V tile -> S^T, z ----------------------------------------------------------
 template <int MODE, bool PRECISE>
 __device__ __forceinline__ void bwd_kv_tile(const RingView& rv, int hl, int rel0, int nvalid, BwdState& s) {
   constexpr bool BF16 = (MODE & 1) != 0;   // I/O dtype bf16
@@ -192,12 +213,7 @@ __device__ __forceinline__ void bwd_kv_tile(const RingView& rv, int hl, int rel0
     for (int mt = 0; mt < KS; ++mt) {
       // S^T (rows r of group mt, cols p of tile nt): A = V^T, B = phi(K)
       mma16816(s.ST[mt][nt], vr[mt][0], vr[mt][1], vr[mt][2], vr[mt][3], bh[kc][hf], bh[kc][2 + hf]);
-      // S (rows p of group mt, cols r of tile nt): A = phi(K)^T, B = V
-      mma16816(s.SS[mt][nt], bh[mt][0], bh[mt][1], bh[mt][2], bh[mt][3], vr[kc][hf], vr[kc][2 + hf]);
-      if (PRECISE) {
-        mma16816(s.ST[mt][nt], vr[mt][0], vr[mt][1], vr[mt][2], vr[mt][3], bl[kc][hf], bl[kc][2 + hf]);
-        mma16816(s.SS[mt][nt], bl[mt][0], bl[mt][1], bl[mt][2], bl[mt][3], vr[kc][hf], vr[kc][2 + hf]);
-      }
+      if (PRECISE) mma16816(s.ST[mt][nt], vr[mt][0], vr[mt][1], vr[mt][2], vr[mt][3], bl[kc][hf], bl[kc][2 + hf]);
     }
   }
 }
@@ -210,7 +226,7 @@ struct PassBOps {
   float eps;                 // epsilon of the denominator on the scale of the operands (eps * s); 0 for elu+1
 };
 
-// ---- pass B: one 16-row Q/dO tile -> dq rows, dS^T, dS, dz accumulators ------------------------------
+// ---- pass B: one 16-row Q/dO tile -> dq rows, dS^T, dz accumulators ----------------------------------
 template <int MODE, bool PRECISE, typename T>
 __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0, int nvalid,
                                            const PassBOps& op, BwdState& s, T* __restrict__ dq_rows,
@@ -363,8 +379,6 @@ __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0,
     for (int mt = 0; mt < KS; ++mt) {
       // dS^T (rows r of group mt, cols p of tile nt): A = dnum^T, B = a
       mma3<PRECISE>(s.dST[mt][nt], th[mt], tl[mt], uh[kc][hf], uh[kc][2 + hf], ul[kc][hf], ul[kc][2 + hf]);
-      // dS (rows p of group mt, cols r of tile nt): A = a^T, B = dnum
-      mma3<PRECISE>(s.dSS[mt][nt], uh[mt], ul[mt], th[kc][hf], th[kc][2 + hf], tl[kc][hf], tl[kc][2 + hf]);
     }
   }
 }
@@ -440,7 +454,7 @@ template <bool PRECISE>
 __device__ __forceinline__ void make_pass_b_ops(const BwdState& st, float scale, float eps, PassBOps& ob) {
   ob.eps = eps * scale;
   make_ops<PRECISE>(st.ST, scale, ob.num);
-  make_ops<PRECISE>(st.SS, scale, ob.da);
+  transpose_ops<PRECISE>(ob.num, ob.da);
 #pragma unroll
   for (int n = 0; n < NT; ++n) { ob.zs[n][0] = st.Z[n][0] * scale; ob.zs[n][1] = st.Z[n][1] * scale; }
 #pragma unroll
@@ -452,7 +466,7 @@ __device__ __forceinline__ void make_pass_b_ops(const BwdState& st, float scale,
 template <bool PRECISE>
 __device__ __forceinline__ void make_pass_c_ops(const BwdState& st, float scale, PassCOps& oc) {
   make_ops<PRECISE>(st.dST, scale, oc.dv);
-  make_ops<PRECISE>(st.dSS, scale, oc.db);
+  transpose_ops<PRECISE>(oc.dv, oc.db);
 #pragma unroll
   for (int n = 0; n < NT; ++n) { oc.dzs[n][0] = st.DZ[n][0] * scale; oc.dzs[n][1] = st.DZ[n][1] * scale; }
 }
@@ -709,8 +723,8 @@ sla_bwd_tc32_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
-          for (int c = 0; c < 4; ++c)      // S fragment: row p, column r
-            atomicAdd(slot + (16 * mt + g + 8 * (c >> 1)) * D + 8 * nt + 2 * t + (c & 1), st.SS[mt][nt][c]);
+          for (int c = 0; c < 4; ++c)      // S^T fragment: row r, column p -> S[p][r]
+            atomicAdd(slot + (8 * nt + 2 * t + (c & 1)) * D + 16 * mt + g + 8 * (c >> 1), st.ST[mt][nt][c]);
       if (g == 0) {
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt)
@@ -726,7 +740,6 @@ sla_bwd_tc32_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_
           for (int c = 0; c < 4; ++c) {
             const int row = 16 * mt + g + 8 * (c >> 1), col = 8 * nt + 2 * t + (c & 1);
             st.ST[mt][nt][c] = slot[col * D + row];     // S^T[r][p] = S[p][r]
-            st.SS[mt][nt][c] = slot[row * D + col];     // S[p][r]
           }
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt)
@@ -745,8 +758,8 @@ sla_bwd_tc32_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
-          for (int c = 0; c < 4; ++c)      // dS fragment (scaled by 1/s): row p, column r
-            atomicAdd(dslot + (16 * mt + g + 8 * (c >> 1)) * D + 8 * nt + 2 * t + (c & 1), st.dSS[mt][nt][c]);
+          for (int c = 0; c < 4; ++c)      // dS^T fragment (scaled by 1/s): row r, column p -> dS[p][r]
+            atomicAdd(dslot + (8 * nt + 2 * t + (c & 1)) * D + 16 * mt + g + 8 * (c >> 1), st.dST[mt][nt][c]);
       if (g == 0) {
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt)
@@ -762,7 +775,6 @@ sla_bwd_tc32_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_
           for (int c = 0; c < 4; ++c) {
             const int row = 16 * mt + g + 8 * (c >> 1), col = 8 * nt + 2 * t + (c & 1);
             st.dST[mt][nt][c] = dslot[col * D + row];   // dS^T[r][p]
-            st.dSS[mt][nt][c] = dslot[row * D + col];   // dS[p][r]
           }
 #pragma unroll
       for (int nt = 0; nt < NT; ++nt)
