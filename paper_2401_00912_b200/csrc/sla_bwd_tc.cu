@@ -4,7 +4,7 @@
 //
 // Gradients of Eq. 3 (the paper is silent on backward), per window
 // and head, a = phi(q), b = phi(k), g = dO:
-//   pass A (K,V):    S = sum_j b_j^T v_j (kept as S and S^T fragments), z = sum_j b_j
+//   pass A (K,V):    S = sum_j b_j^T v_j (kept as S^T fragments; operands that need S are block transposes), z = sum_j b_j
 //   pass B (Q,dO):   num = a S, den = a.z, o = num/den, dnum = g/den, dden = -(g.o)/den
 //                    dq = (dnum S^T + dden z) * phi'(q)
 //                    dS += a^T dnum (kept as dS and dS^T fragments), dz += dden a
@@ -48,17 +48,15 @@ using C = Cfg<D>;
 // fragments of one (window, head); c index: rows g (c<2) / g+8 (c>=2), columns 2t + (c&1)
 struct BwdState {
   float ST[2][4];    // S^T : rows r, column tile nt over p
-  float SS[2][4];    // S   : rows p, column tile nt over r
   float Z[2][4];     // z[p] in columns p (same in every row)
   float dST[2][4];   // dS^T (scaled by 1/s)
-  float dSS[2][4];   // dS   (scaled by 1/s)
   float DZ[2][4];    // dz   (scaled by 1/s)
   __device__ __forceinline__ void clear() {
 #pragma unroll
     for (int a = 0; a < 2; ++a)
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
-        ST[a][c] = 0.f; SS[a][c] = 0.f; Z[a][c] = 0.f; dST[a][c] = 0.f; dSS[a][c] = 0.f; DZ[a][c] = 0.f;
+        ST[a][c] = 0.f; Z[a][c] = 0.f; dST[a][c] = 0.f; DZ[a][c] = 0.f;
       }
   }
 };
@@ -74,6 +72,25 @@ __device__ __forceinline__ void make_ops(const float (&X)[2][4], float scale, Op
       const float x0 = X[b][2 * n] * scale, x1 = X[b][2 * n + 1] * scale;
       if (PRECISE) split_h2(x0, x1, o.hi[n][b], o.lo[n][b]);
       else { o.hi[n][b] = pack_h2(x0, x1); o.lo[n][b] = 0u; }
+    }
+}
+
+// Operands of the transposed matrix: o holds the 8 x 8 blocks (output block n, contraction block b) of X; the same
+// blocks of X^T are the movmatrix transposes of the blocks (b, n) of X.  Only S^T and dS^T are accumulated; the
+// operands that need S and dS come from here.
+__device__ __forceinline__ uint32_t movm_t(uint32_t x) {   // transpose of one 8x8 block of 16-bit elements
+  uint32_t y;
+  asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(y) : "r"(x));
+  return y;
+}
+template <bool PRECISE>
+__device__ __forceinline__ void transpose_ops(const OpPair& o, OpPair& t) {
+#pragma unroll
+  for (int n = 0; n < 2; ++n)
+#pragma unroll
+    for (int b = 0; b < 2; ++b) {
+      t.hi[n][b] = movm_t(o.hi[b][n]);
+      t.lo[n][b] = PRECISE ? movm_t(o.lo[b][n]) : 0u;
     }
 }
 
@@ -176,12 +193,9 @@ __device__ __forceinline__ void bwd_kv_tile(const RingView& rv, int hl, int rel0
     // S^T (rows r, cols p): A = V^T = (vr0..3), B = phi(K) tile nt = (b[nt], b[2+nt])
     mma16816(s.ST[nt], vr[0], vr[1], vr[2], vr[3], bh[nt], bh[2 + nt]);
     mma16816(s.Z[nt], ones, ones, ones, ones, bh[nt], bh[2 + nt]);
-    // S (rows p, cols r): A = phi(K)^T = (b0..3), B = V tile nt = (vr[nt], vr[2+nt])
-    mma16816(s.SS[nt], bh[0], bh[1], bh[2], bh[3], vr[nt], vr[2 + nt]);
     if (PRECISE) {
       mma16816(s.ST[nt], vr[0], vr[1], vr[2], vr[3], bl[nt], bl[2 + nt]);
       mma16816(s.Z[nt], ones, ones, ones, ones, bl[nt], bl[2 + nt]);
-      mma16816(s.SS[nt], bl[0], bl[1], bl[2], bl[3], vr[nt], vr[2 + nt]);
     }
   }
 }
@@ -321,8 +335,6 @@ __device__ __forceinline__ void bwd_q_tile(const RingView& rv, int hl, int rel0,
   for (int nt = 0; nt < 2; ++nt) {
     // dS^T (rows r, cols p): A = dnum^T = (t0..3), B = a tile nt over p = (u[nt], u[2+nt])
     mma3<PRECISE>(s.dST[nt], th, tl, uh[nt], uh[2 + nt], ul[nt], ul[2 + nt]);
-    // dS (rows p, cols r): A = a^T = (u0..3), B = dnum tile nt over r = (t[nt], t[2+nt])
-    mma3<PRECISE>(s.dSS[nt], uh, ul, th[nt], th[2 + nt], tl[nt], tl[2 + nt]);
     // dz[p] = sum_i dden_i a_i[p]: A rows all equal to dden over i, B = a tile nt
     mma3<PRECISE>(s.DZ[nt], dda_h, dda_l, uh[nt], uh[2 + nt], ul[nt], ul[2 + nt]);
   }
@@ -395,11 +407,6 @@ __device__ __forceinline__ void bwd_kv_out_tile(const RingView& rv, int hl, int 
 //   dv_j = sum_i W_ij g_i,   da_i = sum_j dP_ij b_j,   db_j = sum_i dP_ij a_i,   dq = da phi'(q),  dk = db phi'(k)
 // a, b, W and dP are split into fp16 hi+lo operands (as in the forward's packed tiles); g and v are exact.
 // `wid` = window ordinal of tile row `lane` (lanes >= nvalid hold -1).
-__device__ __forceinline__ uint32_t movm_t(uint32_t x) {   // transpose of one 8x8 block of 16-bit elements
-  uint32_t y;
-  asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(y) : "r"(x));
-  return y;
-}
 template <int MODE, typename T>
 __device__ __forceinline__ void bwd_quad_tile(const RingView& kv, const RingView& qg, int hl, int rel0, int nvalid,
                                               int wid, T* __restrict__ dq_rows, T* __restrict__ dk_rows,
@@ -570,7 +577,7 @@ __device__ __forceinline__ void bwd_window(RingView& kv, RingView& qg, RingView&
   PassBOps ob;
   ob.eps = eps * scale;
   make_ops<PRECISE>(st.ST, scale, ob.num);
-  make_ops<PRECISE>(st.SS, scale, ob.da);
+  transpose_ops<PRECISE>(ob.num, ob.da);
 #pragma unroll
   for (int b = 0; b < 2; ++b) {
     ob.zs[b][0] = st.Z[b][0] * scale; ob.zs[b][1] = st.Z[b][1] * scale;
@@ -584,7 +591,7 @@ __device__ __forceinline__ void bwd_window(RingView& kv, RingView& qg, RingView&
   }
   PassCOps oc;
   make_ops<PRECISE>(st.dST, scale, oc.dv);
-  make_ops<PRECISE>(st.dSS, scale, oc.db);
+  transpose_ops<PRECISE>(oc.dv, oc.db);
 #pragma unroll
   for (int b = 0; b < 2; ++b) { oc.dzs[b][0] = st.DZ[b][0] * scale; oc.dzs[b][1] = st.DZ[b][1] * scale; }
   for (int r = s; r < e; r += 16) {
@@ -871,13 +878,12 @@ sla_bwd_tc_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_co
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
           st.ST[nt][c] = slot[(8 * nt + 2 * t + (c & 1)) * D + g + 8 * (c >> 1)];     // S^T[r][p] = S[p][r]
-          st.SS[nt][c] = slot[(g + 8 * (c >> 1)) * D + 8 * nt + 2 * t + (c & 1)];     // S[p][r]
           st.Z[nt][c] = slot[D * D + 8 * nt + 2 * t + (c & 1)];
         }
       PassBOps ob;
       ob.eps = eps * scale;
       make_ops<false>(st.ST, scale, ob.num);
-      make_ops<false>(st.SS, scale, ob.da);
+      transpose_ops<false>(ob.num, ob.da);
 #pragma unroll
       for (int b = 0; b < 2; ++b) {
         ob.zs[b][0] = st.Z[b][0] * scale; ob.zs[b][1] = st.Z[b][1] * scale;
@@ -892,8 +898,8 @@ sla_bwd_tc_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_co
 #pragma unroll
       for (int nt = 0; nt < 2; ++nt)
 #pragma unroll
-        for (int c = 0; c < 4; ++c)      // dS fragment (scaled by 1/s): row p = g + 8 (c/2), column r = 8 nt + 2t + (c%2)
-          atomicAdd(dslot + (g + 8 * (c >> 1)) * D + 8 * nt + 2 * t + (c & 1), st.dSS[nt][c]);
+        for (int c = 0; c < 4; ++c)      // dS^T fragment (scaled by 1/s): row r = g + 8 (c/2), column p = 8 nt + 2t + (c%2)
+          atomicAdd(dslot + (8 * nt + 2 * t + (c & 1)) * D + g + 8 * (c >> 1), st.dST[nt][c]);
       if (g == 0) {
 #pragma unroll
         for (int nt = 0; nt < 2; ++nt)
@@ -907,11 +913,10 @@ sla_bwd_tc_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_co
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
           st.dST[nt][c] = dslot[(8 * nt + 2 * t + (c & 1)) * D + g + 8 * (c >> 1)];   // dS^T[r][p]
-          st.dSS[nt][c] = dslot[(g + 8 * (c >> 1)) * D + 8 * nt + 2 * t + (c & 1)];   // dS[p][r]
           st.DZ[nt][c] = dslot[D * D + 8 * nt + 2 * t + (c & 1)];
         }
       make_ops<false>(st.dST, scale, oc.dv);
-      make_ops<false>(st.dSS, scale, oc.db);
+      transpose_ops<false>(oc.dv, oc.db);
 #pragma unroll
       for (int b = 0; b < 2; ++b) { oc.dzs[b][0] = st.DZ[b][0] * scale; oc.dzs[b][1] = st.DZ[b][1] * scale; }
       for (int r = ps; r < pe; r += 16) {
