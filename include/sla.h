@@ -230,8 +230,9 @@ int sla_sequence_from_coords(const int32_t* coords, int64_t N, int32_t batch, in
  *          rows 0..C-1 give Q (W_Q of the paper is their transpose), C..2C-1 give K, 2C..3C-1 give V (read-only)
  *   bias   DEV fp32 [3C], 16-byte aligned, added before the rounding; NULL = none (the paper's formula has none)
  *   q,k,v  DEV [N, C] of dt out; as [N, H, d_h] they are what sla_forward takes
- * Supported: dt = SLA_F16 / SLA_BF16 and C in {128, 256}; anything else -> SLA_ERR_UNSUPPORTED.  All base pointers
- * 16-byte aligned.  Enqueues one kernel on `stream`; no workspace. */
+ * fp16 / bf16 with C in {128, 256} run on the tensor cores; fp32 I/O and every other C take a plain tiled kernel on the
+ * CUDA cores (fp32 accumulation as well; a fallback, not a fast path).  All base pointers 16-byte aligned.  Enqueues one
+ * kernel on `stream`; no workspace. */
 int sla_qkv_projection(const void* x, const void* w_qkv, const float* bias, int64_t N, int32_t C, int dt,
                        void* q, void* k, void* v, sla_stream_t stream);
 

@@ -389,8 +389,8 @@ def _chk_proj(x, w, bias):
 
 
 def sla_qkv_projection(x, w_qkv, bias=None, q=None, k=None, v=None, stream=None):
-    """x: CUDA [N, C] fp16/bf16, w_qkv: [3C, C] (row j = weights of output feature j; Q, K, V blocks) -> (q, k, v),
-    each [N, C]: y = x w^T (+ bias) on tcgen05."""
+    """x: CUDA [N, C], w_qkv: [3C, C] (row j = weights of output feature j; Q, K, V blocks) -> (q, k, v), each
+    [N, C]: y = x w^T (+ bias); fp16/bf16 with C in {128, 256} on tcgen05, everything else on a generic kernel."""
     import torch
     L = load_library()
     _chk_proj(x, w_qkv, bias)

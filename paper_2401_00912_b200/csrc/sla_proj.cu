@@ -309,16 +309,100 @@ cudaError_t proj_launch(const void* x, const void* w, const float* bias, int N, 
   return cudaLaunchKernelEx(&cfg, kern, maps, bias, N, n_out * C / CHUNK_N);
 }
 
+// ---- generic path: fp32 I/O and every C the tensor-core kernel does not take ------------------------------------------
+// A plain shared-memory tiled product on the CUDA cores, fp32 accumulation in a fixed order: 64 rows x 64 output
+// features per block, 16 columns of x and w per step, 4 x 4 outputs per thread.  A fallback, not a fast path.
+template <typename T> __device__ __forceinline__ float to_f32(T v);
+template <> __device__ __forceinline__ float to_f32<float>(float v) { return v; }
+template <> __device__ __forceinline__ float to_f32<__half>(__half v) { return __half2float(v); }
+template <> __device__ __forceinline__ float to_f32<__nv_bfloat16>(__nv_bfloat16 v) { return __bfloat162float(v); }
+template <typename T> __device__ __forceinline__ T from_f32(float v);
+template <> __device__ __forceinline__ float from_f32<float>(float v) { return v; }
+template <> __device__ __forceinline__ __half from_f32<__half>(float v) { return __float2half_rn(v); }
+template <> __device__ __forceinline__ __nv_bfloat16 from_f32<__nv_bfloat16>(float v) { return __float2bfloat16_rn(v); }
+
+constexpr int GT = 64, GK = 16;
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+sla_proj_generic_kernel(const T* __restrict__ x, const T* __restrict__ w, const float* __restrict__ bias, int N, int C,
+                        int F /* output features = n_out * C */, T* __restrict__ y0, T* __restrict__ y1,
+                        T* __restrict__ y2) {
+  __shared__ float sx[GK][GT + 1], sw[GK][GT + 1];
+  asm volatile("griddepcontrol.launch_dependents;");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  const int row0 = blockIdx.x * GT, f0 = blockIdx.y * GT;
+  const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;      // thread: rows 4 ty .., features 4 tx ..
+  float acc[4][4] = {};
+  for (int k0 = 0; k0 < C; k0 += GK) {
+    for (int i = threadIdx.x; i < GT * GK; i += 256) {
+      const int r = i / GK, kk = i % GK;
+      const bool kin = k0 + kk < C;
+      sx[kk][r] = (kin && row0 + r < N) ? to_f32<T>(x[(size_t)(row0 + r) * C + k0 + kk]) : 0.f;
+      sw[kk][r] = (kin && f0 + r < F) ? to_f32<T>(w[(size_t)(f0 + r) * C + k0 + kk]) : 0.f;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int kk = 0; kk < GK; ++kk) {
+      float a[4], b[4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) { a[i] = sx[kk][4 * ty + i]; b[i] = sw[kk][4 * tx + i]; }
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
+    }
+    __syncthreads();
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int r = row0 + 4 * ty + i;
+    if (r >= N) continue;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const int f = f0 + 4 * tx + j;
+      if (f >= F) continue;
+      const float v = acc[i][j] + (bias != nullptr ? __ldg(bias + f) : 0.f);
+      T* y = (f < C) ? y0 : (f < 2 * C ? y1 : y2);             // feature block -> output tensor
+      y[(size_t)r * C + (f % C)] = from_f32<T>(v);
+    }
+  }
+}
+
+template <typename T>
+cudaError_t proj_generic_launch(const void* x, const void* w, const float* bias, int N, int C, int n_out, void* q,
+                                void* k, void* v, cudaStream_t st) {
+  cudaLaunchAttribute pdl[1];
+  pdl[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  pdl[0].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((N + GT - 1) / GT, (n_out * C + GT - 1) / GT);
+  cfg.blockDim = dim3(256);
+  cfg.stream = st;
+  cfg.attrs = pdl;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, sla_proj_generic_kernel<T>, (const T*)x, (const T*)w, bias, N, C, n_out * C, (T*)q,
+                            (T*)k, (T*)v);
+}
+
 }  // namespace
 
+// the tcgen05 kernel takes fp16 / bf16 with C = 128 or 256; everything else (fp32 I/O, other C) the generic kernel
+static bool projection_on_tensor_cores(int C, int dt) {
+  return (dt == SLA_F16 || dt == SLA_BF16) && (C == 128 || C == 256) && encode_fn() != nullptr;
+}
+
 bool qkv_projection_supported(int C, int dt) {
-  if (dt != SLA_F16 && dt != SLA_BF16) return false;
-  if (C != 128 && C != 256) return false;
-  return encode_fn() != nullptr;
+  return (dt == SLA_F32 || dt == SLA_F16 || dt == SLA_BF16) && C >= 1 && C <= (1 << 20);
 }
 
 cudaError_t launch_qkv_projection(const void* x, const void* w, const float* bias, int N, int C, int dt, int n_out,
                                   void* q, void* k, void* v, cudaStream_t st) {
+  if (!projection_on_tensor_cores(C, dt)) {
+    if (dt == SLA_F32) return proj_generic_launch<float>(x, w, bias, N, C, n_out, q, k, v, st);
+    if (dt == SLA_F16) return proj_generic_launch<__half>(x, w, bias, N, C, n_out, q, k, v, st);
+    return proj_generic_launch<__nv_bfloat16>(x, w, bias, N, C, n_out, q, k, v, st);
+  }
   if (C == 128)
     return dt == SLA_F16 ? proj_launch<128, false, __half>(x, w, bias, N, n_out, q, k, v, st)
                          : proj_launch<128, true, __nv_bfloat16>(x, w, bias, N, n_out, q, k, v, st);

@@ -14,7 +14,7 @@ from oracle import sla_proj_oracle as P
 
 pytestmark = pytest.mark.gpu
 
-UNIT = {"f16": 2.0 ** -11, "bf16": 2.0 ** -8}
+UNIT = {"f32": 2.0 ** -24, "f16": 2.0 ** -11, "bf16": 2.0 ** -8}
 TOL = {"f16": (2e-2, 1e-3), "bf16": (2e-2, 1e-3)}      # the SLA tolerance, for the module test
 
 
@@ -25,7 +25,7 @@ def _torch():
 
 def _tdt(dtype):
     torch = _torch()
-    return {"f16": torch.float16, "bf16": torch.bfloat16}[dtype]
+    return {"f32": torch.float32, "f16": torch.float16, "bf16": torch.bfloat16}[dtype]
 
 
 def _inputs(N, C, dtype, seed, bias):
@@ -130,14 +130,39 @@ def test_linear_against_oracle(N, C, dtype, bias):
     assert np.isfinite(g).all() and (np.abs(g - ref) / allowed).max() <= 1.0
 
 
+@pytest.mark.parametrize("N,C,dtype,bias", [(2000, 128, "f32", True), (777, 64, "f16", False), (130, 48, "bf16", True),
+                                            (65, 20, "f32", False), (1, 512, "f16", True)])
+def test_projection_generic_path(N, C, dtype, bias):
+    """fp32 I/O (config 0's dtype) and the C the tensor-core kernel does not take: the plain tiled kernel."""
+    torch = _torch()
+    x, w, b = _inputs(N, C, dtype, 2000 + N + C, bias)
+    got = pkg.sla_qkv_projection(_dev(x, dtype), _dev(w, dtype), _dev(b) if bias else None)
+    torch.cuda.synchronize()
+    _check_proj(got, x, w, b, dtype)
+    y = pkg.sla_linear(_dev(x, dtype), _dev(w[:C], dtype), _dev(b[:C]) if bias else None)
+    torch.cuda.synchronize()
+    assert torch.equal(y, got[0])                         # the same sums in the same order
+
+
+def test_module_forward_fp32_config0():
+    """The module on the fp32 configuration (generic projection + generic SLA kernels), SLA tolerance of fp32."""
+    torch = _torch()
+    sc = wl.make_config(0)
+    C = sc.H * sc.d_h
+    x, w, _ = _inputs(sc.N, C, "f32", 311, False)
+    out, q, k, v = pkg.sla_module_forward(_dev(x), _dev(w), torch.from_numpy(sc.offsets).cuda(), sc.H)
+    torch.cuda.synchronize()
+    _check_proj([t.reshape(sc.N, C) for t in (q, k, v)], x, w, None, "f32")
+    # the oracle chain on the GPU's q, k, v would break the rule that no oracle input comes from the CUDA path; fp32
+    # roundings of q, k, v (2^-24) are far below the SLA tolerance, so the chained oracles are compared directly
+    qr, kr, vr = (t.astype(np.float32).reshape(sc.N, sc.H, sc.d_h) for t in P.project_qkv(x, w))
+    ref = sla_oracle.forward(qr, kr, vr, sc.offsets)
+    g = out.double().cpu().numpy()
+    assert np.isfinite(g).all() and (np.abs(g - ref) / (1e-5 + 1e-4 * np.abs(ref))).max() <= 1.0
+
+
 def test_projection_errors_and_empty():
     torch = _torch()
-    x = torch.zeros(10, 64, dtype=torch.float16, device="cuda")
-    with pytest.raises(pkg.SlaError, match="UNSUPPORTED"):
-        pkg.sla_qkv_projection(x, torch.zeros(192, 64, dtype=torch.float16, device="cuda"))
-    xf = torch.zeros(10, 128, dtype=torch.float32, device="cuda")
-    with pytest.raises(pkg.SlaError, match="UNSUPPORTED"):
-        pkg.sla_qkv_projection(xf, torch.zeros(384, 128, dtype=torch.float32, device="cuda"))
     with pytest.raises(pkg.SlaError):
         pkg.sla_qkv_projection(torch.zeros(10, 128, dtype=torch.float16, device="cuda"),
                                torch.zeros(128, 384, dtype=torch.float16, device="cuda"))
