@@ -491,3 +491,26 @@ def test_forward_under_cuda_graph_replay():
         g.replay()
         torch.cuda.synchronize()
     assert torch.equal(out, want)
+
+
+def test_second_device_after_first():
+    """Per-device state (shared-memory opt-ins, SM count, the static workspace's address, tensor maps): the same calls
+    on cuda:1 after cuda:0 must give the same results.  Skipped on a one-GPU box."""
+    torch = _torch()
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    sc = wl.make_scene([300, 5, 1, 1000, 17, 64], 8, 16, "f16", seed=55)
+    ref = sla_oracle.forward(sc.tensor("q"), sc.tensor("k"), sc.tensor("v"), sc.offsets)
+    outs = []
+    for dev in ("cuda:0", "cuda:1", "cuda:0"):
+        with torch.cuda.device(dev):
+            q, k, v = (to_dev(sc.tensor(n), "f16").to(dev) for n in ("q", "k", "v"))
+            off = torch.from_numpy(sc.offsets).to(dev)
+            o1 = pkg.sla_forward(q, k, v, off)
+            o2 = pkg.sla_forward_static(q, k, v, off)
+            g = pkg.sla_backward(q, k, v, off, to_dev(sc.tensor("do"), "f16").to(dev))
+            torch.cuda.synchronize()
+            check(f"{dev}.out", o1, ref, "f16", sc.lengths)
+            check(f"{dev}.static", o2, ref, "f16", sc.lengths)
+            outs.append((o1.cpu(), g[0].cpu()))
+    assert torch.equal(outs[0][0][:5], outs[2][0][:5])
