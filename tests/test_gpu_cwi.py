@@ -127,6 +127,46 @@ def test_cwi_writes_nothing_beyond_n_and_ignores_voxels_off_the_grid():
     assert np.all(got[7, :48] == 0) and np.array_equal(got[7, 48:], x[7, 48:].astype(np.float64))
 
 
+def test_cwi_full_size_properties():
+    """The bench's size (60 000 voxels, 468 x 468 x 32 grid), where the oracle's Python loops would take minutes:
+    properties that hold at any size.  (a) Relabelling the voxels permutes the output rows and changes nothing else
+    (fixed tap order: bit for bit).  (b) Shifting the whole scene inside the grid changes nothing.  (c) Sampled
+    voxels against the oracle evaluated on their neighbourhoods only."""
+    torch = _torch()
+    grid = (1, 32, 468, 468)
+    rng = np.random.Generator(np.random.PCG64(2024))
+    coords = wl.coords_waymo_like(2024, N=60000, batch=1, nz=6)
+    coords[:, 2] = np.clip(coords[:, 2], 8, 459)             # room for the shift of (b)
+    coords[:, 3] = np.clip(coords[:, 3], 8, 459)
+    coords = np.unique(coords, axis=0).astype(np.int32)
+    n = coords.shape[0]
+    x = wl.round_to_dtype(rng.standard_normal((n, 128)).astype(np.float32), "f16")
+    ws = _weights(rng, 32, 12, 12)
+    wd = [torch.from_numpy(w).cuda() for w in ws]
+    xd, cd = torch.from_numpy(x).cuda().half(), torch.from_numpy(coords).cuda()
+    out = pkg.sla_cwi_forward(xd, cd, grid, 12, 12, *wd)
+    perm = torch.from_numpy(rng.permutation(n)).cuda()
+    out_p = pkg.sla_cwi_forward(xd[perm].contiguous(), cd[perm].contiguous(), grid, 12, 12, *wd)
+    shift = torch.tensor([0, 1, 7, -5], dtype=torch.int32, device="cuda")
+    out_s = pkg.sla_cwi_forward(xd, (cd + shift).contiguous(), grid, 12, 12, *wd)
+    torch.cuda.synchronize()
+    assert torch.equal(out_p, out[perm])
+    assert torch.equal(out_s, out)
+    sample = rng.choice(n, 300, replace=False)
+    near = np.zeros(n, bool)
+    for i in sample:                                          # every voxel any tap of a sampled voxel can reach
+        d = np.abs(coords - coords[i])
+        near |= (d[:, 0] == 0) & (d[:, 1] <= 1) & (d[:, 2] <= 6) & (d[:, 3] <= 6)
+    idx = np.flatnonzero(near)
+    ref = O.cwi_forward(x[idx], coords[idx], 12, 12, *ws)
+    mag = O.magnitude(x[idx], coords[idx], 12, 12, *ws)
+    pos = {int(v): j for j, v in enumerate(idx)}
+    rows = np.array([pos[int(i)] for i in sample])
+    acc = 54 * 2.0 ** -24 * mag[rows]
+    got = out[torch.from_numpy(sample).cuda()].double().cpu().numpy()
+    assert np.all(np.abs(got - ref[rows]) <= acc + UNIT["f16"] * (np.abs(ref[rows]) + acc) + 2.0 ** -24)
+
+
 def test_cwi_errors():
     torch = _torch()
     x = torch.zeros(10, 128, dtype=torch.float16, device="cuda")
