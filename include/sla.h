@@ -134,6 +134,24 @@ int sla_forward_bounded(const void* q, const void* k, const void* v, const int32
                         int64_t N, int32_t W, int32_t H, int32_t d_h, int dt, void* out,
                         int32_t max_window_len, sla_stream_t stream);
 
+/* The work list of the flat sequence, built once per scene ("chunk -> window map / work list",
+ * PAPER.md:93 Fig. 3a; the paper's "offsets generation" stage, Fig. 5): for every row span the tensor-core forward
+ * hands to a thread block, the window of its first row and the rows the block streams.  A scene's window structure is
+ * the same for every block of the network and for every head, so the table is built once and passed to every
+ * sla_forward_planned call on that scene; without it every thread block finds its windows by a search of the offsets
+ * (three dependent rounds of probes), with it by one 16-byte load.
+ *   table  DEV, >= sla_span_table_bytes(N, H, d_h) bytes, 16-byte aligned; written by sla_build_span_table (one small
+ *          kernel on `stream`), read-only afterwards; valid for this (window_offsets, N, H, d_h) on this device.
+ * sla_forward_planned = sla_forward_bounded (same promise about max_window_len, same results bit for bit, one launch, no
+ * workspace) + the table.  A table that belongs to another N or launch geometry is detected on the device and ignored
+ * (the kernel searches as usual); a table of other offsets with the same N is undefined behaviour. */
+size_t sla_span_table_bytes(int64_t N, int32_t H, int32_t d_h);
+int sla_build_span_table(const int32_t* window_offsets, int64_t N, int32_t W, int32_t H, int32_t d_h,
+                         void* table, size_t table_bytes, sla_stream_t stream);
+int sla_forward_planned(const void* q, const void* k, const void* v, const int32_t* window_offsets,
+                        int64_t N, int32_t W, int32_t H, int32_t d_h, int dt, void* out,
+                        int32_t max_window_len, const void* table, size_t table_bytes, sla_stream_t stream);
+
 /* SLA backward: gradients of L = sum(d_out * SLA(q,k,v)) (the paper is silent on backward; these are
  * the analytic derivatives of Eq. 3):
  *   dnum_i = g_i/den_i, dden_i = -(g_i.o_i)/den_i, da_i = dnum_i S^T + dden_i z, dq_i = da_i*phi'(q_i)

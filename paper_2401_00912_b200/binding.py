@@ -20,7 +20,7 @@ _PHI = {"elu1": SLA_PHI_ELU1, "relu": SLA_PHI_RELU}
 # Every symbol include/sla.h declares (tests check the library exports exactly these).
 SYMBOLS = (
     "sla_status_string", "sla_version", "sla_workspace_bytes", "sla_offsets_from_window_ids",
-    "sla_forward", "sla_forward_phi", "sla_backward_phi", "sla_forward_tcgen05", "sla_forward_static", "sla_forward_bounded", "sla_backward", "sla_backward_bounded", "sla_forward_host",
+    "sla_forward", "sla_forward_phi", "sla_backward_phi", "sla_forward_tcgen05", "sla_forward_static", "sla_forward_bounded", "sla_span_table_bytes", "sla_build_span_table", "sla_forward_planned", "sla_backward", "sla_backward_bounded", "sla_forward_host",
     "sla_bench_stream_ceiling",
     "sla_window_count", "sla_window_keys", "sla_sort_workspace_bytes", "sla_sort_by_window", "sla_gather_rows",
     "sla_scatter_rows", "sla_sequence_workspace_bytes", "sla_sequence_from_coords",
@@ -65,6 +65,12 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     L.sla_forward_static.restype = ci
     L.sla_forward_bounded.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, i32, vp]
     L.sla_forward_bounded.restype = ci
+    L.sla_span_table_bytes.argtypes = [i64, i32, i32]
+    L.sla_span_table_bytes.restype = sz
+    L.sla_build_span_table.argtypes = [vp, i64, i32, i32, i32, vp, sz, vp]
+    L.sla_build_span_table.restype = ci
+    L.sla_forward_planned.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, i32, vp, sz, vp]
+    L.sla_forward_planned.restype = ci
     L.sla_backward.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp, vp, vp, vp, sz, vp]
     L.sla_backward.restype = ci
     L.sla_backward_bounded.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, ci, vp, vp, vp, vp, i32, vp]
@@ -471,4 +477,35 @@ def sla_cwi_forward(x, coords, grid, S_h: int, S_w: int, w_h, w_w, w_3, out=None
     _check(L.sla_cwi_forward(x.data_ptr(), coords.data_ptr(), N, C, dt, batch, gz, gh, gw, S_h, S_w, w_h.data_ptr(),
                              w_w.data_ptr(), w_3.data_ptr(), out.data_ptr(), workspace.data_ptr(), workspace.numel(),
                              _stream(stream)), "sla_cwi_forward")
+    return out
+
+
+# ---- span table ----
+
+def sla_build_span_table(window_offsets, N: int, H: int, d_h: int, table=None, stream=None):
+    """The work list of a scene for sla_forward_planned: CUDA uint8 buffer of sla_span_table_bytes(N, H, d_h)."""
+    import torch
+    L = load_library()
+    _chk_i32(window_offsets, "window_offsets")
+    need = int(L.sla_span_table_bytes(N, H, d_h))
+    if table is None:
+        table = torch.empty(max(need, 16), dtype=torch.uint8, device=window_offsets.device)
+    _check(L.sla_build_span_table(window_offsets.data_ptr(), N, window_offsets.numel() - 1, H, d_h, table.data_ptr(),
+                                  table.numel(), _stream(stream)), "sla_build_span_table")
+    return table
+
+
+def sla_forward_planned(q, k, v, window_offsets, table, max_window_len: int, out=None, stream=None):
+    """sla_forward_bounded with the scene's span table (built once by sla_build_span_table)."""
+    import torch
+    L = load_library()
+    _chk_dev(q, k, v, window_offsets, table)
+    if not (q.shape == k.shape == v.shape and q.dim() == 3 and q.dtype == k.dtype == v.dtype):
+        raise SlaError("q,k,v must share shape [N,H,d_h] and dtype")
+    N, H, d = q.shape
+    if out is None:
+        out = torch.empty_like(q)
+    _check(L.sla_forward_planned(q.data_ptr(), k.data_ptr(), v.data_ptr(), window_offsets.data_ptr(), N,
+                                 window_offsets.numel() - 1, H, d, _dt(q), out.data_ptr(), int(max_window_len),
+                                 table.data_ptr(), table.numel(), _stream(stream)), "sla_forward_planned")
     return out

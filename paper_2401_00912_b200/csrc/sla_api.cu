@@ -328,6 +328,44 @@ int sla_forward_bounded(const void* q, const void* k, const void* v, const int32
   return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
 }
 
+size_t sla_span_table_bytes(int64_t N, int32_t H, int32_t d_h) {
+  if (N < 0 || N >= (int64_t(1) << 31) || H < 1 || (d_h != 16 && d_h != 32)) return 0;
+  return sla::span_table_bytes(N, H, d_h);
+}
+
+int sla_build_span_table(const int32_t* window_offsets, int64_t N, int32_t W, int32_t H, int32_t d_h, void* table,
+                         size_t table_bytes, sla_stream_t stream) {
+  if (N < 0 || W < 0 || H < 1 || N >= (int64_t(1) << 31)) return SLA_ERR_INVALID_ARG;
+  if (d_h != 16 && d_h != 32) return SLA_ERR_UNSUPPORTED;
+  if (!table || table_bytes < sla::span_table_bytes(N, H, d_h) || !aligned16(table)) return SLA_ERR_WORKSPACE;
+  if (N == 0 || W == 0) return SLA_OK;
+  if (!window_offsets) return SLA_ERR_INVALID_ARG;
+  cudaError_t e = sla::launch_span_table(window_offsets, (int)N, W, H, d_h, table, (cudaStream_t)stream);
+  return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
+}
+
+int sla_forward_planned(const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
+                        int32_t W, int32_t H, int32_t d_h, int dt, void* out, int32_t max_window_len,
+                        const void* table, size_t table_bytes, sla_stream_t stream) {
+  int rc = check_common(N, W, H, d_h, dt);
+  if (rc != SLA_OK) return rc;
+  if (max_window_len < 1) return SLA_ERR_INVALID_ARG;
+  if (max_window_len > sla::kFuseMax) return SLA_ERR_UNSUPPORTED;   // use sla_forward
+  if (N == 0 || W == 0) return SLA_OK;
+  if (!q || !k || !v || !window_offsets || !out) return SLA_ERR_INVALID_ARG;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out)) return SLA_ERR_UNSUPPORTED;
+  if (!table || table_bytes < sla::span_table_bytes(N, H, d_h) || !aligned16(table)) return SLA_ERR_WORKSPACE;
+  sla::Problem p{};
+  p.q = q; p.k = k; p.v = v; p.out = out; p.off = window_offsets;
+  p.N = (int)N; p.W = W; p.H = H; p.d = d_h;
+  p.bounded = true;
+  p.span_table = table;
+  const bool tc = sla::forward_tc_supported(p, dt);           // the generic kernels have no use for the table
+  cudaError_t e = tc ? sla::launch_forward_tc(p, dt, (cudaStream_t)stream)
+                     : sla::launch_forward_generic(p, dt, (cudaStream_t)stream);
+  return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
+}
+
 static int backward_impl(int phi, float eps, const void* q, const void* k, const void* v, const int32_t* window_offsets, int64_t N,
                  int32_t W, int32_t H, int32_t d_h, int dt, const void* d_out, void* dq, void* dk,
                  void* dv, void* workspace, size_t workspace_bytes, sla_stream_t stream) {

@@ -43,6 +43,7 @@ constexpr int NW = 8;                       // consumer warps = heads per slab
 #endif
 constexpr int NST = SLA_NST;                // ring stages per stream at d_h = 16 (and the size of the barrier arrays)
 constexpr int QUAD_MAX = 16;                // windows up to this length are packed into quadratic-form tiles
+constexpr int kSpanTableMagic = 0x534c4154; // "SLAT": first word of a span table (sla_build_span_table)
 
 template <int D> struct Cfg {
   static constexpr int SR = SLA_SR;                       // rows per ring stage
@@ -492,7 +493,8 @@ template <int D, int MODE, typename T, bool OUTPASS>
 __global__ void __launch_bounds__(Cfg<D>::THREADS, (D == 16 ? SLA_MINB : 2))
 sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                   const __grid_constant__ CUtensorMap tmV, const int32_t* __restrict__ off,
-                  T* __restrict__ out, float* __restrict__ ws, int N, int W, int H, int span, float eps) {
+                  T* __restrict__ out, float* __restrict__ ws, int N, int W, int H, int span, float eps,
+                  const int4* __restrict__ table) {
   using C = Cfg<D>;
   extern __shared__ uint8_t dyn_smem[];
   __shared__ Ctrl ctrl;
@@ -575,7 +577,21 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   }
 
   // ---------------- consumer warps ----------------
-  if (warp == 0) {
+  // A span table built once per scene (sla_build_span_table: SURVEY a1's work list) replaces the window search: one
+  // 16-byte load instead of three dependent rounds of probes.  A table of another problem or launch geometry is ignored.
+  bool planned = false;
+  if (!OUTPASS && table != nullptr) {
+    const int4 hdr = __ldg(table);
+    planned = hdr.x == kSpanTableMagic && hdr.y == span && hdr.z == (int)gridDim.x && hdr.w == N;
+  }
+  if (planned) {
+    if (threadIdx.x == 0) {
+      const int4 rec = __ldg(table + 1 + sidx);              // (window of R0, stream begin, raw stream end, -)
+      ctrl.wa = rec.x;
+      ctrl.stream_begin = rec.y;
+      ctrl.stream_end = max(rec.z, rec.y);
+    }
+  } else if (warp == 0) {
     int wa, wl;
     warp_windows_of_rows(off, W, R0, R1 - 1, wa, wl);
     if (lane == 0) {
@@ -694,6 +710,47 @@ sla_fwd_tc_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant
   }
 }
 
+// ---- span table ("chunk -> window map / work list", Fig. 3a) ----------------------------------
+// One thread per window w = [s, e): the spans whose first row lies in the window get (w, stream begin), the spans whose
+// last row lies in it get the stream end -- the very rules of the in-kernel search above, evaluated once per scene.
+__global__ void __launch_bounds__(256)
+sla_span_table_kernel(const int32_t* __restrict__ off, int N, int W, int span, int nx, int4* __restrict__ table) {
+  asm volatile("griddepcontrol.launch_dependents;");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w == 0) table[0] = make_int4(kSpanTableMagic, span, nx, N);
+  if (w >= W) return;
+  const int s = __ldg(off + w), e = __ldg(off + w + 1);
+  if (e <= s) return;                                       // an empty window holds no row
+  const int m = e - s, mid = s + (m >> 1);
+  int* t = reinterpret_cast<int*>(table + 1);
+  for (int sp = (s + span - 1) / span; sp < nx && sp * span < e; ++sp) {       // spans with R0 in [s, e)
+    const int R0 = sp * span;
+    t[4 * sp + 0] = w;
+    t[4 * sp + 1] = (m <= kFuseMax) ? (mid >= R0 ? s : e) : R0;
+  }
+  for (int sp = s / span; sp < nx; ++sp) {                                      // spans with R1 - 1 in [s, e)
+    const int R1 = min(sp * span + span, N);
+    if (R1 - 1 < s) continue;
+    if (R1 - 1 >= e) break;
+    t[4 * sp + 2] = (m <= kFuseMax) ? (mid < R1 ? e : s) : R1;
+    t[4 * sp + 3] = 0;
+  }
+}
+
+// launch geometry of the main pass: rows per span and number of spans (shared by the kernel launch and the table)
+template <int D>
+void forward_geometry(int N, int H, int& span, int& nx) {
+  const int slabs = (H + NW - 1) / NW;
+  const int per_sm = (D == 16 ? 3 : 2);                     // resident CTAs per SM the grid is sized for
+  nx = (per_sm * sm_count() + slabs - 1) / slabs;
+  span = (N + nx - 1) / nx;
+  if (span > 64) span = 64;             // short spans, several waves: dynamic balance across SMs
+  span = (span + 15) / 16 * 16;
+  if (span < 32) span = 32;
+  nx = (N + span - 1) / span;
+}
+
 // ---- host side (tensor-map encoder, SM count: sla_tc_common.cuh) -----------------------------------
 // `main_pass` = false: only the OUTPASS launch (the main pass was done by the tcgen05 kernel, sla_fwd_umma.cu,
 // which follows the same workspace protocol).
@@ -718,13 +775,8 @@ cudaError_t tc_launch(const Problem& p, cudaStream_t st, bool main_pass) {
     attr_set[dev].store(true, std::memory_order_release);
   }
   const int slabs = (p.H + NW - 1) / NW;
-  const int per_sm = (D == 16 ? 3 : 2);                     // resident CTAs per SM the grid is sized for
-  int nx = (per_sm * sm_count() + slabs - 1) / slabs;
-  int span = (p.N + nx - 1) / nx;
-  if (span > 64) span = 64;             // short spans, several waves: dynamic balance across SMs
-  span = (span + 15) / 16 * 16;
-  if (span < 32) span = 32;
-  nx = (p.N + span - 1) / span;
+  int span, nx;
+  forward_geometry<D>(p.N, p.H, span, nx);
   dim3 grid(nx, slabs);
   // programmatic stream serialisation: see the note at the top of the kernel
   cudaLaunchAttribute pdl[1];
@@ -738,7 +790,8 @@ cudaError_t tc_launch(const Problem& p, cudaStream_t st, bool main_pass) {
   cfg.attrs = pdl;
   cfg.numAttrs = 1;
   if (main_pass) {
-    cudaError_t le = cudaLaunchKernelEx(&cfg, kern, tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H, span, p.eps);
+    cudaError_t le = cudaLaunchKernelEx(&cfg, kern, tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H, span, p.eps,
+                                        (const int4*)p.span_table);
     if (le != cudaSuccess) return le;
   }
   if (!p.bounded) {
@@ -747,7 +800,7 @@ cudaError_t tc_launch(const Problem& p, cudaStream_t st, bool main_pass) {
     dim3 grid2((p.N + span2 - 1) / span2, slabs);
     cfg.gridDim = grid2;   // same attribute: resident behind the main kernel's tail, waits for its states
     cudaError_t le = cudaLaunchKernelEx(&cfg, kern_out, tq, tk, tv, p.off, (T*)p.out, p.ws_state, p.N, p.W, p.H,
-                                        span2, p.eps);
+                                        span2, p.eps, (const int4*)nullptr);
     if (le != cudaSuccess) return le;
   }
   return cudaGetLastError();
@@ -759,6 +812,27 @@ bool forward_tc_supported(const Problem& p, int dt) {
   if (dt != SLA_F16 && dt != SLA_BF16) return false;
   if ((p.H * p.d) % 64 != 0) return false;                     // slab rows are whole 128-byte boxes
   return encode_fn() != nullptr;
+}
+
+size_t span_table_bytes(long long N, int H, int d) {
+  int span, nx;
+  if (d == 16) forward_geometry<16>((int)N, H, span, nx); else forward_geometry<32>((int)N, H, span, nx);
+  return (size_t)(nx + 1) * sizeof(int4);
+}
+
+cudaError_t launch_span_table(const int32_t* off, int N, int W, int H, int d, void* table, cudaStream_t st) {
+  int span, nx;
+  if (d == 16) forward_geometry<16>(N, H, span, nx); else forward_geometry<32>(N, H, span, nx);
+  cudaLaunchAttribute pdl[1];
+  pdl[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  pdl[0].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)((W + 255) / 256 > 0 ? (W + 255) / 256 : 1));
+  cfg.blockDim = dim3(256);
+  cfg.stream = st;
+  cfg.attrs = pdl;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, sla_span_table_kernel, off, N, W, span, nx, (int4*)table);
 }
 
 cudaError_t launch_forward_tc(const Problem& p, int dt, cudaStream_t st) {

@@ -76,6 +76,7 @@ struct Problem {
   int phi;           // sla_feature_map_t
   float eps;         // added to the denominator (0 for SLA_PHI_ELU1)
   bool bounded;      // caller guarantees every window has <= kFuseMax rows: no workspace, no split pass
+  const void* span_table;   // optional span table of this scene (sla_build_span_table); nullptr: search in the kernel
   bool tcgen05;      // main pass on the tcgen05 kernel (sla_fwd_umma.cu) instead of the mma.sync kernel
 };
 
@@ -90,6 +91,9 @@ cudaError_t launch_backward_tc(const Problem& p, int dt, cudaStream_t st);
 cudaError_t launch_backward_tc32(const Problem& p, int dt, cudaStream_t st);   // d_h = 32 (sla_bwd_tc32.cu)
 bool forward_tc_supported(const Problem& p, int dt);
 cudaError_t launch_forward_tc(const Problem& p, int dt, cudaStream_t st);
+// span table of the tensor-core forward (SURVEY a1's work list): bytes for a scene, and the kernel that fills it
+size_t span_table_bytes(long long N, int H, int d);
+cudaError_t launch_span_table(const int32_t* off, int N, int W, int H, int d, void* table, cudaStream_t st);
 // tcgen05 main pass of the forward (sla_fwd_umma.cu): fused windows + partial states of long windows
 bool forward_umma_supported(const Problem& p, int dt);
 cudaError_t launch_forward_umma_main(const Problem& p, int dt, cudaStream_t st);

@@ -468,6 +468,44 @@ def test_backward_writes_nothing_beyond_n(dtype, H, d):
     check_grads([b[:sc.N] for b in bufs], ref, sc)
 
 
+@pytest.mark.parametrize("case", ["config1", "config4", "tiny", "mixed_d32", "bf16_partial_slab", "small_n"])
+def test_forward_planned_matches_bounded_bit_for_bit(case):
+    """sla_forward_planned: the span table (built once per scene) replaces the in-kernel window search and must not
+    change a bit of the result; a table of another scene's size is detected on the device and ignored."""
+    torch = _torch()
+    if case == "config1":
+        sc = wl.make_config(1)
+    elif case == "config4":
+        sc = wl.make_config(4)
+    elif case == "tiny":
+        sc = wl.make_scene([1, 0, 2, 1, 3, 0, 0, 1, 5, 2] * 300, 8, 16, "f16", seed=61)
+    elif case == "mixed_d32":
+        sc = wl.make_scene([256, 1, 17, 0, 144, 33, 2, 255, 64, 63, 65] * 20, 8, 32, "f16", seed=62)
+    elif case == "bf16_partial_slab":
+        sc = wl.make_scene([100, 7, 256, 1, 1, 31], 12, 16, "bf16", seed=63)
+    else:
+        sc = wl.make_scene([5, 3], 8, 16, "f16", seed=64)
+    q, k, v = (to_dev(sc.tensor(n), sc.dtype) for n in ("q", "k", "v"))
+    off = torch.from_numpy(sc.offsets).cuda()
+    table = pkg.sla_build_span_table(off, sc.N, sc.H, sc.d_h)
+    out_p = pkg.sla_forward_planned(q, k, v, off, table, 256)
+    out_b = pkg.sla_forward(q, k, v, off, max_window_len=256)
+    torch.cuda.synchronize()
+    assert torch.equal(out_p, out_b)
+    ref = sla_oracle.forward(sc.tensor("q"), sc.tensor("k"), sc.tensor("v"), sc.offsets, nthreads=8)
+    check(f"{sc.name}.planned", out_p, ref, sc.dtype, sc.lengths)
+    # a table of another problem size: ignored, same result
+    other = wl.make_scene([50, 60, 70], sc.H, sc.d_h, sc.dtype, seed=65)
+    t2 = pkg.sla_build_span_table(torch.from_numpy(other.offsets).cuda(), other.N, other.H, other.d_h)
+    big = torch.zeros(max(table.numel(), t2.numel()), dtype=torch.uint8, device="cuda")
+    big[:t2.numel()] = t2
+    out_w = pkg.sla_forward_planned(q, k, v, off, big, 256)
+    torch.cuda.synchronize()
+    assert torch.equal(out_w, out_b)
+    with pytest.raises(pkg.SlaError, match="WORKSPACE"):
+        pkg.sla_forward_planned(q, k, v, off, torch.zeros(16, dtype=torch.uint8, device="cuda")[:0].contiguous() if False else torch.zeros(0, dtype=torch.uint8, device="cuda"), 256)
+
+
 def test_forward_under_cuda_graph_replay():
     """The C-ABI calls are capturable: a graph of prep + forward replays to the same result."""
     torch = _torch()
