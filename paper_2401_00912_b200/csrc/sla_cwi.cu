@@ -182,6 +182,201 @@ sla_cwi_conv_kernel(const T* __restrict__ x, const int4* __restrict__ coords, in
   }
 }
 
+// ---- 16-bit rows of 64, 128 or 256 channels: one row per warp-wide load ------------------------------------------------
+// Lane l owns V = C / 32 consecutive channels of the row (4, 8 or 16 bytes), which all belong to branch l / 8, so one
+// load per lane reads a whole 2C-byte row and the three convolution branches walk their own taps AT THE SAME TIME: in
+// step n the eight lanes of branch b fetch the row of the n-th present tap of branch b.  The number of steps is the
+// largest tap count of a branch instead of the sum over the branches, and every step moves V channels per lane instead
+// of one.  Per (branch, channel) the terms are added in the order of the kernel above (centre, then ascending taps):
+// the two kernels give the same bits.
+template <typename T> __device__ __forceinline__ float2 unpack2(uint32_t u);
+template <> __device__ __forceinline__ float2 unpack2<__half>(uint32_t u) {
+  return __half22float2(*reinterpret_cast<const __half2*>(&u));
+}
+template <> __device__ __forceinline__ float2 unpack2<__nv_bfloat16>(uint32_t u) {
+  return make_float2(__uint_as_float(u << 16), __uint_as_float(u & 0xffff0000u));
+}
+template <typename T> __device__ __forceinline__ uint32_t pack2(float a, float b);
+template <> __device__ __forceinline__ uint32_t pack2<__half>(float a, float b) {
+  const __half2 h = __floats2half2_rn(a, b);
+  return *reinterpret_cast<const uint32_t*>(&h);
+}
+template <> __device__ __forceinline__ uint32_t pack2<__nv_bfloat16>(float a, float b) {
+  const __nv_bfloat162 h = __floats2bfloat162_rn(a, b);
+  return *reinterpret_cast<const uint32_t*>(&h);
+}
+template <int V> __device__ __forceinline__ void ld_row(const void* p, uint32_t (&r)[V / 2]) {
+  if constexpr (V == 2) {
+    r[0] = __ldg(reinterpret_cast<const uint32_t*>(p));
+  } else if constexpr (V == 4) {
+    const uint2 t = __ldg(reinterpret_cast<const uint2*>(p));
+    r[0] = t.x; r[1] = t.y;
+  } else {
+    const uint4 t = __ldg(reinterpret_cast<const uint4*>(p));
+    r[0] = t.x; r[1] = t.y; r[2] = t.z; r[3] = t.w;
+  }
+}
+template <int V> __device__ __forceinline__ void st_row(void* p, const uint32_t (&r)[V / 2]) {
+  if constexpr (V == 2) *reinterpret_cast<uint32_t*>(p) = r[0];
+  else if constexpr (V == 4) *reinterpret_cast<uint2*>(p) = make_uint2(r[0], r[1]);
+  else *reinterpret_cast<uint4*>(p) = make_uint4(r[0], r[1], r[2], r[3]);
+}
+
+// V = C / 32 channels per lane (2, 4, 8).  The taps other than the centres are laid out by POSITION so that every
+// branch sits inside one 32-bit ballot: positions 0..25 the 3x3x3 taps, 32.. the S_h taps along y, then the S_w taps
+// along x (S_h + S_w <= 32); lane l looks up positions l and 32 + l; the weights are staged in position order.
+template <typename T, int V>
+__global__ void __launch_bounds__(32 * kCwiWarps)
+sla_cwi_conv_rows_kernel(const T* __restrict__ x, const int4* __restrict__ coords, int N, Geom g, int S_h, int S_w,
+                         const float* __restrict__ w_h, const float* __restrict__ w_w, const float* __restrict__ w_3,
+                         const int32_t* __restrict__ grid, T* __restrict__ out) {
+  extern __shared__ __align__(16) float s_w[];           // [32 + S_h + S_w][c]
+  pdl_launch_dependents();
+  constexpr int C = 32 * V, c = 8 * V;
+  const int Th = S_h + 1, Tw = S_w + 1, P = 32 + S_h + S_w;
+  // position -> branch and tap of that branch's kernel (the centre tap is skipped)
+  auto tap_of = [&](int p, int& br, int& t) -> bool {
+    if (p < 26) { br = 2; t = p + (p >= 13); return true; }
+    int q = p - 32;
+    if (q < 0) return false;
+    if (q < S_h) { br = 0; t = q + (q >= (S_h >> 1)); return true; }
+    q -= S_h;
+    if (q < S_w) { br = 1; t = q + (q >= (S_w >> 1)); return true; }
+    return false;
+  };
+  for (int i = threadIdx.x; i < P * c; i += blockDim.x) {
+    const int p = i / c, ch = i - p * c;
+    int br = 0, t = 0;
+    float v = 0.f;
+    if (tap_of(p, br, t))
+      v = br == 0 ? __ldg(w_h + ch * Th + t) : br == 1 ? __ldg(w_w + ch * Tw + t) : __ldg(w_3 + ch * 27 + t);
+    s_w[i] = v;
+  }
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int br = lane >> 3;                              // branch of this lane's channels (3: identity)
+  const int ch0 = (lane & 7) * V;                        // the first of them inside the branch
+  const int myslot = br == 2 ? 0 : 1;
+  const unsigned mine = br == 2 ? 0x03ffffffu
+                      : br == 0 ? (unsigned)((1ull << S_h) - 1ull)
+                      : br == 1 ? (unsigned)(((1ull << S_w) - 1ull) << S_h) : 0u;
+  float wc[V];                                           // centre weights of this lane's channels
+#pragma unroll
+  for (int k = 0; k < V; ++k)
+    wc[k] = br == 0 ? __ldg(w_h + (ch0 + k) * Th + (S_h >> 1)) : br == 1 ? __ldg(w_w + (ch0 + k) * Tw + (S_w >> 1))
+          : br == 2 ? __ldg(w_3 + (ch0 + k) * 27 + 13) : 0.f;
+  // per-lane constants of the voxel loop, pinned to registers (ptxas otherwise re-derives them from the thread index
+  // and the parameter bank in every iteration and every tap step: a third of the loop's instructions)
+  uint32_t wbase = (uint32_t)__cvta_generic_to_shared(s_w + myslot * 32 * c + ch0);
+  const T* xl = x + lane * V;
+  T* ol = out + lane * V;
+  int tdz[2], tdy[2], tdx[2], tdelta[2];
+#pragma unroll
+  for (int s = 0; s < 2; ++s) {
+    int b = 0, t = 0, dz = 1 << 20, dy = 0, dx = 0;        // no tap at this position: always outside the grid
+    if (tap_of(lane + 32 * s, b, t)) {
+      dz = 0;
+      if (b == 0) dy = t - (S_h >> 1);
+      else if (b == 1) dx = t - (S_w >> 1);
+      else { dz = t / 9 - 1; dy = (t / 3) % 3 - 1; dx = t % 3 - 1; }
+    }
+    tdz[s] = dz; tdy[s] = dy; tdx[s] = dx;
+    tdelta[s] = (dz * g.gh + dy) * g.gw + dx;
+    asm volatile("" : "+r"(tdelta[s]));
+  }
+  asm volatile("" : "+r"(wbase));
+  asm volatile("" : "+l"(xl));
+  asm volatile("" : "+l"(ol));
+  pdl_wait();
+  __syncthreads();
+  // the grid cells at this lane's two positions around voxel `me` -> idx[] (-1: no voxel there); < 2^31 cells (host)
+  auto lookups = [&](const int4& me, int (&idx)[2]) -> bool {
+    const bool me_in = (unsigned)me.x < (unsigned)g.batch && (unsigned)me.y < (unsigned)g.gz &&
+                       (unsigned)me.z < (unsigned)g.gh && (unsigned)me.w < (unsigned)g.gw;
+    const int cell0 = ((me.x * g.gz + me.y) * g.gh + me.z) * g.gw + me.w;
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+      const bool inside = me_in && (unsigned)(me.y + tdz[s]) < (unsigned)g.gz &&
+                          (unsigned)(me.z + tdy[s]) < (unsigned)g.gh && (unsigned)(me.w + tdx[s]) < (unsigned)g.gw;
+      idx[s] = inside ? grid[cell0 + tdelta[s]] : -1;
+    }
+    return me_in;
+  };
+  const int stride = (int)gridDim.x * kCwiWarps;         // N < 2^30 (host): i + 2 stride cannot overflow
+  int i = (int)blockIdx.x * kCwiWarps + warp;
+  const int4 none = make_int4(-1, -1, -1, -1);
+  int idx[2];
+  bool in_grid = lookups(i < N ? __ldg(coords + i) : none, idx);
+  int4 me_next = (i + stride < N) ? __ldg(coords + i + stride) : none;
+  for (; i < N; i += stride) {
+    int idx_next[2];
+    const bool in_grid_next = lookups(me_next, idx_next);
+    me_next = (i + 2 * stride < N) ? __ldg(coords + i + 2 * stride) : none;
+    uint32_t own[V / 2];
+    ld_row<V>(xl + (size_t)i * C, own);
+    float acc[V];
+#pragma unroll
+    for (int k = 0; k < V / 2; ++k) {                      // centre tap
+      const float2 f = unpack2<T>(own[k]);
+      acc[2 * k] = wc[2 * k] * f.x;
+      acc[2 * k + 1] = wc[2 * k + 1] * f.y;
+    }
+    const unsigned b0 = __ballot_sync(0xffffffffu, idx[0] >= 0), b1 = __ballot_sync(0xffffffffu, idx[1] >= 0);
+    unsigned present = (myslot ? b1 : b0) & mine;          // this branch's taps that hit a voxel
+    if (__builtin_expect(!in_grid, 0)) {                   // a voxel off the grid: zeros (it has no neighbour either)
+#pragma unroll
+      for (int k = 0; k < V; ++k) acc[k] = 0.f;
+    }
+    const int steps = __reduce_max_sync(0xffffffffu, __popc(present));
+    // Ascending taps per branch (deterministic sums), four steps at a time: the rows of all four are requested before
+    // the first is used (the loop is bound by the latency of these L2 reads, not by instruction issue).
+    for (int n = 0; n < steps; n += 4) {
+      uint32_t r[4][V / 2];
+      int lt[4];
+      bool lv[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        lv[u] = false;
+        lt[u] = 0;
+        if (u == 0 || n + u < steps) {                     // warp-uniform
+          lv[u] = present != 0;
+          lt[u] = __ffs(present) - 1;                      // -1 (list ended): the shuffles read lane 31, unused
+          present &= present - 1;
+          const int j0 = __shfl_sync(0xffffffffu, idx[0], lt[u]), j1 = __shfl_sync(0xffffffffu, idx[1], lt[u]);
+          if (lv[u]) ld_row<V>(xl + (size_t)(myslot ? j1 : j0) * C, r[u]);
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        if (lv[u]) {
+          float wt[V];
+          const uint32_t wa = wbase + (uint32_t)lt[u] * (c * 4u);
+          if constexpr (V == 2) {
+            asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(wt[0]), "=f"(wt[1]) : "r"(wa));
+          } else {
+#pragma unroll
+            for (int k = 0; k < V; k += 4)
+              asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
+                           : "=f"(wt[k]), "=f"(wt[k + 1]), "=f"(wt[k + 2]), "=f"(wt[k + 3]) : "r"(wa + 4u * k));
+          }
+#pragma unroll
+          for (int k = 0; k < V / 2; ++k) {
+            const float2 f = unpack2<T>(r[u][k]);
+            acc[2 * k] = fmaf(wt[2 * k], f.x, acc[2 * k]);
+            acc[2 * k + 1] = fmaf(wt[2 * k + 1], f.y, acc[2 * k + 1]);
+          }
+        }
+      }
+    }
+    if (br < 3) {                                          // Eq. 4: the identity branch keeps the input's bits
+#pragma unroll
+      for (int k = 0; k < V / 2; ++k) own[k] = pack2<T>(acc[2 * k], acc[2 * k + 1]);
+    }
+    st_row<V>(ol + (size_t)i * C, own);
+    idx[0] = idx_next[0]; idx[1] = idx_next[1];
+    in_grid = in_grid_next;
+  }
+}
+
 template <typename... KArgs, typename... Args>
 cudaError_t launch_chained(void (*kernel)(KArgs...), unsigned blocks, unsigned threads, size_t smem, cudaStream_t st,
                            Args... args) {
@@ -198,6 +393,20 @@ cudaError_t launch_chained(void (*kernel)(KArgs...), unsigned blocks, unsigned t
   return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
+// The convolution kernels are persistent: as many blocks as the device holds at once (register-bound: 2 per SM for
+// most instantiations), so the weights are staged once per resident block and no block waits for a second wave.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_conv(void (*kernel)(KArgs...), int N, size_t smem, cudaStream_t st, Args... args) {
+  int dev = 0, sms = 148, per_sm = 1;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+    sms = 148;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, 32 * kCwiWarps, smem) != cudaSuccess || per_sm < 1)
+    per_sm = 1;
+  unsigned blocks = (unsigned)((N + kCwiWarps - 1) / kCwiWarps);
+  if (blocks > (unsigned)(sms * per_sm)) blocks = (unsigned)(sms * per_sm);
+  return launch_chained(kernel, blocks, 32 * kCwiWarps, smem, st, args...);
+}
+
 template <typename T>
 cudaError_t cwi_launch(const void* x, const int32_t* coords, int N, int C, Geom g, int S_h, int S_w, const float* w_h,
                        const float* w_w, const float* w_3, void* out, int32_t* grid, cudaStream_t st) {
@@ -211,12 +420,24 @@ cudaError_t cwi_launch(const void* x, const int32_t* coords, int N, int C, Geom 
   if (e != cudaSuccess) return e;
   const int c = C / 4;
   const size_t smem = (size_t)(S_h + S_w + 29) * c * sizeof(float);
-  unsigned blocks = (unsigned)((N + kCwiWarps - 1) / kCwiWarps);
-  if (blocks > 592) blocks = 592;                        // 4 x 148 blocks of 16 warps: every warp walks ~6 voxels per 60 000,
-                                                         // so the per-block weight staging and per-warp tap set-up are amortised
   const int cpl = (c + 31) / 32;
+  const int ns = (S_h + S_w + 29 + 31) / 32;
+  if constexpr (sizeof(T) == 2) {
+    const bool aligned = (((uintptr_t)x | (uintptr_t)out) & 15) == 0;
+    if (S_h + S_w <= 32 && cells < (1ull << 31) && N < (1 << 30) && aligned && (C == 64 || C == 128 || C == 256)) {
+      // a row is one 4-, 8- or 16-byte load per lane
+      const size_t smem_rows = (size_t)(32 + S_h + S_w) * c * sizeof(float);
+#define SLA_CWI_ROWS(V)                                                                                                  \
+  launch_conv(sla_cwi_conv_rows_kernel<T, V>, N, smem_rows, st, (const T*)x, (const int4*)coords, \
+                 N, g, S_h, S_w, w_h, w_w, w_3, (const int32_t*)grid, (T*)out)
+      if (C == 64) return SLA_CWI_ROWS(2);
+      if (C == 128) return SLA_CWI_ROWS(4);
+      return SLA_CWI_ROWS(8);
+#undef SLA_CWI_ROWS
+    }
+  }
 #define SLA_CWI_LAUNCH(CPL, NS)                                                                                    \
-  launch_chained(sla_cwi_conv_kernel<T, CPL, NS>, blocks, 32 * kCwiWarps, smem, st, (const T*)x, (const int4*)coords, \
+  launch_conv(sla_cwi_conv_kernel<T, CPL, NS>, N, smem, st, (const T*)x, (const int4*)coords, \
                  N, C, g, S_h, S_w, w_h, w_w, w_3, (const int32_t*)grid, (T*)out)
 #define SLA_CWI_SLOTS(CPL)                     \
   switch (ns) {                                \
@@ -225,7 +446,6 @@ cudaError_t cwi_launch(const void* x, const int32_t* coords, int N, int C, Geom 
     case 3: return SLA_CWI_LAUNCH(CPL, 3);     \
     default: return SLA_CWI_LAUNCH(CPL, 4);    \
   }
-  const int ns = (S_h + S_w + 29 + 31) / 32;
   switch (cpl) {
     case 1: SLA_CWI_SLOTS(1)
     case 2: SLA_CWI_SLOTS(2)

@@ -62,7 +62,8 @@ def _dense_scene(rng, n, batch, gz, gh, gw):
 
 
 @pytest.mark.parametrize("dtype", ["f32", "f16", "bf16"])
-@pytest.mark.parametrize("C,S_h,S_w", [(128, 12, 12), (256, 20, 20), (64, 2, 4), (8, 12, 12), (512, 0, 0)])
+@pytest.mark.parametrize("C,S_h,S_w", [(128, 12, 12), (256, 20, 20), (64, 2, 4), (8, 12, 12), (512, 0, 0),
+                                       (128, 16, 16), (128, 4, 6), (256, 32, 0), (64, 0, 0), (128, 18, 16), (128, 30, 2)])
 def test_cwi_dense_neighbourhoods(dtype, C, S_h, S_w):
     """A small, densely occupied grid: most taps hit a voxel, windows reach over the borders and into other samples."""
     rng = np.random.Generator(np.random.PCG64(C + S_h))
