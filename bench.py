@@ -343,7 +343,7 @@ def sequence_prep_leg(pkg, torch, dev, peak):
     gather_us = timed(lambda: pkg.sla_gather_rows(x, perm, out=y))
     nb = 2 * x.numel() * 2 + 4 * N
     return {"N": N, "W": pkg.sla_window_count(batch, grid, grid, win, win),
-            "sequence_from_coords_us": seq_us, "kernels_per_call": 6,
+            "sequence_from_coords_us": seq_us, "kernels_per_call": 2,
             "gather_rows_us": gather_us, "gather_algorithmic_bytes": nb,
             "gather_frac_of_peak": nb / (gather_us * 1e-6) / 1e9 / peak,
             "timing": "median of 40 eager calls, one event pair per call (includes the binding's launch path), cold L2"}

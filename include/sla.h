@@ -232,7 +232,9 @@ int sla_scatter_rows(const void* src, const int32_t* perm, int64_t N, size_t row
 /* The three steps in one call: keys -> stable sort -> offsets.
  *   perm, key_sorted  DEV int32[N] out (as above)        window_offsets  DEV int32[W+1] out, W = sla_window_count(...)
  *   workspace         DEV, >= sla_sequence_workspace_bytes(N) bytes, 16-byte aligned, scratch
- * off[W] is the number of voxels inside the grid: pass that as N to sla_forward when some voxels lie outside. */
+ * off[W] is the number of voxels inside the grid: pass that as N to sla_forward when some voxels lie outside.
+ * With W + 1 <= 2048 (a single frame) the call is a counting sort in one pass -- two kernels, the offsets fall out of its
+ * scan -- instead of keys + radix passes + offsets; same results bit for bit. */
 size_t sla_sequence_workspace_bytes(int64_t N);
 int sla_sequence_from_coords(const int32_t* coords, int64_t N, int32_t batch, int32_t grid_h, int32_t grid_w,
                              int32_t S_h, int32_t S_w, int32_t* perm, int32_t* key_sorted, int32_t* window_offsets,

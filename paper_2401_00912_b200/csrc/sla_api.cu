@@ -149,6 +149,14 @@ int sla_sequence_from_coords(const int32_t* coords, int64_t N, int32_t batch, in
     return SLA_ERR_WORKSPACE;
   cudaStream_t st = (cudaStream_t)stream;
   int32_t* key = static_cast<int32_t*>(workspace);
+  if (sla::sequence_onepass_fits(N, W, N > 0 ? sla::sort_workspace_bytes(N) : 0)) {
+    // one scene (W + 1 <= 2048 bins, >= ~1000 voxels so that the counts fit the radix sort's scratch): counting sort in
+    // one pass, offsets out of its scan
+    cudaError_t e1 = sla::launch_sequence_onepass(coords, (int)N, batch, grid_h, grid_w, S_h, S_w, key,
+                                                  static_cast<char*>(workspace) + key_bytes, perm, key_sorted,
+                                                  window_offsets, st);
+    return e1 == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
+  }
   if (N > 0) {
     if (sla::launch_window_keys(coords, (int)N, batch, grid_h, grid_w, S_h, S_w, key, st) != cudaSuccess) return SLA_ERR_CUDA;
     if (sla::launch_sort_by_key(key, (int)N, (int)W, perm, key_sorted, static_cast<char*>(workspace) + key_bytes, st) != cudaSuccess)

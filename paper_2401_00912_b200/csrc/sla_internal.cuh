@@ -102,6 +102,10 @@ cudaError_t launch_forward_umma_main(const Problem& p, int dt, cudaStream_t st);
 size_t sort_workspace_bytes(long long N);
 cudaError_t launch_window_keys(const int32_t* coords, int N, int batch, int grid_h, int grid_w, int S_h, int S_w,
                                int32_t* key, cudaStream_t st);
+bool sequence_onepass_fits(long long N, long long W, size_t scratch);
+cudaError_t launch_sequence_onepass(const int32_t* coords, int N, int batch, int grid_h, int grid_w, int S_h, int S_w,
+                                    int32_t* key, void* cnt, int32_t* perm, int32_t* key_sorted, int32_t* off,
+                                    cudaStream_t st);
 cudaError_t launch_sort_by_key(const int32_t* key, int N, int W, int32_t* perm, int32_t* key_sorted, void* ws,
                                cudaStream_t st);
 cudaError_t launch_permute_rows(const void* src, const int32_t* perm, long long N, size_t row_bytes, void* dst,

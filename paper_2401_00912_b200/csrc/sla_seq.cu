@@ -202,6 +202,143 @@ sla_sort_scatter_kernel(const int32_t* __restrict__ key_in, const int32_t* __res
   }
 }
 
+// ---- one scene: counting sort in one pass ------------------------------------------------------------------------------
+// A single frame has W = 1521 windows (468 x 468 cells in 12 x 12 windows): the key itself is the only digit.  Two
+// kernels instead of six (keys, 2 x (hist, scatter), offsets):
+//   count   keys of a tile of 1024 voxels -> key[], their histogram over the W + 1 bins -> cnt[block][bin] (uint16)
+//   place   every block sums the rows before it and all rows (thread = 8 consecutive bins = one 16-byte load per row),
+//           scans the totals -- which ARE the window offsets: block 0 writes them --, ranks its keys warp by warp
+//           and step by step as the radix scatter does (stable), and writes perm / key_sorted
+constexpr int kSeqBins = 2048;                           // W + 1 <= kSeqBins
+constexpr int kSeqSteps = 4;
+constexpr int kSeqTile = 32 * kSortWarps * kSeqSteps;    // 1024 voxels per block
+static_assert(kSeqBins == 8 * 32 * kSortWarps, "a thread owns 8 consecutive bins");
+
+__global__ void __launch_bounds__(32 * kSortWarps)
+sla_seq_count_kernel(const int4* __restrict__ coords, int N, int batch, int grid_h, int grid_w, int S_h, int S_w,
+                     int nwy, int nwx, int W, int32_t* __restrict__ key, uint16_t* __restrict__ cnt) {
+  __shared__ uint32_t h[kSeqBins];
+  pdl_launch_dependents();
+#pragma unroll
+  for (int j = 0; j < kSeqBins / (32 * kSortWarps); ++j) h[threadIdx.x + j * 32 * kSortWarps] = 0;
+  __syncthreads();
+  pdl_wait();
+  const long long base = (long long)blockIdx.x * kSeqTile;
+#pragma unroll
+  for (int s = 0; s < kSeqSteps; ++s) {
+    const long long i = base + s * (32 * kSortWarps) + threadIdx.x;
+    if (i < N) {
+      const int4 c = __ldg(coords + i);                  // (b, z, y, x); z takes no part
+      const bool inside = (unsigned)c.x < (unsigned)batch && (unsigned)c.z < (unsigned)grid_h &&
+                          (unsigned)c.w < (unsigned)grid_w;
+      const int kk = inside ? (c.x * nwy + c.z / S_h) * nwx + c.w / S_w : W;
+      key[i] = kk;
+      atomicAdd(&h[kk], 1u);
+    }
+  }
+  __syncthreads();
+  const uint32_t* m = h + 8 * threadIdx.x;               // counts <= 1024: 16 bits each
+  reinterpret_cast<uint4*>(cnt + (size_t)blockIdx.x * kSeqBins)[threadIdx.x] =
+      make_uint4(m[0] | (m[1] << 16), m[2] | (m[3] << 16), m[4] | (m[5] << 16), m[6] | (m[7] << 16));
+}
+
+__global__ void __launch_bounds__(32 * kSortWarps)
+sla_seq_place_kernel(const int32_t* __restrict__ key_in, int N, int W, int T, const uint16_t* __restrict__ cnt,
+                     int32_t* __restrict__ perm, int32_t* __restrict__ key_sorted, int32_t* __restrict__ off) {
+  __shared__ __align__(16) uint16_t rel[kSortWarps][kSeqBins];   // per warp: count, then start behind the warps before
+  __shared__ uint32_t basepos[kSeqBins];                         // start of this block's keys of a bin in the output
+  __shared__ uint32_t warp_sum[kSortWarps];
+  pdl_launch_dependents();
+  {
+    uint4* z = reinterpret_cast<uint4*>(&rel[0][0]);
+#pragma unroll
+    for (int j = 0; j < (int)(sizeof(rel) / 16) / (32 * kSortWarps); ++j)
+      z[threadIdx.x + j * 32 * kSortWarps] = make_uint4(0, 0, 0, 0);
+  }
+  __syncthreads();
+  pdl_wait();
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const long long base = (long long)blockIdx.x * kSeqTile + warp * (32 * kSeqSteps);
+  int kk[kSeqSteps];
+#pragma unroll
+  for (int s = 0; s < kSeqSteps; ++s) {
+    const long long i = base + s * 32 + lane;
+    kk[s] = i < N ? key_in[i] : kSeqBins;                 // past the end: a group of its own that is never counted
+  }
+#pragma unroll
+  for (int s = 0; s < kSeqSteps; ++s) {
+    const unsigned grp = __match_any_sync(0xffffffffu, kk[s]);
+    if (kk[s] < kSeqBins && lane == __ffs(grp) - 1) rel[warp][kk[s]] += (uint16_t)__popc(grp);
+    __syncwarp();
+  }
+  // bins 8 tid .. 8 tid + 7: keys in the blocks before this one, and in all blocks
+  uint32_t before[8], all[8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) before[j] = all[j] = 0;
+  const uint4* rows = reinterpret_cast<const uint4*>(cnt) + threadIdx.x;
+  auto add_row = [&](const uint4& r, uint32_t (&acc)[8]) {
+    acc[0] += r.x & 0xffffu; acc[1] += r.x >> 16; acc[2] += r.y & 0xffffu; acc[3] += r.y >> 16;
+    acc[4] += r.z & 0xffffu; acc[5] += r.z >> 16; acc[6] += r.w & 0xffffu; acc[7] += r.w >> 16;
+  };
+  constexpr int kRowsInFlight = 16;                      // the rows come out of L2 one latency per batch, not per row
+  for (int t0 = 0; t0 < T; t0 += kRowsInFlight) {
+    uint4 r[kRowsInFlight];
+#pragma unroll
+    for (int u = 0; u < kRowsInFlight; ++u)               // plain loads: the count kernel wrote them
+      r[u] = t0 + u < T ? rows[(size_t)(t0 + u) * (kSeqBins / 8)] : make_uint4(0, 0, 0, 0);
+#pragma unroll
+    for (int u = 0; u < kRowsInFlight; ++u) {
+      if (t0 + u < (int)blockIdx.x) add_row(r[u], before);
+      else add_row(r[u], all);
+    }
+  }
+  uint32_t mine = 0;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) { all[j] += before[j]; mine += all[j]; }
+  uint32_t inc = mine;                                   // block-wide exclusive scan of the bin totals
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint32_t up = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += up;
+  }
+  if (lane == 31) warp_sum[warp] = inc;
+  __syncthreads();                                       // also: every warp's counts are in rel[][]
+  uint32_t ex = inc - mine;
+  for (int w = 0; w < warp; ++w) ex += warp_sum[w];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    const int d = 8 * threadIdx.x + j;
+    if (blockIdx.x == 0 && d <= W) off[d] = (int32_t)ex;  // keys below d = first row of window d; off[W] = voxels inside
+    basepos[d] = ex + before[j];
+    ex += all[j];
+  }
+  {
+    // counts -> starts behind the warps before, for this thread's 8 bins at once (packed 16-bit pairs: a pair of
+    // counts sums to <= 1024, no carry between the halves)
+    uint4 run = make_uint4(0, 0, 0, 0);
+#pragma unroll
+    for (int w = 0; w < kSortWarps; ++w) {
+      uint4* at = reinterpret_cast<uint4*>(&rel[w][8 * threadIdx.x]);
+      const uint4 c = *at;
+      *at = run;
+      run.x += c.x; run.y += c.y; run.z += c.z; run.w += c.w;
+    }
+  }
+  __syncthreads();
+  const unsigned below = (1u << lane) - 1u;
+#pragma unroll
+  for (int s = 0; s < kSeqSteps; ++s) {
+    const bool valid = kk[s] < kSeqBins;
+    const unsigned grp = __match_any_sync(0xffffffffu, kk[s]);
+    uint32_t pos = 0;
+    if (valid) pos = basepos[kk[s]] + rel[warp][kk[s]] + __popc(grp & below);
+    __syncwarp();
+    if (valid && lane == __ffs(grp) - 1) rel[warp][kk[s]] += (uint16_t)__popc(grp);
+    __syncwarp();
+    if (valid) { key_sorted[pos] = kk[s]; perm[pos] = (int32_t)(base + s * 32 + lane); }
+  }
+}
+
 // dst[j] = src[perm[j]] (gather) or dst[perm[j]] = src[j] (scatter), rows of `vpr` vectors of type V.  A row
 // whose perm entry lies outside [0, N) is skipped, so a bad permutation cannot reach outside the buffers.
 // A thread moves kPermUnroll vectors, 256 apart, and has all its loads in flight before the first store.
@@ -312,6 +449,27 @@ cudaError_t launch_sort_by_key(const int32_t* key, int N, int W, int32_t* perm, 
     vin = vout;
   }
   return e;
+}
+
+// `scratch`: bytes available for the per-block counts
+bool sequence_onepass_fits(long long N, long long W, size_t scratch) {
+  if (N <= 0 || W + 1 > kSeqBins) return false;
+  const size_t T = (size_t)((N + kSeqTile - 1) / kSeqTile);
+  return T * kSeqBins * sizeof(uint16_t) <= scratch;
+}
+
+// cnt: ceil(N / 1024) rows of kSeqBins uint16 (4 bytes per voxel, 16-byte aligned)
+cudaError_t launch_sequence_onepass(const int32_t* coords, int N, int batch, int grid_h, int grid_w, int S_h, int S_w,
+                                    int32_t* key, void* cnt, int32_t* perm, int32_t* key_sorted, int32_t* off,
+                                    cudaStream_t st) {
+  const int nwy = (grid_h + S_h - 1) / S_h, nwx = (grid_w + S_w - 1) / S_w;
+  const int W = batch * nwy * nwx;
+  const int T = (int)(((long long)N + kSeqTile - 1) / kSeqTile);
+  cudaError_t e = launch_chained(sla_seq_count_kernel, T, 32 * kSortWarps, st, (const int4*)coords, N, batch, grid_h,
+                                 grid_w, S_h, S_w, nwy, nwx, W, key, (uint16_t*)cnt);
+  if (e != cudaSuccess) return e;
+  return launch_chained(sla_seq_place_kernel, T, 32 * kSortWarps, st, (const int32_t*)key, N, W, T,
+                        (const uint16_t*)cnt, perm, key_sorted, off);
 }
 
 cudaError_t launch_permute_rows(const void* src, const int32_t* perm, long long N, size_t row_bytes, void* dst,
