@@ -288,7 +288,8 @@ int sla_module_forward(const void* x, const void* w_qkv, const float* bias, cons
  *   x, out   DEV [N, C] of dt (fp32 / fp16 / bf16), distinct buffers        coords  DEV int32[N,4], 16-byte aligned
  *   w_h      DEV fp32 [c, S_h+1]     w_w  DEV fp32 [c, S_w+1]     w_3  DEV fp32 [c, 27]     (no bias)
  *   workspace DEV, >= sla_cwi_workspace_bytes(batch, grid_z, grid_h, grid_w) = 4 bytes per grid cell (the dense
- *            voxel-index grid, rebuilt by every call), 16-byte aligned, scratch
+ *            voxel-index grid) + 4 bytes per (b, y, x) column (occupancy words), 16-byte aligned, scratch: its
+ *            contents at entry do not matter and mean nothing afterwards
  * fp32 accumulation in tap order (deterministic), one rounding to dt.  C % 4 == 0, C <= 512, S_h + S_w <= 99, fewer
  * than 2^31 grid cells; otherwise SLA_ERR_UNSUPPORTED / SLA_ERR_INVALID_ARG.  Enqueues three kernels on `stream`. */
 size_t sla_cwi_workspace_bytes(int32_t batch, int32_t grid_z, int32_t grid_h, int32_t grid_w);

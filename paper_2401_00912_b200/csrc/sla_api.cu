@@ -206,7 +206,9 @@ static int64_t cwi_cells(int32_t batch, int32_t gz, int32_t gh, int32_t gw) {
 
 size_t sla_cwi_workspace_bytes(int32_t batch, int32_t grid_z, int32_t grid_h, int32_t grid_w) {
   const int64_t cells = cwi_cells(batch, grid_z, grid_h, grid_w);
-  return cells < 0 ? 0 : ((size_t)cells * 4 + 15) / 16 * 16;
+  if (cells < 0) return 0;
+  // the index grid (4 bytes per cell) + one occupancy word per (b, y, x) column
+  return ((size_t)cells * 4 + 15) / 16 * 16 + ((size_t)batch * grid_h * grid_w * 4 + 15) / 16 * 16;
 }
 
 int sla_cwi_forward(const void* x, const int32_t* coords, int64_t N, int32_t C, int dt, int32_t batch, int32_t grid_z,
@@ -223,7 +225,10 @@ int sla_cwi_forward(const void* x, const int32_t* coords, int64_t N, int32_t C, 
   if (!workspace || workspace_bytes < sla_cwi_workspace_bytes(batch, grid_z, grid_h, grid_w) || !aligned16(workspace))
     return SLA_ERR_WORKSPACE;
   cudaError_t e = sla::launch_cwi(x, coords, (int)N, C, dt, batch, grid_z, grid_h, grid_w, S_h, S_w, w_h, w_w, w_3, out,
-                                  static_cast<int32_t*>(workspace), (cudaStream_t)stream);
+                                  static_cast<int32_t*>(workspace),
+                                  reinterpret_cast<uint32_t*>(static_cast<char*>(workspace) +
+                                      ((size_t)cwi_cells(batch, grid_z, grid_h, grid_w) * 4 + 15) / 16 * 16),
+                                  (cudaStream_t)stream);
   return e == cudaSuccess ? SLA_OK : SLA_ERR_CUDA;
 }
 

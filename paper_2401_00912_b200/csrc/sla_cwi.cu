@@ -20,11 +20,11 @@ namespace {
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
-__global__ void __launch_bounds__(256) sla_cwi_fill_kernel(uint4* __restrict__ p, size_t n16) {
+__global__ void __launch_bounds__(256) sla_cwi_fill_kernel(uint4* __restrict__ p, size_t n16, unsigned word) {
   pdl_launch_dependents();
   pdl_wait();   // a previous call's conv kernel may still be reading the grid
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += (size_t)gridDim.x * blockDim.x)
-    p[i] = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
+    p[i] = make_uint4(word, word, word, word);
 }
 
 struct Geom { int batch, gz, gh, gw; };
@@ -35,15 +35,22 @@ __device__ __forceinline__ long long cell_of(const Geom& g, int b, int z, int y,
   return inside ? (((long long)b * g.gz + z) * g.gh + y) * g.gw + x : -1;
 }
 
+// zmask != nullptr (grid_z <= 32): one word per (b, y, x) column, bit z = "a voxel sits in cell z".  Then only this
+// word array is cleared per call (4 bytes per column instead of 4 bytes per cell) and a cell of the index grid is read
+// only where its bit is set, so whatever an earlier call or anybody else left in the other cells is never looked at.
 __global__ void __launch_bounds__(256)
-sla_cwi_scatter_kernel(const int4* __restrict__ coords, int N, Geom g, int32_t* __restrict__ grid) {
+sla_cwi_scatter_kernel(const int4* __restrict__ coords, int N, Geom g, int32_t* __restrict__ grid,
+                       uint32_t* __restrict__ zmask) {
   pdl_launch_dependents();
   pdl_wait();
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= N) return;
   const int4 c = __ldg(coords + i);                      // (b, z, y, x)
   const long long cell = cell_of(g, c.x, c.y, c.z, c.w);
-  if (cell >= 0) grid[cell] = (int)i;                    // a voxel outside the grid is seen by nobody
+  if (cell >= 0) {                                       // a voxel outside the grid is seen by nobody
+    grid[cell] = (int)i;
+    if (zmask != nullptr) atomicOr(zmask + ((long long)c.x * g.gh + c.z) * g.gw + c.w, 1u << c.y);
+  }
 }
 
 template <typename T> __device__ __forceinline__ float ld_elem(const T* p);
@@ -226,10 +233,10 @@ template <int V> __device__ __forceinline__ void st_row(void* p, const uint32_t 
 // branch sits inside one 32-bit ballot: positions 0..25 the 3x3x3 taps, 32.. the S_h taps along y, then the S_w taps
 // along x (S_h + S_w <= 32); lane l looks up positions l and 32 + l; the weights are staged in position order.
 template <typename T, int V>
-__global__ void __launch_bounds__(32 * kCwiWarps)
+__global__ void __launch_bounds__(32 * kCwiWarps, V == 8 ? 1 : 2)
 sla_cwi_conv_rows_kernel(const T* __restrict__ x, const int4* __restrict__ coords, int N, Geom g, int S_h, int S_w,
                          const float* __restrict__ w_h, const float* __restrict__ w_w, const float* __restrict__ w_3,
-                         const int32_t* __restrict__ grid, T* __restrict__ out) {
+                         const int32_t* __restrict__ grid, const uint32_t* __restrict__ zmask, T* __restrict__ out) {
   extern __shared__ __align__(16) float s_w[];           // [32 + S_h + S_w][c]
   pdl_launch_dependents();
   constexpr int C = 32 * V, c = 8 * V;
@@ -269,7 +276,7 @@ sla_cwi_conv_rows_kernel(const T* __restrict__ x, const int4* __restrict__ coord
   uint32_t wbase = (uint32_t)__cvta_generic_to_shared(s_w + myslot * 32 * c + ch0);
   const T* xl = x + lane * V;
   T* ol = out + lane * V;
-  int tdz[2], tdy[2], tdx[2], tdelta[2];
+  int tdz[2], tdy[2], tdx[2], tdelta[2], tcol[2];
 #pragma unroll
   for (int s = 0; s < 2; ++s) {
     int b = 0, t = 0, dz = 1 << 20, dy = 0, dx = 0;        // no tap at this position: always outside the grid
@@ -281,36 +288,59 @@ sla_cwi_conv_rows_kernel(const T* __restrict__ x, const int4* __restrict__ coord
     }
     tdz[s] = dz; tdy[s] = dy; tdx[s] = dx;
     tdelta[s] = (dz * g.gh + dy) * g.gw + dx;
+    tcol[s] = dy * g.gw + dx;
     asm volatile("" : "+r"(tdelta[s]));
+    asm volatile("" : "+r"(tcol[s]));
   }
   asm volatile("" : "+r"(wbase));
   asm volatile("" : "+l"(xl));
   asm volatile("" : "+l"(ol));
   pdl_wait();
   __syncthreads();
-  // the grid cells at this lane's two positions around voxel `me` -> idx[] (-1: no voxel there); < 2^31 cells (host)
-  auto lookups = [&](const int4& me, int (&idx)[2]) -> bool {
+  // Look-ups of this lane's two positions around a voxel, in two dependent rounds that belong to different iterations of
+  // the voxel loop: round 1 reads the occupancy words of the two columns (0 where the position is outside the grid),
+  // round 2 reads the index grid where the position's z bit is set (-1 elsewhere).  < 2^31 cells (host).
+  auto columns_of = [&](const int4& me, int& cell0, int& z, unsigned (&m)[2]) {
     const bool me_in = (unsigned)me.x < (unsigned)g.batch && (unsigned)me.y < (unsigned)g.gz &&
                        (unsigned)me.z < (unsigned)g.gh && (unsigned)me.w < (unsigned)g.gw;
-    const int cell0 = ((me.x * g.gz + me.y) * g.gh + me.z) * g.gw + me.w;
+    const int col0 = (me.x * g.gh + me.z) * g.gw + me.w;
+    cell0 = ((me.x * g.gz + me.y) * g.gh + me.z) * g.gw + me.w;
+    z = me_in ? me.y : -1;                                 // -1: the voxel is off the grid
 #pragma unroll
     for (int s = 0; s < 2; ++s) {
       const bool inside = me_in && (unsigned)(me.y + tdz[s]) < (unsigned)g.gz &&
                           (unsigned)(me.z + tdy[s]) < (unsigned)g.gh && (unsigned)(me.w + tdx[s]) < (unsigned)g.gw;
-      idx[s] = inside ? grid[cell0 + tdelta[s]] : -1;
+      m[s] = inside ? zmask[col0 + tcol[s]] : 0u;
     }
-    return me_in;
   };
-  const int stride = (int)gridDim.x * kCwiWarps;         // N < 2^30 (host): i + 2 stride cannot overflow
+  auto cells_of = [&](int cell0, int z, const unsigned (&m)[2], int (&idx)[2]) {
+#pragma unroll
+    for (int s = 0; s < 2; ++s)
+      idx[s] = ((m[s] >> ((z + tdz[s]) & 31)) & 1u) ? grid[cell0 + tdelta[s]] : -1;
+  };
+  const int stride = (int)gridDim.x * kCwiWarps;         // N < 2^30 (host): i + 3 stride cannot overflow
   int i = (int)blockIdx.x * kCwiWarps + warp;
-  const int4 none = make_int4(-1, -1, -1, -1);
-  int idx[2];
-  bool in_grid = lookups(i < N ? __ldg(coords + i) : none, idx);
-  int4 me_next = (i + stride < N) ? __ldg(coords + i + stride) : none;
+  const int4 none = make_int4(-1, -1, -1, -1);           // outside every grid: nothing is loaded for it
+  auto coords_of = [&](int j) -> int4 { return j < N ? __ldg(coords + j) : none; };
+  // Software pipeline: while voxel i is accumulated, the index-grid cells of voxel i + stride, the occupancy words of
+  // voxel i + 2 stride and the coordinates of voxel i + 3 stride are in flight.
+  int idx[2], cell1, z1, z0;
+  unsigned m1[2];
+  {
+    unsigned m0[2];
+    int cell0;
+    columns_of(coords_of(i), cell0, z0, m0);
+    cells_of(cell0, z0, m0, idx);
+  }
+  columns_of(coords_of(i + stride), cell1, z1, m1);
+  int4 me2 = coords_of(i + 2 * stride);
   for (; i < N; i += stride) {
+    const bool in_grid = z0 >= 0;
     int idx_next[2];
-    const bool in_grid_next = lookups(me_next, idx_next);
-    me_next = (i + 2 * stride < N) ? __ldg(coords + i + 2 * stride) : none;
+    cells_of(cell1, z1, m1, idx_next);
+    z0 = z1;
+    columns_of(me2, cell1, z1, m1);
+    me2 = coords_of(i + 3 * stride);
     uint32_t own[V / 2];
     ld_row<V>(xl + (size_t)i * C, own);
     float acc[V];
@@ -373,7 +403,6 @@ sla_cwi_conv_rows_kernel(const T* __restrict__ x, const int4* __restrict__ coord
     }
     st_row<V>(ol + (size_t)i * C, own);
     idx[0] = idx_next[0]; idx[1] = idx_next[1];
-    in_grid = in_grid_next;
   }
 }
 
@@ -409,33 +438,43 @@ cudaError_t launch_conv(void (*kernel)(KArgs...), int N, size_t smem, cudaStream
 
 template <typename T>
 cudaError_t cwi_launch(const void* x, const int32_t* coords, int N, int C, Geom g, int S_h, int S_w, const float* w_h,
-                       const float* w_w, const float* w_3, void* out, int32_t* grid, cudaStream_t st) {
+                       const float* w_w, const float* w_3, void* out, int32_t* grid, uint32_t* zmask, cudaStream_t st) {
   const size_t cells = (size_t)g.batch * g.gz * g.gh * g.gw;
-  const size_t n16 = (cells * 4 + 15) / 16;
-  unsigned fb = (unsigned)((n16 + 1023) / 1024);
-  if (fb > 2368) fb = 2368;
-  cudaError_t e = launch_chained(sla_cwi_fill_kernel, fb, 256, 0, st, (uint4*)grid, n16);
-  if (e != cudaSuccess) return e;
-  e = launch_chained(sla_cwi_scatter_kernel, (unsigned)((N + 255) / 256), 256, 0, st, (const int4*)coords, N, g, grid);
-  if (e != cudaSuccess) return e;
   const int c = C / 4;
   const size_t smem = (size_t)(S_h + S_w + 29) * c * sizeof(float);
   const int cpl = (c + 31) / 32;
   const int ns = (S_h + S_w + 29 + 31) / 32;
+  auto fill = [&](void* p, size_t bytes, unsigned word) -> cudaError_t {
+    const size_t n16 = (bytes + 15) / 16;
+    unsigned fb = (unsigned)((n16 + 1023) / 1024);
+    if (fb > 2368) fb = 2368;
+    if (fb == 0) fb = 1;
+    return launch_chained(sla_cwi_fill_kernel, fb, 256, 0, st, (uint4*)p, n16, word);
+  };
+  const unsigned sblocks = (unsigned)((N + 255) / 256);
   if constexpr (sizeof(T) == 2) {
     const bool aligned = (((uintptr_t)x | (uintptr_t)out) & 15) == 0;
-    if (S_h + S_w <= 32 && cells < (1ull << 31) && N < (1 << 30) && aligned && (C == 64 || C == 128 || C == 256)) {
-      // a row is one 4-, 8- or 16-byte load per lane
+    if (S_h + S_w <= 32 && g.gz <= 32 && cells < (1ull << 31) && N < (1 << 30) && aligned &&
+        (C == 64 || C == 128 || C == 256)) {
+      // a row is one 4-, 8- or 16-byte load per lane; occupancy words instead of a cleared index grid
+      cudaError_t e = fill(zmask, (size_t)g.batch * g.gh * g.gw * 4, 0u);
+      if (e != cudaSuccess) return e;
+      e = launch_chained(sla_cwi_scatter_kernel, sblocks, 256, 0, st, (const int4*)coords, N, g, grid, zmask);
+      if (e != cudaSuccess) return e;
       const size_t smem_rows = (size_t)(32 + S_h + S_w) * c * sizeof(float);
-#define SLA_CWI_ROWS(V)                                                                                                  \
-  launch_conv(sla_cwi_conv_rows_kernel<T, V>, N, smem_rows, st, (const T*)x, (const int4*)coords, \
-                 N, g, S_h, S_w, w_h, w_w, w_3, (const int32_t*)grid, (T*)out)
+#define SLA_CWI_ROWS(V)                                                                                    \
+  launch_conv(sla_cwi_conv_rows_kernel<T, V>, N, smem_rows, st, (const T*)x, (const int4*)coords, N, g, S_h, S_w, w_h, \
+              w_w, w_3, (const int32_t*)grid, (const uint32_t*)zmask, (T*)out)
       if (C == 64) return SLA_CWI_ROWS(2);
       if (C == 128) return SLA_CWI_ROWS(4);
       return SLA_CWI_ROWS(8);
 #undef SLA_CWI_ROWS
     }
   }
+  cudaError_t e = fill(grid, cells * 4, 0xFFFFFFFFu);
+  if (e != cudaSuccess) return e;
+  e = launch_chained(sla_cwi_scatter_kernel, sblocks, 256, 0, st, (const int4*)coords, N, g, grid, (uint32_t*)nullptr);
+  if (e != cudaSuccess) return e;
 #define SLA_CWI_LAUNCH(CPL, NS)                                                                                    \
   launch_conv(sla_cwi_conv_kernel<T, CPL, NS>, N, smem, st, (const T*)x, (const int4*)coords, \
                  N, C, g, S_h, S_w, w_h, w_w, w_3, (const int32_t*)grid, (T*)out)
@@ -460,11 +499,11 @@ cudaError_t cwi_launch(const void* x, const int32_t* coords, int N, int C, Geom 
 
 cudaError_t launch_cwi(const void* x, const int32_t* coords, int N, int C, int dt, int batch, int gz, int gh, int gw,
                        int S_h, int S_w, const float* w_h, const float* w_w, const float* w_3, void* out,
-                       int32_t* grid, cudaStream_t st) {
+                       int32_t* grid, uint32_t* zmask, cudaStream_t st) {
   const Geom g{batch, gz, gh, gw};
-  if (dt == SLA_F32) return cwi_launch<float>(x, coords, N, C, g, S_h, S_w, w_h, w_w, w_3, out, grid, st);
-  if (dt == SLA_F16) return cwi_launch<__half>(x, coords, N, C, g, S_h, S_w, w_h, w_w, w_3, out, grid, st);
-  return cwi_launch<__nv_bfloat16>(x, coords, N, C, g, S_h, S_w, w_h, w_w, w_3, out, grid, st);
+  if (dt == SLA_F32) return cwi_launch<float>(x, coords, N, C, g, S_h, S_w, w_h, w_w, w_3, out, grid, zmask, st);
+  if (dt == SLA_F16) return cwi_launch<__half>(x, coords, N, C, g, S_h, S_w, w_h, w_w, w_3, out, grid, zmask, st);
+  return cwi_launch<__nv_bfloat16>(x, coords, N, C, g, S_h, S_w, w_h, w_w, w_3, out, grid, zmask, st);
 }
 
 }  // namespace sla

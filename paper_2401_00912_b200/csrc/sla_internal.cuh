@@ -118,7 +118,7 @@ cudaError_t launch_qkv_projection(const void* x, const void* w, const float* bia
 // Cross-Window Interaction (sla_cwi.cu): depth-wise sparse convolutions on the active voxels
 cudaError_t launch_cwi(const void* x, const int32_t* coords, int N, int C, int dt, int batch, int gz, int gh, int gw,
                        int S_h, int S_w, const float* w_h, const float* w_w, const float* w_3, void* out,
-                       int32_t* grid, cudaStream_t st);
+                       int32_t* grid, uint32_t* zmask, cudaStream_t st);
 cudaError_t launch_stream_ceiling(const void* a, const void* b, const void* c, void* out, size_t bytes,
                                   cudaStream_t st);
 

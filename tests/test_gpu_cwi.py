@@ -74,6 +74,28 @@ def test_cwi_dense_neighbourhoods(dtype, C, S_h, S_w):
     _check(_run(x, coords, grid, S_h, S_w, ws, dtype), x, coords, S_h, S_w, ws, dtype)
 
 
+@pytest.mark.parametrize("gz", [32, 33, 40])
+def test_cwi_tall_grids_and_dirty_workspace(gz):
+    """grid_z = 32 is the largest grid that takes the occupancy words (bit 31 in use); above, the index grid is cleared
+    on every call.  The workspace starts full of values that look like voxel indices: none of them may be read as one."""
+    torch = _torch()
+    rng = np.random.Generator(np.random.PCG64(gz))
+    grid = (2, gz, 9, 11)
+    n = 900
+    coords = _dense_scene(rng, n, *grid)
+    coords[:8, 1] = gz - 1                                                # the top cell is occupied
+    coords = np.unique(coords, axis=0).astype(np.int32)
+    n = coords.shape[0]
+    x = wl.round_to_dtype(rng.standard_normal((n, 128)).astype(np.float32), "f16")
+    ws = _weights(rng, 32, 4, 4)
+    nbytes = int(pkg.load_library().sla_cwi_workspace_bytes(*grid))
+    buf = torch.randint(0, n, (nbytes // 4,), dtype=torch.int32, device="cuda").view(torch.uint8)
+    out = pkg.sla_cwi_forward(torch.from_numpy(x).cuda().half(), torch.from_numpy(coords).cuda(), grid, 4, 4,
+                              *(torch.from_numpy(w).cuda() for w in ws), workspace=buf)
+    torch.cuda.synchronize()
+    _check(out, x, coords, 4, 4, ws, "f16")
+
+
 @pytest.mark.parametrize("n", [1, 31, 257])
 def test_cwi_small_and_isolated(n):
     rng = np.random.Generator(np.random.PCG64(n))
