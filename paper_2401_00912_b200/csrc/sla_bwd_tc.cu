@@ -571,9 +571,7 @@ __device__ __forceinline__ void bwd_window(RingView& kv, RingView& qg, RingView&
     ring_wait_upto(kv, (rel + nv - 1) / C::SR);
     bwd_kv_tile<MODE, PRECISE>(kv, hl, rel, nv, st);
   }
-  const int m = e - s;
-  const int lg = 32 - __clz(m - 1);
-  const float scale = __int_as_float((127 - lg) << 23);   // s = 2^-ceil(log2 m)
+  const float scale = z_scale<2>(st.Z);                   // s: largest z of the window -> [1, 2) (sla_tc_base.cuh)
   PassBOps ob;
   ob.eps = eps * scale;
   make_ops<PRECISE>(st.ST, scale, ob.num);
@@ -850,10 +848,16 @@ sla_bwd_tc_split_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_co
     const int ps = max(s, R0), pe = min(e, R1);
     float* slot = split_slot(ws, s, H, h0 + hl);
     float* dslot = split_slot(wd, s, H, h0 + hl);
-    const int lg = 32 - __clz(m - 1);
-    const float scale = __int_as_float((127 - lg) << 23);
     BwdState st;
     st.clear();
+    float scale = 1.f;
+    if (PASS != 0) {   // the complete z of the window (pass 0 finished it): every block of the window derives the same s
+#pragma unroll
+      for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) st.Z[nt][c] = slot[D * D + 8 * nt + 2 * t + (c & 1)];
+      scale = z_scale<2>(st.Z);
+    }
     if (PASS == 0) {
       for (int r = ps; r < pe; r += 16) {
         const int nv = min(16, pe - r), rel = r - S0;

@@ -18,7 +18,7 @@
 //   * Precision: operands are fp16, accumulation fp32.  Windows of <= 16 rows are packed into 16-row
 //     tiles and evaluated in the quadratic form with phi() in fp32 and split operands (x = hi + lo,
 //     both fp16: ~22-bit products); longer windows use phi() in fp16x2, one term, and the state scaled
-//     by 2^-ceil(log2 m) (the ratio of Eq. 3 is scale invariant).
+//     by the power of two that brings its largest z into [1, 2) (the ratio of Eq. 3 is scale invariant).
 #include <cuda.h>
 
 #include <atomic>
@@ -196,6 +196,10 @@ template <int D> struct OutOperands {
   float eps;   // epsilon of the denominator on the scale of the operands (eps * scale)
 };
 
+// the factor applied to a state before its fp16 rounding: z_scale (sla_tc_base.cuh)
+template <int D>
+__device__ __forceinline__ float state_scale(const State<D>& s) { return z_scale<D / 8>(s.Z); }
+
 template <int D, bool PRECISE>
 __device__ __forceinline__ void make_out_operands(const State<D>& s, float scale, float eps, OutOperands<D>& o) {
   o.eps = eps * scale;
@@ -349,12 +353,9 @@ __device__ __forceinline__ void process_window(RingView& kv, RingView& qv, int h
         }
       }
   }
-  const int m = e - s;
-  const int lg = 32 - __clz(m - 1);                       // ceil(log2 m), 0 for m = 1
-  const float scale = __int_as_float((127 - lg) << 23);   // 2^-lg: keeps fp16 operands O(1)
   OutOperands<D> oo[C::HPW];
 #pragma unroll
-  for (int j = 0; j < C::HPW; ++j) make_out_operands<D, PRECISE>(st[j], scale, eps, oo[j]);
+  for (int j = 0; j < C::HPW; ++j) make_out_operands<D, PRECISE>(st[j], state_scale<D>(st[j]), eps, oo[j]);
   uint32_t aq[C::HPW][2];
   ring_release_below<C::SR>(qv, s - S0);
 #pragma unroll
@@ -458,10 +459,9 @@ __device__ __forceinline__ void output_piece(RingView& qv, int hl, int S0, int p
   for (int nt = 0; nt < D / 8; ++nt)
 #pragma unroll
     for (int c = 0; c < 4; ++c) st.Z[nt][c] = slot[D * D + 8 * nt + 2 * t + (c & 1)];
-  const int lg = 32 - __clz(m - 1);
-  const float scale = __int_as_float((127 - lg) << 23);
+  (void)m;
   OutOperands<D> oo;
-  make_out_operands<D, false>(st, scale, eps, oo);
+  make_out_operands<D, false>(st, state_scale<D>(st), eps, oo);
   uint32_t aq[2];
   ring_release_below<C::SR>(qv, ps - S0);
   aq[0] = lane_tile_addr<D>(qv, C::T_STAGE, hl, ps - S0, 16);

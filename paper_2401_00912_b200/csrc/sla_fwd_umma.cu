@@ -700,8 +700,12 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
       for (int p = 0; p < 16; ++p) x[p] = __uint_as_float((lane & 16) ? v[16 + p] : v[p]);   // S_h[p][r]
       const float zv = __uint_as_float(zr);                                                   // z_h[r]
       if (d.x == IT_WIN) {
-        const int lg = 32 - __clz(m - 1);
-        const float scale = __int_as_float((127 - lg) << 23);   // 2^-ceil(log2 m): fp16 operands stay O(1)
+        // power of two that brings the head's largest z into [1, 2) (as sla_fwd_tc.cu: state_scale); the 16 lanes of a
+        // head hold z_h[0..15]
+        float zm = zv;
+#pragma unroll
+        for (int o = 1; o < 16; o <<= 1) zm = fmaxf(zm, __shfl_xor_sync(0xffffffffu, zm, o));
+        const float scale = __int_as_float((254 - ((__float_as_int(zm) >> 23) & 0xff)) << 23);
         mbar_wait_wd(smem_u32(&ctrl.b_empty[bb.slot]), bb.phase ^ 1u);
         LOG(54, 0);
         uint4 c0, c1;

@@ -311,6 +311,22 @@ bool make_map(CUtensorMap* tm, const void* base, int N, int C, int box_rows) {
              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// Power-of-two factor that brings the largest z[p] of a (window, head) state into [1, 2) before S and z (and, in the
+// backward, dS and dz) are rounded to fp16 operands.  Eq. 3 is a ratio, a common factor of S and z cancels; taken from
+// the state, not from the window length: keys far below zero give phi(k) ~ 1e-5 and a mean z far below the fp16
+// normal range (6.1e-5).  Z[nt][c]: z[8 nt + 2 t + (c & 1)], z >= 0; lanes t = 0..3 of a quad hold all of them between
+// them.  All z zero (ReLU map, no positive key): factor 2^127, 0 stays 0.
+template <int NT>
+__device__ __forceinline__ float z_scale(const float (&Z)[NT][4]) {
+  float zm = 0.f;
+#pragma unroll
+  for (int nt = 0; nt < NT; ++nt) zm = fmaxf(zm, fmaxf(Z[nt][0], Z[nt][1]));
+  zm = fmaxf(zm, __shfl_xor_sync(0xffffffffu, zm, 1));
+  zm = fmaxf(zm, __shfl_xor_sync(0xffffffffu, zm, 2));
+  const int ez = (__float_as_int(zm) >> 23) & 0xff;        // biased exponent (z is finite: <= m * 65504)
+  return __int_as_float((254 - ez) << 23);                 // 2^-(ez - 127)
+}
+
 // Per-device caches (a process may drive several GPUs): index = current CUDA device.
 constexpr int kMaxDevices = 64;
 int current_device() {

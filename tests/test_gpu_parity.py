@@ -179,6 +179,48 @@ def test_large_magnitude_inputs(dtype, d):
         check(f"large_magnitude.{name}", got, want, dtype, sc.lengths)
 
 
+@pytest.mark.parametrize("entry", ["tc", "tcgen05"])
+@pytest.mark.parametrize("dtype", ["f16", "bf16"])
+@pytest.mark.parametrize("shift,lengths", [(-8.0, [3, 12, 17, 40, 144, 200, 700]), (-11.0, [3, 12, 17, 40, 144, 200, 700]),
+                                           (-12.0, [17, 40, 144, 200, 700])])
+def test_forward_windows_whose_keys_are_all_far_below_zero(shift, lengths, dtype, entry):
+    """Every key of a window around -8 ... -12: phi(k) ~ 3e-4 ... 6e-6, so z / m lies far below the fp16 normal range
+    (6.1e-5).  The kernels scale the state by the exponent of its own largest z before the fp16 rounding (Eq. 3 is a
+    ratio: any common factor of S and z cancels), so windows that go through a state stay accurate.  Windows of <= 16
+    rows (packed quadratic tiles) use phi(k) itself as an fp16 operand and keep their accuracy down to k ~ -11; below
+    -12 the fp16 subnormal spacing of phi(k) itself (6e-8) is what limits every path."""
+    if entry == "tcgen05" and dtype != "f16":
+        pytest.skip("the tcgen05 entry takes fp16")
+    sc = wl.make_scene(lengths, 8, 16, dtype, seed=21)
+    q, v = sc.tensor("q"), sc.tensor("v")
+    k = wl.round_to_dtype((0.5 * sc.tensor("k") + shift).astype(np.float32), dtype)
+    torch = _torch()
+    off = torch.from_numpy(sc.offsets).cuda()
+    out = pkg.sla_forward(to_dev(q, dtype), to_dev(k, dtype), to_dev(v, dtype), off, tcgen05=(entry == "tcgen05"))
+    torch.cuda.synchronize()
+    ref = sla_oracle.forward(q, k, v, sc.offsets)
+    check(f"keys_at_{shift}.out", out, ref, dtype, sc.lengths)
+
+
+@pytest.mark.parametrize("d", [16, 32])
+@pytest.mark.parametrize("dtype", ["f16", "bf16"])
+@pytest.mark.parametrize("shift,lengths", [(-8.0, [3, 12, 17, 40, 144, 200, 700]), (-11.0, [3, 12, 17, 40, 144, 200, 700]),
+                                           (-12.0, [40, 144, 200, 700])])
+def test_backward_windows_whose_keys_are_all_far_below_zero(shift, lengths, dtype, d):
+    """The same regime for the gradients: den = phi(q) . z is ~ m * 1e-4, so g / den and dS are large while phi'(k) is
+    tiny; the tensor-core backward scales S, z, dS and dz by the exponent of the window's largest z."""
+    sc = wl.make_scene(lengths, 8 if d == 16 else 4, d, dtype, seed=22)
+    q, v, g = sc.tensor("q"), sc.tensor("v"), sc.tensor("do")
+    k = wl.round_to_dtype((0.5 * sc.tensor("k") + shift).astype(np.float32), dtype)
+    torch = _torch()
+    off = torch.from_numpy(sc.offsets).cuda()
+    grads = pkg.sla_backward(to_dev(q, dtype), to_dev(k, dtype), to_dev(v, dtype), off, to_dev(g, dtype))
+    torch.cuda.synchronize()
+    gref = sla_oracle.backward(q, k, v, g, sc.offsets)
+    for name, got, want in zip(("dq", "dk", "dv"), grads, gref):
+        check(f"keys_at_{shift}.{name}", got, want, dtype, sc.lengths)
+
+
 # ---- the tcgen05 forward (sla_forward_tcgen05): same oracle, same tolerance --------------------------
 TCGEN05_LAYOUTS = dict(EDGE_LAYOUTS, mixed_pack_wrap=[2, 6, 3, 15, 8, 53, 88, 53, 76, 107, 121, 144, 144] * 40,
                        dense_144=[144] * 400, tiny_3=[3] * 3000)
