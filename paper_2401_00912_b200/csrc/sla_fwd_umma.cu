@@ -75,28 +75,6 @@ constexpr int PF_FIRST = 1024, PF_CHUNK = 32;                   // L2 prefetch: 
 static_assert(NB * B_BUF >= 7 * 2048, "an M=128 Q block starting at the last ring tile reads 7 tiles past the ring");
 static_assert(NKV <= 32 && NQT <= 32, "one parity bit per ring tile");
 
-#ifdef SLA_DEVEL_TRACE   // development only (never defined in the product build)
-__device__ unsigned long long g_trace[512 * 64];
-__device__ __forceinline__ void trace_at(int slot) {
-  if (blockIdx.x < 512 && slot < 64) {
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
-    g_trace[blockIdx.x * 64 + slot] = t;
-  }
-}
-#define TR(cond, slot) do { if (cond) trace_at(slot); } while (0)
-// fine-grained event log of two CTAs: per warp (lane 0) a private list of (code, id, SM clock); plain stores only
-__device__ int g_log_cta[2] = {40, 10};
-__device__ int4 g_log[2][32][512];
-#define LOG_DECL int lg_n = 0; const int lg_which = (int)blockIdx.x == g_log_cta[0] ? 0 : ((int)blockIdx.x == g_log_cta[1] ? 1 : -1);
-#define LOG(code, id) do { if (lg_which >= 0 && (threadIdx.x & 31) == 0 && lg_n < 511) { \
-    g_log[lg_which][threadIdx.x >> 5][++lg_n] = make_int4(code, id, (int)clock64(), 0); \
-    g_log[lg_which][threadIdx.x >> 5][0].x = lg_n; } } while (0)
-#else
-#define TR(cond, slot) do {} while (0)
-#define LOG_DECL
-#define LOG(code, id) do {} while (0)
-#endif
 
 enum ItemType { IT_END = 0, IT_PACK = 1, IT_WIN = 2, IT_PIECE = 3 };
 
@@ -196,9 +174,6 @@ __device__ __forceinline__ void l2_prefetch(const void* p, uint32_t bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 // mbarrier wait with a watchdog: a protocol error traps instead of hanging the device
-#ifdef SLA_DEVEL_TRACE
-__device__ int g_abort[8];   // development build: the first wait that times out records itself, every wait then gives up
-#endif
 __device__ __forceinline__ void mbar_wait_wd(uint32_t bar, uint32_t parity) {
   uint32_t done, spins = 0;
   do {
@@ -207,21 +182,7 @@ __device__ __forceinline__ void mbar_wait_wd(uint32_t bar, uint32_t parity) {
         "mbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2, %3;\n\t"
         "selp.b32 %0, 1, 0, P1;\n\t}"
         : "=r"(done) : "r"(bar), "r"(parity), "r"(100000u) : "memory");
-#ifdef SLA_DEVEL_TRACE
-    if (!done) {
-      if (*reinterpret_cast<volatile int*>(&g_abort[0])) return;
-      if (++spins > (1u << 14)) {
-        if (atomicCAS(&g_abort[0], 0, 1) == 0) {
-          g_abort[1] = blockIdx.x; g_abort[2] = threadIdx.x >> 5; g_abort[3] = (int)bar; g_abort[4] = (int)parity;
-          g_abort[5] = threadIdx.x & 31;
-          __threadfence();
-        }
-        return;
-      }
-    }
-#else
     if (!done && ++spins > (1u << 16)) __trap();
-#endif
   } while (!done);
 }
 
@@ -276,10 +237,6 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
   extern __shared__ uint8_t dyn_smem[];
   __shared__ Ctrl ctrl;
   asm volatile("griddepcontrol.launch_dependents;");
-  TR(threadIdx.x == 0, 0);
-#ifdef SLA_DEVEL_TRACE
-  if (threadIdx.x == 0 && blockIdx.x == 0) g_abort[6] = (int)smem_u32(&ctrl);
-#endif
   const uint32_t sbase = (smem_u32(dyn_smem) + 1023u) & ~1023u;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int Ctot = H * D;
@@ -321,10 +278,8 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = ctrl.tmem_base;
-  TR(threadIdx.x == 0, 1);
   // nothing a previous kernel of the stream may have written (offsets, tensors, workspace, out) is touched before
   asm volatile("griddepcontrol.wait;" ::: "memory");
-  TR(threadIdx.x == 0, 2);
   // the rows of this span go to L2 now, in the order they will be needed (whole rows of k, v, q)
   if (warp == WARP_WALK && lane < 3 && R0 < R1) {
     const T* base = lane == 0 ? kg_ : (lane == 1 ? vg : qg);
@@ -339,8 +294,6 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
     if (idx < W && __ldg(off + idx) <= R0) atomicMax(&ctrl.search_lo, (int)idx);
   }
   __syncthreads();
-  LOG_DECL
-
   // every consumer role reads the item ring in order
   auto next_item = [&](Cur& it) -> int4 {
     mbar_wait_wd(smem_u32(&ctrl.item_full[it.slot]), it.phase);
@@ -394,7 +347,6 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
         hi = min(hi, lo + step);
       }
       const int wa = lo;
-      TR(lane == 0, 3);
       int pf_row = min(N, min(R1 + 128, max(0, R0 - 64) + PF_FIRST));
       const int pf_end = min(N, R1 + 128);
       auto prefetch_to = [&](int row) {       // rows beyond the first PF_FIRST: requested as the walk advances
@@ -428,7 +380,6 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
           const int n = min(KVC, T16 - KVC * c);
           const int first = kr.alloc(n);
           if (lane == 0) {
-            LOG(10, y + 16 * KVC * c);
             claim_tiles(ctrl.kv_owner, ctrl.kv_empty, NKV, kr.bits, first, n);
             const uint32_t bar = smem_u32(&ctrl.kv_full[first]);
             mbar_expect_tx(bar, (uint32_t)(n * 8192));
@@ -439,7 +390,6 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
               tma_load_2d(dv, &maps.m[2][mi], bar, col0, yy);
               tma_load_2d(dv + KV_REG, &maps.m[2][mi], bar, col0 + 64, yy);
             });
-            LOG(11, y + 16 * KVC * c);
           }
           kr.used(first);
         }
@@ -482,7 +432,6 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
       }
     }
     emit(IT_END, 0, 0, 0);
-    TR(lane == 0, 4);
   } else if (warp == WARP_QLOAD) {
     // =========================== Q chunk loads ===========================
     Cur it{0, 0};
@@ -496,7 +445,6 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
         const int n = min(8, T16 - 8 * c);
         const int first = qr.alloc(n);
         if (lane == 0) {
-          LOG(12, d.y + 128 * c);
           claim_tiles(ctrl.q_owner, ctrl.q_empty, NQT, qr.bits, first, n);
           const uint32_t bar = smem_u32(&ctrl.q_full[first]);
           mbar_expect_tx(bar, (uint32_t)(n * 4096));
@@ -505,7 +453,6 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
             tma_load_2d(dq, &maps.m[0][mi], bar, col0, yy);
             tma_load_2d(dq + Q_REG, &maps.m[0][mi], bar, col0 + 64, yy);
           });
-          LOG(13, d.y + 128 * c);
         }
         qr.used(first);
       }
@@ -528,11 +475,9 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
       for (int c = 0; c * KVC < T16; ++c) {
         const int n = min(KVC, T16 - KVC * c);
         const int first = kr.alloc(n);
-        LOG(20, d.y + 16 * KVC * c);
         mbar_wait_wd(smem_u32(&ctrl.kphi[first]), (kphi_bits >> first) & 1u);
         kphi_bits ^= 1u << first;
         tc_fence_after();
-        LOG(21, d.y + 16 * KVC * c);
         if (lane == 0) {
           for (int j = 0; j < n; ++j) {
             const uint32_t kt = sbase + OFF_K + (first + j) * 2048;
@@ -547,7 +492,6 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
       }
       if (lane == 0) umma_commit(smem_u32(&ctrl.state_full[rg.slot]));
       __syncwarp();
-      LOG(22, d.y);
       advance<NSL>(rg);
     }
   } else if (warp == WARP_OMMA) {
@@ -565,9 +509,7 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
       const int T16 = (d.z + 15) >> 4;
       const uint32_t region = tmem + (uint32_t)(rg.slot * REGION_COLS);
       const uint32_t bbuf = sbase + OFF_B + bb.slot * B_BUF;
-      LOG(30, d.y);
       mbar_wait_wd(smem_u32(&ctrl.b_full[bb.slot]), bb.phase);
-      LOG(31, d.y);
       for (int b = 0; b * 8 < T16; ++b) {
         const int n = min(8, T16 - 8 * b);
         const int first = qr.alloc(n);
@@ -578,7 +520,6 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
           od_ph ^= 1u << rg.slot;
         }
         tc_fence_after();
-        LOG(32, d.y + 128 * b);
         if (lane == 0) {
           const uint32_t qs0 = sbase + OFF_Q + first * 2048;
 #pragma unroll
@@ -588,7 +529,6 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
           umma_commit(smem_u32(&ctrl.o_full[rg.slot]));
         }
         __syncwarp();
-        LOG(33, d.y + 128 * b);
       }
       if (lane == 0) umma_commit(smem_u32(&ctrl.b_empty[bb.slot]));
       __syncwarp();
@@ -648,28 +588,22 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
       for (int c = 0; c * KVC < T16; ++c) {
         const int n = min(KVC, T16 - KVC * c);
         const int first = kr.alloc(n);
-        LOG(40, d.y + 16 * KVC * c);
         mbar_wait_wd(smem_u32(&ctrl.kv_full[first]), kr.parity(first));
-        LOG(41, d.y + 16 * KVC * c);
         phi_chunk(sbase + OFF_K + (tid_g >> 7) * KV_REG, first, n, 16 * KVC * c, m);
         proxy_fence();
         __syncwarp();
         if (lane == 0) mbar_arrive(smem_u32(&ctrl.kphi[first]));
-        LOG(42, d.y + 16 * KVC * c);
         kr.used(first);
       }
       if (d.x == IT_WIN) {
         for (int b = 0; b * 8 < T16; ++b) {
           const int n = min(8, T16 - 8 * b);
           const int first = qr.alloc(n);
-          LOG(43, d.y + 128 * b);
           mbar_wait_wd(smem_u32(&ctrl.q_full[first]), qr.parity(first));
-          LOG(44, d.y + 128 * b);
           phi_chunk(sbase + OFF_Q + (tid_g >> 7) * Q_REG, first, n, 0, 1 << 30);
           proxy_fence();
           __syncwarp();
           if (lane == 0) mbar_arrive(smem_u32(&ctrl.qphi[first]));
-          LOG(45, d.y + 128 * b);
           qr.used(first);
         }
       }
@@ -684,16 +618,13 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
       if (d.x == IT_PACK) continue;
       const int m = d.z;
       const uint32_t region = tmem + (uint32_t)(rg.slot * REGION_COLS);
-      LOG(50, d.y);
       mbar_wait_wd(smem_u32(&ctrl.state_full[rg.slot]), rg.phase);
       tc_fence_after();
-      LOG(51, d.y);
       uint32_t v[32], zr;
       const uint32_t lane_base = (uint32_t)(32 * quad) << 16;
       tmem_ld32(region + lane_base + 32 * quad, v);       // columns 32q..32q+31: the diagonal blocks of heads 2q, 2q+1
       tmem_ld1(region + lane_base + 128, zr);
       tmem_wait_ld();
-      LOG(53, 0);
       const int h = 2 * quad + (lane >> 4), r = lane & 15;     // this lane = channel (h, r) of the slab
       float x[16];
 #pragma unroll
@@ -707,7 +638,6 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
         for (int o = 1; o < 16; o <<= 1) zm = fmaxf(zm, __shfl_xor_sync(0xffffffffu, zm, o));
         const float scale = __int_as_float((254 - ((__float_as_int(zm) >> 23) & 0xff)) << 23);
         mbar_wait_wd(smem_u32(&ctrl.b_empty[bb.slot]), bb.phase ^ 1u);
-        LOG(54, 0);
         uint4 c0, c1;
         c0.x = pack_h2(x[0] * scale, x[1] * scale);   c0.y = pack_h2(x[2] * scale, x[3] * scale);
         c0.z = pack_h2(x[4] * scale, x[5] * scale);   c0.w = pack_h2(x[6] * scale, x[7] * scale);
@@ -720,11 +650,9 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
         sts128(tile + r * 128 + ((lc ^ (r & 7)) << 4), c0);
         sts128(tile + r * 128 + (((lc + 1) ^ (r & 7)) << 4), c1);
         sts16(tile + 16 * 128 + ((lc + (r >> 3)) << 4) + (r & 7) * 2, __half_as_ushort(__float2half_rn(zv * scale)));
-        LOG(55, 0);
         proxy_fence();
         tc_fence_before();
         __syncwarp();
-        LOG(56, 0);
         if (lane == 0) mbar_arrive(smem_u32(&ctrl.b_full[bb.slot]));
         advance<NB>(bb);
       } else {
@@ -737,7 +665,6 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
         __syncwarp();
         if (lane == 0) mbar_arrive_n(smem_u32(&ctrl.region_free[rg.slot]), NEPI / NCONV);
       }
-      LOG(52, d.y);
       advance<NSL>(rg);
     }
   } else {
@@ -758,11 +685,9 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
       for (int b = 0; b * 8 < T16; ++b) {
         const int first = qr.alloc(min(8, T16 - 8 * b));
         const int rows = min(128, m - 128 * b);          // valid rows of this block
-        LOG(60, s + 128 * b);
         mbar_wait_wd(smem_u32(&ctrl.o_full[rg.slot]), (of_ph >> rg.slot) & 1u);
         of_ph ^= 1u << rg.slot;
         tc_fence_after();
-        LOG(61, s + 128 * b);
         if (32 * quad < rows) {
 #pragma unroll 1
          for (int hf = 0; hf < EPI_HALVES; ++hf) {
@@ -779,7 +704,6 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
             tmem_ld16(taddr + 64 * hp + 32, vb);
             tmem_ld1(taddr + 64 * hp + 48, db);
             tmem_wait_ld();
-            LOG(63, hp);
             const float ia = fast_rcp(__uint_as_float(da)), ib = fast_rcp(__uint_as_float(db));
             uint4 o[4];
 #pragma unroll
@@ -799,7 +723,6 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
             }
           }
           __syncwarp();
-          LOG(64, 0);
           // coalesced copy-out: per instruction 4 rows x 128 bytes (lane -> row 4 it + lane/8, chunk lane%8)
           const int nr = min(32, rows - 32 * quad);
           T* obase = out + (size_t)(s + 128 * b + 32 * quad) * Ctot + col0 + 64 * half + (lane & 7) * 8;
@@ -815,10 +738,8 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
             const int row = 4 * i + (lane >> 3);
             if (row < nr) *reinterpret_cast<uint4*>(obase + (size_t)row * Ctot) = x[i];
           }
-          LOG(65, 0);
          }
           proxy_fence();
-          LOG(66, 0);                                 // the tiles go back to the TMA loader
         }
         tc_fence_before();
         __syncwarp();
@@ -828,7 +749,6 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
           mbar_arrive_relaxed(smem_u32(&ctrl.q_empty[first]));
           mbar_arrive_relaxed(smem_u32((b + 1) * 8 < T16 ? &ctrl.o_drained[rg.slot] : &ctrl.region_free[rg.slot]));
         }
-        LOG(62, s + 128 * b);
       }
       advance<NSL>(rg);
     }
@@ -837,7 +757,6 @@ sla_fwd_umma_kernel(const __grid_constant__ Maps maps, const T* __restrict__ qg,
   // ---- teardown ---------------------------------------------------------------------------------------
   tc_fence_before();
   __syncthreads();
-  TR(threadIdx.x == 0, 5);
   if (warp == WARP_SMMA) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(TMEM_COLS));
@@ -882,26 +801,6 @@ cudaError_t umma_launch(const Problem& p, cudaStream_t st) {
 
 }  // namespace
 
-#ifdef SLA_DEVEL_TRACE
-extern "C" int sla_debug_read_trace(unsigned long long* host, int n) {
-  return (int)cudaMemcpyFromSymbol(host, g_trace, sizeof(unsigned long long) * n);
-}
-extern "C" int sla_debug_read_log(int* host_int4, int cta0, int cta1) {   // host: 2*32*512 int4; then re-arms
-  cudaError_t e = cudaMemcpyFromSymbol(host_int4, g_log, sizeof(int4) * 2 * 32 * 512);
-  void* p = nullptr;
-  cudaGetSymbolAddress(&p, g_log);
-  cudaMemset(p, 0, sizeof(int4) * 2 * 32 * 512);
-  int c[2] = {cta0, cta1};
-  cudaMemcpyToSymbol(g_log_cta, c, sizeof(c));
-  return (int)e;
-}
-extern "C" int sla_debug_read_abort(int* host) {   // host[0..7]; also clears the flag
-  cudaError_t e = cudaMemcpyFromSymbol(host, g_abort, sizeof(int) * 8);
-  int z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-  cudaMemcpyToSymbol(g_abort, z, sizeof(z));
-  return (int)e;
-}
-#endif
 
 bool forward_umma_supported(const Problem& p, int dt) {
   if (dt != SLA_F16 || p.phi != SLA_PHI_ELU1) return false;
@@ -912,9 +811,6 @@ bool forward_umma_supported(const Problem& p, int dt) {
 cudaError_t launch_forward_umma_main(const Problem& p, int dt, cudaStream_t st) {
   (void)dt;
   cudaError_t e = umma_launch<false, __half>(p, st);
-#ifdef SLA_DEVEL_TRACE
-  if (e != cudaSuccess) fprintf(stderr, "umma_launch: %s\n", cudaGetErrorString(e));
-#endif
   return e;
 }
 
