@@ -345,7 +345,7 @@ sla_seq_place_kernel(const int32_t* __restrict__ key_in, int N, int W, int T, co
 constexpr int kPermUnroll = 4;
 template <typename V, bool SCATTER>
 __global__ void __launch_bounds__(256)
-sla_permute_rows_kernel(const V* __restrict__ src, const int32_t* __restrict__ perm, long long N, int vpr,
+sla_permute_rows_kernel(const V* __restrict__ src, const int32_t* __restrict__ perm, long long N, int vpr, int shift,
                         V* __restrict__ dst) {
   pdl_launch_dependents();
   pdl_wait();
@@ -358,7 +358,8 @@ sla_permute_rows_kernel(const V* __restrict__ src, const int32_t* __restrict__ p
     const long long idx = first + u * 256;
     from[u] = -1;
     if (idx < total) {
-      const long long row = idx / vpr;
+      // vectors per row is a power of two for the usual rows (256 or 512 bytes): a shift instead of a 64-bit division
+      const long long row = shift >= 0 ? (idx >> shift) : idx / vpr;
       const int col = (int)(idx - row * vpr);
       const long long p = perm[row];
       if (p >= 0 && p < N) {
@@ -477,15 +478,18 @@ cudaError_t launch_permute_rows(const void* src, const int32_t* perm, long long 
   const bool wide = row_bytes % 16 == 0 && (((uintptr_t)src | (uintptr_t)dst) & 15u) == 0;
   const size_t vec = wide ? 16 : 4;
   const int vpr = (int)(row_bytes / vec);
+  int shift = -1;                                          // log2(vpr) if vpr is a power of two
+  for (int b = 0; b < 31; ++b)
+    if (vpr == (1 << b)) shift = b;
   const unsigned long long total = (unsigned long long)N * (unsigned long long)vpr;
   const unsigned long long per_block = 256ull * kPermUnroll;
   const unsigned blocks = (unsigned)((total + per_block - 1) / per_block);
   if (blocks == 0) return cudaSuccess;
   if (wide)
-    return scatter ? launch_chained(sla_permute_rows_kernel<uint4, true>, blocks, 256, st, (const uint4*)src, perm, N, vpr, (uint4*)dst)
-                   : launch_chained(sla_permute_rows_kernel<uint4, false>, blocks, 256, st, (const uint4*)src, perm, N, vpr, (uint4*)dst);
-  return scatter ? launch_chained(sla_permute_rows_kernel<uint32_t, true>, blocks, 256, st, (const uint32_t*)src, perm, N, vpr, (uint32_t*)dst)
-                 : launch_chained(sla_permute_rows_kernel<uint32_t, false>, blocks, 256, st, (const uint32_t*)src, perm, N, vpr, (uint32_t*)dst);
+    return scatter ? launch_chained(sla_permute_rows_kernel<uint4, true>, blocks, 256, st, (const uint4*)src, perm, N, vpr, shift, (uint4*)dst)
+                   : launch_chained(sla_permute_rows_kernel<uint4, false>, blocks, 256, st, (const uint4*)src, perm, N, vpr, shift, (uint4*)dst);
+  return scatter ? launch_chained(sla_permute_rows_kernel<uint32_t, true>, blocks, 256, st, (const uint32_t*)src, perm, N, vpr, shift, (uint32_t*)dst)
+                 : launch_chained(sla_permute_rows_kernel<uint32_t, false>, blocks, 256, st, (const uint32_t*)src, perm, N, vpr, shift, (uint32_t*)dst);
 }
 
 }  // namespace sla
