@@ -142,6 +142,13 @@ int sla_forward_bounded(const void* q, const void* k, const void* v, const int32
  * (three dependent rounds of probes), with it by one 16-byte load.
  *   table  DEV, >= sla_span_table_bytes(N, H, d_h) bytes, 16-byte aligned; written by sla_build_span_table (one small
  *          kernel on `stream`), read-only afterwards; valid for this (window_offsets, N, H, d_h) on this device.
+ *          Layout (int32, checked bit for bit by tests/test_gpu_parity.py against a CPU restatement): entry 0 =
+ *          {magic, span, nspans, N}; entry 1 + i for the span of rows [i*span, min((i+1)*span, N)) =
+ *          {w0, begin, end, 0}: w0 = the window that holds the span's first row; a window of <= 256 rows belongs to
+ *          the span that holds its middle row off[w] + len/2, so begin = off[w0] if that middle is >= the span's first
+ *          row, else off[w0+1]; end = off[wl+1] if the middle of wl (the window of the span's last row) lies inside the
+ *          span, else off[wl]; longer windows are cut at the span's own borders (begin = first row, end = last row + 1).
+ *          The rows streamed are [begin, max(begin, end)).
  * sla_forward_planned = sla_forward_bounded (same promise about max_window_len, same results bit for bit, one launch, no
  * workspace) + the table.  A table that belongs to another N or launch geometry is detected on the device and ignored
  * (the kernel searches as usual); a table of other offsets with the same N is undefined behaviour. */

@@ -510,6 +510,48 @@ def test_backward_writes_nothing_beyond_n(dtype, H, d):
     check_grads([b[:sc.N] for b in bufs], ref, sc)
 
 
+def _span_table_restated(off, N, span, nspans):
+    """The work list of include/sla.h (sla_build_span_table), restated on the host: per span the window of its first
+    row and the rows it streams under the middle-row ownership rule (windows of more than 256 rows are cut at the span)."""
+    off = np.asarray(off, dtype=np.int64)
+    t = np.zeros((nspans, 4), dtype=np.int32)
+    win_of = lambda r: int(np.searchsorted(off, r, side="right") - 1)       # skips zero-length windows
+    for i in range(nspans):
+        r0, r1 = i * span, min((i + 1) * span, N)
+        w0, wl = win_of(r0), win_of(r1 - 1)
+        s, e = int(off[w0]), int(off[w0 + 1])
+        begin = (s if s + (e - s) // 2 >= r0 else e) if e - s <= 256 else r0
+        s, e = int(off[wl]), int(off[wl + 1])
+        end = (e if s + (e - s) // 2 < r1 else s) if e - s <= 256 else r1
+        t[i] = (w0, begin, end, 0)
+    return t
+
+
+@pytest.mark.parametrize("case", ["config1", "config3", "config2", "gaps_and_long", "one_window", "len1"])
+def test_span_table_bit_exact(case):
+    """SURVEY 8(a) a1 (work list): integer work, bit for bit against the host restatement above."""
+    torch = _torch()
+    if case.startswith("config"):
+        sc = wl.make_config(int(case[-1]))
+    elif case == "gaps_and_long":
+        sc = wl.make_scene([0, 0, 5, 300, 0, 1, 256, 257, 0, 17, 1000, 2, 0], 8, 16, "f16", seed=71)
+    elif case == "one_window":
+        sc = wl.make_scene([777], 8, 16, "f16", seed=72)
+    else:
+        sc = wl.make_scene([1] * 5000, 8, 16, "f16", seed=73)
+    off = torch.from_numpy(sc.offsets).cuda()
+    raw = pkg.sla_build_span_table(off, sc.N, sc.H, sc.d_h)
+    torch.cuda.synchronize()
+    tab = raw.cpu().numpy().view(np.int32).reshape(-1, 4)
+    magic, span, nspans, n = (int(x) for x in tab[0])
+    assert n == sc.N and span % 16 == 0 and nspans == (sc.N + span - 1) // span
+    assert tab.shape[0] >= nspans + 1
+    want = _span_table_restated(sc.offsets, sc.N, span, nspans)
+    got = tab[1:nspans + 1]
+    bad = np.nonzero((got != want).any(axis=1))[0]
+    assert bad.size == 0, f"span {bad[0]}: got {got[bad[0]]} want {want[bad[0]]} (span {span} rows)"
+
+
 @pytest.mark.parametrize("case", ["config1", "config4", "tiny", "mixed_d32", "bf16_partial_slab", "small_n"])
 def test_forward_planned_matches_bounded_bit_for_bit(case):
     """sla_forward_planned: the span table (built once per scene) replaces the in-kernel window search and must not
