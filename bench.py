@@ -239,8 +239,9 @@ def extra_legs(pkg, torch, dev, peak):
                 "sla_backward_bounded (windows <= 144 rows by construction: one launch, no workspace)"}
     del sets
     sweep = []
-    for frames in (1, 2, 4, 8, 16):
-        ln = [wl.lengths_waymo_like(wl.SEED_BASE + 1 + f, 60000) for f in range(frames)]
+    # N from 10 k to ~1 M voxels at config-1 statistics (a sparser single frame, then stacked frames)
+    for per_frame, frames in ((10000, 1), (30000, 1), (60000, 1), (60000, 2), (60000, 4), (60000, 8), (60000, 16)):
+        ln = [wl.lengths_waymo_like(wl.SEED_BASE + 1 + f, per_frame) for f in range(frames)]
         scb = wl.make_scene(__import__("numpy").concatenate(ln), 8, 16, "f16", wl.SEED_BASE + 50 + frames)
         Nb = scb.N
         n_sets = max(2, -(-2 * L2_BYTES // (4 * Nb * 256)) + 1)
@@ -255,7 +256,8 @@ def extra_legs(pkg, torch, dev, peak):
 
         us = timed(fb)
         sweep.append({"frames": frames, "N": Nb, "us": us, "voxels_per_sec": Nb / (us * 1e-6),
-                      "frac_of_peak": (4 * Nb * 256 + 4 * (scb.W + 1)) / (us * 1e-6) / 1e9 / peak})
+                      "frac_of_peak": (4 * Nb * 256 + 4 * (scb.W + 1)) / (us * 1e-6) / 1e9 / peak,
+                      "workspace_bytes_general_entry": pkg.workspace_bytes(Nb, scb.W, 8, 16, 1, False)})
         del bs, base
     out["fwd_batch_sweep"] = sweep
     return out
